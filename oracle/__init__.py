@@ -1,0 +1,168 @@
+"""CPU oracle for the batched pentadiagonal path -- TEST INFRASTRUCTURE, NOT PRODUCT.
+
+Only `tests/`, `__graft_entry__.smoke()` and `bench.py`'s `cpu_baseline` /
+`--impl reference` legs may import this package.  It shares no code with
+`paper_1807_07382_b200/` and neither imports the other.
+
+Thin ctypes wrapper around `pent_oracle.c` / `pent_oracle_step.c` (plain fp64 C,
+PAPER.md:148-244 transcribed step by step).  The wrapper only marshals arrays and
+transposes between the interleaved batch layout (N, M) used by the library
+ and the serial "one system per row" layout (M, N) the paper's CPU
+code uses; all arithmetic is in the C files.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from dataclasses import dataclass
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = [os.path.join(_HERE, "pent_oracle.c"), os.path.join(_HERE, "pent_oracle_step.c")]
+_LIB = os.path.join(_HERE, "libpent_oracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """gcc -O2 -ffp-contract=off (no FMA contraction: one reproducible definition)."""
+    if not force and os.path.exists(_LIB) and all(
+            os.path.getmtime(_LIB) >= os.path.getmtime(s) for s in _SRC):
+        return _LIB
+    cmd = ["gcc", "-O2", "-ffp-contract=off", "-fPIC", "-shared", "-fopenmp",
+           "-o", _LIB] + _SRC + ["-lm"]
+    subprocess.run(cmd, check=True)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        _lib = C.CDLL(_LIB)
+        _lib.pent_oracle_factor.restype = C.c_int
+        _lib.pent_oracle_dense_ge.restype = C.c_int
+    return _lib
+
+
+def _p(x: np.ndarray):
+    assert x.dtype == np.float64 and x.flags.c_contiguous
+    return x.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def _f64(x) -> np.ndarray:
+    return np.ascontiguousarray(x, dtype=np.float64)
+
+
+@dataclass
+class Factors:
+    """L (eps, beta, alpha) and R (gamma, delta) of PAPER.md Eq. 13, plus the
+    original diagonals (kept for residuals and for the (2I-A)C right-hand side)."""
+    N: int
+    eps: np.ndarray
+    beta: np.ndarray
+    alpha: np.ndarray
+    gamma: np.ndarray
+    delta: np.ndarray
+    diags: tuple
+
+
+class SingularPivot(ArithmeticError):
+    def __init__(self, row: int):
+        super().__init__(f"zero or non-finite pivot at row {row} (no pivoting, PAPER.md:275)")
+        self.row = row
+
+
+def factor(a, b, c, d, e) -> Factors:
+    """A = L R.  Raises SingularPivot(row) on a bad pivot."""
+    a, b, c, d, e = (_f64(v) for v in (a, b, c, d, e))
+    N = c.shape[0]
+    out = [np.zeros(N) for _ in range(5)]
+    rc = _load().pent_oracle_factor(C.c_int(N), _p(a), _p(b), _p(c), _p(d), _p(e),
+                                    *[_p(o) for o in out])
+    if rc != 0:
+        raise SingularPivot(rc - 1)
+    return Factors(N, *out, diags=(a, b, c, d, e))
+
+
+def solve(fac: Factors, f) -> np.ndarray:
+    """One system, contiguous f of length N.  PAPER.md:223-242."""
+    f = _f64(f)
+    x = np.empty_like(f)
+    _load().pent_oracle_solve(C.c_int(fac.N), _p(fac.eps), _p(fac.beta), _p(fac.alpha),
+                              _p(fac.gamma), _p(fac.delta), _p(f), _p(x))
+    return x
+
+
+def to_rows(f_interleaved: np.ndarray) -> np.ndarray:
+    """(N, M) interleaved -> (M, N) one system per row."""
+    return np.ascontiguousarray(np.asarray(f_interleaved, dtype=np.float64).T)
+
+
+def solve_rows(fac: Factors, F_rows: np.ndarray, nthreads: int = 1) -> np.ndarray:
+    """Batch solve in the serial layout (M, N); this is what the CPU baseline times."""
+    F_rows = _f64(F_rows)
+    M = F_rows.shape[0]
+    X = np.empty_like(F_rows)
+    _load().pent_oracle_solve_rows(C.c_int(fac.N), C.c_long(M), _p(fac.eps), _p(fac.beta),
+                                   _p(fac.alpha), _p(fac.gamma), _p(fac.delta),
+                                   _p(F_rows), _p(X), C.c_int(nthreads))
+    return X
+
+
+def solve_batch(fac: Factors, f_interleaved, nthreads: int = 1) -> np.ndarray:
+    """Interleaved (N, M) in, interleaved (N, M) out (fp64)."""
+    X = solve_rows(fac, to_rows(f_interleaved), nthreads)
+    return np.ascontiguousarray(X.T)
+
+
+def factor_solve_batch(a, b, c, d, e, f, nthreads: int = 1):
+    """Per-system matrices (PAPER.md:289 'Rewrite' mode); every argument is an
+    interleaved (N, M) array.  Returns (x (N, M), info (M,)): info[i] = 0 or
+    first bad row + 1."""
+    rows = [to_rows(v) for v in (a, b, c, d, e, f)]
+    M, N = rows[5].shape
+    X = np.zeros_like(rows[5])
+    info = np.zeros(M, dtype=np.int32)
+    _load().pent_oracle_factor_solve_rows(
+        C.c_int(N), C.c_long(M), *[_p(r) for r in rows], _p(X),
+        info.ctypes.data_as(C.POINTER(C.c_int)), C.c_int(nthreads))
+    return np.ascontiguousarray(X.T), info
+
+
+def dense_ge(A: np.ndarray, f: np.ndarray) -> np.ndarray:
+    """Dense Gaussian elimination with partial pivoting (second, independent oracle)."""
+    A = _f64(A).copy()
+    f = _f64(f).copy()
+    N = A.shape[0]
+    x = np.zeros(N)
+    rc = _load().pent_oracle_dense_ge(C.c_int(N), _p(A), _p(f), _p(x))
+    if rc:
+        raise ArithmeticError("singular")
+    return x
+
+
+def rhs(fac: Factors, kind: int, bc: int, form: int, r: float, sigma: float, Cvec) -> np.ndarray:
+    """Right-hand side of one time step for one system (see pent_oracle_step.c)."""
+    Cvec = _f64(Cvec)
+    N = fac.N
+    out = np.empty(N)
+    work = np.empty(2 * N)
+    _load().pent_oracle_rhs(C.c_int(N), C.c_int(kind), C.c_int(bc), C.c_int(form),
+                            C.c_double(r), C.c_double(sigma), *[_p(v) for v in fac.diags],
+                            _p(Cvec), _p(out), _p(work))
+    return out
+
+
+def step_batch(fac: Factors, kind: int, bc: int, form: int, r: float, sigma: float,
+               c_interleaved, nsteps: int, nthreads: int = 1) -> np.ndarray:
+    """nsteps fused steps on an interleaved (N, M) state; returns the new state."""
+    Crows = to_rows(c_interleaved)
+    M = Crows.shape[0]
+    _load().pent_oracle_step_rows(
+        C.c_int(fac.N), C.c_long(M), C.c_int(kind), C.c_int(bc), C.c_int(form),
+        C.c_double(r), C.c_double(sigma), *[_p(v) for v in fac.diags],
+        _p(fac.eps), _p(fac.beta), _p(fac.alpha), _p(fac.gamma), _p(fac.delta),
+        _p(Crows), C.c_int(nsteps), C.c_int(nthreads))
+    return np.ascontiguousarray(Crows.T)
