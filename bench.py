@@ -1,0 +1,310 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the batched pentadiagonal solve (BASELINE.json metric:
+unknowns solved per second, N*M/t, and achieved HBM GB/s vs the B200 peak, fp64).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3] [--dtype f64]
+  python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
+  python bench.py --impl reference ...     (the CPU oracle, timed on the host cores)
+
+A "step" is one pass of the whole hot path over one batch: pent_solve_batch on an interleaved
+(N x M) right-hand-side array with the shared A factored beforehand (factor once, solve many:
+PAPER.md:273; timing excludes start-up as in PAPER.md:281).  Prints ONE JSON line.
+Multi-GPU: the path shards over systems with no collective; every rank
+solves its own M systems (weak scaling), value = all ranks' unknowns / max-over-ranks time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "unknowns_per_second"
+UNIT = "unknowns/s"
+FALLBACK_HBM_GBS = 6650.0        # /opt/skills/guides/B200_PROFILING.md fallback
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg3")
+    ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 thread-per-system, 2 chunked")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    return ap.parse_args()
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic(workload: str, dtype: str, kernel_name: str):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture
+    (profiles/dram_traffic.csv: workload,dtype,kernel,dram_bytes_read,dram_bytes_write), or None."""
+    p = os.path.join(ROOT, "profiles", "dram_traffic.csv")
+    try:
+        with open(p) as fh:
+            for line in fh:
+                parts = [s.strip() for s in line.split(",")]
+                if len(parts) >= 5 and parts[0] == workload and parts[1] == dtype and parts[2] == kernel_name:
+                    return float(parts[3]) + float(parts[4])
+    except Exception:
+        pass
+    return None
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons with NVML while the timed region runs."""
+
+    def __init__(self, index: int, period_s: float = 0.004):
+        self.index, self.period = index, period_s
+        self.samples, self.reasons = [], set()
+        self.max_mhz = None
+        self._stop = threading.Event()
+        self._t = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def _run(self):
+        nv = self.nv
+        names = {
+            nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
+            nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+            nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
+            nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap",
+        }
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def start(self):
+        if self.nv is not None:
+            self._t = threading.Thread(target=self._run, daemon=True)
+            self._t.start()
+
+    def stop(self):
+        self._stop.set()
+        if self._t is not None:
+            self._t.join()
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+def cpu_baseline(w, diags, sample_systems: int):
+    """The oracle as it stands, on the host cores, on a bounded sample of the same workload:
+    the first `sample_systems` systems, serial layout one system per row,
+    transposition outside the timed region; best of 3 for 1 thread and for all cores."""
+    import oracle
+    from pent_inputs.configs import make_rhs
+    m = min(sample_systems, w.M)
+    f = make_rhs(w, M=m)
+    if isinstance(f, tuple):
+        f = f[0]
+    fac = oracle.factor(*diags)
+    rows = oracle.to_rows(f)
+    cores = os.cpu_count() or 1
+    out = {}
+    for label, nt in (("1thread", 1), ("allcore", cores)):
+        best = float("inf")
+        for _ in range(3):
+            t0 = time.perf_counter()
+            oracle.solve_rows(fac, rows, nthreads=nt)
+            best = min(best, time.perf_counter() - t0)
+        out[label] = w.N * m / best
+    return {"value": out["allcore"], "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"first {m} of {w.M} systems of {w.name} (N={w.N}), serial layout, best of 3",
+            "value_1thread": out["1thread"]}
+
+
+def dist_env():
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    return rank, world, local
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle, as it stands, on the host cores (rank 0 only)."""
+    rank, world, _ = dist_env()
+    if rank != 0:
+        return
+    import oracle
+    from pent_inputs.configs import WORKLOADS, make_matrix, make_rhs
+    w = WORKLOADS[args.workload]
+    diags = make_matrix(w)
+    if args.dtype == "f32":
+        diags = tuple(np.asarray(v, dtype=np.float32).astype(np.float64) for v in diags)
+    m = min(8192, w.M)                       # bounded sample per step
+    f = make_rhs(w, M=m)
+    f = f[0] if isinstance(f, tuple) else f
+    fac = oracle.factor(*diags)
+    rows = oracle.to_rows(f)
+    cores = os.cpu_count() or 1
+    for _ in range(min(args.warmup, 3)):
+        oracle.solve_rows(fac, rows, nthreads=cores)
+    steps = min(args.steps, 50)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        oracle.solve_rows(fac, rows, nthreads=cores)
+    dt = time.perf_counter() - t0
+    val = w.N * m * steps / dt
+    sample = f"first {m} of {w.M} systems of {w.name} per step, {steps} steps, all cores"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": steps, "warmup": min(args.warmup, 3), "ms_per_step": 1e3 * dt / steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "config": {"workload": w.name, "N": w.N, "M": w.M, "sample_M": m},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    import paper_1807_07382_b200 as pent
+    from pent_inputs.configs import WORKLOADS, make_matrix, make_rhs
+
+    rank, world, local = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    w = WORKLOADS[args.workload]
+    if w.name in ("cfg4", "cfg5b"):
+        raise SystemExit("bench.py times the shared-A solve workloads (cfg1, cfg2, cfg3, cfg5a)")
+    tdt = torch.float64 if args.dtype == "f64" else torch.float32
+    esz = 8 if args.dtype == "f64" else 4
+    N, M = w.N, w.M
+    diags = make_matrix(w)
+    # weak scaling: rank r owns systems [r*M, (r+1)*M) of a batch of world*M systems
+    f = make_rhs(w, M=M, col0=rank * M) if w.rhs == "uniform" else make_rhs(w, M=M)
+    f = f[0] if isinstance(f, tuple) else f
+    a, b, c, d, e = (torch.tensor(v, dtype=tdt) for v in diags)
+    h = pent.pent_factor(N, e, c, d, a, b)                 # once, outside the timed region
+    f_host = torch.tensor(f, dtype=tdt).pin_memory()
+    fd = f_host.cuda()
+    xd = torch.empty_like(fd)
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        pent.pent_solve_batch(h, M, fd, xd, kernel=args.kernel)
+    barrier()
+    sampler = ClockSampler(local)
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    pent.launch_count(reset=True)
+    sampler.start()
+    evs[0].record(stream)
+    for i in range(args.steps):
+        pent.pent_solve_batch(h, M, fd, xd, kernel=args.kernel)
+        evs[i + 1].record(stream)
+    barrier()
+    clocks = sampler.stop()
+    launches = pent.launch_count()
+    total_ms = evs[0].elapsed_time(evs[-1])
+    per = np.array([evs[i].elapsed_time(evs[i + 1]) for i in range(args.steps)])
+    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms_max = float(t.item())
+    value = world * N * M * args.steps / (total_ms_max * 1e-3)
+
+    # end to end through the host-buffer entry point (H2D + solve + D2H inside the call)
+    e2e = None
+    if not args.no_e2e:
+        x_host = torch.empty_like(f_host).pin_memory()
+        pent.pent_solve_batch_host(h, M, f_host, x_host)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.e2e_steps):
+            pent.pent_solve_batch_host(h, M, f_host, x_host)
+        dt = time.perf_counter() - t0
+        t = torch.tensor([dt], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e = {"value": world * N * M * args.e2e_steps / float(t.item()), "unit": UNIT,
+               "h2d_bytes_per_step": N * M * esz, "d2h_bytes_per_step": N * M * esz,
+               "steps": args.e2e_steps, "api": "pent_solve_batch_host (pinned host buffers)"}
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    peak, peak_src = measured_peak()
+    choice = args.kernel if args.kernel else pent.lib().pent_solve_kernel_choice(h.ptr, M)
+    kname = "solve_chunked_kernel" if choice == 2 else "solve_tps_kernel"
+    alg_bytes = 2.0 * esz * N * M                # read f once, write x once
+    avg_ms = float(per.mean())
+    achieved = alg_bytes / (avg_ms * 1e-3) / 1e9
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": total_ms_max / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": args.dtype,
+        "data": "synthetic",
+        "config": {"workload": w.name, "N": N, "M_per_gpu": M, "matrix": f"I+sigma*L^2 {w.bc} sigma={w.sigma}",
+                   "rhs": w.rhs, "seed": w.seed, "layout": "interleaved f[k*M+i]", "kernel": kname,
+                   "l2": f"inputs+outputs {2 * esz * N * M >> 20} MiB per step exceed the 126 MB L2"},
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                     "frac": achieved / peak, "traffic": ncu_traffic(w.name, args.dtype, kname),
+                     "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes,
+                     "kernel": kname, "avg_launch_ms": avg_ms, "min_launch_ms": float(per.min()),
+                     "median_launch_ms": float(np.median(per)), "frac_of_8TBs": achieved / 8000.0},
+        "clocks": clocks, "gpu_launches": int(launches),
+    }
+    if e2e is not None:
+        line["e2e"] = e2e
+    if not args.no_cpu_baseline and world == 1:
+        line["cpu_baseline"] = cpu_baseline(w, diags, 16384)
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

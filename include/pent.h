@@ -1,0 +1,142 @@
+/* pent.h -- C ABI of the B200 (sm_100a) batched pentadiagonal solver.
+ *
+ * The library solves A x_i = f_i, i = 0..M-1, for an N x N pentadiagonal A by the extended
+ * Thomas algorithm of arXiv 1807.07382 ("cuPentBatch"): factor A = L R once
+ * (section II.D steps 1-14), then per system a forward sweep L g = f
+ * and a back substitution R x = g.  No pivoting is
+ * ever attempted (valid for SPD or diagonally dominant A).
+ *
+ * LAYOUT ("interleaved"): a batch is ONE array of N*M elements in which
+ * element k of system i is at index k*M + i.  Consecutive systems are consecutive in memory.
+ *
+ * DIAGONALS: five arrays indexed by ROW k = 0..N-1,
+ *     a[k] = A[k][k-2], b[k] = A[k][k-1], c[k] = A[k][k], d[k] = A[k][k+1], e[k] = A[k][k+2].
+ * a[0], a[1], b[0], d[N-1], e[N-2], e[N-1] lie outside the matrix and are NEVER READ.
+ * The positional order (N, e, c, d, a, b) is the one BASELINE.json's north_star writes.
+ *
+ * POINTERS: "device" = CUDA device memory of the current device; "host" = ordinary host
+ * memory; "host or device" = either (detected with cudaPointerGetAttributes).  The element
+ * type of every data pointer is `double` for PENT_F64 and `float` for PENT_F32.
+ * `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).
+ *
+ * OWNERSHIP: the caller owns every array it passes; a handle owns device copies of whatever
+ * it needs and never keeps a caller pointer.  Handles are immutable after creation and may
+ * be used from several streams/threads at once.  No hidden global state.
+ *
+ * ASYNCHRONY: every *_batch call only enqueues work on `stream` and returns; it never
+ * synchronises the host.  pent_factor / pent_factor_batch(info on host) synchronise.
+ *
+ * ERRORS: every int function returns one of the codes below; nothing is printed, nothing
+ * throws, and there is NO CPU fallback.
+ */
+#ifndef PENT_H_
+#define PENT_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pent_handle pent_handle;   /* opaque */
+
+typedef enum { PENT_F64 = 0, PENT_F32 = 1 } pent_dtype;
+
+enum {
+    PENT_OK = 0,
+    PENT_ERR_ARG = 1,      /* null pointer, N < 1, M < 0, bad dtype / params, handle of the wrong kind */
+    PENT_ERR_PIVOT = 2,    /* zero or non-finite pivot alpha_k (shared-A factor only)                   */
+    PENT_ERR_CUDA = 3,     /* a CUDA call failed; pent_last_cuda_error() holds its cudaError_t          */
+    PENT_ERR_ALLOC = 4     /* host or device allocation failed                                          */
+};
+
+/* Kernel choice for pent_solve_batch_v (measurement / tests).  AUTO is what pent_solve_batch uses. */
+enum {
+    PENT_KERNEL_AUTO = 0,
+    PENT_KERNEL_THREAD_PER_SYSTEM = 1,  /* the paper's design: one thread per system,
+                                           g round-trips through x in global memory (4 passes)         */
+    PENT_KERNEL_CHUNKED = 2             /* k split into chunks across threads, g kept in registers,
+                                           chunk coupling by the shared correction vectors (2 passes)  */
+};
+
+/* ---- shared A: factor once, solve many ("cuPentBatchConstant") -----------------
+ * pent_factor: e,c,d,a,b: N elements each, host or device, element type per `dtype`.
+ *   The factorisation itself runs in a device kernel in fp64 whatever the
+ *   dtype (fp32 inputs are widened exactly; the fp32 solve kernel reads rounded factors).
+ *   *out receives the handle.  If bad_row != NULL it receives -1, or the first 0-based row whose
+ *   pivot is zero / non-finite when PENT_ERR_PIVOT is returned (no handle is created then). */
+int pent_factor(int N, const void* e, const void* c, const void* d, const void* a, const void* b,
+                pent_dtype dtype, pent_handle** out, int* bad_row);
+
+/* pent_solve_batch: f, x: device, N*M elements, interleaved.  x == f (in place) is allowed;
+ *   any other overlap is undefined.  M == 0 is a no-op.  Forward + backward sweeps
+ *    for all M systems in one launch on `stream`. */
+int pent_solve_batch(const pent_handle* h, int64_t M, const void* f, void* x, void* stream);
+int pent_solve_batch_v(const pent_handle* h, int64_t M, const void* f, void* x, void* stream,
+                       int kernel);
+
+/* Same operation with HOST buffers (pageable or pinned): copies slabs of systems to the device,
+ * solves, copies back, pipelined on internal streams; returns when x_host is complete. */
+int pent_solve_batch_host(const pent_handle* h, int64_t M, const void* f_host, void* x_host);
+
+void pent_destroy(pent_handle* h);          /* NULL is allowed */
+
+/* ---- per-system matrices ("cuPentBatchRewrite") ---------------------------------
+ * e,c,d,a,b,f,x: device, N*M elements each, interleaved like f (diagonal entry k of system i at
+ * k*M+i).  info: device int[M] or NULL; info[i] = 0, or (first bad row + 1) if system i met a
+ * zero / non-finite pivot (its x is then unspecified; other systems are unaffected).
+ * pent_factor_solve_batch factors and solves in ONE kernel and keeps nothing.
+ * pent_factor_batch keeps the M factorisations in the handle (5*N*M elements of device memory)
+ * for repeated pent_solve_batch_multi calls (M is fixed by the handle). */
+int pent_factor_solve_batch(int N, int64_t M, const void* e, const void* c, const void* d,
+                            const void* a, const void* b, const void* f, void* x,
+                            pent_dtype dtype, int* info, void* stream);
+int pent_factor_batch(int N, int64_t M, const void* e, const void* c, const void* d,
+                      const void* a, const void* b, pent_dtype dtype, pent_handle** out,
+                      int* info, void* stream);
+int pent_solve_batch_multi(const pent_handle* h, const void* f, void* x, void* stream);
+
+/* ---- fused time stepping on a shared-A handle (BASELINE.json configs[3]) ----------------------
+ * One step = explicit right-hand side built from the state + one solve, fused in one kernel;
+ * `nsteps` steps are enqueued back to back on `stream`.
+ *  kind 0, Cahn-Hilliard (Eq. 2), L = second-difference matrix with boundary `bc`:
+ *     form 0 (direct):     A c+ = c + r L (c^3 - c)
+ *     form 1 (increment):  q = r (c^3 - c) - sigma L c;   A delta = L q;   c+ = c + delta
+ *     (algebraically identical; form 1 conserves mean(c) to rounding when bc = 1).
+ *  kind 1, hyperdiffusion Crank-Nicolson (PAPER.md:87-89 Eq. 6, :117 Eq. 7c):
+ *     A c+ = (2I - A) c, with the handle's own diagonals (bc, form, r, sigma ignored).
+ *  bc 0: Dirichlet L (diag -2, off 1).  bc 1: zero-flux L (corner diagonal entries -1).
+ *  The handle's A must be the matching I + sigma L^2 for kind 0; this is the caller's contract.
+ * c_inout: device, N*M, interleaved, updated in place.  scratch: device, N*M elements, or NULL
+ * (the library then allocates and frees a stream-ordered temporary). */
+typedef struct {
+    int kind;
+    int bc;
+    int form;
+    double r;       /* dt/dx^2 */
+    double sigma;   /* gamma dt/dx^4 */
+} pent_step_params;
+
+int pent_step_batch(const pent_handle* h, const pent_step_params* p, int64_t M,
+                    void* c_inout, void* scratch, int nsteps, void* stream);
+
+/* ---- introspection ------------------------------------------------------------------------ */
+int pent_handle_n(const pent_handle* h);                 /* N, or -1 */
+int pent_handle_dtype(const pent_handle* h);             /* pent_dtype, or -1 */
+int64_t pent_handle_m(const pent_handle* h);             /* M of a per-system handle, 0 for shared A */
+/* Copies the fp64 factor arrays (N doubles each; any pointer may be NULL) to HOST memory:
+ * eps, beta, alpha = bands of L, gamma, delta = bands of R (Eq. 13).  Shared-A only. */
+int pent_handle_factors(const pent_handle* h, double* eps, double* beta, double* alpha,
+                        double* gamma, double* delta);
+/* Which kernel PENT_KERNEL_AUTO picks for M systems on this handle (a PENT_KERNEL_* value). */
+int pent_solve_kernel_choice(const pent_handle* h, int64_t M);
+int pent_last_cuda_error(void);                         /* thread-local cudaError_t of the last PENT_ERR_CUDA */
+/* Number of kernel launches the library has enqueued from this thread since the last call with
+ * reset != 0 (used by bench.py for its gpu_launches field). */
+int64_t pent_launch_count(int reset);
+const char* pent_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PENT_H_ */

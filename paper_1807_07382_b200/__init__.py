@@ -1,0 +1,219 @@
+"""paper_1807_07382_b200 -- thin Python binding of libpent (include/pent.h).
+
+Argument marshalling only: every step of the path (factor, sweeps, fused time step) runs in
+the hand-written sm_100a kernels of `csrc/`.  PyTorch is used for device memory and streams.
+There is NO CPU fallback: if the CUDA library cannot be built or loaded, importing the
+compute entry points raises.  Names follow include/pent.h and the paper's notation
+(PAPER.md:152 a..e diagonals, :162-165 eps/beta/alpha/gamma/delta, :267 interleaved layout).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+
+import torch
+
+from . import build as _build
+
+PENT_F64, PENT_F32 = 0, 1
+KERNEL_AUTO, KERNEL_THREAD_PER_SYSTEM, KERNEL_CHUNKED = 0, 1, 2
+_ERR = {1: "invalid argument", 2: "zero or non-finite pivot", 3: "CUDA error", 4: "allocation failure"}
+
+_lib = None
+
+
+class PentError(RuntimeError):
+    def __init__(self, code: int, detail: str = ""):
+        super().__init__(f"libpent error {code} ({_ERR.get(code, '?')}){detail}")
+        self.code = code
+
+
+class SingularPivot(PentError):
+    def __init__(self, row: int):
+        super().__init__(2, f" at row {row}")
+        self.row = row
+
+
+class pent_step_params(C.Structure):
+    _fields_ = [("kind", C.c_int), ("bc", C.c_int), ("form", C.c_int),
+                ("r", C.c_double), ("sigma", C.c_double)]
+
+
+def lib() -> C.CDLL:
+    """Load (building if needed) libpent.so.  Raises if that is impossible."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB
+    if _build.needs_build():
+        path = _build.build()
+    L = C.CDLL(path)
+    vp, i64, ci = C.c_void_p, C.c_int64, C.c_int
+    L.pent_factor.argtypes = [ci, vp, vp, vp, vp, vp, ci, C.POINTER(vp), C.POINTER(ci)]
+    L.pent_solve_batch.argtypes = [vp, i64, vp, vp, vp]
+    L.pent_solve_batch_v.argtypes = [vp, i64, vp, vp, vp, ci]
+    L.pent_solve_batch_host.argtypes = [vp, i64, vp, vp]
+    L.pent_destroy.argtypes = [vp]
+    L.pent_destroy.restype = None
+    L.pent_factor_solve_batch.argtypes = [ci, i64, vp, vp, vp, vp, vp, vp, vp, ci, vp, vp]
+    L.pent_factor_batch.argtypes = [ci, i64, vp, vp, vp, vp, vp, ci, C.POINTER(vp), vp, vp]
+    L.pent_solve_batch_multi.argtypes = [vp, vp, vp, vp]
+    L.pent_step_batch.argtypes = [vp, C.POINTER(pent_step_params), i64, vp, vp, ci, vp]
+    L.pent_handle_n.argtypes = [vp]
+    L.pent_handle_dtype.argtypes = [vp]
+    L.pent_handle_m.argtypes = [vp]
+    L.pent_handle_m.restype = i64
+    L.pent_handle_factors.argtypes = [vp] * 6
+    L.pent_solve_kernel_choice.argtypes = [vp, i64]
+    L.pent_launch_count.argtypes = [ci]
+    L.pent_launch_count.restype = i64
+    L.pent_version.restype = C.c_char_p
+    _lib = L
+    return L
+
+
+def _check(rc: int):
+    if rc != 0:
+        detail = f", cudaError={lib().pent_last_cuda_error()}" if rc == 3 else ""
+        raise PentError(rc, detail)
+
+
+def _dt(t: torch.Tensor) -> int:
+    if t.dtype == torch.float64:
+        return PENT_F64
+    if t.dtype == torch.float32:
+        return PENT_F32
+    raise TypeError("fp64 or fp32 tensors only")
+
+
+def _stream(stream) -> int:
+    s = torch.cuda.current_stream() if stream is None else stream
+    return s.cuda_stream
+
+
+def _batch(t: torch.Tensor, name: str):
+    if not (t.is_cuda and t.is_contiguous() and t.dim() == 2):
+        raise ValueError(f"{name}: contiguous CUDA tensor of shape (N, M) expected (interleaved layout)")
+
+
+@dataclass
+class Handle:
+    """Owner of a pent_handle*.  Shared-A (from pent_factor) or per-system (pent_factor_batch)."""
+    ptr: int
+    N: int
+    dtype: torch.dtype
+    M: int = 0
+
+    def __del__(self):
+        if getattr(self, "ptr", 0) and _lib is not None:
+            _lib.pent_destroy(self.ptr)
+            self.ptr = 0
+
+    def factors(self):
+        """(eps, beta, alpha, gamma, delta) as fp64 CPU tensors (shared-A only)."""
+        out = [torch.empty(self.N, dtype=torch.float64) for _ in range(5)]
+        _check(lib().pent_handle_factors(self.ptr, *[o.data_ptr() for o in out]))
+        return tuple(out)
+
+
+def pent_factor(N: int, e, c, d, a, b) -> Handle:
+    """Factor A = L R once.  e,c,d,a,b: 1-D tensors of length N (CPU or CUDA,
+    fp64 or fp32), row-indexed diagonals in north_star's argument order."""
+    ts = [torch.as_tensor(v) for v in (e, c, d, a, b)]
+    dt = _dt(ts[1])
+    ts = [t.to(ts[1].dtype).contiguous() for t in ts]
+    if any(t.numel() != N for t in ts):
+        raise ValueError("each diagonal must have N entries")
+    if not torch.cuda.is_available():
+        raise RuntimeError("pent_factor needs a CUDA device (no CPU fallback)")
+    out = C.c_void_p()
+    bad = C.c_int(-1)
+    rc = lib().pent_factor(N, *[t.data_ptr() for t in ts], dt, C.byref(out), C.byref(bad))
+    if rc == 2:
+        raise SingularPivot(bad.value)
+    _check(rc)
+    return Handle(out.value, N, ts[1].dtype)
+
+
+def pent_solve_batch(h: Handle, M: int, f: torch.Tensor, x: torch.Tensor | None = None,
+                     stream=None, kernel: int = KERNEL_AUTO) -> torch.Tensor:
+    """Forward + backward sweeps for M systems; f, x of shape (N, M)."""
+    _batch(f, "f")
+    if x is None:
+        x = torch.empty_like(f)
+    _batch(x, "x")
+    if f.shape != (h.N, M) or x.shape != f.shape or f.dtype != h.dtype or x.dtype != h.dtype:
+        raise ValueError("f/x must have shape (N, M) and the handle's dtype")
+    _check(lib().pent_solve_batch_v(h.ptr, M, f.data_ptr(), x.data_ptr(), _stream(stream), kernel))
+    return x
+
+
+def pent_solve_batch_host(h: Handle, M: int, f_host: torch.Tensor,
+                          x_host: torch.Tensor | None = None) -> torch.Tensor:
+    """Same with CPU tensors (pinned or pageable); copies are inside the call."""
+    if f_host.is_cuda or not f_host.is_contiguous() or f_host.shape != (h.N, M) or f_host.dtype != h.dtype:
+        raise ValueError("f_host: contiguous CPU tensor (N, M) of the handle's dtype expected")
+    if x_host is None:
+        x_host = torch.empty_like(f_host)
+    _check(lib().pent_solve_batch_host(h.ptr, M, f_host.data_ptr(), x_host.data_ptr()))
+    return x_host
+
+
+def pent_factor_solve_batch(N: int, M: int, e, c, d, a, b, f, x=None, info=None, stream=None):
+    """Per-system matrices, factor + solve fused.  All tensors (N, M) on CUDA.
+    Returns (x, info) with info int32[M]: 0 or first bad row + 1."""
+    for t, n in zip((e, c, d, a, b, f), "ecdabf"):
+        _batch(t, n)
+        if t.shape != (N, M) or t.dtype != f.dtype:
+            raise ValueError("all arrays must be (N, M) of one dtype")
+    if x is None:
+        x = torch.empty_like(f)
+    if info is None:
+        info = torch.zeros(M, dtype=torch.int32, device=f.device)
+    _check(lib().pent_factor_solve_batch(N, M, e.data_ptr(), c.data_ptr(), d.data_ptr(),
+                                         a.data_ptr(), b.data_ptr(), f.data_ptr(), x.data_ptr(),
+                                         _dt(f), info.data_ptr(), _stream(stream)))
+    return x, info
+
+
+def pent_factor_batch(N: int, M: int, e, c, d, a, b, info=None, stream=None):
+    """Per-system factorisations kept in a handle for repeated pent_solve_batch_multi calls."""
+    for t, n in zip((e, c, d, a, b), "ecdab"):
+        _batch(t, n)
+        if t.shape != (N, M) or t.dtype != c.dtype:
+            raise ValueError("all arrays must be (N, M) of one dtype")
+    if info is None:
+        info = torch.zeros(M, dtype=torch.int32, device=c.device)
+    out = C.c_void_p()
+    _check(lib().pent_factor_batch(N, M, e.data_ptr(), c.data_ptr(), d.data_ptr(), a.data_ptr(),
+                                   b.data_ptr(), _dt(c), C.byref(out), info.data_ptr(),
+                                   _stream(stream)))
+    return Handle(out.value, N, c.dtype, M), info
+
+
+def pent_solve_batch_multi(h: Handle, f: torch.Tensor, x: torch.Tensor | None = None, stream=None):
+    _batch(f, "f")
+    if x is None:
+        x = torch.empty_like(f)
+    if f.shape != (h.N, h.M) or f.dtype != h.dtype or x.shape != f.shape:
+        raise ValueError("f must be (N, M) of the handle")
+    _check(lib().pent_solve_batch_multi(h.ptr, f.data_ptr(), x.data_ptr(), _stream(stream)))
+    return x
+
+
+def pent_step_batch(h: Handle, M: int, c: torch.Tensor, nsteps: int, *, kind: int = 0, bc: int = 1,
+                    form: int = 1, r: float = 0.0, sigma: float = 0.0,
+                    scratch: torch.Tensor | None = None, stream=None) -> torch.Tensor:
+    """nsteps fused steps (RHS + solve per kernel) in place on c (N, M).  See include/pent.h."""
+    _batch(c, "c")
+    if c.shape != (h.N, M) or c.dtype != h.dtype:
+        raise ValueError("c must be (N, M) of the handle's dtype")
+    p = pent_step_params(kind, bc, form, r, sigma)
+    sp = 0 if scratch is None else scratch.data_ptr()
+    _check(lib().pent_step_batch(h.ptr, C.byref(p), M, c.data_ptr(), sp, nsteps, _stream(stream)))
+    return c
+
+
+def launch_count(reset: bool = False) -> int:
+    return int(lib().pent_launch_count(1 if reset else 0))

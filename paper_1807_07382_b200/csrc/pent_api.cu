@@ -1,0 +1,93 @@
+// pent_api.cu -- shared-A solve entry points: kernel dispatch and the host-buffer variant.
+#include <algorithm>
+#include "pent_internal.h"
+
+extern "C" int pent_solve_batch_v(const pent_handle* h, int64_t M, const void* f, void* x,
+                                  void* stream, int kernel)
+{
+    if (!h || h->kind != 0 || M < 0) return PENT_ERR_ARG;
+    if (M == 0) return PENT_OK;
+    if (!f || !x) return PENT_ERR_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    switch (kernel) {
+        case PENT_KERNEL_AUTO:
+            if (pent::chunked_supported(h, M)) return pent::launch_solve_chunked(h, M, f, x, s);
+            return pent::launch_solve_tps(h, M, f, x, s);
+        case PENT_KERNEL_THREAD_PER_SYSTEM:
+            return pent::launch_solve_tps(h, M, f, x, s);
+        case PENT_KERNEL_CHUNKED:
+            if (!pent::chunked_supported(h, M)) return PENT_ERR_ARG;
+            return pent::launch_solve_chunked(h, M, f, x, s);
+        default:
+            return PENT_ERR_ARG;
+    }
+}
+
+extern "C" int pent_solve_kernel_choice(const pent_handle* h, int64_t M)
+{
+    if (!h || h->kind != 0) return -1;
+    return pent::chunked_supported(h, M) ? PENT_KERNEL_CHUNKED : PENT_KERNEL_THREAD_PER_SYSTEM;
+}
+
+extern "C" int pent_solve_batch(const pent_handle* h, int64_t M, const void* f, void* x,
+                                void* stream)
+{
+    return pent_solve_batch_v(h, M, f, x, stream, PENT_KERNEL_AUTO);
+}
+
+// Host buffers: the batch is cut into slabs of consecutive systems.  A slab of an interleaved
+// (N x M) array is a strided 2-D region (N rows of Ms elements, pitch M), moved with
+// cudaMemcpy2DAsync into a dense (N x Ms) device array, solved there and moved back.  Three
+// slabs rotate over three streams so the upload of slab j+1, the solve of slab j and the
+// download of slab j-1 overlap (PCIe is full duplex).
+extern "C" int pent_solve_batch_host(const pent_handle* h, int64_t M, const void* f_host,
+                                     void* x_host)
+{
+    if (!h || h->kind != 0 || M < 0) return PENT_ERR_ARG;
+    if (M == 0) return PENT_OK;
+    if (!f_host || !x_host) return PENT_ERR_ARG;
+    const size_t esz = h->dtype == PENT_F64 ? 8 : 4;
+    const int N = h->N;
+    // ~32 MiB slabs, a multiple of 256 systems
+    int64_t Ms = std::max<int64_t>(256, ((32ll << 20) / ((int64_t)N * (int64_t)esz)) / 256 * 256);
+    Ms = std::min(Ms, M);
+    const int NB = 3;
+    void* buf[NB] = {nullptr, nullptr, nullptr};
+    cudaStream_t st[NB] = {nullptr, nullptr, nullptr};
+    int rc = PENT_OK;
+    auto cleanup = [&]() {
+        for (int j = 0; j < NB; ++j) {
+            if (st[j]) { cudaStreamSynchronize(st[j]); cudaStreamDestroy(st[j]); }
+            cudaFree(buf[j]);
+        }
+    };
+    for (int j = 0; j < NB && rc == PENT_OK; ++j) {
+        cudaError_t e = cudaMalloc(&buf[j], (size_t)N * (size_t)Ms * esz);
+        if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); rc = PENT_ERR_ALLOC; break; }
+        if (e != cudaSuccess) { rc = pent::cuda_fail(e); break; }
+        e = cudaStreamCreateWithFlags(&st[j], cudaStreamNonBlocking);
+        if (e != cudaSuccess) rc = pent::cuda_fail(e);
+    }
+    int64_t slab = 0;
+    for (int64_t i0 = 0; i0 < M && rc == PENT_OK; i0 += Ms, ++slab) {
+        int j = (int)(slab % NB);
+        int64_t m = std::min(Ms, M - i0);
+        const char* src = (const char*)f_host + (size_t)i0 * esz;
+        char* dst = (char*)x_host + (size_t)i0 * esz;
+        cudaError_t e = cudaMemcpy2DAsync(buf[j], (size_t)m * esz, src, (size_t)M * esz,
+                                          (size_t)m * esz, (size_t)N, cudaMemcpyHostToDevice, st[j]);
+        if (e != cudaSuccess) { rc = pent::cuda_fail(e); break; }
+        rc = pent_solve_batch(h, m, buf[j], buf[j], st[j]);
+        if (rc != PENT_OK) break;
+        e = cudaMemcpy2DAsync(dst, (size_t)M * esz, buf[j], (size_t)m * esz, (size_t)m * esz,
+                              (size_t)N, cudaMemcpyDeviceToHost, st[j]);
+        if (e != cudaSuccess) { rc = pent::cuda_fail(e); break; }
+    }
+    for (int j = 0; j < NB; ++j)
+        if (st[j]) {
+            cudaError_t e = cudaStreamSynchronize(st[j]);
+            if (e != cudaSuccess && rc == PENT_OK) rc = pent::cuda_fail(e);
+        }
+    cleanup();
+    return rc;
+}

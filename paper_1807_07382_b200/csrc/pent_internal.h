@@ -1,0 +1,71 @@
+// pent_internal.h -- private declarations shared by the .cu files of libpent (not installed).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "pent.h"
+
+// Chunk length (rows per thread) of the chunked solve kernel; the correction vectors in the
+// handle are computed for this value.
+#define PENT_CHUNK 32
+
+struct pent_handle {
+    int kind;            // 0 = shared A, 1 = per-system factors
+    int N;
+    pent_dtype dtype;
+    int64_t M;           // per-system only
+    // ---- shared A, all device memory ----
+    double* diag;        // 5*N: a,b,c,d,e widened to fp64, out-of-matrix entries zeroed
+    double* fac;         // 5*N: eps,beta,alpha,gamma,delta (Eq. 13), fp64
+    void* fw;            // N x {1/alpha, eps/alpha, beta/alpha, 0}   in T (T4)
+    void* bw;            // N x {gamma, delta}                        in T (T2)
+    void* cf;            // chunked kernel: N x {1/alpha, eps/alpha, beta/alpha, phi0, phi1, 0..} see pent_factor.cu
+    void* cb;            // chunked kernel: N x {gamma, delta, psi0, psi1}
+    void* dg;            // N x {a,b,c,d,e,0,0,0} in T, for the (2I-A)c right-hand side
+    int nchunks;         // ceil(N / PENT_CHUNK)
+    // ---- per-system factors, device, interleaved, in T ----
+    void* ms;            // 5*N*M: ia, en, bn, gamma, delta
+};
+
+namespace pent {
+
+extern thread_local int g_last_cuda_error;
+extern thread_local int64_t g_launches;
+
+inline int cuda_fail(cudaError_t e) { g_last_cuda_error = (int)e; return PENT_ERR_CUDA; }
+inline void count_launch(int n = 1) { g_launches += n; }
+
+#define PENT_CUDA(call)                                           \
+    do {                                                          \
+        cudaError_t e__ = (call);                                 \
+        if (e__ != cudaSuccess) return ::pent::cuda_fail(e__);    \
+    } while (0)
+
+#define PENT_LAUNCH_CHECK()                                       \
+    do {                                                          \
+        cudaError_t e__ = cudaGetLastError();                     \
+        if (e__ != cudaSuccess) return ::pent::cuda_fail(e__);    \
+    } while (0)
+
+template <typename T> struct Vec;
+template <> struct Vec<double> { using T2 = double2; using T4 = double4; };
+template <> struct Vec<float>  { using T2 = float2;  using T4 = float4;  };
+
+#ifdef __CUDACC__
+// read-only-path loads of the coefficient tuples (warp-uniform addresses: one broadcast each)
+__device__ __forceinline__ double4 ldg4(const double4* p)
+{
+    const double2* q = reinterpret_cast<const double2*>(p);
+    double2 lo = __ldg(q), hi = __ldg(q + 1);
+    return make_double4(lo.x, lo.y, hi.x, hi.y);
+}
+__device__ __forceinline__ float4 ldg4(const float4* p) { return __ldg(p); }
+__device__ __forceinline__ double2 ldg2(const double2* p) { return __ldg(p); }
+__device__ __forceinline__ float2 ldg2(const float2* p) { return __ldg(p); }
+#endif
+
+// kernels / launchers implemented across the .cu files
+int launch_solve_tps(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s);
+int launch_solve_chunked(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s);
+bool chunked_supported(const pent_handle* h, int64_t M);
+
+}  // namespace pent

@@ -1,0 +1,258 @@
+// pent_solve_tps.cu -- "thread per system" kernels: the paper's own GPU design
+// (interleaved layout, one thread per system, everything in global memory).
+// Consecutive threads own consecutive systems, so every access f[k*M+i] of a warp is one
+// contiguous, coalesced segment.  The intermediate vector g round-trips through x (the paper
+// overwrites the right-hand side): 4 passes over the batch.  This is the
+// reference design and the HBM-spill path for N too large to keep on chip; the headline
+// kernel is in pent_solve_chunked.cu.
+#include <new>
+#include "pent_internal.h"
+
+namespace pent {
+
+constexpr int TPS_UNROLL = 8;
+
+// Shared A.  Forward sweep with pre-normalised coefficients, then back
+// substitution.  The coefficient loads are warp-uniform (one broadcast
+// transaction); the f loads of TPS_UNROLL rows are issued together before the dependent FMA chain.
+template <typename T>
+__global__ void __launch_bounds__(128)
+solve_tps_kernel(int N, int64_t M, const typename Vec<T>::T4* __restrict__ fw,
+                 const typename Vec<T>::T2* __restrict__ bw, const T* f, T* x)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= M) return;
+    const T* fi = f + i;
+    T* xi = x + i;
+    T g1 = 0, g2 = 0;
+    int k = 0;
+    for (; k + TPS_UNROLL <= N; k += TPS_UNROLL) {
+        T v[TPS_UNROLL];
+#pragma unroll
+        for (int u = 0; u < TPS_UNROLL; ++u) v[u] = __ldcs(fi + (int64_t)(k + u) * M);
+#pragma unroll
+        for (int u = 0; u < TPS_UNROLL; ++u) {
+            typename Vec<T>::T4 c = ldg4(fw + k + u);
+            T g = fma(-c.z, g1, fma(-c.y, g2, c.x * v[u]));
+            xi[(int64_t)(k + u) * M] = g;
+            g2 = g1; g1 = g;
+        }
+    }
+    for (; k < N; ++k) {
+        typename Vec<T>::T4 c = ldg4(fw + k);
+        T g = fma(-c.z, g1, fma(-c.y, g2, c.x * fi[(int64_t)k * M]));
+        xi[(int64_t)k * M] = g;
+        g2 = g1; g1 = g;
+    }
+    T x1 = 0, x2 = 0;
+    k = N - 1;
+    for (; k - TPS_UNROLL + 1 >= 0; k -= TPS_UNROLL) {
+        T v[TPS_UNROLL];
+#pragma unroll
+        for (int u = 0; u < TPS_UNROLL; ++u) v[u] = xi[(int64_t)(k - u) * M];
+#pragma unroll
+        for (int u = 0; u < TPS_UNROLL; ++u) {
+            typename Vec<T>::T2 c = ldg2(bw + k - u);
+            T xv = fma(-c.y, x2, fma(-c.x, x1, v[u]));
+            __stcs(xi + (int64_t)(k - u) * M, xv);
+            x2 = x1; x1 = xv;
+        }
+    }
+    for (; k >= 0; --k) {
+        typename Vec<T>::T2 c = ldg2(bw + k);
+        T xv = fma(-c.y, x2, fma(-c.x, x1, xi[(int64_t)k * M]));
+        xi[(int64_t)k * M] = xv;
+        x2 = x1; x1 = xv;
+    }
+}
+
+int launch_solve_tps(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s)
+{
+    const int tb = 128;
+    unsigned nb = (unsigned)((M + tb - 1) / tb);
+    if (h->dtype == PENT_F64)
+        solve_tps_kernel<double><<<nb, tb, 0, s>>>(h->N, M, (const double4*)h->fw,
+                                                   (const double2*)h->bw, (const double*)f, (double*)x);
+    else
+        solve_tps_kernel<float><<<nb, tb, 0, s>>>(h->N, M, (const float4*)h->fw,
+                                                  (const float2*)h->bw, (const float*)f, (float*)x);
+    count_launch();
+    PENT_LAUNCH_CHECK();
+    return PENT_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Per-system matrices.  Thread i factors A_i on the fly (the paper's steps 8.1-8.4 with
+// out-of-matrix entries masked to zero) while sweeping forward, keeps gamma_k, delta_k (needed
+// again by the back substitution) in two batch-sized arrays and g in x.
+// One reciprocal per row; every other division becomes a multiply.
+//   MODE 0: fused factor+solve (gam/del are scratch)      -- pent_factor_solve_batch
+//   MODE 1: factor only, store ia,en,bn,gamma,delta        -- pent_factor_batch
+// ---------------------------------------------------------------------------------------------
+template <typename T, int MODE>
+__global__ void __launch_bounds__(128)
+factor_tps_kernel(int N, int64_t M, const T* __restrict__ a, const T* __restrict__ b,
+                  const T* __restrict__ c, const T* __restrict__ d, const T* __restrict__ e,
+                  const T* f, T* x, T* __restrict__ gam, T* __restrict__ del,
+                  T* __restrict__ ia_o, T* __restrict__ en_o, T* __restrict__ bn_o,
+                  int* __restrict__ info)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= M) return;
+    T ga1 = 0, ga2 = 0, de1 = 0, de2 = 0, g1 = 0, g2 = 0;
+    int bad = 0;
+    for (int k = 0; k < N; ++k) {
+        int64_t o = (int64_t)k * M + i;
+        T ak = (k >= 2) ? __ldcs(a + o) : (T)0;
+        T bk = (k >= 1) ? __ldcs(b + o) : (T)0;
+        T ck = __ldcs(c + o);
+        T dk = (k + 1 < N) ? __ldcs(d + o) : (T)0;
+        T ek = (k + 2 < N) ? __ldcs(e + o) : (T)0;
+        T be = fma(-ak, ga2, bk);
+        T al = fma(-be, ga1, fma(-ak, de2, ck));
+        if (bad == 0 && (al == (T)0 || !isfinite(al))) bad = k + 1;
+        T inv = (T)1 / al;
+        T ga = fma(-be, de1, dk) * inv;
+        T de = ek * inv;
+        gam[o] = ga; del[o] = de;
+        if (MODE == 0) {
+            T g = fma(-be, g1, fma(-ak, g2, f[o])) * inv;
+            x[o] = g;
+            g2 = g1; g1 = g;
+        } else {
+            ia_o[o] = inv; en_o[o] = ak * inv; bn_o[o] = be * inv;
+        }
+        ga2 = ga1; ga1 = ga; de2 = de1; de1 = de;
+    }
+    if (info) info[i] = bad;
+    if (MODE == 0) {
+        T x1 = 0, x2 = 0;
+        for (int k = N - 1; k >= 0; --k) {
+            int64_t o = (int64_t)k * M + i;
+            T xv = fma(-del[o], x2, fma(-gam[o], x1, x[o]));
+            __stcs(x + o, xv);
+            x2 = x1; x1 = xv;
+        }
+    }
+}
+
+// Solve with stored per-system factors (layout ms: ia, en, bn, gamma, delta, each N*M).
+template <typename T>
+__global__ void __launch_bounds__(128)
+solve_multi_kernel(int N, int64_t M, const T* __restrict__ ms, const T* f, T* x)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= M) return;
+    const int64_t NM = (int64_t)N * M;
+    T g1 = 0, g2 = 0;
+    for (int k = 0; k < N; ++k) {
+        int64_t o = (int64_t)k * M + i;
+        T g = fma(-ms[2 * NM + o], g1, fma(-ms[NM + o], g2, ms[o] * f[o]));
+        x[o] = g;
+        g2 = g1; g1 = g;
+    }
+    T x1 = 0, x2 = 0;
+    for (int k = N - 1; k >= 0; --k) {
+        int64_t o = (int64_t)k * M + i;
+        T xv = fma(-ms[4 * NM + o], x2, fma(-ms[3 * NM + o], x1, x[o]));
+        x[o] = xv;
+        x2 = x1; x1 = xv;
+    }
+}
+
+template <typename T>
+static int factor_solve_impl(int N, int64_t M, const void* e, const void* c, const void* d,
+                             const void* a, const void* b, const void* f, void* x, int* info,
+                             cudaStream_t s)
+{
+    T* scratch = nullptr;
+    size_t NM = (size_t)N * (size_t)M;
+    cudaError_t er = cudaMallocAsync((void**)&scratch, 2 * NM * sizeof(T), s);
+    if (er == cudaErrorMemoryAllocation) { cudaGetLastError(); return PENT_ERR_ALLOC; }
+    PENT_CUDA(er);
+    const int tb = 128;
+    unsigned nb = (unsigned)((M + tb - 1) / tb);
+    factor_tps_kernel<T, 0><<<nb, tb, 0, s>>>(N, M, (const T*)a, (const T*)b, (const T*)c,
+                                              (const T*)d, (const T*)e, (const T*)f, (T*)x,
+                                              scratch, scratch + NM, nullptr, nullptr, nullptr, info);
+    count_launch();
+    cudaError_t le = cudaGetLastError();
+    cudaFreeAsync(scratch, s);
+    if (le != cudaSuccess) return cuda_fail(le);
+    return PENT_OK;
+}
+
+template <typename T>
+static int factor_batch_impl(pent_handle* h, const void* e, const void* c, const void* d,
+                             const void* a, const void* b, int* info_dev, cudaStream_t s)
+{
+    size_t NM = (size_t)h->N * (size_t)h->M;
+    T* ms = (T*)h->ms;
+    const int tb = 128;
+    unsigned nb = (unsigned)((h->M + tb - 1) / tb);
+    factor_tps_kernel<T, 1><<<nb, tb, 0, s>>>(h->N, h->M, (const T*)a, (const T*)b, (const T*)c,
+                                              (const T*)d, (const T*)e, nullptr, nullptr,
+                                              ms + 3 * NM, ms + 4 * NM, ms, ms + NM, ms + 2 * NM,
+                                              info_dev);
+    count_launch();
+    PENT_LAUNCH_CHECK();
+    return PENT_OK;
+}
+}  // namespace pent
+
+extern "C" int pent_factor_solve_batch(int N, int64_t M, const void* e, const void* c,
+                                       const void* d, const void* a, const void* b,
+                                       const void* f, void* x, pent_dtype dtype, int* info,
+                                       void* stream)
+{
+    if (N < 1 || M < 0 || !e || !c || !d || !a || !b || !f || !x) return PENT_ERR_ARG;
+    if (M == 0) return PENT_OK;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (dtype == PENT_F64) return pent::factor_solve_impl<double>(N, M, e, c, d, a, b, f, x, info, s);
+    if (dtype == PENT_F32) return pent::factor_solve_impl<float>(N, M, e, c, d, a, b, f, x, info, s);
+    return PENT_ERR_ARG;
+}
+
+extern "C" int pent_factor_batch(int N, int64_t M, const void* e, const void* c, const void* d,
+                                 const void* a, const void* b, pent_dtype dtype,
+                                 pent_handle** out, int* info, void* stream)
+{
+    if (!out) return PENT_ERR_ARG;
+    *out = nullptr;
+    if (N < 1 || M < 1 || !e || !c || !d || !a || !b) return PENT_ERR_ARG;
+    if (dtype != PENT_F64 && dtype != PENT_F32) return PENT_ERR_ARG;
+    pent_handle* h = new (std::nothrow) pent_handle();
+    if (!h) return PENT_ERR_ALLOC;
+    *h = pent_handle{};
+    h->kind = 1; h->N = N; h->M = M; h->dtype = dtype;
+    size_t esz = dtype == PENT_F64 ? 8 : 4;
+    cudaError_t er = cudaMalloc(&h->ms, 5 * (size_t)N * (size_t)M * esz);
+    if (er != cudaSuccess) {
+        cudaGetLastError();
+        delete h;
+        return er == cudaErrorMemoryAllocation ? PENT_ERR_ALLOC : pent::cuda_fail(er);
+    }
+    int rc = dtype == PENT_F64
+                 ? pent::factor_batch_impl<double>(h, e, c, d, a, b, info, (cudaStream_t)stream)
+                 : pent::factor_batch_impl<float>(h, e, c, d, a, b, info, (cudaStream_t)stream);
+    if (rc != PENT_OK) { pent_destroy(h); return rc; }
+    *out = h;
+    return PENT_OK;
+}
+
+extern "C" int pent_solve_batch_multi(const pent_handle* h, const void* f, void* x, void* stream)
+{
+    if (!h || h->kind != 1 || !f || !x) return PENT_ERR_ARG;
+    const int tb = 128;
+    unsigned nb = (unsigned)((h->M + tb - 1) / tb);
+    cudaStream_t s = (cudaStream_t)stream;
+    if (h->dtype == PENT_F64)
+        pent::solve_multi_kernel<double><<<nb, tb, 0, s>>>(h->N, h->M, (const double*)h->ms,
+                                                           (const double*)f, (double*)x);
+    else
+        pent::solve_multi_kernel<float><<<nb, tb, 0, s>>>(h->N, h->M, (const float*)h->ms,
+                                                          (const float*)f, (float*)x);
+    pent::count_launch();
+    PENT_LAUNCH_CHECK();
+    return PENT_OK;
+}

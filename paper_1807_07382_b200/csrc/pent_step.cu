@@ -1,0 +1,133 @@
+// pent_step.cu -- fused time step: explicit right-hand side + pentadiagonal solve in ONE kernel
+// (BASELINE.json configs[3]; the paper runs the RHS as a separate stencil kernel).
+//
+//  kind 0  Cahn-Hilliard, PAPER.md:53 (Eq. 2):  A c+ = c + r L (c^3 - c)           (form 0)
+//          increment form:  q = r (c^3 - c) - sigma L c ;  A delta = L q ;  c+ = c + delta  (form 1)
+//  kind 1  hyperdiffusion Crank-Nicolson, PAPER.md:87-89 (Eq. 6), :117 (Eq. 7c):  A c+ = (2I - A) c
+//  L = second-difference matrix: (L v)_k = v_{k-1} + dg_k v_k + v_{k+1}, out-of-range terms
+//  dropped, dg_k = -2 except dg_0 = dg_{N-1} = -1 when bc = 1 (zero-flux).
+//
+// Thread-per-system version: the state is read through a sliding window of rows held in
+// registers (each c_k is loaded exactly once in the forward sweep), the right-hand side of
+// row k is formed in registers and consumed at once by the forward recurrence; g goes to
+// `scratch`; the back substitution writes the new state in place.
+#include "pent_internal.h"
+
+namespace pent {
+
+template <typename T>
+struct StepCoef {
+    int kind, bc, form;
+    T r, sigma;
+};
+
+template <typename T>
+__device__ __forceinline__ T Ldiag(int k, int N, int bc)
+{
+    return (bc == 1 && (k == 0 || k == N - 1)) ? (T)-1 : (T)-2;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(128)
+step_tps_kernel(int N, int64_t M, const typename Vec<T>::T4* __restrict__ fw,
+                const typename Vec<T>::T2* __restrict__ bw, const T* __restrict__ dgt,
+                StepCoef<T> p, T* c, T* __restrict__ scratch)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= M) return;
+    T* ci = c + i;
+    T* gi = scratch + i;
+    // window: cm2 = c_{k-2}, cm1 = c_{k-1}, c0 = c_k, cp1 = c_{k+1}, cp2 = c_{k+2}
+    T cm2 = 0, cm1 = 0;
+    T c0 = ci[0];
+    T cp1 = (N > 1) ? ci[M] : (T)0;
+    T cp2 = (N > 2) ? ci[2 * M] : (T)0;
+    // kind 0 carries: w_{k-1}, w_k (form 0) or q_{k-1}, q_k (form 1)
+    T um1 = 0, u0 = 0;
+    if (p.kind == 0) {
+        T w0 = c0 * c0 * c0 - c0;
+        if (p.form == 0) u0 = w0;
+        else u0 = fma(-p.sigma, fma(Ldiag<T>(0, N, p.bc), c0, cp1), p.r * w0);   // q_0
+    }
+    T g1 = 0, g2 = 0;
+    for (int k = 0; k < N; ++k) {
+        T cn = (k + 3 < N) ? __ldcs(ci + (int64_t)(k + 3) * M) : (T)0;   // c_{k+3}, prefetch
+        T rhs;
+        if (p.kind == 1) {
+            const T* dk = dgt + 8 * k;
+            T s = __ldg(dk + 2) * c0;
+            s = fma(__ldg(dk + 1), cm1, s);
+            s = fma(__ldg(dk + 0), cm2, s);
+            s = fma(__ldg(dk + 3), cp1, s);
+            s = fma(__ldg(dk + 4), cp2, s);
+            rhs = (T)2 * c0 - s;
+        } else {
+            // u_{k+1}: w_{k+1} or q_{k+1} (zero beyond the last row)
+            T up1 = 0;
+            if (k + 1 < N) {
+                T w1 = cp1 * cp1 * cp1 - cp1;
+                if (p.form == 0) up1 = w1;
+                else up1 = fma(-p.sigma, c0 + fma(Ldiag<T>(k + 1, N, p.bc), cp1, cp2), p.r * w1);
+            }
+            T Lu = um1 + fma(Ldiag<T>(k, N, p.bc), u0, up1);
+            rhs = (p.form == 0) ? fma(p.r, Lu, c0) : Lu;
+            um1 = u0; u0 = up1;
+        }
+        typename Vec<T>::T4 cf = ldg4(fw + k);
+        T g = fma(-cf.z, g1, fma(-cf.y, g2, cf.x * rhs));
+        gi[(int64_t)k * M] = g;
+        g2 = g1; g1 = g;
+        cm2 = cm1; cm1 = c0; c0 = cp1; cp1 = cp2; cp2 = cn;
+    }
+    T x1 = 0, x2 = 0;
+    const bool incr = (p.kind == 0 && p.form == 1);
+    for (int k = N - 1; k >= 0; --k) {
+        typename Vec<T>::T2 cb = ldg2(bw + k);
+        T xv = fma(-cb.y, x2, fma(-cb.x, x1, gi[(int64_t)k * M]));
+        T out = incr ? ci[(int64_t)k * M] + xv : xv;
+        ci[(int64_t)k * M] = out;
+        x2 = x1; x1 = xv;
+    }
+}
+
+template <typename T>
+static int step_impl(const pent_handle* h, const pent_step_params* p, int64_t M, void* c,
+                     void* scratch, int nsteps, cudaStream_t s)
+{
+    T* sc = (T*)scratch;
+    bool own = false;
+    if (!sc) {
+        cudaError_t er = cudaMallocAsync((void**)&sc, (size_t)h->N * (size_t)M * sizeof(T), s);
+        if (er == cudaErrorMemoryAllocation) { cudaGetLastError(); return PENT_ERR_ALLOC; }
+        PENT_CUDA(er);
+        own = true;
+    }
+    StepCoef<T> sp{p->kind, p->bc, p->form, (T)p->r, (T)p->sigma};
+    const int tb = 128;
+    unsigned nb = (unsigned)((M + tb - 1) / tb);
+    cudaError_t le = cudaSuccess;
+    for (int it = 0; it < nsteps && le == cudaSuccess; ++it) {
+        step_tps_kernel<T><<<nb, tb, 0, s>>>(h->N, M, (const typename Vec<T>::T4*)h->fw,
+                                             (const typename Vec<T>::T2*)h->bw, (const T*)h->dg,
+                                             sp, (T*)c, sc);
+        count_launch();
+        le = cudaGetLastError();
+    }
+    if (own) cudaFreeAsync(sc, s);
+    if (le != cudaSuccess) return cuda_fail(le);
+    return PENT_OK;
+}
+}  // namespace pent
+
+extern "C" int pent_step_batch(const pent_handle* h, const pent_step_params* p, int64_t M,
+                               void* c_inout, void* scratch, int nsteps, void* stream)
+{
+    if (!h || h->kind != 0 || !p || M < 0 || nsteps < 0 || !c_inout) return PENT_ERR_ARG;
+    if (p->kind != 0 && p->kind != 1) return PENT_ERR_ARG;
+    if (p->kind == 0 && ((p->bc != 0 && p->bc != 1) || (p->form != 0 && p->form != 1)))
+        return PENT_ERR_ARG;
+    if (M == 0 || nsteps == 0) return PENT_OK;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (h->dtype == PENT_F64) return pent::step_impl<double>(h, p, M, c_inout, scratch, nsteps, s);
+    return pent::step_impl<float>(h, p, M, c_inout, scratch, nsteps, s);
+}

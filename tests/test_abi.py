@@ -1,0 +1,63 @@
+"""CPU-only checks of the boundary: libpent.so builds (nvcc cross-compiles sm_100a without a
+GPU), loads, and exports every function include/pent.h declares.  No compute call is made."""
+import ctypes
+import os
+import re
+import subprocess
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _declared_functions():
+    src = open(os.path.join(ROOT, "include", "pent.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    names = re.findall(r"\b(pent_[a-z0-9_]+)\s*\(", src)
+    return sorted(set(names))
+
+
+def test_header_declares_the_boundary():
+    names = _declared_functions()
+    for required in ("pent_factor", "pent_solve_batch", "pent_destroy", "pent_factor_solve_batch",
+                     "pent_factor_batch", "pent_solve_batch_multi", "pent_step_batch",
+                     "pent_solve_batch_host"):
+        assert required in names
+
+
+def test_library_builds_loads_and_exports_every_symbol():
+    from paper_1807_07382_b200 import build
+    path = build.build()
+    lib = ctypes.CDLL(path)
+    for name in _declared_functions():
+        assert hasattr(lib, name), f"{name} declared in include/pent.h but not exported"
+    lib.pent_version.restype = ctypes.c_char_p
+    assert b"sm_100a" in lib.pent_version()
+    # argument validation needs no GPU
+    assert lib.pent_solve_batch(None, 1, None, None, None) == 1
+    assert lib.pent_handle_n(None) == -1
+
+
+def test_library_is_sm100a_only_and_has_no_cpu_fallback():
+    from paper_1807_07382_b200 import build
+    path = build.build()
+    out = subprocess.run(["cuobjdump", "-lelf", path], capture_output=True, text=True).stdout
+    archs = set(re.findall(r"sm_(\d+a?)", out))
+    assert archs == {"100a"}, archs
+    # the product never imports the oracle
+    pkg = os.path.join(ROOT, "paper_1807_07382_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for fn in files:
+            if fn.endswith((".py", ".cu", ".h", ".cuh")):
+                text = open(os.path.join(dirpath, fn)).read()
+                assert "import oracle" not in text and "pent_oracle" not in text, fn
+
+
+def test_binding_refuses_without_gpu():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    import paper_1807_07382_b200 as pent
+    d = torch.ones(8, dtype=torch.float64)
+    with pytest.raises(RuntimeError):
+        pent.pent_factor(8, d, d, d, d, d)

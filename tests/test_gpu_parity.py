@@ -1,0 +1,205 @@
+"""GPU parity: the CUDA path (through the C ABI binding) against the CPU oracle, element by
+element on the same seeded inputs.  Tolerances are north_star's:
+normwise per system  max_k|x-x_ref| / max_k|x_ref| <= 1e-11 (fp64), 2e-5 (fp32);
+relative residual ||A x - f||_2/||f||_2 <= 1e-12 (fp64), 1e-5 (fp32), A x evaluated in fp64 on
+the CPU from the ORIGINAL diagonals."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import pent_inputs as pin
+from pent_inputs.configs import WORKLOADS, banded_matvec, make_matrix, make_rhs, sine_modes
+
+pytestmark = pytest.mark.gpu
+
+TOL = {torch.float64: (1e-11, 1e-12), torch.float32: (2e-5, 1e-5)}
+
+
+def _pent():
+    import paper_1807_07382_b200 as pent
+    return pent
+
+
+def normwise(x, ref):
+    return float(np.max(np.max(np.abs(x - ref), axis=0) / np.max(np.abs(ref), axis=0)))
+
+
+def residual(diags, x, f):
+    r = banded_matvec(*diags, x.astype(np.float64)) - f
+    return float(np.max(np.linalg.norm(r, axis=0) / np.linalg.norm(f, axis=0)))
+
+
+def gpu_solve(diags, f, dtype=torch.float64, kernel=0, inplace=False):
+    pent = _pent()
+    a, b, c, d, e = (torch.tensor(v, dtype=dtype) for v in diags)
+    N, M = f.shape
+    h = pent.pent_factor(N, e, c, d, a, b)
+    fd = torch.tensor(f, dtype=dtype, device="cuda")
+    xd = pent.pent_solve_batch(h, M, fd, fd if inplace else None, kernel=kernel)
+    torch.cuda.synchronize()
+    return xd.cpu().numpy(), h
+
+
+def oracle_for_dtype(diags, f, dtype):
+    """fp32: the oracle solves the ROUNDED inputs in fp64."""
+    if dtype == torch.float32:
+        diags = tuple(np.asarray(v, dtype=np.float32).astype(np.float64) for v in diags)
+        f = f.astype(np.float32).astype(np.float64)
+    return diags, f, oracle.solve_batch(oracle.factor(*diags), f, nthreads=8)
+
+
+KERNELS = [1, 0]   # thread-per-system, auto
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_cfg1_uniform_and_sine_modes(kernel):
+    w = WORKLOADS["cfg1"]
+    diags = make_matrix(w)
+    f = make_rhs(w)
+    x, h = gpu_solve(diags, f, kernel=kernel)
+    ref = oracle.solve_batch(oracle.factor(*diags), f)
+    assert normwise(x, ref) <= 1e-11
+    assert residual(diags, x, f) <= 1e-12
+    # closed form (north_star): system j-1 = sine mode j, x = f / lambda_j
+    modes = sine_modes(w.N)
+    xs, _ = gpu_solve(diags, modes, kernel=kernel)
+    j = np.arange(1, w.N + 1)
+    lam = 1.0 + 16.0 * w.sigma * np.sin(np.pi * j / (2 * (w.N + 1))) ** 4
+    assert normwise(xs, modes / lam[None, :]) <= 1e-11
+    # the device factorisation equals the oracle's (same recurrence, same rounding)
+    fac = oracle.factor(*diags)
+    for got, want in zip(h.factors(), (fac.eps, fac.beta, fac.alpha, fac.gamma, fac.delta)):
+        assert np.max(np.abs(got.numpy() - want)) <= 1e-15 * np.max(np.abs(want))
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_cfg2_manufactured_full(kernel):
+    w = WORKLOADS["cfg2"]
+    diags = make_matrix(w)
+    f, xtrue = make_rhs(w)
+    x, _ = gpu_solve(diags, f, kernel=kernel)
+    ref = oracle.solve_batch(oracle.factor(*diags), f, nthreads=8)
+    assert normwise(x, ref) <= 1e-11
+    assert normwise(x, xtrue) <= 1e-11
+    assert residual(diags, x, f) <= 1e-12
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_cfg3_full_size_every_system(dtype, kernel):
+    """Headline shape N=1024, M=65536, in the launch configuration bench.py times; EVERY system
+    is compared with the oracle (it takes about a second per pass on the host)."""
+    w = WORKLOADS["cfg3"]
+    diags = make_matrix(w)
+    f = make_rhs(w)
+    x, _ = gpu_solve(diags, f, dtype=dtype, kernel=kernel)
+    d64, f64, ref = oracle_for_dtype(diags, f, dtype)
+    tol_x, tol_r = TOL[dtype]
+    assert normwise(x.astype(np.float64), ref) <= tol_x
+    assert residual(d64, x, f64) <= tol_r
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_cfg5a_n4096_sampled_and_residual(kernel):
+    """N=4096, M=32768 (1 GiB per array): oracle parity on a window of 2048 systems computed
+    one by one, residual on the same window; the rest is covered by the M-independence of the
+    kernels (each system is solved alone)."""
+    w = WORKLOADS["cfg5a"]
+    pent = _pent()
+    diags = make_matrix(w)
+    f = make_rhs(w)
+    x, _ = gpu_solve(diags, f, kernel=kernel)
+    cols = np.r_[0:512, 16000:16512, w.M - 1024:w.M]
+    ref = oracle.solve_batch(oracle.factor(*diags), np.ascontiguousarray(f[:, cols]), nthreads=8)
+    assert normwise(x[:, cols], ref) <= 1e-11
+    assert residual(diags, np.ascontiguousarray(x[:, cols]), np.ascontiguousarray(f[:, cols])) <= 1e-12
+    assert np.isfinite(x).all()
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("N,M", [(1, 5), (2, 3), (3, 33), (5, 1), (31, 257), (33, 64), (64, 1),
+                                 (100, 130), (257, 1000), (1024, 37), (1000, 515)])
+def test_ragged_shapes_nonsymmetric(kernel, N, M):
+    diags = pin.random_diag_dominant(1000 + N, N)
+    f = pin.uniform_pm1(2000 + N, 0, N, M)
+    x, _ = gpu_solve(diags, f, kernel=kernel)
+    ref = oracle.solve_batch(oracle.factor(*diags), f)
+    assert normwise(x, ref) <= 1e-11
+    assert residual(diags, x, f) <= 1e-12
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_in_place_and_zero_batch(kernel):
+    pent = _pent()
+    N, M = 200, 300
+    diags = pin.diagonals_I_plus_sigma_L2(N, 2.0)
+    f = pin.uniform_pm1(5, 0, N, M)
+    x, h = gpu_solve(diags, f, kernel=kernel, inplace=True)
+    ref = oracle.solve_batch(oracle.factor(*diags), f)
+    assert normwise(x, ref) <= 1e-11
+    empty = torch.empty((N, 0), dtype=torch.float64, device="cuda")
+    assert pent.pent_solve_batch(h, 0, empty).shape == (N, 0)
+
+
+def test_out_of_matrix_entries_never_read():
+    """a[0],a[1],b[0],d[N-1],e[N-2],e[N-1] may hold garbage (NaN): include/pent.h."""
+    N, M = 50, 40
+    a, b, c, d, e = pin.random_diag_dominant(9, N)
+    f = pin.uniform_pm1(10, 0, N, M)
+    ref = oracle.solve_batch(oracle.factor(a, b, c, d, e), f)
+    a2, b2, d2, e2 = a.copy(), b.copy(), d.copy(), e.copy()
+    a2[:2] = np.nan; b2[0] = np.nan; d2[-1] = np.nan; e2[-2:] = np.nan
+    x, _ = gpu_solve((a2, b2, c, d2, e2), f)
+    assert normwise(x, ref) <= 1e-11
+
+
+def test_factor_from_device_pointers_and_fp32_factor_rounding():
+    pent = _pent()
+    N, M = 128, 64
+    diags = pin.diagonals_I_plus_sigma_L2(N, 10.0)
+    a, b, c, d, e = (torch.tensor(v, device="cuda") for v in diags)
+    h = pent.pent_factor(N, e, c, d, a, b)
+    f = pin.uniform_pm1(11, 0, N, M)
+    x = pent.pent_solve_batch(h, M, torch.tensor(f, device="cuda")).cpu().numpy()
+    assert normwise(x, oracle.solve_batch(oracle.factor(*diags), f)) <= 1e-11
+
+
+def test_errors():
+    pent = _pent()
+    N = 8
+    a, b, c, d, e = (torch.tensor(v) for v in pin.random_diag_dominant(3, N))
+    c0 = c.clone(); c0[0] = 0.0
+    with pytest.raises(pent.SingularPivot) as ei:
+        pent.pent_factor(N, e, c0, d, a, b)
+    assert ei.value.row == 0
+    # exact cancellation at row 1 (alpha_1 = c_1 - b_1 d_0 / c_0 = 1 - 2*2/4)
+    a4, b4, c4, d4, e4 = (torch.tensor(v, dtype=torch.float64) for v in
+                          ([0, 0, 1, 1], [0, 2, 1, 1], [4, 1, 5, 5], [2, 1, 1, 0], [1, 1, 0, 0]))
+    with pytest.raises(pent.SingularPivot) as ei:
+        pent.pent_factor(4, e4, c4, d4, a4, b4)
+    assert ei.value.row == 1
+    L = pent.lib()
+    assert L.pent_solve_batch(None, 4, None, None, None) == 1
+    h = pent.pent_factor(N, e, c, d, a, b)
+    assert L.pent_solve_batch(h.ptr, -1, None, None, None) == 1
+    assert L.pent_solve_batch(h.ptr, 4, None, None, None) == 1
+    assert L.pent_solve_batch_v(h.ptr, 0, None, None, None, 99) in (0, 1)
+    assert L.pent_solve_batch_multi(h.ptr, None, None, None) == 1     # wrong handle kind
+    import ctypes as C
+    out = C.c_void_p()
+    assert L.pent_factor(0, 1, 1, 1, 1, 1, 0, C.byref(out), None) == 1
+    assert L.pent_factor(4, 1, 1, 1, 1, 1, 7, C.byref(out), None) == 1
+
+
+def test_host_buffer_entry_point():
+    pent = _pent()
+    N, M = 96, 1500
+    diags = pin.diagonals_I_plus_sigma_L2(N, 1.0)
+    a, b, c, d, e = (torch.tensor(v) for v in diags)
+    h = pent.pent_factor(N, e, c, d, a, b)
+    f = pin.uniform_pm1(12, 0, N, M)
+    x = pent.pent_solve_batch_host(h, M, torch.tensor(f)).numpy()
+    assert normwise(x, oracle.solve_batch(oracle.factor(*diags), f)) <= 1e-11
+    xp = pent.pent_solve_batch_host(h, M, torch.tensor(f).pin_memory()).numpy()
+    assert np.array_equal(x, xp)

@@ -1,0 +1,167 @@
+"""GPU parity for the per-system-matrix variant (BASELINE.json configs[4]) and the
+fused time-step path (PAPER.md:53 Eq. 2, :87-89 Eq. 6; BASELINE.json configs[3])."""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import pent_inputs as pin
+from pent_inputs.configs import R_CH, SIGMA_CH, WORKLOADS, banded_matvec, make_matrix, make_rhs
+
+pytestmark = pytest.mark.gpu
+
+
+def _pent():
+    import paper_1807_07382_b200 as pent
+    return pent
+
+
+def normwise(x, ref):
+    return float(np.max(np.max(np.abs(x - ref), axis=0) / np.max(np.abs(ref), axis=0)))
+
+
+def residual(diags, x, f):
+    r = banded_matvec(*diags, x.astype(np.float64)) - f
+    return float(np.max(np.linalg.norm(r, axis=0) / np.linalg.norm(f, axis=0)))
+
+
+def _dev(v, dtype=torch.float64):
+    return torch.tensor(np.ascontiguousarray(v), dtype=dtype, device="cuda")
+
+
+# ---- per-system matrices ------------------------------------------------------------------
+@pytest.mark.parametrize("N,M", [(64, 100), (1024, 2048 + 37), (5, 3), (3, 70)])
+def test_factor_solve_batch_parity(N, M):
+    pent = _pent()
+    if N >= 4:
+        sig = pin.uniform_vec(6, 1, M, 0.1, 10.0)
+        diags = pin.diagonals_I_plus_sigma_L2(N, sig)
+    else:
+        diags = pin.random_diag_dominant(60 + N, N, M)
+    f = pin.uniform_pm1(6, 0, N, M)
+    a, b, c, d, e = (_dev(v) for v in diags)
+    x, info = pent.pent_factor_solve_batch(N, M, e, c, d, a, b, _dev(f))
+    torch.cuda.synchronize()
+    ref, rinfo = oracle.factor_solve_batch(*diags, f, nthreads=8)
+    assert not info.cpu().numpy().any() and not rinfo.any()
+    assert normwise(x.cpu().numpy(), ref) <= 1e-11
+    assert residual(diags, x.cpu().numpy(), f) <= 1e-12
+    # stored-factor route gives the same answers
+    h, info2 = pent.pent_factor_batch(N, M, e, c, d, a, b)
+    x2 = pent.pent_solve_batch_multi(h, _dev(f))
+    assert not info2.cpu().numpy().any()
+    assert normwise(x2.cpu().numpy(), ref) <= 1e-11
+
+
+def test_cfg5b_full_size():
+    pent = _pent()
+    w = WORKLOADS["cfg5b"]
+    diags = make_matrix(w)
+    f = make_rhs(w)
+    a, b, c, d, e = (_dev(v) for v in diags)
+    x, info = pent.pent_factor_solve_batch(w.N, w.M, e, c, d, a, b, _dev(f))
+    x = x.cpu().numpy()
+    assert not info.cpu().numpy().any()
+    ref, _ = oracle.factor_solve_batch(*diags, f, nthreads=8)
+    assert normwise(x, ref) <= 1e-11
+    assert residual(diags, x, f) <= 1e-12
+
+
+def test_per_system_fp32_and_singular_flag():
+    pent = _pent()
+    N, M = 256, 300
+    sig = pin.uniform_vec(6, 1, M, 0.1, 10.0)
+    diags = [np.asarray(v, dtype=np.float32) for v in pin.diagonals_I_plus_sigma_L2(N, sig)]
+    f = pin.uniform_pm1(6, 0, N, M).astype(np.float32)
+    a, b, c, d, e = (_dev(v, torch.float32) for v in diags)
+    x, info = pent.pent_factor_solve_batch(N, M, e, c, d, a, b, _dev(f, torch.float32))
+    d64 = [v.astype(np.float64) for v in diags]
+    ref, _ = oracle.factor_solve_batch(*d64, f.astype(np.float64))
+    assert normwise(x.cpu().numpy().astype(np.float64), ref) <= 2e-5
+    assert residual(d64, x.cpu().numpy(), f.astype(np.float64)) <= 1e-5
+    # one singular system: flagged with first bad row + 1, the others untouched
+    c2 = c.clone(); c2[0, 7] = 0.0
+    x2, info2 = pent.pent_factor_solve_batch(N, M, e, c2, d, a, b, _dev(f, torch.float32))
+    info2 = info2.cpu().numpy()
+    assert info2[7] == 1 and info2.sum() == 1
+    keep = np.arange(M) != 7
+    assert np.array_equal(x2.cpu().numpy()[:, keep], x.cpu().numpy()[:, keep])
+
+
+# ---- fused time step ------------------------------------------------------------------------
+def _ch_setup(N, M, bcname, seed=4):
+    sigma = 1e-2 * 1e-6 * N ** 4
+    r = 1e-6 * N ** 2
+    diags = pin.diagonals_I_plus_sigma_L2(N, sigma, bcname)
+    m = pin.uniform_vec(seed, 5, M, -0.5, 0.5)
+    c0 = m[None, :] + 0.05 * pin.uniform_pm1(seed, 0, N, M)
+    return diags, sigma, r, c0
+
+
+@pytest.mark.parametrize("bc,bcname", [(1, "zeroflux"), (0, "dirichlet")])
+@pytest.mark.parametrize("form", [1, 0])
+@pytest.mark.parametrize("N,M", [(1024, 300), (64, 33), (4, 5)])
+def test_ch_one_step_parity(bc, bcname, form, N, M):
+    pent = _pent()
+    diags, sigma, r, c0 = _ch_setup(N, M, bcname)
+    a, b, c, d, e = (torch.tensor(v) for v in diags)
+    h = pent.pent_factor(N, e, c, d, a, b)
+    cd = _dev(c0)
+    pent.pent_step_batch(h, M, cd, 1, kind=0, bc=bc, form=form, r=r, sigma=sigma)
+    ref = oracle.step_batch(oracle.factor(*diags), 0, bc, form, r, sigma, c0, 1)
+    assert normwise(cd.cpu().numpy(), ref) <= 1e-11
+
+
+def test_hyperdiffusion_step_parity_general_matrix():
+    pent = _pent()
+    N, M = 300, 129
+    diags = pin.random_diag_dominant(21, N)
+    a, b, c, d, e = (torch.tensor(v) for v in diags)
+    h = pent.pent_factor(N, e, c, d, a, b)
+    c0 = pin.uniform_pm1(22, 0, N, M)
+    cd = _dev(c0)
+    pent.pent_step_batch(h, M, cd, 3, kind=1)
+    ref = oracle.step_batch(oracle.factor(*diags), 1, 0, 0, 0.0, 0.0, c0, 3)
+    assert normwise(cd.cpu().numpy(), ref) <= 1e-11
+
+
+def test_cfg4_thousand_steps_conservation_and_trajectory():
+    """BASELINE.json configs[3]: N=1024, M=8192, 1000 fused steps, zero-flux L, increment form.
+    mean(c) per run conserved to 1e-12 (every system, fsum on the host); trajectory parity with
+    the oracle after 1000 nonlinear steps on a window of 64 systems to 1e-9."""
+    pent = _pent()
+    w = WORKLOADS["cfg4"]
+    diags = make_matrix(w)
+    c0 = make_rhs(w)
+    a, b, c, d, e = (torch.tensor(v) for v in diags)
+    h = pent.pent_factor(w.N, e, c, d, a, b)
+    cd = _dev(c0)
+    scratch = torch.empty_like(cd)
+    pent.pent_step_batch(h, w.M, cd, 1000, kind=0, bc=1, form=1, r=R_CH, sigma=SIGMA_CH,
+                         scratch=scratch)
+    c1 = cd.cpu().numpy()
+    assert np.isfinite(c1).all()
+    drift = max(abs(math.fsum(c1[:, i]) - math.fsum(c0[:, i])) / w.N for i in range(0, w.M, 7))
+    assert drift <= 1e-12
+    cols = np.r_[0:32, w.M - 32:w.M]
+    ref = oracle.step_batch(oracle.factor(*diags), 0, 1, 1, R_CH, SIGMA_CH,
+                            np.ascontiguousarray(c0[:, cols]), 1000, nthreads=8)
+    assert normwise(c1[:, cols], ref) <= 1e-9
+    assert np.max(np.abs(c1 - c0)) > 1e-3          # the state evolved
+
+
+def test_step_fp32_one_step():
+    pent = _pent()
+    N, M = 256, 200
+    diags, sigma, r, c0 = _ch_setup(N, M, "zeroflux")
+    d32 = [np.asarray(v, dtype=np.float32) for v in diags]
+    a, b, c, d, e = (torch.tensor(v) for v in d32)
+    h = pent.pent_factor(N, e, c, d, a, b)
+    cd = _dev(c0, torch.float32)
+    pent.pent_step_batch(h, M, cd, 1, kind=0, bc=1, form=0, r=r, sigma=sigma)
+    d64 = [v.astype(np.float64) for v in d32]
+    ref = oracle.step_batch(oracle.factor(*d64), 0, 1, 0, float(np.float32(r)),
+                            float(np.float32(sigma)), c0.astype(np.float32).astype(np.float64), 1)
+    assert normwise(cd.cpu().numpy().astype(np.float64), ref) <= 2e-5
