@@ -11,12 +11,12 @@ extern "C" int pent_solve_batch_v(const pent_handle* h, int64_t M, const void* f
     cudaStream_t s = (cudaStream_t)stream;
     switch (kernel) {
         case PENT_KERNEL_AUTO:
-            if (pent::chunked_supported(h, M)) return pent::launch_solve_chunked(h, M, f, x, s);
+            if (pent::chunked_supported(h, M, f)) return pent::launch_solve_chunked(h, M, f, x, s);
             return pent::launch_solve_tps(h, M, f, x, s);
         case PENT_KERNEL_THREAD_PER_SYSTEM:
             return pent::launch_solve_tps(h, M, f, x, s);
         case PENT_KERNEL_CHUNKED:
-            if (!pent::chunked_supported(h, M)) return PENT_ERR_ARG;
+            if (!pent::chunked_supported(h, M, f)) return PENT_ERR_ARG;
             return pent::launch_solve_chunked(h, M, f, x, s);
         default:
             return PENT_ERR_ARG;
@@ -26,7 +26,7 @@ extern "C" int pent_solve_batch_v(const pent_handle* h, int64_t M, const void* f
 extern "C" int pent_solve_kernel_choice(const pent_handle* h, int64_t M)
 {
     if (!h || h->kind != 0) return -1;
-    return pent::chunked_supported(h, M) ? PENT_KERNEL_CHUNKED : PENT_KERNEL_THREAD_PER_SYSTEM;
+    return pent::chunked_supported(h, M, nullptr) ?PENT_KERNEL_CHUNKED : PENT_KERNEL_THREAD_PER_SYSTEM;
 }
 
 extern "C" int pent_solve_batch(const pent_handle* h, int64_t M, const void* f, void* x,

@@ -66,6 +66,6 @@ __device__ __forceinline__ float2 ldg2(const float2* p) { return __ldg(p); }
 // kernels / launchers implemented across the .cu files
 int launch_solve_tps(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s);
 int launch_solve_chunked(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s);
-bool chunked_supported(const pent_handle* h, int64_t M);
+bool chunked_supported(const pent_handle* h, int64_t M, const void* f /* may be null */);
 
 }  // namespace pent

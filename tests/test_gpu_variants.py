@@ -111,7 +111,11 @@ def test_ch_one_step_parity(bc, bcname, form, N, M):
     cd = _dev(c0)
     pent.pent_step_batch(h, M, cd, 1, kind=0, bc=bc, form=form, r=r, sigma=sigma)
     ref = oracle.step_batch(oracle.factor(*diags), 0, bc, form, r, sigma, c0, 1)
-    assert normwise(cd.cpu().numpy(), ref) <= 1e-11
+    # Two correct fp64 evaluations of one step differ by ~cond(A)*eps (no-pivot LU forward
+    # error); cond(I + sigma L^2) <= 1 + 16 sigma.  At N=1024 sigma = 1.1e4, cond*eps = 2e-11:
+    # the oracle's own direct and increment forms differ by 1.6e-11 there (C-15).
+    tol = max(1e-11, 4.0 * (1.0 + 16.0 * sigma) * 2.0 ** -53)
+    assert normwise(cd.cpu().numpy(), ref) <= tol
 
 
 def test_hyperdiffusion_step_parity_general_matrix():
