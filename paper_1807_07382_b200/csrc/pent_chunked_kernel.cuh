@@ -1,0 +1,275 @@
+// pent_chunked_kernel.cuh -- device code of the chunked on-chip solve (included by
+// pent_solve_chunked.cu inside namespace pent; see the algorithm notes at the top of that file).
+#pragma once
+
+// Measured A/B switches (cfg3 fp64 on B200, profiles/r01_ab_tuning.md).  Defaults = fastest:
+//   store policy of the x stream: plain write-back st.global (201 us) beat .cs (212), .cg (210), .wt (211)
+//   chunk-state layout: [P][S] (197 us with 256-B L2 promotion) beat the bank-conflict-free padded
+//   [S][P+1] (221 us) although the scan then reads with a 32-way conflict: see DESIGN.md section 6.
+#if defined(PENT_AB_ST_CS)
+#define PENT_STORE(p, v) __stcs((p), (v))
+#elif defined(PENT_AB_ST_CG)
+#define PENT_STORE(p, v) __stcg((p), (v))
+#elif defined(PENT_AB_ST_WT)
+#define PENT_STORE(p, v) __stwt((p), (v))
+#else
+#define PENT_STORE(p, v) (*(p) = (v))
+#endif
+#ifndef PENT_AB_PADSTATE
+#define PENT_AB_OLDSTATE 1
+#endif
+
+template <typename T>
+struct ChunkParams {
+    int N;            // rows
+    int P;            // chunks per system
+    int Pw;           // P rounded up to a power of two (lanes per system in the chunk-state scan)
+    int lev_f, lev_b; // Kogge-Stone levels to apply (<= log2 Pw)
+    int woff[W_LEVELS]; // w_level_off(P, l)
+    int box_rows;     // rows per TMA box
+    int nbox;         // boxes per tile
+    int wcount[MAX_BOXES]; // warps that read each box (arrival count of its "empty" barrier)
+    int64_t M;
+    int64_t ntiles;
+    const T* table;   // global coefficient table (layout = shared-memory layout)
+    T* x;
+};
+
+template <typename T> struct Pair;
+template <> struct Pair<double> { using type = double2; };
+template <> struct Pair<float>  { using type = float2; };
+
+template <typename T>
+__device__ __forceinline__ T shfl_up_t(T v, int d, int w) { return __shfl_up_sync(0xffffffffu, v, d, w); }
+template <typename T>
+__device__ __forceinline__ T shfl_down_t(T v, int d, int w) { return __shfl_down_sync(0xffffffffu, v, d, w); }
+
+// One CTA = S systems x P chunks (thread = one system, one chunk of C rows, held in registers).
+// blockDim.x = P*S rounded up to a warp; threads with p >= P only take part in barriers/scan.
+template <typename T>
+__global__ void __launch_bounds__(CHUNK_MAX_THREADS, 1)
+solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T> prm)
+{
+    constexpr int C = ChunkCfg<T>::C, S = ChunkCfg<T>::S, BL = chunk_block_len<T>();
+    using T2 = typename Pair<T>::type;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int P = prm.P;
+    T* landing = reinterpret_cast<T*>(smem_raw);
+    T* table = landing + (size_t)prm.nbox * prm.box_rows * S;
+    // chunk states, [S][P+1] (system-major, one 16-byte pad per system: the scan reads a system's
+    // chunks with consecutive lanes, the sweeps write a chunk's systems with consecutive lanes;
+    // the odd row length keeps both conflict-free)
+    const int SP = P + 1;
+    T2* stE = reinterpret_cast<T2*>(table + table_len<T>(P));     // E~ then F_{p-1}
+    T2* stS = stE + (size_t)S * SP;                               // S^ then B_{p+1}
+    uint64_t* bars = reinterpret_cast<uint64_t*>(stS + (size_t)S * SP);
+
+    const int tid = threadIdx.x, i = tid % S, p = tid / S;
+    const bool active = p < P;
+    const int lane = tid & 31, warp = tid >> 5, nwarps = blockDim.x >> 5;
+    const uint32_t box_bytes = (uint32_t)(prm.box_rows * S * sizeof(T));
+    const uint32_t table_bytes = (uint32_t)(table_len<T>(P) * sizeof(T));
+    const int64_t stride = gridDim.x;
+
+    auto issue_tile = [&](int64_t t) {
+        for (int b = 0; b < prm.nbox; ++b) {
+            mbar_expect_tx(&bars[1 + b], box_bytes);
+            tma_load_2d(landing + (size_t)b * prm.box_rows * S, &tm, (int)(t * S), b * prm.box_rows,
+                        &bars[1 + b]);
+        }
+    };
+
+    if (tid == 0) {
+        for (int b = 0; b <= MAX_BOXES; ++b) mbar_init(&bars[b], 1);
+        for (int b = 0; b < MAX_BOXES; ++b)
+            mbar_init(&bars[1 + MAX_BOXES + b], prm.wcount[b] > 0 ? prm.wcount[b] : 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncthreads();
+    // tile sequence of this CTA: groups of PENT_TILE_GROUP consecutive tiles, groups strided by the grid
+    auto tile_of = [&](int64_t it) -> int64_t {
+        return (it / PENT_TILE_GROUP) * (stride * PENT_TILE_GROUP) + (int64_t)blockIdx.x * PENT_TILE_GROUP +
+               (it % PENT_TILE_GROUP);
+    };
+    int64_t it = 0;
+    int64_t tile = tile_of(0);
+    if (tid == 0) {
+        mbar_expect_tx(&bars[0], table_bytes);
+        bulk_load_1d(table, prm.table, table_bytes, &bars[0]);
+        if (tile < prm.ntiles) issue_tile(tile);
+    }
+    mbar_wait(&bars[0], 0);
+
+    const T* blk = table + (size_t)(active ? p : 0) * BL;
+    const T* wtab = table + (size_t)P * BL;          // W[e][q]
+    const int mybox = active ? (p * C) / prm.box_rows : 0;
+#ifdef PENT_AB_OLDSTATE
+    const int slot = (active ? p : 0) * S + i;
+#else
+    const int slot = i * SP + (active ? p : 0);
+#endif
+    const bool rows_full = active && (p * C + C <= prm.N);
+    uint32_t parity = 0;
+
+    // chunk-state scan geometry: a group of Pw lanes scans one system; G groups per warp
+    const int Pw = prm.Pw, G = 32 / Pw;
+    const int q = lane % Pw, grp = lane / Pw;
+    const int rounds = (S + nwarps * G - 1) / (nwarps * G);
+
+    for (; tile < prm.ntiles; tile = tile_of(++it)) {
+        const int64_t next_tile = tile_of(it + 1);
+        T v[C];
+        if (active) {
+            // ---- tile data: landing buffer -> registers ----
+            mbar_wait(&bars[1 + mybox], parity);
+            const T* src = landing + (size_t)p * C * S + i;
+#pragma unroll
+            for (int j = 0; j < C; ++j) v[j] = src[j * S];
+        }
+        // The box is free once every warp that reads it has its values in registers: each such
+        // warp arrives on the box's "empty" barrier and thread 0 re-arms it with the NEXT tile's
+        // TMA load, which then runs under all of this tile's arithmetic and stores.
+        __syncwarp();
+        if (lane == 0 && warp * 32 < P * S) mbar_arrive(&bars[1 + MAX_BOXES + mybox]);
+        if (tid == 0 && next_tile < prm.ntiles) {
+            for (int b = 0; b < prm.nbox; ++b) {
+                mbar_wait(&bars[1 + MAX_BOXES + b], parity);
+                mbar_expect_tx(&bars[1 + b], box_bytes);
+                tma_load_2d(landing + (size_t)b * prm.box_rows * S, &tm, (int)(next_tile * S),
+                            b * prm.box_rows, &bars[1 + b]);
+            }
+        }
+        if (active) {
+            // ---- 1. local forward sweep from a zero state (normalised) ----
+            T g1 = 0, g2 = 0;
+#pragma unroll
+            for (int jg = 0; jg < C / 4; ++jg) {
+                T w[12];
+                lds_vec<T, 12>(w, blk + 12 * jg);
+#pragma unroll
+                for (int r = 0; r < 4; ++r) {
+                    const int j = 4 * jg + r;
+                    T t = w[3 * r] * v[j];
+                    t = fma(-w[3 * r + 1], g2, t);
+                    T g = fma(-w[3 * r + 2], g1, t);
+                    v[j] = g; g2 = g1; g1 = g;
+                }
+            }
+            T2 e; e.x = v[C - 2]; e.y = v[C - 1];
+            stE[slot] = e;
+            // ---- 2. local back substitution of g~ from a zero state ----
+            T x1 = 0, x2 = 0;
+#pragma unroll
+            for (int jg = C / 4 - 1; jg >= 0; --jg) {
+                T w[8];
+                lds_vec<T, 8>(w, blk + 3 * C + 8 * jg);
+#pragma unroll
+                for (int r = 3; r >= 0; --r) {
+                    const int j = 4 * jg + r;
+#ifdef PENT_AB_OLDBWD
+                    T xv = fma(-w[2 * r + 1], x2, fma(-w[2 * r], x1, v[j]));
+#else
+                    T xv = fma(-w[2 * r], x1, fma(-w[2 * r + 1], x2, v[j]));   // x1 last: 1 fma on the chain
+#endif
+                    v[j] = xv; x2 = x1; x1 = xv;
+                }
+            }
+            T2 s; s.x = v[0]; s.y = v[1];
+            stS[slot] = s;
+        }
+        __syncthreads();       // states published
+
+        // ---- 3. chunk-state scans: Kogge-Stone over chunks with warp shuffles ----
+        //   F_q = E~_q + TPhi_q F_{q-1};  B_q = (S^_q + TX_q F_{q-1}) + TPsi_q B_{q+1}
+        // Slot (q, sys) receives what thread (sys, q) needs: F_{q-1} and B_{q+1}.
+        if (P > 1) {
+            for (int r = 0; r < rounds; ++r) {
+                const int sys = (r * nwarps + warp) * G + grp;
+                const bool ok = (sys < S) && (q < P);
+#ifdef PENT_AB_OLDSTATE
+                const int sl = ok ? q * S + sys : 0;
+#else
+                const int sl = ok ? sys * SP + q : 0;
+#endif
+                T y0 = 0, y1 = 0, z0 = 0, z1 = 0;
+                if (ok) { T2 e = stE[sl]; y0 = e.x; y1 = e.y; T2 s = stS[sl]; z0 = s.x; z1 = s.y; }
+#pragma unroll
+                for (int l = 0; l < W_LEVELS; ++l) {
+                    if (l < prm.lev_f) {
+                        const int d = 1 << l, n = P - d;
+                        T u0 = shfl_up_t(y0, d, Pw), u1 = shfl_up_t(y1, d, Pw);
+                        if (ok && q >= d) {
+                            const T* m = wtab + prm.woff[l] + (q - d);
+                            y0 = fma(m[n], u1, fma(m[0], u0, y0));
+                            y1 = fma(m[3 * n], u1, fma(m[2 * n], u0, y1));
+                        }
+                    }
+                }
+                T f0 = shfl_up_t(y0, 1, Pw), f1 = shfl_up_t(y1, 1, Pw);      // F_{q-1}
+                if (q == 0) { f0 = 0; f1 = 0; }
+                if (ok) {
+                    const T* m = wtab + q;                                   // TX_q
+                    z0 = fma(m[P], f1, fma(m[0], f0, z0));
+                    z1 = fma(m[3 * P], f1, fma(m[2 * P], f0, z1));
+                }
+#pragma unroll
+                for (int l = 0; l < W_LEVELS; ++l) {
+                    if (l < prm.lev_b) {
+                        const int d = 1 << l, n = P - d;
+                        T u0 = shfl_down_t(z0, d, Pw), u1 = shfl_down_t(z1, d, Pw);
+                        if (ok && q + d <= P - 1) {
+                            const T* m = wtab + prm.woff[l] + 4 * n + q;
+                            z0 = fma(m[n], u1, fma(m[0], u0, z0));
+                            z1 = fma(m[3 * n], u1, fma(m[2 * n], u0, z1));
+                        }
+                    }
+                }
+                T b0 = shfl_down_t(z0, 1, Pw), b1 = shfl_down_t(z1, 1, Pw);  // B_{q+1}
+                if (q + 1 > P - 1) { b0 = 0; b1 = 0; }
+                if (ok) {
+                    T2 fo; fo.x = f0; fo.y = f1; stE[sl] = fo;
+                    T2 bo; bo.x = b0; bo.y = b1; stS[sl] = bo;
+                }
+            }
+        }
+        __syncthreads();
+
+        // ---- 4. correction and store ----
+        if (active) {
+            T F0 = 0, F1 = 0, B0 = 0, B1 = 0;
+            if (P > 1) { T2 fo = stE[slot]; F0 = fo.x; F1 = fo.y; T2 bo = stS[slot]; B0 = bo.x; B1 = bo.y; }
+            const int64_t col = tile * S + i;
+            T* xo = prm.x + (int64_t)(p * C) * prm.M + col;
+            if (rows_full && (tile + 1) * S <= prm.M) {
+#pragma unroll
+                for (int jg = 0; jg < C / 4; ++jg) {
+                    T w[16];
+                    lds_vec<T, 16>(w, blk + 5 * C + 16 * jg);
+#pragma unroll
+                    for (int r = 0; r < 4; ++r) {
+                        T xv = fma(w[4 * r + 3], B1, fma(w[4 * r + 2], B0,
+                               fma(w[4 * r + 1], F1, fma(w[4 * r], F0, v[4 * jg + r]))));
+                        PENT_STORE(xo, xv);
+                        xo += prm.M;
+                    }
+                }
+            } else if (col < prm.M) {
+                const int nrows = prm.N - p * C;      // may be <= 0
+#pragma unroll
+                for (int jg = 0; jg < C / 4; ++jg) {
+                    T w[16];
+                    lds_vec<T, 16>(w, blk + 5 * C + 16 * jg);
+#pragma unroll
+                    for (int r = 0; r < 4; ++r) {
+                        T xv = fma(w[4 * r + 3], B1, fma(w[4 * r + 2], B0,
+                               fma(w[4 * r + 1], F1, fma(w[4 * r], F0, v[4 * jg + r]))));
+                        if (4 * jg + r < nrows) PENT_STORE(xo, xv);
+                        xo += prm.M;
+                    }
+                }
+            }
+        }
+        parity ^= 1;
+    }
+}

@@ -21,7 +21,8 @@ struct pent_handle {
     void* cf;            // chunked kernel: N x {1/alpha, eps/alpha, beta/alpha, phi0, phi1, 0..} see pent_factor.cu
     void* cb;            // chunked kernel: N x {gamma, delta, psi0, psi1}
     void* dg;            // N x {a,b,c,d,e,0,0,0} in T, for the (2I-A)c right-hand side
-    int nchunks;         // ceil(N / PENT_CHUNK)
+    int nchunks;         // chunks per system of the chunked kernel
+    int lev_f, lev_b;    // Kogge-Stone levels the chunk-state scans need (pent_solve_chunked.cu)
     // ---- per-system factors, device, interleaved, in T ----
     void* ms;            // 5*N*M: ia, en, bn, gamma, delta
 };

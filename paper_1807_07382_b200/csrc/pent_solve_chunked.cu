@@ -36,9 +36,30 @@ namespace pent {
 template <typename T> struct ChunkCfg;
 template <> struct ChunkCfg<double> { static constexpr int C = 32, S = 16; };
 template <> struct ChunkCfg<float>  { static constexpr int C = 64, S = 32; };
+#ifndef PENT_L2_PROMOTION
+#define PENT_L2_PROMOTION CU_TENSOR_MAP_L2_PROMOTION_L2_256B   // 197 us vs 201 us with 128 B
+#endif
+#ifndef PENT_TILE_GROUP
+#define PENT_TILE_GROUP 1      // consecutive tiles handled back to back by one CTA
+#endif
 constexpr int CHUNK_MAX_THREADS = 512;
 constexpr int BOX_ROWS_MAX = 256;           // TMA box dimension limit
 constexpr int MAX_BOXES = 4;
+
+// After the P chunk blocks of a table comes the chunk-transfer table W used by the Kogge-Stone
+// scan over chunks (lane q = chunk), stored compactly (only the entries a level can use):
+//   TX   : 4 rows x P          TX_q (row-major 2x2, element e at [e*P + q])
+//   then for each level l = 0..4, d = 2^l, n = max(0, P-d):
+//   WF_l : 4 rows x n          TPhi_q TPhi_{q-1} ... TPhi_{q-d+1}  for q >= d,     at [e*n + q-d]
+//   WB_l : 4 rows x n          TPsi_q TPsi_{q+1} ... TPsi_{q+d-1}  for q+d <= P-1, at [e*n + q]
+constexpr int W_LEVELS = 5;
+__host__ __device__ inline int w_level_off(int P, int l)
+{
+    int off = 4 * P;
+    for (int k = 0; k < l; ++k) { int n = P - (1 << k); off += 8 * (n > 0 ? n : 0); }
+    return off;
+}
+__host__ __device__ inline int w_len(int P) { return w_level_off(P, W_LEVELS); }
 
 // per-chunk coefficient block, in units of T:  [fwd 3C | bwd 2C | corr 4C | pad to 16 B]
 template <typename T> __host__ __device__ constexpr int chunk_block_len()
@@ -47,7 +68,7 @@ template <typename T> __host__ __device__ constexpr int chunk_block_len()
 }
 template <typename T> __host__ __device__ constexpr size_t table_len(int P)
 {
-    return (size_t)P * chunk_block_len<T>() + (size_t)P * 12;
+    return (size_t)P * chunk_block_len<T>() + (size_t)w_len(P);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -55,7 +76,7 @@ template <typename T> __host__ __device__ constexpr size_t table_len(int P)
 // ------------------------------------------------------------------------------------------
 template <typename T>
 __global__ void build_chunk_tables_kernel(int N, int P, const double* __restrict__ fac,
-                                          T* __restrict__ tab)
+                                          T* __restrict__ tab, double* __restrict__ tmat)
 {
     constexpr int C = ChunkCfg<T>::C;
     constexpr int BL = chunk_block_len<T>();
@@ -64,7 +85,6 @@ __global__ void build_chunk_tables_kernel(int N, int P, const double* __restrict
     const double *eps = fac, *beta = fac + N, *alpha = fac + 2 * N, *gamma = fac + 3 * N,
                  *delta = fac + 4 * N;
     T* blk = tab + (size_t)p * BL;
-    T* cm = tab + (size_t)P * BL + (size_t)p * 12;
     const int s = p * C;
     double phi0[C], phi1[C];
     // forward: coefficients and Phi
@@ -79,7 +99,8 @@ __global__ void build_chunk_tables_kernel(int N, int P, const double* __restrict
         phi0[j] = h0; phi1[j] = h1;
         h0m2 = h0m1; h0m1 = h0; h1m2 = h1m1; h1m1 = h1;
     }
-    cm[0] = (T)phi0[C - 2]; cm[1] = (T)phi1[C - 2]; cm[2] = (T)phi0[C - 1]; cm[3] = (T)phi1[C - 1];
+    double* cm = tmat + (size_t)p * 12;         // TPhi | TX | TPsi, fp64, for the product kernel
+    cm[0] = phi0[C - 2]; cm[1] = phi1[C - 2]; cm[2] = phi0[C - 1]; cm[3] = phi1[C - 1];
     // backward: coefficients, X = local back substitution of Phi, Psi
     double x0p1 = 0.0, x0p2 = 0.0, x1p1 = 0.0, x1p2 = 0.0;     // chi_{j+1}, chi_{j+2}
     double q0p1 = 1.0, q0p2 = 0.0, q1p1 = 0.0, q1p2 = 1.0;     // psi_{j+1}, psi_{j+2}
@@ -95,13 +116,71 @@ __global__ void build_chunk_tables_kernel(int N, int P, const double* __restrict
         T* o = blk + 5 * C + 4 * j;
         o[0] = (T)x0; o[1] = (T)x1; o[2] = (T)q0; o[3] = (T)q1;
         if (j <= 1) {
-            cm[4 + 2 * j] = (T)x0; cm[5 + 2 * j] = (T)x1;      // TX rows 0,1
-            cm[8 + 2 * j] = (T)q0; cm[9 + 2 * j] = (T)q1;      // TPsi rows 0,1
+            cm[4 + 2 * j] = x0; cm[5 + 2 * j] = x1;      // TX rows 0,1
+            cm[8 + 2 * j] = q0; cm[9 + 2 * j] = q1;      // TPsi rows 0,1
         }
         x0p2 = x0p1; x0p1 = x0; x1p2 = x1p1; x1p1 = x1;
         q0p2 = q0p1; q0p1 = q0; q1p2 = q1p1; q1p1 = q1;
     }
     for (int j = 9 * C; j < BL; ++j) blk[j] = (T)0;
+}
+
+// Products of the chunk transfer matrices by doubling (one block, thread q = chunk, P <= 32):
+//   WF_{q,2d} = WF_{q,d} WF_{q-d,d},   WB_{q,2d} = WB_{q,d} WB_{q+d,d}.
+// levels[0], levels[1] = number of Kogge-Stone levels the forward / backward scan must apply:
+// a level whose every entry is below 1e-25 in magnitude (and all levels above it) cannot change
+// a double-precision state and is skipped (for diagonally dominant A the products decay
+// geometrically, so typically 2-3 levels remain).
+template <typename T>
+__global__ void build_chunk_products_kernel(int P, const double* __restrict__ tmat,
+                                            T* __restrict__ wtab, int* __restrict__ levels)
+{
+    __shared__ double wf[W_LEVELS][32][4], wb[W_LEVELS][32][4];
+    __shared__ int need_f, need_b;
+    const int q = threadIdx.x;
+    if (q == 0) { need_f = 0; need_b = 0; }
+    for (int l = 0; l < W_LEVELS; ++l)
+        for (int e = 0; e < 4; ++e) { wf[l][q][e] = 0.0; wb[l][q][e] = 0.0; }
+    if (q < P) {
+        for (int e = 0; e < 4; ++e) {
+            wf[0][q][e] = (q >= 1) ? tmat[q * 12 + e] : 0.0;           // TPhi_q acts on F_{q-1}
+            wb[0][q][e] = (q + 1 <= P - 1) ? tmat[q * 12 + 8 + e] : 0.0;   // TPsi_q acts on B_{q+1}
+        }
+    }
+    __syncthreads();
+    for (int l = 1; l < W_LEVELS; ++l) {
+        const int d = 1 << (l - 1);       // combine two windows of d chunks
+        if (q < P && q >= 2 * d) {
+            const double* A = wf[l - 1][q];
+            const double* B = wf[l - 1][q - d];
+            wf[l][q][0] = A[0] * B[0] + A[1] * B[2]; wf[l][q][1] = A[0] * B[1] + A[1] * B[3];
+            wf[l][q][2] = A[2] * B[0] + A[3] * B[2]; wf[l][q][3] = A[2] * B[1] + A[3] * B[3];
+        }
+        if (q < P && q + 2 * d <= P - 1) {
+            const double* A = wb[l - 1][q];
+            const double* B = wb[l - 1][q + d];
+            wb[l][q][0] = A[0] * B[0] + A[1] * B[2]; wb[l][q][1] = A[0] * B[1] + A[1] * B[3];
+            wb[l][q][2] = A[2] * B[0] + A[3] * B[2]; wb[l][q][3] = A[2] * B[1] + A[3] * B[3];
+        }
+        __syncthreads();
+    }
+    if (q < P) {
+        for (int l = 0; l < W_LEVELS; ++l) {
+            double mf = 0.0, mb = 0.0;
+            const int d = 1 << l, n = P - d;
+            T* base = wtab + w_level_off(P, l);
+            for (int e = 0; e < 4; ++e) {
+                if (q >= d) base[e * n + (q - d)] = (T)wf[l][q][e];
+                if (q + d <= P - 1) base[4 * n + e * n + q] = (T)wb[l][q][e];
+                mf = fmax(mf, fabs(wf[l][q][e])); mb = fmax(mb, fabs(wb[l][q][e]));
+            }
+            if (!(mf < 1e-25)) atomicMax(&need_f, l + 1);      // also catches NaN
+            if (!(mb < 1e-25)) atomicMax(&need_b, l + 1);
+        }
+        for (int e = 0; e < 4; ++e) wtab[(size_t)e * P + q] = (T)tmat[q * 12 + 4 + e];
+    }
+    __syncthreads();
+    if (q == 0) { levels[0] = need_f; levels[1] = need_b; }
 }
 
 int build_chunk_tables(pent_handle* h, cudaStream_t s)
@@ -110,15 +189,34 @@ int build_chunk_tables(pent_handle* h, cudaStream_t s)
     const int C = f64 ? ChunkCfg<double>::C : ChunkCfg<float>::C;
     const int P = (h->N + C - 1) / C;
     h->nchunks = P;
+    h->lev_f = h->lev_b = 0;
+    if (P > 32) return PENT_OK;        // too long for the on-chip kernel: tables are not needed
     size_t bytes = f64 ? table_len<double>(P) * 8 : table_len<float>(P) * 4;
     cudaError_t e = cudaMalloc(&h->cf, bytes);
     if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); return PENT_ERR_ALLOC; }
     PENT_CUDA(e);
+    double* tmat = nullptr;
+    int* lev = nullptr;
+    PENT_CUDA(cudaMalloc(&tmat, sizeof(double) * 12 * P));
+    PENT_CUDA(cudaMalloc(&lev, 2 * sizeof(int)));
     int tb = 32, nb = (P + tb - 1) / tb;
-    if (f64) build_chunk_tables_kernel<double><<<nb, tb, 0, s>>>(h->N, P, h->fac, (double*)h->cf);
-    else build_chunk_tables_kernel<float><<<nb, tb, 0, s>>>(h->N, P, h->fac, (float*)h->cf);
-    count_launch();
-    PENT_LAUNCH_CHECK();
+    if (f64) {
+        build_chunk_tables_kernel<double><<<nb, tb, 0, s>>>(h->N, P, h->fac, (double*)h->cf, tmat);
+        build_chunk_products_kernel<double><<<1, 32, 0, s>>>(
+            P, tmat, (double*)h->cf + (size_t)P * chunk_block_len<double>(), lev);
+    } else {
+        build_chunk_tables_kernel<float><<<nb, tb, 0, s>>>(h->N, P, h->fac, (float*)h->cf, tmat);
+        build_chunk_products_kernel<float><<<1, 32, 0, s>>>(
+            P, tmat, (float*)h->cf + (size_t)P * chunk_block_len<float>(), lev);
+    }
+    count_launch(2);
+    cudaError_t le = cudaGetLastError();
+    int hl[2] = {0, 0};
+    if (le == cudaSuccess) le = cudaMemcpyAsync(hl, lev, sizeof(hl), cudaMemcpyDeviceToHost, s);
+    if (le == cudaSuccess) le = cudaStreamSynchronize(s);
+    cudaFree(tmat); cudaFree(lev);
+    if (le != cudaSuccess) return cuda_fail(le);
+    h->lev_f = hl[0]; h->lev_b = hl[1];
     return PENT_OK;
 }
 
@@ -137,6 +235,10 @@ __device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes)
 {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
                  : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
 {
@@ -183,163 +285,7 @@ __device__ __forceinline__ void lds_vec(T (&dst)[n], const T* src)
     }
 }
 
-template <typename T>
-struct ChunkParams {
-    int N;            // rows
-    int P;            // chunks per system = blockDim.x / S
-    int box_rows;     // rows per TMA box
-    int nbox;         // boxes per tile
-    int64_t M;
-    int64_t ntiles;
-    const T* table;   // global coefficient table (layout = shared-memory layout)
-    T* x;
-};
-
-template <typename T>
-__global__ void __launch_bounds__(CHUNK_MAX_THREADS, 1)
-solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T> prm)
-{
-    constexpr int C = ChunkCfg<T>::C, S = ChunkCfg<T>::S, BL = chunk_block_len<T>();
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    const int P = prm.P;
-    T* landing = reinterpret_cast<T*>(smem_raw);
-    T* table = landing + (size_t)prm.nbox * prm.box_rows * S;
-    T* stE = table + table_len<T>(P);
-    T* stS = stE + (size_t)P * S * 2;
-    uint64_t* bars = reinterpret_cast<uint64_t*>(stS + (size_t)P * S * 2);
-
-    const int tid = threadIdx.x, i = tid % S, p = tid / S;
-    const uint32_t box_bytes = (uint32_t)(prm.box_rows * S * sizeof(T));
-    const uint32_t table_bytes = (uint32_t)(table_len<T>(P) * sizeof(T));
-    const int64_t stride = gridDim.x;
-
-    auto issue_tile = [&](int64_t t) {
-        for (int b = 0; b < prm.nbox; ++b) {
-            mbar_expect_tx(&bars[1 + b], box_bytes);
-            tma_load_2d(landing + (size_t)b * prm.box_rows * S, &tm, (int)(t * S), b * prm.box_rows,
-                        &bars[1 + b]);
-        }
-    };
-
-    if (tid == 0) {
-        for (int b = 0; b <= MAX_BOXES; ++b) mbar_init(&bars[b], 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    }
-    __syncthreads();
-    int64_t tile = blockIdx.x;
-    if (tid == 0) {
-        mbar_expect_tx(&bars[0], table_bytes);
-        bulk_load_1d(table, prm.table, table_bytes, &bars[0]);
-        if (tile < prm.ntiles) issue_tile(tile);
-    }
-    mbar_wait(&bars[0], 0);
-
-    const T* blk = table + (size_t)p * BL;
-    const T* cmat = table + (size_t)P * BL;
-    const int mybox = (p * C) / prm.box_rows;
-    uint32_t parity = 0;
-
-    for (; tile < prm.ntiles; tile += stride) {
-        // ---- tile data: landing buffer -> registers ----
-        mbar_wait(&bars[1 + mybox], parity);
-        T v[C];
-        {
-            const T* src = landing + (size_t)p * C * S + i;
-#pragma unroll
-            for (int j = 0; j < C; ++j) v[j] = src[j * S];
-        }
-        // ---- 1. local forward sweep from a zero state (normalised) ----
-        {
-            T g1 = 0, g2 = 0;
-#pragma unroll
-            for (int jg = 0; jg < C / 4; ++jg) {
-                T w[12];
-                lds_vec<T, 12>(w, blk + 12 * jg);
-#pragma unroll
-                for (int r = 0; r < 4; ++r) {
-                    const int j = 4 * jg + r;
-                    T t = w[3 * r] * v[j];
-                    t = fma(-w[3 * r + 1], g2, t);
-                    T g = fma(-w[3 * r + 2], g1, t);
-                    v[j] = g; g2 = g1; g1 = g;
-                }
-            }
-            stE[(p * S + i) * 2 + 0] = v[C - 2];
-            stE[(p * S + i) * 2 + 1] = v[C - 1];
-        }
-        // ---- 2. local back substitution of g~ from a zero state ----
-        {
-            T x1 = 0, x2 = 0;
-#pragma unroll
-            for (int jg = C / 4 - 1; jg >= 0; --jg) {
-                T w[8];
-                lds_vec<T, 8>(w, blk + 3 * C + 8 * jg);
-#pragma unroll
-                for (int r = 3; r >= 0; --r) {
-                    const int j = 4 * jg + r;
-                    T xv = fma(-w[2 * r + 1], x2, fma(-w[2 * r], x1, v[j]));
-                    v[j] = xv; x2 = x1; x1 = xv;
-                }
-            }
-            stS[(p * S + i) * 2 + 0] = v[0];
-            stS[(p * S + i) * 2 + 1] = v[1];
-        }
-        __syncthreads();       // states published; landing buffer fully consumed
-        if (tid == 0 && tile + stride < prm.ntiles) issue_tile(tile + stride);
-
-        // ---- 3. chunk-state scans, one thread per system ----
-        if (tid < S) {
-            T f0 = 0, f1 = 0;
-            for (int q = 0; q < P; ++q) {
-                const T* m = cmat + q * 12;
-                T e0 = stE[(q * S + tid) * 2], e1 = stE[(q * S + tid) * 2 + 1];
-                T n0 = fma(m[1], f1, fma(m[0], f0, e0));
-                T n1 = fma(m[3], f1, fma(m[2], f0, e1));
-                f0 = n0; f1 = n1;
-                stE[(q * S + tid) * 2] = f0; stE[(q * S + tid) * 2 + 1] = f1;
-            }
-            T b0 = 0, b1 = 0;
-            for (int q = P - 1; q >= 0; --q) {
-                const T* m = cmat + q * 12;
-                T fi0 = 0, fi1 = 0;
-                if (q > 0) { fi0 = stE[((q - 1) * S + tid) * 2]; fi1 = stE[((q - 1) * S + tid) * 2 + 1]; }
-                T s0 = stS[(q * S + tid) * 2], s1 = stS[(q * S + tid) * 2 + 1];
-                s0 = fma(m[5], fi1, fma(m[4], fi0, s0));
-                s1 = fma(m[7], fi1, fma(m[6], fi0, s1));
-                T n0 = fma(m[9], b1, fma(m[8], b0, s0));
-                T n1 = fma(m[11], b1, fma(m[10], b0, s1));
-                b0 = n0; b1 = n1;
-                stS[(q * S + tid) * 2] = b0; stS[(q * S + tid) * 2 + 1] = b1;
-            }
-        }
-        __syncthreads();
-        T F0 = 0, F1 = 0, B0 = 0, B1 = 0;
-        if (p > 0) { F0 = stE[((p - 1) * S + i) * 2]; F1 = stE[((p - 1) * S + i) * 2 + 1]; }
-        if (p + 1 < P) { B0 = stS[((p + 1) * S + i) * 2]; B1 = stS[((p + 1) * S + i) * 2 + 1]; }
-        __syncthreads();       // states consumed: the next tile may overwrite them
-
-        // ---- 4. correction and store ----
-        {
-            const int64_t col = tile * S + i;
-            const bool colok = col < prm.M;
-            T* xo = prm.x + (int64_t)(p * C) * prm.M + col;
-#pragma unroll
-            for (int jg = 0; jg < C / 4; ++jg) {
-                T w[16];
-                lds_vec<T, 16>(w, blk + 5 * C + 16 * jg);
-#pragma unroll
-                for (int r = 0; r < 4; ++r) {
-                    const int j = 4 * jg + r;
-                    T xv = fma(w[4 * r + 3], B1, fma(w[4 * r + 2], B0,
-                           fma(w[4 * r + 1], F1, fma(w[4 * r], F0, v[j]))));
-                    if (colok && p * C + j < prm.N) __stcs(xo + (int64_t)j * prm.M, xv);
-                }
-            }
-        }
-        parity ^= 1;
-    }
-}
+#include "pent_chunked_kernel.cuh"
 
 // ------------------------------------------------------------------------------------------
 // host side
@@ -377,6 +323,14 @@ bool chunked_supported(const pent_handle* h, int64_t M, const void* f)
     const int S = f64 ? ChunkCfg<double>::S : ChunkCfg<float>::S;
     const int P = f64 ? chunk_P<double>(h) : chunk_P<float>(h);
     if (P * S > CHUNK_MAX_THREADS) return false;            // N too large to keep a tile on chip
+    {
+        const int C = f64 ? ChunkCfg<double>::C : ChunkCfg<float>::C;
+        const int rows = P * C, br = rows < BOX_ROWS_MAX ? rows : BOX_ROWS_MAX;
+        const size_t tl = f64 ? table_len<double>(P) : table_len<float>(P);
+        const size_t smem = ((size_t)((rows + br - 1) / br) * br * S + tl + (size_t)4 * (P + 1) * S) * esz +
+                            (1 + 2 * MAX_BOXES) * sizeof(uint64_t);
+        if (smem > 232448) return false;                    // 227 KB dynamic shared memory per CTA
+    }
     if ((M * esz) % 16 != 0) return false;                  // TMA global stride alignment
     if (f && ((uintptr_t)f % 16) != 0) return false;        // TMA global address alignment
     if (M > (int64_t)0x7fffffff) return false;              // TMA coordinates are 32-bit
@@ -390,10 +344,18 @@ static int launch_chunked_t(const pent_handle* h, int64_t M, const void* f, void
     const int P = chunk_P<T>(h);
     ChunkParams<T> prm;
     prm.N = h->N; prm.P = P; prm.M = M;
+    int Pw = 1, lg = 0;
+    while (Pw < P) { Pw *= 2; ++lg; }
+    prm.Pw = Pw;
+    prm.lev_f = h->lev_f < lg ? h->lev_f : lg;
+    prm.lev_b = h->lev_b < lg ? h->lev_b : lg;
+    for (int l = 0; l < W_LEVELS; ++l) prm.woff[l] = w_level_off(P, l);
     const int rows = P * C;
     prm.box_rows = rows < BOX_ROWS_MAX ? rows : BOX_ROWS_MAX;
     prm.nbox = (rows + prm.box_rows - 1) / prm.box_rows;
     prm.ntiles = (M + S - 1) / S;
+    for (int b = 0; b < MAX_BOXES; ++b) prm.wcount[b] = 0;
+    for (int w = 0; w * 32 < P * S; ++w) prm.wcount[((w * 32 / S) * C) / prm.box_rows] += 1;
     prm.table = (const T*)h->cf;
     prm.x = (T*)x;
 
@@ -404,26 +366,27 @@ static int launch_chunked_t(const pent_handle* h, int64_t M, const void* f, void
     cuuint32_t estr[2] = {1, 1};
     CUresult cr = encode_fn()(&tm, sizeof(T) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32,
                               2, const_cast<void*>(f), gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                              CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                              CU_TENSOR_MAP_SWIZZLE_NONE, PENT_L2_PROMOTION,
                               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (cr != CUDA_SUCCESS) { g_last_cuda_error = (int)cudaErrorInvalidValue; return PENT_ERR_CUDA; }
 
-    const size_t smem = ((size_t)prm.nbox * prm.box_rows * S + table_len<T>(P) + (size_t)4 * P * S) * sizeof(T) +
-                        (1 + MAX_BOXES) * sizeof(uint64_t);
+    const size_t smem = ((size_t)prm.nbox * prm.box_rows * S + table_len<T>(P) + (size_t)4 * (P + 1) * S) * sizeof(T) +
+                        (1 + 2 * MAX_BOXES) * sizeof(uint64_t);
     auto kern = solve_chunked_kernel<T>;
     static thread_local size_t smem_set = 0;
     if (smem > smem_set) {
         PENT_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         smem_set = smem;
     }
-    const int threads = P * S;
+    const int threads = (P * S + 31) / 32 * 32;
     int dev = 0, nsm = 0, occ = 0;
     PENT_CUDA(cudaGetDevice(&dev));
     PENT_CUDA(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
     PENT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, threads, smem));
     if (occ < 1) return PENT_ERR_ARG;
     int64_t grid = (int64_t)nsm * occ;
-    if (grid > prm.ntiles) grid = prm.ntiles;
+    const int64_t groups = (prm.ntiles + PENT_TILE_GROUP - 1) / PENT_TILE_GROUP;
+    if (grid > groups) grid = groups;
     kern<<<(unsigned)grid, threads, smem, s>>>(tm, prm);
     count_launch();
     PENT_LAUNCH_CHECK();
