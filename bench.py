@@ -211,9 +211,16 @@ def run_ours(args):
     esz = 8 if args.dtype == "f64" else 4
     N, M = w.N, w.M
     diags = make_matrix(w)
-    # weak scaling: rank r owns systems [r*M, (r+1)*M) of a batch of world*M systems
-    f = make_rhs(w, M=M, col0=rank * M) if w.rhs == "uniform" else make_rhs(w, M=M)
-    f = f[0] if isinstance(f, tuple) else f
+    # weak scaling: rank r owns systems [r*M, (r+1)*M) of ONE seeded batch of world*M systems
+    from paper_1807_07382_b200.sharding import max_over_ranks, shard_columns, whole_job_rate
+    import pent_inputs as pin
+    col0, m_own = shard_columns(world * M, rank, world)
+    assert m_own == M
+    if w.rhs == "uniform":
+        f = pin.uniform_pm1(w.seed, 0, N, M, col0, world * M)
+    else:
+        f = make_rhs(w, M=M)
+        f = f[0] if isinstance(f, tuple) else f
     a, b, c, d, e = (torch.tensor(v, dtype=tdt) for v in diags)
     h = pent.pent_factor(N, e, c, d, a, b)                 # once, outside the timed region
     f_host = torch.tensor(f, dtype=tdt).pin_memory()
@@ -242,11 +249,8 @@ def run_ours(args):
     launches = pent.launch_count()
     total_ms = evs[0].elapsed_time(evs[-1])
     per = np.array([evs[i].elapsed_time(evs[i + 1]) for i in range(args.steps)])
-    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms_max = float(t.item())
-    value = world * N * M * args.steps / (total_ms_max * 1e-3)
+    total_ms_max = max_over_ranks(total_ms, "cuda")
+    value = whole_job_rate(N * M * args.steps, world, total_ms_max * 1e-3)
 
     # end to end through the host-buffer entry point (H2D + solve + D2H inside the call)
     e2e = None
@@ -258,10 +262,8 @@ def run_ours(args):
         for _ in range(args.e2e_steps):
             pent.pent_solve_batch_host(h, M, f_host, x_host)
         dt = time.perf_counter() - t0
-        t = torch.tensor([dt], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e = {"value": world * N * M * args.e2e_steps / float(t.item()), "unit": UNIT,
+        e2e = {"value": whole_job_rate(N * M * args.e2e_steps, world, max_over_ranks(dt, "cuda")),
+               "unit": UNIT,
                "h2d_bytes_per_step": N * M * esz, "d2h_bytes_per_step": N * M * esz,
                "steps": args.e2e_steps, "api": "pent_solve_batch_host (pinned host buffers)"}
     if rank != 0:
