@@ -41,6 +41,8 @@ def parse_args():
     ap.add_argument("--workload", default="cfg3")
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
     ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 thread-per-system, 2 chunked")
+    ap.add_argument("--cluster", type=int, default=0, help="chunked kernel: CTAs per cluster along k (0 auto)")
+    ap.add_argument("--tile", type=int, default=0, help="chunked kernel: systems per tile (0 auto)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=3)
@@ -227,6 +229,8 @@ def run_ours(args):
     fd = f_host.cuda()
     xd = torch.empty_like(fd)
     stream = torch.cuda.current_stream()
+    if args.cluster or args.tile:
+        args.kernel = pent.KERNEL_CHUNKED_CFG(args.cluster, args.tile)
 
     def barrier():
         if world > 1:
@@ -271,8 +275,15 @@ def run_ours(args):
             dist.destroy_process_group()
         return
     peak, peak_src = measured_peak()
-    choice = args.kernel if args.kernel else pent.lib().pent_solve_kernel_choice(h.ptr, M)
-    kname = "solve_chunked_kernel" if choice == 2 else "solve_tps_kernel"
+    if args.kernel == 0:
+        ch = pent.kernel_choice(h, M)
+    elif (args.kernel & 0xff) == 2:
+        ch = {"kernel": "solve_chunked_kernel", "Q": (args.kernel >> 8) & 0xff, "S": (args.kernel >> 16) & 0xff}
+        if not (ch["Q"] and ch["S"]):
+            ch = {**pent.kernel_choice(h, M), **{k: v for k, v in ch.items() if v}}
+    else:
+        ch = {"kernel": "solve_tps_kernel", "Q": 0, "S": 0}
+    kname = ch["kernel"]
     alg_bytes = 2.0 * esz * N * M                # read f once, write x once
     avg_ms = float(per.mean())
     achieved = alg_bytes / (avg_ms * 1e-3) / 1e9
@@ -283,6 +294,7 @@ def run_ours(args):
         "data": "synthetic",
         "config": {"workload": w.name, "N": N, "M_per_gpu": M, "matrix": f"I+sigma*L^2 {w.bc} sigma={w.sigma}",
                    "rhs": w.rhs, "seed": w.seed, "layout": "interleaved f[k*M+i]", "kernel": kname,
+                   "cluster_ctas_along_k": ch["Q"], "systems_per_tile": ch["S"],
                    "l2": f"inputs+outputs {2 * esz * N * M >> 20} MiB per step exceed the 126 MB L2"},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak, "traffic": ncu_traffic(w.name, args.dtype, kname),

@@ -58,6 +58,10 @@ enum {
     PENT_KERNEL_CHUNKED = 2             /* k split into chunks across threads, g kept in registers,
                                            chunk coupling by the shared correction vectors (2 passes)  */
 };
+/* PENT_KERNEL_CHUNKED with an explicit shape (measurement): Q = CTAs of a thread-block cluster that
+ * split k between them (1, 2, 4, 8; 0 = choose), S = systems per tile (16, 32 for fp64; 32, 64 for
+ * fp32; 0 = choose).  PENT_ERR_ARG if that shape does not fit N / M / shared memory. */
+#define PENT_KERNEL_CHUNKED_CFG(Q, S) (2 | ((Q) << 8) | ((S) << 16))
 
 /* ---- shared A: factor once, solve many ("cuPentBatchConstant") -----------------
  * pent_factor: e,c,d,a,b: N elements each, host or device, element type per `dtype`.
@@ -128,7 +132,8 @@ int64_t pent_handle_m(const pent_handle* h);             /* M of a per-system ha
  * eps, beta, alpha = bands of L, gamma, delta = bands of R (Eq. 13).  Shared-A only. */
 int pent_handle_factors(const pent_handle* h, double* eps, double* beta, double* alpha,
                         double* gamma, double* delta);
-/* Which kernel PENT_KERNEL_AUTO picks for M systems on this handle (a PENT_KERNEL_* value). */
+/* Which kernel PENT_KERNEL_AUTO picks for M systems on this handle: PENT_KERNEL_THREAD_PER_SYSTEM,
+ * or PENT_KERNEL_CHUNKED_CFG(Q, S) with the chosen shape (low byte = PENT_KERNEL_CHUNKED). */
 int pent_solve_kernel_choice(const pent_handle* h, int64_t M);
 int pent_last_cuda_error(void);                         /* thread-local cudaError_t of the last PENT_ERR_CUDA */
 /* Number of kernel launches the library has enqueued from this thread since the last call with

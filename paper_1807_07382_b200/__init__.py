@@ -18,6 +18,19 @@ from . import build as _build
 
 PENT_F64, PENT_F32 = 0, 1
 KERNEL_AUTO, KERNEL_THREAD_PER_SYSTEM, KERNEL_CHUNKED = 0, 1, 2
+
+
+def KERNEL_CHUNKED_CFG(Q: int = 0, S: int = 0) -> int:
+    """PENT_KERNEL_CHUNKED_CFG of include/pent.h: explicit cluster size Q and tile width S."""
+    return 2 | (Q << 8) | (S << 16)
+
+
+def kernel_choice(h: "Handle", M: int) -> dict:
+    """What PENT_KERNEL_AUTO runs for M systems: {'kernel': name, 'Q': .., 'S': ..}."""
+    v = lib().pent_solve_kernel_choice(h.ptr, M)
+    if (v & 0xff) == KERNEL_CHUNKED:
+        return {"kernel": "solve_chunked_kernel", "Q": (v >> 8) & 0xff, "S": (v >> 16) & 0xff}
+    return {"kernel": "solve_tps_kernel", "Q": 0, "S": 0}
 _ERR = {1: "invalid argument", 2: "zero or non-finite pivot", 3: "CUDA error", 4: "allocation failure"}
 
 _lib = None

@@ -9,15 +9,19 @@ extern "C" int pent_solve_batch_v(const pent_handle* h, int64_t M, const void* f
     if (M == 0) return PENT_OK;
     if (!f || !x) return PENT_ERR_ARG;
     cudaStream_t s = (cudaStream_t)stream;
-    switch (kernel) {
+    if (kernel < 0 || (kernel >> 24) != 0) return PENT_ERR_ARG;
+    const int Q = (kernel >> 8) & 0xff, S = (kernel >> 16) & 0xff;
+    switch (kernel & 0xff) {
         case PENT_KERNEL_AUTO:
-            if (pent::chunked_supported(h, M, f)) return pent::launch_solve_chunked(h, M, f, x, s);
+            if (Q || S) return PENT_ERR_ARG;
+            if (pent::chunked_supported(h, M, f, 0, 0)) return pent::launch_solve_chunked(h, M, f, x, s, 0, 0);
             return pent::launch_solve_tps(h, M, f, x, s);
         case PENT_KERNEL_THREAD_PER_SYSTEM:
+            if (Q || S) return PENT_ERR_ARG;
             return pent::launch_solve_tps(h, M, f, x, s);
         case PENT_KERNEL_CHUNKED:
-            if (!pent::chunked_supported(h, M, f)) return PENT_ERR_ARG;
-            return pent::launch_solve_chunked(h, M, f, x, s);
+            if (!pent::chunked_supported(h, M, f, Q, S)) return PENT_ERR_ARG;
+            return pent::launch_solve_chunked(h, M, f, x, s, Q, S);
         default:
             return PENT_ERR_ARG;
     }
@@ -26,7 +30,9 @@ extern "C" int pent_solve_batch_v(const pent_handle* h, int64_t M, const void* f
 extern "C" int pent_solve_kernel_choice(const pent_handle* h, int64_t M)
 {
     if (!h || h->kind != 0) return -1;
-    return pent::chunked_supported(h, M, nullptr) ?PENT_KERNEL_CHUNKED : PENT_KERNEL_THREAD_PER_SYSTEM;
+    int Q = 0, S = 0;
+    if (!pent::chunked_choice(h, M, &Q, &S)) return PENT_KERNEL_THREAD_PER_SYSTEM;
+    return PENT_KERNEL_CHUNKED_CFG(Q, S);
 }
 
 extern "C" int pent_solve_batch(const pent_handle* h, int64_t M, const void* f, void* x,

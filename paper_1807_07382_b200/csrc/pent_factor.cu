@@ -96,7 +96,6 @@ static int factor_impl(int N, const void* const src[5], pent_dtype dtype, pent_h
     if (!h) return PENT_ERR_ALLOC;
     std::memset(h, 0, sizeof(*h));
     h->kind = 0; h->N = N; h->dtype = dtype;
-    h->nchunks = (N + PENT_CHUNK - 1) / PENT_CHUNK;
     T* stage = nullptr;
     int* status = nullptr;
     int rc = PENT_OK;
@@ -161,7 +160,8 @@ extern "C" void pent_destroy(pent_handle* h)
 {
     if (!h) return;
     cudaFree(h->diag); cudaFree(h->fac); cudaFree(h->fw); cudaFree(h->bw);
-    cudaFree(h->cf); cudaFree(h->cb); cudaFree(h->dg); cudaFree(h->ms);
+    for (int j = 0; j < PENT_NQ; ++j) cudaFree(h->cf[j]);
+    cudaFree(h->dg); cudaFree(h->ms);
     delete h;
 }
 

@@ -4,9 +4,8 @@
 #include <stdint.h>
 #include "pent.h"
 
-// Chunk length (rows per thread) of the chunked solve kernel; the correction vectors in the
-// handle are computed for this value.
-#define PENT_CHUNK 32
+// Cluster sizes (CTAs along k) the chunked kernel has tables for: Q = 1 << j, j < PENT_NQ.
+#define PENT_NQ 4
 
 struct pent_handle {
     int kind;            // 0 = shared A, 1 = per-system factors
@@ -18,11 +17,12 @@ struct pent_handle {
     double* fac;         // 5*N: eps,beta,alpha,gamma,delta (Eq. 13), fp64
     void* fw;            // N x {1/alpha, eps/alpha, beta/alpha, 0}   in T (T4)
     void* bw;            // N x {gamma, delta}                        in T (T2)
-    void* cf;            // chunked kernel: N x {1/alpha, eps/alpha, beta/alpha, phi0, phi1, 0..} see pent_factor.cu
-    void* cb;            // chunked kernel: N x {gamma, delta, psi0, psi1}
     void* dg;            // N x {a,b,c,d,e,0,0,0} in T, for the (2I-A)c right-hand side
-    int nchunks;         // chunks per system of the chunked kernel
-    int lev_f, lev_b;    // Kogge-Stone levels the chunk-state scans need (pent_solve_chunked.cu)
+    // chunked kernel (pent_solve_chunked.cu): for cluster size Q = 1 << j, Q per-rank coefficient
+    // tables in T, laid out as they sit in shared memory; cfP[j] = chunks per CTA (0: not built)
+    void* cf[PENT_NQ];
+    int cfP[PENT_NQ];
+    int lev_f[PENT_NQ], lev_b[PENT_NQ];   // Kogge-Stone levels the chunk-state scans need
     // ---- per-system factors, device, interleaved, in T ----
     void* ms;            // 5*N*M: ia, en, bn, gamma, delta
 };
@@ -66,7 +66,10 @@ __device__ __forceinline__ float2 ldg2(const float2* p) { return __ldg(p); }
 
 // kernels / launchers implemented across the .cu files
 int launch_solve_tps(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s);
-int launch_solve_chunked(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s);
-bool chunked_supported(const pent_handle* h, int64_t M, const void* f /* may be null */);
+// Q = CTAs per cluster along k, S = systems per tile; 0 = choose (pent_solve_chunked.cu)
+int launch_solve_chunked(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s,
+                         int Q, int S);
+bool chunked_supported(const pent_handle* h, int64_t M, const void* f /* may be null */, int Q, int S);
+int chunked_choice(const pent_handle* h, int64_t M, int* Q, int* S);   // 1 and the default plan, or 0
 
 }  // namespace pent

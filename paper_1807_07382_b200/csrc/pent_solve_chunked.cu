@@ -34,28 +34,32 @@
 namespace pent {
 
 template <typename T> struct ChunkCfg;
-template <> struct ChunkCfg<double> { static constexpr int C = 32, S = 16; };
-template <> struct ChunkCfg<float>  { static constexpr int C = 64, S = 32; };
+template <> struct ChunkCfg<double> { static constexpr int C = 32; };   // rows per thread
+template <> struct ChunkCfg<float>  { static constexpr int C = 64; };
 #ifndef PENT_L2_PROMOTION
 #define PENT_L2_PROMOTION CU_TENSOR_MAP_L2_PROMOTION_L2_256B   // 197 us vs 201 us with 128 B
-#endif
-#ifndef PENT_TILE_GROUP
-#define PENT_TILE_GROUP 1      // consecutive tiles handled back to back by one CTA
 #endif
 constexpr int CHUNK_MAX_THREADS = 512;
 constexpr int BOX_ROWS_MAX = 256;           // TMA box dimension limit
 constexpr int MAX_BOXES = 4;
+constexpr int MAX_PL = 32;                  // chunks per CTA (one warp scans a system's chunks)
+constexpr size_t SMEM_LIMIT = 232448;       // 227 KB dynamic shared memory per CTA
 
-// After the P chunk blocks of a table comes the chunk-transfer table W used by the Kogge-Stone
-// scan over chunks (lane q = chunk), stored compactly (only the entries a level can use):
-//   TX   : 4 rows x P          TX_q (row-major 2x2, element e at [e*P + q])
-//   then for each level l = 0..4, d = 2^l, n = max(0, P-d):
-//   WF_l : 4 rows x n          TPhi_q TPhi_{q-1} ... TPhi_{q-d+1}  for q >= d,     at [e*n + q-d]
-//   WB_l : 4 rows x n          TPsi_q TPsi_{q+1} ... TPsi_{q+d-1}  for q+d <= P-1, at [e*n + q]
+// After the P chunk blocks of a (per-rank) table comes the chunk-transfer table W (P = chunks of
+// this CTA, q = local chunk; every 2x2 matrix is row-major with element e at [e*len + index]):
+//   TX   : 4 x P     TX_q
+//   PF   : 4 x P     TPhi_q TPhi_{q-1} ... TPhi_{first chunk of the block}   (acts on the F entering the block)
+//   PB   : 4 x P     TPsi_q TPsi_{q+1} ... TPsi_{last chunk of the block}    (acts on the B entering the block)
+//   BLK  : 64        block products of every cluster rank r: TPhiBlock(r) at [4r..4r+3] (contiguous
+//                    2x2), TPsiBlock(r) at [32+4r..]
+//   then for each Kogge-Stone level l = 0..4, d = 2^l, n = max(0, P-d):
+//   WF_l : 4 x n     TPhi_q TPhi_{q-1} ... TPhi_{q-d+1}  for q >= d,     at [e*n + q-d]
+//   WB_l : 4 x n     TPsi_q TPsi_{q+1} ... TPsi_{q+d-1}  for q+d <= P-1, at [e*n + q]
+// Only the levels a handle needs are staged into shared memory (they come last).
 constexpr int W_LEVELS = 5;
 __host__ __device__ inline int w_level_off(int P, int l)
 {
-    int off = 4 * P;
+    int off = 12 * P + 64;
     for (int k = 0; k < l; ++k) { int n = P - (1 << k); off += 8 * (n > 0 ? n : 0); }
     return off;
 }
@@ -72,19 +76,22 @@ template <typename T> __host__ __device__ constexpr size_t table_len(int P)
 }
 
 // ------------------------------------------------------------------------------------------
-// table construction (once per handle): one thread per chunk, fp64 arithmetic, rounded to T
+// table construction (once per handle and cluster size): fp64 arithmetic, rounded to T
 // ------------------------------------------------------------------------------------------
+// One thread per GLOBAL chunk p = rank*Pl + local chunk; writes the chunk's coefficient block
+// into its rank's table and its three 2x2 end matrices (TPhi | TX | TPsi) into tmat.
 template <typename T>
-__global__ void build_chunk_tables_kernel(int N, int P, const double* __restrict__ fac,
-                                          T* __restrict__ tab, double* __restrict__ tmat)
+__global__ void build_chunk_tables_kernel(int N, int Pl, int Q, const double* __restrict__ fac,
+                                          T* __restrict__ tab, size_t tab_stride,
+                                          double* __restrict__ tmat)
 {
     constexpr int C = ChunkCfg<T>::C;
     constexpr int BL = chunk_block_len<T>();
     int p = blockIdx.x * blockDim.x + threadIdx.x;
-    if (p >= P) return;
+    if (p >= Pl * Q) return;
     const double *eps = fac, *beta = fac + N, *alpha = fac + 2 * N, *gamma = fac + 3 * N,
                  *delta = fac + 4 * N;
-    T* blk = tab + (size_t)p * BL;
+    T* blk = tab + (size_t)(p / Pl) * tab_stride + (size_t)(p % Pl) * BL;
     const int s = p * C;
     double phi0[C], phi1[C];
     // forward: coefficients and Phi
@@ -125,90 +132,113 @@ __global__ void build_chunk_tables_kernel(int N, int P, const double* __restrict
     for (int j = 9 * C; j < BL; ++j) blk[j] = (T)0;
 }
 
-// Products of the chunk transfer matrices by doubling (one block, thread q = chunk, P <= 32):
-//   WF_{q,2d} = WF_{q,d} WF_{q-d,d},   WB_{q,2d} = WB_{q,d} WB_{q+d,d}.
-// levels[0], levels[1] = number of Kogge-Stone levels the forward / backward scan must apply:
-// a level whose every entry is below 1e-25 in magnitude (and all levels above it) cannot change
-// a double-precision state and is skipped (for diagonally dominant A the products decay
-// geometrically, so typically 2-3 levels remain).
-template <typename T>
-__global__ void build_chunk_products_kernel(int P, const double* __restrict__ tmat,
-                                            T* __restrict__ wtab, int* __restrict__ levels)
+__device__ inline void mat2_mul(double* o, const double* A, const double* B)     // o = A B (row-major 2x2)
 {
-    __shared__ double wf[W_LEVELS][32][4], wb[W_LEVELS][32][4];
+    double r0 = A[0] * B[0] + A[1] * B[2], r1 = A[0] * B[1] + A[1] * B[3];
+    double r2 = A[2] * B[0] + A[3] * B[2], r3 = A[2] * B[1] + A[3] * B[3];
+    o[0] = r0; o[1] = r1; o[2] = r2; o[3] = r3;
+}
+
+// Products of the chunk transfer matrices.  One block per cluster rank (blockIdx.x), thread q =
+// local chunk (Pl <= 32).  Windows never cross the block: inside a CTA the scan starts from a zero
+// state and the state entering the block is applied afterwards through PF / PB.
+//   WF_{q,2d} = WF_{q,d} WF_{q-d,d},   WB_{q,2d} = WB_{q,d} WB_{q+d,d}   (doubling)
+// levels[0], levels[1] (atomicMax over ranks) = number of Kogge-Stone levels the forward /
+// backward scan must apply: a level whose every entry is below 1e-25 in magnitude (and all levels
+// above it) cannot change a double-precision state and is skipped (for diagonally dominant A the
+// products decay geometrically, so typically 2-3 levels remain).
+template <typename T>
+__global__ void build_chunk_products_kernel(int Pl, int Q, const double* __restrict__ tmat,
+                                            T* __restrict__ tab, size_t tab_stride,
+                                            int* __restrict__ levels)
+{
+    __shared__ double wf[W_LEVELS][MAX_PL][4], wb[W_LEVELS][MAX_PL][4];
+    __shared__ double pf[MAX_PL][4], pb[MAX_PL][4], blkm[64];
     __shared__ int need_f, need_b;
-    const int q = threadIdx.x;
+    const int q = threadIdx.x, rank = blockIdx.x;
+    const double* tm = tmat + (size_t)rank * Pl * 12;
+    T* wtab = tab + (size_t)rank * tab_stride + (size_t)Pl * chunk_block_len<T>();
     if (q == 0) { need_f = 0; need_b = 0; }
     for (int l = 0; l < W_LEVELS; ++l)
         for (int e = 0; e < 4; ++e) { wf[l][q][e] = 0.0; wb[l][q][e] = 0.0; }
-    if (q < P) {
+    if (q < Pl) {
         for (int e = 0; e < 4; ++e) {
-            wf[0][q][e] = (q >= 1) ? tmat[q * 12 + e] : 0.0;           // TPhi_q acts on F_{q-1}
-            wb[0][q][e] = (q + 1 <= P - 1) ? tmat[q * 12 + 8 + e] : 0.0;   // TPsi_q acts on B_{q+1}
+            wf[0][q][e] = (q >= 1) ? tm[q * 12 + e] : 0.0;                 // TPhi_q acts on F_{q-1}
+            wb[0][q][e] = (q + 1 <= Pl - 1) ? tm[q * 12 + 8 + e] : 0.0;    // TPsi_q acts on B_{q+1}
+        }
+    }
+    if (q == 0) {            // prefix products, serial
+        for (int e = 0; e < 4; ++e) pf[0][e] = tm[e];
+        for (int j = 1; j < Pl; ++j) mat2_mul(pf[j], tm + j * 12, pf[j - 1]);
+    }
+    if (q == 1) {
+        for (int e = 0; e < 4; ++e) pb[Pl - 1][e] = tm[(Pl - 1) * 12 + 8 + e];
+        for (int j = Pl - 2; j >= 0; --j) mat2_mul(pb[j], tm + j * 12 + 8, pb[j + 1]);
+    }
+    if (q == 2) {   // block products of every rank (each block computes all of them)
+        for (int r = 0; r < 8; ++r) {
+            double f[4] = {1.0, 0.0, 0.0, 1.0}, b[4] = {1.0, 0.0, 0.0, 1.0};
+            if (r < Q) {
+                const double* t = tmat + (size_t)r * Pl * 12;
+                for (int j = 0; j < Pl; ++j) mat2_mul(f, t + j * 12, f);            // TPhi_j ... TPhi_0
+                for (int j = Pl - 1; j >= 0; --j) mat2_mul(b, t + j * 12 + 8, b);   // TPsi_j ... TPsi_last
+            }
+            for (int e = 0; e < 4; ++e) { blkm[4 * r + e] = f[e]; blkm[32 + 4 * r + e] = b[e]; }
         }
     }
     __syncthreads();
     for (int l = 1; l < W_LEVELS; ++l) {
         const int d = 1 << (l - 1);       // combine two windows of d chunks
-        if (q < P && q >= 2 * d) {
-            const double* A = wf[l - 1][q];
-            const double* B = wf[l - 1][q - d];
-            wf[l][q][0] = A[0] * B[0] + A[1] * B[2]; wf[l][q][1] = A[0] * B[1] + A[1] * B[3];
-            wf[l][q][2] = A[2] * B[0] + A[3] * B[2]; wf[l][q][3] = A[2] * B[1] + A[3] * B[3];
-        }
-        if (q < P && q + 2 * d <= P - 1) {
-            const double* A = wb[l - 1][q];
-            const double* B = wb[l - 1][q + d];
-            wb[l][q][0] = A[0] * B[0] + A[1] * B[2]; wb[l][q][1] = A[0] * B[1] + A[1] * B[3];
-            wb[l][q][2] = A[2] * B[0] + A[3] * B[2]; wb[l][q][3] = A[2] * B[1] + A[3] * B[3];
-        }
+        if (q < Pl && q >= 2 * d) mat2_mul(wf[l][q], wf[l - 1][q], wf[l - 1][q - d]);
+        if (q < Pl && q + 2 * d <= Pl - 1) mat2_mul(wb[l][q], wb[l - 1][q], wb[l - 1][q + d]);
         __syncthreads();
     }
-    if (q < P) {
+    if (q < Pl) {
         for (int l = 0; l < W_LEVELS; ++l) {
             double mf = 0.0, mb = 0.0;
-            const int d = 1 << l, n = P - d;
-            T* base = wtab + w_level_off(P, l);
+            const int d = 1 << l, n = Pl - d;
+            T* base = wtab + w_level_off(Pl, l);
             for (int e = 0; e < 4; ++e) {
                 if (q >= d) base[e * n + (q - d)] = (T)wf[l][q][e];
-                if (q + d <= P - 1) base[4 * n + e * n + q] = (T)wb[l][q][e];
+                if (q + d <= Pl - 1) base[4 * n + e * n + q] = (T)wb[l][q][e];
                 mf = fmax(mf, fabs(wf[l][q][e])); mb = fmax(mb, fabs(wb[l][q][e]));
             }
             if (!(mf < 1e-25)) atomicMax(&need_f, l + 1);      // also catches NaN
             if (!(mb < 1e-25)) atomicMax(&need_b, l + 1);
         }
-        for (int e = 0; e < 4; ++e) wtab[(size_t)e * P + q] = (T)tmat[q * 12 + 4 + e];
+        for (int e = 0; e < 4; ++e) {
+            wtab[(size_t)e * Pl + q] = (T)tm[q * 12 + 4 + e];
+            wtab[(size_t)(4 + e) * Pl + q] = (T)pf[q][e];
+            wtab[(size_t)(8 + e) * Pl + q] = (T)pb[q][e];
+        }
     }
+    for (int j = q; j < 64; j += blockDim.x) wtab[12 * Pl + j] = (T)blkm[j];
     __syncthreads();
-    if (q == 0) { levels[0] = need_f; levels[1] = need_b; }
+    if (q == 0) { atomicMax(&levels[0], need_f); atomicMax(&levels[1], need_b); }
 }
 
-int build_chunk_tables(pent_handle* h, cudaStream_t s)
+template <typename T>
+static int build_tables_t(pent_handle* h, int j, cudaStream_t s)
 {
-    const bool f64 = h->dtype == PENT_F64;
-    const int C = f64 ? ChunkCfg<double>::C : ChunkCfg<float>::C;
+    constexpr int C = ChunkCfg<T>::C;
+    const int Q = 1 << j;
     const int P = (h->N + C - 1) / C;
-    h->nchunks = P;
-    h->lev_f = h->lev_b = 0;
-    if (P > 32) return PENT_OK;        // too long for the on-chip kernel: tables are not needed
-    size_t bytes = f64 ? table_len<double>(P) * 8 : table_len<float>(P) * 4;
-    cudaError_t e = cudaMalloc(&h->cf, bytes);
+    const int Pl = (P + Q - 1) / Q;
+    h->cf[j] = nullptr; h->cfP[j] = 0; h->lev_f[j] = h->lev_b[j] = 0;
+    if (Pl > MAX_PL || (Q > 1 && Q > P)) return PENT_OK;     // not a usable split: no tables
+    const size_t tlen = table_len<T>(Pl);
+    cudaError_t e = cudaMalloc(&h->cf[j], tlen * Q * sizeof(T));
     if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); return PENT_ERR_ALLOC; }
     PENT_CUDA(e);
     double* tmat = nullptr;
     int* lev = nullptr;
-    PENT_CUDA(cudaMalloc(&tmat, sizeof(double) * 12 * P));
+    PENT_CUDA(cudaMalloc(&tmat, sizeof(double) * 12 * Pl * Q));
     PENT_CUDA(cudaMalloc(&lev, 2 * sizeof(int)));
-    int tb = 32, nb = (P + tb - 1) / tb;
-    if (f64) {
-        build_chunk_tables_kernel<double><<<nb, tb, 0, s>>>(h->N, P, h->fac, (double*)h->cf, tmat);
-        build_chunk_products_kernel<double><<<1, 32, 0, s>>>(
-            P, tmat, (double*)h->cf + (size_t)P * chunk_block_len<double>(), lev);
-    } else {
-        build_chunk_tables_kernel<float><<<nb, tb, 0, s>>>(h->N, P, h->fac, (float*)h->cf, tmat);
-        build_chunk_products_kernel<float><<<1, 32, 0, s>>>(
-            P, tmat, (float*)h->cf + (size_t)P * chunk_block_len<float>(), lev);
-    }
+    PENT_CUDA(cudaMemsetAsync(lev, 0, 2 * sizeof(int), s));
+    PENT_CUDA(cudaMemsetAsync(h->cf[j], 0, tlen * Q * sizeof(T), s));
+    const int tb = 32, nb = (Pl * Q + tb - 1) / tb;
+    build_chunk_tables_kernel<T><<<nb, tb, 0, s>>>(h->N, Pl, Q, h->fac, (T*)h->cf[j], tlen, tmat);
+    build_chunk_products_kernel<T><<<Q, 32, 0, s>>>(Pl, Q, tmat, (T*)h->cf[j], tlen, lev);
     count_launch(2);
     cudaError_t le = cudaGetLastError();
     int hl[2] = {0, 0};
@@ -216,7 +246,16 @@ int build_chunk_tables(pent_handle* h, cudaStream_t s)
     if (le == cudaSuccess) le = cudaStreamSynchronize(s);
     cudaFree(tmat); cudaFree(lev);
     if (le != cudaSuccess) return cuda_fail(le);
-    h->lev_f = hl[0]; h->lev_b = hl[1];
+    h->cfP[j] = Pl; h->lev_f[j] = hl[0]; h->lev_b[j] = hl[1];
+    return PENT_OK;
+}
+
+int build_chunk_tables(pent_handle* h, cudaStream_t s)
+{
+    for (int j = 0; j < PENT_NQ; ++j) {
+        int rc = h->dtype == PENT_F64 ? build_tables_t<double>(h, j, s) : build_tables_t<float>(h, j, s);
+        if (rc != PENT_OK) return rc;
+    }
     return PENT_OK;
 }
 
@@ -310,53 +349,115 @@ static EncodeTiledFn encode_fn()
     return fn;
 }
 
-template <typename T> static int chunk_P(const pent_handle* h)
+// A launch plan: cluster size Q (CTAs along k), S systems per tile, Pl chunks per CTA.
+struct ChunkPlan {
+    bool ok = false;
+    int j = 0, Q = 1, S = 0, Pl = 0, Pw = 1, threads = 0, levels = 0, box_rows = 0, nbox = 0;
+    size_t table_bytes = 0, smem = 0;
+};
+
+static bool s_instantiated(bool f64, int S, bool cluster)
 {
-    return (h->N + ChunkCfg<T>::C - 1) / ChunkCfg<T>::C;
+    (void)cluster;
+    return f64 ? (S == 16 || S == 32) : (S == 32 || S == 64);
 }
 
-bool chunked_supported(const pent_handle* h, int64_t M, const void* f)
+static ChunkPlan make_plan(const pent_handle* h, int64_t M, const void* f, int Q, int S)
 {
-    if (!h || h->kind != 0 || !h->cf) return false;
+    ChunkPlan pl;
+    if (!h || h->kind != 0) return pl;
     const bool f64 = h->dtype == PENT_F64;
-    const int esz = f64 ? 8 : 4;
-    const int S = f64 ? ChunkCfg<double>::S : ChunkCfg<float>::S;
-    const int P = f64 ? chunk_P<double>(h) : chunk_P<float>(h);
-    if (P * S > CHUNK_MAX_THREADS) return false;            // N too large to keep a tile on chip
-    {
-        const int C = f64 ? ChunkCfg<double>::C : ChunkCfg<float>::C;
-        const int rows = P * C, br = rows < BOX_ROWS_MAX ? rows : BOX_ROWS_MAX;
-        const size_t tl = f64 ? table_len<double>(P) : table_len<float>(P);
-        const size_t smem = ((size_t)((rows + br - 1) / br) * br * S + tl + (size_t)4 * (P + 1) * S) * esz +
-                            (1 + 2 * MAX_BOXES) * sizeof(uint64_t);
-        if (smem > 232448) return false;                    // 227 KB dynamic shared memory per CTA
-    }
-    if ((M * esz) % 16 != 0) return false;                  // TMA global stride alignment
-    if (f && ((uintptr_t)f % 16) != 0) return false;        // TMA global address alignment
-    if (M > (int64_t)0x7fffffff) return false;              // TMA coordinates are 32-bit
-    return encode_fn() != nullptr;
+    const size_t esz = f64 ? 8 : 4;
+    int j = 0;
+    while ((1 << j) < Q) ++j;
+    if ((1 << j) != Q || j >= PENT_NQ || !h->cf[j] || h->cfP[j] < 1) return pl;
+    if (!s_instantiated(f64, S, Q > 1)) return pl;
+    const int C = f64 ? ChunkCfg<double>::C : ChunkCfg<float>::C;
+    pl.j = j; pl.Q = Q; pl.S = S; pl.Pl = h->cfP[j];
+    while (pl.Pw < pl.Pl) pl.Pw *= 2;
+    int lg = 0;
+    while ((1 << lg) < pl.Pw) ++lg;
+    pl.levels = h->lev_f[j] > h->lev_b[j] ? h->lev_f[j] : h->lev_b[j];
+    if (pl.levels > lg) pl.levels = lg;
+    // cluster: one scan round (the scan registers live across the cluster barriers)
+    pl.threads = Q > 1 ? pl.Pw * S : (pl.Pl * S + 31) / 32 * 32;
+    if (pl.threads > CHUNK_MAX_THREADS) return pl;
+    const int rows = pl.Pl * C;
+    pl.box_rows = rows < BOX_ROWS_MAX ? rows : BOX_ROWS_MAX;
+    pl.nbox = (rows + pl.box_rows - 1) / pl.box_rows;
+    if (pl.nbox > MAX_BOXES) return pl;
+    const size_t bl = f64 ? chunk_block_len<double>() : chunk_block_len<float>();
+    pl.table_bytes = ((size_t)pl.Pl * bl + (size_t)w_level_off(pl.Pl, pl.levels)) * esz;
+    pl.smem = (size_t)pl.nbox * pl.box_rows * S * esz + pl.table_bytes + (size_t)4 * pl.Pl * S * esz +
+              (Q > 1 ? (size_t)4 * Q * S * esz : 0) + (1 + 2 * MAX_BOXES) * sizeof(uint64_t);
+    if (pl.smem > SMEM_LIMIT) return pl;
+    if ((M * (int64_t)esz) % 16 != 0) return pl;            // TMA global stride alignment
+    if (f && ((uintptr_t)f % 16) != 0) return pl;           // TMA global address alignment
+    if (M > (int64_t)0x7fffffff) return pl;                 // TMA coordinates are 32-bit
+    if (!encode_fn()) return pl;
+    pl.ok = true;
+    return pl;
 }
 
-template <typename T>
-static int launch_chunked_t(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s)
+// Default plan: the smallest cluster that holds the system on chip, the widest tile it allows
+// (wider row segments per DRAM access); measured alternatives are in profiles/.
+static ChunkPlan auto_plan(const pent_handle* h, int64_t M, const void* f)
 {
-    constexpr int C = ChunkCfg<T>::C, S = ChunkCfg<T>::S;
-    const int P = chunk_P<T>(h);
+    if (!h || h->kind != 0) return ChunkPlan{};
+    const int cand[3] = {64, 32, 16};
+    for (int Q = 1; Q <= (1 << (PENT_NQ - 1)); Q *= 2)
+        for (int S : cand) {
+            ChunkPlan pl = make_plan(h, M, f, Q, S);
+            if (pl.ok) return pl;
+        }
+    return ChunkPlan{};
+}
+
+static ChunkPlan resolve_plan(const pent_handle* h, int64_t M, const void* f, int Q, int S)
+{
+    if (Q == 0 && S == 0) return auto_plan(h, M, f);
+    if (Q != 0 && S != 0) return make_plan(h, M, f, Q, S);
+    const int cand[3] = {64, 32, 16};
+    if (Q != 0) {
+        for (int s : cand) { ChunkPlan pl = make_plan(h, M, f, Q, s); if (pl.ok) return pl; }
+    } else {
+        for (int q = 1; q <= (1 << (PENT_NQ - 1)); q *= 2) { ChunkPlan pl = make_plan(h, M, f, q, S); if (pl.ok) return pl; }
+    }
+    return ChunkPlan{};
+}
+
+bool chunked_supported(const pent_handle* h, int64_t M, const void* f, int Q, int S)
+{
+    return resolve_plan(h, M, f, Q, S).ok;
+}
+
+int chunked_choice(const pent_handle* h, int64_t M, int* Q, int* S)
+{
+    ChunkPlan pl = auto_plan(h, M, nullptr);
+    if (!pl.ok) return 0;
+    *Q = pl.Q; *S = pl.S;
+    return 1;
+}
+
+template <typename T, int S, bool CLUSTER>
+static int launch_inst(const pent_handle* h, const ChunkPlan& pl, int64_t M, const void* f, void* x,
+                       cudaStream_t s)
+{
+    constexpr int C = ChunkCfg<T>::C;
     ChunkParams<T> prm;
-    prm.N = h->N; prm.P = P; prm.M = M;
-    int Pw = 1, lg = 0;
-    while (Pw < P) { Pw *= 2; ++lg; }
-    prm.Pw = Pw;
-    prm.lev_f = h->lev_f < lg ? h->lev_f : lg;
-    prm.lev_b = h->lev_b < lg ? h->lev_b : lg;
-    for (int l = 0; l < W_LEVELS; ++l) prm.woff[l] = w_level_off(P, l);
-    const int rows = P * C;
-    prm.box_rows = rows < BOX_ROWS_MAX ? rows : BOX_ROWS_MAX;
-    prm.nbox = (rows + prm.box_rows - 1) / prm.box_rows;
+    prm.N = h->N; prm.P = pl.Pl; prm.Q = pl.Q; prm.Pw = pl.Pw; prm.M = M;
+    int lg = 0;
+    while ((1 << lg) < pl.Pw) ++lg;
+    prm.lev_f = h->lev_f[pl.j] < lg ? h->lev_f[pl.j] : lg;
+    prm.lev_b = h->lev_b[pl.j] < lg ? h->lev_b[pl.j] : lg;
+    for (int l = 0; l < W_LEVELS; ++l) prm.woff[l] = w_level_off(pl.Pl, l);
+    prm.box_rows = pl.box_rows; prm.nbox = pl.nbox;
     prm.ntiles = (M + S - 1) / S;
     for (int b = 0; b < MAX_BOXES; ++b) prm.wcount[b] = 0;
-    for (int w = 0; w * 32 < P * S; ++w) prm.wcount[((w * 32 / S) * C) / prm.box_rows] += 1;
-    prm.table = (const T*)h->cf;
+    for (int w = 0; w * 32 < pl.Pl * S; ++w) prm.wcount[((w * 32 / S) * C) / prm.box_rows] += 1;
+    prm.table = (const T*)h->cf[pl.j];
+    prm.table_stride = (int64_t)table_len<T>(pl.Pl);
+    prm.table_bytes = (uint32_t)pl.table_bytes;
     prm.x = (T*)x;
 
     CUtensorMap tm;
@@ -370,32 +471,56 @@ static int launch_chunked_t(const pent_handle* h, int64_t M, const void* f, void
                               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (cr != CUDA_SUCCESS) { g_last_cuda_error = (int)cudaErrorInvalidValue; return PENT_ERR_CUDA; }
 
-    const size_t smem = ((size_t)prm.nbox * prm.box_rows * S + table_len<T>(P) + (size_t)4 * (P + 1) * S) * sizeof(T) +
-                        (1 + 2 * MAX_BOXES) * sizeof(uint64_t);
-    auto kern = solve_chunked_kernel<T>;
+    auto kern = solve_chunked_kernel<T, S, CLUSTER>;
     static thread_local size_t smem_set = 0;
-    if (smem > smem_set) {
-        PENT_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        smem_set = smem;
+    if (pl.smem > smem_set) {
+        PENT_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
+        smem_set = pl.smem;
     }
-    const int threads = (P * S + 31) / 32 * 32;
-    int dev = 0, nsm = 0, occ = 0;
+    int dev = 0, nsm = 0;
     PENT_CUDA(cudaGetDevice(&dev));
     PENT_CUDA(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
-    PENT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, threads, smem));
-    if (occ < 1) return PENT_ERR_ARG;
-    int64_t grid = (int64_t)nsm * occ;
-    const int64_t groups = (prm.ntiles + PENT_TILE_GROUP - 1) / PENT_TILE_GROUP;
-    if (grid > groups) grid = groups;
-    kern<<<(unsigned)grid, threads, smem, s>>>(tm, prm);
+    if constexpr (!CLUSTER) {
+        int occ = 0;
+        PENT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, pl.threads, pl.smem));
+        if (occ < 1) return PENT_ERR_ARG;
+        int64_t grid = (int64_t)nsm * occ;
+        if (grid > prm.ntiles) grid = prm.ntiles;
+        kern<<<(unsigned)grid, pl.threads, pl.smem, s>>>(tm, prm);
+    } else {
+        cudaLaunchConfig_t cfg = {};
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = (unsigned)pl.Q; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.blockDim = dim3((unsigned)pl.threads); cfg.dynamicSmemBytes = pl.smem; cfg.stream = s;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        cfg.gridDim = dim3((unsigned)(pl.Q * nsm));          // upper bound for the occupancy query
+        int ncl = 0;
+        PENT_CUDA(cudaOccupancyMaxActiveClusters(&ncl, kern, &cfg));
+        if (ncl < 1) return PENT_ERR_ARG;
+        int64_t clusters = ncl;
+        if (clusters > prm.ntiles) clusters = prm.ntiles;
+        cfg.gridDim = dim3((unsigned)(clusters * pl.Q));
+        PENT_CUDA(cudaLaunchKernelEx(&cfg, kern, tm, prm));
+    }
     count_launch();
     PENT_LAUNCH_CHECK();
     return PENT_OK;
 }
 
-int launch_solve_chunked(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s)
+int launch_solve_chunked(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s,
+                         int Q, int S)
 {
-    if (h->dtype == PENT_F64) return launch_chunked_t<double>(h, M, f, x, s);
-    return launch_chunked_t<float>(h, M, f, x, s);
+    const ChunkPlan pl = resolve_plan(h, M, f, Q, S);
+    if (!pl.ok) return PENT_ERR_ARG;
+    const bool cl = pl.Q > 1;
+    if (h->dtype == PENT_F64) {
+        if (pl.S == 16) return cl ? launch_inst<double, 16, true>(h, pl, M, f, x, s) : launch_inst<double, 16, false>(h, pl, M, f, x, s);
+        if (pl.S == 32) return cl ? launch_inst<double, 32, true>(h, pl, M, f, x, s) : launch_inst<double, 32, false>(h, pl, M, f, x, s);
+    } else {
+        if (pl.S == 32) return cl ? launch_inst<float, 32, true>(h, pl, M, f, x, s) : launch_inst<float, 32, false>(h, pl, M, f, x, s);
+        if (pl.S == 64) return cl ? launch_inst<float, 64, true>(h, pl, M, f, x, s) : launch_inst<float, 64, false>(h, pl, M, f, x, s);
+    }
+    return PENT_ERR_ARG;
 }
 }  // namespace pent

@@ -203,3 +203,56 @@ def test_host_buffer_entry_point():
     assert normwise(x, oracle.solve_batch(oracle.factor(*diags), f)) <= 1e-11
     xp = pent.pent_solve_batch_host(h, M, torch.tensor(f).pin_memory()).numpy()
     assert np.array_equal(x, xp)
+
+
+# ---- explicit shapes of the chunked kernel: cluster split along k, tile widths ---------------
+def _shape_case(N, M, Q, S, dtype=torch.float64, sigma=None, seed=70):
+    pent = _pent()
+    diags = pin.random_diag_dominant(seed + N, N) if sigma is None else pin.diagonals_I_plus_sigma_L2(N, sigma)
+    f = pin.uniform_pm1(seed + 1, 0, N, M)
+    x, _ = gpu_solve(diags, f, dtype=dtype, kernel=pent.KERNEL_CHUNKED_CFG(Q, S))
+    d64, f64, ref = oracle_for_dtype(diags, f, dtype)
+    tol_x, tol_r = TOL[dtype]
+    assert normwise(x.astype(np.float64), ref) <= tol_x
+    assert residual(d64, x, f64) <= tol_r
+
+
+@pytest.mark.parametrize("N,M,Q,S", [
+    (1024, 2048 + 32, 2, 32), (1024, 512, 4, 32), (1024, 512, 2, 16), (512, 1000, 1, 32), (512, 992, 2, 32),
+    (2048, 520, 2, 16), (2048, 512, 4, 32), (4096, 304, 4, 16), (4096, 512, 8, 32), (8192, 64, 8, 16),
+    (1000, 200, 2, 32), (3000, 100, 4, 16), (700, 96, 2, 16), (96, 40, 2, 16), (65, 34, 2, 32), (5000, 48, 8, 16),
+])
+def test_chunked_shapes_nonsymmetric_fp64(N, M, Q, S):
+    _shape_case(N, M, Q, S)
+
+
+@pytest.mark.parametrize("N,M,Q,S", [(1024, 2048 + 64, 2, 64), (1024, 1024, 1, 32), (512, 640, 1, 64),
+                                     (4096, 512, 4, 32), (4096, 256, 8, 64), (3000, 128, 2, 32)])
+def test_chunked_shapes_fp32(N, M, Q, S):
+    _shape_case(N, M, Q, S, dtype=torch.float32, sigma=10.0)
+
+
+@pytest.mark.parametrize("Q,S", [(2, 32), (4, 32), (2, 16)])
+def test_chunked_cluster_slowly_decaying_coupling(Q, S):
+    """sigma = 1.1e4 (the Cahn-Hilliard matrix of cfg4): the chunk transfer products decay over
+    ~20 chunks, so every Kogge-Stone level and the cross-CTA block products carry weight."""
+    pent = _pent()
+    N, M = 1024, 256
+    sigma = 1e-2 * 1e-6 * 1024.0 ** 4
+    diags = pin.diagonals_I_plus_sigma_L2(N, sigma, "zeroflux")
+    f = pin.uniform_pm1(81, 0, N, M)
+    x, _ = gpu_solve(diags, f, kernel=pent.KERNEL_CHUNKED_CFG(Q, S))
+    ref = oracle.solve_batch(oracle.factor(*diags), f)
+    # cond(A) ~ 1 + 16 sigma = 1.8e5: two correct fp64 solves differ by ~cond*eps (DESIGN.md C-15)
+    assert normwise(x, ref) <= 4.0 * (1.0 + 16.0 * sigma) * 2.0 ** -53
+    assert residual(diags, x, f) <= 1e-12
+
+
+def test_auto_choice_is_on_chip_for_every_config_shape():
+    pent = _pent()
+    for N, M in ((64, 256), (512, 16384), (1024, 65536), (4096, 32768), (2048, 1024), (8192, 512)):
+        diags = pin.diagonals_I_plus_sigma_L2(N, 1.0)
+        a, b, c, d, e = (torch.tensor(v) for v in diags)
+        h = pent.pent_factor(N, e, c, d, a, b)
+        ch = pent.kernel_choice(h, M)
+        assert ch["kernel"] == "solve_chunked_kernel", (N, M, ch)
