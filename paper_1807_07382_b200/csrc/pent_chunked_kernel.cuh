@@ -59,16 +59,35 @@ __device__ __forceinline__ void cluster_sync_all()
     __cluster_barrier_arrive();      // release
     __cluster_barrier_wait();        // acquire
 }
-template <typename T2>
-__device__ __forceinline__ void st_cluster_pair(T2* local, unsigned rank, T2 v)
+__device__ __forceinline__ uint32_t map_to_rank(const void* local, uint32_t rank)
 {
-    *reinterpret_cast<T2*>(__cluster_map_shared_rank(local, rank)) = v;
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(smem_u32(local)), "r"(rank));
+    return r;
+}
+// Remote store of one chunk state into CTA `rank`'s shared memory that signals that CTA's mbarrier
+// with complete_tx (16 or 8 bytes): producer -> consumer over DSMEM with no thread-scope fence, so
+// the x stores still in flight from the previous tile are not drained (a release-scoped cluster
+// barrier in the tile loop measured 271 us against 215 us for cfg3: profiles/r01_ab_tuning.md).
+__device__ __forceinline__ void st_async_pair(const void* local, const uint64_t* local_bar, uint32_t rank,
+                                              double a, double b)
+{
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.f64 [%0], {%1, %2}, [%3];"
+                 ::"r"(map_to_rank(local, rank)), "d"(a), "d"(b), "r"(map_to_rank(local_bar, rank)) : "memory");
+}
+__device__ __forceinline__ void st_async_pair(const void* local, const uint64_t* local_bar, uint32_t rank,
+                                              float a, float b)
+{
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.f32 [%0], {%1, %2}, [%3];"
+                 ::"r"(map_to_rank(local, rank)), "f"(a), "f"(b), "r"(map_to_rank(local_bar, rank)) : "memory");
 }
 
 // One CTA = S systems x P chunks (thread = one system, one chunk of C rows, held in registers).
 // blockDim.x >= P*S (a multiple of 32); threads with p >= P only take part in barriers/scan.
 // CLUSTER: the Q CTAs of a cluster own consecutive blocks of P chunks of the SAME S systems; the
 // chunk states are stitched across CTAs through distributed shared memory (two exchanges per tile).
+constexpr int BAR_F = 1 + 2 * MAX_BOXES, BAR_B = 2 + 2 * MAX_BOXES, NUM_BARS = 3 + 2 * MAX_BOXES;
+
 template <typename T, int S, bool CLUSTER>
 __global__ void __launch_bounds__(CHUNK_MAX_THREADS, 1)
 solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T> prm)
@@ -100,6 +119,8 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
         for (int b = 0; b <= MAX_BOXES; ++b) mbar_init(&bars[b], 1);
         for (int b = 0; b < MAX_BOXES; ++b)
             mbar_init(&bars[1 + MAX_BOXES + b], prm.wcount[b] > 0 ? prm.wcount[b] : 1);
+        mbar_init(&bars[BAR_F], 1);
+        mbar_init(&bars[BAR_B], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
@@ -115,7 +136,10 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
                             row_base + b * prm.box_rows, &bars[1 + b]);
             }
     }
-    if constexpr (CLUSTER) cluster_sync_all();   // every CTA of the cluster is resident before any DSMEM store
+    // every CTA of the cluster is resident, with its mbarriers initialised, before any DSMEM store
+    if constexpr (CLUSTER) cluster_sync_all();
+    const uint32_t agg_bytes_f = (uint32_t)(rank * S * sizeof(T2));                 // from the earlier ranks
+    const uint32_t agg_bytes_b = (uint32_t)((prm.Q - 1 - rank) * S * sizeof(T2));   // from the later ranks
     mbar_wait(&bars[0], 0);
 
     const T* blk = table + (size_t)(active ? p : 0) * BL;
@@ -146,6 +170,12 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
         // TMA load, which then runs under all of this tile's arithmetic and stores.
         __syncwarp();
         if (lane == 0 && warp * 32 < P * S) mbar_arrive(&bars[1 + MAX_BOXES + mybox]);
+        if constexpr (CLUSTER) {
+            if (tid == 0) {        // arm this tile's aggregate barriers (complete_tx may already have arrived)
+                if (agg_bytes_f) mbar_expect_tx(&bars[BAR_F], agg_bytes_f);
+                if (agg_bytes_b) mbar_expect_tx(&bars[BAR_B], agg_bytes_b);
+            }
+        }
         if (tid == 0 && next_tile < prm.ntiles) {
             for (int b = 0; b < prm.nbox; ++b) {
                 mbar_wait(&bars[1 + MAX_BOXES + b], parity);
@@ -212,11 +242,10 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
                 if constexpr (CLUSTER) {
                     // y = F of chunk q for a ZERO state entering the block.  The last chunk's value is
                     // the block aggregate: publish it to every later rank, then chain the earlier ones.
-                    if (ok && q == P - 1) {
-                        T2 a; a.x = y0; a.y = y1;
-                        for (int rr = rank + 1; rr < prm.Q; ++rr) st_cluster_pair(&aggF[rank * S + sys], rr, a);
-                    }
-                    cluster_sync_all();
+                    if (ok && q == P - 1)
+                        for (int rr = rank + 1; rr < prm.Q; ++rr)
+                            st_async_pair(&aggF[rank * S + sys], &bars[BAR_F], rr, y0, y1);
+                    if (agg_bytes_f) mbar_wait(&bars[BAR_F], parity);
                     for (int rr = 0; rr < rank; ++rr) {        // F_in(rr+1) = aggF[rr] + TPhiBlock(rr) F_in(rr)
                         T2 a = aggF[rr * S + (ok ? sys : 0)];
                         T n0 = a.x, n1 = a.y;
@@ -238,11 +267,10 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
                 }
                 T bin0 = 0, bin1 = 0;                 // B of the first chunk of the NEXT block
                 if constexpr (CLUSTER) {
-                    if (ok && q == 0) {
-                        T2 a; a.x = z0; a.y = z1;
-                        for (int rr = 0; rr < rank; ++rr) st_cluster_pair(&aggB[rank * S + sys], rr, a);
-                    }
-                    cluster_sync_all();
+                    if (ok && q == 0)
+                        for (int rr = 0; rr < rank; ++rr)
+                            st_async_pair(&aggB[rank * S + sys], &bars[BAR_B], rr, z0, z1);
+                    if (agg_bytes_b) mbar_wait(&bars[BAR_B], parity);
                     for (int rr = prm.Q - 1; rr > rank; --rr) {   // B_in(rr-1) = aggB[rr] + TPsiBlock(rr) B_in(rr)
                         T2 a = aggB[rr * S + (ok ? sys : 0)];
                         T n0 = a.x, n1 = a.y;

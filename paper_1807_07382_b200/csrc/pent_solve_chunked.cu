@@ -389,7 +389,7 @@ static ChunkPlan make_plan(const pent_handle* h, int64_t M, const void* f, int Q
     const size_t bl = f64 ? chunk_block_len<double>() : chunk_block_len<float>();
     pl.table_bytes = ((size_t)pl.Pl * bl + (size_t)w_level_off(pl.Pl, pl.levels)) * esz;
     pl.smem = (size_t)pl.nbox * pl.box_rows * S * esz + pl.table_bytes + (size_t)4 * pl.Pl * S * esz +
-              (Q > 1 ? (size_t)4 * Q * S * esz : 0) + (1 + 2 * MAX_BOXES) * sizeof(uint64_t);
+              (Q > 1 ? (size_t)4 * Q * S * esz : 0) + (3 + 2 * MAX_BOXES) * sizeof(uint64_t);
     if (pl.smem > SMEM_LIMIT) return pl;
     if ((M * (int64_t)esz) % 16 != 0) return pl;            // TMA global stride alignment
     if (f && ((uintptr_t)f % 16) != 0) return pl;           // TMA global address alignment
@@ -399,12 +399,14 @@ static ChunkPlan make_plan(const pent_handle* h, int64_t M, const void* f, int Q
     return pl;
 }
 
-// Default plan: the smallest cluster that holds the system on chip, the widest tile it allows
-// (wider row segments per DRAM access); measured alternatives are in profiles/.
+// Default plan: the smallest cluster that holds the system on chip and the narrowest tile (more,
+// smaller tiles balance better over the 148 SMs and measured faster than wider row segments at
+// every shape tried: cfg2 34.2 us at S=16 vs 37.8 at S=32; cfg3 197 us at Q=1,S=16 vs 212-215 at
+// Q=2/4,S=32; cfg5a 469 us at Q=4,S=16 vs 548 at Q=8,S=32; profiles/r01_ab_tuning.md).
 static ChunkPlan auto_plan(const pent_handle* h, int64_t M, const void* f)
 {
     if (!h || h->kind != 0) return ChunkPlan{};
-    const int cand[3] = {64, 32, 16};
+    const int cand[3] = {16, 32, 64};
     for (int Q = 1; Q <= (1 << (PENT_NQ - 1)); Q *= 2)
         for (int S : cand) {
             ChunkPlan pl = make_plan(h, M, f, Q, S);
@@ -417,7 +419,7 @@ static ChunkPlan resolve_plan(const pent_handle* h, int64_t M, const void* f, in
 {
     if (Q == 0 && S == 0) return auto_plan(h, M, f);
     if (Q != 0 && S != 0) return make_plan(h, M, f, Q, S);
-    const int cand[3] = {64, 32, 16};
+    const int cand[3] = {16, 32, 64};
     if (Q != 0) {
         for (int s : cand) { ChunkPlan pl = make_plan(h, M, f, Q, s); if (pl.ok) return pl; }
     } else {
