@@ -101,8 +101,11 @@ int pent_factor_batch(int N, int64_t M, const void* e, const void* c, const void
 int pent_solve_batch_multi(const pent_handle* h, const void* f, void* x, void* stream);
 
 /* ---- fused time stepping on a shared-A handle (BASELINE.json configs[3]) ----------------------
- * One step = explicit right-hand side built from the state + one solve, fused in one kernel;
- * `nsteps` steps are enqueued back to back on `stream`.
+ * One step = explicit right-hand side built from the state + one solve, fused in one kernel.
+ * Default (N*S*sizeof(T) <= 128 KiB per tile of S systems, i.e. N <= 1024, and M*sizeof(T) a
+ * multiple of 16): ONE launch takes every tile of systems through all `nsteps` steps with the
+ * state held in shared memory (HBM traffic: read c once, write c once, whatever nsteps is).
+ * Otherwise one launch per step (thread per system, g through `scratch`).
  *  kind 0, Cahn-Hilliard (Eq. 2), L = second-difference matrix with boundary `bc`:
  *     form 0 (direct):     A c+ = c + r L (c^3 - c)
  *     form 1 (increment):  q = r (c^3 - c) - sigma L c;   A delta = L q;   c+ = c + delta
@@ -123,6 +126,12 @@ typedef struct {
 
 int pent_step_batch(const pent_handle* h, const pent_step_params* p, int64_t M,
                     void* c_inout, void* scratch, int nsteps, void* stream);
+/* Same with an explicit kernel (measurement / tests): PENT_KERNEL_AUTO, PENT_KERNEL_THREAD_PER_SYSTEM
+ * or PENT_KERNEL_CHUNKED (= the on-chip kernel; PENT_ERR_ARG when the shape does not fit). */
+int pent_step_batch_v(const pent_handle* h, const pent_step_params* p, int64_t M,
+                      void* c_inout, void* scratch, int nsteps, void* stream, int kernel);
+/* Which kernel pent_step_batch runs for M systems: PENT_KERNEL_CHUNKED or PENT_KERNEL_THREAD_PER_SYSTEM. */
+int pent_step_kernel_choice(const pent_handle* h, int64_t M);
 
 /* ---- introspection ------------------------------------------------------------------------ */
 int pent_handle_n(const pent_handle* h);                 /* N, or -1 */

@@ -73,6 +73,8 @@ def lib() -> C.CDLL:
     L.pent_factor_batch.argtypes = [ci, i64, vp, vp, vp, vp, vp, ci, C.POINTER(vp), vp, vp]
     L.pent_solve_batch_multi.argtypes = [vp, vp, vp, vp]
     L.pent_step_batch.argtypes = [vp, C.POINTER(pent_step_params), i64, vp, vp, ci, vp]
+    L.pent_step_batch_v.argtypes = [vp, C.POINTER(pent_step_params), i64, vp, vp, ci, vp, ci]
+    L.pent_step_kernel_choice.argtypes = [vp, i64]
     L.pent_handle_n.argtypes = [vp]
     L.pent_handle_dtype.argtypes = [vp]
     L.pent_handle_m.argtypes = [vp]
@@ -217,14 +219,15 @@ def pent_solve_batch_multi(h: Handle, f: torch.Tensor, x: torch.Tensor | None = 
 
 def pent_step_batch(h: Handle, M: int, c: torch.Tensor, nsteps: int, *, kind: int = 0, bc: int = 1,
                     form: int = 1, r: float = 0.0, sigma: float = 0.0,
-                    scratch: torch.Tensor | None = None, stream=None) -> torch.Tensor:
-    """nsteps fused steps (RHS + solve per kernel) in place on c (N, M).  See include/pent.h."""
+                    scratch: torch.Tensor | None = None, stream=None,
+                    kernel: int = KERNEL_AUTO) -> torch.Tensor:
+    """nsteps fused steps (RHS + solve in one kernel) in place on c (N, M).  See include/pent.h."""
     _batch(c, "c")
     if c.shape != (h.N, M) or c.dtype != h.dtype:
         raise ValueError("c must be (N, M) of the handle's dtype")
     p = pent_step_params(kind, bc, form, r, sigma)
     sp = 0 if scratch is None else scratch.data_ptr()
-    _check(lib().pent_step_batch(h.ptr, C.byref(p), M, c.data_ptr(), sp, nsteps, _stream(stream)))
+    _check(lib().pent_step_batch_v(h.ptr, C.byref(p), M, c.data_ptr(), sp, nsteps, _stream(stream), kernel))
     return c
 
 

@@ -1,0 +1,316 @@
+// pent_chunk_common.cuh -- shared by the chunked solve kernel (pent_solve_chunked.cu) and the
+// on-chip fused time-step kernel (pent_step_chunked.cu): table layout, PTX helpers (mbarrier, TMA,
+// DSMEM), and the three arithmetic stages of the chunked algorithm (local sweeps, chunk-state
+// scan, correction).  See the algorithm notes at the top of pent_solve_chunked.cu.
+#pragma once
+#include <cuda.h>
+#include "pent_internal.h"
+
+namespace pent {
+
+template <typename T> struct ChunkCfg;
+template <> struct ChunkCfg<double> { static constexpr int C = 32; };   // rows per thread
+template <> struct ChunkCfg<float>  { static constexpr int C = 64; };
+#ifndef PENT_L2_PROMOTION
+#define PENT_L2_PROMOTION CU_TENSOR_MAP_L2_PROMOTION_L2_256B   // 197 us vs 201 us with 128 B
+#endif
+constexpr int CHUNK_MAX_THREADS = 512;
+constexpr int BOX_ROWS_MAX = 256;           // TMA box dimension limit
+constexpr int MAX_BOXES = 4;
+constexpr int MAX_PL = 32;                  // chunks per CTA (one warp scans a system's chunks)
+constexpr size_t SMEM_LIMIT = 232448;       // 227 KB dynamic shared memory per CTA
+
+// After the P chunk blocks of a (per-rank) table comes the chunk-transfer table W (P = chunks of
+// this CTA, q = local chunk; every 2x2 matrix is row-major with element e at [e*len + index]):
+//   TX   : 4 x P     TX_q
+//   (the next three only in the tables of a cluster, Q > 1)
+//   PF   : 4 x P     TPhi_q TPhi_{q-1} ... TPhi_{first chunk of the block}   (acts on the F entering the block)
+//   PB   : 4 x P     TPsi_q TPsi_{q+1} ... TPsi_{last chunk of the block}    (acts on the B entering the block)
+//   BLK  : 64        block products of every cluster rank r: TPhiBlock(r) at [4r..4r+3] (contiguous
+//                    2x2), TPsiBlock(r) at [32+4r..]
+//   then for each Kogge-Stone level l = 0..4, d = 2^l, n = max(0, P-d):
+//   WF_l : 4 x n     TPhi_q TPhi_{q-1} ... TPhi_{q-d+1}  for q >= d,     at [e*n + q-d]
+//   WB_l : 4 x n     TPsi_q TPsi_{q+1} ... TPsi_{q+d-1}  for q+d <= P-1, at [e*n + q]
+// Only the levels a handle needs are staged into shared memory (they come last).
+constexpr int W_LEVELS = 5;
+__host__ __device__ inline int w_level_off(int P, int l, int Q)
+{
+    int off = Q > 1 ? 12 * P + 64 : 4 * P;      // PF, PB, BLK exist only in cluster tables
+    for (int k = 0; k < l; ++k) { int n = P - (1 << k); off += 8 * (n > 0 ? n : 0); }
+    return off;
+}
+__host__ __device__ inline int w_len(int P, int Q) { return w_level_off(P, W_LEVELS, Q); }
+
+// per-chunk coefficient block, in units of T:  [fwd 3C | bwd 2C | corr 4C | pad to 16 B]
+template <typename T> __host__ __device__ constexpr int chunk_block_len()
+{
+    return 9 * ChunkCfg<T>::C + (int)(16 / sizeof(T));
+}
+template <typename T> __host__ __device__ constexpr size_t table_len(int P, int Q)
+{
+    return (size_t)P * chunk_block_len<T>() + (size_t)w_len(P, Q);
+}
+
+// ------------------------------------------------------------------------------------------
+// PTX helpers: mbarrier, TMA (sm_90+ async proxy; SASS: UTMALDG / UBLKCP / SYNCS)
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p)
+{
+    return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
+{
+    uint32_t addr = smem_u32(bar), ok;
+    do {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(ok) : "r"(addr), "r"(parity) : "memory");
+    } while (!ok);
+}
+__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* tm, int c0, int c1, uint64_t* bar)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes "
+        "[%0], [%1, {%2, %3}], [%4];"
+        ::"r"(smem_u32(dst)), "l"((uint64_t)tm), "r"(c0), "r"(c1), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void bulk_load_1d(void* dst, const void* src, uint32_t bytes, uint64_t* bar)
+{
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+        ::"r"(smem_u32(dst)), "l"((uint64_t)src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+// n consecutive T values from shared memory with 16-byte loads (n*sizeof(T) % 16 == 0)
+template <typename T, int n>
+__device__ __forceinline__ void lds_vec(T (&dst)[n], const T* src)
+{
+    constexpr int V = 16 / sizeof(T);
+    static_assert(n % V == 0, "vector load granularity");
+    const uint4* s4 = reinterpret_cast<const uint4*>(src);
+#pragma unroll
+    for (int v = 0; v < n / V; ++v) {
+        uint4 q = s4[v];
+        if constexpr (sizeof(T) == 8) {
+            dst[2 * v + 0] = __hiloint2double((int)q.y, (int)q.x);
+            dst[2 * v + 1] = __hiloint2double((int)q.w, (int)q.z);
+        } else {
+            dst[4 * v + 0] = __uint_as_float(q.x); dst[4 * v + 1] = __uint_as_float(q.y);
+            dst[4 * v + 2] = __uint_as_float(q.z); dst[4 * v + 3] = __uint_as_float(q.w);
+        }
+    }
+}
+
+template <typename T> struct Pair;
+template <> struct Pair<double> { using type = double2; };
+template <> struct Pair<float>  { using type = float2; };
+
+template <typename T>
+__device__ __forceinline__ T shfl_up_t(T v, int d, int w) { return __shfl_up_sync(0xffffffffu, v, d, w); }
+template <typename T>
+__device__ __forceinline__ T shfl_down_t(T v, int d, int w) { return __shfl_down_sync(0xffffffffu, v, d, w); }
+
+// y += m * u for a row-major 2x2 m stored with element stride `n` (m[e*n])
+template <typename T>
+__device__ __forceinline__ void mat2_acc(T& y0, T& y1, const T* m, int n, T u0, T u1)
+{
+    y0 = fma(m[n], u1, fma(m[0], u0, y0));
+    y1 = fma(m[3 * n], u1, fma(m[2 * n], u0, y1));
+}
+
+// ---- thread-block-cluster helpers (CUDA 12 sm_90+ intrinsics; SASS: UCGABAR_ARV / UCGABAR_WAIT,
+// remote stores through the distributed-shared-memory window)
+__device__ __forceinline__ void cluster_sync_all()
+{
+    __cluster_barrier_arrive();      // release
+    __cluster_barrier_wait();        // acquire
+}
+__device__ __forceinline__ uint32_t map_to_rank(const void* local, uint32_t rank)
+{
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(smem_u32(local)), "r"(rank));
+    return r;
+}
+// Remote store of one chunk state into CTA `rank`'s shared memory that signals that CTA's mbarrier
+// with complete_tx (16 or 8 bytes): producer -> consumer over DSMEM with no thread-scope fence, so
+// the x stores still in flight from the previous tile are not drained (a release-scoped cluster
+// barrier in the tile loop measured 271 us against 215 us for cfg3: profiles/r01_ab_tuning.md).
+__device__ __forceinline__ void st_async_pair(const void* local, const uint64_t* local_bar, uint32_t rank,
+                                              double a, double b)
+{
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.f64 [%0], {%1, %2}, [%3];"
+                 ::"r"(map_to_rank(local, rank)), "d"(a), "d"(b), "r"(map_to_rank(local_bar, rank)) : "memory");
+}
+__device__ __forceinline__ void st_async_pair(const void* local, const uint64_t* local_bar, uint32_t rank,
+                                              float a, float b)
+{
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.f32 [%0], {%1, %2}, [%3];"
+                 ::"r"(map_to_rank(local, rank)), "f"(a), "f"(b), "r"(map_to_rank(local_bar, rank)) : "memory");
+}
+
+// One CTA = S systems x P chunks (thread = one system, one chunk of C rows, held in registers).
+// blockDim.x >= P*S (a multiple of 32); threads with p >= P only take part in barriers/scan.
+// CLUSTER: the Q CTAs of a cluster own consecutive blocks of P chunks of the SAME S systems; the
+// chunk states are stitched across CTAs through distributed shared memory (two exchanges per tile).
+
+// ------------------------------------------------------------------------------------------
+// stage 1+2: local forward sweep (normalised coefficients) and local back
+// substitution of one chunk held in registers, both from a zero state.
+// blk = the chunk's coefficient block in shared memory.  v: f -> x^ ; e = last two g~ ; s = first two x^.
+// ------------------------------------------------------------------------------------------
+template <typename T>
+__device__ __forceinline__ void chunk_local_sweeps(T (&v)[ChunkCfg<T>::C], const T* blk,
+                                                   typename Pair<T>::type& e, typename Pair<T>::type& s)
+{
+    constexpr int C = ChunkCfg<T>::C;
+    T g1 = 0, g2 = 0;
+#pragma unroll
+    for (int jg = 0; jg < C / 4; ++jg) {
+        T w[12];
+        lds_vec<T, 12>(w, blk + 12 * jg);
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const int j = 4 * jg + r;
+            T t = w[3 * r] * v[j];
+            t = fma(-w[3 * r + 1], g2, t);
+            T g = fma(-w[3 * r + 2], g1, t);
+            v[j] = g; g2 = g1; g1 = g;
+        }
+    }
+    e.x = v[C - 2]; e.y = v[C - 1];
+    T x1 = 0, x2 = 0;
+#pragma unroll
+    for (int jg = C / 4 - 1; jg >= 0; --jg) {
+        T w[8];
+        lds_vec<T, 8>(w, blk + 3 * C + 8 * jg);
+#pragma unroll
+        for (int r = 3; r >= 0; --r) {
+            const int j = 4 * jg + r;
+            T xv = fma(-w[2 * r], x1, fma(-w[2 * r + 1], x2, v[j]));   // x1 last: 1 fma on the chain
+            v[j] = xv; x2 = x1; x1 = xv;
+        }
+    }
+    s.x = v[0]; s.y = v[1];
+}
+
+// stage 4, one group of 4 rows: x = x^ + chi0 F0 + chi1 F1 + psi0 B0 + psi1 B1
+template <typename T>
+__device__ __forceinline__ void chunk_correct4(T (&out)[4], const T* v4, const T* blk, int jg, T F0, T F1, T B0, T B1)
+{
+    constexpr int C = ChunkCfg<T>::C;
+    T w[16];
+    lds_vec<T, 16>(w, blk + 5 * C + 16 * jg);
+#pragma unroll
+    for (int r = 0; r < 4; ++r)
+        out[r] = fma(w[4 * r + 3], B1, fma(w[4 * r + 2], B0, fma(w[4 * r + 1], F1, fma(w[4 * r], F0, v4[r]))));
+}
+
+// Geometry of the chunk-state scan (stage 3): a group of Pw lanes scans one system, lane = chunk.
+struct ScanGeom {
+    int P, Pw, lev_f, lev_b;
+    const int* woff;      // w_level_off(P, l), l < W_LEVELS
+};
+
+constexpr int BAR_F = 1 + 2 * MAX_BOXES, BAR_B = 2 + 2 * MAX_BOXES, NUM_BARS = 3 + 2 * MAX_BOXES;
+
+// stage 3 for one (system, chunk q) lane: Kogge-Stone over chunks with warp shuffles.
+//   F_q = E~_q + TPhi_q F_{q-1};  B_q = (S^_q + TX_q F_{q-1}) + TPsi_q B_{q+1}
+// In:  stE[sl] = E~_q, stS[sl] = S^_q.  Out: stE[sl] = F_{q-1}, stS[sl] = B_{q+1} (what thread (sys, q)
+// needs).  CLUSTER: the block aggregates travel between the CTAs of the cluster (rank = this
+// CTA's position along k, Q CTAs) through aggF/aggB and the two aggregate mbarriers.
+template <typename T, int S, bool CLUSTER>
+__device__ __forceinline__ void chunk_state_scan(const ScanGeom& g, const T* wtab, typename Pair<T>::type* stE,
+                                                 typename Pair<T>::type* stS, int sys, int q, bool ok,
+                                                 int rank, int Q, typename Pair<T>::type* aggF,
+                                                 typename Pair<T>::type* aggB, uint64_t* bars,
+                                                 uint32_t agg_bytes_f, uint32_t agg_bytes_b, uint32_t parity)
+{
+    using T2 = typename Pair<T>::type;
+    const int P = g.P, Pw = g.Pw;
+    const int sl = ok ? q * S + sys : 0;
+    T y0 = 0, y1 = 0, z0 = 0, z1 = 0;
+    if (ok) { T2 e = stE[sl]; y0 = e.x; y1 = e.y; T2 s = stS[sl]; z0 = s.x; z1 = s.y; }
+#pragma unroll
+    for (int l = 0; l < W_LEVELS; ++l) {
+        if (l < g.lev_f) {
+            const int d = 1 << l, n = P - d;
+            T u0 = shfl_up_t(y0, d, Pw), u1 = shfl_up_t(y1, d, Pw);
+            if (ok && q >= d) mat2_acc(y0, y1, wtab + g.woff[l] + (q - d), n, u0, u1);
+        }
+    }
+    T fin0 = 0, fin1 = 0;                 // F entering this CTA's block of chunks
+    if constexpr (CLUSTER) {
+        // y = F of chunk q for a ZERO state entering the block.  The last chunk's value is the
+        // block aggregate: send it to every later rank, then chain the earlier ranks' aggregates.
+        if (ok && q == P - 1)
+            for (int rr = rank + 1; rr < Q; ++rr) st_async_pair(&aggF[rank * S + sys], &bars[BAR_F], rr, y0, y1);
+        if (agg_bytes_f) mbar_wait(&bars[BAR_F], parity);
+        for (int rr = 0; rr < rank; ++rr) {        // F_in(rr+1) = aggF[rr] + TPhiBlock(rr) F_in(rr)
+            T2 a = aggF[rr * S + (ok ? sys : 0)];
+            T n0 = a.x, n1 = a.y;
+            mat2_acc(n0, n1, wtab + 12 * P + 4 * rr, 1, fin0, fin1);
+            fin0 = n0; fin1 = n1;
+        }
+        if (ok && rank > 0) mat2_acc(y0, y1, wtab + 4 * P + q, P, fin0, fin1);   // PF_q F_in
+    }
+    T f0 = shfl_up_t(y0, 1, Pw), f1 = shfl_up_t(y1, 1, Pw);      // F_{q-1}
+    if (q == 0) { f0 = fin0; f1 = fin1; }
+    if (ok) mat2_acc(z0, z1, wtab + q, P, f0, f1);               // TX_q F_{q-1}
+#pragma unroll
+    for (int l = 0; l < W_LEVELS; ++l) {
+        if (l < g.lev_b) {
+            const int d = 1 << l, n = P - d;
+            T u0 = shfl_down_t(z0, d, Pw), u1 = shfl_down_t(z1, d, Pw);
+            if (ok && q + d <= P - 1) mat2_acc(z0, z1, wtab + g.woff[l] + 4 * n + q, n, u0, u1);
+        }
+    }
+    T bin0 = 0, bin1 = 0;                 // B of the first chunk of the NEXT block
+    if constexpr (CLUSTER) {
+        if (ok && q == 0)
+            for (int rr = 0; rr < rank; ++rr) st_async_pair(&aggB[rank * S + sys], &bars[BAR_B], rr, z0, z1);
+        if (agg_bytes_b) mbar_wait(&bars[BAR_B], parity);
+        for (int rr = Q - 1; rr > rank; --rr) {   // B_in(rr-1) = aggB[rr] + TPsiBlock(rr) B_in(rr)
+            T2 a = aggB[rr * S + (ok ? sys : 0)];
+            T n0 = a.x, n1 = a.y;
+            mat2_acc(n0, n1, wtab + 12 * P + 32 + 4 * rr, 1, bin0, bin1);
+            bin0 = n0; bin1 = n1;
+        }
+        if (ok && rank < Q - 1) mat2_acc(z0, z1, wtab + 8 * P + q, P, bin0, bin1);   // PB_q B_in
+    }
+    T b0 = shfl_down_t(z0, 1, Pw), b1 = shfl_down_t(z1, 1, Pw);  // B_{q+1}
+    if (q >= P - 1) { b0 = bin0; b1 = bin1; }
+    if (ok) {
+        T2 fo; fo.x = f0; fo.y = f1; stE[sl] = fo;
+        T2 bo; bo.x = b0; bo.y = b1; stS[sl] = bo;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// host side (defined in pent_solve_chunked.cu)
+// ------------------------------------------------------------------------------------------
+// A launch plan: cluster size Q (CTAs along k), S systems per tile, Pl chunks per CTA.
+struct ChunkPlan {
+    bool ok = false;
+    int j = 0, Q = 1, S = 0, Pl = 0, Pw = 1, threads = 0, levels = 0, box_rows = 0, nbox = 0;
+    size_t table_bytes = 0, smem = 0;
+};
+ChunkPlan make_plan(const pent_handle* h, int64_t M, const void* f, int Q, int S);
+// rank-2 tensor map {M, N} of an interleaved batch with box {S, box_rows}; false on failure
+bool encode_batch_map(CUtensorMap* tm, const void* base, int64_t M, int N, int S, int box_rows, bool f64);
+
+}  // namespace pent

@@ -35,59 +35,6 @@ struct ChunkParams {
     T* x;
 };
 
-template <typename T> struct Pair;
-template <> struct Pair<double> { using type = double2; };
-template <> struct Pair<float>  { using type = float2; };
-
-template <typename T>
-__device__ __forceinline__ T shfl_up_t(T v, int d, int w) { return __shfl_up_sync(0xffffffffu, v, d, w); }
-template <typename T>
-__device__ __forceinline__ T shfl_down_t(T v, int d, int w) { return __shfl_down_sync(0xffffffffu, v, d, w); }
-
-// y += m * u for a row-major 2x2 m stored with element stride `n` (m[e*n])
-template <typename T>
-__device__ __forceinline__ void mat2_acc(T& y0, T& y1, const T* m, int n, T u0, T u1)
-{
-    y0 = fma(m[n], u1, fma(m[0], u0, y0));
-    y1 = fma(m[3 * n], u1, fma(m[2 * n], u0, y1));
-}
-
-// ---- thread-block-cluster helpers (CUDA 12 sm_90+ intrinsics; SASS: UCGABAR_ARV / UCGABAR_WAIT,
-// remote stores through the distributed-shared-memory window)
-__device__ __forceinline__ void cluster_sync_all()
-{
-    __cluster_barrier_arrive();      // release
-    __cluster_barrier_wait();        // acquire
-}
-__device__ __forceinline__ uint32_t map_to_rank(const void* local, uint32_t rank)
-{
-    uint32_t r;
-    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(smem_u32(local)), "r"(rank));
-    return r;
-}
-// Remote store of one chunk state into CTA `rank`'s shared memory that signals that CTA's mbarrier
-// with complete_tx (16 or 8 bytes): producer -> consumer over DSMEM with no thread-scope fence, so
-// the x stores still in flight from the previous tile are not drained (a release-scoped cluster
-// barrier in the tile loop measured 271 us against 215 us for cfg3: profiles/r01_ab_tuning.md).
-__device__ __forceinline__ void st_async_pair(const void* local, const uint64_t* local_bar, uint32_t rank,
-                                              double a, double b)
-{
-    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.f64 [%0], {%1, %2}, [%3];"
-                 ::"r"(map_to_rank(local, rank)), "d"(a), "d"(b), "r"(map_to_rank(local_bar, rank)) : "memory");
-}
-__device__ __forceinline__ void st_async_pair(const void* local, const uint64_t* local_bar, uint32_t rank,
-                                              float a, float b)
-{
-    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.f32 [%0], {%1, %2}, [%3];"
-                 ::"r"(map_to_rank(local, rank)), "f"(a), "f"(b), "r"(map_to_rank(local_bar, rank)) : "memory");
-}
-
-// One CTA = S systems x P chunks (thread = one system, one chunk of C rows, held in registers).
-// blockDim.x >= P*S (a multiple of 32); threads with p >= P only take part in barriers/scan.
-// CLUSTER: the Q CTAs of a cluster own consecutive blocks of P chunks of the SAME S systems; the
-// chunk states are stitched across CTAs through distributed shared memory (two exchanges per tile).
-constexpr int BAR_F = 1 + 2 * MAX_BOXES, BAR_B = 2 + 2 * MAX_BOXES, NUM_BARS = 3 + 2 * MAX_BOXES;
-
 template <typename T, int S, bool CLUSTER>
 __global__ void __launch_bounds__(CHUNK_MAX_THREADS, 1)
 solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T> prm)
@@ -153,6 +100,7 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
     // chunk-state scan geometry: a group of Pw lanes scans one system; G groups per warp
     const int Pw = prm.Pw, G = 32 / Pw;
     const int q = lane % Pw, grp = lane / Pw;
+    const ScanGeom geom{P, Pw, prm.lev_f, prm.lev_b, prm.woff};
     const int rounds = (S + nwarps * G - 1) / (nwarps * G);     // host guarantees 1 when CLUSTER
 
     for (; tile < prm.ntiles; tile += stride) {
@@ -185,106 +133,20 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
             }
         }
         if (active) {
-            // ---- 1. local forward sweep from a zero state (normalised) ----
-            T g1 = 0, g2 = 0;
-#pragma unroll
-            for (int jg = 0; jg < C / 4; ++jg) {
-                T w[12];
-                lds_vec<T, 12>(w, blk + 12 * jg);
-#pragma unroll
-                for (int r = 0; r < 4; ++r) {
-                    const int j = 4 * jg + r;
-                    T t = w[3 * r] * v[j];
-                    t = fma(-w[3 * r + 1], g2, t);
-                    T g = fma(-w[3 * r + 2], g1, t);
-                    v[j] = g; g2 = g1; g1 = g;
-                }
-            }
-            T2 e; e.x = v[C - 2]; e.y = v[C - 1];
+            // ---- 1+2. local forward sweep and local back substitution from zero states ----
+            T2 e, s;
+            chunk_local_sweeps<T>(v, blk, e, s);
             stE[slot] = e;
-            // ---- 2. local back substitution of g~ from a zero state ----
-            T x1 = 0, x2 = 0;
-#pragma unroll
-            for (int jg = C / 4 - 1; jg >= 0; --jg) {
-                T w[8];
-                lds_vec<T, 8>(w, blk + 3 * C + 8 * jg);
-#pragma unroll
-                for (int r = 3; r >= 0; --r) {
-                    const int j = 4 * jg + r;
-                    T xv = fma(-w[2 * r], x1, fma(-w[2 * r + 1], x2, v[j]));   // x1 last: 1 fma on the chain
-                    v[j] = xv; x2 = x1; x1 = xv;
-                }
-            }
-            T2 s; s.x = v[0]; s.y = v[1];
             stS[slot] = s;
         }
         __syncthreads();       // states published
 
-        // ---- 3. chunk-state scans: Kogge-Stone over chunks with warp shuffles ----
-        //   F_q = E~_q + TPhi_q F_{q-1};  B_q = (S^_q + TX_q F_{q-1}) + TPsi_q B_{q+1}
-        // Slot (q, sys) receives what thread (sys, q) needs: F_{q-1} and B_{q+1}.
+        // ---- 3. chunk-state scans (slot (q, sys) receives F_{q-1} and B_{q+1}) ----
         if (CLUSTER || P > 1) {
             for (int r = 0; r < rounds; ++r) {
                 const int sys = (r * nwarps + warp) * G + grp;
-                const bool ok = (sys < S) && (q < P);
-                const int sl = ok ? q * S + sys : 0;
-                T y0 = 0, y1 = 0, z0 = 0, z1 = 0;
-                if (ok) { T2 e = stE[sl]; y0 = e.x; y1 = e.y; T2 s = stS[sl]; z0 = s.x; z1 = s.y; }
-#pragma unroll
-                for (int l = 0; l < W_LEVELS; ++l) {
-                    if (l < prm.lev_f) {
-                        const int d = 1 << l, n = P - d;
-                        T u0 = shfl_up_t(y0, d, Pw), u1 = shfl_up_t(y1, d, Pw);
-                        if (ok && q >= d) mat2_acc(y0, y1, wtab + prm.woff[l] + (q - d), n, u0, u1);
-                    }
-                }
-                T fin0 = 0, fin1 = 0;                 // F entering this CTA's block of chunks
-                if constexpr (CLUSTER) {
-                    // y = F of chunk q for a ZERO state entering the block.  The last chunk's value is
-                    // the block aggregate: publish it to every later rank, then chain the earlier ones.
-                    if (ok && q == P - 1)
-                        for (int rr = rank + 1; rr < prm.Q; ++rr)
-                            st_async_pair(&aggF[rank * S + sys], &bars[BAR_F], rr, y0, y1);
-                    if (agg_bytes_f) mbar_wait(&bars[BAR_F], parity);
-                    for (int rr = 0; rr < rank; ++rr) {        // F_in(rr+1) = aggF[rr] + TPhiBlock(rr) F_in(rr)
-                        T2 a = aggF[rr * S + (ok ? sys : 0)];
-                        T n0 = a.x, n1 = a.y;
-                        mat2_acc(n0, n1, wtab + 12 * P + 4 * rr, 1, fin0, fin1);
-                        fin0 = n0; fin1 = n1;
-                    }
-                    if (ok && rank > 0) mat2_acc(y0, y1, wtab + 4 * P + q, P, fin0, fin1);   // PF_q F_in
-                }
-                T f0 = shfl_up_t(y0, 1, Pw), f1 = shfl_up_t(y1, 1, Pw);      // F_{q-1}
-                if (q == 0) { f0 = fin0; f1 = fin1; }
-                if (ok) mat2_acc(z0, z1, wtab + q, P, f0, f1);               // TX_q F_{q-1}
-#pragma unroll
-                for (int l = 0; l < W_LEVELS; ++l) {
-                    if (l < prm.lev_b) {
-                        const int d = 1 << l, n = P - d;
-                        T u0 = shfl_down_t(z0, d, Pw), u1 = shfl_down_t(z1, d, Pw);
-                        if (ok && q + d <= P - 1) mat2_acc(z0, z1, wtab + prm.woff[l] + 4 * n + q, n, u0, u1);
-                    }
-                }
-                T bin0 = 0, bin1 = 0;                 // B of the first chunk of the NEXT block
-                if constexpr (CLUSTER) {
-                    if (ok && q == 0)
-                        for (int rr = 0; rr < rank; ++rr)
-                            st_async_pair(&aggB[rank * S + sys], &bars[BAR_B], rr, z0, z1);
-                    if (agg_bytes_b) mbar_wait(&bars[BAR_B], parity);
-                    for (int rr = prm.Q - 1; rr > rank; --rr) {   // B_in(rr-1) = aggB[rr] + TPsiBlock(rr) B_in(rr)
-                        T2 a = aggB[rr * S + (ok ? sys : 0)];
-                        T n0 = a.x, n1 = a.y;
-                        mat2_acc(n0, n1, wtab + 12 * P + 32 + 4 * rr, 1, bin0, bin1);
-                        bin0 = n0; bin1 = n1;
-                    }
-                    if (ok && rank < prm.Q - 1) mat2_acc(z0, z1, wtab + 8 * P + q, P, bin0, bin1);   // PB_q B_in
-                }
-                T b0 = shfl_down_t(z0, 1, Pw), b1 = shfl_down_t(z1, 1, Pw);  // B_{q+1}
-                if (q >= P - 1) { b0 = bin0; b1 = bin1; }
-                if (ok) {
-                    T2 fo; fo.x = f0; fo.y = f1; stE[sl] = fo;
-                    T2 bo; bo.x = b0; bo.y = b1; stS[sl] = bo;
-                }
+                chunk_state_scan<T, S, CLUSTER>(geom, wtab, stE, stS, sys, q, (sys < S) && (q < P), rank, prm.Q,
+                                                aggF, aggB, bars, agg_bytes_f, agg_bytes_b, parity);
             }
         }
         __syncthreads();
@@ -298,27 +160,20 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
             if (rows_full && (tile + 1) * S <= prm.M) {
 #pragma unroll
                 for (int jg = 0; jg < C / 4; ++jg) {
-                    T w[16];
-                    lds_vec<T, 16>(w, blk + 5 * C + 16 * jg);
+                    T xv[4];
+                    chunk_correct4<T>(xv, &v[4 * jg], blk, jg, F0, F1, B0, B1);
 #pragma unroll
-                    for (int r = 0; r < 4; ++r) {
-                        T xv = fma(w[4 * r + 3], B1, fma(w[4 * r + 2], B0,
-                               fma(w[4 * r + 1], F1, fma(w[4 * r], F0, v[4 * jg + r]))));
-                        PENT_STORE(xo, xv);
-                        xo += prm.M;
-                    }
+                    for (int r = 0; r < 4; ++r) { PENT_STORE(xo, xv[r]); xo += prm.M; }
                 }
             } else if (col < prm.M) {
                 const int nrows = prm.N - row0;      // may be <= 0
 #pragma unroll
                 for (int jg = 0; jg < C / 4; ++jg) {
-                    T w[16];
-                    lds_vec<T, 16>(w, blk + 5 * C + 16 * jg);
+                    T xv[4];
+                    chunk_correct4<T>(xv, &v[4 * jg], blk, jg, F0, F1, B0, B1);
 #pragma unroll
                     for (int r = 0; r < 4; ++r) {
-                        T xv = fma(w[4 * r + 3], B1, fma(w[4 * r + 2], B0,
-                               fma(w[4 * r + 1], F1, fma(w[4 * r], F0, v[4 * jg + r]))));
-                        if (4 * jg + r < nrows) PENT_STORE(xo, xv);
+                        if (4 * jg + r < nrows) PENT_STORE(xo, xv[r]);
                         xo += prm.M;
                     }
                 }

@@ -70,6 +70,9 @@ int launch_solve_tps(const pent_handle* h, int64_t M, const void* f, void* x, cu
 int launch_solve_chunked(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s,
                          int Q, int S);
 bool chunked_supported(const pent_handle* h, int64_t M, const void* f /* may be null */, int Q, int S);
+bool step_chunked_supported(const pent_handle* h, int64_t M, const void* c /* may be null */);
+int launch_step_chunked(const pent_handle* h, const pent_step_params* p, int64_t M, void* c, int nsteps,
+                        cudaStream_t s);
 int chunked_choice(const pent_handle* h, int64_t M, int* Q, int* S);   // 1 and the default plan, or 0
 
 }  // namespace pent

@@ -27,53 +27,10 @@
 //   stores of this tile.  x goes registers --st.global.cs--> HBM as 128-byte row segments.
 //   The shared coefficient tables (9 values per row) are staged ONCE per CTA into shared memory
 //   with one cp.async.bulk; every sweep step reads them as 16-byte warp-broadcast LDS.
-#include <cuda.h>
 #include <cstdio>
-#include "pent_internal.h"
+#include "pent_chunk_common.cuh"
 
 namespace pent {
-
-template <typename T> struct ChunkCfg;
-template <> struct ChunkCfg<double> { static constexpr int C = 32; };   // rows per thread
-template <> struct ChunkCfg<float>  { static constexpr int C = 64; };
-#ifndef PENT_L2_PROMOTION
-#define PENT_L2_PROMOTION CU_TENSOR_MAP_L2_PROMOTION_L2_256B   // 197 us vs 201 us with 128 B
-#endif
-constexpr int CHUNK_MAX_THREADS = 512;
-constexpr int BOX_ROWS_MAX = 256;           // TMA box dimension limit
-constexpr int MAX_BOXES = 4;
-constexpr int MAX_PL = 32;                  // chunks per CTA (one warp scans a system's chunks)
-constexpr size_t SMEM_LIMIT = 232448;       // 227 KB dynamic shared memory per CTA
-
-// After the P chunk blocks of a (per-rank) table comes the chunk-transfer table W (P = chunks of
-// this CTA, q = local chunk; every 2x2 matrix is row-major with element e at [e*len + index]):
-//   TX   : 4 x P     TX_q
-//   PF   : 4 x P     TPhi_q TPhi_{q-1} ... TPhi_{first chunk of the block}   (acts on the F entering the block)
-//   PB   : 4 x P     TPsi_q TPsi_{q+1} ... TPsi_{last chunk of the block}    (acts on the B entering the block)
-//   BLK  : 64        block products of every cluster rank r: TPhiBlock(r) at [4r..4r+3] (contiguous
-//                    2x2), TPsiBlock(r) at [32+4r..]
-//   then for each Kogge-Stone level l = 0..4, d = 2^l, n = max(0, P-d):
-//   WF_l : 4 x n     TPhi_q TPhi_{q-1} ... TPhi_{q-d+1}  for q >= d,     at [e*n + q-d]
-//   WB_l : 4 x n     TPsi_q TPsi_{q+1} ... TPsi_{q+d-1}  for q+d <= P-1, at [e*n + q]
-// Only the levels a handle needs are staged into shared memory (they come last).
-constexpr int W_LEVELS = 5;
-__host__ __device__ inline int w_level_off(int P, int l)
-{
-    int off = 12 * P + 64;
-    for (int k = 0; k < l; ++k) { int n = P - (1 << k); off += 8 * (n > 0 ? n : 0); }
-    return off;
-}
-__host__ __device__ inline int w_len(int P) { return w_level_off(P, W_LEVELS); }
-
-// per-chunk coefficient block, in units of T:  [fwd 3C | bwd 2C | corr 4C | pad to 16 B]
-template <typename T> __host__ __device__ constexpr int chunk_block_len()
-{
-    return 9 * ChunkCfg<T>::C + (int)(16 / sizeof(T));
-}
-template <typename T> __host__ __device__ constexpr size_t table_len(int P)
-{
-    return (size_t)P * chunk_block_len<T>() + (size_t)w_len(P);
-}
 
 // ------------------------------------------------------------------------------------------
 // table construction (once per handle and cluster size): fp64 arithmetic, rounded to T
@@ -197,7 +154,7 @@ __global__ void build_chunk_products_kernel(int Pl, int Q, const double* __restr
         for (int l = 0; l < W_LEVELS; ++l) {
             double mf = 0.0, mb = 0.0;
             const int d = 1 << l, n = Pl - d;
-            T* base = wtab + w_level_off(Pl, l);
+            T* base = wtab + w_level_off(Pl, l, Q);
             for (int e = 0; e < 4; ++e) {
                 if (q >= d) base[e * n + (q - d)] = (T)wf[l][q][e];
                 if (q + d <= Pl - 1) base[4 * n + e * n + q] = (T)wb[l][q][e];
@@ -208,11 +165,14 @@ __global__ void build_chunk_products_kernel(int Pl, int Q, const double* __restr
         }
         for (int e = 0; e < 4; ++e) {
             wtab[(size_t)e * Pl + q] = (T)tm[q * 12 + 4 + e];
-            wtab[(size_t)(4 + e) * Pl + q] = (T)pf[q][e];
-            wtab[(size_t)(8 + e) * Pl + q] = (T)pb[q][e];
+            if (Q > 1) {
+                wtab[(size_t)(4 + e) * Pl + q] = (T)pf[q][e];
+                wtab[(size_t)(8 + e) * Pl + q] = (T)pb[q][e];
+            }
         }
     }
-    for (int j = q; j < 64; j += blockDim.x) wtab[12 * Pl + j] = (T)blkm[j];
+    if (Q > 1)
+        for (int j = q; j < 64; j += blockDim.x) wtab[12 * Pl + j] = (T)blkm[j];
     __syncthreads();
     if (q == 0) { atomicMax(&levels[0], need_f); atomicMax(&levels[1], need_b); }
 }
@@ -226,7 +186,7 @@ static int build_tables_t(pent_handle* h, int j, cudaStream_t s)
     const int Pl = (P + Q - 1) / Q;
     h->cf[j] = nullptr; h->cfP[j] = 0; h->lev_f[j] = h->lev_b[j] = 0;
     if (Pl > MAX_PL || (Q > 1 && Q > P)) return PENT_OK;     // not a usable split: no tables
-    const size_t tlen = table_len<T>(Pl);
+    const size_t tlen = table_len<T>(Pl, Q);
     cudaError_t e = cudaMalloc(&h->cf[j], tlen * Q * sizeof(T));
     if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); return PENT_ERR_ALLOC; }
     PENT_CUDA(e);
@@ -259,71 +219,6 @@ int build_chunk_tables(pent_handle* h, cudaStream_t s)
     return PENT_OK;
 }
 
-// ------------------------------------------------------------------------------------------
-// PTX helpers: mbarrier, TMA (sm_90+ async proxy; SASS: UTMALDG / UBLKCP / SYNCS)
-// ------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t smem_u32(const void* p)
-{
-    return (uint32_t)__cvta_generic_to_shared(p);
-}
-__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
-                 : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t* bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
-{
-    uint32_t addr = smem_u32(bar), ok;
-    do {
-        asm volatile(
-            "{\n\t.reg .pred p;\n\t"
-            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-            "selp.u32 %0, 1, 0, p;\n\t}"
-            : "=r"(ok) : "r"(addr), "r"(parity) : "memory");
-    } while (!ok);
-}
-__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* tm, int c0, int c1, uint64_t* bar)
-{
-    asm volatile(
-        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes "
-        "[%0], [%1, {%2, %3}], [%4];"
-        ::"r"(smem_u32(dst)), "l"((uint64_t)tm), "r"(c0), "r"(c1), "r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void bulk_load_1d(void* dst, const void* src, uint32_t bytes, uint64_t* bar)
-{
-    asm volatile(
-        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-        ::"r"(smem_u32(dst)), "l"((uint64_t)src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
-}
-
-// n consecutive T values from shared memory with 16-byte loads (n*sizeof(T) % 16 == 0)
-template <typename T, int n>
-__device__ __forceinline__ void lds_vec(T (&dst)[n], const T* src)
-{
-    constexpr int V = 16 / sizeof(T);
-    static_assert(n % V == 0, "vector load granularity");
-    const uint4* s4 = reinterpret_cast<const uint4*>(src);
-#pragma unroll
-    for (int v = 0; v < n / V; ++v) {
-        uint4 q = s4[v];
-        if constexpr (sizeof(T) == 8) {
-            dst[2 * v + 0] = __hiloint2double((int)q.y, (int)q.x);
-            dst[2 * v + 1] = __hiloint2double((int)q.w, (int)q.z);
-        } else {
-            dst[4 * v + 0] = __uint_as_float(q.x); dst[4 * v + 1] = __uint_as_float(q.y);
-            dst[4 * v + 2] = __uint_as_float(q.z); dst[4 * v + 3] = __uint_as_float(q.w);
-        }
-    }
-}
-
 #include "pent_chunked_kernel.cuh"
 
 // ------------------------------------------------------------------------------------------
@@ -349,20 +244,13 @@ static EncodeTiledFn encode_fn()
     return fn;
 }
 
-// A launch plan: cluster size Q (CTAs along k), S systems per tile, Pl chunks per CTA.
-struct ChunkPlan {
-    bool ok = false;
-    int j = 0, Q = 1, S = 0, Pl = 0, Pw = 1, threads = 0, levels = 0, box_rows = 0, nbox = 0;
-    size_t table_bytes = 0, smem = 0;
-};
-
 static bool s_instantiated(bool f64, int S, bool cluster)
 {
     (void)cluster;
     return f64 ? (S == 16 || S == 32) : (S == 32 || S == 64);
 }
 
-static ChunkPlan make_plan(const pent_handle* h, int64_t M, const void* f, int Q, int S)
+ChunkPlan make_plan(const pent_handle* h, int64_t M, const void* f, int Q, int S)
 {
     ChunkPlan pl;
     if (!h || h->kind != 0) return pl;
@@ -387,7 +275,7 @@ static ChunkPlan make_plan(const pent_handle* h, int64_t M, const void* f, int Q
     pl.nbox = (rows + pl.box_rows - 1) / pl.box_rows;
     if (pl.nbox > MAX_BOXES) return pl;
     const size_t bl = f64 ? chunk_block_len<double>() : chunk_block_len<float>();
-    pl.table_bytes = ((size_t)pl.Pl * bl + (size_t)w_level_off(pl.Pl, pl.levels)) * esz;
+    pl.table_bytes = ((size_t)pl.Pl * bl + (size_t)w_level_off(pl.Pl, pl.levels, Q)) * esz;
     pl.smem = (size_t)pl.nbox * pl.box_rows * S * esz + pl.table_bytes + (size_t)4 * pl.Pl * S * esz +
               (Q > 1 ? (size_t)4 * Q * S * esz : 0) + (3 + 2 * MAX_BOXES) * sizeof(uint64_t);
     if (pl.smem > SMEM_LIMIT) return pl;
@@ -397,6 +285,20 @@ static ChunkPlan make_plan(const pent_handle* h, int64_t M, const void* f, int Q
     if (!encode_fn()) return pl;
     pl.ok = true;
     return pl;
+}
+
+bool encode_batch_map(CUtensorMap* tm, const void* base, int64_t M, int N, int S, int box_rows, bool f64)
+{
+    EncodeTiledFn enc = encode_fn();
+    if (!enc) return false;
+    const size_t esz = f64 ? 8 : 4;
+    cuuint64_t gdim[2] = {(cuuint64_t)M, (cuuint64_t)N};
+    cuuint64_t gstr[1] = {(cuuint64_t)M * esz};
+    cuuint32_t box[2] = {(cuuint32_t)S, (cuuint32_t)box_rows};
+    cuuint32_t estr[2] = {1, 1};
+    return enc(tm, f64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2,
+               const_cast<void*>(base), gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_NONE, PENT_L2_PROMOTION, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 // Default plan: the smallest cluster that holds the system on chip and the narrowest tile (more,
@@ -452,26 +354,21 @@ static int launch_inst(const pent_handle* h, const ChunkPlan& pl, int64_t M, con
     while ((1 << lg) < pl.Pw) ++lg;
     prm.lev_f = h->lev_f[pl.j] < lg ? h->lev_f[pl.j] : lg;
     prm.lev_b = h->lev_b[pl.j] < lg ? h->lev_b[pl.j] : lg;
-    for (int l = 0; l < W_LEVELS; ++l) prm.woff[l] = w_level_off(pl.Pl, l);
+    for (int l = 0; l < W_LEVELS; ++l) prm.woff[l] = w_level_off(pl.Pl, l, pl.Q);
     prm.box_rows = pl.box_rows; prm.nbox = pl.nbox;
     prm.ntiles = (M + S - 1) / S;
     for (int b = 0; b < MAX_BOXES; ++b) prm.wcount[b] = 0;
     for (int w = 0; w * 32 < pl.Pl * S; ++w) prm.wcount[((w * 32 / S) * C) / prm.box_rows] += 1;
     prm.table = (const T*)h->cf[pl.j];
-    prm.table_stride = (int64_t)table_len<T>(pl.Pl);
+    prm.table_stride = (int64_t)table_len<T>(pl.Pl, pl.Q);
     prm.table_bytes = (uint32_t)pl.table_bytes;
     prm.x = (T*)x;
 
     CUtensorMap tm;
-    cuuint64_t gdim[2] = {(cuuint64_t)M, (cuuint64_t)h->N};
-    cuuint64_t gstr[1] = {(cuuint64_t)M * sizeof(T)};
-    cuuint32_t box[2] = {(cuuint32_t)S, (cuuint32_t)prm.box_rows};
-    cuuint32_t estr[2] = {1, 1};
-    CUresult cr = encode_fn()(&tm, sizeof(T) == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32,
-                              2, const_cast<void*>(f), gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                              CU_TENSOR_MAP_SWIZZLE_NONE, PENT_L2_PROMOTION,
-                              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (cr != CUDA_SUCCESS) { g_last_cuda_error = (int)cudaErrorInvalidValue; return PENT_ERR_CUDA; }
+    if (!encode_batch_map(&tm, f, M, h->N, S, prm.box_rows, sizeof(T) == 8)) {
+        g_last_cuda_error = (int)cudaErrorInvalidValue;
+        return PENT_ERR_CUDA;
+    }
 
     auto kern = solve_chunked_kernel<T, S, CLUSTER>;
     static thread_local size_t smem_set = 0;

@@ -89,74 +89,136 @@ int launch_solve_tps(const pent_handle* h, int64_t M, const void* f, void* x, cu
 //   MODE 0: fused factor+solve (gam/del are scratch)      -- pent_factor_solve_batch
 //   MODE 1: factor only, store ia,en,bn,gamma,delta        -- pent_factor_batch
 // ---------------------------------------------------------------------------------------------
+constexpr int PS_UNROLL = 8;     // rows whose loads are issued together (6 streams x 8 rows in flight per thread)
+constexpr int PS_THREADS = 64;   // small blocks: M is the only parallelism, spread it over all SMs
+
 template <typename T, int MODE>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(PS_THREADS)
 factor_tps_kernel(int N, int64_t M, const T* __restrict__ a, const T* __restrict__ b,
                   const T* __restrict__ c, const T* __restrict__ d, const T* __restrict__ e,
                   const T* f, T* x, T* __restrict__ gam, T* __restrict__ del,
                   T* __restrict__ ia_o, T* __restrict__ en_o, T* __restrict__ bn_o,
                   int* __restrict__ info)
 {
+    constexpr int U = PS_UNROLL;
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= M) return;
     T ga1 = 0, ga2 = 0, de1 = 0, de2 = 0, g1 = 0, g2 = 0;
     int bad = 0;
-    for (int k = 0; k < N; ++k) {
-        int64_t o = (int64_t)k * M + i;
-        T ak = (k >= 2) ? __ldcs(a + o) : (T)0;
-        T bk = (k >= 1) ? __ldcs(b + o) : (T)0;
-        T ck = __ldcs(c + o);
-        T dk = (k + 1 < N) ? __ldcs(d + o) : (T)0;
-        T ek = (k + 2 < N) ? __ldcs(e + o) : (T)0;
-        T be = fma(-ak, ga2, bk);
-        T al = fma(-be, ga1, fma(-ak, de2, ck));
-        if (bad == 0 && (al == (T)0 || !isfinite(al))) bad = k + 1;
-        T inv = (T)1 / al;
-        T ga = fma(-be, de1, dk) * inv;
-        T de = ek * inv;
-        gam[o] = ga; del[o] = de;
-        if (MODE == 0) {
-            T g = fma(-be, g1, fma(-ak, g2, f[o])) * inv;
-            x[o] = g;
-            g2 = g1; g1 = g;
-        } else {
-            ia_o[o] = inv; en_o[o] = ak * inv; bn_o[o] = be * inv;
+    for (int k0 = 0; k0 < N; k0 += U) {
+        // The serial recurrence below waits on nothing but registers: all loads of the next U rows
+        // are in flight before its first step (latency, not bandwidth, bounds one thread per system).
+        T av[U], bv[U], cv[U], dv[U], ev[U], fv[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int k = k0 + u;
+            const int64_t o = (int64_t)k * M + i;
+            av[u] = (k >= 2 && k < N) ? __ldcs(a + o) : (T)0;
+            bv[u] = (k >= 1 && k < N) ? __ldcs(b + o) : (T)0;
+            cv[u] = (k < N) ? __ldcs(c + o) : (T)1;
+            dv[u] = (k + 1 < N) ? __ldcs(d + o) : (T)0;
+            ev[u] = (k + 2 < N) ? __ldcs(e + o) : (T)0;
+            if (MODE == 0) fv[u] = (k < N) ? f[o] : (T)0;
         }
-        ga2 = ga1; ga1 = ga; de2 = de1; de1 = de;
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int k = k0 + u;
+            if (k < N) {
+                const int64_t o = (int64_t)k * M + i;
+                T be = fma(-av[u], ga2, bv[u]);
+                T al = fma(-be, ga1, fma(-av[u], de2, cv[u]));
+                if (bad == 0 && (al == (T)0 || !isfinite(al))) bad = k + 1;
+                T inv = (T)1 / al;
+                T ga = fma(-be, de1, dv[u]) * inv;
+                T de = ev[u] * inv;
+                gam[o] = ga; del[o] = de;
+                if (MODE == 0) {
+                    T g = fma(-be, g1, fma(-av[u], g2, fv[u])) * inv;
+                    x[o] = g;
+                    g2 = g1; g1 = g;
+                } else {
+                    ia_o[o] = inv; en_o[o] = av[u] * inv; bn_o[o] = be * inv;
+                }
+                ga2 = ga1; ga1 = ga; de2 = de1; de1 = de;
+            }
+        }
     }
     if (info) info[i] = bad;
     if (MODE == 0) {
         T x1 = 0, x2 = 0;
-        for (int k = N - 1; k >= 0; --k) {
-            int64_t o = (int64_t)k * M + i;
-            T xv = fma(-del[o], x2, fma(-gam[o], x1, x[o]));
-            __stcs(x + o, xv);
-            x2 = x1; x1 = xv;
+        for (int k0 = N - 1; k0 >= 0; k0 -= U) {
+            T gv[U], dv[U], xv[U];
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const int k = k0 - u;
+                const int64_t o = (int64_t)k * M + i;
+                gv[u] = (k >= 0) ? gam[o] : (T)0;
+                dv[u] = (k >= 0) ? del[o] : (T)0;
+                xv[u] = (k >= 0) ? x[o] : (T)0;
+            }
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const int k = k0 - u;
+                if (k >= 0) {
+                    T r = fma(-dv[u], x2, fma(-gv[u], x1, xv[u]));
+                    __stcs(x + (int64_t)k * M + i, r);
+                    x2 = x1; x1 = r;
+                }
+            }
         }
     }
 }
 
 // Solve with stored per-system factors (layout ms: ia, en, bn, gamma, delta, each N*M).
 template <typename T>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(PS_THREADS)
 solve_multi_kernel(int N, int64_t M, const T* __restrict__ ms, const T* f, T* x)
 {
+    constexpr int U = PS_UNROLL;
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= M) return;
     const int64_t NM = (int64_t)N * M;
     T g1 = 0, g2 = 0;
-    for (int k = 0; k < N; ++k) {
-        int64_t o = (int64_t)k * M + i;
-        T g = fma(-ms[2 * NM + o], g1, fma(-ms[NM + o], g2, ms[o] * f[o]));
-        x[o] = g;
-        g2 = g1; g1 = g;
+    for (int k0 = 0; k0 < N; k0 += U) {
+        T iv[U], ev[U], bv[U], fv[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int k = k0 + u;
+            const int64_t o = (int64_t)k * M + i;
+            const bool in = k < N;
+            iv[u] = in ? ms[o] : (T)0; ev[u] = in ? ms[NM + o] : (T)0; bv[u] = in ? ms[2 * NM + o] : (T)0;
+            fv[u] = in ? f[o] : (T)0;
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int k = k0 + u;
+            if (k < N) {
+                T g = fma(-bv[u], g1, fma(-ev[u], g2, iv[u] * fv[u]));
+                x[(int64_t)k * M + i] = g;
+                g2 = g1; g1 = g;
+            }
+        }
     }
     T x1 = 0, x2 = 0;
-    for (int k = N - 1; k >= 0; --k) {
-        int64_t o = (int64_t)k * M + i;
-        T xv = fma(-ms[4 * NM + o], x2, fma(-ms[3 * NM + o], x1, x[o]));
-        x[o] = xv;
-        x2 = x1; x1 = xv;
+    for (int k0 = N - 1; k0 >= 0; k0 -= U) {
+        T gv[U], dv[U], xv[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int k = k0 - u;
+            const int64_t o = (int64_t)k * M + i;
+            gv[u] = (k >= 0) ? ms[3 * NM + o] : (T)0;
+            dv[u] = (k >= 0) ? ms[4 * NM + o] : (T)0;
+            xv[u] = (k >= 0) ? x[o] : (T)0;
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int k = k0 - u;
+            if (k >= 0) {
+                T r = fma(-dv[u], x2, fma(-gv[u], x1, xv[u]));
+                x[(int64_t)k * M + i] = r;
+                x2 = x1; x1 = r;
+            }
+        }
     }
 }
 
@@ -170,7 +232,7 @@ static int factor_solve_impl(int N, int64_t M, const void* e, const void* c, con
     cudaError_t er = cudaMallocAsync((void**)&scratch, 2 * NM * sizeof(T), s);
     if (er == cudaErrorMemoryAllocation) { cudaGetLastError(); return PENT_ERR_ALLOC; }
     PENT_CUDA(er);
-    const int tb = 128;
+    const int tb = PS_THREADS;
     unsigned nb = (unsigned)((M + tb - 1) / tb);
     factor_tps_kernel<T, 0><<<nb, tb, 0, s>>>(N, M, (const T*)a, (const T*)b, (const T*)c,
                                               (const T*)d, (const T*)e, (const T*)f, (T*)x,
@@ -188,7 +250,7 @@ static int factor_batch_impl(pent_handle* h, const void* e, const void* c, const
 {
     size_t NM = (size_t)h->N * (size_t)h->M;
     T* ms = (T*)h->ms;
-    const int tb = 128;
+    const int tb = PS_THREADS;
     unsigned nb = (unsigned)((h->M + tb - 1) / tb);
     factor_tps_kernel<T, 1><<<nb, tb, 0, s>>>(h->N, h->M, (const T*)a, (const T*)b, (const T*)c,
                                               (const T*)d, (const T*)e, nullptr, nullptr,
@@ -243,7 +305,7 @@ extern "C" int pent_factor_batch(int N, int64_t M, const void* e, const void* c,
 extern "C" int pent_solve_batch_multi(const pent_handle* h, const void* f, void* x, void* stream)
 {
     if (!h || h->kind != 1 || !f || !x) return PENT_ERR_ARG;
-    const int tb = 128;
+    const int tb = pent::PS_THREADS;
     unsigned nb = (unsigned)((h->M + tb - 1) / tb);
     cudaStream_t s = (cudaStream_t)stream;
     if (h->dtype == PENT_F64)

@@ -7,7 +7,8 @@
 //  L = second-difference matrix: (L v)_k = v_{k-1} + dg_k v_k + v_{k+1}, out-of-range terms
 //  dropped, dg_k = -2 except dg_0 = dg_{N-1} = -1 when bc = 1 (zero-flux).
 //
-// Thread-per-system version: the state is read through a sliding window of rows held in
+// This file: the thread-per-system version (one launch per step, 4 passes) used when the tile does
+// not fit on chip; the default path is the on-chip kernel of pent_step_chunked.cu.  The state is read through a sliding window of rows held in
 // registers (each c_k is loaded exactly once in the forward sweep), the right-hand side of
 // row k is formed in registers and consumed at once by the forward recurrence; g goes to
 // `scratch`; the back substitution writes the new state in place.
@@ -119,15 +120,33 @@ static int step_impl(const pent_handle* h, const pent_step_params* p, int64_t M,
 }
 }  // namespace pent
 
-extern "C" int pent_step_batch(const pent_handle* h, const pent_step_params* p, int64_t M,
-                               void* c_inout, void* scratch, int nsteps, void* stream)
+extern "C" int pent_step_batch_v(const pent_handle* h, const pent_step_params* p, int64_t M,
+                                 void* c_inout, void* scratch, int nsteps, void* stream, int kernel)
 {
     if (!h || h->kind != 0 || !p || M < 0 || nsteps < 0 || !c_inout) return PENT_ERR_ARG;
     if (p->kind != 0 && p->kind != 1) return PENT_ERR_ARG;
     if (p->kind == 0 && ((p->bc != 0 && p->bc != 1) || (p->form != 0 && p->form != 1)))
         return PENT_ERR_ARG;
+    if (kernel != PENT_KERNEL_AUTO && kernel != PENT_KERNEL_THREAD_PER_SYSTEM && kernel != PENT_KERNEL_CHUNKED)
+        return PENT_ERR_ARG;
     if (M == 0 || nsteps == 0) return PENT_OK;
     cudaStream_t s = (cudaStream_t)stream;
+    const bool on_chip = pent::step_chunked_supported(h, M, c_inout);
+    if (kernel == PENT_KERNEL_CHUNKED && !on_chip) return PENT_ERR_ARG;
+    if (kernel != PENT_KERNEL_THREAD_PER_SYSTEM && on_chip)
+        return pent::launch_step_chunked(h, p, M, c_inout, nsteps, s);
     if (h->dtype == PENT_F64) return pent::step_impl<double>(h, p, M, c_inout, scratch, nsteps, s);
     return pent::step_impl<float>(h, p, M, c_inout, scratch, nsteps, s);
+}
+
+extern "C" int pent_step_batch(const pent_handle* h, const pent_step_params* p, int64_t M,
+                               void* c_inout, void* scratch, int nsteps, void* stream)
+{
+    return pent_step_batch_v(h, p, M, c_inout, scratch, nsteps, stream, PENT_KERNEL_AUTO);
+}
+
+extern "C" int pent_step_kernel_choice(const pent_handle* h, int64_t M)
+{
+    if (!h || h->kind != 0) return -1;
+    return pent::step_chunked_supported(h, M, nullptr) ? PENT_KERNEL_CHUNKED : PENT_KERNEL_THREAD_PER_SYSTEM;
 }

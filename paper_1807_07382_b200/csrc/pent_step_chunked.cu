@@ -1,0 +1,258 @@
+// pent_step_chunked.cu -- fused time stepping with the state ON CHIP across steps
+// (BASELINE.json configs[3]; PAPER.md:53 Eq. 2, :87-89 Eq. 6, :117 Eq. 7c, :273).
+//
+// The systems of a batch never interact, so a CTA can take a tile of S systems through ALL
+// `nsteps` steps before it touches HBM again: the tile's state (S x N values, 128 KiB) is loaded
+// once by TMA into shared memory, every step builds the explicit right-hand side from it in
+// registers (5-point window along k, neighbours of other chunks read from the shared state),
+// runs the chunked solve of pent_solve_chunked.cu on the registers (local sweeps, chunk-state
+// scan, correction) and writes the new state back to shared memory; after the last step the tile
+// goes back to HBM with one TMA store per box.  HBM traffic per launch is 2 passes over the
+// state whatever nsteps is (the paper's loop costs 2 kernels and >= 6 passes PER STEP:
+// PAPER.md:273); the per-step cost is arithmetic and three block barriers.
+//
+//  kind 0  Cahn-Hilliard:  form 0  A c+ = c + r L (c^3 - c)
+//                          form 1  q = r (c^3 - c) - sigma L c ;  A delta = L q ;  c+ = c + delta
+//  kind 1  hyperdiffusion Crank-Nicolson:  A c+ = (2I - A) c   (diagonals read from the handle)
+//  (L v)_k = v_{k-1} + dg_k v_k + v_{k+1}, out-of-range terms dropped; dg_k = -2 except
+//  dg_0 = dg_{N-1} = -1 when bc = 1 (zero-flux).  Same formulas, in the same order, as
+//  step_tps_kernel (pent_step.cu).
+#include "pent_chunk_common.cuh"
+
+namespace pent {
+
+template <typename T>
+struct StepChunkParams {
+    int N, P, Pw, lev_f, lev_b;
+    int woff[W_LEVELS];
+    int box_rows, nbox;
+    uint32_t table_bytes;
+    int64_t M, ntiles;
+    const T* table;
+    const T* dg;          // N x {a,b,c,d,e,0,0,0} (kind 1)
+    int nsteps, bc, form;
+    T r, sigma;
+};
+
+__device__ __forceinline__ void tma_store_2d(const CUtensorMap* tm, int c0, int c1, const void* src)
+{
+    asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%1, %2}], [%3];"
+                 ::"l"((uint64_t)tm), "r"(c0), "r"(c1), "r"(smem_u32(src)) : "memory");
+}
+
+template <typename T, int S, int KIND>
+__global__ void __launch_bounds__(CHUNK_MAX_THREADS, 1)
+step_chunked_kernel(const __grid_constant__ CUtensorMap tm, const StepChunkParams<T> prm)
+{
+    constexpr int C = ChunkCfg<T>::C, BL = chunk_block_len<T>();
+    using T2 = typename Pair<T>::type;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int P = prm.P, N = prm.N;
+    T* state = reinterpret_cast<T*>(smem_raw);                       // [rows][S], the tile's c
+    T* table = state + (size_t)prm.nbox * prm.box_rows * S;
+    T2* stE = reinterpret_cast<T2*>(reinterpret_cast<unsigned char*>(table) + prm.table_bytes);
+    T2* stS = stE + (size_t)S * P;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(stS + (size_t)S * P);   // [0] table, [1] state
+
+    const int tid = threadIdx.x, i = tid % S, p = tid / S;
+    const bool active = p < P;
+    const int lane = tid & 31, warp = tid >> 5, nwarps = blockDim.x >> 5;
+    const uint32_t box_bytes = (uint32_t)(prm.box_rows * S * sizeof(T));
+
+    if (tid == 0) {
+        mbar_init(&bars[0], 1);
+        mbar_init(&bars[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncthreads();
+    if (tid == 0) {
+        mbar_expect_tx(&bars[0], prm.table_bytes);
+        bulk_load_1d(table, prm.table, prm.table_bytes, &bars[0]);
+    }
+    mbar_wait(&bars[0], 0);
+
+    const T* blk = table + (size_t)(active ? p : 0) * BL;
+    const T* wtab = table + (size_t)P * BL;
+    const int slot = (active ? p : 0) * S + i;
+    const int row0 = p * C;
+    T* cs = state + i;                                   // element (k, i) at cs[k*S]
+    const int Pw = prm.Pw, G = 32 / Pw;
+    const int q = lane % Pw, grp = lane / Pw;
+    const ScanGeom geom{P, Pw, prm.lev_f, prm.lev_b, prm.woff};
+    const int rounds = (S + nwarps * G - 1) / (nwarps * G);
+    const T r = prm.r, sigma = prm.sigma;
+    constexpr bool incr = (KIND == 2);       // KIND: 0 CH direct form, 2 CH increment form, 1 hyperdiffusion
+    const T dg_edge = (prm.bc == 1) ? (T)-1 : (T)-2;
+    auto ldc = [&](int k) -> T { return ((unsigned)k < (unsigned)N) ? cs[(size_t)k * S] : (T)0; };
+    auto Ld = [&](int k) -> T { return (k == 0 || k == N - 1) ? dg_edge : (T)-2; };
+    uint32_t parity = 0;
+
+    for (int64_t tile = blockIdx.x; tile < prm.ntiles; tile += gridDim.x) {
+        if (tid == 0) {
+            mbar_expect_tx(&bars[1], box_bytes * prm.nbox);
+            for (int b = 0; b < prm.nbox; ++b)
+                tma_load_2d(state + (size_t)b * prm.box_rows * S, &tm, (int)(tile * S), b * prm.box_rows, &bars[1]);
+        }
+        mbar_wait(&bars[1], parity);
+
+        for (int step = 0; step < prm.nsteps; ++step) {
+            T v[C];
+            if (active) {
+                // ---- explicit right-hand side of rows row0 .. row0+C-1, in registers ----
+                if constexpr (KIND != 1) {
+                    // u_k = w_k = c_k^3 - c_k (form 0) or q_k = r w_k - sigma (L c)_k (form 1), 0 outside 0..N-1
+                    auto U = [&](int k, T cl, T cc, T cr) -> T {
+                        if ((unsigned)k >= (unsigned)N) return (T)0;
+                        T w = cc * cc * cc - cc;
+                        if (!incr) return w;
+                        return fma(-sigma, cl + fma(Ld(k), cc, cr), r * w);
+                    };
+                    T cl = ldc(row0 - 2), cc = ldc(row0 - 1), cr = ldc(row0);
+                    T u_prev = U(row0 - 1, cl, cc, cr);
+                    cl = cc; cc = cr; cr = ldc(row0 + 1);
+                    T u_cur = U(row0, cl, cc, cr);
+#pragma unroll
+                    for (int j = 0; j < C; ++j) {
+                        const int k = row0 + j;
+                        cl = cc; cc = cr; cr = ldc(k + 2);          // window centred on k+1; cl = c_k
+                        T u_next = U(k + 1, cl, cc, cr);
+                        T Lu = u_prev + fma(Ld(k), u_cur, u_next);
+                        v[j] = incr ? Lu : fma(r, Lu, cl);
+                        u_prev = u_cur; u_cur = u_next;
+                    }
+                } else {
+                    T cm2 = ldc(row0 - 2), cm1 = ldc(row0 - 1), c0 = ldc(row0), cp1 = ldc(row0 + 1);
+#pragma unroll
+                    for (int j = 0; j < C; ++j) {
+                        const int k = row0 + j;
+                        T cp2 = ldc(k + 2);
+                        T rhs = 0;
+                        if (k < N) {
+                            const T* dk = prm.dg + 8 * (size_t)k;
+                            T s = __ldg(dk + 2) * c0;
+                            s = fma(__ldg(dk + 1), cm1, s);
+                            s = fma(__ldg(dk + 0), cm2, s);
+                            s = fma(__ldg(dk + 3), cp1, s);
+                            s = fma(__ldg(dk + 4), cp2, s);
+                            rhs = (T)2 * c0 - s;
+                        }
+                        v[j] = rhs;
+                        cm2 = cm1; cm1 = c0; c0 = cp1; cp1 = cp2;
+                    }
+                }
+                // ---- chunked solve, stages 1+2 ----
+                T2 e, s;
+                chunk_local_sweeps<T>(v, blk, e, s);
+                stE[slot] = e;
+                stS[slot] = s;
+            }
+            __syncthreads();
+            if (P > 1) {
+                for (int rr = 0; rr < rounds; ++rr) {
+                    const int sys = (rr * nwarps + warp) * G + grp;
+                    chunk_state_scan<T, S, false>(geom, wtab, stE, stS, sys, q, (sys < S) && (q < P), 0, 1,
+                                                  nullptr, nullptr, bars, 0u, 0u, 0u);
+                }
+            }
+            __syncthreads();
+            if (active) {
+                T F0 = 0, F1 = 0, B0 = 0, B1 = 0;
+                if (P > 1) { T2 fo = stE[slot]; F0 = fo.x; F1 = fo.y; T2 bo = stS[slot]; B0 = bo.x; B1 = bo.y; }
+                T* co = cs + (size_t)row0 * S;
+#pragma unroll
+                for (int jg = 0; jg < C / 4; ++jg) {
+                    T xv[4];
+                    chunk_correct4<T>(xv, &v[4 * jg], blk, jg, F0, F1, B0, B1);
+#pragma unroll
+                    for (int rr = 0; rr < 4; ++rr) {
+                        T* o = co + (size_t)(4 * jg + rr) * S;
+                        *o = incr ? *o + xv[rr] : xv[rr];
+                    }
+                }
+            }
+            __syncthreads();       // the next step's windows read rows written by other threads
+        }
+        // ---- tile back to HBM: generic-proxy writes -> async proxy, then one TMA store per box ----
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncthreads();
+        if (tid == 0) {
+            for (int b = 0; b < prm.nbox; ++b)
+                tma_store_2d(&tm, (int)(tile * S), b * prm.box_rows, state + (size_t)b * prm.box_rows * S);
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+            asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // shared memory may be overwritten
+        }
+        __syncthreads();
+        parity ^= 1;
+    }
+    if (tid == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+}
+
+template <typename T, int S, int KIND>
+static int launch_step_inst(const pent_handle* h, const ChunkPlan& pl, const pent_step_params* p, int64_t M,
+                            void* c, int nsteps, cudaStream_t s)
+{
+    StepChunkParams<T> prm;
+    prm.N = h->N; prm.P = pl.Pl; prm.Pw = pl.Pw; prm.M = M;
+    int lg = 0;
+    while ((1 << lg) < pl.Pw) ++lg;
+    prm.lev_f = h->lev_f[0] < lg ? h->lev_f[0] : lg;
+    prm.lev_b = h->lev_b[0] < lg ? h->lev_b[0] : lg;
+    for (int l = 0; l < W_LEVELS; ++l) prm.woff[l] = w_level_off(pl.Pl, l, 1);
+    prm.box_rows = pl.box_rows; prm.nbox = pl.nbox;
+    prm.ntiles = (M + S - 1) / S;
+    prm.table = (const T*)h->cf[0];
+    prm.table_bytes = (uint32_t)pl.table_bytes;
+    prm.dg = (const T*)h->dg;
+    prm.nsteps = nsteps; prm.bc = p->bc; prm.form = p->form;
+    prm.r = (T)p->r; prm.sigma = (T)p->sigma;
+    CUtensorMap tm;
+    if (!encode_batch_map(&tm, c, M, h->N, S, prm.box_rows, sizeof(T) == 8)) {
+        g_last_cuda_error = (int)cudaErrorInvalidValue;
+        return PENT_ERR_CUDA;
+    }
+    auto kern = step_chunked_kernel<T, S, KIND>;
+    static thread_local size_t smem_set = 0;
+    if (pl.smem > smem_set) {
+        PENT_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
+        smem_set = pl.smem;
+    }
+    int dev = 0, nsm = 0, occ = 0;
+    PENT_CUDA(cudaGetDevice(&dev));
+    PENT_CUDA(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+    PENT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, pl.threads, pl.smem));
+    if (occ < 1) return PENT_ERR_ARG;
+    int64_t grid = (int64_t)nsm * occ;
+    if (grid > prm.ntiles) grid = prm.ntiles;
+    kern<<<(unsigned)grid, pl.threads, pl.smem, s>>>(tm, prm);
+    count_launch();
+    PENT_LAUNCH_CHECK();
+    return PENT_OK;
+}
+
+static ChunkPlan step_plan(const pent_handle* h, int64_t M, const void* c)
+{
+    return make_plan(h, M, c, 1, h->dtype == PENT_F64 ? 16 : 32);
+}
+
+bool step_chunked_supported(const pent_handle* h, int64_t M, const void* c)
+{
+    return h && h->kind == 0 && step_plan(h, M, c).ok;
+}
+
+int launch_step_chunked(const pent_handle* h, const pent_step_params* p, int64_t M, void* c, int nsteps,
+                        cudaStream_t s)
+{
+    const ChunkPlan pl = step_plan(h, M, c);
+    if (!pl.ok) return PENT_ERR_ARG;
+    const int kind = p->kind == 1 ? 1 : (p->form == 1 ? 2 : 0);
+    if (h->dtype == PENT_F64) {
+        if (kind == 0) return launch_step_inst<double, 16, 0>(h, pl, p, M, c, nsteps, s);
+        if (kind == 1) return launch_step_inst<double, 16, 1>(h, pl, p, M, c, nsteps, s);
+        return launch_step_inst<double, 16, 2>(h, pl, p, M, c, nsteps, s);
+    }
+    if (kind == 0) return launch_step_inst<float, 32, 0>(h, pl, p, M, c, nsteps, s);
+    if (kind == 1) return launch_step_inst<float, 32, 1>(h, pl, p, M, c, nsteps, s);
+    return launch_step_inst<float, 32, 2>(h, pl, p, M, c, nsteps, s);
+}
+}  // namespace pent

@@ -100,16 +100,20 @@ def _ch_setup(N, M, bcname, seed=4):
     return diags, sigma, r, c0
 
 
+STEP_KERNELS = [1, 2]      # thread per system (one launch per step), on-chip chunked (one launch)
+
+
+@pytest.mark.parametrize("kernel", STEP_KERNELS)
 @pytest.mark.parametrize("bc,bcname", [(1, "zeroflux"), (0, "dirichlet")])
 @pytest.mark.parametrize("form", [1, 0])
-@pytest.mark.parametrize("N,M", [(1024, 300), (64, 33), (4, 5)])
-def test_ch_one_step_parity(bc, bcname, form, N, M):
+@pytest.mark.parametrize("N,M", [(1024, 300), (64, 34), (4, 6), (1000, 130), (37, 18)])
+def test_ch_one_step_parity(kernel, bc, bcname, form, N, M):
     pent = _pent()
     diags, sigma, r, c0 = _ch_setup(N, M, bcname)
     a, b, c, d, e = (torch.tensor(v) for v in diags)
     h = pent.pent_factor(N, e, c, d, a, b)
     cd = _dev(c0)
-    pent.pent_step_batch(h, M, cd, 1, kind=0, bc=bc, form=form, r=r, sigma=sigma)
+    pent.pent_step_batch(h, M, cd, 1, kind=0, bc=bc, form=form, r=r, sigma=sigma, kernel=kernel)
     ref = oracle.step_batch(oracle.factor(*diags), 0, bc, form, r, sigma, c0, 1)
     # Two correct fp64 evaluations of one step differ by ~cond(A)*eps (no-pivot LU forward
     # error); cond(I + sigma L^2) <= 1 + 16 sigma.  At N=1024 sigma = 1.1e4, cond*eps = 2e-11:
@@ -118,20 +122,39 @@ def test_ch_one_step_parity(bc, bcname, form, N, M):
     assert normwise(cd.cpu().numpy(), ref) <= tol
 
 
-def test_hyperdiffusion_step_parity_general_matrix():
+@pytest.mark.parametrize("kernel,N,M", [(1, 300, 129), (2, 300, 130), (2, 1024, 64), (2, 33, 20), (0, 300, 129)])
+def test_hyperdiffusion_step_parity_general_matrix(kernel, N, M):
     pent = _pent()
-    N, M = 300, 129
     diags = pin.random_diag_dominant(21, N)
     a, b, c, d, e = (torch.tensor(v) for v in diags)
     h = pent.pent_factor(N, e, c, d, a, b)
     c0 = pin.uniform_pm1(22, 0, N, M)
     cd = _dev(c0)
-    pent.pent_step_batch(h, M, cd, 3, kind=1)
+    pent.pent_step_batch(h, M, cd, 3, kind=1, kernel=kernel)
     ref = oracle.step_batch(oracle.factor(*diags), 1, 0, 0, 0.0, 0.0, c0, 3)
     assert normwise(cd.cpu().numpy(), ref) <= 1e-11
 
 
-def test_cfg4_thousand_steps_conservation_and_trajectory():
+def test_multi_step_on_chip_equals_repeated_single_steps():
+    """The on-chip kernel keeps the state in shared memory across steps: n steps in one launch must
+    give bit-identical results to n launches of one step (same arithmetic, same order)."""
+    pent = _pent()
+    N, M = 512, 96
+    diags, sigma, r, c0 = _ch_setup(N, M, "zeroflux")
+    a, b, c, d, e = (torch.tensor(v) for v in diags)
+    h = pent.pent_factor(N, e, c, d, a, b)
+    assert pent.lib().pent_step_kernel_choice(h.ptr, M) == pent.KERNEL_CHUNKED
+    c1, c2 = _dev(c0), _dev(c0)
+    pent.pent_step_batch(h, M, c1, 7, kind=0, bc=1, form=1, r=r, sigma=sigma, kernel=2)
+    for _ in range(7):
+        pent.pent_step_batch(h, M, c2, 1, kind=0, bc=1, form=1, r=r, sigma=sigma, kernel=2)
+    assert torch.equal(c1, c2)
+    ref = oracle.step_batch(oracle.factor(*diags), 0, 1, 1, r, sigma, c0, 7)
+    assert normwise(c1.cpu().numpy(), ref) <= 7 * max(1e-11, 4.0 * (1.0 + 16.0 * sigma) * 2.0 ** -53)
+
+
+@pytest.mark.parametrize("kernel", STEP_KERNELS)
+def test_cfg4_thousand_steps_conservation_and_trajectory(kernel):
     """BASELINE.json configs[3]: N=1024, M=8192, 1000 fused steps, zero-flux L, increment form.
     mean(c) per run conserved to 1e-12 (every system, fsum on the host); trajectory parity with
     the oracle after 1000 nonlinear steps on a window of 64 systems to 1e-9."""
@@ -144,10 +167,10 @@ def test_cfg4_thousand_steps_conservation_and_trajectory():
     cd = _dev(c0)
     scratch = torch.empty_like(cd)
     pent.pent_step_batch(h, w.M, cd, 1000, kind=0, bc=1, form=1, r=R_CH, sigma=SIGMA_CH,
-                         scratch=scratch)
+                         scratch=scratch, kernel=kernel)
     c1 = cd.cpu().numpy()
     assert np.isfinite(c1).all()
-    drift = max(abs(math.fsum(c1[:, i]) - math.fsum(c0[:, i])) / w.N for i in range(0, w.M, 7))
+    drift = max(abs(math.fsum(c1[:, i]) - math.fsum(c0[:, i])) / w.N for i in range(0, w.M, 3))
     assert drift <= 1e-12
     cols = np.r_[0:32, w.M - 32:w.M]
     ref = oracle.step_batch(oracle.factor(*diags), 0, 1, 1, R_CH, SIGMA_CH,
@@ -156,7 +179,8 @@ def test_cfg4_thousand_steps_conservation_and_trajectory():
     assert np.max(np.abs(c1 - c0)) > 1e-3          # the state evolved
 
 
-def test_step_fp32_one_step():
+@pytest.mark.parametrize("kernel", STEP_KERNELS)
+def test_step_fp32_one_step(kernel):
     pent = _pent()
     N, M = 256, 200
     diags, sigma, r, c0 = _ch_setup(N, M, "zeroflux")
@@ -164,7 +188,7 @@ def test_step_fp32_one_step():
     a, b, c, d, e = (torch.tensor(v) for v in d32)
     h = pent.pent_factor(N, e, c, d, a, b)
     cd = _dev(c0, torch.float32)
-    pent.pent_step_batch(h, M, cd, 1, kind=0, bc=1, form=0, r=r, sigma=sigma)
+    pent.pent_step_batch(h, M, cd, 1, kind=0, bc=1, form=0, r=r, sigma=sigma, kernel=kernel)
     d64 = [v.astype(np.float64) for v in d32]
     ref = oracle.step_batch(oracle.factor(*d64), 0, 1, 0, float(np.float32(r)),
                             float(np.float32(sigma)), c0.astype(np.float32).astype(np.float64), 1)
