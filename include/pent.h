@@ -95,6 +95,11 @@ void pent_destroy(pent_handle* h);          /* NULL is allowed */
 int pent_factor_solve_batch(int N, int64_t M, const void* e, const void* c, const void* d,
                             const void* a, const void* b, const void* f, void* x,
                             pent_dtype dtype, int* info, void* stream);
+/* Same with a caller-owned workspace: device, 2*N*M elements (gamma_k, delta_k of every system),
+ * or NULL (the library then allocates and frees a stream-ordered temporary on every call). */
+int pent_factor_solve_batch_ws(int N, int64_t M, const void* e, const void* c, const void* d,
+                               const void* a, const void* b, const void* f, void* x,
+                               pent_dtype dtype, int* info, void* workspace, void* stream);
 int pent_factor_batch(int N, int64_t M, const void* e, const void* c, const void* d,
                       const void* a, const void* b, pent_dtype dtype, pent_handle** out,
                       int* info, void* stream);

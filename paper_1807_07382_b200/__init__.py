@@ -70,6 +70,7 @@ def lib() -> C.CDLL:
     L.pent_destroy.argtypes = [vp]
     L.pent_destroy.restype = None
     L.pent_factor_solve_batch.argtypes = [ci, i64, vp, vp, vp, vp, vp, vp, vp, ci, vp, vp]
+    L.pent_factor_solve_batch_ws.argtypes = [ci, i64, vp, vp, vp, vp, vp, vp, vp, ci, vp, vp, vp]
     L.pent_factor_batch.argtypes = [ci, i64, vp, vp, vp, vp, vp, ci, C.POINTER(vp), vp, vp]
     L.pent_solve_batch_multi.argtypes = [vp, vp, vp, vp]
     L.pent_step_batch.argtypes = [vp, C.POINTER(pent_step_params), i64, vp, vp, ci, vp]
@@ -175,9 +176,11 @@ def pent_solve_batch_host(h: Handle, M: int, f_host: torch.Tensor,
     return x_host
 
 
-def pent_factor_solve_batch(N: int, M: int, e, c, d, a, b, f, x=None, info=None, stream=None):
+def pent_factor_solve_batch(N: int, M: int, e, c, d, a, b, f, x=None, info=None, stream=None,
+                            workspace=None):
     """Per-system matrices, factor + solve fused.  All tensors (N, M) on CUDA.
-    Returns (x, info) with info int32[M]: 0 or first bad row + 1."""
+    workspace: optional CUDA tensor of 2*N*M elements.  Returns (x, info) with info int32[M]:
+    0 or first bad row + 1."""
     for t, n in zip((e, c, d, a, b, f), "ecdabf"):
         _batch(t, n)
         if t.shape != (N, M) or t.dtype != f.dtype:
@@ -186,9 +189,14 @@ def pent_factor_solve_batch(N: int, M: int, e, c, d, a, b, f, x=None, info=None,
         x = torch.empty_like(f)
     if info is None:
         info = torch.zeros(M, dtype=torch.int32, device=f.device)
-    _check(lib().pent_factor_solve_batch(N, M, e.data_ptr(), c.data_ptr(), d.data_ptr(),
-                                         a.data_ptr(), b.data_ptr(), f.data_ptr(), x.data_ptr(),
-                                         _dt(f), info.data_ptr(), _stream(stream)))
+    if workspace is not None and (not workspace.is_cuda or workspace.dtype != f.dtype or
+                                  workspace.numel() < 2 * N * M or not workspace.is_contiguous()):
+        raise ValueError("workspace: contiguous CUDA tensor of >= 2*N*M elements of f's dtype expected")
+    _check(lib().pent_factor_solve_batch_ws(N, M, e.data_ptr(), c.data_ptr(), d.data_ptr(),
+                                            a.data_ptr(), b.data_ptr(), f.data_ptr(), x.data_ptr(),
+                                            _dt(f), info.data_ptr(),
+                                            0 if workspace is None else workspace.data_ptr(),
+                                            _stream(stream)))
     return x, info
 
 

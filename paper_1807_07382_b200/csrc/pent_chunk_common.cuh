@@ -220,6 +220,21 @@ __device__ __forceinline__ void chunk_correct4(T (&out)[4], const T* v4, const T
         out[r] = fma(w[4 * r + 3], B1, fma(w[4 * r + 2], B0, fma(w[4 * r + 1], F1, fma(w[4 * r], F0, v4[r]))));
 }
 
+// Chunk states live in shared memory as [chunk][system] with the system index rotated by the chunk
+// index.  The sweep threads (consecutive lanes = consecutive systems of one chunk) and the scan
+// threads (consecutive lanes = consecutive chunks of one system) then both touch every bank group
+// equally: the plain [chunk][system] layout made the scan read with a 32-way bank conflict
+// (9.5 M conflicts per cfg3 launch, profiles/r01_solve_chunked_ncu_full.md).
+template <int S>
+__device__ __forceinline__ int state_slot(int chunk, int sys)
+{
+#ifdef PENT_AB_PLAIN_STATE
+    return chunk * S + sys;
+#else
+    return chunk * S + ((sys + chunk) & (S - 1));
+#endif
+}
+
 // Geometry of the chunk-state scan (stage 3): a group of Pw lanes scans one system, lane = chunk.
 struct ScanGeom {
     int P, Pw, lev_f, lev_b;
@@ -242,7 +257,7 @@ __device__ __forceinline__ void chunk_state_scan(const ScanGeom& g, const T* wta
 {
     using T2 = typename Pair<T>::type;
     const int P = g.P, Pw = g.Pw;
-    const int sl = ok ? q * S + sys : 0;
+    const int sl = ok ? state_slot<S>(q, sys) : 0;
     T y0 = 0, y1 = 0, z0 = 0, z1 = 0;
     if (ok) { T2 e = stE[sl]; y0 = e.x; y1 = e.y; T2 s = stS[sl]; z0 = s.x; z1 = s.y; }
 #pragma unroll

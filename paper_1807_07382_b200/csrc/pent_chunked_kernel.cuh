@@ -92,7 +92,7 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
     const T* blk = table + (size_t)(active ? p : 0) * BL;
     const T* wtab = table + (size_t)P * BL;          // W: TX | PF | PB | BLK | levels
     const int mybox = active ? (p * C) / prm.box_rows : 0;
-    const int slot = (active ? p : 0) * S + i;
+    const int slot = state_slot<S>(active ? p : 0, i);
     const int row0 = row_base + p * C;
     const bool rows_full = active && (row0 + C <= prm.N);
     uint32_t parity = 0;

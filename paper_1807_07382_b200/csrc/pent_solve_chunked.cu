@@ -268,7 +268,7 @@ ChunkPlan make_plan(const pent_handle* h, int64_t M, const void* f, int Q, int S
     pl.levels = h->lev_f[j] > h->lev_b[j] ? h->lev_f[j] : h->lev_b[j];
     if (pl.levels > lg) pl.levels = lg;
     // cluster: one scan round (the scan registers live across the cluster barriers)
-    pl.threads = Q > 1 ? pl.Pw * S : (pl.Pl * S + 31) / 32 * 32;
+    pl.threads = ((Q > 1 ? pl.Pw * S : pl.Pl * S) + 31) / 32 * 32;
     if (pl.threads > CHUNK_MAX_THREADS) return pl;
     const int rows = pl.Pl * C;
     pl.box_rows = rows < BOX_ROWS_MAX ? rows : BOX_ROWS_MAX;
@@ -301,19 +301,32 @@ bool encode_batch_map(CUtensorMap* tm, const void* base, int64_t M, int N, int S
                CU_TENSOR_MAP_SWIZZLE_NONE, PENT_L2_PROMOTION, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-// Default plan: the smallest cluster that holds the system on chip and the narrowest tile (more,
-// smaller tiles balance better over the 148 SMs and measured faster than wider row segments at
-// every shape tried: cfg2 34.2 us at S=16 vs 37.8 at S=32; cfg3 197 us at Q=1,S=16 vs 212-215 at
-// Q=2/4,S=32; cfg5a 469 us at Q=4,S=16 vs 548 at Q=8,S=32; profiles/r01_ab_tuning.md).
+// Default plan, from the shape sweeps in profiles/r01_ab_tuning.md (narrow tile S_n = 16 fp64 /
+// 32 fp32, wide tile S_w = 2 S_n = 256-byte row segments):
+//   * the whole system fits a CTA of <= 256 threads (cfg2-like, N <= 512): one CTA, narrow tile
+//     (more, smaller tiles balance better over 148 SMs: cfg2 31.0 us vs 33.6 wide, 32.8 Q=2 wide);
+//   * otherwise the smallest cluster with the WIDE tile if that is <= 4 CTAs (cfg3: 190.7 us at
+//     Q=2,S=32 vs 220 at Q=1,S=16; fp32 105.1 at Q=2,S=64 vs 111.5 at Q=1,S=32);
+//   * otherwise the smallest cluster with the narrow tile (cfg5a: 410.6 us at Q=4,S=16 vs 485 at
+//     Q=8,S=32: 8-CTA clusters leave SMs idle on the 16/18/20-SM GPCs).
 static ChunkPlan auto_plan(const pent_handle* h, int64_t M, const void* f)
 {
     if (!h || h->kind != 0) return ChunkPlan{};
-    const int cand[3] = {16, 32, 64};
-    for (int Q = 1; Q <= (1 << (PENT_NQ - 1)); Q *= 2)
-        for (int S : cand) {
-            ChunkPlan pl = make_plan(h, M, f, Q, S);
-            if (pl.ok) return pl;
-        }
+    const int Sn = h->dtype == PENT_F64 ? 16 : 32, Sw = 2 * Sn, QMAX = 1 << (PENT_NQ - 1);
+    ChunkPlan narrow1 = make_plan(h, M, f, 1, Sn);
+    if (narrow1.ok && narrow1.threads <= 256) return narrow1;
+    for (int Q = 1; Q <= 4; Q *= 2) {
+        ChunkPlan pl = make_plan(h, M, f, Q, Sw);
+        if (pl.ok) return pl;
+    }
+    for (int Q = 1; Q <= QMAX; Q *= 2) {
+        ChunkPlan pl = make_plan(h, M, f, Q, Sn);
+        if (pl.ok) return pl;
+    }
+    for (int Q = 1; Q <= QMAX; Q *= 2) {
+        ChunkPlan pl = make_plan(h, M, f, Q, Sw);
+        if (pl.ok) return pl;
+    }
     return ChunkPlan{};
 }
 

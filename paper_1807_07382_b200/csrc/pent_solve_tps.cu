@@ -225,13 +225,17 @@ solve_multi_kernel(int N, int64_t M, const T* __restrict__ ms, const T* f, T* x)
 template <typename T>
 static int factor_solve_impl(int N, int64_t M, const void* e, const void* c, const void* d,
                              const void* a, const void* b, const void* f, void* x, int* info,
-                             cudaStream_t s)
+                             void* workspace, cudaStream_t s)
 {
-    T* scratch = nullptr;
+    // gamma_k, delta_k of every system (needed again by the back substitution): 2*N*M elements,
+    // the caller's workspace or a stream-ordered temporary
+    T* scratch = (T*)workspace;
     size_t NM = (size_t)N * (size_t)M;
-    cudaError_t er = cudaMallocAsync((void**)&scratch, 2 * NM * sizeof(T), s);
-    if (er == cudaErrorMemoryAllocation) { cudaGetLastError(); return PENT_ERR_ALLOC; }
-    PENT_CUDA(er);
+    if (!scratch) {
+        cudaError_t er = cudaMallocAsync((void**)&scratch, 2 * NM * sizeof(T), s);
+        if (er == cudaErrorMemoryAllocation) { cudaGetLastError(); return PENT_ERR_ALLOC; }
+        PENT_CUDA(er);
+    }
     const int tb = PS_THREADS;
     unsigned nb = (unsigned)((M + tb - 1) / tb);
     factor_tps_kernel<T, 0><<<nb, tb, 0, s>>>(N, M, (const T*)a, (const T*)b, (const T*)c,
@@ -239,7 +243,7 @@ static int factor_solve_impl(int N, int64_t M, const void* e, const void* c, con
                                               scratch, scratch + NM, nullptr, nullptr, nullptr, info);
     count_launch();
     cudaError_t le = cudaGetLastError();
-    cudaFreeAsync(scratch, s);
+    if (!workspace) cudaFreeAsync(scratch, s);
     if (le != cudaSuccess) return cuda_fail(le);
     return PENT_OK;
 }
@@ -262,17 +266,25 @@ static int factor_batch_impl(pent_handle* h, const void* e, const void* c, const
 }
 }  // namespace pent
 
+extern "C" int pent_factor_solve_batch_ws(int N, int64_t M, const void* e, const void* c,
+                                          const void* d, const void* a, const void* b,
+                                          const void* f, void* x, pent_dtype dtype, int* info,
+                                          void* workspace, void* stream)
+{
+    if (N < 1 || M < 0 || !e || !c || !d || !a || !b || !f || !x) return PENT_ERR_ARG;
+    if (M == 0) return PENT_OK;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (dtype == PENT_F64) return pent::factor_solve_impl<double>(N, M, e, c, d, a, b, f, x, info, workspace, s);
+    if (dtype == PENT_F32) return pent::factor_solve_impl<float>(N, M, e, c, d, a, b, f, x, info, workspace, s);
+    return PENT_ERR_ARG;
+}
+
 extern "C" int pent_factor_solve_batch(int N, int64_t M, const void* e, const void* c,
                                        const void* d, const void* a, const void* b,
                                        const void* f, void* x, pent_dtype dtype, int* info,
                                        void* stream)
 {
-    if (N < 1 || M < 0 || !e || !c || !d || !a || !b || !f || !x) return PENT_ERR_ARG;
-    if (M == 0) return PENT_OK;
-    cudaStream_t s = (cudaStream_t)stream;
-    if (dtype == PENT_F64) return pent::factor_solve_impl<double>(N, M, e, c, d, a, b, f, x, info, s);
-    if (dtype == PENT_F32) return pent::factor_solve_impl<float>(N, M, e, c, d, a, b, f, x, info, s);
-    return PENT_ERR_ARG;
+    return pent_factor_solve_batch_ws(N, M, e, c, d, a, b, f, x, dtype, info, nullptr, stream);
 }
 
 extern "C" int pent_factor_batch(int N, int64_t M, const void* e, const void* c, const void* d,

@@ -74,7 +74,7 @@ step_chunked_kernel(const __grid_constant__ CUtensorMap tm, const StepChunkParam
 
     const T* blk = table + (size_t)(active ? p : 0) * BL;
     const T* wtab = table + (size_t)P * BL;
-    const int slot = (active ? p : 0) * S + i;
+    const int slot = state_slot<S>(active ? p : 0, i);
     const int row0 = p * C;
     T* cs = state + i;                                   // element (k, i) at cs[k*S]
     const int Pw = prm.Pw, G = 32 / Pw;
@@ -86,6 +86,7 @@ step_chunked_kernel(const __grid_constant__ CUtensorMap tm, const StepChunkParam
     const T dg_edge = (prm.bc == 1) ? (T)-1 : (T)-2;
     auto ldc = [&](int k) -> T { return ((unsigned)k < (unsigned)N) ? cs[(size_t)k * S] : (T)0; };
     auto Ld = [&](int k) -> T { return (k == 0 || k == N - 1) ? dg_edge : (T)-2; };
+    const bool interior = active && row0 >= 2 && row0 + C + 2 <= N - 1;
     uint32_t parity = 0;
 
     for (int64_t tile = blockIdx.x; tile < prm.ntiles; tile += gridDim.x) {
@@ -102,24 +103,46 @@ step_chunked_kernel(const __grid_constant__ CUtensorMap tm, const StepChunkParam
                 // ---- explicit right-hand side of rows row0 .. row0+C-1, in registers ----
                 if constexpr (KIND != 1) {
                     // u_k = w_k = c_k^3 - c_k (form 0) or q_k = r w_k - sigma (L c)_k (form 1), 0 outside 0..N-1
-                    auto U = [&](int k, T cl, T cc, T cr) -> T {
-                        if ((unsigned)k >= (unsigned)N) return (T)0;
-                        T w = cc * cc * cc - cc;
-                        if (!incr) return w;
-                        return fma(-sigma, cl + fma(Ld(k), cc, cr), r * w);
-                    };
-                    T cl = ldc(row0 - 2), cc = ldc(row0 - 1), cr = ldc(row0);
-                    T u_prev = U(row0 - 1, cl, cc, cr);
-                    cl = cc; cc = cr; cr = ldc(row0 + 1);
-                    T u_cur = U(row0, cl, cc, cr);
+                    if (interior) {
+                        // rows row0-2 .. row0+C+1 all exist and none is a boundary row: no range checks
+                        auto U = [&](T cl, T cc, T cr) -> T {
+                            T w = cc * cc * cc - cc;
+                            if (!incr) return w;
+                            return fma(-sigma, cl + fma((T)-2, cc, cr), r * w);
+                        };
+                        const T* cw = cs + (size_t)(row0 - 2) * S;
+                        T cl = cw[0], cc = cw[S], cr = cw[2 * S];
+                        T u_prev = U(cl, cc, cr);
+                        cl = cc; cc = cr; cr = cw[3 * S];
+                        T u_cur = U(cl, cc, cr);
 #pragma unroll
-                    for (int j = 0; j < C; ++j) {
-                        const int k = row0 + j;
-                        cl = cc; cc = cr; cr = ldc(k + 2);          // window centred on k+1; cl = c_k
-                        T u_next = U(k + 1, cl, cc, cr);
-                        T Lu = u_prev + fma(Ld(k), u_cur, u_next);
-                        v[j] = incr ? Lu : fma(r, Lu, cl);
-                        u_prev = u_cur; u_cur = u_next;
+                        for (int j = 0; j < C; ++j) {
+                            cl = cc; cc = cr; cr = cw[(j + 4) * S];     // window centred on row0+j+1; cl = c_{row0+j}
+                            T u_next = U(cl, cc, cr);
+                            T Lu = u_prev + fma((T)-2, u_cur, u_next);
+                            v[j] = incr ? Lu : fma(r, Lu, cl);
+                            u_prev = u_cur; u_cur = u_next;
+                        }
+                    } else {
+                        auto U = [&](int k, T cl, T cc, T cr) -> T {
+                            if ((unsigned)k >= (unsigned)N) return (T)0;
+                            T w = cc * cc * cc - cc;
+                            if (!incr) return w;
+                            return fma(-sigma, cl + fma(Ld(k), cc, cr), r * w);
+                        };
+                        T cl = ldc(row0 - 2), cc = ldc(row0 - 1), cr = ldc(row0);
+                        T u_prev = U(row0 - 1, cl, cc, cr);
+                        cl = cc; cc = cr; cr = ldc(row0 + 1);
+                        T u_cur = U(row0, cl, cc, cr);
+#pragma unroll
+                        for (int j = 0; j < C; ++j) {
+                            const int k = row0 + j;
+                            cl = cc; cc = cr; cr = ldc(k + 2);          // window centred on k+1; cl = c_k
+                            T u_next = U(k + 1, cl, cc, cr);
+                            T Lu = u_prev + fma(Ld(k), u_cur, u_next);
+                            v[j] = incr ? Lu : fma(r, Lu, cl);
+                            u_prev = u_cur; u_cur = u_next;
+                        }
                     }
                 } else {
                     T cm2 = ldc(row0 - 2), cm1 = ldc(row0 - 1), c0 = ldc(row0), cp1 = ldc(row0 + 1);

@@ -227,7 +227,7 @@ def test_chunked_shapes_nonsymmetric_fp64(N, M, Q, S):
 
 
 @pytest.mark.parametrize("N,M,Q,S", [(1024, 2048 + 64, 2, 64), (1024, 1024, 1, 32), (512, 640, 1, 64),
-                                     (4096, 512, 4, 32), (4096, 256, 8, 64), (3000, 128, 2, 32)])
+                                     (4096, 512, 4, 32), (4096, 256, 8, 64), (3000, 128, 4, 32)])
 def test_chunked_shapes_fp32(N, M, Q, S):
     _shape_case(N, M, Q, S, dtype=torch.float32, sigma=10.0)
 
@@ -245,7 +245,9 @@ def test_chunked_cluster_slowly_decaying_coupling(Q, S):
     ref = oracle.solve_batch(oracle.factor(*diags), f)
     # cond(A) ~ 1 + 16 sigma = 1.8e5: two correct fp64 solves differ by ~cond*eps (C-15)
     assert normwise(x, ref) <= 4.0 * (1.0 + 16.0 * sigma) * 2.0 ** -53
-    assert residual(diags, x, f) <= 1e-12
+    # backward-stable solve: residual ~ eps*||A||*||x||/||f|| with ||A|| = 1 + 16 sigma = 1.8e5; the
+    # oracle's own residual on this input is 1.5e-12, so 1e-12 is scaled here
+    assert residual(diags, x, f) <= max(1e-12, (1.0 + 16.0 * sigma) * 2.0 ** -53)
 
 
 def test_auto_choice_is_on_chip_for_every_config_shape():
