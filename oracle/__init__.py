@@ -20,7 +20,8 @@ from dataclasses import dataclass
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SRC = [os.path.join(_HERE, "pent_oracle.c"), os.path.join(_HERE, "pent_oracle_step.c")]
+_SRC = [os.path.join(_HERE, "pent_oracle.c"), os.path.join(_HERE, "pent_oracle_step.c"),
+        os.path.join(_HERE, "pent_oracle_periodic.c")]
 _LIB = os.path.join(_HERE, "libpent_oracle.so")
 _lib = None
 
@@ -43,6 +44,7 @@ def _load():
         _lib = C.CDLL(_LIB)
         _lib.pent_oracle_factor.restype = C.c_int
         _lib.pent_oracle_dense_ge.restype = C.c_int
+        _lib.pent_oracle_periodic_setup.restype = C.c_int
     return _lib
 
 
@@ -165,4 +167,54 @@ def step_batch(fac: Factors, kind: int, bc: int, form: int, r: float, sigma: flo
         C.c_double(r), C.c_double(sigma), *[_p(v) for v in fac.diags],
         _p(fac.eps), _p(fac.beta), _p(fac.alpha), _p(fac.gamma), _p(fac.delta),
         _p(Crows), C.c_int(nsteps), C.c_int(nthreads))
+    return np.ascontiguousarray(Crows.T)
+
+
+# ---- periodic (cyclic) pentadiagonal systems, PAPER.md:104-146 (pent_oracle_periodic.c) -----------
+@dataclass
+class PeriodicFactors:
+    """Set-up of the periodic reduction (Eqs. 8-12): factors of E, the stored
+    h^T E^{-1} (Y, shape (2, N-2)), the columns k (shape (2, N-2)) and the inverted 2x2 matrix."""
+    N: int
+    facE: np.ndarray
+    Y: np.ndarray
+    kk: np.ndarray
+    s2inv: np.ndarray
+    diags: tuple
+
+
+def factor_periodic(a, b, c, d, e) -> PeriodicFactors:
+    """Diagonals are length-N, row-indexed and wrapped cyclically (every entry is used)."""
+    a, b, c, d, e = (_f64(v) for v in (a, b, c, d, e))
+    N = c.shape[0]
+    if N < 6:
+        raise ValueError("periodic reduction needs N >= 6")
+    n = N - 2
+    facE, Y, kk, s2 = np.zeros(5 * n), np.zeros(2 * n), np.zeros(2 * n), np.zeros(4)
+    rc = _load().pent_oracle_periodic_setup(C.c_int(N), _p(a), _p(b), _p(c), _p(d), _p(e),
+                                            _p(facE), _p(Y), _p(kk), _p(s2))
+    if rc != 0:
+        raise SingularPivot(rc - 1)
+    return PeriodicFactors(N, facE, Y.reshape(2, n), kk.reshape(2, n), s2.reshape(2, 2),
+                           (a, b, c, d, e))
+
+
+def solve_periodic_batch(pf: PeriodicFactors, f_interleaved, nthreads: int = 1) -> np.ndarray:
+    """Interleaved (N, M) in, interleaved (N, M) out."""
+    F = to_rows(f_interleaved)
+    X = np.empty_like(F)
+    _load().pent_oracle_periodic_solve_rows(
+        C.c_int(pf.N), C.c_long(F.shape[0]), _p(pf.facE), _p(np.ascontiguousarray(pf.Y.ravel())),
+        _p(np.ascontiguousarray(pf.kk.ravel())), _p(np.ascontiguousarray(pf.s2inv.ravel())),
+        _p(F), _p(X), C.c_int(nthreads))
+    return np.ascontiguousarray(X.T)
+
+
+def step_periodic_batch(pf: PeriodicFactors, c_interleaved, nsteps: int, nthreads: int = 1) -> np.ndarray:
+    """nsteps Crank-Nicolson steps A c+ = (2I - A) c with the cyclic A (Eq. 6, 7c)."""
+    Crows = to_rows(c_interleaved)
+    _load().pent_oracle_periodic_step_rows(
+        C.c_int(pf.N), C.c_long(Crows.shape[0]), *[_p(v) for v in pf.diags], _p(pf.facE),
+        _p(np.ascontiguousarray(pf.Y.ravel())), _p(np.ascontiguousarray(pf.kk.ravel())),
+        _p(np.ascontiguousarray(pf.s2inv.ravel())), _p(Crows), C.c_int(nsteps), C.c_int(nthreads))
     return np.ascontiguousarray(Crows.T)

@@ -183,3 +183,35 @@ def random_diag_dominant(seed: int, N: int, M: int | None = None):
     if M is None:
         return tuple(v[:, 0].copy() for v in (a, b, c, d, e))
     return a, b, c, d, e
+
+
+# ----------------------------------------------------------------------------
+# periodic (cyclic) matrices, Eq. 7a-7b
+# ----------------------------------------------------------------------------
+def periodic_hyperdiffusion_diagonals(N: int, sigma_x: float):
+    """Constant diagonals of PAPER.md Eq. 7b: a = e = sigma_x, b = d = -4 sigma_x,
+    c = 1 + 6 sigma_x, as five length-N arrays (every entry used: the matrix is cyclic)."""
+    one = np.ones(N)
+    return sigma_x * one, -4.0 * sigma_x * one, (1.0 + 6.0 * sigma_x) * one, -4.0 * sigma_x * one, sigma_x * one
+
+
+def dense_from_periodic_diagonals(a, b, c, d, e) -> np.ndarray:
+    """Dense N x N cyclic matrix: a[k] = A[k][(k-2)%N], b[k] = A[k][(k-1)%N], c[k] = A[k][k],
+    d[k] = A[k][(k+1)%N], e[k] = A[k][(k+2)%N]  (Eq. 7a with row-indexed entries)."""
+    N = len(c)
+    A = np.zeros((N, N))
+    for k in range(N):
+        A[k, (k - 2) % N] += a[k]
+        A[k, (k - 1) % N] += b[k]
+        A[k, k] += c[k]
+        A[k, (k + 1) % N] += d[k]
+        A[k, (k + 2) % N] += e[k]
+    return A
+
+
+def random_periodic_diag_dominant(seed: int, N: int):
+    """Random NON-symmetric strictly diagonally dominant cyclic diagonals (all entries used)."""
+    a = uniform_pm1(seed, 21, N, 1)[:, 0]; b = uniform_pm1(seed, 22, N, 1)[:, 0]
+    d = uniform_pm1(seed, 23, N, 1)[:, 0]; e = uniform_pm1(seed, 24, N, 1)[:, 0]
+    c = 1.5 + np.abs(a) + np.abs(b) + np.abs(d) + np.abs(e)
+    return a, b, c, d, e
