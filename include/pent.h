@@ -85,6 +85,19 @@ int pent_solve_batch_host(const pent_handle* h, int64_t M, const void* f_host, v
 
 void pent_destroy(pent_handle* h);          /* NULL is allowed */
 
+/* ---- periodic (cyclic) shared A: the matrix of the paper's own benchmark ------
+ * a[k] = A[k][(k-2) mod N], b[k] = A[k][(k-1) mod N], c[k] = A[k][k], d[k] = A[k][(k+1) mod N],
+ * e[k] = A[k][(k+2) mod N]: ALL N entries of every array are read (Eq. 7a with row-indexed
+ * entries).  N >= 6.  Set-up = the reduction of Eqs. 8-12: factor the (N-2) x (N-2) block E,
+ * E^{-1} k and the inverted 2 x 2 Schur complement are computed once and kept in the handle.
+ * The handle is used with pent_solve_batch / _v / _host (f, x: N*M elements, interleaved) and with
+ * pent_step_batch (kind 1 only: A c+ = (2I - A) c with the cyclic A, Eq. 6 / 7c; `scratch` = N*M
+ * elements or NULL).  PENT_ERR_PIVOT: *bad_row = failing row of E, or N-2 if the 2 x 2 Schur
+ * complement is singular. */
+int pent_factor_periodic(int N, const void* e, const void* c, const void* d, const void* a, const void* b,
+                         pent_dtype dtype, pent_handle** out, int* bad_row);
+int pent_handle_periodic(const pent_handle* h);          /* 1 for a periodic handle, 0 otherwise, -1 for NULL */
+
 /* ---- per-system matrices ("cuPentBatchRewrite") ---------------------------------
  * e,c,d,a,b,f,x: device, N*M elements each, interleaved like f (diagonal entry k of system i at
  * k*M+i).  info: device int[M] or NULL; info[i] = 0, or (first bad row + 1) if system i met a

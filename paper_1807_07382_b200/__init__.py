@@ -64,6 +64,8 @@ def lib() -> C.CDLL:
     L = C.CDLL(path)
     vp, i64, ci = C.c_void_p, C.c_int64, C.c_int
     L.pent_factor.argtypes = [ci, vp, vp, vp, vp, vp, ci, C.POINTER(vp), C.POINTER(ci)]
+    L.pent_factor_periodic.argtypes = [ci, vp, vp, vp, vp, vp, ci, C.POINTER(vp), C.POINTER(ci)]
+    L.pent_handle_periodic.argtypes = [vp]
     L.pent_solve_batch.argtypes = [vp, i64, vp, vp, vp]
     L.pent_solve_batch_v.argtypes = [vp, i64, vp, vp, vp, ci]
     L.pent_solve_batch_host.argtypes = [vp, i64, vp, vp]
@@ -146,6 +148,26 @@ def pent_factor(N: int, e, c, d, a, b) -> Handle:
     out = C.c_void_p()
     bad = C.c_int(-1)
     rc = lib().pent_factor(N, *[t.data_ptr() for t in ts], dt, C.byref(out), C.byref(bad))
+    if rc == 2:
+        raise SingularPivot(bad.value)
+    _check(rc)
+    return Handle(out.value, N, ts[1].dtype)
+
+
+def pent_factor_periodic(N: int, e, c, d, a, b) -> Handle:
+    """Set-up of the periodic (cyclic) solve, Eqs. 7a-12: every entry of every length-N
+    diagonal is used (a[k] = A[k][(k-2) mod N], ...).  The handle works with pent_solve_batch,
+    pent_solve_batch_host and pent_step_batch(kind=1)."""
+    ts = [torch.as_tensor(v) for v in (e, c, d, a, b)]
+    dt = _dt(ts[1])
+    ts = [t.to(ts[1].dtype).contiguous() for t in ts]
+    if any(t.numel() != N for t in ts):
+        raise ValueError("each diagonal must have N entries")
+    if not torch.cuda.is_available():
+        raise RuntimeError("pent_factor_periodic needs a CUDA device (no CPU fallback)")
+    out = C.c_void_p()
+    bad = C.c_int(-1)
+    rc = lib().pent_factor_periodic(N, *[t.data_ptr() for t in ts], dt, C.byref(out), C.byref(bad))
     if rc == 2:
         raise SingularPivot(bad.value)
     _check(rc)

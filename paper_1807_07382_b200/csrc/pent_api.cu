@@ -10,6 +10,7 @@ extern "C" int pent_solve_batch_v(const pent_handle* h, int64_t M, const void* f
     if (!f || !x) return PENT_ERR_ARG;
     cudaStream_t s = (cudaStream_t)stream;
     if (kernel < 0 || (kernel >> 24) != 0) return PENT_ERR_ARG;
+    if (h->periodic) return pent::solve_periodic(h, M, f, x, s, kernel);
     const int Q = (kernel >> 8) & 0xff, S = (kernel >> 16) & 0xff;
     switch (kernel & 0xff) {
         case PENT_KERNEL_AUTO:
@@ -30,6 +31,7 @@ extern "C" int pent_solve_batch_v(const pent_handle* h, int64_t M, const void* f
 extern "C" int pent_solve_kernel_choice(const pent_handle* h, int64_t M)
 {
     if (!h || h->kind != 0) return -1;
+    if (h->periodic) return pent_solve_kernel_choice(h->inner, M);
     int Q = 0, S = 0;
     if (!pent::chunked_choice(h, M, &Q, &S)) return PENT_KERNEL_THREAD_PER_SYSTEM;
     return PENT_KERNEL_CHUNKED_CFG(Q, S);

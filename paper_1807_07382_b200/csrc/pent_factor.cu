@@ -161,7 +161,8 @@ extern "C" void pent_destroy(pent_handle* h)
     if (!h) return;
     cudaFree(h->diag); cudaFree(h->fac); cudaFree(h->fw); cudaFree(h->bw);
     for (int j = 0; j < PENT_NQ; ++j) cudaFree(h->cf[j]);
-    cudaFree(h->dg); cudaFree(h->ms);
+    cudaFree(h->dg); cudaFree(h->ms); cudaFree(h->Zt); cudaFree(h->dgp);
+    pent_destroy(h->inner);
     delete h;
 }
 
@@ -173,6 +174,7 @@ extern "C" int pent_handle_factors(const pent_handle* h, double* eps, double* be
                                    double* gamma, double* delta)
 {
     if (!h || h->kind != 0) return PENT_ERR_ARG;
+    if (h->periodic) return pent_handle_factors(h->inner, eps, beta, alpha, gamma, delta);   // factors of E
     double* dst[5] = {eps, beta, alpha, gamma, delta};
     for (int j = 0; j < 5; ++j)
         if (dst[j])
@@ -190,4 +192,6 @@ extern "C" int64_t pent_launch_count(int reset)
     return v;
 }
 
-extern "C" const char* pent_version(void) { return "pent 0.1 (sm_100a)"; }
+extern "C" int pent_handle_periodic(const pent_handle* h) { return h ? h->periodic : -1; }
+
+extern "C" const char* pent_version(void) { return "pent 0.2 (sm_100a)"; }

@@ -23,6 +23,15 @@ struct pent_handle {
     void* cf[PENT_NQ];
     int cfP[PENT_NQ];
     int lev_f[PENT_NQ], lev_b[PENT_NQ];   // Kogge-Stone levels the chunk-state scans need
+    // ---- periodic (cyclic) A, Eqs. 7a-12 (pent_periodic.cu): N is the full size, `inner`
+    // is the shared-A handle of the (N-2) x (N-2) block E, Zt = E^{-1} k as (N-2) x {z0, z1} in T,
+    // dgp = N x {a,b,c,d,e,0,0,0} in T with the wrapped entries kept, pc = the six entries of h
+    // (row N-2: cols 0, N-4, N-3; row N-1: cols 0, 1, N-3) and the inverted 2x2 Schur complement
+    int periodic;
+    pent_handle* inner;
+    void* Zt;
+    void* dgp;
+    double pc[10];
     // ---- per-system factors, device, interleaved, in T ----
     void* ms;            // 5*N*M: ia, en, bn, gamma, delta
 };
@@ -73,6 +82,8 @@ bool chunked_supported(const pent_handle* h, int64_t M, const void* f /* may be 
 bool step_chunked_supported(const pent_handle* h, int64_t M, const void* c /* may be null */);
 int launch_step_chunked(const pent_handle* h, const pent_step_params* p, int64_t M, void* c, int nsteps,
                         cudaStream_t s);
+int solve_periodic(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s, int kernel);
+int step_periodic(const pent_handle* h, int64_t M, void* c, void* scratch, int nsteps, cudaStream_t s);
 int chunked_choice(const pent_handle* h, int64_t M, int* Q, int* S);   // 1 and the default plan, or 0
 
 }  // namespace pent

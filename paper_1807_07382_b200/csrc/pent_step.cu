@@ -131,6 +131,10 @@ extern "C" int pent_step_batch_v(const pent_handle* h, const pent_step_params* p
         return PENT_ERR_ARG;
     if (M == 0 || nsteps == 0) return PENT_OK;
     cudaStream_t s = (cudaStream_t)stream;
+    if (h->periodic) {       // the paper's own loop: periodic hyperdiffusion, Eq. 6 / 7c
+        if (p->kind != 1 || kernel != PENT_KERNEL_AUTO) return PENT_ERR_ARG;
+        return pent::step_periodic(h, M, c_inout, scratch, nsteps, s);
+    }
     const bool on_chip = pent::step_chunked_supported(h, M, c_inout);
     if (kernel == PENT_KERNEL_CHUNKED && !on_chip) return PENT_ERR_ARG;
     if (kernel != PENT_KERNEL_THREAD_PER_SYSTEM && on_chip)
@@ -148,5 +152,6 @@ extern "C" int pent_step_batch(const pent_handle* h, const pent_step_params* p, 
 extern "C" int pent_step_kernel_choice(const pent_handle* h, int64_t M)
 {
     if (!h || h->kind != 0) return -1;
+    if (h->periodic) return PENT_KERNEL_THREAD_PER_SYSTEM;
     return pent::step_chunked_supported(h, M, nullptr) ? PENT_KERNEL_CHUNKED : PENT_KERNEL_THREAD_PER_SYSTEM;
 }

@@ -21,7 +21,8 @@ def test_header_declares_the_boundary():
     names = _declared_functions()
     for required in ("pent_factor", "pent_solve_batch", "pent_destroy", "pent_factor_solve_batch",
                      "pent_factor_batch", "pent_solve_batch_multi", "pent_step_batch",
-                     "pent_solve_batch_host"):
+                     "pent_solve_batch_host", "pent_factor_periodic", "pent_step_batch_v",
+                     "pent_factor_solve_batch_ws"):
         assert required in names
 
 

@@ -1,0 +1,128 @@
+"""GPU parity of the periodic (cyclic) pentadiagonal path (Eqs. 7a-12) and of the
+paper's own time loop (periodic hyperdiffusion, Crank-Nicolson) against
+the periodic oracle, through the C ABI."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import pent_inputs as pin
+
+pytestmark = pytest.mark.gpu
+
+
+def _pent():
+    import paper_1807_07382_b200 as pent
+    return pent
+
+
+def normwise(x, ref):
+    return float(np.max(np.max(np.abs(x - ref), axis=0) / np.max(np.abs(ref), axis=0)))
+
+
+def residual(diags, x, f):
+    A = pin.dense_from_periodic_diagonals(*diags)
+    r = A @ x.astype(np.float64) - f
+    return float(np.max(np.linalg.norm(r, axis=0) / np.linalg.norm(f, axis=0)))
+
+
+def _handle(diags, dtype=torch.float64):
+    pent = _pent()
+    a, b, c, d, e = (torch.tensor(v, dtype=dtype) for v in diags)
+    return pent.pent_factor_periodic(len(diags[2]), e, c, d, a, b)
+
+
+@pytest.mark.parametrize("kernel", [0, 1])
+@pytest.mark.parametrize("N,M", [(6, 4), (7, 33), (64, 256), (258, 130), (1026, 544), (1000, 37), (2050, 96)])
+def test_periodic_nonsymmetric_parity(kernel, N, M):
+    pent = _pent()
+    diags = pin.random_periodic_diag_dominant(300 + N, N)
+    f = pin.uniform_pm1(301 + N, 0, N, M)
+    h = _handle(diags)
+    x = pent.pent_solve_batch(h, M, torch.tensor(f, device="cuda"), kernel=kernel).cpu().numpy()
+    ref = oracle.solve_periodic_batch(oracle.factor_periodic(*diags), f)
+    assert normwise(x, ref) <= 1e-11
+    assert residual(diags, x, f) <= 1e-12
+
+
+def test_periodic_hyperdiffusion_matrix_full_batch_in_place_and_closed_form():
+    """The paper's matrix (Eq. 7b) at N=1024, sigma_x = dt/(2 dx^4) with dt=1e-8 (sigma_x = 5497.6):
+    oracle parity on every system, in place, plus the circulant closed form x = f/lambda_m."""
+    pent = _pent()
+    N, M = 1024, 4096
+    sx = 1e-8 / (2.0 * (1.0 / N) ** 4)
+    diags = pin.periodic_hyperdiffusion_diagonals(N, sx)
+    h = _handle(diags)
+    f = pin.uniform_pm1(31, 0, N, M)
+    fd = torch.tensor(f, device="cuda")
+    x = pent.pent_solve_batch(h, M, fd, fd).cpu().numpy()
+    ref = oracle.solve_periodic_batch(oracle.factor_periodic(*diags), f, nthreads=8)
+    # cond(A) = 1 + 16 sigma_x = 8.8e4: two correct fp64 solves differ by ~cond*eps
+    assert normwise(x, ref) <= max(1e-11, 4.0 * (1.0 + 16.0 * sx) * 2.0 ** -53)
+    j = np.arange(N)[:, None]
+    m = np.arange(0, 64)[None, :]
+    modes = np.cos(2 * np.pi * m * j / N)
+    lam = 1.0 + 16.0 * sx * np.sin(np.pi * np.arange(64) / N) ** 4
+    xm = pent.pent_solve_batch(h, 64, torch.tensor(modes, device="cuda")).cpu().numpy()
+    assert normwise(xm, modes / lam[None, :]) <= 4.0 * (1.0 + 16.0 * sx) * 2.0 ** -53
+
+
+def test_periodic_fp32_and_host_entry_point():
+    pent = _pent()
+    N, M = 514, 320
+    diags = [np.asarray(v, dtype=np.float32) for v in pin.periodic_hyperdiffusion_diagonals(N, 3.0)]
+    f = pin.uniform_pm1(41, 0, N, M).astype(np.float32)
+    h = _handle(diags, torch.float32)
+    x = pent.pent_solve_batch(h, M, torch.tensor(f, device="cuda")).cpu().numpy()
+    d64 = [v.astype(np.float64) for v in diags]
+    ref = oracle.solve_periodic_batch(oracle.factor_periodic(*d64), f.astype(np.float64))
+    assert normwise(x.astype(np.float64), ref) <= 2e-5
+    assert residual(d64, x, f.astype(np.float64)) <= 1e-5
+    xh = pent.pent_solve_batch_host(h, M, torch.tensor(f)).numpy()
+    assert np.array_equal(xh, x)
+
+
+def test_periodic_errors():
+    pent = _pent()
+    one = torch.ones(5, dtype=torch.float64)
+    with pytest.raises(pent.PentError):
+        pent.pent_factor_periodic(5, one, one, one, one, one)
+    N = 16
+    a, b, c, d, e = (v.copy() for v in pin.random_periodic_diag_dominant(7, N))
+    c[0] = 0.0
+    with pytest.raises(pent.SingularPivot) as ei:
+        _handle((a, b, c, d, e))
+    assert ei.value.row == 0
+    h = _handle(pin.random_periodic_diag_dominant(7, N))
+    assert pent.lib().pent_handle_periodic(h.ptr) == 1
+    cd = torch.zeros((N, 4), dtype=torch.float64, device="cuda")
+    with pytest.raises(pent.PentError):       # only the hyperdiffusion step is defined for a periodic handle
+        pent.pent_step_batch(h, 4, cd, 1, kind=0)
+
+
+def test_paper_time_loop_decay_and_convergence_order():
+    """gamma = D = L = 1, C(x,0) = cos(2 pi 2 x), T = 1e-4; batch of identical
+    systems as in the paper's benchmark.  dt = 1e-7 here (1000 steps per N; the
+    temporal error of Crank-Nicolson stays far below the spatial one): the GPU trajectory matches
+    the oracle's and the error against Eq. 14 falls like N^-2."""
+    pent = _pent()
+    T, dt, n = 1e-4, 1e-7, 2
+    steps = int(round(T / dt))
+    Ns, errs = [32, 64, 128, 256], []
+    for N in Ns:
+        dx = 1.0 / N
+        diags = pin.periodic_hyperdiffusion_diagonals(N, dt / (2.0 * dx ** 4))
+        h = _handle(diags)
+        xg = np.arange(1, N + 1) * dx
+        M = 64
+        c0 = np.repeat(np.cos(2 * np.pi * n * xg)[:, None], M, axis=1)
+        cd = torch.tensor(c0, device="cuda")
+        pent.pent_step_batch(h, M, cd, steps, kind=1)
+        c = cd.cpu().numpy()
+        ref = oracle.step_periodic_batch(oracle.factor_periodic(*diags), c0[:, :2], steps)
+        assert normwise(c[:, :2], ref) <= 1e-9
+        assert np.max(np.abs(c - c[:, :1])) == 0.0            # identical systems stay identical
+        exact = np.exp(-((2 * np.pi * n) ** 4) * T) * np.cos(2 * np.pi * n * xg)
+        errs.append(np.sqrt(np.mean((c[:, 0] - exact) ** 2)))
+    slope = np.polyfit(np.log(Ns), np.log(errs), 1)[0]
+    assert abs(slope + 2.0) <= 0.05
