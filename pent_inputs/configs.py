@@ -39,6 +39,10 @@ WORKLOADS = {
     "cfg4":  Workload("cfg4", 1024, 8192, SIGMA_CH, "zeroflux", 4, "ch_state",
                       "Cahn-Hilliard, 1000 steps"),
     "cfg5a": Workload("cfg5a", 4096, 32768, 0.5, "dirichlet", 5, "uniform"),
+    # the paper's own benchmark shape: a batch of identical periodic
+    # hyperdiffusion systems, Crank-Nicolson, N=1024, batch 8192, dt=1e-8 (sigma_x = dt/(2 dx^4))
+    "paper_hd": Workload("paper_hd", 1024, 8192, 1e-8 / (2.0 * (1.0 / 1024) ** 4), "periodic", 7, "cos_mode",
+                         "periodic hyperdiffusion, identical systems, 250 steps"),
     "cfg5b": Workload("cfg5b", 1024, 16384, float("nan"), "dirichlet", 6, "uniform",
                       "per-system sigma_i ~ U[0.1,10]"),
 }
