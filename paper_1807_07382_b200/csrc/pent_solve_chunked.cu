@@ -250,7 +250,7 @@ static bool s_instantiated(bool f64, int S, bool cluster)
     return f64 ? (S == 16 || S == 32) : (S == 32 || S == 64);
 }
 
-ChunkPlan make_plan(const pent_handle* h, int64_t M, const void* f, int Q, int S)
+ChunkPlan make_plan(const pent_handle* h, int64_t M, const void* f, int Q, int S, bool any_S)
 {
     ChunkPlan pl;
     if (!h || h->kind != 0) return pl;
@@ -259,7 +259,8 @@ ChunkPlan make_plan(const pent_handle* h, int64_t M, const void* f, int Q, int S
     int j = 0;
     while ((1 << j) < Q) ++j;
     if ((1 << j) != Q || j >= PENT_NQ || !h->cf[j] || h->cfP[j] < 1) return pl;
-    if (!s_instantiated(f64, S, Q > 1)) return pl;
+    if (!any_S && !s_instantiated(f64, S, Q > 1)) return pl;
+    if (S < 4 || (S & (S - 1)) != 0) return pl;
     const int C = f64 ? ChunkCfg<double>::C : ChunkCfg<float>::C;
     pl.j = j; pl.Q = Q; pl.S = S; pl.Pl = h->cfP[j];
     while (pl.Pw < pl.Pl) pl.Pw *= 2;

@@ -30,7 +30,7 @@ struct StepChunkParams {
     int64_t M, ntiles;
     const T* table;
     const T* dg;          // N x {a,b,c,d,e,0,0,0} (kind 1)
-    int nsteps, bc, form;
+    int nsteps, bc;
     T r, sigma;
 };
 
@@ -40,7 +40,20 @@ __device__ __forceinline__ void tma_store_2d(const CUtensorMap* tm, int c0, int 
                  ::"l"((uint64_t)tm), "r"(c0), "r"(c1), "r"(smem_u32(src)) : "memory");
 }
 
-template <typename T, int S, int KIND>
+// Barrier of one thread group of a CTA (named barrier 1+g); the whole CTA when there is one group.
+template <int NG>
+__device__ __forceinline__ void group_sync(int g, int nthreads)
+{
+    if constexpr (NG == 1) __syncthreads();
+    else asm volatile("bar.sync %0, %1;" ::"r"(1 + g), "r"(nthreads) : "memory");
+}
+
+// NG independent thread groups per CTA, each taking its OWN tile of S systems through the steps
+// (own state buffer, own chunk states, own named barrier); they share the coefficient table.  The
+// phases of a step alternate between FP64-throughput-bound (right-hand side), latency-bound
+// (sweeps, scan) and shared-memory-bound (write-back) work; two groups out of phase fill the pipes
+// that one group in lockstep leaves idle.
+template <typename T, int S, int KIND, int NG>
 __global__ void __launch_bounds__(CHUNK_MAX_THREADS, 1)
 step_chunked_kernel(const __grid_constant__ CUtensorMap tm, const StepChunkParams<T> prm)
 {
@@ -48,25 +61,29 @@ step_chunked_kernel(const __grid_constant__ CUtensorMap tm, const StepChunkParam
     using T2 = typename Pair<T>::type;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int P = prm.P, N = prm.N;
-    T* state = reinterpret_cast<T*>(smem_raw);                       // [rows][S], the tile's c
-    T* table = state + (size_t)prm.nbox * prm.box_rows * S;
-    T2* stE = reinterpret_cast<T2*>(reinterpret_cast<unsigned char*>(table) + prm.table_bytes);
+    const int TG = blockDim.x / NG, grp_id = threadIdx.x / TG, tid = threadIdx.x % TG;
+    const size_t state_elems = (size_t)prm.nbox * prm.box_rows * S;
+    T* state = reinterpret_cast<T*>(smem_raw) + grp_id * state_elems;          // [rows][S], this group's tile
+    T* table = reinterpret_cast<T*>(smem_raw) + NG * state_elems;
+    T2* stE = reinterpret_cast<T2*>(reinterpret_cast<unsigned char*>(table) + prm.table_bytes) +
+              (size_t)grp_id * 2 * S * P;
     T2* stS = stE + (size_t)S * P;
-    uint64_t* bars = reinterpret_cast<uint64_t*>(stS + (size_t)S * P);   // [0] table, [1] state
+    uint64_t* bars = reinterpret_cast<uint64_t*>(
+        reinterpret_cast<T2*>(reinterpret_cast<unsigned char*>(table) + prm.table_bytes) + (size_t)NG * 2 * S * P);
+    uint64_t* bar_state = &bars[1 + grp_id];                                   // [0] table, [1+g] state of group g
 
-    const int tid = threadIdx.x, i = tid % S, p = tid / S;
+    const int i = tid % S, p = tid / S;
     const bool active = p < P;
-    const int lane = tid & 31, warp = tid >> 5, nwarps = blockDim.x >> 5;
+    const int lane = tid & 31, warp = tid >> 5, nwarps = TG >> 5;
     const uint32_t box_bytes = (uint32_t)(prm.box_rows * S * sizeof(T));
 
-    if (tid == 0) {
-        mbar_init(&bars[0], 1);
-        mbar_init(&bars[1], 1);
+    if (threadIdx.x == 0) {
+        for (int b = 0; b <= NG; ++b) mbar_init(&bars[b], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
     __syncthreads();
-    if (tid == 0) {
+    if (threadIdx.x == 0) {
         mbar_expect_tx(&bars[0], prm.table_bytes);
         bulk_load_1d(table, prm.table, prm.table_bytes, &bars[0]);
     }
@@ -86,16 +103,19 @@ step_chunked_kernel(const __grid_constant__ CUtensorMap tm, const StepChunkParam
     const T dg_edge = (prm.bc == 1) ? (T)-1 : (T)-2;
     auto ldc = [&](int k) -> T { return ((unsigned)k < (unsigned)N) ? cs[(size_t)k * S] : (T)0; };
     auto Ld = [&](int k) -> T { return (k == 0 || k == N - 1) ? dg_edge : (T)-2; };
-    const bool interior = active && row0 >= 2 && row0 + C + 2 <= N - 1;
+    // Warp-uniform choice: a warp that holds one boundary chunk (S=16: two chunks per warp) takes the
+    // general path with ALL its lanes instead of executing both paths one after the other; that warp
+    // is the straggler every block barrier waits for.
+    const bool interior = __all_sync(0xffffffffu, active && row0 >= 2 && row0 + C + 2 <= N - 1);
     uint32_t parity = 0;
 
-    for (int64_t tile = blockIdx.x; tile < prm.ntiles; tile += gridDim.x) {
+    for (int64_t tile = (int64_t)blockIdx.x * NG + grp_id; tile < prm.ntiles; tile += (int64_t)gridDim.x * NG) {
         if (tid == 0) {
-            mbar_expect_tx(&bars[1], box_bytes * prm.nbox);
+            mbar_expect_tx(bar_state, box_bytes * prm.nbox);
             for (int b = 0; b < prm.nbox; ++b)
-                tma_load_2d(state + (size_t)b * prm.box_rows * S, &tm, (int)(tile * S), b * prm.box_rows, &bars[1]);
+                tma_load_2d(state + (size_t)b * prm.box_rows * S, &tm, (int)(tile * S), b * prm.box_rows, bar_state);
         }
-        mbar_wait(&bars[1], parity);
+        mbar_wait(bar_state, parity);
 
         for (int step = 0; step < prm.nsteps; ++step) {
             T v[C];
@@ -170,7 +190,7 @@ step_chunked_kernel(const __grid_constant__ CUtensorMap tm, const StepChunkParam
                 stE[slot] = e;
                 stS[slot] = s;
             }
-            __syncthreads();
+            group_sync<NG>(grp_id, TG);
             if (P > 1) {
                 for (int rr = 0; rr < rounds; ++rr) {
                     const int sys = (rr * nwarps + warp) * G + grp;
@@ -178,7 +198,7 @@ step_chunked_kernel(const __grid_constant__ CUtensorMap tm, const StepChunkParam
                                                   nullptr, nullptr, bars, 0u, 0u, 0u);
                 }
             }
-            __syncthreads();
+            group_sync<NG>(grp_id, TG);
             if (active) {
                 T F0 = 0, F1 = 0, B0 = 0, B1 = 0;
                 if (P > 1) { T2 fo = stE[slot]; F0 = fo.x; F1 = fo.y; T2 bo = stS[slot]; B0 = bo.x; B1 = bo.y; }
@@ -194,27 +214,64 @@ step_chunked_kernel(const __grid_constant__ CUtensorMap tm, const StepChunkParam
                     }
                 }
             }
-            __syncthreads();       // the next step's windows read rows written by other threads
+            group_sync<NG>(grp_id, TG);       // the next step's windows read rows written by other threads
         }
         // ---- tile back to HBM: generic-proxy writes -> async proxy, then one TMA store per box ----
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        __syncthreads();
+        group_sync<NG>(grp_id, TG);
         if (tid == 0) {
             for (int b = 0; b < prm.nbox; ++b)
                 tma_store_2d(&tm, (int)(tile * S), b * prm.box_rows, state + (size_t)b * prm.box_rows * S);
             asm volatile("cp.async.bulk.commit_group;" ::: "memory");
             asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // shared memory may be overwritten
         }
-        __syncthreads();
+        group_sync<NG>(grp_id, TG);
         parity ^= 1;
     }
     if (tid == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }
 
-template <typename T, int S, int KIND>
-static int launch_step_inst(const pent_handle* h, const ChunkPlan& pl, const pent_step_params* p, int64_t M,
+// Shape of a step launch: NG groups of TG threads, each with a tile of S systems.
+struct StepPlan {
+    bool ok = false;
+    ChunkPlan pl;
+    int S = 0, NG = 1, TG = 0;
+    size_t smem = 0;
+};
+
+static StepPlan step_plan(const pent_handle* h, int64_t M, const void* c, int S, int NG)
+{
+    StepPlan sp;
+    if (!h || h->kind != 0 || h->periodic) return sp;
+    const size_t esz = h->dtype == PENT_F64 ? 8 : 4;
+    sp.pl = make_plan(h, M, c, 1, S, /*any_S=*/true);
+    if (!sp.pl.ok) return sp;
+    sp.S = S; sp.NG = NG; sp.TG = sp.pl.threads;
+    if (sp.TG * NG > CHUNK_MAX_THREADS) return sp;
+    sp.smem = (size_t)NG * ((size_t)sp.pl.nbox * sp.pl.box_rows * S * esz + (size_t)4 * sp.pl.Pl * S * esz) +
+              sp.pl.table_bytes + (size_t)(1 + NG) * sizeof(uint64_t);
+    sp.ok = sp.smem <= SMEM_LIMIT;
+    return sp;
+}
+
+// Default, measured on cfg4 (1000 steps, same box, profiles/r01_ab_tuning.md): fp64 one group of 16
+// systems 29.15 us per step against 30.8 for two groups of 8 (narrower tiles double the coefficient
+// broadcasts per system and the shared-memory pipe is the busiest unit); fp32 two groups of 16
+// systems 20.2 us against 22.2 for one group of 32.
+static StepPlan step_auto_plan(const pent_handle* h, int64_t M, const void* c)
+{
+    if (!h) return StepPlan{};
+    if (h->dtype == PENT_F64) return step_plan(h, M, c, 16, 1);
+    StepPlan two = step_plan(h, M, c, 16, 2);
+    if (two.ok) return two;
+    return step_plan(h, M, c, 32, 1);
+}
+
+template <typename T, int S, int KIND, int NG>
+static int launch_step_inst(const pent_handle* h, const StepPlan& sp, const pent_step_params* p, int64_t M,
                             void* c, int nsteps, cudaStream_t s)
 {
+    const ChunkPlan& pl = sp.pl;
     StepChunkParams<T> prm;
     prm.N = h->N; prm.P = pl.Pl; prm.Pw = pl.Pw; prm.M = M;
     int lg = 0;
@@ -227,55 +284,55 @@ static int launch_step_inst(const pent_handle* h, const ChunkPlan& pl, const pen
     prm.table = (const T*)h->cf[0];
     prm.table_bytes = (uint32_t)pl.table_bytes;
     prm.dg = (const T*)h->dg;
-    prm.nsteps = nsteps; prm.bc = p->bc; prm.form = p->form;
+    prm.nsteps = nsteps; prm.bc = p->bc;
     prm.r = (T)p->r; prm.sigma = (T)p->sigma;
     CUtensorMap tm;
     if (!encode_batch_map(&tm, c, M, h->N, S, prm.box_rows, sizeof(T) == 8)) {
         g_last_cuda_error = (int)cudaErrorInvalidValue;
         return PENT_ERR_CUDA;
     }
-    auto kern = step_chunked_kernel<T, S, KIND>;
+    auto kern = step_chunked_kernel<T, S, KIND, NG>;
     static thread_local size_t smem_set = 0;
-    if (pl.smem > smem_set) {
-        PENT_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
-        smem_set = pl.smem;
+    if (sp.smem > smem_set) {
+        PENT_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sp.smem));
+        smem_set = sp.smem;
     }
+    const int threads = sp.TG * NG;
     int dev = 0, nsm = 0, occ = 0;
     PENT_CUDA(cudaGetDevice(&dev));
     PENT_CUDA(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
-    PENT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, pl.threads, pl.smem));
+    PENT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, threads, sp.smem));
     if (occ < 1) return PENT_ERR_ARG;
     int64_t grid = (int64_t)nsm * occ;
-    if (grid > prm.ntiles) grid = prm.ntiles;
-    kern<<<(unsigned)grid, pl.threads, pl.smem, s>>>(tm, prm);
+    const int64_t need = (prm.ntiles + NG - 1) / NG;
+    if (grid > need) grid = need;
+    kern<<<(unsigned)grid, threads, sp.smem, s>>>(tm, prm);
     count_launch();
     PENT_LAUNCH_CHECK();
     return PENT_OK;
 }
 
-static ChunkPlan step_plan(const pent_handle* h, int64_t M, const void* c)
-{
-    return make_plan(h, M, c, 1, h->dtype == PENT_F64 ? 16 : 32);
-}
-
 bool step_chunked_supported(const pent_handle* h, int64_t M, const void* c)
 {
-    return h && h->kind == 0 && step_plan(h, M, c).ok;
+    return h && h->kind == 0 && step_auto_plan(h, M, c).ok;
+}
+
+template <typename T, int S, int NG>
+static int launch_step_kind(const pent_handle* h, const StepPlan& sp, const pent_step_params* p, int64_t M,
+                            void* c, int nsteps, cudaStream_t s)
+{
+    if (p->kind == 1) return launch_step_inst<T, S, 1, NG>(h, sp, p, M, c, nsteps, s);
+    if (p->form == 1) return launch_step_inst<T, S, 2, NG>(h, sp, p, M, c, nsteps, s);
+    return launch_step_inst<T, S, 0, NG>(h, sp, p, M, c, nsteps, s);
 }
 
 int launch_step_chunked(const pent_handle* h, const pent_step_params* p, int64_t M, void* c, int nsteps,
                         cudaStream_t s)
 {
-    const ChunkPlan pl = step_plan(h, M, c);
-    if (!pl.ok) return PENT_ERR_ARG;
-    const int kind = p->kind == 1 ? 1 : (p->form == 1 ? 2 : 0);
-    if (h->dtype == PENT_F64) {
-        if (kind == 0) return launch_step_inst<double, 16, 0>(h, pl, p, M, c, nsteps, s);
-        if (kind == 1) return launch_step_inst<double, 16, 1>(h, pl, p, M, c, nsteps, s);
-        return launch_step_inst<double, 16, 2>(h, pl, p, M, c, nsteps, s);
-    }
-    if (kind == 0) return launch_step_inst<float, 32, 0>(h, pl, p, M, c, nsteps, s);
-    if (kind == 1) return launch_step_inst<float, 32, 1>(h, pl, p, M, c, nsteps, s);
-    return launch_step_inst<float, 32, 2>(h, pl, p, M, c, nsteps, s);
+    const StepPlan sp = step_auto_plan(h, M, c);
+    if (!sp.ok) return PENT_ERR_ARG;
+    if (h->dtype == PENT_F64) return launch_step_kind<double, 16, 1>(h, sp, p, M, c, nsteps, s);
+    if (sp.NG == 2) return launch_step_kind<float, 16, 2>(h, sp, p, M, c, nsteps, s);
+    return launch_step_kind<float, 32, 1>(h, sp, p, M, c, nsteps, s);
 }
 }  // namespace pent
