@@ -169,6 +169,140 @@ factor_tps_kernel(int N, int64_t M, const T* __restrict__ a, const T* __restrict
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Fused per-system factor + solve with a cp.async ring (default for pent_factor_solve_batch).
+// One thread per system still (the factor recurrence is serial and nonlinear in the matrix
+// entries), but M is the only parallelism (cfg5b: 16384 threads on 148 SMs), so every thread must
+// keep ~0.5-1 KB of loads in flight on its own: each thread streams ITS column of the six input
+// arrays through a private slice of a shared-memory ring with 8-byte cp.async copies, RING_STAGES-1
+// stages ahead of the recurrence.  No block barrier: a thread only reads what it copied itself.
+// Forward: stage = RING_ROWS rows x {a,b,c,d,e,f}; backward: stage = 2*RING_ROWS rows x {gamma,
+// delta, g} (same stage size).  cfg5b: 418 us with register load-ahead -> see profiles/r01_ab_tuning.md.
+// ---------------------------------------------------------------------------------------------
+constexpr int RING_ROWS = 4, RING_STAGES = 6, RING_SLOTS = 6 * RING_ROWS;   // values per thread and stage
+
+__device__ __forceinline__ void cp_async_elem(double* dst, const double* src)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_elem(float* dst, const float* src)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N_>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N_) : "memory"); }
+
+template <typename T>
+__global__ void __launch_bounds__(PS_THREADS)
+factor_solve_ring_kernel(int N, int64_t M, const T* __restrict__ a, const T* __restrict__ b,
+                         const T* __restrict__ c, const T* __restrict__ d, const T* __restrict__ e,
+                         const T* f, T* x, T* gam, T* del, int* __restrict__ info)
+{
+    constexpr int R = RING_ROWS, NST = RING_STAGES, TB = PS_THREADS;
+    extern __shared__ __align__(16) unsigned char ring_raw[];
+    T* ring = reinterpret_cast<T*>(ring_raw);           // [NST][RING_SLOTS][TB]
+    int64_t i = (int64_t)blockIdx.x * TB + threadIdx.x;
+    if (i >= M) i = M - 1;                                // tail threads redo the last system (no divergent exits)
+    const bool writer = ((int64_t)blockIdx.x * TB + threadIdx.x) < M;
+    T* mine = ring + threadIdx.x;
+    auto slot = [&](int stage, int v) -> T* { return mine + (size_t)(stage * RING_SLOTS + v) * TB; };
+
+    // ---------------- forward: factor rows and sweep in the same loop ----------------
+    const int nblk = (N + R - 1) / R;
+    auto issue_fwd = [&](int blk) {
+        if (blk < nblk) {
+            const int st = blk % NST;
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const int k = blk * R + r;
+                if (k < N) {
+                    const int64_t o = (int64_t)k * M + i;
+                    cp_async_elem(slot(st, 0 * R + r), a + o);
+                    cp_async_elem(slot(st, 1 * R + r), b + o);
+                    cp_async_elem(slot(st, 2 * R + r), c + o);
+                    cp_async_elem(slot(st, 3 * R + r), d + o);
+                    cp_async_elem(slot(st, 4 * R + r), e + o);
+                    cp_async_elem(slot(st, 5 * R + r), f + o);
+                }
+            }
+        }
+        cp_async_commit();
+    };
+    for (int blk = 0; blk < NST - 1; ++blk) issue_fwd(blk);
+    T ga1 = 0, ga2 = 0, de1 = 0, de2 = 0, g1 = 0, g2 = 0;
+    int bad = 0;
+    for (int blk = 0; blk < nblk; ++blk) {
+        issue_fwd(blk + NST - 1);
+        cp_async_wait<NST - 1>();
+        const int st = blk % NST;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int k = blk * R + r;
+            if (k < N) {
+                const int64_t o = (int64_t)k * M + i;
+                const T ak = (k >= 2) ? *slot(st, 0 * R + r) : (T)0;
+                const T bk = (k >= 1) ? *slot(st, 1 * R + r) : (T)0;
+                const T ck = *slot(st, 2 * R + r);
+                const T dk = (k + 1 < N) ? *slot(st, 3 * R + r) : (T)0;
+                const T ek = (k + 2 < N) ? *slot(st, 4 * R + r) : (T)0;
+                const T fk = *slot(st, 5 * R + r);
+                T be = fma(-ak, ga2, bk);
+                T al = fma(-be, ga1, fma(-ak, de2, ck));
+                if (bad == 0 && (al == (T)0 || !isfinite(al))) bad = k + 1;
+                T inv = (T)1 / al;
+                T ga = fma(-be, de1, dk) * inv;
+                T de = ek * inv;
+                T g = fma(-be, g1, fma(-ak, g2, fk)) * inv;
+                if (writer) { gam[o] = ga; del[o] = de; x[o] = g; }
+                g2 = g1; g1 = g;
+                ga2 = ga1; ga1 = ga; de2 = de1; de1 = de;
+            }
+        }
+    }
+    if (info && writer) info[i] = bad;
+    cp_async_wait<0>();
+    __threadfence();              // this thread's gamma, delta, g are in L2 before it copies them back
+    __syncthreads();              // tail threads share a column with a writer of the same block
+
+    // ---------------- backward: x_k = g_k - gamma_k x_{k+1} - delta_k x_{k+2} ----------------
+    constexpr int RB = 2 * R;
+    const int nblk_b = (N + RB - 1) / RB;
+    auto issue_bwd = [&](int blk) {
+        if (blk < nblk_b) {
+            const int st = blk % NST;
+#pragma unroll
+            for (int r = 0; r < RB; ++r) {
+                const int k = N - 1 - (blk * RB + r);
+                if (k >= 0) {
+                    const int64_t o = (int64_t)k * M + i;
+                    cp_async_elem(slot(st, 0 * RB + r), gam + o);
+                    cp_async_elem(slot(st, 1 * RB + r), del + o);
+                    cp_async_elem(slot(st, 2 * RB + r), x + o);
+                }
+            }
+        }
+        cp_async_commit();
+    };
+    for (int blk = 0; blk < NST - 1; ++blk) issue_bwd(blk);
+    T x1 = 0, x2 = 0;
+    for (int blk = 0; blk < nblk_b; ++blk) {
+        issue_bwd(blk + NST - 1);
+        cp_async_wait<NST - 1>();
+        const int st = blk % NST;
+#pragma unroll
+        for (int r = 0; r < RB; ++r) {
+            const int k = N - 1 - (blk * RB + r);
+            if (k >= 0) {
+                T xv = fma(-*slot(st, 1 * RB + r), x2, fma(-*slot(st, 0 * RB + r), x1, *slot(st, 2 * RB + r)));
+                if (writer) __stcs(x + (int64_t)k * M + i, xv);
+                x2 = x1; x1 = xv;
+            }
+        }
+    }
+    cp_async_wait<0>();
+}
+
 // Solve with stored per-system factors (layout ms: ia, en, bn, gamma, delta, each N*M).
 template <typename T>
 __global__ void __launch_bounds__(PS_THREADS)
@@ -238,9 +372,20 @@ static int factor_solve_impl(int N, int64_t M, const void* e, const void* c, con
     }
     const int tb = PS_THREADS;
     unsigned nb = (unsigned)((M + tb - 1) / tb);
+#ifdef PENT_AB_NO_RING
     factor_tps_kernel<T, 0><<<nb, tb, 0, s>>>(N, M, (const T*)a, (const T*)b, (const T*)c,
                                               (const T*)d, (const T*)e, (const T*)f, (T*)x,
                                               scratch, scratch + NM, nullptr, nullptr, nullptr, info);
+#else
+    const size_t smem = (size_t)RING_STAGES * RING_SLOTS * PS_THREADS * sizeof(T);
+    static thread_local bool attr_set = false;
+    if (!attr_set) {
+        PENT_CUDA(cudaFuncSetAttribute(factor_solve_ring_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_set = true;
+    }
+    factor_solve_ring_kernel<T><<<nb, tb, smem, s>>>(N, M, (const T*)a, (const T*)b, (const T*)c, (const T*)d,
+                                                     (const T*)e, (const T*)f, (T*)x, scratch, scratch + NM, info);
+#endif
     count_launch();
     cudaError_t le = cudaGetLastError();
     if (!workspace) cudaFreeAsync(scratch, s);
