@@ -228,7 +228,8 @@ def run_ours(args):
         f = make_rhs(w, M=M)
         f = f[0] if isinstance(f, tuple) else f
     a, b, c, d, e = (torch.tensor(v, dtype=tdt) for v in diags)
-    h = pent.pent_factor(N, e, c, d, a, b)                 # once, outside the timed region
+    periodic = w.bc == "periodic"
+    h = (pent.pent_factor_periodic if periodic else pent.pent_factor)(N, e, c, d, a, b)   # once, outside the timed region
     f_host = torch.tensor(f, dtype=tdt).pin_memory()
     fd = f_host.cuda()
     xd = torch.empty_like(fd)
@@ -279,7 +280,11 @@ def run_ours(args):
             dist.destroy_process_group()
         return
     peak, peak_src = measured_peak()
-    if args.kernel == 0:
+    if periodic:
+        fused = args.kernel == 0 and bool(pent.lib().pent_periodic_fused(h.ptr, M))
+        ch = {**pent.kernel_choice(h, M), "kernel": "solve_chunked_kernel" if fused else
+              "solve_chunked_kernel + periodic_tail_kernel + periodic_update_kernel"}
+    elif args.kernel == 0:
         ch = pent.kernel_choice(h, M)
     elif (args.kernel & 0xff) == 2:
         ch = {"kernel": "solve_chunked_kernel", "Q": (args.kernel >> 8) & 0xff, "S": (args.kernel >> 16) & 0xff}
@@ -309,7 +314,7 @@ def run_ours(args):
     }
     if e2e is not None:
         line["e2e"] = e2e
-    if not args.no_cpu_baseline and world == 1:
+    if not args.no_cpu_baseline and world == 1 and not periodic:
         line["cpu_baseline"] = cpu_baseline(w, diags, 16384)
     print(json.dumps(line))
     if world > 1:

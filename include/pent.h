@@ -96,6 +96,12 @@ void pent_destroy(pent_handle* h);          /* NULL is allowed */
  * complement is singular. */
 int pent_factor_periodic(int N, const void* e, const void* c, const void* d, const void* a, const void* b,
                          pent_dtype dtype, pent_handle** out, int* bad_row);
+/* pent_solve_batch on a periodic handle runs ONE fused kernel (solve of E, 2 x 2 tail, rank-2 update:
+ * 2 passes over the batch) when the shape allows it, else three kernels (4 passes).
+ * pent_periodic_fused: 1 / 0 = which of the two PENT_KERNEL_AUTO runs for M systems; -1 = not periodic.
+ * pent_solve_batch_v(kernel = PENT_KERNEL_CHUNKED or PENT_KERNEL_THREAD_PER_SYSTEM) forces the
+ * three-kernel path with that inner solve kernel. */
+int pent_periodic_fused(const pent_handle* h, int64_t M);
 int pent_handle_periodic(const pent_handle* h);          /* 1 for a periodic handle, 0 otherwise, -1 for NULL */
 
 /* ---- per-system matrices ("cuPentBatchRewrite") ---------------------------------

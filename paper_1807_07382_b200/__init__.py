@@ -66,6 +66,7 @@ def lib() -> C.CDLL:
     L.pent_factor.argtypes = [ci, vp, vp, vp, vp, vp, ci, C.POINTER(vp), C.POINTER(ci)]
     L.pent_factor_periodic.argtypes = [ci, vp, vp, vp, vp, vp, ci, C.POINTER(vp), C.POINTER(ci)]
     L.pent_handle_periodic.argtypes = [vp]
+    L.pent_periodic_fused.argtypes = [vp, i64]
     L.pent_solve_batch.argtypes = [vp, i64, vp, vp, vp]
     L.pent_solve_batch_v.argtypes = [vp, i64, vp, vp, vp, ci]
     L.pent_solve_batch_host.argtypes = [vp, i64, vp, vp]

@@ -10,7 +10,7 @@ PKG = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
 LIB = os.path.join(PKG, "libpent.so")
-SOURCES = ["pent_factor.cu", "pent_solve_tps.cu", "pent_solve_chunked.cu", "pent_step.cu", "pent_step_chunked.cu", "pent_periodic.cu",
+SOURCES = ["pent_factor.cu", "pent_solve_tps.cu", "pent_solve_chunked.cu", "pent_step.cu", "pent_step_chunked.cu", "pent_periodic.cu", "pent_solve_chunked_periodic.cu",
            "pent_api.cu"]
 
 
@@ -30,20 +30,38 @@ def needs_build() -> bool:
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
+    """Compile every .cu to an object file (in parallel) and link libpent.so."""
     if not force and not needs_build():
         return LIB
-    cmd = [nvcc_path(), "-O3", "-std=c++17", "-lineinfo",
-           "-gencode", "arch=compute_100a,code=sm_100a",
-           "-Xcompiler", "-fPIC", "-shared",
-           "-I", os.path.join(ROOT, "include"), "-I", CSRC,
-           "-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES] + os.environ.get("PENT_NVCC_FLAGS", "").split()
+    from concurrent.futures import ThreadPoolExecutor
+    objdir = os.path.join(PKG, "build")
+    os.makedirs(objdir, exist_ok=True)
+    common = [nvcc_path(), "-O3", "-std=c++17", "-lineinfo",
+              "-gencode", "arch=compute_100a,code=sm_100a",
+              "-Xcompiler", "-fPIC",
+              "-I", os.path.join(ROOT, "include"), "-I", CSRC] + os.environ.get("PENT_NVCC_FLAGS", "").split()
     if verbose:
-        cmd.insert(1, "-Xptxas=-v")
-    r = subprocess.run(cmd, capture_output=True, text=True)
-    if verbose or r.returncode != 0:
-        sys.stderr.write(r.stdout + r.stderr)
-    if r.returncode != 0:
+        common.insert(1, "-Xptxas=-v")
+
+    def compile_one(src):
+        obj = os.path.join(objdir, src.replace(".cu", ".o"))
+        r = subprocess.run(common + ["-c", os.path.join(CSRC, src), "-o", obj], capture_output=True, text=True)
+        return src, obj, r
+
+    with ThreadPoolExecutor(max_workers=min(8, len(SOURCES))) as ex:
+        results = list(ex.map(compile_one, SOURCES))
+    failed = False
+    for src, _, r in results:
+        if verbose or r.returncode != 0:
+            sys.stderr.write(f"---- {src}\n" + r.stdout + r.stderr)
+        failed |= r.returncode != 0
+    if failed:
         raise RuntimeError("nvcc failed building libpent.so")
+    r = subprocess.run([nvcc_path(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB] +
+                       [obj for _, obj, _ in results], capture_output=True, text=True)
+    if r.returncode != 0:
+        sys.stderr.write(r.stdout + r.stderr)
+        raise RuntimeError("nvcc failed linking libpent.so")
     return LIB
 
 

@@ -96,6 +96,19 @@ __device__ __forceinline__ void bulk_load_1d(void* dst, const void* src, uint32_
         ::"r"(smem_u32(dst)), "l"((uint64_t)src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
+// per-thread asynchronous copies global -> shared (LDGSTS), 8 or 4 bytes
+__device__ __forceinline__ void cp_async_elem(double* dst, const double* src)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_elem(float* dst, const float* src)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N_>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N_) : "memory"); }
+
 // n consecutive T values from shared memory with 16-byte loads (n*sizeof(T) % 16 == 0)
 template <typename T, int n>
 __device__ __forceinline__ void lds_vec(T (&dst)[n], const T* src)
@@ -243,21 +256,50 @@ struct ScanGeom {
 
 constexpr int BAR_F = 1 + 2 * MAX_BOXES, BAR_B = 2 + 2 * MAX_BOXES, NUM_BARS = 3 + 2 * MAX_BOXES;
 
+// Periodic (cyclic) systems, Eqs. 8-12, fused into the scan: the kernel solves y = E^{-1} f^
+// for the (N-2) x (N-2) block E (n = N-2 rows) and needs, per system,
+//     t = S2^{-1} [ (f_n, f_{n+1}) - h^T y ],     h^T y = six entries: y_0, y_1, y_{n-2}, y_{n-1}
+// before it can store x^ = y - Z t.  (y_0, y_1) is the true state B of the first chunk;
+// y_{n-2}, y_{n-1} are rows (pa, ja), (pb, jb) of cluster rank ra (the last rank with real rows, whose
+// state entering from the right is zero, so its values are final right after its own scan).
+template <typename T>
+struct PeriodicParams {                   // kernel parameter (constant bank)
+    int ra, pa, ja, pb, jb;               // location of rows n-2 and n-1: cluster rank, local chunk, row in chunk
+    T h00, h0a, h0b, h10, h11, h1a;       // h (Eq. 9): row N-2 of A at cols 0, N-4, N-3; row N-1 at cols 0, 1, N-3
+    T i00, i01, i10, i11;                 // inverse of the 2 x 2 Schur complement (Eq. 12)
+    const T* zt;                          // Z = E^{-1} k as [Q][P*C] x {z0, z1}: rank r's rows at zt + r * 2*P*C
+    const T* f;                           // the caller's right-hand side (rows n, n+1 are read directly)
+};
+template <typename T>
+struct PeriodicCtx {
+    const PeriodicParams<T>* pp;
+    T* ypub;                              // smem [S][2]: x^ of rows n-2 / n-1 (written by the sweep threads of rank ra)
+    typename Pair<T>::type *yab, *ftail, *stT;   // smem [S]: (y_{n-2}, y_{n-1}); (f_n, f_{n+1}); t
+    const T* table;                       // smem chunk blocks (correction rows of chunks pa, pb)
+    T* x; int64_t M, col0; int n;         // tail rows go to x[n*M + col], x[(n+1)*M + col]
+};
+
 // stage 3 for one (system, chunk q) lane: Kogge-Stone over chunks with warp shuffles.
 //   F_q = E~_q + TPhi_q F_{q-1};  B_q = (S^_q + TX_q F_{q-1}) + TPsi_q B_{q+1}
 // In:  stE[sl] = E~_q, stS[sl] = S^_q.  Out: stE[sl] = F_{q-1}, stS[sl] = B_{q+1} (what thread (sys, q)
 // needs).  CLUSTER: the block aggregates travel between the CTAs of the cluster (rank = this
 // CTA's position along k, Q CTAs) through aggF/aggB and the two aggregate mbarriers.
-template <typename T, int S, bool CLUSTER>
+// PER: also computes t of the periodic reduction (PeriodicCtx) into per.stT[sys] and stores the two
+// tail rows of x; in a cluster every rank then receives every rank's backward aggregate (not only
+// the later ranks') plus (y_{n-2}, y_{n-1}) from rank ra, all under the same mbarrier phase.
+template <typename T, int S, bool CLUSTER, bool PER = false>
 __device__ __forceinline__ void chunk_state_scan(const ScanGeom& g, const T* wtab, typename Pair<T>::type* stE,
                                                  typename Pair<T>::type* stS, int sys, int q, bool ok,
                                                  int rank, int Q, typename Pair<T>::type* aggF,
                                                  typename Pair<T>::type* aggB, uint64_t* bars,
-                                                 uint32_t agg_bytes_f, uint32_t agg_bytes_b, uint32_t parity)
+                                                 uint32_t agg_bytes_f, uint32_t agg_bytes_b, uint32_t parity,
+                                                 const PeriodicCtx<T>* per = nullptr)
 {
     using T2 = typename Pair<T>::type;
+    constexpr int C = ChunkCfg<T>::C, BL = chunk_block_len<T>();
     const int P = g.P, Pw = g.Pw;
     const int sl = ok ? state_slot<S>(q, sys) : 0;
+    const int sy = ok ? sys : 0;
     T y0 = 0, y1 = 0, z0 = 0, z1 = 0;
     if (ok) { T2 e = stE[sl]; y0 = e.x; y1 = e.y; T2 s = stS[sl]; z0 = s.x; z1 = s.y; }
 #pragma unroll
@@ -276,7 +318,7 @@ __device__ __forceinline__ void chunk_state_scan(const ScanGeom& g, const T* wta
             for (int rr = rank + 1; rr < Q; ++rr) st_async_pair(&aggF[rank * S + sys], &bars[BAR_F], rr, y0, y1);
         if (agg_bytes_f) mbar_wait(&bars[BAR_F], parity);
         for (int rr = 0; rr < rank; ++rr) {        // F_in(rr+1) = aggF[rr] + TPhiBlock(rr) F_in(rr)
-            T2 a = aggF[rr * S + (ok ? sys : 0)];
+            T2 a = aggF[rr * S + sy];
             T n0 = a.x, n1 = a.y;
             mat2_acc(n0, n1, wtab + 12 * P + 4 * rr, 1, fin0, fin1);
             fin0 = n0; fin1 = n1;
@@ -294,24 +336,78 @@ __device__ __forceinline__ void chunk_state_scan(const ScanGeom& g, const T* wta
             if (ok && q + d <= P - 1) mat2_acc(z0, z1, wtab + g.woff[l] + 4 * n + q, n, u0, u1);
         }
     }
+    T ya = 0, yb = 0;                     // y_{n-2}, y_{n-1}
+    if constexpr (PER) {
+        // rank ra: nothing enters its block from the right, so z is the true B of its chunks already
+        T bq0 = shfl_down_t(z0, 1, Pw), bq1 = shfl_down_t(z1, 1, Pw);
+        if (q >= P - 1) { bq0 = 0; bq1 = 0; }
+        if (ok && rank == per->pp->ra) {
+            if (q == per->pp->pa) {
+                const T* cr = per->table + (size_t)per->pp->pa * BL + 5 * C + 4 * per->pp->ja;
+                ya = fma(cr[3], bq1, fma(cr[2], bq0, fma(cr[1], f1, fma(cr[0], f0, per->ypub[2 * sys]))));
+            }
+            if (q == per->pp->pb) {
+                const T* cr = per->table + (size_t)per->pp->pb * BL + 5 * C + 4 * per->pp->jb;
+                yb = fma(cr[3], bq1, fma(cr[2], bq0, fma(cr[1], f1, fma(cr[0], f0, per->ypub[2 * sys + 1]))));
+            }
+        }
+        ya = __shfl_sync(0xffffffffu, ya, per->pp->pa, Pw);
+        yb = __shfl_sync(0xffffffffu, yb, per->pp->pb, Pw);
+    }
     T bin0 = 0, bin1 = 0;                 // B of the first chunk of the NEXT block
+    T B00 = 0, B01 = 0;                   // PER: (y_0, y_1) = true B of the system's first chunk
     if constexpr (CLUSTER) {
-        if (ok && q == 0)
-            for (int rr = 0; rr < rank; ++rr) st_async_pair(&aggB[rank * S + sys], &bars[BAR_B], rr, z0, z1);
+        if (ok && q == 0) {
+            if constexpr (PER) {
+                for (int rr = 0; rr < Q; ++rr) st_async_pair(&aggB[rank * S + sys], &bars[BAR_B], rr, z0, z1);
+                if (rank == per->pp->ra)
+                    for (int rr = 0; rr < Q; ++rr) st_async_pair(&per->yab[sys], &bars[BAR_B], rr, ya, yb);
+            } else {
+                for (int rr = 0; rr < rank; ++rr) st_async_pair(&aggB[rank * S + sys], &bars[BAR_B], rr, z0, z1);
+            }
+        }
         if (agg_bytes_b) mbar_wait(&bars[BAR_B], parity);
         for (int rr = Q - 1; rr > rank; --rr) {   // B_in(rr-1) = aggB[rr] + TPsiBlock(rr) B_in(rr)
-            T2 a = aggB[rr * S + (ok ? sys : 0)];
+            T2 a = aggB[rr * S + sy];
             T n0 = a.x, n1 = a.y;
             mat2_acc(n0, n1, wtab + 12 * P + 32 + 4 * rr, 1, bin0, bin1);
             bin0 = n0; bin1 = n1;
         }
         if (ok && rank < Q - 1) mat2_acc(z0, z1, wtab + 8 * P + q, P, bin0, bin1);   // PB_q B_in
+        if constexpr (PER) {
+            for (int rr = Q - 1; rr >= 0; --rr) {  // continue the chain down to the first block: B of chunk 0
+                T2 a = aggB[rr * S + sy];
+                T n0 = a.x, n1 = a.y;
+                mat2_acc(n0, n1, wtab + 12 * P + 32 + 4 * rr, 1, B00, B01);
+                B00 = n0; B01 = n1;
+            }
+            T2 yy = per->yab[sy];
+            ya = yy.x; yb = yy.y;
+        }
+    } else if constexpr (PER) {
+        B00 = __shfl_sync(0xffffffffu, z0, 0, Pw);
+        B01 = __shfl_sync(0xffffffffu, z1, 0, Pw);
     }
     T b0 = shfl_down_t(z0, 1, Pw), b1 = shfl_down_t(z1, 1, Pw);  // B_{q+1}
     if (q >= P - 1) { b0 = bin0; b1 = bin1; }
     if (ok) {
         T2 fo; fo.x = f0; fo.y = f1; stE[sl] = fo;
         T2 bo; bo.x = b0; bo.y = b1; stS[sl] = bo;
+    }
+    if constexpr (PER) {
+        if (ok && q == 0) {
+            const T2 ft = per->ftail[sys];
+            const T r0 = ft.x - fma(per->pp->h0b, yb, fma(per->pp->h0a, ya, per->pp->h00 * B00));
+            const T r1 = ft.y - fma(per->pp->h1a, yb, fma(per->pp->h11, B01, per->pp->h10 * B00));
+            T2 t;
+            t.x = fma(per->pp->i01, r1, per->pp->i00 * r0);
+            t.y = fma(per->pp->i11, r1, per->pp->i10 * r0);
+            per->stT[sys] = t;
+            if (rank == 0 && per->col0 + sys < per->M) {
+                per->x[(int64_t)per->n * per->M + per->col0 + sys] = t.x;
+                per->x[(int64_t)(per->n + 1) * per->M + per->col0 + sys] = t.y;
+            }
+        }
     }
 }
 
@@ -326,6 +422,7 @@ struct ChunkPlan {
 };
 // any_S: accept tile widths the SOLVE kernel is not instantiated for (the step kernel has its own)
 ChunkPlan make_plan(const pent_handle* h, int64_t M, const void* f, int Q, int S, bool any_S = false);
+ChunkPlan chunk_auto_plan(const pent_handle* h, int64_t M, const void* f);   // what PENT_KERNEL_AUTO runs
 // rank-2 tensor map {M, N} of an interleaved batch with box {S, box_rows}; false on failure
 bool encode_batch_map(CUtensorMap* tm, const void* base, int64_t M, int N, int S, int box_rows, bool f64);
 

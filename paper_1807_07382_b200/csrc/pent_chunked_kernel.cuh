@@ -1,6 +1,9 @@
 // pent_chunked_kernel.cuh -- device code of the chunked on-chip solve (included by
 // pent_solve_chunked.cu inside namespace pent; see the algorithm notes at the top of that file).
 #pragma once
+#ifndef PENT_AB_NO_Z
+#define PENT_AB_NO_Z 0
+#endif
 
 // Measured A/B switches (cfg3 fp64 on B200, profiles/r01_ab_tuning.md).  Defaults = fastest:
 //   store policy of the x stream: plain write-back st.global (201 us) beat .cs (212), .cg (210), .wt (211)
@@ -35,9 +38,11 @@ struct ChunkParams {
     T* x;
 };
 
-template <typename T, int S, bool CLUSTER>
+// PER = true: the periodic (cyclic) solve fused into the kernel, see PeriodicCtx in pent_chunk_common.cuh.
+template <typename T, int S, bool CLUSTER, bool PER>
 __global__ void __launch_bounds__(CHUNK_MAX_THREADS, 1)
-solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T> prm)
+solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T> prm,
+                     const __grid_constant__ PeriodicParams<T> pp)
 {
     constexpr int C = ChunkCfg<T>::C, BL = chunk_block_len<T>();
     using T2 = typename Pair<T>::type;
@@ -51,7 +56,13 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
     // cluster: block aggregates of every rank, [Q][S] each (written by the owning rank through DSMEM)
     T2* aggF = stS + (size_t)S * P;
     T2* aggB = aggF + (CLUSTER ? (size_t)prm.Q * S : 0);
-    uint64_t* bars = reinterpret_cast<uint64_t*>(aggB + (CLUSTER ? (size_t)prm.Q * S : 0));
+    // periodic: this CTA's rows of Z, then x^ of rows n-2/n-1, (y_{n-2}, y_{n-1}), (f_n, f_{n+1}), t  ([S] each)
+    T2* zs = aggB + (CLUSTER ? (size_t)prm.Q * S : 0);
+    T2* ypub = zs + (PER ? (size_t)P * C : 0);
+    T2* yab = ypub + (PER ? S : 0);
+    T2* ftail2 = yab + (PER ? S : 0);             // [2][S]
+    T2* stT = ftail2 + (PER ? 2 * S : 0);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(stT + (PER ? S : 0));
 
     const int tid = threadIdx.x, i = tid % S, p = tid / S;
     const bool active = p < P;
@@ -74,8 +85,10 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
     __syncthreads();
     int64_t tile = first;
     if (tid == 0) {
-        mbar_expect_tx(&bars[0], prm.table_bytes);
+        const uint32_t z_bytes = PER ? (uint32_t)(P * C * sizeof(T2)) : 0u;
+        mbar_expect_tx(&bars[0], prm.table_bytes + z_bytes);
         bulk_load_1d(table, prm.table + (size_t)rank * prm.table_stride, prm.table_bytes, &bars[0]);
+        if constexpr (PER) bulk_load_1d(zs, pp.zt + (size_t)rank * 2 * P * C, z_bytes, &bars[0]);
         if (tile < prm.ntiles)
             for (int b = 0; b < prm.nbox; ++b) {
                 mbar_expect_tx(&bars[1 + b], box_bytes);
@@ -86,7 +99,9 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
     // every CTA of the cluster is resident, with its mbarriers initialised, before any DSMEM store
     if constexpr (CLUSTER) cluster_sync_all();
     const uint32_t agg_bytes_f = (uint32_t)(rank * S * sizeof(T2));                 // from the earlier ranks
-    const uint32_t agg_bytes_b = (uint32_t)((prm.Q - 1 - rank) * S * sizeof(T2));   // from the later ranks
+    // from the later ranks; periodic: from EVERY rank (itself included) plus (y_{n-2}, y_{n-1}) from rank ra
+    const uint32_t agg_bytes_b = PER ? (uint32_t)((prm.Q + 1) * S * sizeof(T2))
+                                     : (uint32_t)((prm.Q - 1 - rank) * S * sizeof(T2));
     mbar_wait(&bars[0], 0);
 
     const T* blk = table + (size_t)(active ? p : 0) * BL;
@@ -103,9 +118,33 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
     const ScanGeom geom{P, Pw, prm.lev_f, prm.lev_b, prm.woff};
     const int rounds = (S + nwarps * G - 1) / (nwarps * G);     // host guarantees 1 when CLUSTER
 
+    int tcount = 0;
+    if constexpr (PER) {
+        if (tid < S) {
+            if (tile < prm.ntiles && tile * S + tid < prm.M) {
+                T* dst = reinterpret_cast<T*>(ftail2 + tid);
+                cp_async_elem(dst, pp.f + (int64_t)prm.N * prm.M + tile * S + tid);
+                cp_async_elem(dst + 1, pp.f + (int64_t)(prm.N + 1) * prm.M + tile * S + tid);
+            }
+            cp_async_commit();
+        }
+    }
     for (; tile < prm.ntiles; tile += stride) {
         const int64_t next_tile = tile + stride;
         T v[C];
+        // periodic: (f_n, f_{n+1}) of system tid travel global -> shared by cp.async, one tile ahead
+        // (double-buffered), so no thread waits for them and they hold no registers
+        T2* ftail = ftail2 + (tcount & 1) * S;
+        if constexpr (PER) {
+            if (tid < S) {
+                if (next_tile < prm.ntiles && next_tile * S + tid < prm.M) {
+                    T* dst = reinterpret_cast<T*>(ftail2 + ((tcount + 1) & 1) * S + tid);
+                    cp_async_elem(dst, pp.f + (int64_t)prm.N * prm.M + next_tile * S + tid);
+                    cp_async_elem(dst + 1, pp.f + (int64_t)(prm.N + 1) * prm.M + next_tile * S + tid);
+                }
+                cp_async_commit();
+            }
+        }
         if (active) {
             // ---- tile data: landing buffer -> registers ----
             mbar_wait(&bars[1 + mybox], parity);
@@ -138,15 +177,36 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
             chunk_local_sweeps<T>(v, blk, e, s);
             stE[slot] = e;
             stS[slot] = s;
+            if constexpr (PER) {
+                // x^ of rows n-2 and n-1 (compile-time register indices: predicated scan of the chunk)
+                if (rank == pp.ra && (p == pp.pa || p == pp.pb)) {
+                    T va = 0, vb = 0;
+#pragma unroll
+                    for (int j = 0; j < C; ++j) {
+                        if (j == pp.ja) va = v[j];
+                        if (j == pp.jb) vb = v[j];
+                    }
+                    if (p == pp.pa) reinterpret_cast<T*>(ypub)[2 * i] = va;
+                    if (p == pp.pb) reinterpret_cast<T*>(ypub)[2 * i + 1] = vb;
+                }
+            }
+        }
+        if constexpr (PER) {
+            if (tid < S) cp_async_wait<1>();      // this tile's pair has landed (the next tile's may be in flight)
         }
         __syncthreads();       // states published
 
         // ---- 3. chunk-state scans (slot (q, sys) receives F_{q-1} and B_{q+1}) ----
-        if (CLUSTER || P > 1) {
+        if (CLUSTER || PER || P > 1) {
+            PeriodicCtx<T> per;
+            if constexpr (PER) {
+                per.pp = &pp; per.ypub = reinterpret_cast<T*>(ypub); per.yab = yab; per.ftail = ftail; per.stT = stT;
+                per.table = table; per.x = prm.x; per.M = prm.M; per.n = prm.N; per.col0 = tile * S;
+            }
             for (int r = 0; r < rounds; ++r) {
                 const int sys = (r * nwarps + warp) * G + grp;
-                chunk_state_scan<T, S, CLUSTER>(geom, wtab, stE, stS, sys, q, (sys < S) && (q < P), rank, prm.Q,
-                                                aggF, aggB, bars, agg_bytes_f, agg_bytes_b, parity);
+                chunk_state_scan<T, S, CLUSTER, PER>(geom, wtab, stE, stS, sys, q, (sys < S) && (q < P), rank,
+                                                     prm.Q, aggF, aggB, bars, agg_bytes_f, agg_bytes_b, parity, &per);
             }
         }
         __syncthreads();
@@ -154,14 +214,21 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
         // ---- 4. correction and store ----
         if (active) {
             T F0 = 0, F1 = 0, B0 = 0, B1 = 0;
-            if (CLUSTER || P > 1) { T2 fo = stE[slot]; F0 = fo.x; F1 = fo.y; T2 bo = stS[slot]; B0 = bo.x; B1 = bo.y; }
+            if (CLUSTER || PER || P > 1) { T2 fo = stE[slot]; F0 = fo.x; F1 = fo.y; T2 bo = stS[slot]; B0 = bo.x; B1 = bo.y; }
             const int64_t col = tile * S + i;
             T* xo = prm.x + (int64_t)row0 * prm.M + col;
+            T t0 = 0, t1 = 0;         // periodic: x^ = y - Z t
+            if constexpr (PER) { T2 t = stT[i]; t0 = t.x; t1 = t.y; }
+            const T2* zr = zs + (size_t)(active ? p : 0) * C;
             if (rows_full && (tile + 1) * S <= prm.M) {
 #pragma unroll
                 for (int jg = 0; jg < C / 4; ++jg) {
                     T xv[4];
                     chunk_correct4<T>(xv, &v[4 * jg], blk, jg, F0, F1, B0, B1);
+                    if constexpr (PER && !PENT_AB_NO_Z) {
+#pragma unroll
+                        for (int r = 0; r < 4; ++r) { T2 z = zr[4 * jg + r]; xv[r] = fma(-z.y, t1, fma(-z.x, t0, xv[r])); }
+                    }
 #pragma unroll
                     for (int r = 0; r < 4; ++r) { PENT_STORE(xo, xv[r]); xo += prm.M; }
                 }
@@ -171,6 +238,10 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
                 for (int jg = 0; jg < C / 4; ++jg) {
                     T xv[4];
                     chunk_correct4<T>(xv, &v[4 * jg], blk, jg, F0, F1, B0, B1);
+                    if constexpr (PER && !PENT_AB_NO_Z) {
+#pragma unroll
+                        for (int r = 0; r < 4; ++r) { T2 z = zr[4 * jg + r]; xv[r] = fma(-z.y, t1, fma(-z.x, t0, xv[r])); }
+                    }
 #pragma unroll
                     for (int r = 0; r < 4; ++r) {
                         if (4 * jg + r < nrows) PENT_STORE(xo, xv[r]);
@@ -180,6 +251,7 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
             }
         }
         parity ^= 1;
+        ++tcount;
     }
     if constexpr (CLUSTER) cluster_sync_all();   // no CTA leaves while a peer may still address its shared memory
 }

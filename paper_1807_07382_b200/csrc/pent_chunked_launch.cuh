@@ -1,0 +1,84 @@
+// pent_chunked_launch.cuh -- host launcher of solve_chunked_kernel, shared by pent_solve_chunked.cu
+// (PER = false) and pent_solve_chunked_periodic.cu (PER = true) so that the two sets of template
+// instantiations compile in parallel.
+#pragma once
+#include "pent_chunk_common.cuh"
+
+namespace pent {
+#include "pent_chunked_kernel.cuh"
+
+// extra dynamic shared memory of the periodic kernel: this CTA's rows of Z and four [S] pair arrays
+template <typename T>
+inline size_t periodic_extra_smem(const ChunkPlan& pl)
+{
+    return ((size_t)pl.Pl * ChunkCfg<T>::C + 5 * (size_t)pl.S) * 2 * sizeof(T);
+}
+
+template <typename T, int S, bool CLUSTER, bool PER>
+static int launch_inst(const pent_handle* h, const ChunkPlan& pl, int64_t M, const void* f, void* x,
+                       cudaStream_t s, const PeriodicParams<T>* per)
+{
+    constexpr int C = ChunkCfg<T>::C;
+    ChunkParams<T> prm;
+    prm.N = h->N; prm.P = pl.Pl; prm.Q = pl.Q; prm.Pw = pl.Pw; prm.M = M;
+    int lg = 0;
+    while ((1 << lg) < pl.Pw) ++lg;
+    prm.lev_f = h->lev_f[pl.j] < lg ? h->lev_f[pl.j] : lg;
+    prm.lev_b = h->lev_b[pl.j] < lg ? h->lev_b[pl.j] : lg;
+    for (int l = 0; l < W_LEVELS; ++l) prm.woff[l] = w_level_off(pl.Pl, l, pl.Q);
+    prm.box_rows = pl.box_rows; prm.nbox = pl.nbox;
+    prm.ntiles = (M + S - 1) / S;
+    for (int b = 0; b < MAX_BOXES; ++b) prm.wcount[b] = 0;
+    for (int w = 0; w * 32 < pl.Pl * S; ++w) prm.wcount[((w * 32 / S) * C) / prm.box_rows] += 1;
+    prm.table = (const T*)h->cf[pl.j];
+    prm.table_stride = (int64_t)table_len<T>(pl.Pl, pl.Q);
+    prm.table_bytes = (uint32_t)pl.table_bytes;
+    prm.x = (T*)x;
+
+    CUtensorMap tm;
+    if (!encode_batch_map(&tm, f, M, h->N, S, prm.box_rows, sizeof(T) == 8)) {
+        g_last_cuda_error = (int)cudaErrorInvalidValue;
+        return PENT_ERR_CUDA;
+    }
+
+    PeriodicParams<T> pp = {};
+    if (PER) pp = *per;
+    const size_t smem_total = pl.smem + (PER ? periodic_extra_smem<T>(pl) : 0);
+    auto kern = solve_chunked_kernel<T, S, CLUSTER, PER>;
+    static thread_local size_t smem_set = 0;
+    if (smem_total > smem_set) {
+        PENT_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_total));
+        smem_set = smem_total;
+    }
+    int dev = 0, nsm = 0;
+    PENT_CUDA(cudaGetDevice(&dev));
+    PENT_CUDA(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+    if constexpr (!CLUSTER) {
+        int occ = 0;
+        PENT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, pl.threads, smem_total));
+        if (occ < 1) return PENT_ERR_ARG;
+        int64_t grid = (int64_t)nsm * occ;
+        if (grid > prm.ntiles) grid = prm.ntiles;
+        kern<<<(unsigned)grid, pl.threads, smem_total, s>>>(tm, prm, pp);
+    } else {
+        cudaLaunchConfig_t cfg = {};
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = (unsigned)pl.Q; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.blockDim = dim3((unsigned)pl.threads); cfg.dynamicSmemBytes = smem_total; cfg.stream = s;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        cfg.gridDim = dim3((unsigned)(pl.Q * nsm));          // upper bound for the occupancy query
+        int ncl = 0;
+        PENT_CUDA(cudaOccupancyMaxActiveClusters(&ncl, kern, &cfg));
+        if (ncl < 1) return PENT_ERR_ARG;
+        int64_t clusters = ncl;
+        if (clusters > prm.ntiles) clusters = prm.ntiles;
+        cfg.gridDim = dim3((unsigned)(clusters * pl.Q));
+        PENT_CUDA(cudaLaunchKernelEx(&cfg, kern, tm, prm, pp));
+    }
+    count_launch();
+    PENT_LAUNCH_CHECK();
+    return PENT_OK;
+}
+
+}  // namespace pent

@@ -30,6 +30,7 @@ struct pent_handle {
     int periodic;
     pent_handle* inner;
     void* Zt;
+    void* pz[PENT_NQ];   // Z rows per cluster rank for the fused kernel: [Q][Pl*C] x {z0, z1} in T (0: not built)
     void* dgp;
     double pc[10];
     // ---- per-system factors, device, interleaved, in T ----
@@ -82,6 +83,8 @@ bool chunked_supported(const pent_handle* h, int64_t M, const void* f /* may be 
 bool step_chunked_supported(const pent_handle* h, int64_t M, const void* c /* may be null */);
 int launch_step_chunked(const pent_handle* h, const pent_step_params* p, int64_t M, void* c, int nsteps,
                         cudaStream_t s);
+bool periodic_fused_supported(const pent_handle* h, int64_t M, const void* f /* may be null */);
+int launch_solve_chunked_periodic(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s);
 int solve_periodic(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s, int kernel);
 int step_periodic(const pent_handle* h, int64_t M, void* c, void* scratch, int nsteps, cudaStream_t s);
 int chunked_choice(const pent_handle* h, int64_t M, int* Q, int* S);   // 1 and the default plan, or 0

@@ -12,7 +12,7 @@
 // In the interleaved layout the first N-2 rows of a batch ARE an interleaved (N-2) x M batch,
 // so the inner solve needs no copy.
 #include <new>
-#include "pent_internal.h"
+#include "pent_chunk_common.cuh"
 
 namespace pent {
 
@@ -72,6 +72,19 @@ __global__ void periodic_tables_kernel(int N, const T* __restrict__ stage, const
     }
     for (int j = 5; j < 8; ++j) dgp[8 * (size_t)k + j] = (T)0;
     if (Z && k < n) { typename Vec<T>::T2 z; z.x = (T)Z[k]; z.y = (T)Z[n + k]; Zt[k] = z; }
+}
+
+// Z rows regrouped per cluster rank for the fused kernel: out[(r*PlC + j)] = {Z0, Z1}[r*PlC + j], 0 beyond n
+template <typename T>
+__global__ void periodic_zslices_kernel(int n, int rows_total, const double* __restrict__ Z,
+                                        typename Vec<T>::T2* __restrict__ out)
+{
+    int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= rows_total) return;
+    typename Vec<T>::T2 z;
+    z.x = k < n ? (T)Z[k] : (T)0;
+    z.y = k < n ? (T)Z[n + k] : (T)0;
+    out[k] = z;
 }
 
 template <typename T>
@@ -149,7 +162,11 @@ static PeriodicCoef<T> coef_of(const pent_handle* h)
 template <typename T>
 static int solve_periodic_t(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s, int kernel)
 {
-    int rc = pent_solve_batch_v(h->inner, M, f, x, (void*)s, kernel);
+    if (kernel == PENT_KERNEL_AUTO && periodic_fused_supported(h, M, f))
+        return launch_solve_chunked_periodic(h, M, f, x, s);          // one kernel, 2 passes
+    if ((kernel & 0xff) == PENT_KERNEL_CHUNKED && kernel != PENT_KERNEL_CHUNKED) return PENT_ERR_ARG;
+    // unfused: inner solve (chunked when kernel == PENT_KERNEL_CHUNKED or AUTO) + tail + rank-2 update
+    int rc = pent_solve_batch_v(h->inner, M, f, x, (void*)s, kernel == PENT_KERNEL_CHUNKED ? PENT_KERNEL_AUTO : kernel);
     if (rc != PENT_OK) return rc;
     const int tb = 128;
     const unsigned nb = (unsigned)((M + tb - 1) / tb);
@@ -249,6 +266,14 @@ static int factor_periodic_t(int N, const void* const src[5], pent_dtype dtype, 
     periodic_setup_kernel<<<1, 32>>>(N, h->inner->fac, dg64, Z, coef, status);
     periodic_tables_kernel<T><<<nb, tb>>>(N, stage, Z, (typename Vec<T>::T2*)h->Zt, (T*)h->dgp, nullptr);
     count_launch(3);
+    for (int j = 0; j < PENT_NQ; ++j) {
+        const int Pl = h->inner->cfP[j];
+        if (Pl < 1) continue;
+        const int rows_total = (1 << j) * Pl * ChunkCfg<T>::C;
+        if (!alloc(&h->pz[j], sizeof(T) * 2 * (size_t)rows_total)) return done(rc);
+        periodic_zslices_kernel<T><<<(rows_total + tb - 1) / tb, tb>>>(n, rows_total, Z, (typename Vec<T>::T2*)h->pz[j]);
+        count_launch();
+    }
     cudaError_t le = cudaGetLastError();
     int st = 0;
     if (le == cudaSuccess) le = cudaMemcpy(&st, status, sizeof(int), cudaMemcpyDeviceToHost);
@@ -259,6 +284,12 @@ static int factor_periodic_t(int N, const void* const src[5], pent_dtype dtype, 
     return done(PENT_OK);
 }
 }  // namespace pent
+
+extern "C" int pent_periodic_fused(const pent_handle* h, int64_t M)
+{
+    if (!h || !h->periodic) return -1;
+    return pent::periodic_fused_supported(h, M, nullptr) ? 1 : 0;
+}
 
 extern "C" int pent_factor_periodic(int N, const void* e, const void* c, const void* d, const void* a,
                                     const void* b, pent_dtype dtype, pent_handle** out, int* bad_row)

@@ -28,7 +28,7 @@
 //   The shared coefficient tables (9 values per row) are staged ONCE per CTA into shared memory
 //   with one cp.async.bulk; every sweep step reads them as 16-byte warp-broadcast LDS.
 #include <cstdio>
-#include "pent_chunk_common.cuh"
+#include "pent_chunked_launch.cuh"
 
 namespace pent {
 
@@ -219,7 +219,6 @@ int build_chunk_tables(pent_handle* h, cudaStream_t s)
     return PENT_OK;
 }
 
-#include "pent_chunked_kernel.cuh"
 
 // ------------------------------------------------------------------------------------------
 // host side
@@ -310,7 +309,7 @@ bool encode_batch_map(CUtensorMap* tm, const void* base, int64_t M, int N, int S
 //     Q=2,S=32 vs 220 at Q=1,S=16; fp32 105.1 at Q=2,S=64 vs 111.5 at Q=1,S=32);
 //   * otherwise the smallest cluster with the narrow tile (cfg5a: 410.6 us at Q=4,S=16 vs 485 at
 //     Q=8,S=32: 8-CTA clusters leave SMs idle on the 16/18/20-SM GPCs).
-static ChunkPlan auto_plan(const pent_handle* h, int64_t M, const void* f)
+ChunkPlan chunk_auto_plan(const pent_handle* h, int64_t M, const void* f)
 {
     if (!h || h->kind != 0) return ChunkPlan{};
     const int Sn = h->dtype == PENT_F64 ? 16 : 32, Sw = 2 * Sn, QMAX = 1 << (PENT_NQ - 1);
@@ -333,7 +332,7 @@ static ChunkPlan auto_plan(const pent_handle* h, int64_t M, const void* f)
 
 static ChunkPlan resolve_plan(const pent_handle* h, int64_t M, const void* f, int Q, int S)
 {
-    if (Q == 0 && S == 0) return auto_plan(h, M, f);
+    if (Q == 0 && S == 0) return chunk_auto_plan(h, M, f);
     if (Q != 0 && S != 0) return make_plan(h, M, f, Q, S);
     const int cand[3] = {16, 32, 64};
     if (Q != 0) {
@@ -351,74 +350,10 @@ bool chunked_supported(const pent_handle* h, int64_t M, const void* f, int Q, in
 
 int chunked_choice(const pent_handle* h, int64_t M, int* Q, int* S)
 {
-    ChunkPlan pl = auto_plan(h, M, nullptr);
+    ChunkPlan pl = chunk_auto_plan(h, M, nullptr);
     if (!pl.ok) return 0;
     *Q = pl.Q; *S = pl.S;
     return 1;
-}
-
-template <typename T, int S, bool CLUSTER>
-static int launch_inst(const pent_handle* h, const ChunkPlan& pl, int64_t M, const void* f, void* x,
-                       cudaStream_t s)
-{
-    constexpr int C = ChunkCfg<T>::C;
-    ChunkParams<T> prm;
-    prm.N = h->N; prm.P = pl.Pl; prm.Q = pl.Q; prm.Pw = pl.Pw; prm.M = M;
-    int lg = 0;
-    while ((1 << lg) < pl.Pw) ++lg;
-    prm.lev_f = h->lev_f[pl.j] < lg ? h->lev_f[pl.j] : lg;
-    prm.lev_b = h->lev_b[pl.j] < lg ? h->lev_b[pl.j] : lg;
-    for (int l = 0; l < W_LEVELS; ++l) prm.woff[l] = w_level_off(pl.Pl, l, pl.Q);
-    prm.box_rows = pl.box_rows; prm.nbox = pl.nbox;
-    prm.ntiles = (M + S - 1) / S;
-    for (int b = 0; b < MAX_BOXES; ++b) prm.wcount[b] = 0;
-    for (int w = 0; w * 32 < pl.Pl * S; ++w) prm.wcount[((w * 32 / S) * C) / prm.box_rows] += 1;
-    prm.table = (const T*)h->cf[pl.j];
-    prm.table_stride = (int64_t)table_len<T>(pl.Pl, pl.Q);
-    prm.table_bytes = (uint32_t)pl.table_bytes;
-    prm.x = (T*)x;
-
-    CUtensorMap tm;
-    if (!encode_batch_map(&tm, f, M, h->N, S, prm.box_rows, sizeof(T) == 8)) {
-        g_last_cuda_error = (int)cudaErrorInvalidValue;
-        return PENT_ERR_CUDA;
-    }
-
-    auto kern = solve_chunked_kernel<T, S, CLUSTER>;
-    static thread_local size_t smem_set = 0;
-    if (pl.smem > smem_set) {
-        PENT_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem));
-        smem_set = pl.smem;
-    }
-    int dev = 0, nsm = 0;
-    PENT_CUDA(cudaGetDevice(&dev));
-    PENT_CUDA(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
-    if constexpr (!CLUSTER) {
-        int occ = 0;
-        PENT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, pl.threads, pl.smem));
-        if (occ < 1) return PENT_ERR_ARG;
-        int64_t grid = (int64_t)nsm * occ;
-        if (grid > prm.ntiles) grid = prm.ntiles;
-        kern<<<(unsigned)grid, pl.threads, pl.smem, s>>>(tm, prm);
-    } else {
-        cudaLaunchConfig_t cfg = {};
-        cudaLaunchAttribute at[1];
-        at[0].id = cudaLaunchAttributeClusterDimension;
-        at[0].val.clusterDim.x = (unsigned)pl.Q; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
-        cfg.blockDim = dim3((unsigned)pl.threads); cfg.dynamicSmemBytes = pl.smem; cfg.stream = s;
-        cfg.attrs = at; cfg.numAttrs = 1;
-        cfg.gridDim = dim3((unsigned)(pl.Q * nsm));          // upper bound for the occupancy query
-        int ncl = 0;
-        PENT_CUDA(cudaOccupancyMaxActiveClusters(&ncl, kern, &cfg));
-        if (ncl < 1) return PENT_ERR_ARG;
-        int64_t clusters = ncl;
-        if (clusters > prm.ntiles) clusters = prm.ntiles;
-        cfg.gridDim = dim3((unsigned)(clusters * pl.Q));
-        PENT_CUDA(cudaLaunchKernelEx(&cfg, kern, tm, prm));
-    }
-    count_launch();
-    PENT_LAUNCH_CHECK();
-    return PENT_OK;
 }
 
 int launch_solve_chunked(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s,
@@ -428,11 +363,11 @@ int launch_solve_chunked(const pent_handle* h, int64_t M, const void* f, void* x
     if (!pl.ok) return PENT_ERR_ARG;
     const bool cl = pl.Q > 1;
     if (h->dtype == PENT_F64) {
-        if (pl.S == 16) return cl ? launch_inst<double, 16, true>(h, pl, M, f, x, s) : launch_inst<double, 16, false>(h, pl, M, f, x, s);
-        if (pl.S == 32) return cl ? launch_inst<double, 32, true>(h, pl, M, f, x, s) : launch_inst<double, 32, false>(h, pl, M, f, x, s);
+        if (pl.S == 16) return cl ? launch_inst<double, 16, true, false>(h, pl, M, f, x, s, nullptr) : launch_inst<double, 16, false, false>(h, pl, M, f, x, s, nullptr);
+        if (pl.S == 32) return cl ? launch_inst<double, 32, true, false>(h, pl, M, f, x, s, nullptr) : launch_inst<double, 32, false, false>(h, pl, M, f, x, s, nullptr);
     } else {
-        if (pl.S == 32) return cl ? launch_inst<float, 32, true>(h, pl, M, f, x, s) : launch_inst<float, 32, false>(h, pl, M, f, x, s);
-        if (pl.S == 64) return cl ? launch_inst<float, 64, true>(h, pl, M, f, x, s) : launch_inst<float, 64, false>(h, pl, M, f, x, s);
+        if (pl.S == 32) return cl ? launch_inst<float, 32, true, false>(h, pl, M, f, x, s, nullptr) : launch_inst<float, 32, false, false>(h, pl, M, f, x, s, nullptr);
+        if (pl.S == 64) return cl ? launch_inst<float, 64, true, false>(h, pl, M, f, x, s, nullptr) : launch_inst<float, 64, false, false>(h, pl, M, f, x, s, nullptr);
     }
     return PENT_ERR_ARG;
 }

@@ -6,7 +6,7 @@
 // reference design and the HBM-spill path for N too large to keep on chip; the headline
 // kernel is in pent_solve_chunked.cu.
 #include <new>
-#include "pent_internal.h"
+#include "pent_chunk_common.cuh"
 
 namespace pent {
 
@@ -180,18 +180,6 @@ factor_tps_kernel(int N, int64_t M, const T* __restrict__ a, const T* __restrict
 // delta, g} (same stage size).  cfg5b: 418 us with register load-ahead -> see profiles/r01_ab_tuning.md.
 // ---------------------------------------------------------------------------------------------
 constexpr int RING_ROWS = 4, RING_STAGES = 6, RING_SLOTS = 6 * RING_ROWS;   // values per thread and stage
-
-__device__ __forceinline__ void cp_async_elem(double* dst, const double* src)
-{
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
-}
-__device__ __forceinline__ void cp_async_elem(float* dst, const float* src)
-{
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N_>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N_) : "memory"); }
 
 template <typename T>
 __global__ void __launch_bounds__(PS_THREADS)

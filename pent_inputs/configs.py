@@ -43,6 +43,8 @@ WORKLOADS = {
     # hyperdiffusion systems, Crank-Nicolson, N=1024, batch 8192, dt=1e-8 (sigma_x = dt/(2 dx^4))
     "paper_hd": Workload("paper_hd", 1024, 8192, 1e-8 / (2.0 * (1.0 / 1024) ** 4), "periodic", 7, "cos_mode",
                          "periodic hyperdiffusion, identical systems, 250 steps"),
+    # cfg3's shape with the paper's periodic matrix (Eq. 7a-7b), for the periodic solve on its own
+    "cfg3p": Workload("cfg3p", 1024, 65536, 10.0, "periodic", 8, "uniform", "periodic solve, N=1024, M=65536"),
     "cfg5b": Workload("cfg5b", 1024, 16384, float("nan"), "dirichlet", 6, "uniform",
                       "per-system sigma_i ~ U[0.1,10]"),
 }
@@ -68,6 +70,9 @@ def make_matrix(w: Workload, M: int | None = None, col0: int = 0):
         M = w.M if M is None else M
         sig = uniform_vec(w.seed, 1, M, 0.1, 10.0, col0)
         return diagonals_I_plus_sigma_L2(w.N, sig, w.bc)
+    if w.bc == "periodic":
+        from . import periodic_hyperdiffusion_diagonals
+        return periodic_hyperdiffusion_diagonals(w.N, w.sigma)
     return diagonals_I_plus_sigma_L2(w.N, w.sigma, w.bc)
 
 
