@@ -364,8 +364,25 @@ def run_step_workload(args, w, rank, world, local):
     on_chip = (kern == 2) or (kern == 0 and pent.lib().pent_step_kernel_choice(h.ptr, M) == 2)
     kname = "step_chunked_kernel" if on_chip else "step_tps_kernel"
     peak, peak_src = measured_peak()
-    alg = 2.0 * esz * N * M * args.steps          # read c, write c per step if the state streamed through HBM
-    achieved = alg / (ms * 1e-3) / 1e9
+    hbm_equiv = 2.0 * esz * N * M * args.steps / (ms * 1e-3) / 1e9   # GB/s if the state streamed through HBM every step
+    # ALU bound: 19 fused multiply-adds per unknown and step (9 right-hand
+    # side of the increment form, 9 solve, 1 update); fp64 issues 64 FMA/clk/SM (measured 63.7),
+    # fp32 128 FMA/clk/SM; x 148 SMs x the SM clock sampled during the run
+    fma_per_unknown = 19.0
+    sm_mhz = clocks.get("sm_max_mhz") or 1965.0
+    alu_peak = 2.0 * (64.0 if args.dtype == "f64" else 128.0) * 148 * sm_mhz * 1e6 / 1e12
+    achieved = 2.0 * fma_per_unknown * N * M * args.steps / (ms * 1e-3) / 1e12
+    if on_chip:
+        roof = {"bound": "alu", "achieved": achieved, "peak": alu_peak, "unit": "TFLOP/s", "frac": achieved / alu_peak,
+                "traffic": None, "peak_source": "derived: FMA/clk/SM x 148 SMs x SM clock (DESIGN.md section 6.4)",
+                "flops_per_unknown_step": 2.0 * fma_per_unknown, "kernel": kname,
+                "hbm_equivalent_gbs": hbm_equiv, "hbm_equivalent_frac": hbm_equiv / peak,
+                "note": "state stays in shared memory across the steps of a launch: HBM is touched twice per LAUNCH; "
+                        "hbm_equivalent = rate of streaming the state once in, once out per step"}
+    else:
+        roof = {"bound": "hbm", "achieved": hbm_equiv, "peak": peak, "unit": "GB/s", "frac": hbm_equiv / peak,
+                "traffic": None, "peak_source": peak_src, "algorithmic_bytes_per_launch": 2.0 * esz * N * M,
+                "kernel": kname}
     line = {
         "metric": METRIC, "value": whole_job_rate(N * M * args.steps, world, ms * 1e-3), "unit": UNIT,
         "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps,
@@ -374,11 +391,7 @@ def run_step_workload(args, w, rank, world, local):
                    "step": "Cahn-Hilliard semi-implicit, increment form, RHS fused into the solve",
                    "kernel": kname, "state_on_chip_across_steps": bool(on_chip),
                    "l2": "state 64 MiB; the on-chip kernel reads and writes it once per launch"},
-        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": None, "peak_source": peak_src,
-                     "algorithmic_bytes_per_launch": alg, "kernel": kname,
-                     "note": "HBM-equivalent rate of streaming the state once in, once out per step; the on-chip "
-                             "kernel is bound by arithmetic and barriers, not HBM, so frac may exceed 1"},
+        "roofline": roof,
         "clocks": clocks, "gpu_launches": int(launches),
     }
     _finish_line(line, world)
