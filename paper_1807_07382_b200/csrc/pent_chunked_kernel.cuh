@@ -5,10 +5,8 @@
 #define PENT_AB_NO_Z 0
 #endif
 
-// Measured A/B switches (cfg3 fp64 on B200, profiles/r01_ab_tuning.md).  Defaults = fastest:
+// Measured A/B switches (cfg3 fp64 on B200, profiles/r01_ab_tuning.md).  Default = fastest:
 //   store policy of the x stream: plain write-back st.global (201 us) beat .cs (212), .cg (210), .wt (211)
-//   chunk-state layout: [P][S] (197 us with 256-B L2 promotion) beat the bank-conflict-free padded
-//   [S][P+1] (221 us) although the scan then reads with a 32-way conflict: see DESIGN.md section 6.2.
 #if defined(PENT_AB_ST_CS)
 #define PENT_STORE(p, v) __stcs((p), (v))
 #elif defined(PENT_AB_ST_CG)

@@ -50,14 +50,23 @@ static int launch_inst(const pent_handle* h, const ChunkPlan& pl, int64_t M, con
         PENT_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_total));
         smem_set = smem_total;
     }
-    int dev = 0, nsm = 0;
+    // the occupancy answer depends only on (device, threads, shared memory, cluster size): keep the last
+    // one per thread and kernel instance, so a small solve is not bound by host-side queries
+    struct OccCache { int dev = -1, threads = 0, Q = 0, nsm = 0, resident = 0; size_t smem = 0; };
+    static thread_local OccCache oc;
+    int dev = 0;
     PENT_CUDA(cudaGetDevice(&dev));
-    PENT_CUDA(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+    const bool hit = oc.dev == dev && oc.threads == pl.threads && oc.smem == smem_total && oc.Q == pl.Q;
+    if (!hit) PENT_CUDA(cudaDeviceGetAttribute(&oc.nsm, cudaDevAttrMultiProcessorCount, dev));
     if constexpr (!CLUSTER) {
-        int occ = 0;
-        PENT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, pl.threads, smem_total));
-        if (occ < 1) return PENT_ERR_ARG;
-        int64_t grid = (int64_t)nsm * occ;
+        if (!hit) {
+            int occ = 0;
+            PENT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, pl.threads, smem_total));
+            oc.resident = oc.nsm * occ;                          // CTAs resident at once
+            oc.dev = dev; oc.threads = pl.threads; oc.smem = smem_total; oc.Q = pl.Q;
+        }
+        if (oc.resident < 1) return PENT_ERR_ARG;
+        int64_t grid = oc.resident;
         if (grid > prm.ntiles) grid = prm.ntiles;
         kern<<<(unsigned)grid, pl.threads, smem_total, s>>>(tm, prm, pp);
     } else {
@@ -67,11 +76,15 @@ static int launch_inst(const pent_handle* h, const ChunkPlan& pl, int64_t M, con
         at[0].val.clusterDim.x = (unsigned)pl.Q; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
         cfg.blockDim = dim3((unsigned)pl.threads); cfg.dynamicSmemBytes = smem_total; cfg.stream = s;
         cfg.attrs = at; cfg.numAttrs = 1;
-        cfg.gridDim = dim3((unsigned)(pl.Q * nsm));          // upper bound for the occupancy query
-        int ncl = 0;
-        PENT_CUDA(cudaOccupancyMaxActiveClusters(&ncl, kern, &cfg));
-        if (ncl < 1) return PENT_ERR_ARG;
-        int64_t clusters = ncl;
+        if (!hit) {
+            cfg.gridDim = dim3((unsigned)(pl.Q * oc.nsm));       // upper bound for the occupancy query
+            int ncl = 0;
+            PENT_CUDA(cudaOccupancyMaxActiveClusters(&ncl, kern, &cfg));
+            oc.resident = ncl;                                   // clusters resident at once
+            oc.dev = dev; oc.threads = pl.threads; oc.smem = smem_total; oc.Q = pl.Q;
+        }
+        if (oc.resident < 1) return PENT_ERR_ARG;
+        int64_t clusters = oc.resident;
         if (clusters > prm.ntiles) clusters = prm.ntiles;
         cfg.gridDim = dim3((unsigned)(clusters * pl.Q));
         PENT_CUDA(cudaLaunchKernelEx(&cfg, kern, tm, prm, pp));

@@ -20,13 +20,16 @@
 //   All are functions of the shared factors only and are built once in pent_factor.  Exact in
 //   exact arithmetic; in fp64 it differs from the serial sweep by rounding only.
 //
-// DATA MOVEMENT (one persistent CTA per SM, tile = S systems x all N rows):
-//   f tile --TMA (cp.async.bulk.tensor.2d, 4 boxes, mbarrier complete_tx)--> smem landing
-//   buffer --LDS--> registers; the landing buffer is free again after the first block barrier,
-//   so the TMA load of the NEXT tile runs under the chunk-state scan, the correction and the
-//   stores of this tile.  x goes registers --st.global.cs--> HBM as 128-byte row segments.
+// DATA MOVEMENT (persistent CTAs, tile = S systems x the rows of this CTA):
+//   f tile --TMA (cp.async.bulk.tensor.2d, <= 4 boxes, mbarrier complete_tx)--> smem landing
+//   buffer --LDS--> registers; each box is re-armed with the NEXT tile's load as soon as the warps
+//   that read it have their rows in registers, so that load runs under this tile's arithmetic,
+//   scan and stores.  x goes registers --st.global--> HBM as full 128/256-byte row segments.
 //   The shared coefficient tables (9 values per row) are staged ONCE per CTA into shared memory
 //   with one cp.async.bulk; every sweep step reads them as 16-byte warp-broadcast LDS.
+// LARGER N / WIDER TILES: a thread-block cluster splits k between its CTAs and stitches the block
+//   aggregates through distributed shared memory (chunk_state_scan in pent_chunk_common.cuh).
+// This file: the tables (built once per handle and cluster size), the launch plans and dispatch.
 #include <cstdio>
 #include "pent_chunked_launch.cuh"
 
