@@ -52,8 +52,11 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
     T2* stE = reinterpret_cast<T2*>(reinterpret_cast<unsigned char*>(table) + prm.table_bytes);
     T2* stS = stE + (size_t)S * P;
     // cluster: block aggregates of every rank, [Q][S] each (written by the owning rank through DSMEM)
+    // Slot rr holds rank rr's FORWARD aggregate when rr < rank and its BACKWARD aggregate when rr > rank
+    // (a CTA needs nothing else), so both directions share one array; the periodic kernel needs every
+    // rank's backward aggregate and keeps two.
     T2* aggF = stS + (size_t)S * P;
-    T2* aggB = aggF + (CLUSTER ? (size_t)prm.Q * S : 0);
+    T2* aggB = aggF + ((CLUSTER && PER) ? (size_t)prm.Q * S : 0);
     // periodic: this CTA's rows of Z, then x^ of rows n-2/n-1, (y_{n-2}, y_{n-1}), (f_n, f_{n+1}), t  ([S] each)
     T2* zs = aggB + (CLUSTER ? (size_t)prm.Q * S : 0);
     T2* ypub = zs + (PER ? (size_t)P * C : 0);

@@ -11,7 +11,7 @@ namespace pent {
 template <typename T>
 inline size_t periodic_extra_smem(const ChunkPlan& pl)
 {
-    return ((size_t)pl.Pl * ChunkCfg<T>::C + 5 * (size_t)pl.S) * 2 * sizeof(T);
+    return ((size_t)pl.Pl * ChunkCfg<T>::C + 5 * (size_t)pl.S + (pl.Q > 1 ? (size_t)pl.Q * pl.S : 0)) * 2 * sizeof(T);   // + second aggregate array
 }
 
 template <typename T, int S, bool CLUSTER, bool PER>

@@ -280,7 +280,7 @@ ChunkPlan make_plan(const pent_handle* h, int64_t M, const void* f, int Q, int S
     const size_t bl = f64 ? chunk_block_len<double>() : chunk_block_len<float>();
     pl.table_bytes = ((size_t)pl.Pl * bl + (size_t)w_level_off(pl.Pl, pl.levels, Q)) * esz;
     pl.smem = (size_t)pl.nbox * pl.box_rows * S * esz + pl.table_bytes + (size_t)4 * pl.Pl * S * esz +
-              (Q > 1 ? (size_t)4 * Q * S * esz : 0) + (3 + 2 * MAX_BOXES) * sizeof(uint64_t);
+              (Q > 1 ? (size_t)2 * Q * S * esz : 0) + (3 + 2 * MAX_BOXES) * sizeof(uint64_t);   // one [Q][S] pair array
     if (pl.smem > SMEM_LIMIT) return pl;
     if ((M * (int64_t)esz) % 16 != 0) return pl;            // TMA global stride alignment
     if (f && ((uintptr_t)f % 16) != 0) return pl;           // TMA global address alignment

@@ -219,7 +219,7 @@ def _shape_case(N, M, Q, S, dtype=torch.float64, sigma=None, seed=70):
 
 @pytest.mark.parametrize("N,M,Q,S", [
     (1024, 2048 + 32, 2, 32), (1024, 512, 4, 32), (1024, 512, 2, 16), (512, 1000, 1, 32), (512, 992, 2, 32),
-    (2048, 520, 2, 16), (2048, 512, 4, 32), (4096, 304, 4, 16), (4096, 512, 8, 32), (6000, 64, 8, 16), (64, 32, 2, 16),
+    (2048, 520, 2, 16), (2048, 512, 4, 32), (4096, 304, 4, 16), (4096, 512, 8, 32), (6000, 64, 8, 16), (8192, 48, 8, 16), (64, 32, 2, 16),
     (1000, 200, 2, 32), (3000, 100, 4, 16), (700, 96, 2, 16), (96, 40, 2, 16), (65, 34, 2, 32), (5000, 48, 8, 16),
 ])
 def test_chunked_shapes_nonsymmetric_fp64(N, M, Q, S):
@@ -252,7 +252,7 @@ def test_chunked_cluster_slowly_decaying_coupling(Q, S):
 
 def test_auto_choice_is_on_chip_for_every_config_shape():
     pent = _pent()
-    for N, M in ((64, 256), (512, 16384), (1024, 65536), (4096, 32768), (2048, 1024)):
+    for N, M in ((64, 256), (512, 16384), (1024, 65536), (4096, 32768), (2048, 1024), (8192, 512)):
         diags = pin.diagonals_I_plus_sigma_L2(N, 1.0)
         a, b, c, d, e = (torch.tensor(v) for v in diags)
         h = pent.pent_factor(N, e, c, d, a, b)
