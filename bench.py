@@ -43,6 +43,7 @@ def parse_args():
     ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 thread-per-system, 2 chunked")
     ap.add_argument("--cluster", type=int, default=0, help="chunked kernel: CTAs per cluster along k (0 auto)")
     ap.add_argument("--tile", type=int, default=0, help="chunked kernel: systems per tile (0 auto)")
+    ap.add_argument("--systems", type=int, default=0, help="override M of the workload (shape experiments)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=3)
@@ -215,7 +216,7 @@ def run_ours(args):
         return run_paper_workload(args, w, rank, world, local)
     tdt = torch.float64 if args.dtype == "f64" else torch.float32
     esz = 8 if args.dtype == "f64" else 4
-    N, M = w.N, w.M
+    N, M = w.N, (args.systems or w.M)
     diags = make_matrix(w)
     # weak scaling: rank r owns systems [r*M, (r+1)*M) of ONE seeded batch of world*M systems
     from paper_1807_07382_b200.sharding import max_over_ranks, shard_columns, whole_job_rate

@@ -418,10 +418,13 @@ __device__ __forceinline__ void chunk_state_scan(const ScanGeom& g, const T* wta
 struct ChunkPlan {
     bool ok = false;
     int j = 0, Q = 1, S = 0, Pl = 0, Pw = 1, threads = 0, levels = 0, box_rows = 0, nbox = 0;
+    bool ldg = false;          // LDG loader instead of TMA (pitch not a multiple of 16 bytes)
     size_t table_bytes = 0, smem = 0;
 };
 // any_S: accept tile widths the SOLVE kernel is not instantiated for (the step kernel has its own)
-ChunkPlan make_plan(const pent_handle* h, int64_t M, const void* f, int Q, int S, bool any_S = false);
+// ldg: plan for the LDG loader (no TMA alignment requirements, no landing buffer)
+ChunkPlan make_plan(const pent_handle* h, int64_t M, const void* f, int Q, int S, bool any_S = false,
+                    bool ldg = false);
 ChunkPlan chunk_auto_plan(const pent_handle* h, int64_t M, const void* f);   // what PENT_KERNEL_AUTO runs
 // rank-2 tensor map {M, N} of an interleaved batch with box {S, box_rows}; false on failure
 bool encode_batch_map(CUtensorMap* tm, const void* base, int64_t M, int N, int S, int box_rows, bool f64);

@@ -33,6 +33,9 @@ struct ChunkParams {
     int64_t M;
     int64_t ntiles;
     const T* table;   // global coefficient tables (layout = shared-memory layout), one per rank
+    const T* f;       // right-hand side (used by the LDG loader)
+    int ldg;          // 1: the pitch M*sizeof(T) is not a multiple of 16 bytes, so TMA cannot address the batch:
+                      // every thread loads its rows with coalesced LDG instead (no landing buffer, nbox = 0)
     T* x;
 };
 
@@ -147,17 +150,26 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
             }
         }
         if (active) {
-            // ---- tile data: landing buffer -> registers ----
-            mbar_wait(&bars[1 + mybox], parity);
-            const T* src = landing + (size_t)p * C * S + i;
+            if (prm.ldg) {
+                // ---- tile data: global -> registers (C independent loads in flight per thread) ----
+                const int64_t col = tile * S + i;
+                const T* src = prm.f + (int64_t)row0 * prm.M + col;
+                const int nrows = col < prm.M ? prm.N - row0 : 0;
 #pragma unroll
-            for (int j = 0; j < C; ++j) v[j] = src[j * S];
+                for (int j = 0; j < C; ++j) v[j] = (j < nrows) ? __ldcs(src + (int64_t)j * prm.M) : (T)0;
+            } else {
+                // ---- tile data: landing buffer -> registers ----
+                mbar_wait(&bars[1 + mybox], parity);
+                const T* src = landing + (size_t)p * C * S + i;
+#pragma unroll
+                for (int j = 0; j < C; ++j) v[j] = src[j * S];
+            }
         }
         // The box is free once every warp that reads it has its values in registers: each such
         // warp arrives on the box's "empty" barrier and thread 0 re-arms it with the NEXT tile's
         // TMA load, which then runs under all of this tile's arithmetic and stores.
         __syncwarp();
-        if (lane == 0 && warp * 32 < P * S) mbar_arrive(&bars[1 + MAX_BOXES + mybox]);
+        if (lane == 0 && warp * 32 < P * S && !prm.ldg) mbar_arrive(&bars[1 + MAX_BOXES + mybox]);
         if constexpr (CLUSTER) {
             if (tid == 0) {        // arm this tile's aggregate barriers (complete_tx may already have arrived)
                 if (agg_bytes_f) mbar_expect_tx(&bars[BAR_F], agg_bytes_f);

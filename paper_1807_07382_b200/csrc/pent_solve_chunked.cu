@@ -252,7 +252,7 @@ static bool s_instantiated(bool f64, int S, bool cluster)
     return f64 ? (S == 16 || S == 32) : (S == 32 || S == 64);
 }
 
-ChunkPlan make_plan(const pent_handle* h, int64_t M, const void* f, int Q, int S, bool any_S)
+ChunkPlan make_plan(const pent_handle* h, int64_t M, const void* f, int Q, int S, bool any_S, bool ldg)
 {
     ChunkPlan pl;
     if (!h || h->kind != 0) return pl;
@@ -279,13 +279,17 @@ ChunkPlan make_plan(const pent_handle* h, int64_t M, const void* f, int Q, int S
     if (pl.nbox > MAX_BOXES) return pl;
     const size_t bl = f64 ? chunk_block_len<double>() : chunk_block_len<float>();
     pl.table_bytes = ((size_t)pl.Pl * bl + (size_t)w_level_off(pl.Pl, pl.levels, Q)) * esz;
+    pl.ldg = ldg;
+    if (ldg) pl.nbox = 0;                                    // no landing buffer
     pl.smem = (size_t)pl.nbox * pl.box_rows * S * esz + pl.table_bytes + (size_t)4 * pl.Pl * S * esz +
               (Q > 1 ? (size_t)2 * Q * S * esz : 0) + (3 + 2 * MAX_BOXES) * sizeof(uint64_t);   // one [Q][S] pair array
     if (pl.smem > SMEM_LIMIT) return pl;
-    if ((M * (int64_t)esz) % 16 != 0) return pl;            // TMA global stride alignment
-    if (f && ((uintptr_t)f % 16) != 0) return pl;           // TMA global address alignment
-    if (M > (int64_t)0x7fffffff) return pl;                 // TMA coordinates are 32-bit
-    if (!encode_fn()) return pl;
+    if (!ldg) {
+        if ((M * (int64_t)esz) % 16 != 0) return pl;        // TMA global stride alignment
+        if (f && ((uintptr_t)f % 16) != 0) return pl;       // TMA global address alignment
+        if (M > (int64_t)0x7fffffff) return pl;             // TMA coordinates are 32-bit
+        if (!encode_fn()) return pl;
+    }
     pl.ok = true;
     return pl;
 }
@@ -330,13 +334,27 @@ ChunkPlan chunk_auto_plan(const pent_handle* h, int64_t M, const void* f)
         ChunkPlan pl = make_plan(h, M, f, Q, Sw);
         if (pl.ok) return pl;
     }
+    // TMA cannot address this batch (pitch or base not 16-byte aligned): LDG loader.  It has no
+    // prefetch of the next tile, so prefer CTAs of <= 256 threads: two of them share an SM and one
+    // loads while the other computes.
+    for (int Q = 1; Q <= QMAX; Q *= 2) {
+        ChunkPlan pl = make_plan(h, M, f, Q, Sn, false, true);
+        if (pl.ok && pl.threads <= 256) return pl;
+    }
+    for (int Q = 1; Q <= QMAX; Q *= 2) {
+        ChunkPlan pl = make_plan(h, M, f, Q, Sn, false, true);
+        if (pl.ok) return pl;
+    }
     return ChunkPlan{};
 }
 
 static ChunkPlan resolve_plan(const pent_handle* h, int64_t M, const void* f, int Q, int S)
 {
     if (Q == 0 && S == 0) return chunk_auto_plan(h, M, f);
-    if (Q != 0 && S != 0) return make_plan(h, M, f, Q, S);
+    if (Q != 0 && S != 0) {
+        ChunkPlan pl = make_plan(h, M, f, Q, S);
+        return pl.ok ? pl : make_plan(h, M, f, Q, S, false, true);
+    }
     const int cand[3] = {16, 32, 64};
     if (Q != 0) {
         for (int s : cand) { ChunkPlan pl = make_plan(h, M, f, Q, s); if (pl.ok) return pl; }

@@ -250,6 +250,27 @@ def test_chunked_cluster_slowly_decaying_coupling(Q, S):
     assert residual(diags, x, f) <= max(1e-12, (1.0 + 16.0 * sigma) * 2.0 ** -53)
 
 
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("N,M", [(1024, 1001), (512, 333), (4096, 77), (2000, 129), (100, 7)])
+def test_unaligned_pitch_runs_on_chip_with_the_ldg_loader(dtype, N, M):
+    """M*sizeof(T) not a multiple of 16 bytes: TMA cannot address the batch; the chunked kernel then
+    loads with LDG (still 2 passes) instead of falling back to the 4-pass kernel."""
+    pent = _pent()
+    diags = pin.diagonals_I_plus_sigma_L2(N, 2.0)
+    f = pin.uniform_pm1(90 + N, 0, N, M)
+    a, b, c, d, e = (torch.tensor(v, dtype=dtype) for v in diags)
+    h = pent.pent_factor(N, e, c, d, a, b)
+    assert pent.kernel_choice(h, M)["kernel"] == "solve_chunked_kernel"
+    x, _ = gpu_solve(diags, f, dtype=dtype)
+    d64, f64, ref = oracle_for_dtype(diags, f, dtype)
+    tol_x, tol_r = TOL[dtype]
+    assert normwise(x.astype(np.float64), ref) <= tol_x
+    assert residual(d64, x, f64) <= tol_r
+    # in place too
+    xi, _ = gpu_solve(diags, f, dtype=dtype, inplace=True)
+    assert np.array_equal(xi, x)
+
+
 def test_auto_choice_is_on_chip_for_every_config_shape():
     pent = _pent()
     for N, M in ((64, 256), (512, 16384), (1024, 65536), (4096, 32768), (2048, 1024), (8192, 512)):

@@ -35,7 +35,7 @@ def _handle(diags, dtype=torch.float64):
 # kernel 0 = auto (fused single kernel when the shape allows), 2 = chunked solve + tail + update, 1 = thread per system
 @pytest.mark.parametrize("kernel", [0, 2, 1])
 @pytest.mark.parametrize("N,M", [(6, 4), (7, 34), (34, 18), (35, 64), (64, 256), (258, 130), (1026, 544), (1000, 38),
-                                 (1024, 96), (1058, 64), (2050, 96), (4098, 48), (3000, 32)])
+                                 (1024, 96), (1058, 64), (2050, 96), (4098, 48), (3000, 32), (1024, 545), (64, 255), (2050, 33)])
 def test_periodic_nonsymmetric_parity(kernel, N, M):
     pent = _pent()
     diags = pin.random_periodic_diag_dominant(300 + N, N)
@@ -49,7 +49,7 @@ def test_periodic_nonsymmetric_parity(kernel, N, M):
 
 def test_fused_kernel_is_the_default_where_it_fits():
     pent = _pent()
-    for N, M, want in ((1024, 65536, 1), (512, 4096, 1), (64, 256, 1), (2048, 1024, 1), (1024, 65535, 0)):
+    for N, M, want in ((1024, 65536, 1), (512, 4096, 1), (64, 256, 1), (2048, 1024, 1), (1024, 65535, 1), (4096, 1024, 0)):
         h = _handle(pin.periodic_hyperdiffusion_diagonals(N, 1.0))
         assert pent.lib().pent_periodic_fused(h.ptr, M) == want, (N, M)
 
