@@ -87,12 +87,22 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
     __syncthreads();
+#if PENT_PDL
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+#endif
     int64_t tile = first;
     if (tid == 0) {
         const uint32_t z_bytes = PER ? (uint32_t)(P * C * sizeof(T2)) : 0u;
         mbar_expect_tx(&bars[0], prm.table_bytes + z_bytes);
         bulk_load_1d(table, prm.table + (size_t)rank * prm.table_stride, prm.table_bytes, &bars[0]);
         if constexpr (PER) bulk_load_1d(zs, pp.zt + (size_t)rank * 2 * P * C, z_bytes, &bars[0]);
+    }
+#if PENT_PDL
+    // the previous kernel on the stream may have written f or may still read x: wait for it before the
+    // first access to the batch (the tables staged above are constant)
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+#endif
+    if (tid == 0) {
         if (tile < prm.ntiles)
             for (int b = 0; b < prm.nbox; ++b) {
                 mbar_expect_tx(&bars[1 + b], box_bytes);

@@ -4,6 +4,10 @@
 #pragma once
 #include "pent_chunk_common.cuh"
 
+#ifndef PENT_PDL
+#define PENT_PDL 1      // programmatic dependent launch (A/B: -DPENT_PDL=0), see the kernel prologue
+#endif
+
 namespace pent {
 #include "pent_chunked_kernel.cuh"
 
@@ -70,14 +74,29 @@ static int launch_inst(const pent_handle* h, const ChunkPlan& pl, int64_t M, con
         if (oc.resident < 1) return PENT_ERR_ARG;
         int64_t grid = oc.resident;
         if (grid > prm.ntiles) grid = prm.ntiles;
-        kern<<<(unsigned)grid, pl.threads, smem_total, s>>>(tm, prm, pp);
-    } else {
+#if PENT_PDL
+        // programmatic dependent launch: this grid's prologue (mbarrier init, staging of the constant
+        // coefficient table) may overlap the tail of the previous kernel on the stream; the kernel
+        // waits (griddepcontrol.wait) before it touches f or x
         cudaLaunchConfig_t cfg = {};
         cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)pl.threads);
+        cfg.dynamicSmemBytes = smem_total; cfg.stream = s; cfg.attrs = at; cfg.numAttrs = 1;
+        PENT_CUDA(cudaLaunchKernelEx(&cfg, kern, tm, prm, pp));
+#else
+        kern<<<(unsigned)grid, pl.threads, smem_total, s>>>(tm, prm, pp);
+#endif
+    } else {
+        cudaLaunchConfig_t cfg = {};
+        cudaLaunchAttribute at[2];
+        at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[1].val.programmaticStreamSerializationAllowed = 1;
         at[0].id = cudaLaunchAttributeClusterDimension;
         at[0].val.clusterDim.x = (unsigned)pl.Q; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
         cfg.blockDim = dim3((unsigned)pl.threads); cfg.dynamicSmemBytes = smem_total; cfg.stream = s;
-        cfg.attrs = at; cfg.numAttrs = 1;
+        cfg.attrs = at; cfg.numAttrs = 1 + PENT_PDL;
         if (!hit) {
             cfg.gridDim = dim3((unsigned)(pl.Q * oc.nsm));       // upper bound for the occupancy query
             int ncl = 0;
