@@ -51,11 +51,8 @@ static int launch_inst(const pent_handle* h, const ChunkPlan& pl, int64_t M, con
     if (PER) pp = *per;
     const size_t smem_total = pl.smem + (PER ? periodic_extra_smem<T>(pl) : 0);
     auto kern = solve_chunked_kernel<T, S, CLUSTER, PER>;
-    static thread_local size_t smem_set = 0;
-    if (smem_total > smem_set) {
-        PENT_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_total));
-        smem_set = smem_total;
-    }
+    static thread_local SmemMark mark;
+    PENT_CUDA(ensure_dynamic_smem(mark, kern, smem_total));
     // the occupancy answer depends only on (device, threads, shared memory, cluster size): keep the last
     // one per thread and kernel instance, so a small solve is not bound by host-side queries
     struct OccCache { int dev = -1, threads = 0, Q = 0, nsm = 0, resident = 0; size_t smem = 0; };

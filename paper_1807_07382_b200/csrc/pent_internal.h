@@ -45,6 +45,24 @@ extern thread_local int64_t g_launches;
 inline int cuda_fail(cudaError_t e) { g_last_cuda_error = (int)e; return PENT_ERR_CUDA; }
 inline void count_launch(int n = 1) { g_launches += n; }
 
+// cudaFuncAttributeMaxDynamicSharedMemorySize is per device: one high-water mark per (calling thread,
+// kernel instance, device).  `mark` is a `static thread_local SmemMark` at the launch site.
+struct SmemMark { size_t bytes[16] = {}; };
+template <typename K>
+inline cudaError_t ensure_dynamic_smem(SmemMark& mark, K kernel, size_t bytes)
+{
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    const int d = dev & 15;
+    if (bytes > mark.bytes[d]) {
+        e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+        if (e != cudaSuccess) return e;
+        mark.bytes[d] = bytes;
+    }
+    return cudaSuccess;
+}
+
 #define PENT_CUDA(call)                                           \
     do {                                                          \
         cudaError_t e__ = (call);                                 \

@@ -195,15 +195,20 @@ static int build_tables_t(pent_handle* h, int j, cudaStream_t s)
     PENT_CUDA(e);
     double* tmat = nullptr;
     int* lev = nullptr;
-    PENT_CUDA(cudaMalloc(&tmat, sizeof(double) * 12 * Pl * Q));
-    PENT_CUDA(cudaMalloc(&lev, 2 * sizeof(int)));
-    PENT_CUDA(cudaMemsetAsync(lev, 0, 2 * sizeof(int), s));
-    PENT_CUDA(cudaMemsetAsync(h->cf[j], 0, tlen * Q * sizeof(T), s));
+    cudaError_t le = cudaMalloc(&tmat, sizeof(double) * 12 * Pl * Q);
+    if (le == cudaSuccess) le = cudaMalloc(&lev, 2 * sizeof(int));
+    if (le == cudaSuccess) le = cudaMemsetAsync(lev, 0, 2 * sizeof(int), s);
+    if (le == cudaSuccess) le = cudaMemsetAsync(h->cf[j], 0, tlen * Q * sizeof(T), s);
+    if (le != cudaSuccess) {            // temporaries are released on every path; h->cf[j] belongs to the handle
+        cudaFree(tmat); cudaFree(lev);
+        if (le == cudaErrorMemoryAllocation) { cudaGetLastError(); return PENT_ERR_ALLOC; }
+        return cuda_fail(le);
+    }
     const int tb = 32, nb = (Pl * Q + tb - 1) / tb;
     build_chunk_tables_kernel<T><<<nb, tb, 0, s>>>(h->N, Pl, Q, h->fac, (T*)h->cf[j], tlen, tmat);
     build_chunk_products_kernel<T><<<Q, 32, 0, s>>>(Pl, Q, tmat, (T*)h->cf[j], tlen, lev);
     count_launch(2);
-    cudaError_t le = cudaGetLastError();
+    le = cudaGetLastError();
     int hl[2] = {0, 0};
     if (le == cudaSuccess) le = cudaMemcpyAsync(hl, lev, sizeof(hl), cudaMemcpyDeviceToHost, s);
     if (le == cudaSuccess) le = cudaStreamSynchronize(s);

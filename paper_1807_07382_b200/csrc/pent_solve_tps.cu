@@ -366,11 +366,8 @@ static int factor_solve_impl(int N, int64_t M, const void* e, const void* c, con
                                               scratch, scratch + NM, nullptr, nullptr, nullptr, info);
 #else
     const size_t smem = (size_t)RING_STAGES * RING_SLOTS * PS_THREADS * sizeof(T);
-    static thread_local bool attr_set = false;
-    if (!attr_set) {
-        PENT_CUDA(cudaFuncSetAttribute(factor_solve_ring_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_set = true;
-    }
+    static thread_local SmemMark mark;
+    PENT_CUDA(ensure_dynamic_smem(mark, factor_solve_ring_kernel<T>, smem));
     factor_solve_ring_kernel<T><<<nb, tb, smem, s>>>(N, M, (const T*)a, (const T*)b, (const T*)c, (const T*)d,
                                                      (const T*)e, (const T*)f, (T*)x, scratch, scratch + NM, info);
 #endif

@@ -292,11 +292,8 @@ static int launch_step_inst(const pent_handle* h, const StepPlan& sp, const pent
         return PENT_ERR_CUDA;
     }
     auto kern = step_chunked_kernel<T, S, KIND, NG>;
-    static thread_local size_t smem_set = 0;
-    if (sp.smem > smem_set) {
-        PENT_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sp.smem));
-        smem_set = sp.smem;
-    }
+    static thread_local SmemMark mark;
+    PENT_CUDA(ensure_dynamic_smem(mark, kern, sp.smem));
     const int threads = sp.TG * NG;
     int dev = 0, nsm = 0, occ = 0;
     PENT_CUDA(cudaGetDevice(&dev));
