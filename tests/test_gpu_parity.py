@@ -279,3 +279,24 @@ def test_auto_choice_is_on_chip_for_every_config_shape():
         h = pent.pent_factor(N, e, c, d, a, b)
         ch = pent.kernel_choice(h, M)
         assert ch["kernel"] == "solve_chunked_kernel", (N, M, ch)
+
+
+# ---- tridiagonal systems (cuThomasBatch's case) through the same path ----
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("N,M", [(1024, 4096), (300, 130), (4096, 64)])
+def test_tridiagonal_special_case_matches_textbook_thomas(kernel, N, M):
+    """a = e = 0: the extended Thomas algorithm reduces to the Thomas algorithm.  The GPU result is
+    compared with the oracle AND with LAPACK's banded solver on the tridiagonal matrix."""
+    from scipy.linalg import solve_banded
+    a, b, c, d, e = pin.random_diag_dominant(500 + N, N)
+    a[:] = 0.0
+    e[:] = 0.0
+    f = pin.uniform_pm1(501 + N, 0, N, M)
+    x, _ = gpu_solve((a, b, c, d, e), f, kernel=kernel)
+    ref = oracle.solve_batch(oracle.factor(a, b, c, d, e), f, nthreads=8)
+    assert normwise(x, ref) <= 1e-11
+    ab = np.zeros((3, N))
+    ab[0, 1:] = d[:-1]
+    ab[1] = c
+    ab[2, :-1] = b[1:]
+    assert normwise(x, solve_banded((1, 1), ab, f)) <= 1e-11
