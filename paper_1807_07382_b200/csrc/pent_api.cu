@@ -45,9 +45,48 @@ extern "C" int pent_solve_batch(const pent_handle* h, int64_t M, const void* f, 
 
 // Host buffers: the batch is cut into slabs of consecutive systems.  A slab of an interleaved
 // (N x M) array is a strided 2-D region (N rows of Ms elements, pitch M), moved with
-// cudaMemcpy2DAsync into a dense (N x Ms) device array, solved there and moved back.  Three
-// slabs rotate over three streams so the upload of slab j+1, the solve of slab j and the
-// download of slab j-1 overlap (PCIe is full duplex).
+// cudaMemcpy2DAsync into a dense (N x Ms) device array, solved there and moved back.  NB slabs
+// rotate over NB streams so the upload of slab j+1, the solve of slab j and the download of slab
+// j-1 overlap (PCIe is full duplex).  The staging buffers and streams are a per-thread cache (a call
+// used to spend ~1 ms of its 14 ms in cudaMalloc / cudaFree); they hold no state between calls.
+namespace {
+constexpr int NB = 4;
+struct HostPipe {
+    int dev = -1;
+    size_t cap = 0;                      // bytes per buffer
+    void* buf[NB] = {};
+    cudaStream_t st[NB] = {};
+    void release()
+    {
+        for (int j = 0; j < NB; ++j) {
+            if (buf[j]) cudaFree(buf[j]);
+            if (st[j]) cudaStreamDestroy(st[j]);
+            buf[j] = nullptr; st[j] = nullptr;
+        }
+        cap = 0; dev = -1;
+        cudaGetLastError();              // at thread exit the context may already be gone
+    }
+    ~HostPipe() { release(); }
+    int ensure(size_t bytes)
+    {
+        int d = 0;
+        cudaError_t e = cudaGetDevice(&d);
+        if (e != cudaSuccess) return pent::cuda_fail(e);
+        if (d == dev && bytes <= cap) return PENT_OK;
+        release();
+        for (int j = 0; j < NB; ++j) {
+            e = cudaMalloc(&buf[j], bytes);
+            if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); release(); return PENT_ERR_ALLOC; }
+            if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&st[j], cudaStreamNonBlocking);
+            if (e != cudaSuccess) { release(); return pent::cuda_fail(e); }
+        }
+        dev = d; cap = bytes;
+        return PENT_OK;
+    }
+};
+thread_local HostPipe g_pipe;
+}  // namespace
+
 extern "C" int pent_solve_batch_host(const pent_handle* h, int64_t M, const void* f_host,
                                      void* x_host)
 {
@@ -56,46 +95,29 @@ extern "C" int pent_solve_batch_host(const pent_handle* h, int64_t M, const void
     if (!f_host || !x_host) return PENT_ERR_ARG;
     const size_t esz = h->dtype == PENT_F64 ? 8 : 4;
     const int N = h->N;
-    // ~32 MiB slabs, a multiple of 256 systems
-    int64_t Ms = std::max<int64_t>(256, ((32ll << 20) / ((int64_t)N * (int64_t)esz)) / 256 * 256);
+    // ~16 MiB slabs, a multiple of 256 systems (keeps the slab pitch 16-byte aligned for TMA)
+    int64_t Ms = std::max<int64_t>(256, ((16ll << 20) / ((int64_t)N * (int64_t)esz)) / 256 * 256);
     Ms = std::min(Ms, M);
-    const int NB = 3;
-    void* buf[NB] = {nullptr, nullptr, nullptr};
-    cudaStream_t st[NB] = {nullptr, nullptr, nullptr};
-    int rc = PENT_OK;
-    auto cleanup = [&]() {
-        for (int j = 0; j < NB; ++j) {
-            if (st[j]) { cudaStreamSynchronize(st[j]); cudaStreamDestroy(st[j]); }
-            cudaFree(buf[j]);
-        }
-    };
-    for (int j = 0; j < NB && rc == PENT_OK; ++j) {
-        cudaError_t e = cudaMalloc(&buf[j], (size_t)N * (size_t)Ms * esz);
-        if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); rc = PENT_ERR_ALLOC; break; }
-        if (e != cudaSuccess) { rc = pent::cuda_fail(e); break; }
-        e = cudaStreamCreateWithFlags(&st[j], cudaStreamNonBlocking);
-        if (e != cudaSuccess) rc = pent::cuda_fail(e);
-    }
+    int rc = g_pipe.ensure((size_t)N * (size_t)Ms * esz);
+    if (rc != PENT_OK) return rc;
     int64_t slab = 0;
     for (int64_t i0 = 0; i0 < M && rc == PENT_OK; i0 += Ms, ++slab) {
-        int j = (int)(slab % NB);
-        int64_t m = std::min(Ms, M - i0);
+        const int j = (int)(slab % NB);
+        const int64_t m = std::min(Ms, M - i0);
         const char* src = (const char*)f_host + (size_t)i0 * esz;
         char* dst = (char*)x_host + (size_t)i0 * esz;
-        cudaError_t e = cudaMemcpy2DAsync(buf[j], (size_t)m * esz, src, (size_t)M * esz,
-                                          (size_t)m * esz, (size_t)N, cudaMemcpyHostToDevice, st[j]);
+        cudaError_t e = cudaMemcpy2DAsync(g_pipe.buf[j], (size_t)m * esz, src, (size_t)M * esz,
+                                          (size_t)m * esz, (size_t)N, cudaMemcpyHostToDevice, g_pipe.st[j]);
         if (e != cudaSuccess) { rc = pent::cuda_fail(e); break; }
-        rc = pent_solve_batch(h, m, buf[j], buf[j], st[j]);
+        rc = pent_solve_batch(h, m, g_pipe.buf[j], g_pipe.buf[j], g_pipe.st[j]);
         if (rc != PENT_OK) break;
-        e = cudaMemcpy2DAsync(dst, (size_t)M * esz, buf[j], (size_t)m * esz, (size_t)m * esz,
-                              (size_t)N, cudaMemcpyDeviceToHost, st[j]);
+        e = cudaMemcpy2DAsync(dst, (size_t)M * esz, g_pipe.buf[j], (size_t)m * esz, (size_t)m * esz,
+                              (size_t)N, cudaMemcpyDeviceToHost, g_pipe.st[j]);
         if (e != cudaSuccess) { rc = pent::cuda_fail(e); break; }
     }
-    for (int j = 0; j < NB; ++j)
-        if (st[j]) {
-            cudaError_t e = cudaStreamSynchronize(st[j]);
-            if (e != cudaSuccess && rc == PENT_OK) rc = pent::cuda_fail(e);
-        }
-    cleanup();
+    for (int j = 0; j < NB; ++j) {
+        cudaError_t e = cudaStreamSynchronize(g_pipe.st[j]);
+        if (e != cudaSuccess && rc == PENT_OK) rc = pent::cuda_fail(e);
+    }
     return rc;
 }
