@@ -300,3 +300,53 @@ def test_tridiagonal_special_case_matches_textbook_thomas(kernel, N, M):
     ab[1] = c
     ab[2, :-1] = b[1:]
     assert normwise(x, solve_banded((1, 1), ab, f)) <= 1e-11
+
+
+# ---- maximum sizes and concurrency -----------------------------------------------------------------
+def test_batch_beyond_2_pow_32_elements_in_place():
+    """N*M = 2^32 elements (fp32, 16 GiB, solved in place): element offsets no longer fit 32 bits.
+    The batch is a seeded 4096-system block repeated along M; the oracle solves the block once and
+    first / middle / last repeats are compared (every repeat must also equal the first bit for bit)."""
+    pent = _pent()
+    N, Mb, reps = 4096, 4096, 256
+    M = Mb * reps
+    if torch.cuda.mem_get_info()[0] < 20 * 2 ** 30:
+        pytest.skip("needs 20 GiB of free device memory")
+    diags = pin.diagonals_I_plus_sigma_L2(N, 0.5)
+    fb = pin.uniform_pm1(97, 0, N, Mb).astype(np.float32)
+    a, b, c, d, e = (torch.tensor(v, dtype=torch.float32) for v in diags)
+    h = pent.pent_factor(N, e, c, d, a, b)
+    fd = torch.tensor(fb, device="cuda").repeat(1, reps).contiguous()
+    assert fd.shape == (N, M) and fd.numel() == 2 ** 32
+    pent.pent_solve_batch(h, M, fd, fd)
+    torch.cuda.synchronize()
+    d64 = tuple(np.asarray(v, dtype=np.float32).astype(np.float64) for v in diags)
+    ref = oracle.solve_batch(oracle.factor(*d64), fb.astype(np.float64), nthreads=8)
+    first = fd[:, :Mb].cpu().numpy()
+    assert normwise(first.astype(np.float64), ref) <= 2e-5
+    for r in (reps // 2, reps - 1):
+        assert torch.equal(fd[:, r * Mb:(r + 1) * Mb], fd[:, :Mb])
+    del fd
+    torch.cuda.empty_cache()
+
+
+def test_one_handle_on_two_streams():
+    """Handles are immutable: the same handle serves concurrent launches on different streams."""
+    pent = _pent()
+    N, M = 1024, 8192
+    diags = pin.diagonals_I_plus_sigma_L2(N, 10.0)
+    a, b, c, d, e = (torch.tensor(v) for v in diags)
+    h = pent.pent_factor(N, e, c, d, a, b)
+    f1 = pin.uniform_pm1(98, 0, N, M)
+    f2 = pin.uniform_pm1(99, 0, N, M)
+    d1, d2 = torch.tensor(f1, device="cuda"), torch.tensor(f2, device="cuda")
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    torch.cuda.synchronize()
+    outs = []
+    for _ in range(4):
+        outs.append((pent.pent_solve_batch(h, M, d1, stream=s1), pent.pent_solve_batch(h, M, d2, stream=s2)))
+    torch.cuda.synchronize()
+    fac = oracle.factor(*diags)
+    r1, r2 = oracle.solve_batch(fac, f1, nthreads=8), oracle.solve_batch(fac, f2, nthreads=8)
+    for x1, x2 in outs:
+        assert normwise(x1.cpu().numpy(), r1) <= 1e-11 and normwise(x2.cpu().numpy(), r2) <= 1e-11
