@@ -477,7 +477,7 @@ def run_per_system_workload(args, w, rank, world, local):
     f = torch.tensor(make_rhs(w), dtype=tdt, device="cuda")
     x = torch.empty_like(f)
     info = torch.zeros(M, dtype=torch.int32, device="cuda")
-    ws = torch.empty(2 * N * M, dtype=tdt, device="cuda")
+    ws = torch.empty(3 * N * ((M + 63) // 64 * 64), dtype=tdt, device="cuda")
     stream = torch.cuda.current_stream()
     for _ in range(max(args.warmup, 3)):
         pent.pent_factor_solve_batch(N, M, e, c, d, a, b, f, x, info, workspace=ws)

@@ -114,7 +114,8 @@ int pent_handle_periodic(const pent_handle* h);          /* 1 for a periodic han
 int pent_factor_solve_batch(int N, int64_t M, const void* e, const void* c, const void* d,
                             const void* a, const void* b, const void* f, void* x,
                             pent_dtype dtype, int* info, void* stream);
-/* Same with a caller-owned workspace: device, 2*N*M elements (gamma_k, delta_k of every system),
+/* Same with a caller-owned workspace: device, 3*N*M' elements, M' = M rounded up to a multiple of 64
+ * (gamma_k, delta_k, g_k of every system, in a block-contiguous layout),
  * or NULL (the library then allocates and frees a stream-ordered temporary on every call). */
 int pent_factor_solve_batch_ws(int N, int64_t M, const void* e, const void* c, const void* d,
                                const void* a, const void* b, const void* f, void* x,

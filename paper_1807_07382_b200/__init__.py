@@ -202,7 +202,7 @@ def pent_solve_batch_host(h: Handle, M: int, f_host: torch.Tensor,
 def pent_factor_solve_batch(N: int, M: int, e, c, d, a, b, f, x=None, info=None, stream=None,
                             workspace=None):
     """Per-system matrices, factor + solve fused.  All tensors (N, M) on CUDA.
-    workspace: optional CUDA tensor of 2*N*M elements.  Returns (x, info) with info int32[M]:
+    workspace: optional CUDA tensor of 3*N*M' elements, M' = M rounded up to a multiple of 64.  Returns (x, info) with info int32[M]:
     0 or first bad row + 1."""
     for t, n in zip((e, c, d, a, b, f), "ecdabf"):
         _batch(t, n)
@@ -213,8 +213,8 @@ def pent_factor_solve_batch(N: int, M: int, e, c, d, a, b, f, x=None, info=None,
     if info is None:
         info = torch.zeros(M, dtype=torch.int32, device=f.device)
     if workspace is not None and (not workspace.is_cuda or workspace.dtype != f.dtype or
-                                  workspace.numel() < 2 * N * M or not workspace.is_contiguous()):
-        raise ValueError("workspace: contiguous CUDA tensor of >= 2*N*M elements of f's dtype expected")
+                                  workspace.numel() < 3 * N * ((M + 63) // 64 * 64) or not workspace.is_contiguous()):
+        raise ValueError("workspace: contiguous CUDA tensor of >= 3*N*roundup(M, 64) elements of f's dtype expected")
     _check(lib().pent_factor_solve_batch_ws(N, M, e.data_ptr(), c.data_ptr(), d.data_ptr(),
                                             a.data_ptr(), b.data_ptr(), f.data_ptr(), x.data_ptr(),
                                             _dt(f), info.data_ptr(),

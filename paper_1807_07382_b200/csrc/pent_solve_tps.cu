@@ -185,7 +185,7 @@ template <typename T>
 __global__ void __launch_bounds__(PS_THREADS)
 factor_solve_ring_kernel(int N, int64_t M, const T* __restrict__ a, const T* __restrict__ b,
                          const T* __restrict__ c, const T* __restrict__ d, const T* __restrict__ e,
-                         const T* f, T* x, T* gam, T* del, int* __restrict__ info)
+                         const T* f, T* x, T* __restrict__ scratch, int* __restrict__ info)
 {
     constexpr int R = RING_ROWS, NST = RING_STAGES, TB = PS_THREADS;
     extern __shared__ __align__(16) unsigned char ring_raw[];
@@ -194,6 +194,10 @@ factor_solve_ring_kernel(int N, int64_t M, const T* __restrict__ a, const T* __r
     if (i >= M) i = M - 1;                                // tail threads redo the last system (no divergent exits)
     const bool writer = ((int64_t)blockIdx.x * TB + threadIdx.x) < M;
     T* mine = ring + threadIdx.x;
+    // gamma_k, delta_k, g_k of this block's systems: [k][3][TB], private to the block and contiguous, so the
+    // six scratch words per unknown (3 written, 3 read back) are sequential DRAM streams, not three more
+    // arrays of pitch M
+    T* sc = scratch + (size_t)blockIdx.x * N * 3 * TB + threadIdx.x;
     auto slot = [&](int stage, int v) -> T* { return mine + (size_t)(stage * RING_SLOTS + v) * TB; };
 
     // ---------------- forward: factor rows and sweep in the same loop ----------------
@@ -242,7 +246,7 @@ factor_solve_ring_kernel(int N, int64_t M, const T* __restrict__ a, const T* __r
                 T ga = fma(-be, de1, dk) * inv;
                 T de = ek * inv;
                 T g = fma(-be, g1, fma(-ak, g2, fk)) * inv;
-                if (writer) { gam[o] = ga; del[o] = de; x[o] = g; }
+                { T* w = sc + (size_t)k * 3 * TB; w[0] = ga; w[TB] = de; w[2 * TB] = g; }
                 g2 = g1; g1 = g;
                 ga2 = ga1; ga1 = ga; de2 = de1; de1 = de;
             }
@@ -251,7 +255,6 @@ factor_solve_ring_kernel(int N, int64_t M, const T* __restrict__ a, const T* __r
     if (info && writer) info[i] = bad;
     cp_async_wait<0>();
     __threadfence();              // this thread's gamma, delta, g are in L2 before it copies them back
-    __syncthreads();              // tail threads share a column with a writer of the same block
 
     // ---------------- backward: x_k = g_k - gamma_k x_{k+1} - delta_k x_{k+2} ----------------
     constexpr int RB = 2 * R;
@@ -264,9 +267,10 @@ factor_solve_ring_kernel(int N, int64_t M, const T* __restrict__ a, const T* __r
                 const int k = N - 1 - (blk * RB + r);
                 if (k >= 0) {
                     const int64_t o = (int64_t)k * M + i;
-                    cp_async_elem(slot(st, 0 * RB + r), gam + o);
-                    cp_async_elem(slot(st, 1 * RB + r), del + o);
-                    cp_async_elem(slot(st, 2 * RB + r), x + o);
+                    const T* w = sc + (size_t)k * 3 * TB;
+                    cp_async_elem(slot(st, 0 * RB + r), w);
+                    cp_async_elem(slot(st, 1 * RB + r), w + TB);
+                    cp_async_elem(slot(st, 2 * RB + r), w + 2 * TB);
                 }
             }
         }
@@ -349,12 +353,12 @@ static int factor_solve_impl(int N, int64_t M, const void* e, const void* c, con
                              const void* a, const void* b, const void* f, void* x, int* info,
                              void* workspace, cudaStream_t s)
 {
-    // gamma_k, delta_k of every system (needed again by the back substitution): 2*N*M elements,
-    // the caller's workspace or a stream-ordered temporary
+    // gamma_k, delta_k, g_k of every system (needed again by the back substitution): 3*N*M' elements,
+    // M' = M rounded up to a multiple of 64; the caller's workspace or a stream-ordered temporary
     T* scratch = (T*)workspace;
     size_t NM = (size_t)N * (size_t)M;
     if (!scratch) {
-        cudaError_t er = cudaMallocAsync((void**)&scratch, 2 * NM * sizeof(T), s);
+        cudaError_t er = cudaMallocAsync((void**)&scratch, 3 * (size_t)N * (size_t)((M + 63) / 64 * 64) * sizeof(T), s);
         if (er == cudaErrorMemoryAllocation) { cudaGetLastError(); return PENT_ERR_ALLOC; }
         PENT_CUDA(er);
     }
@@ -369,7 +373,7 @@ static int factor_solve_impl(int N, int64_t M, const void* e, const void* c, con
     static thread_local SmemMark mark;
     PENT_CUDA(ensure_dynamic_smem(mark, factor_solve_ring_kernel<T>, smem));
     factor_solve_ring_kernel<T><<<nb, tb, smem, s>>>(N, M, (const T*)a, (const T*)b, (const T*)c, (const T*)d,
-                                                     (const T*)e, (const T*)f, (T*)x, scratch, scratch + NM, info);
+                                                     (const T*)e, (const T*)f, (T*)x, scratch, info);
 #endif
     count_launch();
     cudaError_t le = cudaGetLastError();

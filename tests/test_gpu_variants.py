@@ -61,7 +61,7 @@ def test_cfg5b_full_size():
     diags = make_matrix(w)
     f = make_rhs(w)
     a, b, c, d, e = (_dev(v) for v in diags)
-    ws = torch.empty(2 * w.N * w.M, dtype=torch.float64, device="cuda")
+    ws = torch.empty(3 * w.N * ((w.M + 63) // 64 * 64), dtype=torch.float64, device="cuda")
     x, info = pent.pent_factor_solve_batch(w.N, w.M, e, c, d, a, b, _dev(f), workspace=ws)
     x = x.cpu().numpy()
     assert not info.cpu().numpy().any()
