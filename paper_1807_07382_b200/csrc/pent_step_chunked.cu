@@ -106,7 +106,10 @@ step_chunked_kernel(const __grid_constant__ CUtensorMap tm, const StepChunkParam
     // Warp-uniform choice: a warp that holds one boundary chunk (S=16: two chunks per warp) takes the
     // general path with ALL its lanes instead of executing both paths one after the other; that warp
     // is the straggler every block barrier waits for.
-    const bool interior = __all_sync(0xffffffffu, active && row0 >= 2 && row0 + C + 2 <= N - 1);
+    const bool first = row0 == 0, last = row0 + C == N;
+    const T dfirst = first ? dg_edge : (T)-2, dlast = last ? dg_edge : (T)-2;
+    const bool interior = __all_sync(0xffffffffu, active && (first || row0 >= 2) && (last || row0 + C + 2 <= N - 1) &&
+                                                      C >= 4 && N >= 2 * C);
     uint32_t parity = 0;
 
     for (int64_t tile = (int64_t)blockIdx.x * NG + grp_id; tile < prm.ntiles; tile += (int64_t)gridDim.x * NG) {
@@ -124,22 +127,28 @@ step_chunked_kernel(const __grid_constant__ CUtensorMap tm, const StepChunkParam
                 if constexpr (KIND != 1) {
                     // u_k = w_k = c_k^3 - c_k (form 0) or q_k = r w_k - sigma (L c)_k (form 1), 0 outside 0..N-1
                     if (interior) {
-                        // rows row0-2 .. row0+C+1 all exist and none is a boundary row: no range checks
-                        auto U = [&](T cl, T cc, T cr) -> T {
+                        // Interior chunk, or the first / last chunk of a system whose length is a multiple
+                        // of C: the special rows then sit at compile-time positions (j = -1, 0 and C-1, C),
+                        // so the loop body carries no range checks; `dfirst`, `dlast` are the diagonal
+                        // entries of L at rows row0 and row0+C-1 (-2 unless that row is 0 or N-1).
+                        auto U = [&](T cl, T cc, T cr, T dg) -> T {
                             T w = cc * cc * cc - cc;
                             if (!incr) return w;
-                            return fma(-sigma, cl + fma((T)-2, cc, cr), r * w);
+                            return fma(-sigma, cl + fma(dg, cc, cr), r * w);
                         };
-                        const T* cw = cs + (size_t)(row0 - 2) * S;
-                        T cl = cw[0], cc = cw[S], cr = cw[2 * S];
-                        T u_prev = U(cl, cc, cr);
-                        cl = cc; cc = cr; cr = cw[3 * S];
-                        T u_cur = U(cl, cc, cr);
+                        const T* cw = cs + (size_t)row0 * S;          // cw[j*S] = c_{row0+j}
+                        T cl = first ? (T)0 : *(cw - 2 * S), cc = first ? (T)0 : *(cw - S), cr = cw[0];
+                        T u_prev = first ? (T)0 : U(cl, cc, cr, (T)-2);                    // u_{row0-1}
+                        cl = cc; cc = cr; cr = cw[S];
+                        T u_cur = U(cl, cc, cr, dfirst);                                   // u_{row0}
 #pragma unroll
                         for (int j = 0; j < C; ++j) {
-                            cl = cc; cc = cr; cr = cw[(j + 4) * S];     // window centred on row0+j+1; cl = c_{row0+j}
-                            T u_next = U(cl, cc, cr);
-                            T Lu = u_prev + fma((T)-2, u_cur, u_next);
+                            cl = cc; cc = cr;                                              // cl = c_{row0+j}, cc = c_{row0+j+1}
+                            if (j + 2 < C) cr = cw[(j + 2) * S];
+                            else cr = last ? (T)0 : cw[(j + 2) * S];                       // rows N, N+1 do not exist
+                            T u_next = U(cl, cc, cr, (j + 1 == C - 1) ? dlast : (T)-2);    // u_{row0+j+1}
+                            if (j == C - 1 && last) u_next = 0;                            // u_N
+                            T Lu = u_prev + fma(j == 0 ? dfirst : (j == C - 1 ? dlast : (T)-2), u_cur, u_next);
                             v[j] = incr ? Lu : fma(r, Lu, cl);
                             u_prev = u_cur; u_cur = u_next;
                         }
