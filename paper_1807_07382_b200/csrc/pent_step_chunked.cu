@@ -173,6 +173,25 @@ step_chunked_kernel(const __grid_constant__ CUtensorMap tm, const StepChunkParam
                             u_prev = u_cur; u_cur = u_next;
                         }
                     }
+                } else if (interior) {
+                    // (2I - A) c, rows row0 .. row0+C-1 all inside the matrix (see `interior` above); the
+                    // entries of the diagonals that fall outside the matrix are zero in prm.dg
+                    const T* cw = cs + (size_t)row0 * S;
+                    T cm2 = first ? (T)0 : *(cw - 2 * S), cm1 = first ? (T)0 : *(cw - S), c0 = cw[0], cp1 = cw[S];
+                    const T* dk = prm.dg + 8 * (size_t)row0;
+#pragma unroll
+                    for (int j = 0; j < C; ++j) {
+                        T cp2;
+                        if (j + 2 < C) cp2 = cw[(j + 2) * S];
+                        else cp2 = last ? (T)0 : cw[(j + 2) * S];
+                        T s = __ldg(dk + 8 * j + 2) * c0;
+                        s = fma(__ldg(dk + 8 * j + 1), cm1, s);
+                        s = fma(__ldg(dk + 8 * j + 0), cm2, s);
+                        s = fma(__ldg(dk + 8 * j + 3), cp1, s);
+                        s = fma(__ldg(dk + 8 * j + 4), cp2, s);
+                        v[j] = (T)2 * c0 - s;
+                        cm2 = cm1; cm1 = c0; c0 = cp1; cp1 = cp2;
+                    }
                 } else {
                     T cm2 = ldc(row0 - 2), cm1 = ldc(row0 - 1), c0 = ldc(row0), cp1 = ldc(row0 + 1);
 #pragma unroll
