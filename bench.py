@@ -43,6 +43,8 @@ def parse_args():
     ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 thread-per-system, 2 chunked")
     ap.add_argument("--cluster", type=int, default=0, help="chunked kernel: CTAs per cluster along k (0 auto)")
     ap.add_argument("--tile", type=int, default=0, help="chunked kernel: systems per tile (0 auto)")
+    ap.add_argument("--layout", default="interleaved", choices=["interleaved", "rows"],
+                    help="rows: system-major batch through pent_solve_batch_rows")
     ap.add_argument("--systems", type=int, default=0, help="override M of the workload (shape experiments)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -235,6 +237,12 @@ def run_ours(args):
     fd = f_host.cuda()
     xd = torch.empty_like(fd)
     stream = torch.cuda.current_stream()
+    if args.layout == "rows":
+        fd = fd.t().contiguous()
+        xd = torch.empty_like(fd)
+        solve = lambda: pent.pent_solve_batch_rows(h, M, fd, xd)
+    else:
+        solve = lambda: pent.pent_solve_batch(h, M, fd, xd, kernel=args.kernel)
     if args.cluster or args.tile:
         args.kernel = pent.KERNEL_CHUNKED_CFG(args.cluster, args.tile)
 
@@ -244,7 +252,7 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     for _ in range(max(args.warmup, 3)):
-        pent.pent_solve_batch(h, M, fd, xd, kernel=args.kernel)
+        solve()
     barrier()
     sampler = ClockSampler(local)
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -254,7 +262,7 @@ def run_ours(args):
     # (an event between launches costs 2-3 us of stream latency: 10 % of a 28 us cfg2 kernel)
     ev0.record(stream)
     for i in range(args.steps):
-        pent.pent_solve_batch(h, M, fd, xd, kernel=args.kernel)
+        solve()
     ev1.record(stream)
     barrier()
     clocks = sampler.stop()
@@ -265,7 +273,7 @@ def run_ours(args):
     evs = [torch.cuda.Event(enable_timing=True) for _ in range(nper + 1)]
     evs[0].record(stream)
     for i in range(nper):
-        pent.pent_solve_batch(h, M, fd, xd, kernel=args.kernel)
+        solve()
         evs[i + 1].record(stream)
     barrier()
     per = np.array([evs[i].elapsed_time(evs[i + 1]) for i in range(nper)])
@@ -313,7 +321,7 @@ def run_ours(args):
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": args.dtype,
         "data": "synthetic",
         "config": {"workload": w.name, "N": N, "M_per_gpu": M, "matrix": f"I+sigma*L^2 {w.bc} sigma={w.sigma}",
-                   "rhs": w.rhs, "seed": w.seed, "layout": "interleaved f[k*M+i]", "kernel": kname,
+                   "rhs": w.rhs, "seed": w.seed, "layout": "interleaved f[k*M+i]" if args.layout == "interleaved" else "system-major f[i*N+k]", "kernel": kname,
                    "cluster_ctas_along_k": ch["Q"], "systems_per_tile": ch["S"],
                    "l2": f"inputs+outputs {2 * esz * N * M >> 20} MiB per step exceed the 126 MB L2"},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",

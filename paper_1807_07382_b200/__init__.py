@@ -70,6 +70,7 @@ def lib() -> C.CDLL:
     L.pent_solve_batch.argtypes = [vp, i64, vp, vp, vp]
     L.pent_solve_batch_v.argtypes = [vp, i64, vp, vp, vp, ci]
     L.pent_solve_batch_host.argtypes = [vp, i64, vp, vp]
+    L.pent_solve_batch_rows.argtypes = [vp, i64, vp, vp, vp]
     L.pent_destroy.argtypes = [vp]
     L.pent_destroy.restype = None
     L.pent_factor_solve_batch.argtypes = [ci, i64, vp, vp, vp, vp, vp, vp, vp, ci, vp, vp]
@@ -185,6 +186,18 @@ def pent_solve_batch(h: Handle, M: int, f: torch.Tensor, x: torch.Tensor | None 
     if f.shape != (h.N, M) or x.shape != f.shape or f.dtype != h.dtype or x.dtype != h.dtype:
         raise ValueError("f/x must have shape (N, M) and the handle's dtype")
     _check(lib().pent_solve_batch_v(h.ptr, M, f.data_ptr(), x.data_ptr(), _stream(stream), kernel))
+    return x
+
+
+def pent_solve_batch_rows(h: Handle, M: int, f: torch.Tensor, x: torch.Tensor | None = None, stream=None) -> torch.Tensor:
+    """Same solve on a system-major batch: f, x of shape (M, N), one system per row."""
+    _batch(f, "f")
+    if x is None:
+        x = torch.empty_like(f)
+    _batch(x, "x")
+    if f.shape != (M, h.N) or x.shape != f.shape or f.dtype != h.dtype or x.dtype != h.dtype:
+        raise ValueError("f/x must have shape (M, N) and the handle's dtype")
+    _check(lib().pent_solve_batch_rows(h.ptr, M, f.data_ptr(), x.data_ptr(), _stream(stream)))
     return x
 
 

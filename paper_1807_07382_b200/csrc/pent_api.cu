@@ -28,6 +28,17 @@ extern "C" int pent_solve_batch_v(const pent_handle* h, int64_t M, const void* f
     }
 }
 
+// System-major batches ("one system per row", the layout of the paper's serial code; also
+// the access an ADI sweep along the contiguous axis of a 2-D field needs).
+extern "C" int pent_solve_batch_rows(const pent_handle* h, int64_t M, const void* f, void* x, void* stream)
+{
+    if (!h || h->kind != 0 || h->periodic || M < 0) return PENT_ERR_ARG;
+    if (M == 0) return PENT_OK;
+    if (!f || !x) return PENT_ERR_ARG;
+    if (!pent::chunked_rows_supported(h, M)) return PENT_ERR_ARG;      // N too long to keep a tile on chip
+    return pent::launch_solve_chunked_rows(h, M, f, x, (cudaStream_t)stream);
+}
+
 extern "C" int pent_solve_kernel_choice(const pent_handle* h, int64_t M)
 {
     if (!h || h->kind != 0) return -1;

@@ -418,7 +418,8 @@ __device__ __forceinline__ void chunk_state_scan(const ScanGeom& g, const T* wta
 struct ChunkPlan {
     bool ok = false;
     int j = 0, Q = 1, S = 0, Pl = 0, Pw = 1, threads = 0, levels = 0, box_rows = 0, nbox = 0;
-    bool ldg = false;          // LDG loader instead of TMA (pitch not a multiple of 16 bytes)
+    bool ldg = false;          // LDG loader instead of TMA (pitch not a multiple of 16 bytes, or system-major batch)
+    bool rows = false;         // system-major batch: implies ldg
     size_t table_bytes = 0, smem = 0;
 };
 // any_S: accept tile widths the SOLVE kernel is not instantiated for (the step kernel has its own)

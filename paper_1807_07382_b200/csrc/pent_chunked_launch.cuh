@@ -39,7 +39,7 @@ static int launch_inst(const pent_handle* h, const ChunkPlan& pl, int64_t M, con
     prm.table_bytes = (uint32_t)pl.table_bytes;
     prm.x = (T*)x;
     prm.f = (const T*)f;
-    prm.ldg = pl.ldg ? 1 : 0;
+    prm.ldg = pl.rows ? 2 : (pl.ldg ? 1 : 0);
 
     CUtensorMap tm = {};
     if (!pl.ldg && !encode_batch_map(&tm, f, M, h->N, S, prm.box_rows, sizeof(T) == 8)) {

@@ -382,11 +382,46 @@ int chunked_choice(const pent_handle* h, int64_t M, int* Q, int* S)
     return 1;
 }
 
+// System-major batch (element k of system i at f[i*N + k]): the chunked kernel with its per-thread
+// contiguous loader.  CTAs of <= 256 threads are preferred (no prefetch: two CTAs per SM overlap).
+static ChunkPlan rows_plan(const pent_handle* h, int64_t M)
+{
+    if (!h || h->kind != 0 || h->periodic) return ChunkPlan{};
+    const int Sn = h->dtype == PENT_F64 ? 16 : 32, QMAX = 1 << (PENT_NQ - 1);
+    ChunkPlan best;
+    for (int Q = 1; Q <= QMAX && !best.ok; Q *= 2) {
+        ChunkPlan pl = make_plan(h, M, nullptr, Q, Sn, false, true);
+        if (pl.ok && pl.threads <= 256) best = pl;
+    }
+    for (int Q = 1; Q <= QMAX && !best.ok; Q *= 2) {
+        ChunkPlan pl = make_plan(h, M, nullptr, Q, Sn, false, true);
+        if (pl.ok) best = pl;
+    }
+    best.rows = best.ok;
+    return best;
+}
+
+bool chunked_rows_supported(const pent_handle* h, int64_t M) { return rows_plan(h, M).ok; }
+
+static int launch_plan(const pent_handle* h, const ChunkPlan& pl, int64_t M, const void* f, void* x, cudaStream_t s);
+
+int launch_solve_chunked_rows(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s)
+{
+    const ChunkPlan pl = rows_plan(h, M);
+    if (!pl.ok) return PENT_ERR_ARG;
+    return launch_plan(h, pl, M, f, x, s);
+}
+
 int launch_solve_chunked(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s,
                          int Q, int S)
 {
     const ChunkPlan pl = resolve_plan(h, M, f, Q, S);
     if (!pl.ok) return PENT_ERR_ARG;
+    return launch_plan(h, pl, M, f, x, s);
+}
+
+static int launch_plan(const pent_handle* h, const ChunkPlan& pl, int64_t M, const void* f, void* x, cudaStream_t s)
+{
     const bool cl = pl.Q > 1;
     if (h->dtype == PENT_F64) {
         if (pl.S == 16) return cl ? launch_inst<double, 16, true, false>(h, pl, M, f, x, s, nullptr) : launch_inst<double, 16, false, false>(h, pl, M, f, x, s, nullptr);

@@ -350,3 +350,42 @@ def test_one_handle_on_two_streams():
     r1, r2 = oracle.solve_batch(fac, f1, nthreads=8), oracle.solve_batch(fac, f2, nthreads=8)
     for x1, x2 in outs:
         assert normwise(x1.cpu().numpy(), r1) <= 1e-11 and normwise(x2.cpu().numpy(), r2) <= 1e-11
+
+
+# ---- system-major batches ("one system per row"; the transposed access of an ADI sweep) ----
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("N,M", [(1024, 2048 + 17), (512, 333), (64, 40), (4096, 96), (1000, 130), (33, 7), (2047, 65)])
+def test_system_major_layout_parity(dtype, N, M):
+    pent = _pent()
+    diags = pin.random_diag_dominant(600 + N, N)
+    f = pin.uniform_pm1(601 + N, 0, N, M)                      # interleaved (N, M)
+    a, b, c, d, e = (torch.tensor(v, dtype=dtype) for v in diags)
+    h = pent.pent_factor(N, e, c, d, a, b)
+    f_rows = torch.tensor(np.ascontiguousarray(f.T), dtype=dtype, device="cuda")     # (M, N), one system per row
+    x_rows = pent.pent_solve_batch_rows(h, M, f_rows)
+    d64, f64, ref = oracle_for_dtype(diags, f, dtype)
+    tol_x, tol_r = TOL[dtype]
+    x = x_rows.cpu().numpy().T
+    assert normwise(x.astype(np.float64), ref) <= tol_x
+    assert residual(d64, np.ascontiguousarray(x), f64) <= tol_r
+    # in place, and identical to the interleaved solve of the same systems (same kernel arithmetic)
+    pent.pent_solve_batch_rows(h, M, f_rows, f_rows)
+    assert torch.equal(f_rows, x_rows)
+
+
+def test_adi_like_two_axis_sweeps_on_a_2d_field():
+    """A 2-D field u[y][x] (row-major): the sweep along x solves every ROW (system-major batch), the sweep
+    along y solves every COLUMN (interleaved batch, the library's native layout)."""
+    pent = _pent()
+    Ny, Nx = 512, 768
+    u = pin.uniform_pm1(77, 0, Ny, Nx)
+    dx_ = pin.diagonals_I_plus_sigma_L2(Nx, 3.0)
+    dy_ = pin.diagonals_I_plus_sigma_L2(Ny, 0.7)
+    hx = pent.pent_factor(Nx, *(torch.tensor(v) for v in (dx_[4], dx_[2], dx_[3], dx_[0], dx_[1])))
+    hy = pent.pent_factor(Ny, *(torch.tensor(v) for v in (dy_[4], dy_[2], dy_[3], dy_[0], dy_[1])))
+    ud = torch.tensor(u, device="cuda")
+    pent.pent_solve_batch_rows(hx, Ny, ud, ud)        # x-sweep: Ny systems of length Nx, each a row
+    pent.pent_solve_batch(hy, Nx, ud, ud)             # y-sweep: Nx systems of length Ny, interleaved
+    ref = oracle.solve_rows(oracle.factor(*dx_), np.ascontiguousarray(u), nthreads=8)        # rows
+    ref = oracle.solve_batch(oracle.factor(*dy_), ref, nthreads=8)                           # columns
+    assert normwise(ud.cpu().numpy(), ref) <= 1e-11
