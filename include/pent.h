@@ -84,7 +84,8 @@ int pent_solve_batch_v(const pent_handle* h, int64_t M, const void* f, void* x, 
  * sweep along the contiguous axis of a 2-D field needs: the sweep along the other axis is
  * pent_solve_batch itself).  x == f allowed.  Shared-A, non-periodic handles with N <= 8192 (fp64);
  * PENT_ERR_ARG otherwise.  Every thread reads and writes one contiguous run of 32 (fp64) / 64 (fp32)
- * elements with 16-byte accesses: 2 passes over the batch, no transpose. */
+ * elements with 32-byte accesses (16-byte aligned runs fall back to narrower ones): 2 passes over the
+ * batch, no transpose. */
 int pent_solve_batch_rows(const pent_handle* h, int64_t M, const void* f, void* x, void* stream);
 
 /* Same operation with HOST buffers (pageable or pinned): copies slabs of systems to the device,

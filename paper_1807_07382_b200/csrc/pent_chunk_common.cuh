@@ -109,6 +109,27 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N_>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N_) : "memory"); }
 
+// 32 bytes per thread in one global access (LDG.256 / STG.256, sm_100): a whole DRAM sector per lane, so a
+// lane that walks a contiguous run never splits a sector between two requests.  addr must be 32-byte aligned.
+__device__ __forceinline__ void ldg256(double (&o)[4], const double* p)
+{
+    asm volatile("ld.global.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(o[0]), "=d"(o[1]), "=d"(o[2]), "=d"(o[3]) : "l"(p));
+}
+__device__ __forceinline__ void ldg256(float (&o)[8], const float* p)
+{
+    asm volatile("ld.global.v8.f32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                 : "=f"(o[0]), "=f"(o[1]), "=f"(o[2]), "=f"(o[3]), "=f"(o[4]), "=f"(o[5]), "=f"(o[6]), "=f"(o[7]) : "l"(p));
+}
+__device__ __forceinline__ void stg256(double* p, const double (&v)[4])
+{
+    asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(v[0]), "d"(v[1]), "d"(v[2]), "d"(v[3]) : "memory");
+}
+__device__ __forceinline__ void stg256(float* p, const float (&v)[8])
+{
+    asm volatile("st.global.v8.f32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};"
+                 ::"l"(p), "f"(v[0]), "f"(v[1]), "f"(v[2]), "f"(v[3]), "f"(v[4]), "f"(v[5]), "f"(v[6]), "f"(v[7]) : "memory");
+}
+
 // n consecutive T values from shared memory with 16-byte loads (n*sizeof(T) % 16 == 0)
 template <typename T, int n>
 __device__ __forceinline__ void lds_vec(T (&dst)[n], const T* src)

@@ -163,24 +163,19 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
             }
         }
         if (active) {
-            if (prm.ldg == 2) {
+            if (!PER && prm.ldg == 2) {
                 // ---- system-major batch: this thread's chunk is contiguous in memory ----
                 const int64_t col = tile * S + i;
                 const T* src = prm.f + col * (int64_t)prm.N + row0;
                 const int nrows = col < prm.M ? prm.N - row0 : 0;
-                if (nrows >= C && ((reinterpret_cast<uintptr_t>(src) & 15) == 0)) {
-                    constexpr int V = 16 / sizeof(T);
-                    const uint4* s4 = reinterpret_cast<const uint4*>(src);
+                if (nrows >= C && ((reinterpret_cast<uintptr_t>(src) & 31) == 0)) {
+                    constexpr int W = 32 / sizeof(T);                 // elements per 256-bit access
 #pragma unroll
-                    for (int m = 0; m < C / V; ++m) {
-                        const uint4 w = __ldcs(s4 + m);
-                        if constexpr (sizeof(T) == 8) {
-                            v[2 * m] = __hiloint2double((int)w.y, (int)w.x);
-                            v[2 * m + 1] = __hiloint2double((int)w.w, (int)w.z);
-                        } else {
-                            v[4 * m] = __uint_as_float(w.x); v[4 * m + 1] = __uint_as_float(w.y);
-                            v[4 * m + 2] = __uint_as_float(w.z); v[4 * m + 3] = __uint_as_float(w.w);
-                        }
+                    for (int m = 0; m < C / W; ++m) {
+                        T w[W];
+                        ldg256(w, src + m * W);
+#pragma unroll
+                        for (int u = 0; u < W; ++u) v[m * W + u] = w[u];
                     }
                 } else {
 #pragma unroll
@@ -266,22 +261,21 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
             if (CLUSTER || PER || P > 1) { T2 fo = stE[slot]; F0 = fo.x; F1 = fo.y; T2 bo = stS[slot]; B0 = bo.x; B1 = bo.y; }
             const int64_t col = tile * S + i;
             T* xo = prm.x + (int64_t)row0 * prm.M + col;
-            if (prm.ldg == 2) {
-                // system-major batch: contiguous run of this thread's chunk, 16-byte stores where possible
+            if (!PER && prm.ldg == 2) {
+                // system-major batch: contiguous run of this thread's chunk, 32-byte stores where possible
                 T* xr = prm.x + col * (int64_t)prm.N + row0;
                 const int nrows = col < prm.M ? prm.N - row0 : 0;
-                const bool vec = nrows >= C && ((reinterpret_cast<uintptr_t>(xr) & 15) == 0);
+                const bool vec = nrows >= C && ((reinterpret_cast<uintptr_t>(xr) & 31) == 0);
+                constexpr int W = 32 / sizeof(T);
+                T acc[W];
 #pragma unroll
                 for (int jg = 0; jg < C / 4; ++jg) {
                     T xv[4];
                     chunk_correct4<T>(xv, &v[4 * jg], blk, jg, F0, F1, B0, B1);
                     if (vec) {
-                        if constexpr (sizeof(T) == 8) {
-                            reinterpret_cast<double2*>(xr)[2 * jg] = make_double2(xv[0], xv[1]);
-                            reinterpret_cast<double2*>(xr)[2 * jg + 1] = make_double2(xv[2], xv[3]);
-                        } else {
-                            reinterpret_cast<float4*>(xr)[jg] = make_float4(xv[0], xv[1], xv[2], xv[3]);
-                        }
+#pragma unroll
+                        for (int r = 0; r < 4; ++r) acc[(4 * jg + r) % W] = xv[r];
+                        if ((4 * jg + 4) % W == 0) stg256(xr + (4 * jg + 4 - W), acc);
                     } else {
 #pragma unroll
                         for (int r = 0; r < 4; ++r)
@@ -292,7 +286,7 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
             T t0 = 0, t1 = 0;         // periodic: x^ = y - Z t
             if constexpr (PER) { T2 t = stT[i]; t0 = t.x; t1 = t.y; }
             const T2* zr = zs + (size_t)(active ? p : 0) * C;
-            if (prm.ldg == 2) {
+            if (!PER && prm.ldg == 2) {
                 // stored above
             } else if (rows_full && (tile + 1) * S <= prm.M) {
 #pragma unroll
