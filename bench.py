@@ -127,7 +127,7 @@ class ClockSampler:
                 "samples": len(self.samples)}
 
 
-def cpu_baseline(w, diags, sample_systems: int, budget_s: float = 7.0):
+def cpu_baseline(w, diags, sample_systems: int, budget_s: float = 7.0, x_gpu=None, f32=False):
     """The oracle as it stands, on the host cores, on a bounded sample of the same workload:
     the first `sample_systems` systems, serial layout one system per row,
     transposition outside the timed region.  Passes are repeated for about `budget_s` seconds of CPU
@@ -138,6 +138,9 @@ def cpu_baseline(w, diags, sample_systems: int, budget_s: float = 7.0):
     f = make_rhs(w, M=m)
     if isinstance(f, tuple):
         f = f[0]
+    if f32:                      # the oracle solves the ROUNDED inputs in fp64 (C-9)
+        diags = tuple(np.asarray(v, dtype=np.float32).astype(np.float64) for v in diags)
+        f = f.astype(np.float32).astype(np.float64)
     fac = oracle.factor(*diags)
     rows = oracle.to_rows(f)
     cores = os.cpu_count() or 1
@@ -150,7 +153,14 @@ def cpu_baseline(w, diags, sample_systems: int, budget_s: float = 7.0):
             best = min(best, time.perf_counter() - t0)
             n += 1
         out[label], passes[label] = w.N * m / best, n
-    return {"value": out["allcore"], "unit": UNIT, "cores": cores, "kind": "oracle",
+    extra = {}
+    if x_gpu is not None:        # the timed GPU result against the oracle on the same sample (normwise per system)
+        ref = oracle.solve_rows(fac, rows, nthreads=cores)                       # (m, N)
+        got = x_gpu[:, :m].to("cpu", dtype=__import__("torch").float64).numpy().T
+        extra["gpu_vs_oracle_max_norm_rel_err"] = float(
+            np.max(np.max(np.abs(got - ref), axis=1) / np.max(np.abs(ref), axis=1)))
+        extra["systems_compared"] = int(m)
+    return {**extra, "value": out["allcore"], "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": f"first {m} of {w.M} systems of {w.name} (N={w.N}), serial layout, best of "
                       f"{passes['allcore']} all-core passes (and of {passes['1thread']} 1-thread passes), ~{2 * budget_s:.0f} s of CPU work",
             "value_1thread": out["1thread"]}
@@ -337,7 +347,8 @@ def run_ours(args):
     if e2e is not None:
         line["e2e"] = e2e
     if not args.no_cpu_baseline and world == 1 and not periodic:
-        line["cpu_baseline"] = cpu_baseline(w, diags, 32768)
+        line["cpu_baseline"] = cpu_baseline(w, diags, 32768, x_gpu=xd if args.layout == "interleaved" else xd.t(),
+                                             f32=args.dtype == "f32")
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
