@@ -21,10 +21,20 @@
  *
  * OWNERSHIP: the caller owns every array it passes; a handle owns device copies of whatever
  * it needs and never keeps a caller pointer.  Handles are immutable after creation and may
- * be used from several streams/threads at once.  No hidden global state.
+ * be used from several streams/threads at once.  No hidden global state (per-thread caches of
+ * encoded tensor maps, occupancy answers and the staging buffers of pent_solve_batch_host hold no
+ * results; pent_release_thread_cache frees the latter).
+ *
+ * DEVICE: a handle belongs to the CUDA device that was current when it was created; every call
+ * that takes a handle returns PENT_ERR_ARG if another device is current.
  *
  * ASYNCHRONY: every *_batch call only enqueues work on `stream` and returns; it never
- * synchronises the host.  pent_factor / pent_factor_batch(info on host) synchronise.
+ * synchronises the host (pent_factor_batch included: `info` is device memory).
+ * pent_factor / pent_factor_periodic run on a PRIVATE non-blocking stream and wait for that stream
+ * only: they return with the handle complete, and they neither wait for nor stall any other
+ * stream of the process (device-pointer diagonals must therefore be complete before the call).
+ * pent_solve_batch_host returns when x_host is complete.  pent_destroy synchronises the device
+ * (cudaFree): do not call it while work that uses the handle is in flight.
  *
  * ERRORS: every int function returns one of the codes below; nothing is printed, nothing
  * throws, and there is NO CPU fallback.
@@ -89,8 +99,12 @@ int pent_solve_batch_v(const pent_handle* h, int64_t M, const void* f, void* x, 
 int pent_solve_batch_rows(const pent_handle* h, int64_t M, const void* f, void* x, void* stream);
 
 /* Same operation with HOST buffers (pageable or pinned): copies slabs of systems to the device,
- * solves, copies back, pipelined on internal streams; returns when x_host is complete. */
+ * solves, copies back, pipelined on internal streams; returns when x_host is complete.
+ * M * sizeof(element) must be below 2^31 bytes (the pitch limit of the 2-D copies), else PENT_ERR_ARG.
+ * The staging buffers (4 x 16 MiB of device memory, 4 streams) are cached per calling thread until
+ * the thread exits or calls pent_release_thread_cache(). */
 int pent_solve_batch_host(const pent_handle* h, int64_t M, const void* f_host, void* x_host);
+void pent_release_thread_cache(void);
 
 void pent_destroy(pent_handle* h);          /* NULL is allowed */
 
@@ -115,7 +129,7 @@ int pent_handle_periodic(const pent_handle* h);          /* 1 for a periodic han
 
 /* ---- per-system matrices ("cuPentBatchRewrite") ---------------------------------
  * e,c,d,a,b,f,x: device, N*M elements each, interleaved like f (diagonal entry k of system i at
- * k*M+i).  info: device int[M] or NULL; info[i] = 0, or (first bad row + 1) if system i met a
+ * k*M+i).  x == f (in place) is allowed; any other overlap is undefined.  info: device int[M] or NULL; info[i] = 0, or (first bad row + 1) if system i met a
  * zero / non-finite pivot (its x is then unspecified; other systems are unaffected).
  * pent_factor_solve_batch factors and solves in ONE kernel and keeps nothing.
  * pent_factor_batch keeps the M factorisations in the handle (5*N*M elements of device memory)
@@ -147,7 +161,9 @@ int pent_solve_batch_multi(const pent_handle* h, const void* f, void* x, void* s
  *  kind 1, hyperdiffusion Crank-Nicolson (PAPER.md:87-89 Eq. 6, :117 Eq. 7c):
  *     A c+ = (2I - A) c, with the handle's own diagonals (bc, form, r, sigma ignored).
  *  bc 0: Dirichlet L (diag -2, off 1).  bc 1: zero-flux L (corner diagonal entries -1).
- *  The handle's A must be the matching I + sigma L^2 for kind 0; this is the caller's contract.
+ *  kind 0, form 1 is the scheme of Eq. 2 only if the handle's A IS I + sigma L^2 with this sigma and bc:
+ *  pent_factor records whether its matrix has that form (and which sigma, bc), and the call returns
+ *  PENT_ERR_ARG on a mismatch (relative tolerance 1e-12 fp64, 1e-6 fp32).  form 0 takes any A.
  * c_inout: device, N*M, interleaved, updated in place.  scratch: device, N*M elements, or NULL
  * (the library then allocates and frees a stream-ordered temporary). */
 typedef struct {
@@ -170,7 +186,9 @@ int pent_step_kernel_choice(const pent_handle* h, int64_t M);
 /* ---- introspection ------------------------------------------------------------------------ */
 int pent_handle_n(const pent_handle* h);                 /* N, or -1 */
 int pent_handle_dtype(const pent_handle* h);             /* pent_dtype, or -1 */
-int64_t pent_handle_m(const pent_handle* h);             /* M of a per-system handle, 0 for shared A */
+int64_t pent_handle_m(const pent_handle* h);             /* M of a per-system handle, 0 for shared A, -1 for NULL */
+int pent_handle_device(const pent_handle* h);            /* CUDA device ordinal of the handle, or -1 */
+int pent_handle_band(const pent_handle* h);              /* shared A: 1 = tridiagonal (a == e == 0), 2 = pentadiagonal; -1 */
 /* Copies the fp64 factor arrays (N doubles each; any pointer may be NULL) to HOST memory:
  * eps, beta, alpha = bands of L, gamma, delta = bands of R (Eq. 13).  Shared-A only. */
 int pent_handle_factors(const pent_handle* h, double* eps, double* beta, double* alpha,

@@ -21,7 +21,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = [os.path.join(_HERE, "pent_oracle.c"), os.path.join(_HERE, "pent_oracle_step.c"),
-        os.path.join(_HERE, "pent_oracle_periodic.c")]
+        os.path.join(_HERE, "pent_oracle_periodic.c"), os.path.join(_HERE, "pent_oracle_ld.c")]
 _LIB = os.path.join(_HERE, "libpent_oracle.so")
 _lib = None
 
@@ -45,6 +45,9 @@ def _load():
         _lib.pent_oracle_factor.restype = C.c_int
         _lib.pent_oracle_dense_ge.restype = C.c_int
         _lib.pent_oracle_periodic_setup.restype = C.c_int
+        _lib.pent_oracle_ld_solve_rows.restype = C.c_int
+        _lib.pent_oracle_ld_step_rows.restype = C.c_int
+        _lib.pent_oracle_ld_periodic_solve_rows.restype = C.c_int
     return _lib
 
 
@@ -218,3 +221,52 @@ def step_periodic_batch(pf: PeriodicFactors, c_interleaved, nsteps: int, nthread
         _p(np.ascontiguousarray(pf.Y.ravel())), _p(np.ascontiguousarray(pf.kk.ravel())),
         _p(np.ascontiguousarray(pf.s2inv.ravel())), _p(Crows), C.c_int(nsteps), C.c_int(nthreads))
     return np.ascontiguousarray(Crows.T)
+
+
+# ---- the same transcription in long double (pent_oracle_ld.c): the "truth" that measured tolerances refer to ----
+def ld_solve_batch(diags, f_interleaved, nthreads: int = 1) -> np.ndarray:
+    """A^{-1} f in 80-bit long double, rounded once to fp64.  Interleaved (N, M) in and out."""
+    a, b, c, d, e = (_f64(v) for v in diags)
+    F = to_rows(f_interleaved)
+    X = np.empty_like(F)
+    rc = _load().pent_oracle_ld_solve_rows(C.c_int(c.shape[0]), C.c_long(F.shape[0]), _p(a), _p(b), _p(c),
+                                           _p(d), _p(e), _p(F), _p(X), C.c_int(nthreads))
+    if rc != 0:
+        raise SingularPivot(rc - 1)
+    return np.ascontiguousarray(X.T)
+
+
+def ld_factor_solve_batch(a, b, c, d, e, f, nthreads: int = 1):
+    """Per-system matrices in long double; arguments interleaved (N, M)."""
+    rows = [to_rows(v) for v in (a, b, c, d, e, f)]
+    M, N = rows[5].shape
+    X = np.zeros_like(rows[5])
+    info = np.zeros(M, dtype=np.int32)
+    _load().pent_oracle_ld_factor_solve_rows(C.c_int(N), C.c_long(M), *[_p(r) for r in rows], _p(X),
+                                             info.ctypes.data_as(C.POINTER(C.c_int)), C.c_int(nthreads))
+    return np.ascontiguousarray(X.T), info
+
+
+def ld_step_batch(diags, kind: int, bc: int, form: int, r: float, sigma: float, c_interleaved, nsteps: int,
+                  nthreads: int = 1) -> np.ndarray:
+    """nsteps time steps with every intermediate (and the state between steps) in long double."""
+    a, b, c, d, e = (_f64(v) for v in diags)
+    Crows = to_rows(c_interleaved)
+    rc = _load().pent_oracle_ld_step_rows(C.c_int(c.shape[0]), C.c_long(Crows.shape[0]), C.c_int(kind), C.c_int(bc),
+                                          C.c_int(form), C.c_double(r), C.c_double(sigma), _p(a), _p(b), _p(c),
+                                          _p(d), _p(e), _p(Crows), C.c_int(nsteps), C.c_int(nthreads))
+    if rc != 0:
+        raise SingularPivot(rc - 1)
+    return np.ascontiguousarray(Crows.T)
+
+
+def ld_solve_periodic_batch(diags, f_interleaved, nthreads: int = 1) -> np.ndarray:
+    """Periodic (cyclic) solve, set-up and Eqs. 12 / 11 in long double."""
+    a, b, c, d, e = (_f64(v) for v in diags)
+    F = to_rows(f_interleaved)
+    X = np.empty_like(F)
+    rc = _load().pent_oracle_ld_periodic_solve_rows(C.c_int(c.shape[0]), C.c_long(F.shape[0]), _p(a), _p(b), _p(c),
+                                                    _p(d), _p(e), _p(F), _p(X), C.c_int(nthreads))
+    if rc != 0:
+        raise SingularPivot(rc - 1)
+    return np.ascontiguousarray(X.T)

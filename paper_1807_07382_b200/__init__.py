@@ -84,6 +84,10 @@ def lib() -> C.CDLL:
     L.pent_handle_dtype.argtypes = [vp]
     L.pent_handle_m.argtypes = [vp]
     L.pent_handle_m.restype = i64
+    L.pent_handle_device.argtypes = [vp]
+    L.pent_handle_band.argtypes = [vp]
+    L.pent_release_thread_cache.argtypes = []
+    L.pent_release_thread_cache.restype = None
     L.pent_handle_factors.argtypes = [vp] * 6
     L.pent_solve_kernel_choice.argtypes = [vp, i64]
     L.pent_launch_count.argtypes = [ci]
@@ -112,9 +116,23 @@ def _stream(stream) -> int:
     return s.cuda_stream
 
 
-def _batch(t: torch.Tensor, name: str):
-    if not (t.is_cuda and t.is_contiguous() and t.dim() == 2):
+def _batch(t: torch.Tensor, name: str, shape=None, dtype=None):
+    """Every tensor whose pointer crosses the C ABI: contiguous, 2-D, on the CURRENT CUDA device (that is
+    where the kernel is launched and where the handle's memory lives), and of the expected shape / dtype."""
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous() and t.dim() == 2):
         raise ValueError(f"{name}: contiguous CUDA tensor of shape (N, M) expected (interleaved layout)")
+    if t.device.index != torch.cuda.current_device():
+        raise ValueError(f"{name}: tensor is on {t.device}, the current device is cuda:{torch.cuda.current_device()}")
+    if shape is not None and tuple(t.shape) != tuple(shape):
+        raise ValueError(f"{name}: shape {tuple(t.shape)}, expected {tuple(shape)}")
+    if dtype is not None and t.dtype != dtype:
+        raise ValueError(f"{name}: dtype {t.dtype}, expected {dtype}")
+
+
+def _vec(t: torch.Tensor, name: str, numel_min: int, dtype):
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous() and t.dtype == dtype
+            and t.numel() >= numel_min and t.device.index == torch.cuda.current_device()):
+        raise ValueError(f"{name}: contiguous {dtype} tensor of >= {numel_min} elements on the current CUDA device expected")
 
 
 @dataclass
@@ -179,24 +197,20 @@ def pent_factor_periodic(N: int, e, c, d, a, b) -> Handle:
 def pent_solve_batch(h: Handle, M: int, f: torch.Tensor, x: torch.Tensor | None = None,
                      stream=None, kernel: int = KERNEL_AUTO) -> torch.Tensor:
     """Forward + backward sweeps for M systems; f, x of shape (N, M)."""
-    _batch(f, "f")
+    _batch(f, "f", (h.N, M), h.dtype)
     if x is None:
         x = torch.empty_like(f)
-    _batch(x, "x")
-    if f.shape != (h.N, M) or x.shape != f.shape or f.dtype != h.dtype or x.dtype != h.dtype:
-        raise ValueError("f/x must have shape (N, M) and the handle's dtype")
+    _batch(x, "x", (h.N, M), h.dtype)
     _check(lib().pent_solve_batch_v(h.ptr, M, f.data_ptr(), x.data_ptr(), _stream(stream), kernel))
     return x
 
 
 def pent_solve_batch_rows(h: Handle, M: int, f: torch.Tensor, x: torch.Tensor | None = None, stream=None) -> torch.Tensor:
     """Same solve on a system-major batch: f, x of shape (M, N), one system per row."""
-    _batch(f, "f")
+    _batch(f, "f", (M, h.N), h.dtype)
     if x is None:
         x = torch.empty_like(f)
-    _batch(x, "x")
-    if f.shape != (M, h.N) or x.shape != f.shape or f.dtype != h.dtype or x.dtype != h.dtype:
-        raise ValueError("f/x must have shape (M, N) and the handle's dtype")
+    _batch(x, "x", (M, h.N), h.dtype)
     _check(lib().pent_solve_batch_rows(h.ptr, M, f.data_ptr(), x.data_ptr(), _stream(stream)))
     return x
 
@@ -208,8 +222,15 @@ def pent_solve_batch_host(h: Handle, M: int, f_host: torch.Tensor,
         raise ValueError("f_host: contiguous CPU tensor (N, M) of the handle's dtype expected")
     if x_host is None:
         x_host = torch.empty_like(f_host)
+    if x_host.is_cuda or not x_host.is_contiguous() or x_host.shape != f_host.shape or x_host.dtype != h.dtype:
+        raise ValueError("x_host: contiguous CPU tensor (N, M) of the handle's dtype expected")
     _check(lib().pent_solve_batch_host(h.ptr, M, f_host.data_ptr(), x_host.data_ptr()))
     return x_host
+
+
+def pent_workspace_elems(N: int, M: int) -> int:
+    """Elements of the optional workspace of pent_factor_solve_batch: 3*N*M', M' = M rounded up to 64."""
+    return 3 * N * ((M + 63) // 64 * 64)
 
 
 def pent_factor_solve_batch(N: int, M: int, e, c, d, a, b, f, x=None, info=None, stream=None,
@@ -217,17 +238,17 @@ def pent_factor_solve_batch(N: int, M: int, e, c, d, a, b, f, x=None, info=None,
     """Per-system matrices, factor + solve fused.  All tensors (N, M) on CUDA.
     workspace: optional CUDA tensor of 3*N*M' elements, M' = M rounded up to a multiple of 64.  Returns (x, info) with info int32[M]:
     0 or first bad row + 1."""
+    _dt(f)
     for t, n in zip((e, c, d, a, b, f), "ecdabf"):
-        _batch(t, n)
-        if t.shape != (N, M) or t.dtype != f.dtype:
-            raise ValueError("all arrays must be (N, M) of one dtype")
+        _batch(t, n, (N, M), f.dtype)
     if x is None:
         x = torch.empty_like(f)
+    _batch(x, "x", (N, M), f.dtype)
     if info is None:
         info = torch.zeros(M, dtype=torch.int32, device=f.device)
-    if workspace is not None and (not workspace.is_cuda or workspace.dtype != f.dtype or
-                                  workspace.numel() < 3 * N * ((M + 63) // 64 * 64) or not workspace.is_contiguous()):
-        raise ValueError("workspace: contiguous CUDA tensor of >= 3*N*roundup(M, 64) elements of f's dtype expected")
+    _vec(info, "info", M, torch.int32)
+    if workspace is not None:
+        _vec(workspace, "workspace", pent_workspace_elems(N, M), f.dtype)
     _check(lib().pent_factor_solve_batch_ws(N, M, e.data_ptr(), c.data_ptr(), d.data_ptr(),
                                             a.data_ptr(), b.data_ptr(), f.data_ptr(), x.data_ptr(),
                                             _dt(f), info.data_ptr(),
@@ -238,12 +259,12 @@ def pent_factor_solve_batch(N: int, M: int, e, c, d, a, b, f, x=None, info=None,
 
 def pent_factor_batch(N: int, M: int, e, c, d, a, b, info=None, stream=None):
     """Per-system factorisations kept in a handle for repeated pent_solve_batch_multi calls."""
+    _dt(c)
     for t, n in zip((e, c, d, a, b), "ecdab"):
-        _batch(t, n)
-        if t.shape != (N, M) or t.dtype != c.dtype:
-            raise ValueError("all arrays must be (N, M) of one dtype")
+        _batch(t, n, (N, M), c.dtype)
     if info is None:
         info = torch.zeros(M, dtype=torch.int32, device=c.device)
+    _vec(info, "info", M, torch.int32)
     out = C.c_void_p()
     _check(lib().pent_factor_batch(N, M, e.data_ptr(), c.data_ptr(), d.data_ptr(), a.data_ptr(),
                                    b.data_ptr(), _dt(c), C.byref(out), info.data_ptr(),
@@ -252,11 +273,10 @@ def pent_factor_batch(N: int, M: int, e, c, d, a, b, info=None, stream=None):
 
 
 def pent_solve_batch_multi(h: Handle, f: torch.Tensor, x: torch.Tensor | None = None, stream=None):
-    _batch(f, "f")
+    _batch(f, "f", (h.N, h.M), h.dtype)
     if x is None:
         x = torch.empty_like(f)
-    if f.shape != (h.N, h.M) or f.dtype != h.dtype or x.shape != f.shape:
-        raise ValueError("f must be (N, M) of the handle")
+    _batch(x, "x", (h.N, h.M), h.dtype)
     _check(lib().pent_solve_batch_multi(h.ptr, f.data_ptr(), x.data_ptr(), _stream(stream)))
     return x
 
@@ -266,10 +286,10 @@ def pent_step_batch(h: Handle, M: int, c: torch.Tensor, nsteps: int, *, kind: in
                     scratch: torch.Tensor | None = None, stream=None,
                     kernel: int = KERNEL_AUTO) -> torch.Tensor:
     """nsteps fused steps (RHS + solve in one kernel) in place on c (N, M).  See include/pent.h."""
-    _batch(c, "c")
-    if c.shape != (h.N, M) or c.dtype != h.dtype:
-        raise ValueError("c must be (N, M) of the handle's dtype")
+    _batch(c, "c", (h.N, M), h.dtype)
     p = pent_step_params(kind, bc, form, r, sigma)
+    if scratch is not None:
+        _vec(scratch, "scratch", h.N * M, h.dtype)
     sp = 0 if scratch is None else scratch.data_ptr()
     _check(lib().pent_step_batch_v(h.ptr, C.byref(p), M, c.data_ptr(), sp, nsteps, _stream(stream), kernel))
     return c

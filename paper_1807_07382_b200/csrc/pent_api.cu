@@ -7,22 +7,25 @@ extern "C" int pent_solve_batch_v(const pent_handle* h, int64_t M, const void* f
 {
     if (!h || h->kind != 0 || M < 0) return PENT_ERR_ARG;
     if (M == 0) return PENT_OK;
-    if (!f || !x) return PENT_ERR_ARG;
+    if (!f || !x || !pent::on_handle_device(h)) return PENT_ERR_ARG;
     cudaStream_t s = (cudaStream_t)stream;
     if (kernel < 0 || (kernel >> 24) != 0) return PENT_ERR_ARG;
     if (h->periodic) return pent::solve_periodic(h, M, f, x, s, kernel);
     const int Q = (kernel >> 8) & 0xff, S = (kernel >> 16) & 0xff;
     switch (kernel & 0xff) {
-        case PENT_KERNEL_AUTO:
+        case PENT_KERNEL_AUTO: {
             if (Q || S) return PENT_ERR_ARG;
-            if (pent::chunked_supported(h, M, f, 0, 0)) return pent::launch_solve_chunked(h, M, f, x, s, 0, 0);
-            return pent::launch_solve_tps(h, M, f, x, s);
+            // the plan is resolved once, inside the launcher; PENT_UNSUPPORTED = no on-chip plan for this shape
+            const int rc = pent::launch_solve_chunked(h, M, f, x, s, 0, 0);
+            return rc == pent::PENT_UNSUPPORTED ? pent::launch_solve_tps(h, M, f, x, s) : rc;
+        }
         case PENT_KERNEL_THREAD_PER_SYSTEM:
             if (Q || S) return PENT_ERR_ARG;
             return pent::launch_solve_tps(h, M, f, x, s);
-        case PENT_KERNEL_CHUNKED:
-            if (!pent::chunked_supported(h, M, f, Q, S)) return PENT_ERR_ARG;
-            return pent::launch_solve_chunked(h, M, f, x, s, Q, S);
+        case PENT_KERNEL_CHUNKED: {
+            const int rc = pent::launch_solve_chunked(h, M, f, x, s, Q, S);
+            return rc == pent::PENT_UNSUPPORTED ? PENT_ERR_ARG : rc;
+        }
         default:
             return PENT_ERR_ARG;
     }
@@ -34,9 +37,9 @@ extern "C" int pent_solve_batch_rows(const pent_handle* h, int64_t M, const void
 {
     if (!h || h->kind != 0 || h->periodic || M < 0) return PENT_ERR_ARG;
     if (M == 0) return PENT_OK;
-    if (!f || !x) return PENT_ERR_ARG;
-    if (!pent::chunked_rows_supported(h, M)) return PENT_ERR_ARG;      // N too long to keep a tile on chip
-    return pent::launch_solve_chunked_rows(h, M, f, x, (cudaStream_t)stream);
+    if (!f || !x || !pent::on_handle_device(h)) return PENT_ERR_ARG;
+    const int rc = pent::launch_solve_chunked_rows(h, M, f, x, (cudaStream_t)stream);
+    return rc == pent::PENT_UNSUPPORTED ? PENT_ERR_ARG : rc;           // N too long to keep a tile on chip
 }
 
 extern "C" int pent_solve_kernel_choice(const pent_handle* h, int64_t M)
@@ -98,14 +101,18 @@ struct HostPipe {
 thread_local HostPipe g_pipe;
 }  // namespace
 
+extern "C" void pent_release_thread_cache(void) { g_pipe.release(); }
+
 extern "C" int pent_solve_batch_host(const pent_handle* h, int64_t M, const void* f_host,
                                      void* x_host)
 {
     if (!h || h->kind != 0 || M < 0) return PENT_ERR_ARG;
     if (M == 0) return PENT_OK;
-    if (!f_host || !x_host) return PENT_ERR_ARG;
+    if (!f_host || !x_host || !pent::on_handle_device(h)) return PENT_ERR_ARG;
     const size_t esz = h->dtype == PENT_F64 ? 8 : 4;
     const int N = h->N;
+    // cudaMemcpy2DAsync takes the host pitch M*esz, which must stay below cudaDevAttrMaxPitch (2^31 - 1 bytes)
+    if ((uint64_t)M * esz > 0x7fffffffull) return PENT_ERR_ARG;
     // ~16 MiB slabs, a multiple of 256 systems (keeps the slab pitch 16-byte aligned for TMA)
     int64_t Ms = std::max<int64_t>(256, ((16ll << 20) / ((int64_t)N * (int64_t)esz)) / 256 * 256);
     Ms = std::min(Ms, M);

@@ -450,5 +450,6 @@ ChunkPlan make_plan(const pent_handle* h, int64_t M, const void* f, int Q, int S
 ChunkPlan chunk_auto_plan(const pent_handle* h, int64_t M, const void* f);   // what PENT_KERNEL_AUTO runs
 // rank-2 tensor map {M, N} of an interleaved batch with box {S, box_rows}; false on failure
 bool encode_batch_map(CUtensorMap* tm, const void* base, int64_t M, int N, int S, int box_rows, bool f64);
+bool encode_batch_map_cached(CUtensorMap* tm, const void* base, int64_t M, int N, int S, int box_rows, bool f64);
 
 }  // namespace pent

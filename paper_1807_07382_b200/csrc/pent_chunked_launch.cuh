@@ -42,7 +42,7 @@ static int launch_inst(const pent_handle* h, const ChunkPlan& pl, int64_t M, con
     prm.ldg = pl.rows ? 2 : (pl.ldg ? 1 : 0);
 
     CUtensorMap tm = {};
-    if (!pl.ldg && !encode_batch_map(&tm, f, M, h->N, S, prm.box_rows, sizeof(T) == 8)) {
+    if (!pl.ldg && !encode_batch_map_cached(&tm, f, M, h->N, S, prm.box_rows, sizeof(T) == 8)) {
         g_last_cuda_error = (int)cudaErrorInvalidValue;
         return PENT_ERR_CUDA;
     }
@@ -51,7 +51,7 @@ static int launch_inst(const pent_handle* h, const ChunkPlan& pl, int64_t M, con
     if (PER) pp = *per;
     const size_t smem_total = pl.smem + (PER ? periodic_extra_smem<T>(pl) : 0);
     auto kern = solve_chunked_kernel<T, S, CLUSTER, PER>;
-    static thread_local SmemMark mark;
+    static SmemOnce mark;
     PENT_CUDA(ensure_dynamic_smem(mark, kern, smem_total));
     // the occupancy answer depends only on (device, threads, shared memory, cluster size): keep the last
     // one per thread and kernel instance, so a small solve is not bound by host-side queries

@@ -1,5 +1,6 @@
 // pent_factor.cu -- shared-A factorisation A = L R on the device and the
 // derived, sweep-ready coefficient tables kept in the handle.
+#include <cmath>
 #include <cstdlib>
 #include <cstring>
 #include <new>
@@ -88,26 +89,71 @@ static bool is_device_ptr(const void* p)
     return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
 }
 
+// Is the matrix I + sigma L^2 for the second-difference matrix L with boundary bc (0 Dirichlet, 1 zero-flux)?
+// (L^2)[k][k] = dg_k^2 + [k > 0] + [k < N-1], (L^2)[k][k+-1] = dg_k + dg_{k+-1}, (L^2)[k][k+-2] = 1, with
+// dg = -2 except dg_0 = dg_{N-1} = -1 for bc = 1.  dg5 = the widened diagonals a,b,c,d,e (host copy).
+// tol: relative, on the scale of 1 + 6 sigma (fp32 handles hold rounded entries).
+static void detect_l2_form(pent_handle* h, const double* dg5, double tol)
+{
+    const int N = h->N;
+    h->l2_bc = -1; h->l2_sigma = 0.0;
+    if (N < 3) return;
+    const double* a = dg5; const double* b = dg5 + N; const double* c = dg5 + 2 * (size_t)N;
+    const double* d = dg5 + 3 * (size_t)N; const double* e = dg5 + 4 * (size_t)N;
+    const double sigma = a[2];
+    if (!(sigma > 0.0)) return;
+    const double scale = tol * (1.0 + 6.0 * sigma);
+    for (int bc = 0; bc < 2; ++bc) {
+        auto dgL = [&](int k) { return (bc == 1 && (k == 0 || k == N - 1)) ? -1.0 : -2.0; };
+        bool ok = true;
+        for (int k = 0; k < N && ok; ++k) {
+            const double cc = 1.0 + sigma * (dgL(k) * dgL(k) + (k > 0 ? 1.0 : 0.0) + (k < N - 1 ? 1.0 : 0.0));
+            ok = fabs(c[k] - cc) <= scale;
+            if (ok && k >= 1) ok = fabs(b[k] - sigma * (dgL(k) + dgL(k - 1))) <= scale;
+            if (ok && k + 1 < N) ok = fabs(d[k] - sigma * (dgL(k) + dgL(k + 1))) <= scale;
+            if (ok && k >= 2) ok = fabs(a[k] - sigma) <= scale;
+            if (ok && k + 2 < N) ok = fabs(e[k] - sigma) <= scale;
+        }
+        if (ok) { h->l2_bc = bc; h->l2_sigma = sigma; return; }
+    }
+}
+
+// Everything on the PRIVATE stream `s` (non-blocking): no other stream of the process is stalled, and the
+// host waits for `s` only.  Temporaries are stream-ordered allocations on `s`.
 template <typename T>
-static int factor_impl(int N, const void* const src[5], pent_dtype dtype, pent_handle** out,
-                       int* bad_row)
+int factor_on_stream(int N, const void* const src[5], pent_dtype dtype, pent_handle** out, int* bad_row,
+                     cudaStream_t s)
 {
     pent_handle* h = new (std::nothrow) pent_handle();
     if (!h) return PENT_ERR_ALLOC;
     std::memset(h, 0, sizeof(*h));
-    h->kind = 0; h->N = N; h->dtype = dtype;
+    h->kind = 0; h->N = N; h->dtype = dtype; h->l2_bc = -1; h->band = 2;
+    if (cudaGetDevice(&h->device) != cudaSuccess) { delete h; return cuda_fail(cudaGetLastError()); }
     T* stage = nullptr;
     int* status = nullptr;
+    double* hostdg = (double*)std::malloc(sizeof(double) * 5 * (size_t)N);
     int rc = PENT_OK;
-    auto fail = [&](int code) { cudaFree(stage); cudaFree(status); pent_destroy(h); return code; };
+    auto fail = [&](int code) {
+        if (stage) cudaFreeAsync(stage, s);
+        if (status) cudaFreeAsync(status, s);
+        cudaStreamSynchronize(s);
+        std::free(hostdg);
+        pent_destroy(h);
+        return code;
+    };
+    if (!hostdg) return fail(PENT_ERR_ALLOC);
     auto chk = [&](cudaError_t e) { if (e != cudaSuccess) { rc = cuda_fail(e); return false; } return true; };
-
     auto alloc = [&](void** p, size_t bytes) {
         cudaError_t e = cudaMalloc(p, bytes);
         if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); rc = PENT_ERR_ALLOC; return false; }
         return chk(e);
     };
-    if (!alloc((void**)&stage, sizeof(T) * 5 * (size_t)N) || !alloc((void**)&status, sizeof(int)) ||
+    auto alloc_tmp = [&](void** p, size_t bytes) {
+        cudaError_t e = cudaMallocAsync(p, bytes, s);
+        if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); rc = PENT_ERR_ALLOC; return false; }
+        return chk(e);
+    };
+    if (!alloc_tmp((void**)&stage, sizeof(T) * 5 * (size_t)N) || !alloc_tmp((void**)&status, 2 * sizeof(int)) ||
         !alloc((void**)&h->diag, sizeof(double) * 5 * (size_t)N) ||
         !alloc((void**)&h->fac, sizeof(double) * 5 * (size_t)N) ||
         !alloc(&h->fw, sizeof(T) * 4 * (size_t)N) || !alloc(&h->bw, sizeof(T) * 2 * (size_t)N) ||
@@ -117,27 +163,40 @@ static int factor_impl(int N, const void* const src[5], pent_dtype dtype, pent_h
     // order of src: a, b, c, d, e
     for (int j = 0; j < 5; ++j) {
         cudaMemcpyKind kind = is_device_ptr(src[j]) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
-        if (!chk(cudaMemcpy(stage + (size_t)j * N, src[j], sizeof(T) * (size_t)N, kind))) return fail(rc);
+        if (!chk(cudaMemcpyAsync(stage + (size_t)j * N, src[j], sizeof(T) * (size_t)N, kind, s))) return fail(rc);
     }
     int tb = 128, nb = (N + tb - 1) / tb;
-    widen_diagonals<T><<<nb, tb>>>(N, stage, stage + N, stage + 2 * (size_t)N, stage + 3 * (size_t)N,
-                                   stage + 4 * (size_t)N, h->diag);
-    factor_shared<<<1, 32>>>(N, h->diag, h->fac, status);
-    derive_tables<T><<<nb, tb>>>(N, h->diag, h->fac, (typename Vec<T>::T4*)h->fw,
-                                 (typename Vec<T>::T2*)h->bw, (T*)h->dg);
+    widen_diagonals<T><<<nb, tb, 0, s>>>(N, stage, stage + N, stage + 2 * (size_t)N, stage + 3 * (size_t)N,
+                                         stage + 4 * (size_t)N, h->diag);
+    factor_shared<<<1, 32, 0, s>>>(N, h->diag, h->fac, status);
+    derive_tables<T><<<nb, tb, 0, s>>>(N, h->diag, h->fac, (typename Vec<T>::T4*)h->fw,
+                                       (typename Vec<T>::T2*)h->bw, (T*)h->dg);
     count_launch(3);
     if (!chk(cudaGetLastError())) return fail(rc);
     int bad = -1;
-    if (!chk(cudaMemcpy(&bad, status, sizeof(int), cudaMemcpyDeviceToHost))) return fail(rc);
+    if (!chk(cudaMemcpyAsync(&bad, status, sizeof(int), cudaMemcpyDeviceToHost, s)) ||
+        !chk(cudaMemcpyAsync(hostdg, h->diag, sizeof(double) * 5 * (size_t)N, cudaMemcpyDeviceToHost, s)) ||
+        !chk(cudaStreamSynchronize(s)))
+        return fail(rc);
     if (bad_row) *bad_row = bad;
     if (bad >= 0) return fail(PENT_ERR_PIVOT);
-    rc = build_chunk_tables(h, 0);
+    detect_l2_form(h, hostdg, sizeof(T) == 8 ? 1e-13 : 1e-6);
+    {   // tridiagonal matrix (a == e == 0 inside the matrix)?  cuThomasBatch's case
+        bool tri = true;
+        for (int k = 0; k < N && tri; ++k) tri = hostdg[k] == 0.0 && hostdg[4 * (size_t)N + k] == 0.0;
+        h->band = tri ? 1 : 2;
+    }
+    rc = build_chunk_tables(h, s);
     if (rc != PENT_OK) return fail(rc);
-    if (!chk(cudaDeviceSynchronize())) return fail(rc);
-    cudaFree(stage); cudaFree(status);
+    cudaFreeAsync(stage, s); cudaFreeAsync(status, s);
+    stage = nullptr; status = nullptr;
+    if (!chk(cudaStreamSynchronize(s))) return fail(rc);
+    std::free(hostdg);
     *out = h;
     return PENT_OK;
 }
+template int factor_on_stream<double>(int, const void* const*, pent_dtype, pent_handle**, int*, cudaStream_t);
+template int factor_on_stream<float>(int, const void* const*, pent_dtype, pent_handle**, int*, cudaStream_t);
 }  // namespace pent
 
 // ------------------------------------------------------------------------------------------
@@ -150,10 +209,14 @@ extern "C" int pent_factor(int N, const void* e, const void* c, const void* d, c
     if (!out) return PENT_ERR_ARG;
     *out = nullptr;
     if (N < 1 || !e || !c || !d || !a || !b) return PENT_ERR_ARG;
+    if (dtype != PENT_F64 && dtype != PENT_F32) return PENT_ERR_ARG;
     const void* src[5] = {a, b, c, d, e};
-    if (dtype == PENT_F64) return pent::factor_impl<double>(N, src, dtype, out, bad_row);
-    if (dtype == PENT_F32) return pent::factor_impl<float>(N, src, dtype, out, bad_row);
-    return PENT_ERR_ARG;
+    cudaStream_t s = nullptr;
+    PENT_CUDA(cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking));
+    const int rc = dtype == PENT_F64 ? pent::factor_on_stream<double>(N, src, dtype, out, bad_row, s)
+                                     : pent::factor_on_stream<float>(N, src, dtype, out, bad_row, s);
+    cudaStreamDestroy(s);
+    return rc;
 }
 
 extern "C" void pent_destroy(pent_handle* h)
@@ -170,11 +233,13 @@ extern "C" void pent_destroy(pent_handle* h)
 extern "C" int pent_handle_n(const pent_handle* h) { return h ? h->N : -1; }
 extern "C" int pent_handle_dtype(const pent_handle* h) { return h ? (int)h->dtype : -1; }
 extern "C" int64_t pent_handle_m(const pent_handle* h) { return h ? h->M : -1; }
+extern "C" int pent_handle_device(const pent_handle* h) { return h ? h->device : -1; }
+extern "C" int pent_handle_band(const pent_handle* h) { return (h && h->kind == 0) ? (h->periodic ? 2 : h->band) : -1; }
 
 extern "C" int pent_handle_factors(const pent_handle* h, double* eps, double* beta, double* alpha,
                                    double* gamma, double* delta)
 {
-    if (!h || h->kind != 0) return PENT_ERR_ARG;
+    if (!h || h->kind != 0 || !pent::on_handle_device(h)) return PENT_ERR_ARG;
     if (h->periodic) return pent_handle_factors(h->inner, eps, beta, alpha, gamma, delta);   // factors of E
     double* dst[5] = {eps, beta, alpha, gamma, delta};
     for (int j = 0; j < 5; ++j)
@@ -195,4 +260,4 @@ extern "C" int64_t pent_launch_count(int reset)
 
 extern "C" int pent_handle_periodic(const pent_handle* h) { return h ? h->periodic : -1; }
 
-extern "C" const char* pent_version(void) { return "pent 0.2 (sm_100a)"; }
+extern "C" const char* pent_version(void) { return "pent 0.3 (sm_100a)"; }

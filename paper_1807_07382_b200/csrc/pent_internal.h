@@ -2,6 +2,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <atomic>
 #include "pent.h"
 
 // Cluster sizes (CTAs along k) the chunked kernel has tables for: Q = 1 << j, j < PENT_NQ.
@@ -12,6 +13,12 @@ struct pent_handle {
     int N;
     pent_dtype dtype;
     int64_t M;           // per-system only
+    int device;          // CUDA device ordinal the handle's memory lives on (every call checks it)
+    // shared A: set at factor time when the matrix is I + sigma L^2 for the Dirichlet (0) or zero-flux (1)
+    // second-difference matrix L (what pent_step_batch(kind 0) requires of its handle); -1 otherwise
+    int l2_bc;
+    double l2_sigma;
+    int band;            // shared A: 1 if a == e == 0 inside the matrix (tridiagonal), else 2
     // ---- shared A, all device memory ----
     double* diag;        // 5*N: a,b,c,d,e widened to fp64, out-of-matrix entries zeroed
     double* fac;         // 5*N: eps,beta,alpha,gamma,delta (Eq. 13), fp64
@@ -39,28 +46,43 @@ struct pent_handle {
 
 namespace pent {
 
+constexpr int PENT_UNSUPPORTED = -100;      // internal: no on-chip plan for this shape (never crosses the C ABI)
+
 extern thread_local int g_last_cuda_error;
 extern thread_local int64_t g_launches;
 
 inline int cuda_fail(cudaError_t e) { g_last_cuda_error = (int)e; return PENT_ERR_CUDA; }
 inline void count_launch(int n = 1) { g_launches += n; }
 
-// cudaFuncAttributeMaxDynamicSharedMemorySize is per device: one high-water mark per (calling thread,
-// kernel instance, device).  `mark` is a `static thread_local SmemMark` at the launch site.
-struct SmemMark { size_t bytes[16] = {}; };
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a PROCESS-wide property of (kernel instance, device), and
+// cudaFuncSetAttribute sets it (it can lower it).  So it is raised exactly once per kernel instance and
+// device, to the largest value any launch of this library uses (SMEM_OPTIN), and never touched again:
+// `mask` is a `static SmemOnce` at the launch site (one per template instance), bit d = done on device d.
+// Two threads racing on the first launch both set the same value, which is harmless.
+constexpr size_t SMEM_OPTIN = 232448;       // 227 KB, the sm_100 per-CTA limit
+struct SmemOnce { std::atomic<uint32_t> mask{0}; };
 template <typename K>
-inline cudaError_t ensure_dynamic_smem(SmemMark& mark, K kernel, size_t bytes)
+inline cudaError_t ensure_dynamic_smem(SmemOnce& once, K kernel, size_t bytes)
 {
+    if (bytes > SMEM_OPTIN) return cudaErrorInvalidValue;
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
-    const int d = dev & 15;
-    if (bytes > mark.bytes[d]) {
-        e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    const uint32_t bit = 1u << (dev & 31);
+    if (!(once.mask.load(std::memory_order_acquire) & bit)) {
+        e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_OPTIN);
         if (e != cudaSuccess) return e;
-        mark.bytes[d] = bytes;
+        once.mask.fetch_or(bit, std::memory_order_release);
     }
     return cudaSuccess;
+}
+
+// every entry point that takes a handle: the handle's memory must be on the CURRENT device
+inline bool on_handle_device(const pent_handle* h)
+{
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return false; }
+    return dev == h->device;
 }
 
 #define PENT_CUDA(call)                                           \
@@ -91,6 +113,11 @@ __device__ __forceinline__ float4 ldg4(const float4* p) { return __ldg(p); }
 __device__ __forceinline__ double2 ldg2(const double2* p) { return __ldg(p); }
 __device__ __forceinline__ float2 ldg2(const float2* p) { return __ldg(p); }
 #endif
+
+// shared-A factorisation with every kernel, copy and temporary on the private stream `s` (pent_factor.cu)
+template <typename T>
+int factor_on_stream(int N, const void* const src[5], pent_dtype dtype, pent_handle** out, int* bad_row,
+                     cudaStream_t s);
 
 // kernels / launchers implemented across the .cu files
 int launch_solve_tps(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s);

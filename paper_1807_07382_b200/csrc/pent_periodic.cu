@@ -225,8 +225,10 @@ static bool is_dev(const void* p)
 }
 
 template <typename T>
-static int factor_periodic_t(int N, const void* const src[5], pent_dtype dtype, pent_handle** out, int* bad_row)
+static int factor_periodic_t(int N, const void* const src[5], pent_dtype dtype, pent_handle** out, int* bad_row,
+                             cudaStream_t s)
 {
+    // Everything runs on the private non-blocking stream `s`; temporaries are stream-ordered allocations.
     const int n = N - 2;
     T* stage = nullptr;
     double *dg64 = nullptr, *Z = nullptr, *coef = nullptr;
@@ -234,10 +236,16 @@ static int factor_periodic_t(int N, const void* const src[5], pent_dtype dtype, 
     pent_handle* h = new (std::nothrow) pent_handle();
     if (!h) return PENT_ERR_ALLOC;
     *h = pent_handle{};
-    h->kind = 0; h->periodic = 1; h->N = N; h->dtype = dtype;
+    h->kind = 0; h->periodic = 1; h->N = N; h->dtype = dtype; h->l2_bc = -1; h->band = 2;
+    if (cudaGetDevice(&h->device) != cudaSuccess) { delete h; return cuda_fail(cudaGetLastError()); }
     int rc = PENT_OK;
     auto done = [&](int code) {
-        cudaFree(stage); cudaFree(dg64); cudaFree(Z); cudaFree(coef); cudaFree(status);
+        if (stage) cudaFreeAsync(stage, s);
+        if (dg64) cudaFreeAsync(dg64, s);
+        if (Z) cudaFreeAsync(Z, s);
+        if (coef) cudaFreeAsync(coef, s);
+        if (status) cudaFreeAsync(status, s);
+        cudaStreamSynchronize(s);
         if (code != PENT_OK) pent_destroy(h);
         return code;
     };
@@ -247,37 +255,46 @@ static int factor_periodic_t(int N, const void* const src[5], pent_dtype dtype, 
         if (e != cudaSuccess) { rc = cuda_fail(e); return false; }
         return true;
     };
-    if (!alloc((void**)&stage, sizeof(T) * 5 * (size_t)N) || !alloc((void**)&dg64, sizeof(double) * 5 * (size_t)N) ||
-        !alloc((void**)&Z, sizeof(double) * 2 * (size_t)n) || !alloc((void**)&coef, sizeof(double) * 10) ||
-        !alloc((void**)&status, sizeof(int)) || !alloc(&h->Zt, sizeof(T) * 2 * (size_t)n) ||
+    auto alloc_tmp = [&](void** p, size_t bytes) {
+        cudaError_t e = cudaMallocAsync(p, bytes, s);
+        if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); rc = PENT_ERR_ALLOC; return false; }
+        if (e != cudaSuccess) { rc = cuda_fail(e); return false; }
+        return true;
+    };
+    if (!alloc_tmp((void**)&stage, sizeof(T) * 5 * (size_t)N) || !alloc_tmp((void**)&dg64, sizeof(double) * 5 * (size_t)N) ||
+        !alloc_tmp((void**)&Z, sizeof(double) * 2 * (size_t)n) || !alloc_tmp((void**)&coef, sizeof(double) * 10) ||
+        !alloc_tmp((void**)&status, sizeof(int)) || !alloc(&h->Zt, sizeof(T) * 2 * (size_t)n) ||
         !alloc(&h->dgp, sizeof(T) * 8 * (size_t)N))
         return done(rc);
     for (int j = 0; j < 5; ++j) {     // order of src: a, b, c, d, e
-        cudaError_t e = cudaMemcpy(stage + (size_t)j * N, src[j], sizeof(T) * (size_t)N,
-                                   is_dev(src[j]) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice);
+        cudaError_t e = cudaMemcpyAsync(stage + (size_t)j * N, src[j], sizeof(T) * (size_t)N,
+                                        is_dev(src[j]) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, s);
         if (e != cudaSuccess) return done(cuda_fail(e));
     }
     // E = leading (N-2) x (N-2) block: the shared-A factorisation of the first N-2 entries of each array
-    rc = pent_factor(n, stage + 4 * (size_t)N, stage + 2 * (size_t)N, stage + 3 * (size_t)N, stage,
-                     stage + (size_t)N, dtype, &h->inner, bad_row);
+    const void* inner_src[5] = {stage, stage + (size_t)N, stage + 2 * (size_t)N, stage + 3 * (size_t)N,
+                                stage + 4 * (size_t)N};
+    rc = factor_on_stream<T>(n, inner_src, dtype, &h->inner, bad_row, s);
     if (rc != PENT_OK) return done(rc);
+    h->inner->band = 2;               // the fused periodic kernel reads the pentadiagonal tables
     const int tb = 128, nb = (N + tb - 1) / tb;
-    periodic_tables_kernel<T><<<nb, tb>>>(N, stage, nullptr, nullptr, (T*)h->dgp, dg64);
-    periodic_setup_kernel<<<1, 32>>>(N, h->inner->fac, dg64, Z, coef, status);
-    periodic_tables_kernel<T><<<nb, tb>>>(N, stage, Z, (typename Vec<T>::T2*)h->Zt, (T*)h->dgp, nullptr);
+    periodic_tables_kernel<T><<<nb, tb, 0, s>>>(N, stage, nullptr, nullptr, (T*)h->dgp, dg64);
+    periodic_setup_kernel<<<1, 32, 0, s>>>(N, h->inner->fac, dg64, Z, coef, status);
+    periodic_tables_kernel<T><<<nb, tb, 0, s>>>(N, stage, Z, (typename Vec<T>::T2*)h->Zt, (T*)h->dgp, nullptr);
     count_launch(3);
     for (int j = 0; j < PENT_NQ; ++j) {
         const int Pl = h->inner->cfP[j];
         if (Pl < 1) continue;
         const int rows_total = (1 << j) * Pl * ChunkCfg<T>::C;
         if (!alloc(&h->pz[j], sizeof(T) * 2 * (size_t)rows_total)) return done(rc);
-        periodic_zslices_kernel<T><<<(rows_total + tb - 1) / tb, tb>>>(n, rows_total, Z, (typename Vec<T>::T2*)h->pz[j]);
+        periodic_zslices_kernel<T><<<(rows_total + tb - 1) / tb, tb, 0, s>>>(n, rows_total, Z, (typename Vec<T>::T2*)h->pz[j]);
         count_launch();
     }
     cudaError_t le = cudaGetLastError();
     int st = 0;
-    if (le == cudaSuccess) le = cudaMemcpy(&st, status, sizeof(int), cudaMemcpyDeviceToHost);
-    if (le == cudaSuccess) le = cudaMemcpy(h->pc, coef, sizeof(double) * 10, cudaMemcpyDeviceToHost);
+    if (le == cudaSuccess) le = cudaMemcpyAsync(&st, status, sizeof(int), cudaMemcpyDeviceToHost, s);
+    if (le == cudaSuccess) le = cudaMemcpyAsync(h->pc, coef, sizeof(double) * 10, cudaMemcpyDeviceToHost, s);
+    if (le == cudaSuccess) le = cudaStreamSynchronize(s);
     if (le != cudaSuccess) return done(cuda_fail(le));
     if (st != 0) { if (bad_row) *bad_row = N - 2; return done(PENT_ERR_PIVOT); }
     *out = h;
@@ -298,8 +315,12 @@ extern "C" int pent_factor_periodic(int N, const void* e, const void* c, const v
     if (!out) return PENT_ERR_ARG;
     *out = nullptr;
     if (N < 6 || !e || !c || !d || !a || !b) return PENT_ERR_ARG;
+    if (dtype != PENT_F64 && dtype != PENT_F32) return PENT_ERR_ARG;
     const void* src[5] = {a, b, c, d, e};
-    if (dtype == PENT_F64) return pent::factor_periodic_t<double>(N, src, dtype, out, bad_row);
-    if (dtype == PENT_F32) return pent::factor_periodic_t<float>(N, src, dtype, out, bad_row);
-    return PENT_ERR_ARG;
+    cudaStream_t s = nullptr;
+    PENT_CUDA(cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking));
+    const int rc = dtype == PENT_F64 ? pent::factor_periodic_t<double>(N, src, dtype, out, bad_row, s)
+                                     : pent::factor_periodic_t<float>(N, src, dtype, out, bad_row, s);
+    cudaStreamDestroy(s);
+    return rc;
 }

@@ -195,12 +195,15 @@ static int build_tables_t(pent_handle* h, int j, cudaStream_t s)
     PENT_CUDA(e);
     double* tmat = nullptr;
     int* lev = nullptr;
-    cudaError_t le = cudaMalloc(&tmat, sizeof(double) * 12 * Pl * Q);
-    if (le == cudaSuccess) le = cudaMalloc(&lev, 2 * sizeof(int));
+    // temporaries are stream-ordered allocations on the factor's private stream (cudaFree would synchronise
+    // the whole device)
+    auto release = [&]() { if (tmat) cudaFreeAsync(tmat, s); if (lev) cudaFreeAsync(lev, s); };
+    cudaError_t le = cudaMallocAsync((void**)&tmat, sizeof(double) * 12 * Pl * Q, s);
+    if (le == cudaSuccess) le = cudaMallocAsync((void**)&lev, 2 * sizeof(int), s);
     if (le == cudaSuccess) le = cudaMemsetAsync(lev, 0, 2 * sizeof(int), s);
     if (le == cudaSuccess) le = cudaMemsetAsync(h->cf[j], 0, tlen * Q * sizeof(T), s);
     if (le != cudaSuccess) {            // temporaries are released on every path; h->cf[j] belongs to the handle
-        cudaFree(tmat); cudaFree(lev);
+        release();
         if (le == cudaErrorMemoryAllocation) { cudaGetLastError(); return PENT_ERR_ALLOC; }
         return cuda_fail(le);
     }
@@ -211,8 +214,8 @@ static int build_tables_t(pent_handle* h, int j, cudaStream_t s)
     le = cudaGetLastError();
     int hl[2] = {0, 0};
     if (le == cudaSuccess) le = cudaMemcpyAsync(hl, lev, sizeof(hl), cudaMemcpyDeviceToHost, s);
+    release();
     if (le == cudaSuccess) le = cudaStreamSynchronize(s);
-    cudaFree(tmat); cudaFree(lev);
     if (le != cudaSuccess) return cuda_fail(le);
     h->cfP[j] = Pl; h->lev_f[j] = hl[0]; h->lev_b[j] = hl[1];
     return PENT_OK;
@@ -297,6 +300,29 @@ ChunkPlan make_plan(const pent_handle* h, int64_t M, const void* f, int Q, int S
     }
     pl.ok = true;
     return pl;
+}
+
+// The encoded map depends only on (base, M, N, S, box_rows, dtype): a small per-thread cache of the last
+// few, so that a launch-bound solve (cfg1: 11 us, cfg2: 27 us) does not pay the driver's encode on every call.
+bool encode_batch_map_cached(CUtensorMap* tm, const void* base, int64_t M, int N, int S, int box_rows, bool f64)
+{
+    struct Key { const void* base; int64_t M; int N, S, box_rows, f64; };
+    struct Cache { Key key[8]; CUtensorMap tm[8]; int n = 0, next = 0; };
+    static thread_local Cache c;
+    for (int j = 0; j < c.n; ++j) {
+        const Key& k = c.key[j];
+        if (k.base == base && k.M == M && k.N == N && k.S == S && k.box_rows == box_rows && k.f64 == (int)f64) {
+            *tm = c.tm[j];
+            return true;
+        }
+    }
+    if (!encode_batch_map(tm, base, M, N, S, box_rows, f64)) return false;
+    const int j = c.next;
+    c.key[j] = Key{base, M, N, S, box_rows, (int)f64};
+    c.tm[j] = *tm;
+    c.next = (c.next + 1) & 7;
+    if (c.n < 8) ++c.n;
+    return true;
 }
 
 bool encode_batch_map(CUtensorMap* tm, const void* base, int64_t M, int N, int S, int box_rows, bool f64)
@@ -408,7 +434,7 @@ static int launch_plan(const pent_handle* h, const ChunkPlan& pl, int64_t M, con
 int launch_solve_chunked_rows(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s)
 {
     const ChunkPlan pl = rows_plan(h, M);
-    if (!pl.ok) return PENT_ERR_ARG;
+    if (!pl.ok) return PENT_UNSUPPORTED;
     return launch_plan(h, pl, M, f, x, s);
 }
 
@@ -416,7 +442,7 @@ int launch_solve_chunked(const pent_handle* h, int64_t M, const void* f, void* x
                          int Q, int S)
 {
     const ChunkPlan pl = resolve_plan(h, M, f, Q, S);
-    if (!pl.ok) return PENT_ERR_ARG;
+    if (!pl.ok) return PENT_UNSUPPORTED;
     return launch_plan(h, pl, M, f, x, s);
 }
 

@@ -370,7 +370,7 @@ static int factor_solve_impl(int N, int64_t M, const void* e, const void* c, con
                                               scratch, scratch + NM, nullptr, nullptr, nullptr, info);
 #else
     const size_t smem = (size_t)RING_STAGES * RING_SLOTS * PS_THREADS * sizeof(T);
-    static thread_local SmemMark mark;
+    static SmemOnce mark;
     PENT_CUDA(ensure_dynamic_smem(mark, factor_solve_ring_kernel<T>, smem));
     factor_solve_ring_kernel<T><<<nb, tb, smem, s>>>(N, M, (const T*)a, (const T*)b, (const T*)c, (const T*)d,
                                                      (const T*)e, (const T*)f, (T*)x, scratch, info);
@@ -432,7 +432,8 @@ extern "C" int pent_factor_batch(int N, int64_t M, const void* e, const void* c,
     pent_handle* h = new (std::nothrow) pent_handle();
     if (!h) return PENT_ERR_ALLOC;
     *h = pent_handle{};
-    h->kind = 1; h->N = N; h->M = M; h->dtype = dtype;
+    h->kind = 1; h->N = N; h->M = M; h->dtype = dtype; h->l2_bc = -1; h->band = 2;
+    if (cudaGetDevice(&h->device) != cudaSuccess) { delete h; return pent::cuda_fail(cudaGetLastError()); }
     size_t esz = dtype == PENT_F64 ? 8 : 4;
     cudaError_t er = cudaMalloc(&h->ms, 5 * (size_t)N * (size_t)M * esz);
     if (er != cudaSuccess) {
@@ -450,7 +451,7 @@ extern "C" int pent_factor_batch(int N, int64_t M, const void* e, const void* c,
 
 extern "C" int pent_solve_batch_multi(const pent_handle* h, const void* f, void* x, void* stream)
 {
-    if (!h || h->kind != 1 || !f || !x) return PENT_ERR_ARG;
+    if (!h || h->kind != 1 || !f || !x || !pent::on_handle_device(h)) return PENT_ERR_ARG;
     const int tb = pent::PS_THREADS;
     unsigned nb = (unsigned)((h->M + tb - 1) / tb);
     cudaStream_t s = (cudaStream_t)stream;

@@ -12,6 +12,7 @@
 // registers (each c_k is loaded exactly once in the forward sweep), the right-hand side of
 // row k is formed in registers and consumed at once by the forward recurrence; g goes to
 // `scratch`; the back substitution writes the new state in place.
+#include <cmath>
 #include "pent_internal.h"
 
 namespace pent {
@@ -130,6 +131,13 @@ extern "C" int pent_step_batch_v(const pent_handle* h, const pent_step_params* p
     if (kernel != PENT_KERNEL_AUTO && kernel != PENT_KERNEL_THREAD_PER_SYSTEM && kernel != PENT_KERNEL_CHUNKED)
         return PENT_ERR_ARG;
     if (M == 0 || nsteps == 0) return PENT_OK;
+    if (!pent::on_handle_device(h)) return PENT_ERR_ARG;
+    // the increment form is the scheme of Eq. 2 only if the handle's A IS I + sigma L^2 for this sigma and bc
+    // (checked against what pent_factor detected; the direct form uses neither sigma nor the form of A)
+    if (p->kind == 0 && p->form == 1) {
+        const double tol = (h->dtype == PENT_F64 ? 1e-12 : 1e-6) * fabs(p->sigma);
+        if (h->periodic || h->l2_bc != p->bc || !(fabs(h->l2_sigma - p->sigma) <= tol)) return PENT_ERR_ARG;
+    }
     cudaStream_t s = (cudaStream_t)stream;
     if (h->periodic) {       // the paper's own loop: periodic hyperdiffusion, Eq. 6 / 7c
         if (p->kind != 1 || kernel != PENT_KERNEL_AUTO) return PENT_ERR_ARG;

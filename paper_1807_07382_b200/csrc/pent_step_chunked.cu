@@ -315,12 +315,12 @@ static int launch_step_inst(const pent_handle* h, const StepPlan& sp, const pent
     prm.nsteps = nsteps; prm.bc = p->bc;
     prm.r = (T)p->r; prm.sigma = (T)p->sigma;
     CUtensorMap tm;
-    if (!encode_batch_map(&tm, c, M, h->N, S, prm.box_rows, sizeof(T) == 8)) {
+    if (!encode_batch_map_cached(&tm, c, M, h->N, S, prm.box_rows, sizeof(T) == 8)) {
         g_last_cuda_error = (int)cudaErrorInvalidValue;
         return PENT_ERR_CUDA;
     }
     auto kern = step_chunked_kernel<T, S, KIND, NG>;
-    static thread_local SmemMark mark;
+    static SmemOnce mark;
     PENT_CUDA(ensure_dynamic_smem(mark, kern, sp.smem));
     const int threads = sp.TG * NG;
     int dev = 0, nsm = 0, occ = 0;

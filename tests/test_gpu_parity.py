@@ -9,6 +9,7 @@ import torch
 
 import oracle
 import pent_inputs as pin
+from gpu_helpers import Guarded, guarded, normwise, pinned_tol
 from pent_inputs.configs import WORKLOADS, banded_matvec, make_matrix, make_rhs, sine_modes
 
 pytestmark = pytest.mark.gpu
@@ -21,24 +22,25 @@ def _pent():
     return pent
 
 
-def normwise(x, ref):
-    return float(np.max(np.max(np.abs(x - ref), axis=0) / np.max(np.abs(ref), axis=0)))
-
-
 def residual(diags, x, f):
     r = banded_matvec(*diags, x.astype(np.float64)) - f
     return float(np.max(np.linalg.norm(r, axis=0) / np.linalg.norm(f, axis=0)))
 
 
 def gpu_solve(diags, f, dtype=torch.float64, kernel=0, inplace=False):
+    """f and x live between 1 MiB guard bands (gpu_helpers.Guarded); x starts as NaN sentinels."""
     pent = _pent()
     a, b, c, d, e = (torch.tensor(v, dtype=dtype) for v in diags)
     N, M = f.shape
     h = pent.pent_factor(N, e, c, d, a, b)
-    fd = torch.tensor(f, dtype=dtype, device="cuda")
-    xd = pent.pent_solve_batch(h, M, fd, fd if inplace else None, kernel=kernel)
-    torch.cuda.synchronize()
-    return xd.cpu().numpy(), h
+    fg = guarded(f, dtype)
+    xg = fg if inplace else Guarded((N, M), dtype)
+    pent.pent_solve_batch(h, M, fg.t, xg.t, kernel=kernel)
+    fg.check("(f)")
+    xg.check("(x)")
+    if not inplace:
+        assert torch.equal(fg.t.cpu(), torch.as_tensor(np.ascontiguousarray(f)).to(dtype)), "f was modified"
+    return xg.numpy(), h
 
 
 def oracle_for_dtype(diags, f, dtype):
@@ -101,20 +103,23 @@ def test_cfg3_full_size_every_system(dtype, kernel):
 
 
 @pytest.mark.parametrize("kernel", KERNELS)
-def test_cfg5a_n4096_sampled_and_residual(kernel):
-    """N=4096, M=32768 (1 GiB per array): oracle parity on a window of 2048 systems computed
-    one by one, residual on the same window; the rest is covered by the M-independence of the
-    kernels (each system is solved alone)."""
+def test_cfg5a_n4096_every_system(kernel):
+    """N=4096, M=32768 (1 GiB per array), in the launch configuration bench.py times: EVERY system is
+    compared with the oracle and the residual is taken over all of them (in slabs of 4096 systems to
+    bound the host memory of the transposed copies)."""
     w = WORKLOADS["cfg5a"]
-    pent = _pent()
     diags = make_matrix(w)
     f = make_rhs(w)
     x, _ = gpu_solve(diags, f, kernel=kernel)
-    cols = np.r_[0:512, 16000:16512, w.M - 1024:w.M]
-    ref = oracle.solve_batch(oracle.factor(*diags), np.ascontiguousarray(f[:, cols]), nthreads=8)
-    assert normwise(x[:, cols], ref) <= 1e-11
-    assert residual(diags, np.ascontiguousarray(x[:, cols]), np.ascontiguousarray(f[:, cols])) <= 1e-12
-    assert np.isfinite(x).all()
+    fac = oracle.factor(*diags)
+    worst_x = worst_r = 0.0
+    for c0 in range(0, w.M, 4096):
+        fs = np.ascontiguousarray(f[:, c0:c0 + 4096])
+        xs = np.ascontiguousarray(x[:, c0:c0 + 4096])
+        worst_x = max(worst_x, normwise(xs, oracle.solve_batch(fac, fs, nthreads=8)))
+        worst_r = max(worst_r, residual(diags, xs, fs))
+    assert worst_x <= 1e-11
+    assert worst_r <= 1e-12
 
 
 @pytest.mark.parametrize("kernel", KERNELS)
@@ -243,11 +248,17 @@ def test_chunked_cluster_slowly_decaying_coupling(Q, S):
     f = pin.uniform_pm1(81, 0, N, M)
     x, _ = gpu_solve(diags, f, kernel=pent.KERNEL_CHUNKED_CFG(Q, S))
     ref = oracle.solve_batch(oracle.factor(*diags), f)
-    # cond(A) ~ 1 + 16 sigma = 1.8e5: two correct fp64 solves differ by ~cond*eps (C-15)
-    assert normwise(x, ref) <= 4.0 * (1.0 + 16.0 * sigma) * 2.0 ** -53
-    # backward-stable solve: residual ~ eps*||A||*||x||/||f|| with ||A|| = 1 + 16 sigma = 1.8e5; the
-    # oracle's own residual on this input is 1.5e-12, so 1e-12 is scaled here
-    assert residual(diags, x, f) <= max(1e-12, (1.0 + 16.0 * sigma) * 2.0 ** -53)
+    # cond(A) ~ 1 + 16 sigma = 1.8e5: the error is measured against the long-double truth, and the bar is
+    # north_star's 1e-11 unless the fp64 oracle itself is further than half of that from the truth (C-15)
+    truth = oracle.ld_solve_batch(diags, f)
+    err_gpu, err_o64 = normwise(x, truth), normwise(ref, truth)
+    print(f"sigma=1.1e4 solve Q={Q} S={S}: GPU vs long double {err_gpu:.3e}, fp64 oracle vs long double {err_o64:.3e}")
+    assert err_gpu <= pinned_tol(1e-11, ref, truth)
+    # residual: north_star's 1e-12, unless the correctly ROUNDED truth itself leaves more than half of that
+    # (rounding x to fp64 alone leaves ~2^-53 ||A|| ||x|| / ||f||, with ||A|| = 1 + 16 sigma = 1.8e5)
+    res_gpu, res_truth = residual(diags, x, f), residual(diags, truth, f)
+    print(f"  residual: GPU {res_gpu:.3e}, rounded long-double truth {res_truth:.3e}, fp64 oracle {residual(diags, ref, f):.3e}")
+    assert res_gpu <= max(1e-12, 2.0 * res_truth)
 
 
 @pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
@@ -361,8 +372,11 @@ def test_system_major_layout_parity(dtype, N, M):
     f = pin.uniform_pm1(601 + N, 0, N, M)                      # interleaved (N, M)
     a, b, c, d, e = (torch.tensor(v, dtype=dtype) for v in diags)
     h = pent.pent_factor(N, e, c, d, a, b)
-    f_rows = torch.tensor(np.ascontiguousarray(f.T), dtype=dtype, device="cuda")     # (M, N), one system per row
-    x_rows = pent.pent_solve_batch_rows(h, M, f_rows)
+    fg = guarded(f.T, dtype)                                  # (M, N), one system per row
+    xg = Guarded((M, N), dtype)
+    f_rows, x_rows = fg.t, xg.t
+    pent.pent_solve_batch_rows(h, M, f_rows, x_rows)
+    fg.check("(f rows)"); xg.check("(x rows)")
     d64, f64, ref = oracle_for_dtype(diags, f, dtype)
     tol_x, tol_r = TOL[dtype]
     x = x_rows.cpu().numpy().T
@@ -370,6 +384,7 @@ def test_system_major_layout_parity(dtype, N, M):
     assert residual(d64, np.ascontiguousarray(x), f64) <= tol_r
     # in place, and identical to the interleaved solve of the same systems (same kernel arithmetic)
     pent.pent_solve_batch_rows(h, M, f_rows, f_rows)
+    fg.check("(in place rows)")
     assert torch.equal(f_rows, x_rows)
 
 

@@ -7,6 +7,7 @@ import torch
 
 import oracle
 import pent_inputs as pin
+from gpu_helpers import Guarded, check_all, guarded, normwise, pinned_tol
 
 pytestmark = pytest.mark.gpu
 
@@ -14,10 +15,6 @@ pytestmark = pytest.mark.gpu
 def _pent():
     import paper_1807_07382_b200 as pent
     return pent
-
-
-def normwise(x, ref):
-    return float(np.max(np.max(np.abs(x - ref), axis=0) / np.max(np.abs(ref), axis=0)))
 
 
 def residual(diags, x, f):
@@ -41,7 +38,10 @@ def test_periodic_nonsymmetric_parity(kernel, N, M):
     diags = pin.random_periodic_diag_dominant(300 + N, N)
     f = pin.uniform_pm1(301 + N, 0, N, M)
     h = _handle(diags)
-    x = pent.pent_solve_batch(h, M, torch.tensor(f, device="cuda"), kernel=kernel).cpu().numpy()
+    fg, xg = guarded(f), Guarded((N, M))
+    pent.pent_solve_batch(h, M, fg.t, xg.t, kernel=kernel)
+    check_all(fg, xg)
+    x = xg.numpy()
     ref = oracle.solve_periodic_batch(oracle.factor_periodic(*diags), f)
     assert normwise(x, ref) <= 1e-11
     assert residual(diags, x, f) <= 1e-12
@@ -63,17 +63,26 @@ def test_periodic_hyperdiffusion_matrix_full_batch_in_place_and_closed_form():
     diags = pin.periodic_hyperdiffusion_diagonals(N, sx)
     h = _handle(diags)
     f = pin.uniform_pm1(31, 0, N, M)
-    fd = torch.tensor(f, device="cuda")
-    x = pent.pent_solve_batch(h, M, fd, fd).cpu().numpy()
+    fg = guarded(f)
+    pent.pent_solve_batch(h, M, fg.t, fg.t)
+    fg.check("(in place)")
+    x = fg.numpy()
     ref = oracle.solve_periodic_batch(oracle.factor_periodic(*diags), f, nthreads=8)
-    # cond(A) = 1 + 16 sigma_x = 8.8e4: two correct fp64 solves differ by ~cond*eps
-    assert normwise(x, ref) <= max(1e-11, 4.0 * (1.0 + 16.0 * sx) * 2.0 ** -53)
+    # cond(A) = 1 + 16 sigma_x = 8.8e4: measured against the periodic solve in long double; bar = north_star's
+    # 1e-11, or twice the fp64 oracle's own distance from that truth if larger (reading C-15)
+    truth = oracle.ld_solve_periodic_batch(diags, f, nthreads=8)
+    err_gpu, err_o64 = normwise(x, truth), normwise(ref, truth)
+    print(f"periodic sigma_x=5.5e3: GPU vs long double {err_gpu:.3e}, fp64 oracle vs long double {err_o64:.3e}")
+    assert err_gpu <= pinned_tol(1e-11, ref, truth)
     j = np.arange(N)[:, None]
     m = np.arange(0, 64)[None, :]
     modes = np.cos(2 * np.pi * m * j / N)
     lam = 1.0 + 16.0 * sx * np.sin(np.pi * np.arange(64) / N) ** 4
     xm = pent.pent_solve_batch(h, 64, torch.tensor(modes, device="cuda")).cpu().numpy()
-    assert normwise(xm, modes / lam[None, :]) <= 4.0 * (1.0 + 16.0 * sx) * 2.0 ** -53
+    # the fp64 cosine samples are eigenvectors only up to their own rounding, which A^{-1} amplifies relative to
+    # the small high-mode answers f/lambda: the closed form is compared at the oracle's own distance from it
+    om = oracle.solve_periodic_batch(oracle.factor_periodic(*diags), modes)
+    assert normwise(xm, modes / lam[None, :]) <= max(1e-11, 2.0 * normwise(om, modes / lam[None, :]))
 
 
 def test_periodic_fp32_and_host_entry_point():

@@ -8,6 +8,7 @@ import torch
 
 import oracle
 import pent_inputs as pin
+from gpu_helpers import Guarded, check_all, guarded, normwise, pinned_tol
 from pent_inputs.configs import R_CH, SIGMA_CH, WORKLOADS, banded_matvec, make_matrix, make_rhs
 
 pytestmark = pytest.mark.gpu
@@ -16,10 +17,6 @@ pytestmark = pytest.mark.gpu
 def _pent():
     import paper_1807_07382_b200 as pent
     return pent
-
-
-def normwise(x, ref):
-    return float(np.max(np.max(np.abs(x - ref), axis=0) / np.max(np.abs(ref), axis=0)))
 
 
 def residual(diags, x, f):
@@ -41,16 +38,22 @@ def test_factor_solve_batch_parity(N, M):
     else:
         diags = pin.random_diag_dominant(60 + N, N, M)
     f = pin.uniform_pm1(6, 0, N, M)
-    a, b, c, d, e = (_dev(v) for v in diags)
-    x, info = pent.pent_factor_solve_batch(N, M, e, c, d, a, b, _dev(f))
-    torch.cuda.synchronize()
+    gs = [guarded(v) for v in diags]
+    a, b, c, d, e = (g.t for g in gs)
+    fg, xg = guarded(f), Guarded((N, M))
+    ig = Guarded((M,), torch.int32)
+    wg = Guarded((3 * N * ((M + 63) // 64 * 64),))
+    x, info = pent.pent_factor_solve_batch(N, M, e, c, d, a, b, fg.t, xg.t, ig.t, workspace=wg.t)
+    check_all(fg, xg, ig, wg, *gs)
     ref, rinfo = oracle.factor_solve_batch(*diags, f, nthreads=8)
     assert not info.cpu().numpy().any() and not rinfo.any()
     assert normwise(x.cpu().numpy(), ref) <= 1e-11
     assert residual(diags, x.cpu().numpy(), f) <= 1e-12
     # stored-factor route gives the same answers
-    h, info2 = pent.pent_factor_batch(N, M, e, c, d, a, b)
-    x2 = pent.pent_solve_batch_multi(h, _dev(f))
+    ig2, xg2 = Guarded((M,), torch.int32), Guarded((N, M))
+    h, info2 = pent.pent_factor_batch(N, M, e, c, d, a, b, ig2.t)
+    x2 = pent.pent_solve_batch_multi(h, fg.t, xg2.t)
+    check_all(fg, xg2, ig2, *gs)
     assert not info2.cpu().numpy().any()
     assert normwise(x2.cpu().numpy(), ref) <= 1e-11
 
@@ -113,14 +116,21 @@ def test_ch_one_step_parity(kernel, bc, bcname, form, N, M):
     diags, sigma, r, c0 = _ch_setup(N, M, bcname)
     a, b, c, d, e = (torch.tensor(v) for v in diags)
     h = pent.pent_factor(N, e, c, d, a, b)
-    cd = _dev(c0)
-    pent.pent_step_batch(h, M, cd, 1, kind=0, bc=bc, form=form, r=r, sigma=sigma, kernel=kernel)
+    cg = guarded(c0)
+    sg = Guarded((N, M))
+    pent.pent_step_batch(h, M, cg.t, 1, kind=0, bc=bc, form=form, r=r, sigma=sigma, kernel=kernel, scratch=sg.t)
+    check_all(cg, sg)
     ref = oracle.step_batch(oracle.factor(*diags), 0, bc, form, r, sigma, c0, 1)
-    # Two correct fp64 evaluations of one step differ by ~cond(A)*eps (no-pivot LU forward
-    # error); cond(I + sigma L^2) <= 1 + 16 sigma.  At N=1024 sigma = 1.1e4, cond*eps = 2e-11:
-    # the oracle's own direct and increment forms differ by 1.6e-11 there (C-15).
-    tol = max(1e-11, 4.0 * (1.0 + 16.0 * sigma) * 2.0 ** -53)
-    assert normwise(cd.cpu().numpy(), ref) <= tol
+    # The error is measured against the same step evaluated in long double (oracle/pent_oracle_ld.c).  Bar:
+    # north_star's 1e-11, or twice the fp64 oracle's own distance from that truth where it is larger (at
+    # N >= 1000, sigma = 1.1e4, the increment form of the fp64 oracle is 1.2e-11 away: DESIGN.md C-15).
+    truth = oracle.ld_step_batch(diags, 0, bc, form, r, sigma, c0, 1)
+    got = cg.numpy()
+    err_gpu, err_o64 = normwise(got, truth), normwise(ref, truth)
+    if N >= 1000:
+        print(f"CH one step N={N} bc={bc} form={form} kernel={kernel}: GPU vs long double {err_gpu:.3e}, "
+              f"fp64 oracle vs long double {err_o64:.3e}, GPU vs fp64 oracle {normwise(got, ref):.3e}")
+    assert err_gpu <= pinned_tol(1e-11, ref, truth)
 
 
 @pytest.mark.parametrize("kernel,N,M", [(1, 300, 129), (2, 300, 130), (2, 1024, 64), (2, 33, 20), (0, 300, 129)])
@@ -130,10 +140,11 @@ def test_hyperdiffusion_step_parity_general_matrix(kernel, N, M):
     a, b, c, d, e = (torch.tensor(v) for v in diags)
     h = pent.pent_factor(N, e, c, d, a, b)
     c0 = pin.uniform_pm1(22, 0, N, M)
-    cd = _dev(c0)
-    pent.pent_step_batch(h, M, cd, 3, kind=1, kernel=kernel)
+    cg, sg = guarded(c0), Guarded((N, M))
+    pent.pent_step_batch(h, M, cg.t, 3, kind=1, kernel=kernel, scratch=sg.t)
+    check_all(cg, sg)
     ref = oracle.step_batch(oracle.factor(*diags), 1, 0, 0, 0.0, 0.0, c0, 3)
-    assert normwise(cd.cpu().numpy(), ref) <= 1e-11
+    assert normwise(cg.numpy(), ref) <= 1e-11
 
 
 def test_multi_step_on_chip_equals_repeated_single_steps():
@@ -151,29 +162,31 @@ def test_multi_step_on_chip_equals_repeated_single_steps():
         pent.pent_step_batch(h, M, c2, 1, kind=0, bc=1, form=1, r=r, sigma=sigma, kernel=2)
     assert torch.equal(c1, c2)
     ref = oracle.step_batch(oracle.factor(*diags), 0, 1, 1, r, sigma, c0, 7)
-    assert normwise(c1.cpu().numpy(), ref) <= 7 * max(1e-11, 4.0 * (1.0 + 16.0 * sigma) * 2.0 ** -53)
+    truth = oracle.ld_step_batch(diags, 0, 1, 1, r, sigma, c0, 7)
+    assert normwise(c1.cpu().numpy(), truth) <= pinned_tol(7e-11, ref, truth)     # 7 steps of the 1e-11 bar
 
 
 @pytest.mark.parametrize("kernel", STEP_KERNELS)
 def test_cfg4_thousand_steps_conservation_and_trajectory(kernel):
     """BASELINE.json configs[3]: N=1024, M=8192, 1000 fused steps, zero-flux L, increment form.
-    mean(c) per run conserved to 1e-12 (every system, fsum on the host); trajectory parity with
-    the oracle after 1000 nonlinear steps on a window of 64 systems to 1e-9."""
+    mean(c) per run conserved to 1e-12 on EVERY system (fsum on the host); trajectory parity with
+    the oracle after 1000 nonlinear steps on 1024 systems (every eighth) to 1e-9."""
     pent = _pent()
     w = WORKLOADS["cfg4"]
     diags = make_matrix(w)
     c0 = make_rhs(w)
     a, b, c, d, e = (torch.tensor(v) for v in diags)
     h = pent.pent_factor(w.N, e, c, d, a, b)
-    cd = _dev(c0)
-    scratch = torch.empty_like(cd)
-    pent.pent_step_batch(h, w.M, cd, 1000, kind=0, bc=1, form=1, r=R_CH, sigma=SIGMA_CH,
-                         scratch=scratch, kernel=kernel)
-    c1 = cd.cpu().numpy()
+    cg, sg = guarded(c0), Guarded((w.N, w.M))
+    pent.pent_step_batch(h, w.M, cg.t, 1000, kind=0, bc=1, form=1, r=R_CH, sigma=SIGMA_CH,
+                         scratch=sg.t, kernel=kernel)
+    check_all(cg, sg)
+    c1 = cg.numpy()
     assert np.isfinite(c1).all()
-    drift = max(abs(math.fsum(c1[:, i]) - math.fsum(c0[:, i])) / w.N for i in range(0, w.M, 3))
+    c1r, c0r = np.ascontiguousarray(c1.T), np.ascontiguousarray(c0.T)
+    drift = max(abs(math.fsum(c1r[i]) - math.fsum(c0r[i])) / w.N for i in range(w.M))
     assert drift <= 1e-12
-    cols = np.r_[0:32, w.M - 32:w.M]
+    cols = np.arange(0, w.M, 8)
     ref = oracle.step_batch(oracle.factor(*diags), 0, 1, 1, R_CH, SIGMA_CH,
                             np.ascontiguousarray(c0[:, cols]), 1000, nthreads=8)
     assert normwise(c1[:, cols], ref) <= 1e-9
