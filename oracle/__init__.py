@@ -173,6 +173,28 @@ def step_batch(fac: Factors, kind: int, bc: int, form: int, r: float, sigma: flo
     return np.ascontiguousarray(Crows.T)
 
 
+def forcing(N: int, t: float, mu1: float, mu2: float) -> np.ndarray:
+    """Phi(x_k, t; mu1, mu2) of the forced Cahn-Hilliard equation (reading C-22)."""
+    out = np.empty(N)
+    _load().pent_oracle_forcing(C.c_int(N), C.c_double(t), C.c_double(mu1), C.c_double(mu2), _p(out))
+    return out
+
+
+def step_forced_batch(fac: Factors, bc: int, form: int, r: float, sigma: float, dt: float, t0: float,
+                      mu1, mu2, c_interleaved, nsteps: int, nthreads: int = 1) -> np.ndarray:
+    """nsteps forced Cahn-Hilliard steps (Eq. 3) with per-system parameters mu1[i], mu2[i]."""
+    Crows = to_rows(c_interleaved)
+    M = Crows.shape[0]
+    mu1, mu2 = _f64(mu1), _f64(mu2)
+    assert mu1.shape == (M,) and mu2.shape == (M,)
+    _load().pent_oracle_step_forced_rows(
+        C.c_int(fac.N), C.c_long(M), C.c_int(bc), C.c_int(form), C.c_double(r), C.c_double(sigma),
+        C.c_double(dt), C.c_double(t0), _p(mu1), _p(mu2), *[_p(v) for v in fac.diags],
+        _p(fac.eps), _p(fac.beta), _p(fac.alpha), _p(fac.gamma), _p(fac.delta),
+        _p(Crows), C.c_int(nsteps), C.c_int(nthreads))
+    return np.ascontiguousarray(Crows.T)
+
+
 # ---- periodic (cyclic) pentadiagonal systems, PAPER.md:104-146 (pent_oracle_periodic.c) -----------
 @dataclass
 class PeriodicFactors:

@@ -102,3 +102,61 @@ void pent_oracle_step_rows(int N, long M, int kind, int bc, int form, double r, 
         free(buf);
     }
 }
+
+/* ---------------------------------------------------------------------------------------
+ * Forced Cahn-Hilliard, PAPER.md:63-67 (Remark 1, Eq. 3): dC/dt = [Eq. 1a] + Phi(x, t, mu_1, mu_2, ...),
+ * "a parameter study based on the model (3) provides the motivation for batch programming in this
+ * work": every system i of the batch has its own parameters (mu_1[i], mu_2[i]).
+ * The paper specifies no Phi.  Reading C-22: a zero-mean travelling wave
+ *     Phi(x, t; mu_1, mu_2) = mu_1 cos(2 pi (x - mu_2 t)),     x_k = (k + 1/2) / N  (cell centres, L = 1),
+ * treated explicitly like the other bracketed term of Eq. 2 (evaluated at t_n = t0 + n dt):
+ *     (C+ - C)/dt = [D d_xx (C^3 - C)]^n - gamma D d_xxxx C+ + Phi^n
+ *  => form 0:  A C+ = C + r L w + dt Phi^n ;     form 1:  A delta = L q + dt Phi^n,  C+ = C + delta.
+ * sum_k Phi(x_k) = 0 on this grid, so the zero-flux scheme still conserves mean(C).
+ * ------------------------------------------------------------------------------------- */
+#include <math.h>
+
+void pent_oracle_forcing(int N, double t, double mu1, double mu2, double *phi)
+{
+    const double two_pi = 6.283185307179586476925286766559;
+    int k;
+    for (k = 0; k < N; ++k) {
+        double x = ((double)k + 0.5) / (double)N;
+        phi[k] = mu1 * cos(two_pi * (x - mu2 * t));
+    }
+}
+
+/* nsteps forced steps (kind 0 only) on a batch in the serial layout (M x N row-major, in place);
+ * mu1, mu2: M per-system parameters; step n of the call is taken at t_n = t0 + n dt. */
+void pent_oracle_step_forced_rows(int N, long M, int bc, int form, double r, double sigma,
+                                  double dt, double t0, const double *mu1, const double *mu2,
+                                  const double *a, const double *b, const double *c, const double *d,
+                                  const double *e,
+                                  const double *eps, const double *beta, const double *alpha,
+                                  const double *gamma, const double *delta,
+                                  double *C, int nsteps, int nthreads)
+{
+    long i;
+    (void)nthreads;
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static) num_threads(nthreads > 0 ? nthreads : 1)
+#endif
+    for (i = 0; i < M; ++i) {
+        double *buf = (double *)malloc((size_t)5 * N * sizeof(double));
+        double *rhs = buf, *sol = buf + N, *work = buf + 2 * N, *phi = buf + 4 * N;
+        double *Ci = C + (size_t)i * N;
+        int s, k;
+        for (s = 0; s < nsteps; ++s) {
+            double t = t0 + (double)s * dt;
+            pent_oracle_rhs(N, 0, bc, form, r, sigma, a, b, c, d, e, Ci, rhs, work);
+            pent_oracle_forcing(N, t, mu1[i], mu2[i], phi);
+            for (k = 0; k < N; ++k) rhs[k] = rhs[k] + dt * phi[k];
+            pent_oracle_solve(N, eps, beta, alpha, gamma, delta, rhs, sol);
+            if (form == 1)
+                for (k = 0; k < N; ++k) Ci[k] = Ci[k] + sol[k];
+            else
+                for (k = 0; k < N; ++k) Ci[k] = sol[k];
+        }
+        free(buf);
+    }
+}

@@ -63,3 +63,62 @@ def pinned_tol(floor, oracle64, truth):
     """Parity tolerance tied to a measurement (reading C-15): the north_star bar `floor`, or twice
     the distance of the fp64 oracle from the long-double truth on the same inputs when that is larger."""
     return max(floor, 2.0 * normwise(oracle64, truth))
+
+
+def chunked_order_solve_fp64(fac, f, C=32):
+    """The SAME linear solve A^{-1} f evaluated in plain numpy fp64 in the ORDER the on-chip kernel uses
+    (DESIGN.md section 6.2): rows cut into chunks of C, each chunk swept forward and
+    backward from a ZERO state, the chunks stitched exactly through the responses of
+    the two recurrences to a unit incoming state.  Written from DESIGN.md for the tests only (it shares
+    no code with csrc/): it measures what this evaluation order costs in fp64 rounding on a given input,
+    so that the parity tolerance on stiff matrices is a measured envelope, not a fitted constant
+    (reading C-15).  fac: oracle.Factors; f: interleaved (N, M).  Returns x (N, M)."""
+    N, M = f.shape
+    P = (N + C - 1) // C
+    Np = P * C
+    pad = lambda v, fill=0.0: np.concatenate([np.asarray(v, dtype=np.float64), np.full(Np - N, fill)])
+    ia = pad(1.0 / fac.alpha); en = pad(fac.eps / fac.alpha); bn = pad(fac.beta / fac.alpha)
+    ga = pad(fac.gamma); de = pad(fac.delta)
+    ia[N:] = 0.0
+    fp = np.zeros((Np, M)); fp[:N] = f
+    g = np.zeros((Np, M)); xh = np.zeros((Np, M))
+    phi = np.zeros((Np, 2)); chi = np.zeros((Np, 2)); psi = np.zeros((Np, 2))
+    for p in range(P):
+        s = p * C
+        g1 = g2 = np.zeros(M)
+        h1, h2 = np.array([0.0, 1.0]), np.array([1.0, 0.0])              # unit incoming states (g_{s-1}, g_{s-2})
+        for k in range(s, s + C):
+            gk = ia[k] * fp[k] - en[k] * g2 - bn[k] * g1
+            g[k] = gk; g2, g1 = g1, gk
+            hk = -en[k] * h2 - bn[k] * h1
+            phi[k] = hk; h2, h1 = h1, hk
+        x1 = x2 = np.zeros(M)
+        c1 = c2 = np.zeros(2)
+        q1, q2 = np.array([1.0, 0.0]), np.array([0.0, 1.0])              # unit incoming states (x_{e+1}, x_{e+2})
+        for k in range(s + C - 1, s - 1, -1):
+            xk = g[k] - ga[k] * x1 - de[k] * x2
+            xh[k] = xk; x2, x1 = x1, xk
+            ck = phi[k] - ga[k] * c1 - de[k] * c2
+            chi[k] = ck; c2, c1 = c1, ck
+            qk = -ga[k] * q1 - de[k] * q2
+            psi[k] = qk; q2, q1 = q1, qk
+    F = np.zeros((P + 1, 2, M))                                          # F[p+1] = (g_{e-1}, g_e) of chunk p
+    for p in range(P):
+        e = p * C + C
+        F[p + 1] = g[e - 2:e] + phi[e - 2:e] @ F[p]
+    B = np.zeros((P + 1, 2, M))                                          # B[p] = (x_s, x_{s+1}) of chunk p
+    for p in range(P - 1, -1, -1):
+        s = p * C
+        B[p] = xh[s:s + 2] + chi[s:s + 2] @ F[p] + psi[s:s + 2] @ B[p + 1]
+    x = np.zeros((Np, M))
+    for p in range(P):
+        sl = slice(p * C, p * C + C)
+        x[sl] = xh[sl] + chi[sl] @ F[p] + psi[sl] @ B[p + 1]
+    return x[:N]
+
+
+def envelope_tol(floor, truth, *fp64_evaluations):
+    """Parity tolerance tied to measurements (reading C-15): north_star's bar `floor`, or twice the
+    largest distance from the long-double truth of the given plain-fp64 CPU evaluations of the same quantity
+    (the oracle's serial sweep; the chunked evaluation order) when that is larger."""
+    return max(floor, 2.0 * max(normwise(v, truth) for v in fp64_evaluations))

@@ -36,7 +36,7 @@ def test_factor_runs_on_a_private_stream_and_stalls_nobody():
     """pent_factor / pent_factor_periodic while a long kernel runs on another stream: the call returns long
     before that kernel ends (it neither waits for it nor synchronises the device)."""
     pent = _pent()
-    N, M = 1024, 148 * 16
+    N, M = 1024, 64 * 16          # 64 persistent CTAs: the long kernel leaves 84 SMs free for the factor kernels
     diags = pin.diagonals_I_plus_sigma_L2(N, 10.0, "zeroflux")
     h = _handle(diags)
     _periodic_handle(pin.periodic_hyperdiffusion_diagonals(64, 1.0))          # warm-up: module load, lazy init
