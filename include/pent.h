@@ -183,6 +183,28 @@ int pent_step_batch_v(const pent_handle* h, const pent_step_params* p, int64_t M
 /* Which kernel pent_step_batch runs for M systems: PENT_KERNEL_CHUNKED or PENT_KERNEL_THREAD_PER_SYSTEM. */
 int pent_step_kernel_choice(const pent_handle* h, int64_t M);
 
+/* ---- forced Cahn-Hilliard, one parameter set per system (Remark 1, Eq. 3) -----------
+ * "A parameter study based on the model (3) provides the motivation for batch programming in this work":
+ * system i of the batch is the run with parameters (mu1[i], mu2[i]).  The paper names no Phi; this library
+ * implements a zero-mean travelling wave (reading C-22)
+ *     Phi(x, t; mu1, mu2) = mu1 cos(2 pi (x - mu2 t)),   x_k = (k + 1/2) / N   (cell centres of the unit interval),
+ * treated explicitly like the other bracketed term of Eq. 2: step n of a call is taken at t_n = t0 + n dt and adds
+ * dt * Phi(x_k, t_n) to row k of the right-hand side of pent_step_batch(kind 0) (either form).  sum_k Phi(x_k) = 0,
+ * so the zero-flux scheme still conserves mean(c).  p->kind must be 0; g->kind 0 = no forcing (= pent_step_batch).
+ * mu1, mu2: device, M elements of the handle's dtype.  Everything else as pent_step_batch; still ONE kernel for
+ * all nsteps (the forcing is formed in registers from two per-system amplitudes per step). */
+typedef struct {
+    int kind;           /* 0 none, 1 travelling wave */
+    double dt;          /* time step (the forcing enters the right-hand side as dt * Phi) */
+    double t0;          /* time of the first step of this call */
+    const void* mu1;    /* device, M: amplitude */
+    const void* mu2;    /* device, M: wave speed */
+} pent_forcing;
+int pent_step_batch_forced(const pent_handle* h, const pent_step_params* p, const pent_forcing* g, int64_t M,
+                           void* c_inout, void* scratch, int nsteps, void* stream);
+int pent_step_batch_forced_v(const pent_handle* h, const pent_step_params* p, const pent_forcing* g, int64_t M,
+                             void* c_inout, void* scratch, int nsteps, void* stream, int kernel);
+
 /* ---- introspection ------------------------------------------------------------------------ */
 int pent_handle_n(const pent_handle* h);                 /* N, or -1 */
 int pent_handle_dtype(const pent_handle* h);             /* pent_dtype, or -1 */

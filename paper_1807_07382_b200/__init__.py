@@ -53,6 +53,11 @@ class pent_step_params(C.Structure):
                 ("r", C.c_double), ("sigma", C.c_double)]
 
 
+class pent_forcing(C.Structure):
+    _fields_ = [("kind", C.c_int), ("dt", C.c_double), ("t0", C.c_double),
+                ("mu1", C.c_void_p), ("mu2", C.c_void_p)]
+
+
 def lib() -> C.CDLL:
     """Load (building if needed) libpent.so.  Raises if that is impossible."""
     global _lib
@@ -80,6 +85,9 @@ def lib() -> C.CDLL:
     L.pent_step_batch.argtypes = [vp, C.POINTER(pent_step_params), i64, vp, vp, ci, vp]
     L.pent_step_batch_v.argtypes = [vp, C.POINTER(pent_step_params), i64, vp, vp, ci, vp, ci]
     L.pent_step_kernel_choice.argtypes = [vp, i64]
+    L.pent_step_batch_forced.argtypes = [vp, C.POINTER(pent_step_params), C.POINTER(pent_forcing), i64, vp, vp, ci, vp]
+    L.pent_step_batch_forced_v.argtypes = [vp, C.POINTER(pent_step_params), C.POINTER(pent_forcing), i64, vp, vp, ci,
+                                           vp, ci]
     L.pent_handle_n.argtypes = [vp]
     L.pent_handle_dtype.argtypes = [vp]
     L.pent_handle_m.argtypes = [vp]
@@ -284,14 +292,24 @@ def pent_solve_batch_multi(h: Handle, f: torch.Tensor, x: torch.Tensor | None = 
 def pent_step_batch(h: Handle, M: int, c: torch.Tensor, nsteps: int, *, kind: int = 0, bc: int = 1,
                     form: int = 1, r: float = 0.0, sigma: float = 0.0,
                     scratch: torch.Tensor | None = None, stream=None,
-                    kernel: int = KERNEL_AUTO) -> torch.Tensor:
-    """nsteps fused steps (RHS + solve in one kernel) in place on c (N, M).  See include/pent.h."""
+                    kernel: int = KERNEL_AUTO, forcing=None) -> torch.Tensor:
+    """nsteps fused steps (RHS + solve in one kernel) in place on c (N, M).  See include/pent.h.
+    forcing = (mu1, mu2, dt, t0): the forced Cahn-Hilliard equation with per-system
+    parameters mu1, mu2 (CUDA tensors of M elements of the handle's dtype); pent_step_batch_forced."""
     _batch(c, "c", (h.N, M), h.dtype)
     p = pent_step_params(kind, bc, form, r, sigma)
     if scratch is not None:
         _vec(scratch, "scratch", h.N * M, h.dtype)
     sp = 0 if scratch is None else scratch.data_ptr()
-    _check(lib().pent_step_batch_v(h.ptr, C.byref(p), M, c.data_ptr(), sp, nsteps, _stream(stream), kernel))
+    if forcing is None:
+        _check(lib().pent_step_batch_v(h.ptr, C.byref(p), M, c.data_ptr(), sp, nsteps, _stream(stream), kernel))
+        return c
+    mu1, mu2, dt, t0 = forcing
+    _vec(mu1, "mu1", M, h.dtype)
+    _vec(mu2, "mu2", M, h.dtype)
+    g = pent_forcing(1, float(dt), float(t0), mu1.data_ptr(), mu2.data_ptr())
+    _check(lib().pent_step_batch_forced_v(h.ptr, C.byref(p), C.byref(g), M, c.data_ptr(), sp, nsteps,
+                                          _stream(stream), kernel))
     return c
 
 

@@ -58,7 +58,8 @@ __global__ void factor_shared(int N, const double* __restrict__ dg, double* __re
 // Sweep-ready tables (one thread per row):
 //   fw[k] = {1/alpha, eps/alpha, beta/alpha, 0}:  g_k = fw.x f_k - fw.y g_{k-2} - fw.z g_{k-1}
 //   bw[k] = {gamma, delta}:                        x_k = g_k - bw.x x_{k+1} - bw.y x_{k+2}
-//   dgT[k] = {a,b,c,d,e,0,0,0} in T (original diagonals, for the (2I-A)c right-hand side)
+//   dgT[k] = {a,b,c,d,e, cos(2 pi x_k), sin(2 pi x_k), 0} in T: the original diagonals (for the (2I-A)c
+//            right-hand side) and the space factors of the travelling-wave forcing at x_k = (k + 1/2)/N
 // All divisions of the solve are done here, once (fp64 division is a long software sequence
 // on the GPU); the per-unknown work of the sweeps is then 1 mul + 4 fma.
 template <typename T>
@@ -76,7 +77,9 @@ __global__ void derive_tables(int N, const double* __restrict__ dg, const double
     v.x = (T)fac[3 * N + k]; v.y = (T)fac[4 * N + k];
     bw[k] = v;
     for (int j = 0; j < 5; ++j) dgT[8 * k + j] = (T)dg[j * N + k];
-    for (int j = 5; j < 8; ++j) dgT[8 * k + j] = (T)0;
+    double sx, cx;
+    sincospi((2.0 * k + 1.0) / (double)N, &sx, &cx);
+    dgT[8 * k + 5] = (T)cx; dgT[8 * k + 6] = (T)sx; dgT[8 * k + 7] = (T)0;
 }
 
 int build_chunk_tables(pent_handle* h, cudaStream_t s);   // pent_solve_chunked.cu

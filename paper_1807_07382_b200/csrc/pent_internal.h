@@ -126,8 +126,8 @@ int launch_solve_chunked(const pent_handle* h, int64_t M, const void* f, void* x
                          int Q, int S);
 bool chunked_supported(const pent_handle* h, int64_t M, const void* f /* may be null */, int Q, int S);
 bool step_chunked_supported(const pent_handle* h, int64_t M, const void* c /* may be null */);
-int launch_step_chunked(const pent_handle* h, const pent_step_params* p, int64_t M, void* c, int nsteps,
-                        cudaStream_t s);
+int launch_step_chunked(const pent_handle* h, const pent_step_params* p, const pent_forcing* g, int64_t M, void* c,
+                        int nsteps, cudaStream_t s);
 bool periodic_fused_supported(const pent_handle* h, int64_t M, const void* f /* may be null */);
 int launch_solve_chunked_periodic(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s);
 int solve_periodic(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s, int kernel);

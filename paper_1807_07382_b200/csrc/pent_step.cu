@@ -21,6 +21,10 @@ template <typename T>
 struct StepCoef {
     int kind, bc, form;
     T r, sigma;
+    // forcing (reading C-22): rhs_k += dt mu1_i cos(2 pi (x_k - mu2_i t)); mu1 == nullptr: none
+    const T* mu1;
+    const T* mu2;
+    double dt, t;
 };
 
 template <typename T>
@@ -51,6 +55,15 @@ step_tps_kernel(int N, int64_t M, const typename Vec<T>::T4* __restrict__ fw,
         if (p.form == 0) u0 = w0;
         else u0 = fma(-p.sigma, fma(Ldiag<T>(0, N, p.bc), c0, cp1), p.r * w0);   // q_0
     }
+    // forcing amplitudes of this system at this step: dt mu1 (cos, sin)(2 pi mu2 t); the space factors
+    // cos / sin(2 pi x_k) sit in slots 5, 6 of the dg table
+    T fa = 0, fb = 0;
+    if (p.mu1) {
+        double sn, cs;
+        sincospi(2.0 * (double)p.mu2[i] * p.t, &sn, &cs);
+        const double am = p.dt * (double)p.mu1[i];
+        fa = (T)(am * cs); fb = (T)(am * sn);
+    }
     T g1 = 0, g2 = 0;
     for (int k = 0; k < N; ++k) {
         T cn = (k + 3 < N) ? __ldcs(ci + (int64_t)(k + 3) * M) : (T)0;   // c_{k+3}, prefetch
@@ -73,6 +86,7 @@ step_tps_kernel(int N, int64_t M, const typename Vec<T>::T4* __restrict__ fw,
             }
             T Lu = um1 + fma(Ldiag<T>(k, N, p.bc), u0, up1);
             rhs = (p.form == 0) ? fma(p.r, Lu, c0) : Lu;
+            if (p.mu1) rhs = fma(fa, __ldg(dgt + 8 * k + 5), fma(fb, __ldg(dgt + 8 * k + 6), rhs));
             um1 = u0; u0 = up1;
         }
         typename Vec<T>::T4 cf = ldg4(fw + k);
@@ -93,7 +107,7 @@ step_tps_kernel(int N, int64_t M, const typename Vec<T>::T4* __restrict__ fw,
 }
 
 template <typename T>
-static int step_impl(const pent_handle* h, const pent_step_params* p, int64_t M, void* c,
+static int step_impl(const pent_handle* h, const pent_step_params* p, const pent_forcing* fg, int64_t M, void* c,
                      void* scratch, int nsteps, cudaStream_t s)
 {
     T* sc = (T*)scratch;
@@ -104,11 +118,13 @@ static int step_impl(const pent_handle* h, const pent_step_params* p, int64_t M,
         PENT_CUDA(er);
         own = true;
     }
-    StepCoef<T> sp{p->kind, p->bc, p->form, (T)p->r, (T)p->sigma};
+    StepCoef<T> sp{p->kind, p->bc, p->form, (T)p->r, (T)p->sigma, nullptr, nullptr, 0.0, 0.0};
+    if (fg && fg->kind == 1) { sp.mu1 = (const T*)fg->mu1; sp.mu2 = (const T*)fg->mu2; sp.dt = fg->dt; }
     const int tb = 128;
     unsigned nb = (unsigned)((M + tb - 1) / tb);
     cudaError_t le = cudaSuccess;
     for (int it = 0; it < nsteps && le == cudaSuccess; ++it) {
+        if (sp.mu1) sp.t = fg->t0 + (double)it * fg->dt;
         step_tps_kernel<T><<<nb, tb, 0, s>>>(h->N, M, (const typename Vec<T>::T4*)h->fw,
                                              (const typename Vec<T>::T2*)h->bw, (const T*)h->dg,
                                              sp, (T*)c, sc);
@@ -121,8 +137,8 @@ static int step_impl(const pent_handle* h, const pent_step_params* p, int64_t M,
 }
 }  // namespace pent
 
-extern "C" int pent_step_batch_v(const pent_handle* h, const pent_step_params* p, int64_t M,
-                                 void* c_inout, void* scratch, int nsteps, void* stream, int kernel)
+extern "C" int pent_step_batch_forced_v(const pent_handle* h, const pent_step_params* p, const pent_forcing* g,
+                                        int64_t M, void* c_inout, void* scratch, int nsteps, void* stream, int kernel)
 {
     if (!h || h->kind != 0 || !p || M < 0 || nsteps < 0 || !c_inout) return PENT_ERR_ARG;
     if (p->kind != 0 && p->kind != 1) return PENT_ERR_ARG;
@@ -130,6 +146,11 @@ extern "C" int pent_step_batch_v(const pent_handle* h, const pent_step_params* p
         return PENT_ERR_ARG;
     if (kernel != PENT_KERNEL_AUTO && kernel != PENT_KERNEL_THREAD_PER_SYSTEM && kernel != PENT_KERNEL_CHUNKED)
         return PENT_ERR_ARG;
+    if (g) {
+        if (g->kind != 0 && g->kind != 1) return PENT_ERR_ARG;
+        if (g->kind == 1 && (p->kind != 0 || !g->mu1 || !g->mu2)) return PENT_ERR_ARG;   // Eq. 3 forces Eq. 1 only
+        if (g->kind == 0) g = nullptr;
+    }
     if (M == 0 || nsteps == 0) return PENT_OK;
     if (!pent::on_handle_device(h)) return PENT_ERR_ARG;
     // the increment form is the scheme of Eq. 2 only if the handle's A IS I + sigma L^2 for this sigma and bc
@@ -146,15 +167,27 @@ extern "C" int pent_step_batch_v(const pent_handle* h, const pent_step_params* p
     const bool on_chip = pent::step_chunked_supported(h, M, c_inout);
     if (kernel == PENT_KERNEL_CHUNKED && !on_chip) return PENT_ERR_ARG;
     if (kernel != PENT_KERNEL_THREAD_PER_SYSTEM && on_chip)
-        return pent::launch_step_chunked(h, p, M, c_inout, nsteps, s);
-    if (h->dtype == PENT_F64) return pent::step_impl<double>(h, p, M, c_inout, scratch, nsteps, s);
-    return pent::step_impl<float>(h, p, M, c_inout, scratch, nsteps, s);
+        return pent::launch_step_chunked(h, p, g, M, c_inout, nsteps, s);
+    if (h->dtype == PENT_F64) return pent::step_impl<double>(h, p, g, M, c_inout, scratch, nsteps, s);
+    return pent::step_impl<float>(h, p, g, M, c_inout, scratch, nsteps, s);
+}
+
+extern "C" int pent_step_batch_forced(const pent_handle* h, const pent_step_params* p, const pent_forcing* g,
+                                      int64_t M, void* c_inout, void* scratch, int nsteps, void* stream)
+{
+    return pent_step_batch_forced_v(h, p, g, M, c_inout, scratch, nsteps, stream, PENT_KERNEL_AUTO);
+}
+
+extern "C" int pent_step_batch_v(const pent_handle* h, const pent_step_params* p, int64_t M,
+                                 void* c_inout, void* scratch, int nsteps, void* stream, int kernel)
+{
+    return pent_step_batch_forced_v(h, p, nullptr, M, c_inout, scratch, nsteps, stream, kernel);
 }
 
 extern "C" int pent_step_batch(const pent_handle* h, const pent_step_params* p, int64_t M,
                                void* c_inout, void* scratch, int nsteps, void* stream)
 {
-    return pent_step_batch_v(h, p, M, c_inout, scratch, nsteps, stream, PENT_KERNEL_AUTO);
+    return pent_step_batch_forced_v(h, p, nullptr, M, c_inout, scratch, nsteps, stream, PENT_KERNEL_AUTO);
 }
 
 extern "C" int pent_step_kernel_choice(const pent_handle* h, int64_t M)

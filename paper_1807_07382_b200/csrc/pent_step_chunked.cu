@@ -29,9 +29,13 @@ struct StepChunkParams {
     uint32_t table_bytes;
     int64_t M, ntiles;
     const T* table;
-    const T* dg;          // N x {a,b,c,d,e,0,0,0} (kind 1)
+    const T* dg;          // N x {a,b,c,d,e, cos 2 pi x_k, sin 2 pi x_k, 0} (kind 1; forcing)
     int nsteps, bc;
     T r, sigma;
+    // forcing (FORCED = true, reading C-22): per-system parameters and the time axis
+    const T* mu1;
+    const T* mu2;
+    double dt, t0;
 };
 
 __device__ __forceinline__ void tma_store_2d(const CUtensorMap* tm, int c0, int c1, const void* src)
@@ -53,7 +57,14 @@ __device__ __forceinline__ void group_sync(int g, int nthreads)
 // phases of a step alternate between FP64-throughput-bound (right-hand side), latency-bound
 // (sweeps, scan) and shared-memory-bound (write-back) work; two groups out of phase fill the pipes
 // that one group in lockstep leaves idle.
-template <typename T, int S, int KIND, int NG>
+// FORCED: the travelling-wave forcing of Eq. 3 with per-system (mu1, mu2).  dt Phi(x_k, t_n) = fa cos(2 pi x_k) +
+// fb sin(2 pi x_k) with (fa, fb) = dt mu1 (cos, sin)(2 pi mu2 t_n): ONE sincospi per system and step (computed by the
+// S threads of chunk 0 one step ahead, under the scan of the current step, double-buffered in shared memory).
+// Along k the forcing of one system is a sampled sinusoid, so a thread needs no table loads for its rows: it
+// keeps the space factors of its FIRST row in registers for the whole launch and steps the sinusoid with the
+// small-angle-stable recurrence  Phi_{j+1} = Phi_j + d_j,  d_{j+1} = d_j - 4 sin^2(pi/N) Phi_{j+1}
+// (error growth ~ j u, not j u / sin(2 pi / N) as for the three-term cosine recurrence): 3 flops per unknown.
+template <typename T, int S, int KIND, int NG, bool FORCED>
 __global__ void __launch_bounds__(CHUNK_MAX_THREADS, 1)
 step_chunked_kernel(const __grid_constant__ CUtensorMap tm, const StepChunkParams<T> prm)
 {
@@ -68,8 +79,9 @@ step_chunked_kernel(const __grid_constant__ CUtensorMap tm, const StepChunkParam
     T2* stE = reinterpret_cast<T2*>(reinterpret_cast<unsigned char*>(table) + prm.table_bytes) +
               (size_t)grp_id * 2 * S * P;
     T2* stS = stE + (size_t)S * P;
-    uint64_t* bars = reinterpret_cast<uint64_t*>(
-        reinterpret_cast<T2*>(reinterpret_cast<unsigned char*>(table) + prm.table_bytes) + (size_t)NG * 2 * S * P);
+    T2* amp_all = reinterpret_cast<T2*>(reinterpret_cast<unsigned char*>(table) + prm.table_bytes) + (size_t)NG * 2 * S * P;
+    T2* amp = amp_all + (FORCED ? (size_t)grp_id * 2 * S : 0);                 // [2][S] forcing amplitudes, double-buffered
+    uint64_t* bars = reinterpret_cast<uint64_t*>(amp_all + (FORCED ? (size_t)NG * 2 * S : 0));
     uint64_t* bar_state = &bars[1 + grp_id];                                   // [0] table, [1+g] state of group g
 
     const int i = tid % S, p = tid / S;
@@ -119,6 +131,38 @@ step_chunked_kernel(const __grid_constant__ CUtensorMap tm, const StepChunkParam
                 tma_load_2d(state + (size_t)b * prm.box_rows * S, &tm, (int)(tile * S), b * prm.box_rows, bar_state);
         }
         mbar_wait(bar_state, parity);
+        // forcing amplitudes of system tid (threads of chunk 0) at step n -> amp[n & 1][tid]
+        double fm1 = 0.0, fm2 = 0.0;
+        // space factors of this thread's first row: (cos, sin)(2 pi x_row0) and their first differences along k,
+        // (cos, sin)(theta + dl) - (cos, sin)(theta) = -2 sin^2(dl/2) (cos, sin) -+ sin(dl) (sin, cos), dl = 2 pi / N
+        T fcx = 0, fsx = 0, fdcx = 0, fdsx = 0, fkap = 0;
+        if constexpr (FORCED) {
+            if (active && row0 < N) {
+                double sh, ch, sd, cd;
+                sincospi(1.0 / (double)N, &sh, &ch);                   // dl / 2
+                sincospi(2.0 / (double)N, &sd, &cd);                   // dl
+                const double cx = (double)__ldg(prm.dg + 8 * (size_t)row0 + 5), sx = (double)__ldg(prm.dg + 8 * (size_t)row0 + 6);
+                const double k2 = 2.0 * sh * sh;
+                fcx = (T)cx; fsx = (T)sx;
+                fdcx = (T)(-k2 * cx - sd * sx); fdsx = (T)(-k2 * sx + sd * cx);
+                fkap = (T)(2.0 * k2);
+            }
+        }
+        auto amp_for_step = [&](int n) {
+            double sn, cs;
+            sincospi(2.0 * fm2 * (prm.t0 + (double)n * prm.dt), &sn, &cs);
+            const double am = prm.dt * fm1;
+            T2 ab; ab.x = (T)(am * cs); ab.y = (T)(am * sn);
+            amp[(n & 1) * S + tid] = ab;
+        };
+        if constexpr (FORCED) {
+            if (tid < S) {
+                const int64_t col = tile * S + tid;
+                if (col < prm.M) { fm1 = (double)prm.mu1[col]; fm2 = (double)prm.mu2[col]; }
+                amp_for_step(0);
+            }
+            group_sync<NG>(grp_id, TG);
+        }
 
         for (int step = 0; step < prm.nsteps; ++step) {
             T v[C];
@@ -212,6 +256,21 @@ step_chunked_kernel(const __grid_constant__ CUtensorMap tm, const StepChunkParam
                         cm2 = cm1; cm1 = c0; c0 = cp1; cp1 = cp2;
                     }
                 }
+                if constexpr (FORCED) {
+                    const T2 ab = amp[(step & 1) * S + i];
+                    T ph = fma(ab.x, fcx, ab.y * fsx), dph = fma(ab.x, fdcx, ab.y * fdsx);
+                    if (row0 + C <= N) {
+#pragma unroll
+                        for (int j = 0; j < C; ++j) { v[j] += ph; ph += dph; dph = fma(-fkap, ph, dph); }
+                    } else {
+#pragma unroll
+                        for (int j = 0; j < C; ++j) {
+                            if (row0 + j < N) v[j] += ph;
+                            ph += dph;
+                            dph = fma(-fkap, ph, dph);
+                        }
+                    }
+                }
                 // ---- chunked solve, stages 1+2 ----
                 T2 e, s;
                 chunk_local_sweeps<T>(v, blk, e, s);
@@ -219,6 +278,9 @@ step_chunked_kernel(const __grid_constant__ CUtensorMap tm, const StepChunkParam
                 stS[slot] = s;
             }
             group_sync<NG>(grp_id, TG);
+            if constexpr (FORCED) {
+                if (tid < S && step + 1 < prm.nsteps) amp_for_step(step + 1);   // read after two more barriers
+            }
             if (P > 1) {
                 for (int rr = 0; rr < rounds; ++rr) {
                     const int sys = (rr * nwarps + warp) * G + grp;
@@ -277,7 +339,8 @@ static StepPlan step_plan(const pent_handle* h, int64_t M, const void* c, int S,
     sp.S = S; sp.NG = NG; sp.TG = sp.pl.threads;
     if (sp.TG * NG > CHUNK_MAX_THREADS) return sp;
     sp.smem = (size_t)NG * ((size_t)sp.pl.nbox * sp.pl.box_rows * S * esz + (size_t)4 * sp.pl.Pl * S * esz) +
-              sp.pl.table_bytes + (size_t)(1 + NG) * sizeof(uint64_t);
+              sp.pl.table_bytes + (size_t)(1 + NG) * sizeof(uint64_t) +
+              (size_t)NG * 4 * S * esz;                                    // forcing amplitudes (used when FORCED)
     sp.ok = sp.smem <= SMEM_LIMIT;
     return sp;
 }
@@ -295,9 +358,9 @@ static StepPlan step_auto_plan(const pent_handle* h, int64_t M, const void* c)
     return step_plan(h, M, c, 32, 1);
 }
 
-template <typename T, int S, int KIND, int NG>
-static int launch_step_inst(const pent_handle* h, const StepPlan& sp, const pent_step_params* p, int64_t M,
-                            void* c, int nsteps, cudaStream_t s)
+template <typename T, int S, int KIND, int NG, bool FORCED>
+static int launch_step_inst(const pent_handle* h, const StepPlan& sp, const pent_step_params* p, const pent_forcing* fg,
+                            int64_t M, void* c, int nsteps, cudaStream_t s)
 {
     const ChunkPlan& pl = sp.pl;
     StepChunkParams<T> prm;
@@ -314,12 +377,14 @@ static int launch_step_inst(const pent_handle* h, const StepPlan& sp, const pent
     prm.dg = (const T*)h->dg;
     prm.nsteps = nsteps; prm.bc = p->bc;
     prm.r = (T)p->r; prm.sigma = (T)p->sigma;
+    prm.mu1 = prm.mu2 = nullptr; prm.dt = prm.t0 = 0.0;
+    if (FORCED) { prm.mu1 = (const T*)fg->mu1; prm.mu2 = (const T*)fg->mu2; prm.dt = fg->dt; prm.t0 = fg->t0; }
     CUtensorMap tm;
     if (!encode_batch_map_cached(&tm, c, M, h->N, S, prm.box_rows, sizeof(T) == 8)) {
         g_last_cuda_error = (int)cudaErrorInvalidValue;
         return PENT_ERR_CUDA;
     }
-    auto kern = step_chunked_kernel<T, S, KIND, NG>;
+    auto kern = step_chunked_kernel<T, S, KIND, NG, FORCED>;
     static SmemOnce mark;
     PENT_CUDA(ensure_dynamic_smem(mark, kern, sp.smem));
     const int threads = sp.TG * NG;
@@ -343,21 +408,25 @@ bool step_chunked_supported(const pent_handle* h, int64_t M, const void* c)
 }
 
 template <typename T, int S, int NG>
-static int launch_step_kind(const pent_handle* h, const StepPlan& sp, const pent_step_params* p, int64_t M,
-                            void* c, int nsteps, cudaStream_t s)
+static int launch_step_kind(const pent_handle* h, const StepPlan& sp, const pent_step_params* p, const pent_forcing* fg,
+                            int64_t M, void* c, int nsteps, cudaStream_t s)
 {
-    if (p->kind == 1) return launch_step_inst<T, S, 1, NG>(h, sp, p, M, c, nsteps, s);
-    if (p->form == 1) return launch_step_inst<T, S, 2, NG>(h, sp, p, M, c, nsteps, s);
-    return launch_step_inst<T, S, 0, NG>(h, sp, p, M, c, nsteps, s);
+    if (p->kind == 1) return launch_step_inst<T, S, 1, NG, false>(h, sp, p, nullptr, M, c, nsteps, s);
+    if (fg) {
+        if (p->form == 1) return launch_step_inst<T, S, 2, NG, true>(h, sp, p, fg, M, c, nsteps, s);
+        return launch_step_inst<T, S, 0, NG, true>(h, sp, p, fg, M, c, nsteps, s);
+    }
+    if (p->form == 1) return launch_step_inst<T, S, 2, NG, false>(h, sp, p, nullptr, M, c, nsteps, s);
+    return launch_step_inst<T, S, 0, NG, false>(h, sp, p, nullptr, M, c, nsteps, s);
 }
 
-int launch_step_chunked(const pent_handle* h, const pent_step_params* p, int64_t M, void* c, int nsteps,
-                        cudaStream_t s)
+int launch_step_chunked(const pent_handle* h, const pent_step_params* p, const pent_forcing* fg, int64_t M, void* c,
+                        int nsteps, cudaStream_t s)
 {
     const StepPlan sp = step_auto_plan(h, M, c);
     if (!sp.ok) return PENT_ERR_ARG;
-    if (h->dtype == PENT_F64) return launch_step_kind<double, 16, 1>(h, sp, p, M, c, nsteps, s);
-    if (sp.NG == 2) return launch_step_kind<float, 16, 2>(h, sp, p, M, c, nsteps, s);
-    return launch_step_kind<float, 32, 1>(h, sp, p, M, c, nsteps, s);
+    if (h->dtype == PENT_F64) return launch_step_kind<double, 16, 1>(h, sp, p, fg, M, c, nsteps, s);
+    if (sp.NG == 2) return launch_step_kind<float, 16, 2>(h, sp, p, fg, M, c, nsteps, s);
+    return launch_step_kind<float, 32, 1>(h, sp, p, fg, M, c, nsteps, s);
 }
 }  // namespace pent

@@ -216,3 +216,116 @@ def test_step_fp32_one_step(kernel):
     ref = oracle.step_batch(oracle.factor(*d64), 0, 1, 0, float(np.float32(r)),
                             float(np.float32(sigma)), c0.astype(np.float32).astype(np.float64), 1)
     assert normwise(cd.cpu().numpy().astype(np.float64), ref) <= 2e-5
+
+
+# ---- forced Cahn-Hilliard with per-system parameters (Remark 1 / Eq. 3) ----
+def _forcing_params(M, seed=70, dtype=torch.float64):
+    mu1 = pin.uniform_vec(seed, 1, M, 50.0, 5000.0)         # dt * mu1 ~ 5e-5 .. 5e-3 per step
+    mu2 = pin.uniform_vec(seed, 2, M, -2e4, 2e4)            # up to 20 periods over 1000 steps of dt = 1e-6
+    return mu1, mu2, guarded(mu1, dtype), guarded(mu2, dtype)
+
+
+@pytest.mark.parametrize("kernel", STEP_KERNELS)
+@pytest.mark.parametrize("form", [1, 0])
+@pytest.mark.parametrize("N,M,nsteps", [(256, 200, 3), (1024, 130, 2), (100, 38, 5), (64, 16, 1)])
+def test_forced_ch_parity(kernel, form, N, M, nsteps):
+    pent = _pent()
+    diags, sigma, r, c0 = _ch_setup(N, M, "zeroflux")
+    a, b, c, d, e = (torch.tensor(v) for v in diags)
+    h = pent.pent_factor(N, e, c, d, a, b)
+    mu1, mu2, g1, g2 = _forcing_params(M)
+    dt, t0 = 1e-6, 3.5e-5
+    cg, sg = guarded(c0), Guarded((N, M))
+    pent.pent_step_batch(h, M, cg.t, nsteps, kind=0, bc=1, form=form, r=r, sigma=sigma, kernel=kernel, scratch=sg.t,
+                         forcing=(g1.t, g2.t, dt, t0))
+    check_all(cg, sg, g1, g2)
+    fac = oracle.factor(*diags)
+    ref = oracle.step_forced_batch(fac, 1, form, r, sigma, dt, t0, mu1, mu2, c0, nsteps)
+    unforced = oracle.step_batch(fac, 0, 1, form, r, sigma, c0, nsteps)
+    assert normwise(ref, unforced) > 1e-6                                    # the forcing is visible at this scale
+    tol = 1e-11 * nsteps
+    if N >= 1000:   # stiff matrix: same measured envelope as the unforced step (the forcing adds nothing to it)
+        truth = oracle.ld_step_batch(diags, 0, 1, form, r, sigma, c0, 1)
+        one = oracle.step_batch(fac, 0, 1, form, r, sigma, c0, 1)
+        rhs = np.stack([oracle.rhs(fac, 0, 1, form, r, sigma, c0[:, i]) for i in range(M)], axis=1)
+        sol = chunked_order_solve_fp64(fac, rhs)
+        tol = nsteps * envelope_tol(1e-11, truth, one, c0 + sol if form == 1 else sol)
+    assert normwise(cg.numpy(), ref) <= tol
+
+
+def test_forced_ch_multi_step_launch_equals_single_step_launches_and_conserves_mean():
+    """n forced steps in one launch == n launches of one step with t0 advanced by the caller (bit for bit), and the
+    zero-mean forcing leaves mean(c) invariant (zero-flux operator, increment form)."""
+    pent = _pent()
+    N, M, n = 512, 96, 9
+    diags, sigma, r, c0 = _ch_setup(N, M, "zeroflux")
+    a, b, c, d, e = (torch.tensor(v) for v in diags)
+    h = pent.pent_factor(N, e, c, d, a, b)
+    mu1, mu2, g1, g2 = _forcing_params(M)
+    dt, t0 = 1e-6, 0.0
+    c1, c2 = _dev(c0), _dev(c0)
+    kw = dict(kind=0, bc=1, form=1, r=r, sigma=sigma, kernel=2)
+    pent.pent_step_batch(h, M, c1, n, forcing=(g1.t, g2.t, dt, t0), **kw)
+    for k in range(n):
+        pent.pent_step_batch(h, M, c2, 1, forcing=(g1.t, g2.t, dt, t0 + k * dt), **kw)
+    assert torch.equal(c1, c2)
+    got = c1.cpu().numpy()
+    drift = max(abs(math.fsum(got[:, i]) - math.fsum(c0[:, i])) / N for i in range(M))
+    assert drift <= 1e-13
+    ref = oracle.step_forced_batch(oracle.factor(*diags), 1, 1, r, sigma, dt, t0, mu1, mu2, c0, n)
+    assert normwise(got, ref) <= 1e-11 * n
+
+
+def test_forced_ch_cfg4_shape_conservation_and_cost():
+    """cfg4's shape (N=1024, M=8192), 200 forced steps in one launch: mean(c) of every run conserved to 1e-12, parity
+    with the oracle on every 16th system, and the forced step costs about what the unforced one does."""
+    pent = _pent()
+    w = WORKLOADS["cfg4"]
+    diags = make_matrix(w)
+    c0 = make_rhs(w)
+    a, b, c, d, e = (torch.tensor(v) for v in diags)
+    h = pent.pent_factor(w.N, e, c, d, a, b)
+    mu1, mu2, g1, g2 = _forcing_params(w.M)
+    n, dt = 200, 1e-6
+    cg = guarded(c0)
+    kw = dict(kind=0, bc=1, form=1, r=R_CH, sigma=SIGMA_CH)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+    pent.pent_step_batch(h, w.M, cg.t, n, forcing=(g1.t, g2.t, dt, 0.0), **kw)      # also the warm-up
+    cg.check()
+    c1 = cg.numpy()
+    c1r, c0r = np.ascontiguousarray(c1.T), np.ascontiguousarray(c0.T)
+    assert max(abs(math.fsum(c1r[i]) - math.fsum(c0r[i])) / w.N for i in range(w.M)) <= 1e-12
+    cols = np.arange(0, w.M, 16)
+    ref = oracle.step_forced_batch(oracle.factor(*diags), 1, 1, R_CH, SIGMA_CH, dt, 0.0, mu1[cols], mu2[cols],
+                                   np.ascontiguousarray(c0[:, cols]), n, nthreads=8)
+    assert normwise(c1[:, cols], ref) <= 1e-9
+    cd = _dev(c0)
+    pent.pent_step_batch(h, w.M, cd, n, **kw)
+    torch.cuda.synchronize()
+    ev[0].record(); pent.pent_step_batch(h, w.M, cd, n, **kw); ev[1].record()
+    ev[2].record(); pent.pent_step_batch(h, w.M, cd, n, forcing=(g1.t, g2.t, dt, 0.0), **kw); ev[3].record()
+    torch.cuda.synchronize()
+    t_plain, t_forced = ev[0].elapsed_time(ev[1]) / n * 1e3, ev[2].elapsed_time(ev[3]) / n * 1e3
+    print(f"cfg4 shape: unforced {t_plain:.2f} us per step, forced {t_forced:.2f} us per step ({t_forced / t_plain:.3f} x)")
+    assert t_forced <= 1.25 * t_plain
+
+
+@pytest.mark.parametrize("kernel", STEP_KERNELS)
+def test_forced_ch_fp32(kernel):
+    pent = _pent()
+    N, M, n = 256, 200, 4
+    diags, sigma, r, c0 = _ch_setup(N, M, "zeroflux")
+    d32 = [np.asarray(v, dtype=np.float32) for v in diags]
+    a, b, c, d, e = (torch.tensor(v) for v in d32)
+    h = pent.pent_factor(N, e, c, d, a, b)
+    mu1, mu2, g1, g2 = _forcing_params(M, dtype=torch.float32)
+    dt, t0 = 1e-6, 2e-5
+    cg = guarded(c0, torch.float32)
+    pent.pent_step_batch(h, M, cg.t, n, kind=0, bc=1, form=0, r=r, sigma=sigma, kernel=kernel,
+                         forcing=(g1.t, g2.t, dt, t0))
+    check_all(cg, g1, g2)
+    d64 = [v.astype(np.float64) for v in d32]
+    f32 = lambda v: np.asarray(v, dtype=np.float32).astype(np.float64)
+    ref = oracle.step_forced_batch(oracle.factor(*d64), 1, 0, float(np.float32(r)), float(np.float32(sigma)), dt, t0,
+                                   f32(mu1), f32(mu2), f32(c0), n)
+    assert normwise(cg.numpy().astype(np.float64), ref) <= 2e-5 * n
