@@ -102,7 +102,9 @@ def solve(fac: Factors, f) -> np.ndarray:
 
 def to_rows(f_interleaved: np.ndarray) -> np.ndarray:
     """(N, M) interleaved -> (M, N) one system per row."""
-    return np.ascontiguousarray(np.asarray(f_interleaved, dtype=np.float64).T)
+    # always a fresh array: for M == 1 the transpose of a contiguous (N, 1) array is itself contiguous, and the
+    # in-place C routines (step_rows) would then overwrite the caller's input
+    return np.array(np.asarray(f_interleaved, dtype=np.float64).T, order="C", copy=True)
 
 
 def solve_rows(fac: Factors, F_rows: np.ndarray, nthreads: int = 1) -> np.ndarray:

@@ -32,23 +32,28 @@ constexpr size_t SMEM_LIMIT = 232448;       // 227 KB dynamic shared memory per 
 //   WF_l : 4 x n     TPhi_q TPhi_{q-1} ... TPhi_{q-d+1}  for q >= d,     at [e*n + q-d]
 //   WB_l : 4 x n     TPsi_q TPsi_{q+1} ... TPsi_{q+d-1}  for q+d <= P-1, at [e*n + q]
 // Only the levels a handle needs are staged into shared memory (they come last).
+// BAND = 1 (tridiagonal A, a = e = 0: cuThomasBatch's case): the recurrences have ONE term, the
+// chunk states and every transfer "matrix" are scalars, so every 4 above becomes 1 (BLK: 8 + 8 scalars).
 constexpr int W_LEVELS = 5;
-__host__ __device__ inline int w_level_off(int P, int l, int Q)
+__host__ __device__ inline int w_level_off(int P, int l, int Q, int BAND = 2)
 {
-    int off = Q > 1 ? 12 * P + 64 : 4 * P;      // PF, PB, BLK exist only in cluster tables
-    for (int k = 0; k < l; ++k) { int n = P - (1 << k); off += 8 * (n > 0 ? n : 0); }
+    const int u = BAND == 2 ? 4 : 1;
+    int off = Q > 1 ? 3 * u * P + 16 * u : u * P;      // PF, PB, BLK exist only in cluster tables
+    for (int k = 0; k < l; ++k) { int n = P - (1 << k); off += 2 * u * (n > 0 ? n : 0); }
     return off;
 }
-__host__ __device__ inline int w_len(int P, int Q) { return w_level_off(P, W_LEVELS, Q); }
+__host__ __device__ inline int w_len(int P, int Q, int BAND = 2) { return w_level_off(P, W_LEVELS, Q, BAND); }
 
-// per-chunk coefficient block, in units of T:  [fwd 3C | bwd 2C | corr 4C | pad to 16 B]
-template <typename T> __host__ __device__ constexpr int chunk_block_len()
+// per-chunk coefficient block, in units of T:  [fwd 3C | bwd 2C | corr 4C | pad to 16 B]   (BAND 2)
+//                                              [fwd 2C | bwd  C | corr 2C | pad to 16 B]   (BAND 1)
+template <typename T, int BAND = 2> __host__ __device__ constexpr int chunk_block_len()
 {
-    return 9 * ChunkCfg<T>::C + (int)(16 / sizeof(T));
+    return (BAND == 2 ? 9 : 5) * ChunkCfg<T>::C + (int)(16 / sizeof(T));
 }
-template <typename T> __host__ __device__ constexpr size_t table_len(int P, int Q)
+template <typename T, int BAND = 2> __host__ __device__ constexpr size_t table_len(int P, int Q)
 {
-    return (size_t)P * chunk_block_len<T>() + (size_t)w_len(P, Q);
+    // rounded up to 4 words: every rank's table starts 16-byte aligned in global memory (cp.async.bulk source)
+    return ((size_t)P * chunk_block_len<T, BAND>() + (size_t)w_len(P, Q, BAND) + 3) & ~(size_t)3;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -153,6 +158,9 @@ __device__ __forceinline__ void lds_vec(T (&dst)[n], const T* src)
 template <typename T> struct Pair;
 template <> struct Pair<double> { using type = double2; };
 template <> struct Pair<float>  { using type = float2; };
+// chunk state: the last two g / first two x of a chunk (BAND 2), or the last g / first x (BAND 1)
+template <typename T, int BAND> struct ChunkState { using type = typename Pair<T>::type; };
+template <typename T> struct ChunkState<T, 1> { using type = T; };
 
 template <typename T>
 __device__ __forceinline__ T shfl_up_t(T v, int d, int w) { return __shfl_up_sync(0xffffffffu, v, d, w); }
@@ -195,6 +203,17 @@ __device__ __forceinline__ void st_async_pair(const void* local, const uint64_t*
 {
     asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.f32 [%0], {%1, %2}, [%3];"
                  ::"r"(map_to_rank(local, rank)), "f"(a), "f"(b), "r"(map_to_rank(local_bar, rank)) : "memory");
+}
+
+__device__ __forceinline__ void st_async_one(const void* local, const uint64_t* local_bar, uint32_t rank, double a)
+{
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.f64 [%0], %1, [%2];"
+                 ::"r"(map_to_rank(local, rank)), "d"(a), "r"(map_to_rank(local_bar, rank)) : "memory");
+}
+__device__ __forceinline__ void st_async_one(const void* local, const uint64_t* local_bar, uint32_t rank, float a)
+{
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.f32 [%0], %1, [%2];"
+                 ::"r"(map_to_rank(local, rank)), "f"(a), "r"(map_to_rank(local_bar, rank)) : "memory");
 }
 
 // One CTA = S systems x P chunks (thread = one system, one chunk of C rows, held in registers).
@@ -252,6 +271,50 @@ __device__ __forceinline__ void chunk_correct4(T (&out)[4], const T* v4, const T
 #pragma unroll
     for (int r = 0; r < 4; ++r)
         out[r] = fma(w[4 * r + 3], B1, fma(w[4 * r + 2], B0, fma(w[4 * r + 1], F1, fma(w[4 * r], F0, v4[r]))));
+}
+
+// ---- BAND = 1: the same three stages for a tridiagonal A (one-term recurrences) -----------------
+// blk: [ {1/alpha, beta/alpha} x C | gamma x C | {chi, psi} x C ].  v: f -> x^ ; e = last g~ ; s = first x^.
+template <typename T>
+__device__ __forceinline__ void tri_local_sweeps(T (&v)[ChunkCfg<T>::C], const T* blk, T& e, T& s)
+{
+    constexpr int C = ChunkCfg<T>::C;
+    T g1 = 0;
+#pragma unroll
+    for (int jg = 0; jg < C / 4; ++jg) {
+        T w[8];
+        lds_vec<T, 8>(w, blk + 8 * jg);
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const int j = 4 * jg + r;
+            T g = fma(-w[2 * r + 1], g1, w[2 * r] * v[j]);
+            v[j] = g; g1 = g;
+        }
+    }
+    e = v[C - 1];
+    T x1 = 0;
+#pragma unroll
+    for (int jg = C / 4 - 1; jg >= 0; --jg) {
+        T w[4];
+        lds_vec<T, 4>(w, blk + 2 * C + 4 * jg);
+#pragma unroll
+        for (int r = 3; r >= 0; --r) {
+            const int j = 4 * jg + r;
+            T xv = fma(-w[r], x1, v[j]);
+            v[j] = xv; x1 = xv;
+        }
+    }
+    s = v[0];
+}
+
+template <typename T>
+__device__ __forceinline__ void tri_correct4(T (&out)[4], const T* v4, const T* blk, int jg, T F, T B)
+{
+    constexpr int C = ChunkCfg<T>::C;
+    T w[8];
+    lds_vec<T, 8>(w, blk + 3 * C + 8 * jg);
+#pragma unroll
+    for (int r = 0; r < 4; ++r) out[r] = fma(w[2 * r + 1], B, fma(w[2 * r], F, v4[r]));
 }
 
 // Chunk states live in shared memory as [chunk][system] with the system index rotated by the chunk
@@ -432,6 +495,58 @@ __device__ __forceinline__ void chunk_state_scan(const ScanGeom& g, const T* wta
     }
 }
 
+// stage 3 for BAND = 1: scalar states, scalar transfer coefficients (layout: see w_level_off with BAND = 1).
+//   F_q = E~_q + TPhi_q F_{q-1};  B_q = (S^_q + TX_q F_{q-1}) + TPsi_q B_{q+1}
+template <typename T, int S, bool CLUSTER>
+__device__ __forceinline__ void tri_state_scan(const ScanGeom& g, const T* wtab, T* stE, T* stS, int sys, int q, bool ok,
+                                               int rank, int Q, T* aggF, T* aggB, uint64_t* bars,
+                                               uint32_t agg_bytes_f, uint32_t agg_bytes_b, uint32_t parity)
+{
+    const int P = g.P, Pw = g.Pw;
+    const int sl = ok ? state_slot<S>(q, sys) : 0;
+    const int sy = ok ? sys : 0;
+    T y = 0, z = 0;
+    if (ok) { y = stE[sl]; z = stS[sl]; }
+#pragma unroll
+    for (int l = 0; l < W_LEVELS; ++l) {
+        if (l < g.lev_f) {
+            const int d = 1 << l;
+            T u = shfl_up_t(y, d, Pw);
+            if (ok && q >= d) y = fma(wtab[g.woff[l] + (q - d)], u, y);
+        }
+    }
+    T fin = 0;
+    if constexpr (CLUSTER) {
+        if (ok && q == P - 1)
+            for (int rr = rank + 1; rr < Q; ++rr) st_async_one(&aggF[rank * S + sys], &bars[BAR_F], rr, y);
+        if (agg_bytes_f) mbar_wait(&bars[BAR_F], parity);
+        for (int rr = 0; rr < rank; ++rr) fin = fma(wtab[3 * P + rr], fin, aggF[rr * S + sy]);
+        if (ok && rank > 0) y = fma(wtab[P + q], fin, y);                     // PF_q F_in
+    }
+    T f = shfl_up_t(y, 1, Pw);
+    if (q == 0) f = fin;
+    if (ok) z = fma(wtab[q], f, z);                                           // TX_q F_{q-1}
+#pragma unroll
+    for (int l = 0; l < W_LEVELS; ++l) {
+        if (l < g.lev_b) {
+            const int d = 1 << l, n = P - d;
+            T u = shfl_down_t(z, d, Pw);
+            if (ok && q + d <= P - 1) z = fma(wtab[g.woff[l] + n + q], u, z);
+        }
+    }
+    T bin = 0;
+    if constexpr (CLUSTER) {
+        if (ok && q == 0)
+            for (int rr = 0; rr < rank; ++rr) st_async_one(&aggB[rank * S + sys], &bars[BAR_B], rr, z);
+        if (agg_bytes_b) mbar_wait(&bars[BAR_B], parity);
+        for (int rr = Q - 1; rr > rank; --rr) bin = fma(wtab[3 * P + 8 + rr], bin, aggB[rr * S + sy]);
+        if (ok && rank < Q - 1) z = fma(wtab[2 * P + q], bin, z);             // PB_q B_in
+    }
+    T b = shfl_down_t(z, 1, Pw);
+    if (q >= P - 1) b = bin;
+    if (ok) { stE[sl] = f; stS[sl] = b; }
+}
+
 // ------------------------------------------------------------------------------------------
 // host side (defined in pent_solve_chunked.cu)
 // ------------------------------------------------------------------------------------------
@@ -441,12 +556,13 @@ struct ChunkPlan {
     int j = 0, Q = 1, S = 0, Pl = 0, Pw = 1, threads = 0, levels = 0, box_rows = 0, nbox = 0;
     bool ldg = false;          // LDG loader instead of TMA (pitch not a multiple of 16 bytes, or system-major batch)
     bool rows = false;         // system-major batch: implies ldg
+    int band = 2;              // 1: the tridiagonal instantiation and its tables (handle with a == e == 0)
     size_t table_bytes = 0, smem = 0;
 };
 // any_S: accept tile widths the SOLVE kernel is not instantiated for (the step kernel has its own)
 // ldg: plan for the LDG loader (no TMA alignment requirements, no landing buffer)
 ChunkPlan make_plan(const pent_handle* h, int64_t M, const void* f, int Q, int S, bool any_S = false,
-                    bool ldg = false);
+                    bool ldg = false, int band = 2);
 ChunkPlan chunk_auto_plan(const pent_handle* h, int64_t M, const void* f);   // what PENT_KERNEL_AUTO runs
 // rank-2 tensor map {M, N} of an interleaved batch with box {S, box_rows}; false on failure
 bool encode_batch_map(CUtensorMap* tm, const void* base, int64_t M, int N, int S, int box_rows, bool f64);

@@ -43,28 +43,32 @@ struct ChunkParams {
 };
 
 // PER = true: the periodic (cyclic) solve fused into the kernel, see PeriodicCtx in pent_chunk_common.cuh.
-template <typename T, int S, bool CLUSTER, bool PER>
+// BAND = 1: tridiagonal A (a == e == 0, cuThomasBatch's case): one-term recurrences, a 5-word
+// coefficient row instead of 9, scalar chunk states; same data movement.
+template <typename T, int S, bool CLUSTER, bool PER, int BAND>
 __global__ void __launch_bounds__(CHUNK_MAX_THREADS, 1)
 solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T> prm,
                      const __grid_constant__ PeriodicParams<T> pp)
 {
-    constexpr int C = ChunkCfg<T>::C, BL = chunk_block_len<T>();
+    static_assert(BAND == 2 || !PER, "the fused periodic tail is built on the pentadiagonal tables");
+    constexpr int C = ChunkCfg<T>::C, BL = chunk_block_len<T, BAND>();
     using T2 = typename Pair<T>::type;
+    using ST = typename ChunkState<T, BAND>::type;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int P = prm.P;
     T* landing = reinterpret_cast<T*>(smem_raw);
     T* table = landing + (size_t)prm.nbox * prm.box_rows * S;
     // chunk states [P][S]: E~ then F_{p-1};  S^ then B_{p+1}
-    T2* stE = reinterpret_cast<T2*>(reinterpret_cast<unsigned char*>(table) + prm.table_bytes);
-    T2* stS = stE + (size_t)S * P;
+    ST* stE = reinterpret_cast<ST*>(reinterpret_cast<unsigned char*>(table) + prm.table_bytes);
+    ST* stS = stE + (size_t)S * P;
     // cluster: block aggregates of every rank, [Q][S] each (written by the owning rank through DSMEM)
     // Slot rr holds rank rr's FORWARD aggregate when rr < rank and its BACKWARD aggregate when rr > rank
     // (a CTA needs nothing else), so both directions share one array; the periodic kernel needs every
     // rank's backward aggregate and keeps two.
-    T2* aggF = stS + (size_t)S * P;
-    T2* aggB = aggF + ((CLUSTER && PER) ? (size_t)prm.Q * S : 0);
+    ST* aggF = stS + (size_t)S * P;
+    ST* aggB = aggF + ((CLUSTER && PER) ? (size_t)prm.Q * S : 0);
     // periodic: this CTA's rows of Z, then x^ of rows n-2/n-1, (y_{n-2}, y_{n-1}), (f_n, f_{n+1}), t  ([S] each)
-    T2* zs = aggB + (CLUSTER ? (size_t)prm.Q * S : 0);
+    T2* zs = reinterpret_cast<T2*>(aggB + (CLUSTER ? (size_t)prm.Q * S : 0));
     T2* ypub = zs + (PER ? (size_t)P * C : 0);
     T2* yab = ypub + (PER ? S : 0);
     T2* ftail2 = yab + (PER ? S : 0);             // [2][S]
@@ -115,10 +119,10 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
     }
     // every CTA of the cluster is resident, with its mbarriers initialised, before any DSMEM store
     if constexpr (CLUSTER) cluster_sync_all();
-    const uint32_t agg_bytes_f = (uint32_t)(rank * S * sizeof(T2));                 // from the earlier ranks
+    const uint32_t agg_bytes_f = (uint32_t)(rank * S * sizeof(ST));                 // from the earlier ranks
     // from the later ranks; periodic: from EVERY rank (itself included) plus (y_{n-2}, y_{n-1}) from rank ra
-    const uint32_t agg_bytes_b = PER ? (uint32_t)((prm.Q + 1) * S * sizeof(T2))
-                                     : (uint32_t)((prm.Q - 1 - rank) * S * sizeof(T2));
+    const uint32_t agg_bytes_b = PER ? (uint32_t)((prm.Q + 1) * S * sizeof(ST))
+                                     : (uint32_t)((prm.Q - 1 - rank) * S * sizeof(ST));
     mbar_wait(&bars[0], 0);
 
     const T* blk = table + (size_t)(active ? p : 0) * BL;
@@ -217,8 +221,9 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
         }
         if (active) {
             // ---- 1+2. local forward sweep and local back substitution from zero states ----
-            T2 e, s;
-            chunk_local_sweeps<T>(v, blk, e, s);
+            ST e, s;
+            if constexpr (BAND == 2) chunk_local_sweeps<T>(v, blk, e, s);
+            else tri_local_sweeps<T>(v, blk, e, s);
             stE[slot] = e;
             stS[slot] = s;
             if constexpr (PER) {
@@ -249,8 +254,12 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
             }
             for (int r = 0; r < rounds; ++r) {
                 const int sys = (r * nwarps + warp) * G + grp;
-                chunk_state_scan<T, S, CLUSTER, PER>(geom, wtab, stE, stS, sys, q, (sys < S) && (q < P), rank,
-                                                     prm.Q, aggF, aggB, bars, agg_bytes_f, agg_bytes_b, parity, &per);
+                if constexpr (BAND == 2)
+                    chunk_state_scan<T, S, CLUSTER, PER>(geom, wtab, stE, stS, sys, q, (sys < S) && (q < P), rank,
+                                                         prm.Q, aggF, aggB, bars, agg_bytes_f, agg_bytes_b, parity, &per);
+                else
+                    tri_state_scan<T, S, CLUSTER>(geom, wtab, stE, stS, sys, q, (sys < S) && (q < P), rank, prm.Q,
+                                                  aggF, aggB, bars, agg_bytes_f, agg_bytes_b, parity);
             }
         }
         __syncthreads();
@@ -258,7 +267,15 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
         // ---- 4. correction and store ----
         if (active) {
             T F0 = 0, F1 = 0, B0 = 0, B1 = 0;
-            if (CLUSTER || PER || P > 1) { T2 fo = stE[slot]; F0 = fo.x; F1 = fo.y; T2 bo = stS[slot]; B0 = bo.x; B1 = bo.y; }
+            if (CLUSTER || PER || P > 1) {
+                if constexpr (BAND == 2) { T2 fo = stE[slot]; F0 = fo.x; F1 = fo.y; T2 bo = stS[slot]; B0 = bo.x; B1 = bo.y; }
+                else { F0 = stE[slot]; B0 = stS[slot]; }
+            }
+            // rows 4 jg .. 4 jg + 3 of this thread's chunk: x = x^ + responses to the incoming chunk states
+            auto correct4 = [&](T (&out)[4], int jg) {
+                if constexpr (BAND == 2) chunk_correct4<T>(out, &v[4 * jg], blk, jg, F0, F1, B0, B1);
+                else tri_correct4<T>(out, &v[4 * jg], blk, jg, F0, B0);
+            };
             const int64_t col = tile * S + i;
             T* xo = prm.x + (int64_t)row0 * prm.M + col;
             if (!PER && prm.ldg == 2) {
@@ -271,7 +288,7 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
 #pragma unroll
                 for (int jg = 0; jg < C / 4; ++jg) {
                     T xv[4];
-                    chunk_correct4<T>(xv, &v[4 * jg], blk, jg, F0, F1, B0, B1);
+                    correct4(xv, jg);
                     if (vec) {
 #pragma unroll
                         for (int r = 0; r < 4; ++r) acc[(4 * jg + r) % W] = xv[r];
@@ -292,7 +309,7 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
 #pragma unroll
                 for (int jg = 0; jg < C / 4; ++jg) {
                     T xv[4];
-                    chunk_correct4<T>(xv, &v[4 * jg], blk, jg, F0, F1, B0, B1);
+                    correct4(xv, jg);
                     if constexpr (PER && !PENT_AB_NO_Z) {
 #pragma unroll
                         for (int r = 0; r < 4; ++r) { T2 z = zr[4 * jg + r]; xv[r] = fma(-z.y, t1, fma(-z.x, t0, xv[r])); }
@@ -305,7 +322,7 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
 #pragma unroll
                 for (int jg = 0; jg < C / 4; ++jg) {
                     T xv[4];
-                    chunk_correct4<T>(xv, &v[4 * jg], blk, jg, F0, F1, B0, B1);
+                    correct4(xv, jg);
                     if constexpr (PER && !PENT_AB_NO_Z) {
 #pragma unroll
                         for (int r = 0; r < 4; ++r) { T2 z = zr[4 * jg + r]; xv[r] = fma(-z.y, t1, fma(-z.x, t0, xv[r])); }

@@ -18,7 +18,7 @@ inline size_t periodic_extra_smem(const ChunkPlan& pl)
     return ((size_t)pl.Pl * ChunkCfg<T>::C + 5 * (size_t)pl.S + (pl.Q > 1 ? (size_t)pl.Q * pl.S : 0)) * 2 * sizeof(T);   // + second aggregate array
 }
 
-template <typename T, int S, bool CLUSTER, bool PER>
+template <typename T, int S, bool CLUSTER, bool PER, int BAND = 2>
 static int launch_inst(const pent_handle* h, const ChunkPlan& pl, int64_t M, const void* f, void* x,
                        cudaStream_t s, const PeriodicParams<T>* per)
 {
@@ -27,15 +27,16 @@ static int launch_inst(const pent_handle* h, const ChunkPlan& pl, int64_t M, con
     prm.N = h->N; prm.P = pl.Pl; prm.Q = pl.Q; prm.Pw = pl.Pw; prm.M = M;
     int lg = 0;
     while ((1 << lg) < pl.Pw) ++lg;
-    prm.lev_f = h->lev_f[pl.j] < lg ? h->lev_f[pl.j] : lg;
-    prm.lev_b = h->lev_b[pl.j] < lg ? h->lev_b[pl.j] : lg;
-    for (int l = 0; l < W_LEVELS; ++l) prm.woff[l] = w_level_off(pl.Pl, l, pl.Q);
+    const int hlf = BAND == 2 ? h->lev_f[pl.j] : h->lev_f1[pl.j], hlb = BAND == 2 ? h->lev_b[pl.j] : h->lev_b1[pl.j];
+    prm.lev_f = hlf < lg ? hlf : lg;
+    prm.lev_b = hlb < lg ? hlb : lg;
+    for (int l = 0; l < W_LEVELS; ++l) prm.woff[l] = w_level_off(pl.Pl, l, pl.Q, BAND);
     prm.box_rows = pl.box_rows; prm.nbox = pl.nbox;
     prm.ntiles = (M + S - 1) / S;
     for (int b = 0; b < MAX_BOXES; ++b) prm.wcount[b] = 0;
     for (int w = 0; w * 32 < pl.Pl * S; ++w) prm.wcount[((w * 32 / S) * C) / prm.box_rows] += 1;
-    prm.table = (const T*)h->cf[pl.j];
-    prm.table_stride = (int64_t)table_len<T>(pl.Pl, pl.Q);
+    prm.table = (const T*)(BAND == 2 ? h->cf[pl.j] : h->cf1[pl.j]);
+    prm.table_stride = (int64_t)table_len<T, BAND>(pl.Pl, pl.Q);
     prm.table_bytes = (uint32_t)pl.table_bytes;
     prm.x = (T*)x;
     prm.f = (const T*)f;
@@ -50,7 +51,7 @@ static int launch_inst(const pent_handle* h, const ChunkPlan& pl, int64_t M, con
     PeriodicParams<T> pp = {};
     if (PER) pp = *per;
     const size_t smem_total = pl.smem + (PER ? periodic_extra_smem<T>(pl) : 0);
-    auto kern = solve_chunked_kernel<T, S, CLUSTER, PER>;
+    auto kern = solve_chunked_kernel<T, S, CLUSTER, PER, BAND>;
     static SmemOnce mark;
     PENT_CUDA(ensure_dynamic_smem(mark, kern, smem_total));
     // the occupancy answer depends only on (device, threads, shared memory, cluster size): keep the last

@@ -30,6 +30,9 @@ struct pent_handle {
     void* cf[PENT_NQ];
     int cfP[PENT_NQ];
     int lev_f[PENT_NQ], lev_b[PENT_NQ];   // Kogge-Stone levels the chunk-state scans need
+    // the same for the tridiagonal instantiation (band == 1 only): 5-word coefficient rows, scalar transfers
+    void* cf1[PENT_NQ];
+    int lev_f1[PENT_NQ], lev_b1[PENT_NQ];
     // ---- periodic (cyclic) A, Eqs. 7a-12 (pent_periodic.cu): N is the full size, `inner`
     // is the shared-A handle of the (N-2) x (N-2) block E, Zt = E^{-1} k as (N-2) x {z0, z1} in T,
     // dgp = N x {a,b,c,d,e,0,0,0} in T with the wrapped entries kept, pc = the six entries of h

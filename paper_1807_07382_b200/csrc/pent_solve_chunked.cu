@@ -180,17 +180,110 @@ __global__ void build_chunk_products_kernel(int Pl, int Q, const double* __restr
     if (q == 0) { atomicMax(&levels[0], need_f); atomicMax(&levels[1], need_b); }
 }
 
+// ---- BAND = 1 (tridiagonal A): scalar versions of the two kernels above --------------------------------------
+// block: [ {1/alpha, beta/alpha} x C | gamma x C | {chi, psi} x C | pad ];  tmat: TPhi | TX | TPsi (3 per chunk)
 template <typename T>
+__global__ void build_tri_tables_kernel(int N, int Pl, int Q, const double* __restrict__ fac,
+                                        T* __restrict__ tab, size_t tab_stride, double* __restrict__ tmat)
+{
+    constexpr int C = ChunkCfg<T>::C;
+    constexpr int BL = chunk_block_len<T, 1>();
+    int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= Pl * Q) return;
+    const double *beta = fac + N, *alpha = fac + 2 * N, *gamma = fac + 3 * N;
+    T* blk = tab + (size_t)(p / Pl) * tab_stride + (size_t)(p % Pl) * BL;
+    const int s = p * C;
+    double phi[C];
+    double hm1 = 1.0;                               // response of g to a unit incoming g_{s-1}
+    for (int j = 0; j < C; ++j) {
+        int k = s + j;
+        double ia = 0.0, bn = 0.0;
+        if (k < N) { ia = 1.0 / alpha[k]; bn = beta[k] / alpha[k]; }
+        blk[2 * j + 0] = (T)ia; blk[2 * j + 1] = (T)bn;
+        double h = -bn * hm1;
+        phi[j] = h; hm1 = h;
+    }
+    double* cm = tmat + (size_t)p * 3;
+    cm[0] = phi[C - 1];
+    double xp1 = 0.0, qp1 = 1.0;                    // chi_{j+1}, psi_{j+1}
+    for (int j = C - 1; j >= 0; --j) {
+        int k = s + j;
+        double ga = (k < N) ? gamma[k] : 0.0;
+        blk[2 * C + j] = (T)ga;
+        double x = phi[j] - ga * xp1;
+        double q = -ga * qp1;
+        blk[3 * C + 2 * j + 0] = (T)x; blk[3 * C + 2 * j + 1] = (T)q;
+        if (j == 0) { cm[1] = x; cm[2] = q; }
+        xp1 = x; qp1 = q;
+    }
+    for (int j = 5 * C; j < BL; ++j) blk[j] = (T)0;
+}
+
+template <typename T>
+__global__ void build_tri_products_kernel(int Pl, int Q, const double* __restrict__ tmat,
+                                          T* __restrict__ tab, size_t tab_stride, int* __restrict__ levels)
+{
+    __shared__ double wf[W_LEVELS][MAX_PL], wb[W_LEVELS][MAX_PL], pf[MAX_PL], pb[MAX_PL], blkm[16];
+    __shared__ int need_f, need_b;
+    const int q = threadIdx.x, rank = blockIdx.x;
+    const double* tm = tmat + (size_t)rank * Pl * 3;
+    T* wtab = tab + (size_t)rank * tab_stride + (size_t)Pl * chunk_block_len<T, 1>();
+    if (q == 0) { need_f = 0; need_b = 0; }
+    for (int l = 0; l < W_LEVELS; ++l) { wf[l][q] = 0.0; wb[l][q] = 0.0; }
+    if (q < Pl) {
+        wf[0][q] = (q >= 1) ? tm[q * 3] : 0.0;
+        wb[0][q] = (q + 1 <= Pl - 1) ? tm[q * 3 + 2] : 0.0;
+    }
+    if (q == 0) { pf[0] = tm[0]; for (int j = 1; j < Pl; ++j) pf[j] = tm[j * 3] * pf[j - 1]; }
+    if (q == 1) { pb[Pl - 1] = tm[(Pl - 1) * 3 + 2]; for (int j = Pl - 2; j >= 0; --j) pb[j] = tm[j * 3 + 2] * pb[j + 1]; }
+    if (q == 2) {
+        for (int r = 0; r < 8; ++r) {
+            double f = 1.0, b = 1.0;
+            if (r < Q) {
+                const double* t = tmat + (size_t)r * Pl * 3;
+                for (int j = 0; j < Pl; ++j) { f *= t[j * 3]; b *= t[j * 3 + 2]; }
+            }
+            blkm[r] = f; blkm[8 + r] = b;
+        }
+    }
+    __syncthreads();
+    for (int l = 1; l < W_LEVELS; ++l) {
+        const int d = 1 << (l - 1);
+        if (q < Pl && q >= 2 * d) wf[l][q] = wf[l - 1][q] * wf[l - 1][q - d];
+        if (q < Pl && q + 2 * d <= Pl - 1) wb[l][q] = wb[l - 1][q] * wb[l - 1][q + d];
+        __syncthreads();
+    }
+    if (q < Pl) {
+        for (int l = 0; l < W_LEVELS; ++l) {
+            const int d = 1 << l, n = Pl - d;
+            T* base = wtab + w_level_off(Pl, l, Q, 1);
+            if (q >= d) base[q - d] = (T)wf[l][q];
+            if (q + d <= Pl - 1) base[n + q] = (T)wb[l][q];
+            if (!(fabs(wf[l][q]) < 1e-25)) atomicMax(&need_f, l + 1);
+            if (!(fabs(wb[l][q]) < 1e-25)) atomicMax(&need_b, l + 1);
+        }
+        wtab[q] = (T)tm[q * 3 + 1];
+        if (Q > 1) { wtab[Pl + q] = (T)pf[q]; wtab[2 * Pl + q] = (T)pb[q]; }
+    }
+    if (Q > 1)
+        for (int j = q; j < 16; j += blockDim.x) wtab[3 * Pl + j] = (T)blkm[j];
+    __syncthreads();
+    if (q == 0) { atomicMax(&levels[0], need_f); atomicMax(&levels[1], need_b); }
+}
+
+template <typename T, int BAND>
 static int build_tables_t(pent_handle* h, int j, cudaStream_t s)
 {
     constexpr int C = ChunkCfg<T>::C;
     const int Q = 1 << j;
     const int P = (h->N + C - 1) / C;
     const int Pl = (P + Q - 1) / Q;
-    h->cf[j] = nullptr; h->cfP[j] = 0; h->lev_f[j] = h->lev_b[j] = 0;
+    void*& cfj = BAND == 2 ? h->cf[j] : h->cf1[j];
+    cfj = nullptr;
+    if (BAND == 2) { h->cfP[j] = 0; h->lev_f[j] = h->lev_b[j] = 0; } else { h->lev_f1[j] = h->lev_b1[j] = 0; }
     if (Pl > MAX_PL || (Q > 1 && Q > P)) return PENT_OK;     // not a usable split: no tables
-    const size_t tlen = table_len<T>(Pl, Q);
-    cudaError_t e = cudaMalloc(&h->cf[j], tlen * Q * sizeof(T));
+    const size_t tlen = table_len<T, BAND>(Pl, Q);
+    cudaError_t e = cudaMalloc(&cfj, tlen * Q * sizeof(T));
     if (e == cudaErrorMemoryAllocation) { cudaGetLastError(); return PENT_ERR_ALLOC; }
     PENT_CUDA(e);
     double* tmat = nullptr;
@@ -201,15 +294,20 @@ static int build_tables_t(pent_handle* h, int j, cudaStream_t s)
     cudaError_t le = cudaMallocAsync((void**)&tmat, sizeof(double) * 12 * Pl * Q, s);
     if (le == cudaSuccess) le = cudaMallocAsync((void**)&lev, 2 * sizeof(int), s);
     if (le == cudaSuccess) le = cudaMemsetAsync(lev, 0, 2 * sizeof(int), s);
-    if (le == cudaSuccess) le = cudaMemsetAsync(h->cf[j], 0, tlen * Q * sizeof(T), s);
+    if (le == cudaSuccess) le = cudaMemsetAsync(cfj, 0, tlen * Q * sizeof(T), s);
     if (le != cudaSuccess) {            // temporaries are released on every path; h->cf[j] belongs to the handle
         release();
         if (le == cudaErrorMemoryAllocation) { cudaGetLastError(); return PENT_ERR_ALLOC; }
         return cuda_fail(le);
     }
     const int tb = 32, nb = (Pl * Q + tb - 1) / tb;
-    build_chunk_tables_kernel<T><<<nb, tb, 0, s>>>(h->N, Pl, Q, h->fac, (T*)h->cf[j], tlen, tmat);
-    build_chunk_products_kernel<T><<<Q, 32, 0, s>>>(Pl, Q, tmat, (T*)h->cf[j], tlen, lev);
+    if constexpr (BAND == 2) {
+        build_chunk_tables_kernel<T><<<nb, tb, 0, s>>>(h->N, Pl, Q, h->fac, (T*)cfj, tlen, tmat);
+        build_chunk_products_kernel<T><<<Q, 32, 0, s>>>(Pl, Q, tmat, (T*)cfj, tlen, lev);
+    } else {
+        build_tri_tables_kernel<T><<<nb, tb, 0, s>>>(h->N, Pl, Q, h->fac, (T*)cfj, tlen, tmat);
+        build_tri_products_kernel<T><<<Q, 32, 0, s>>>(Pl, Q, tmat, (T*)cfj, tlen, lev);
+    }
     count_launch(2);
     le = cudaGetLastError();
     int hl[2] = {0, 0};
@@ -217,15 +315,20 @@ static int build_tables_t(pent_handle* h, int j, cudaStream_t s)
     release();
     if (le == cudaSuccess) le = cudaStreamSynchronize(s);
     if (le != cudaSuccess) return cuda_fail(le);
-    h->cfP[j] = Pl; h->lev_f[j] = hl[0]; h->lev_b[j] = hl[1];
+    if (BAND == 2) { h->cfP[j] = Pl; h->lev_f[j] = hl[0]; h->lev_b[j] = hl[1]; }
+    else { h->lev_f1[j] = hl[0]; h->lev_b1[j] = hl[1]; }
     return PENT_OK;
 }
 
 int build_chunk_tables(pent_handle* h, cudaStream_t s)
 {
     for (int j = 0; j < PENT_NQ; ++j) {
-        int rc = h->dtype == PENT_F64 ? build_tables_t<double>(h, j, s) : build_tables_t<float>(h, j, s);
+        int rc = h->dtype == PENT_F64 ? build_tables_t<double, 2>(h, j, s) : build_tables_t<float, 2>(h, j, s);
         if (rc != PENT_OK) return rc;
+        if (h->band == 1) {       // tridiagonal A: also the 5-word tables of the BAND = 1 instantiation
+            rc = h->dtype == PENT_F64 ? build_tables_t<double, 1>(h, j, s) : build_tables_t<float, 1>(h, j, s);
+            if (rc != PENT_OK) return rc;
+        }
     }
     return PENT_OK;
 }
@@ -260,7 +363,7 @@ static bool s_instantiated(bool f64, int S, bool cluster)
     return f64 ? (S == 16 || S == 32) : (S == 32 || S == 64);
 }
 
-ChunkPlan make_plan(const pent_handle* h, int64_t M, const void* f, int Q, int S, bool any_S, bool ldg)
+ChunkPlan make_plan(const pent_handle* h, int64_t M, const void* f, int Q, int S, bool any_S, bool ldg, int band)
 {
     ChunkPlan pl;
     if (!h || h->kind != 0) return pl;
@@ -269,6 +372,8 @@ ChunkPlan make_plan(const pent_handle* h, int64_t M, const void* f, int Q, int S
     int j = 0;
     while ((1 << j) < Q) ++j;
     if ((1 << j) != Q || j >= PENT_NQ || !h->cf[j] || h->cfP[j] < 1) return pl;
+    if (band != 2 && (band != 1 || !h->cf1[j])) return pl;
+    pl.band = band;
     if (!any_S && !s_instantiated(f64, S, Q > 1)) return pl;
     if (S < 4 || (S & (S - 1)) != 0) return pl;
     const int C = f64 ? ChunkCfg<double>::C : ChunkCfg<float>::C;
@@ -276,7 +381,8 @@ ChunkPlan make_plan(const pent_handle* h, int64_t M, const void* f, int Q, int S
     while (pl.Pw < pl.Pl) pl.Pw *= 2;
     int lg = 0;
     while ((1 << lg) < pl.Pw) ++lg;
-    pl.levels = h->lev_f[j] > h->lev_b[j] ? h->lev_f[j] : h->lev_b[j];
+    const int hlf = band == 2 ? h->lev_f[j] : h->lev_f1[j], hlb = band == 2 ? h->lev_b[j] : h->lev_b1[j];
+    pl.levels = hlf > hlb ? hlf : hlb;
     if (pl.levels > lg) pl.levels = lg;
     // cluster: one scan round (the scan registers live across the cluster barriers)
     pl.threads = ((Q > 1 ? pl.Pw * S : pl.Pl * S) + 31) / 32 * 32;
@@ -285,12 +391,16 @@ ChunkPlan make_plan(const pent_handle* h, int64_t M, const void* f, int Q, int S
     pl.box_rows = rows < BOX_ROWS_MAX ? rows : BOX_ROWS_MAX;
     pl.nbox = (rows + pl.box_rows - 1) / pl.box_rows;
     if (pl.nbox > MAX_BOXES) return pl;
-    const size_t bl = f64 ? chunk_block_len<double>() : chunk_block_len<float>();
-    pl.table_bytes = ((size_t)pl.Pl * bl + (size_t)w_level_off(pl.Pl, pl.levels, Q)) * esz;
+    const size_t bl = band == 2 ? (f64 ? chunk_block_len<double, 2>() : chunk_block_len<float, 2>())
+                                : (f64 ? chunk_block_len<double, 1>() : chunk_block_len<float, 1>());
+    pl.table_bytes = ((size_t)pl.Pl * bl + (size_t)w_level_off(pl.Pl, pl.levels, Q, band)) * esz;
+    pl.table_bytes = (pl.table_bytes + 15) & ~(size_t)15;     // cp.async.bulk moves multiples of 16 bytes (the
+                                                              // scalar W entries of BAND = 1 need not end on one)
     pl.ldg = ldg;
     if (ldg) pl.nbox = 0;                                    // no landing buffer
-    pl.smem = (size_t)pl.nbox * pl.box_rows * S * esz + pl.table_bytes + (size_t)4 * pl.Pl * S * esz +
-              (Q > 1 ? (size_t)2 * Q * S * esz : 0) + (3 + 2 * MAX_BOXES) * sizeof(uint64_t);   // one [Q][S] pair array
+    const size_t st = band == 2 ? 2 : 1;                     // words per chunk state
+    pl.smem = (size_t)pl.nbox * pl.box_rows * S * esz + pl.table_bytes + (size_t)2 * st * pl.Pl * S * esz +
+              (Q > 1 ? st * Q * S * esz : 0) + (3 + 2 * MAX_BOXES) * sizeof(uint64_t);   // one [Q][S] state array
     if (pl.smem > SMEM_LIMIT) return pl;
     if (!ldg) {
         if ((M * (int64_t)esz) % 16 != 0) return pl;        // TMA global stride alignment
@@ -350,30 +460,31 @@ bool encode_batch_map(CUtensorMap* tm, const void* base, int64_t M, int N, int S
 ChunkPlan chunk_auto_plan(const pent_handle* h, int64_t M, const void* f)
 {
     if (!h || h->kind != 0) return ChunkPlan{};
+    const int hb = h->band == 1 ? 1 : 2;        // tridiagonal handle: the BAND = 1 instantiation
     const int Sn = h->dtype == PENT_F64 ? 16 : 32, Sw = 2 * Sn, QMAX = 1 << (PENT_NQ - 1);
-    ChunkPlan narrow1 = make_plan(h, M, f, 1, Sn);
+    ChunkPlan narrow1 = make_plan(h, M, f, 1, Sn, false, false, hb);
     if (narrow1.ok && narrow1.threads <= 256) return narrow1;
     for (int Q = 1; Q <= 4; Q *= 2) {
-        ChunkPlan pl = make_plan(h, M, f, Q, Sw);
+        ChunkPlan pl = make_plan(h, M, f, Q, Sw, false, false, hb);
         if (pl.ok) return pl;
     }
     for (int Q = 1; Q <= QMAX; Q *= 2) {
-        ChunkPlan pl = make_plan(h, M, f, Q, Sn);
+        ChunkPlan pl = make_plan(h, M, f, Q, Sn, false, false, hb);
         if (pl.ok) return pl;
     }
     for (int Q = 1; Q <= QMAX; Q *= 2) {
-        ChunkPlan pl = make_plan(h, M, f, Q, Sw);
+        ChunkPlan pl = make_plan(h, M, f, Q, Sw, false, false, hb);
         if (pl.ok) return pl;
     }
     // TMA cannot address this batch (pitch or base not 16-byte aligned): LDG loader.  It has no
     // prefetch of the next tile, so prefer CTAs of <= 256 threads: two of them share an SM and one
     // loads while the other computes.
     for (int Q = 1; Q <= QMAX; Q *= 2) {
-        ChunkPlan pl = make_plan(h, M, f, Q, Sn, false, true);
+        ChunkPlan pl = make_plan(h, M, f, Q, Sn, false, true, hb);
         if (pl.ok && pl.threads <= 256) return pl;
     }
     for (int Q = 1; Q <= QMAX; Q *= 2) {
-        ChunkPlan pl = make_plan(h, M, f, Q, Sn, false, true);
+        ChunkPlan pl = make_plan(h, M, f, Q, Sn, false, true, hb);
         if (pl.ok) return pl;
     }
     return ChunkPlan{};
@@ -381,16 +492,17 @@ ChunkPlan chunk_auto_plan(const pent_handle* h, int64_t M, const void* f)
 
 static ChunkPlan resolve_plan(const pent_handle* h, int64_t M, const void* f, int Q, int S)
 {
+    const int hb = (h && h->kind == 0 && h->band == 1) ? 1 : 2;
     if (Q == 0 && S == 0) return chunk_auto_plan(h, M, f);
     if (Q != 0 && S != 0) {
-        ChunkPlan pl = make_plan(h, M, f, Q, S);
-        return pl.ok ? pl : make_plan(h, M, f, Q, S, false, true);
+        ChunkPlan pl = make_plan(h, M, f, Q, S, false, false, hb);
+        return pl.ok ? pl : make_plan(h, M, f, Q, S, false, true, hb);
     }
     const int cand[3] = {16, 32, 64};
     if (Q != 0) {
-        for (int s : cand) { ChunkPlan pl = make_plan(h, M, f, Q, s); if (pl.ok) return pl; }
+        for (int s : cand) { ChunkPlan pl = make_plan(h, M, f, Q, s, false, false, hb); if (pl.ok) return pl; }
     } else {
-        for (int q = 1; q <= (1 << (PENT_NQ - 1)); q *= 2) { ChunkPlan pl = make_plan(h, M, f, q, S); if (pl.ok) return pl; }
+        for (int q = 1; q <= (1 << (PENT_NQ - 1)); q *= 2) { ChunkPlan pl = make_plan(h, M, f, q, S, false, false, hb); if (pl.ok) return pl; }
     }
     return ChunkPlan{};
 }
@@ -413,14 +525,15 @@ int chunked_choice(const pent_handle* h, int64_t M, int* Q, int* S)
 static ChunkPlan rows_plan(const pent_handle* h, int64_t M)
 {
     if (!h || h->kind != 0 || h->periodic) return ChunkPlan{};
+    const int hb = h->band == 1 ? 1 : 2;
     const int Sn = h->dtype == PENT_F64 ? 16 : 32, QMAX = 1 << (PENT_NQ - 1);
     ChunkPlan best;
     for (int Q = 1; Q <= QMAX && !best.ok; Q *= 2) {
-        ChunkPlan pl = make_plan(h, M, nullptr, Q, Sn, false, true);
+        ChunkPlan pl = make_plan(h, M, nullptr, Q, Sn, false, true, hb);
         if (pl.ok && pl.threads <= 256) best = pl;
     }
     for (int Q = 1; Q <= QMAX && !best.ok; Q *= 2) {
-        ChunkPlan pl = make_plan(h, M, nullptr, Q, Sn, false, true);
+        ChunkPlan pl = make_plan(h, M, nullptr, Q, Sn, false, true, hb);
         if (pl.ok) best = pl;
     }
     best.rows = best.ok;
@@ -449,13 +562,16 @@ int launch_solve_chunked(const pent_handle* h, int64_t M, const void* f, void* x
 static int launch_plan(const pent_handle* h, const ChunkPlan& pl, int64_t M, const void* f, void* x, cudaStream_t s)
 {
     const bool cl = pl.Q > 1;
+#define PENT_INST(T_, S_, B_) (cl ? launch_inst<T_, S_, true, false, B_>(h, pl, M, f, x, s, nullptr) \
+                                  : launch_inst<T_, S_, false, false, B_>(h, pl, M, f, x, s, nullptr))
     if (h->dtype == PENT_F64) {
-        if (pl.S == 16) return cl ? launch_inst<double, 16, true, false>(h, pl, M, f, x, s, nullptr) : launch_inst<double, 16, false, false>(h, pl, M, f, x, s, nullptr);
-        if (pl.S == 32) return cl ? launch_inst<double, 32, true, false>(h, pl, M, f, x, s, nullptr) : launch_inst<double, 32, false, false>(h, pl, M, f, x, s, nullptr);
+        if (pl.S == 16) return pl.band == 1 ? PENT_INST(double, 16, 1) : PENT_INST(double, 16, 2);
+        if (pl.S == 32) return pl.band == 1 ? PENT_INST(double, 32, 1) : PENT_INST(double, 32, 2);
     } else {
-        if (pl.S == 32) return cl ? launch_inst<float, 32, true, false>(h, pl, M, f, x, s, nullptr) : launch_inst<float, 32, false, false>(h, pl, M, f, x, s, nullptr);
-        if (pl.S == 64) return cl ? launch_inst<float, 64, true, false>(h, pl, M, f, x, s, nullptr) : launch_inst<float, 64, false, false>(h, pl, M, f, x, s, nullptr);
+        if (pl.S == 32) return pl.band == 1 ? PENT_INST(float, 32, 1) : PENT_INST(float, 32, 2);
+        if (pl.S == 64) return pl.band == 1 ? PENT_INST(float, 64, 1) : PENT_INST(float, 64, 2);
     }
+#undef PENT_INST
     return PENT_ERR_ARG;
 }
 }  // namespace pent

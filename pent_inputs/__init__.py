@@ -152,6 +152,33 @@ def diagonals_I_plus_sigma_L2(N: int, sigma, bc: str = "dirichlet"):
     return a, b, c, d, e
 
 
+def heat4_cn_diagonals(N: int, s_h: float, bc: str = "dirichlet"):
+    """The pentadiagonal matrix of PAPER.md:96 (Remark 3): heat equation C_t = C_xx, Crank-Nicolson in time,
+    fourth-order centred differences in space (nearest and next-nearest neighbours),
+        C_xx ~ (-C_{i-2} + 16 C_{i-1} - 30 C_i + 16 C_{i+1} - C_{i+2}) / (12 dx^2) = (12 L - L^2) C / (12 dx^2),
+    so  A = I - (dt/2) (12 L - L^2) / (12 dx^2) = I + s_h (L^2 - 12 L),   s_h = dt / (24 dx^2),
+    and one step is A C+ = (2I - A) C (the library's kind-1 step).  Entries written out:
+      interior rows  (s_h, -16 s_h, 1 + 30 s_h, -16 s_h, s_h);
+      bc='dirichlet': L, L^2 formed exactly (corner diagonal 1 + 29 s_h), i.e. odd reflection at the walls;
+      bc='periodic' : five constant length-N arrays, every entry used (cyclic matrix, like Eq. 7a).
+    Returns (a, b, c, d, e), row-indexed like every other generator here."""
+    if N < 4:
+        raise ValueError("N >= 4 required")
+    one = np.ones(N)
+    if bc == "periodic":
+        return s_h * one, -16.0 * s_h * one, (1.0 + 30.0 * s_h) * one, -16.0 * s_h * one, s_h * one
+    if bc != "dirichlet":
+        raise ValueError(bc)
+    a = np.zeros(N); b = np.zeros(N); c = np.zeros(N); d = np.zeros(N); e = np.zeros(N)
+    c[:] = 1.0 + 30.0 * s_h
+    c[0] = c[-1] = 1.0 + 29.0 * s_h
+    d[:-1] = -16.0 * s_h
+    b[1:] = -16.0 * s_h
+    e[:-2] = s_h
+    a[2:] = s_h
+    return a, b, c, d, e
+
+
 def dense_from_diagonals(a, b, c, d, e) -> np.ndarray:
     """Assemble the dense N x N matrix from row-indexed diagonals (1 system)."""
     N = len(c)

@@ -408,3 +408,104 @@ def test_adi_like_two_axis_sweeps_on_a_2d_field():
     ref = oracle.solve_rows(oracle.factor(*dx_), np.ascontiguousarray(u), nthreads=8)        # rows
     ref = oracle.solve_batch(oracle.factor(*dy_), ref, nthreads=8)                           # columns
     assert normwise(ud.cpu().numpy(), ref) <= 1e-11
+
+
+# ---- BAND = 1: the tridiagonal instantiation of the chunked kernel (chosen when a == e == 0), every shape ----
+def _tri_case(N, M, Q, S, dtype, rows=False):
+    from scipy.linalg import solve_banded
+    pent = _pent()
+    a, b, c, d, e = pin.random_diag_dominant(700 + N, N)
+    a[:] = 0.0
+    e[:] = 0.0
+    f = pin.uniform_pm1(701 + N, 0, N, M)
+    h = pent.pent_factor(N, *(torch.tensor(v, dtype=dtype) for v in (e, c, d, a, b)))
+    assert pent.lib().pent_handle_band(h.ptr) == 1
+    if rows:
+        fg, xg = guarded(f.T, dtype), Guarded((M, N), dtype)
+        pent.pent_solve_batch_rows(h, M, fg.t, xg.t)
+        fg.check(); xg.check()
+        x = xg.numpy().T
+    else:
+        x, _ = gpu_solve((a, b, c, d, e), f, dtype=dtype, kernel=pent.KERNEL_CHUNKED_CFG(Q, S))
+    d64, f64, ref = oracle_for_dtype((a, b, c, d, e), f, dtype)
+    tol_x, tol_r = TOL[dtype]
+    assert normwise(x.astype(np.float64), ref) <= tol_x
+    assert residual(d64, np.ascontiguousarray(x), f64) <= tol_r
+    if dtype == torch.float64:                     # LAPACK's banded solver on the tridiagonal matrix
+        ab = np.zeros((3, N))
+        ab[0, 1:] = d[:-1]; ab[1] = c; ab[2, :-1] = b[1:]
+        assert normwise(x, solve_banded((1, 1), ab, f)) <= 1e-11
+
+
+@pytest.mark.parametrize("N,M,Q,S", [(1024, 2048 + 32, 2, 32), (1024, 512, 1, 16), (512, 1000, 1, 32), (2048, 520, 2, 16),
+                                     (4096, 304, 4, 16), (8192, 48, 8, 16), (64, 32, 2, 16), (1000, 200, 2, 32),
+                                     (3000, 100, 4, 16), (33, 18, 1, 16), (5, 4, 1, 16), (1, 6, 1, 16), (1024, 77, 2, 16)])
+def test_tridiagonal_instantiation_shapes_fp64(N, M, Q, S):
+    _tri_case(N, M, Q, S, torch.float64)
+
+
+@pytest.mark.parametrize("N,M,Q,S", [(1024, 2048 + 64, 2, 64), (1024, 1024, 1, 32), (4096, 512, 4, 32), (700, 333, 1, 32)])
+def test_tridiagonal_instantiation_shapes_fp32(N, M, Q, S):
+    _tri_case(N, M, Q, S, torch.float32)
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+def test_tridiagonal_instantiation_system_major(dtype):
+    _tri_case(1024, 300, 0, 0, dtype, rows=True)
+
+
+def test_tridiagonal_full_size_cfg3_shape_every_system():
+    """cfg3's shape with a tridiagonal matrix (I - sigma L, the Crank-Nicolson heat matrix of cuThomasBatch's
+    use case): AUTO runs the BAND = 1 instantiation; every system against the oracle."""
+    pent = _pent()
+    w = WORKLOADS["cfg3"]
+    N, M = w.N, w.M
+    z = np.zeros(N)
+    b = np.full(N, -10.0); b[0] = 0.0
+    d = np.full(N, -10.0); d[-1] = 0.0
+    c = np.full(N, 21.0)
+    f = make_rhs(w)
+    x, h = gpu_solve((z, b, c, d, z), f)
+    assert pent.lib().pent_handle_band(h.ptr) == 1
+    ref = oracle.solve_batch(oracle.factor(z, b, c, d, z), f, nthreads=8)
+    assert normwise(x, ref) <= 1e-11
+    assert residual((z, b, c, d, z), x, f) <= 1e-12
+
+
+# ---- PAPER.md:96 (Remark 3): the fourth-order Crank-Nicolson heat matrix, solve and time step ----
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_heat4_matrix_solve_and_closed_form(kernel):
+    N, M, s_h = 1024, 2048 + 8, 40.0
+    diags = pin.heat4_cn_diagonals(N, s_h)
+    f = pin.uniform_pm1(801, 0, N, M)
+    x, _ = gpu_solve(diags, f, kernel=kernel)
+    assert normwise(x, oracle.solve_batch(oracle.factor(*diags), f, nthreads=8)) <= 1e-11
+    assert residual(diags, x, f) <= 1e-12
+    j = np.arange(1, N + 1)[:, None]
+    k = np.arange(1, 33)[None, :]
+    modes = np.sin(np.pi * ((k * j) % (2 * (N + 1))) / (N + 1))
+    mu = 4.0 * np.sin(np.pi * np.arange(1, 33) / (2 * (N + 1))) ** 2
+    lam = 1.0 + s_h * (mu * mu + 12.0 * mu)
+    xm, _ = gpu_solve(diags, modes, kernel=kernel)
+    assert normwise(xm, modes / lam[None, :]) <= 1e-11
+
+
+def test_heat4_crank_nicolson_steps_on_chip():
+    """A C+ = (2I - A) C with the Remark-3 matrix = the kind-1 step; 50 steps on chip against the oracle and the
+    exact amplification factor of sine mode 3."""
+    pent = _pent()
+    N, M, steps = 512, 128, 50
+    dx = 1.0 / (N + 1)
+    s_h = 1e-5 / (24.0 * dx * dx)
+    diags = pin.heat4_cn_diagonals(N, s_h)
+    h = pent.pent_factor(N, *(torch.tensor(v) for v in (diags[4], diags[2], diags[3], diags[0], diags[1])))
+    xg = np.arange(1, N + 1) * dx
+    c0 = np.repeat(np.sin(3 * np.pi * xg)[:, None], M, axis=1) * pin.uniform_vec(802, 1, M, 0.5, 2.0)[None, :]
+    cg = guarded(c0)
+    pent.pent_step_batch(h, M, cg.t, steps, kind=1)
+    cg.check()
+    ref = oracle.step_batch(oracle.factor(*diags), 1, 0, 0, 0.0, 0.0, c0, steps, nthreads=8)
+    assert normwise(cg.numpy(), ref) <= 1e-11 * steps
+    mu = 4.0 * np.sin(3 * np.pi / (2 * (N + 1))) ** 2
+    lam = 1.0 + s_h * (mu * mu + 12.0 * mu)
+    assert normwise(cg.numpy(), ((2.0 - lam) / lam) ** steps * c0) <= 1e-10
