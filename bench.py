@@ -45,7 +45,11 @@ def parse_args():
     ap.add_argument("--tile", type=int, default=0, help="chunked kernel: systems per tile (0 auto)")
     ap.add_argument("--layout", default="interleaved", choices=["interleaved", "rows"],
                     help="rows: system-major batch through pent_solve_batch_rows")
+    ap.add_argument("--rows-ldg", action="store_true", help="--layout rows: the per-thread LDG.256 loader instead of swizzled TMA")
+    ap.add_argument("--rows-stg", action="store_true", help="--layout rows: bulk loads but STG.256 stores (A/B)")
+    ap.add_argument("--rows-tma2d", action="store_true", help="--layout rows: swizzled tensor-tile TMA loads, STG.256 stores (A/B)")
     ap.add_argument("--systems", type=int, default=0, help="override M of the workload (shape experiments)")
+    ap.add_argument("--rows-n", type=int, default=0, help="override N of the workload (shape experiments; matrix regenerated)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=3)
@@ -235,6 +239,11 @@ def run_ours(args):
         return run_per_system_workload(args, w, rank, world, local)
     if w.name == "paper_hd":
         return run_paper_workload(args, w, rank, world, local)
+    if w.name == "adi2d":
+        return run_adi_workload(args, w, rank, world, local)
+    if args.rows_n:
+        import dataclasses
+        w = dataclasses.replace(w, N=args.rows_n)
     tdt = torch.float64 if args.dtype == "f64" else torch.float32
     esz = 8 if args.dtype == "f64" else 4
     N, M = w.N, (args.systems or w.M)
@@ -256,14 +265,15 @@ def run_ours(args):
     fd = f_host.cuda()
     xd = torch.empty_like(fd)
     stream = torch.cuda.current_stream()
+    if args.cluster or args.tile:
+        args.kernel = pent.KERNEL_CHUNKED_CFG(args.cluster, args.tile)
     if args.layout == "rows":
         fd = fd.t().contiguous()
         xd = torch.empty_like(fd)
-        solve = lambda: pent.pent_solve_batch_rows(h, M, fd, xd)
+        rk = (args.kernel if (args.cluster and args.tile) else 0) | (pent.ROWS_LDG if args.rows_ldg else 0) | (pent.ROWS_STG if args.rows_stg else 0) | (pent.ROWS_TMA2D if args.rows_tma2d else 0)
+        solve = lambda: pent.pent_solve_batch_rows(h, M, fd, xd, kernel=rk)
     else:
         solve = lambda: pent.pent_solve_batch(h, M, fd, xd, kernel=args.kernel)
-    if args.cluster or args.tile:
-        args.kernel = pent.KERNEL_CHUNKED_CFG(args.cluster, args.tile)
 
     def barrier():
         if world > 1:
@@ -339,8 +349,14 @@ def run_ours(args):
         "warmup": max(args.warmup, 3), "ms_per_step": total_ms_max / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": args.dtype,
         "data": "synthetic",
-        "config": {"workload": w.name, "N": N, "M_per_gpu": M, "matrix": f"I+sigma*L^2 {w.bc} sigma={w.sigma}",
-                   "rhs": w.rhs, "seed": w.seed, "layout": "interleaved f[k*M+i]" if args.layout == "interleaved" else "system-major f[i*N+k]", "kernel": kname,
+        "config": {"workload": w.name, "N": N, "M_per_gpu": M,
+                   "matrix": (f"I+sigma*L^2 {w.bc} sigma={w.sigma}" if w.bc in ("dirichlet", "zeroflux", "periodic")
+                              else f"{w.bc} sigma={w.sigma}"),
+                   "rhs": w.rhs, "seed": w.seed,
+                   "layout": "interleaved f[k*M+i]" if args.layout == "interleaved" else
+                             ("system-major f[i*N+k], " + ("LDG.256 loader" if args.rows_ldg else "bulk loads + STG.256 stores" if args.rows_stg
+                                                         else "swizzled TMA loads + STG.256 stores" if args.rows_tma2d else "1-D bulk copies both ways")),
+                   "kernel": kname, "band": int(pent.lib().pent_handle_band(h.ptr)),
                    "cluster_ctas_along_k": ch["Q"], "systems_per_tile": ch["S"],
                    "l2": f"inputs+outputs {2 * esz * N * M >> 20} MiB per step exceed the 126 MB L2"},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
@@ -487,6 +503,63 @@ def run_paper_workload(args, w, rank, world, local):
                      "kernel": "solve_chunked_kernel",
                      "note": "algorithmic = read the state once, write it once per step; the unfused path makes 6 "
                              "passes per step, mostly served by L2 at this size"},
+        "clocks": clocks, "gpu_launches": int(launches),
+    }
+    _finish_line(line, world)
+
+
+def run_adi_workload(args, w, rank, world, local):
+    """adi2d: a step = ONE Peaceman-Rachford ADI time step of the 2-D heat equation on an N x N field
+    (PAPER.md:379, :96): (2I - A_y) u along y, solve A_x along x (rows of the field), (2I - A_x) u* along x,
+    solve A_y along y (columns).  2 N^2 unknowns are solved per step."""
+    import torch
+    import paper_1807_07382_b200 as pent
+    import pent_inputs as pin
+    from pent_inputs.configs import make_matrix
+    from paper_1807_07382_b200.sharding import max_over_ranks, whole_job_rate
+    tdt = torch.float64 if args.dtype == "f64" else torch.float32
+    esz = 8 if args.dtype == "f64" else 4
+    N = args.rows_n or w.N
+    import dataclasses
+    w = dataclasses.replace(w, N=N, M=N)
+    a, b, c, d, e = (torch.tensor(v, dtype=tdt) for v in make_matrix(w))
+    hx = pent.pent_factor(N, e, c, d, a, b)
+    hy = pent.pent_factor(N, e, c, d, a, b)
+    u = torch.tensor(pin.uniform_pm1(w.seed, rank, N, N), dtype=tdt, device="cuda")
+    scratch = torch.empty_like(u)
+    stream = torch.cuda.current_stream()
+    pent.pent_adi_step_batch(hx, hy, u, max(args.warmup, 3), scratch=scratch)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    pent.launch_count(reset=True)
+    sampler.start()
+    e0.record(stream)
+    pent.pent_adi_step_batch(hx, hy, u, args.steps, scratch=scratch)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    launches = pent.launch_count()
+    ms = max_over_ranks(e0.elapsed_time(e1), "cuda")
+    if rank != 0:
+        return
+    peak, peak_src = measured_peak()
+    unknowns = 2.0 * N * N                         # two half steps, each solves every grid point once
+    alg = 2.0 * esz * unknowns                     # per half step: read the field once, write it once
+    achieved = alg * args.steps / (ms * 1e-3) / 1e9
+    line = {
+        "metric": METRIC, "value": whole_job_rate(int(unknowns) * args.steps, world, ms * 1e-3), "unit": UNIT,
+        "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
+        "config": {"workload": w.name, "N": N, "M_per_gpu": N, "field": f"{N} x {N}, row-major",
+                   "matrix": f"Remark-3 fourth-order Crank-Nicolson heat matrix, sigma={w.sigma}, both axes",
+                   "step": "Peaceman-Rachford ADI: rhs along y, solve rows (system-major), rhs along x, solve columns (interleaved)",
+                   "kernel": "adi_rhs_cols_kernel + solve_chunked_kernel(rows) + adi_rhs_rows_kernel + solve_chunked_kernel",
+                   "l2": f"field {esz * N * N >> 20} MiB + scratch of the same size"},
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": None, "peak_source": peak_src, "algorithmic_bytes_per_launch": alg,
+                     "kernel": "solve_chunked_kernel",
+                     "note": "algorithmic = 2 passes over the field per half step (4 per step); the unfused path makes 8"},
         "clocks": clocks, "gpu_launches": int(launches),
     }
     _finish_line(line, world)

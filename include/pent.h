@@ -97,6 +97,14 @@ int pent_solve_batch_v(const pent_handle* h, int64_t M, const void* f, void* x, 
  * elements with 32-byte accesses (16-byte aligned runs fall back to narrower ones): 2 passes over the
  * batch, no transpose. */
 int pent_solve_batch_rows(const pent_handle* h, int64_t M, const void* f, void* x, void* stream);
+/* Same with an explicit shape / data path (measurement): kernel = PENT_KERNEL_AUTO or PENT_KERNEL_CHUNKED_CFG(Q, S),
+ * optionally OR-ed with one of the flags below.  Default: one 1-D bulk copy (cp.async.bulk) per system and tile in
+ * each direction, through padded shared-memory buffers; when the staging buffer does not fit, bulk loads with 32-byte
+ * STG stores; when N * sizeof(element) or a base address is not 16-byte aligned, the per-thread LDG loader. */
+#define PENT_ROWS_LDG   (1 << 24)   /* per-thread 32-byte LDG / STG accesses */
+#define PENT_ROWS_STG   (1 << 25)   /* bulk loads, 32-byte STG stores */
+#define PENT_ROWS_TMA2D (1 << 26)   /* swizzled tensor-tile TMA loads (128-byte rows), 32-byte STG stores (A/B baseline) */
+int pent_solve_batch_rows_v(const pent_handle* h, int64_t M, const void* f, void* x, void* stream, int kernel);
 
 /* Same operation with HOST buffers (pageable or pinned): copies slabs of systems to the device,
  * solves, copies back, pipelined on internal streams; returns when x_host is complete.
@@ -204,6 +212,17 @@ int pent_step_batch_forced(const pent_handle* h, const pent_step_params* p, cons
                            void* c_inout, void* scratch, int nsteps, void* stream);
 int pent_step_batch_forced_v(const pent_handle* h, const pent_step_params* p, const pent_forcing* g, int64_t M,
                              void* c_inout, void* scratch, int nsteps, void* stream, int kernel);
+
+/* ---- 2-D ADI time step built on the 1-D solves (section IV; reading C-23) ---------
+ * Peaceman-Rachford splitting of u_t = D_x u + D_y u with A_x = I - (dt/2) D_x (handle hx, N = Nx) and
+ * A_y = I - (dt/2) D_y (handle hy, N = Ny), e.g. the Remark-3 heat matrices:
+ *     A_x u* = (2I - A_y) u^n  (explicit along y, implicit along x),   A_y u^{n+1} = (2I - A_x) u*.
+ * u: device, Ny x Nx elements, row-major (u[y*Nx + x]), updated in place: its rows are solved as a system-major
+ * batch (pent_solve_batch_rows), its columns as an interleaved batch (pent_solve_batch).  scratch: device,
+ * Ny*Nx elements, or NULL (stream-ordered temporary).  hx, hy: shared-A, non-periodic, same dtype;
+ * PENT_ERR_ARG otherwise, or when Nx is too long for the on-chip row solve.  Asynchronous on `stream`. */
+int pent_adi_step_batch(const pent_handle* hx, const pent_handle* hy, void* u, void* scratch, int nsteps,
+                        void* stream);
 
 /* ---- introspection ------------------------------------------------------------------------ */
 int pent_handle_n(const pent_handle* h);                 /* N, or -1 */

@@ -21,7 +21,8 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = [os.path.join(_HERE, "pent_oracle.c"), os.path.join(_HERE, "pent_oracle_step.c"),
-        os.path.join(_HERE, "pent_oracle_periodic.c"), os.path.join(_HERE, "pent_oracle_ld.c")]
+        os.path.join(_HERE, "pent_oracle_periodic.c"), os.path.join(_HERE, "pent_oracle_ld.c"),
+        os.path.join(_HERE, "pent_oracle_adi.c")]
 _LIB = os.path.join(_HERE, "libpent_oracle.so")
 _lib = None
 
@@ -294,3 +295,20 @@ def ld_solve_periodic_batch(diags, f_interleaved, nthreads: int = 1) -> np.ndarr
     if rc != 0:
         raise SingularPivot(rc - 1)
     return np.ascontiguousarray(X.T)
+
+
+# ---- 2-D ADI time step on top of the 1-D solver (pent_oracle_adi.c, reading C-23) ----
+def adi_steps(fac_x: Factors, fac_y: Factors, u, nsteps: int, nthreads: int = 1) -> np.ndarray:
+    """nsteps Peaceman-Rachford steps on a field u of shape (Ny, Nx) (row-major): A_x u* = (2I - A_y) u,
+    A_y u+ = (2I - A_x) u*.  fac_x / fac_y: factors of A_x (N = Nx) and A_y (N = Ny)."""
+    U = np.array(u, dtype=np.float64, order="C", copy=True)
+    Ny, Nx = U.shape
+    assert fac_x.N == Nx and fac_y.N == Ny
+    W = np.empty_like(U)
+    pack = lambda vs: np.ascontiguousarray(np.concatenate([_f64(v) for v in vs]))
+    dx, dy = pack(fac_x.diags), pack(fac_y.diags)
+    fx = pack((fac_x.eps, fac_x.beta, fac_x.alpha, fac_x.gamma, fac_x.delta))
+    fy = pack((fac_y.eps, fac_y.beta, fac_y.alpha, fac_y.gamma, fac_y.delta))
+    _load().pent_oracle_adi_steps(C.c_int(Nx), C.c_int(Ny), _p(dx), _p(fx), _p(dy), _p(fy), _p(U), _p(W),
+                                  C.c_int(nsteps), C.c_int(nthreads))
+    return U

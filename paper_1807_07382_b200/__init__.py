@@ -76,6 +76,7 @@ def lib() -> C.CDLL:
     L.pent_solve_batch_v.argtypes = [vp, i64, vp, vp, vp, ci]
     L.pent_solve_batch_host.argtypes = [vp, i64, vp, vp]
     L.pent_solve_batch_rows.argtypes = [vp, i64, vp, vp, vp]
+    L.pent_solve_batch_rows_v.argtypes = [vp, i64, vp, vp, vp, ci]
     L.pent_destroy.argtypes = [vp]
     L.pent_destroy.restype = None
     L.pent_factor_solve_batch.argtypes = [ci, i64, vp, vp, vp, vp, vp, vp, vp, ci, vp, vp]
@@ -88,6 +89,7 @@ def lib() -> C.CDLL:
     L.pent_step_batch_forced.argtypes = [vp, C.POINTER(pent_step_params), C.POINTER(pent_forcing), i64, vp, vp, ci, vp]
     L.pent_step_batch_forced_v.argtypes = [vp, C.POINTER(pent_step_params), C.POINTER(pent_forcing), i64, vp, vp, ci,
                                            vp, ci]
+    L.pent_adi_step_batch.argtypes = [vp, vp, vp, vp, ci, vp]
     L.pent_handle_n.argtypes = [vp]
     L.pent_handle_dtype.argtypes = [vp]
     L.pent_handle_m.argtypes = [vp]
@@ -213,13 +215,19 @@ def pent_solve_batch(h: Handle, M: int, f: torch.Tensor, x: torch.Tensor | None 
     return x
 
 
-def pent_solve_batch_rows(h: Handle, M: int, f: torch.Tensor, x: torch.Tensor | None = None, stream=None) -> torch.Tensor:
+ROWS_LDG = 1 << 24
+ROWS_STG = 1 << 25
+ROWS_TMA2D = 1 << 26
+
+
+def pent_solve_batch_rows(h: Handle, M: int, f: torch.Tensor, x: torch.Tensor | None = None, stream=None,
+                          kernel: int = KERNEL_AUTO) -> torch.Tensor:
     """Same solve on a system-major batch: f, x of shape (M, N), one system per row."""
     _batch(f, "f", (M, h.N), h.dtype)
     if x is None:
         x = torch.empty_like(f)
     _batch(x, "x", (M, h.N), h.dtype)
-    _check(lib().pent_solve_batch_rows(h.ptr, M, f.data_ptr(), x.data_ptr(), _stream(stream)))
+    _check(lib().pent_solve_batch_rows_v(h.ptr, M, f.data_ptr(), x.data_ptr(), _stream(stream), kernel))
     return x
 
 
@@ -311,6 +319,20 @@ def pent_step_batch(h: Handle, M: int, c: torch.Tensor, nsteps: int, *, kind: in
     _check(lib().pent_step_batch_forced_v(h.ptr, C.byref(p), C.byref(g), M, c.data_ptr(), sp, nsteps,
                                           _stream(stream), kernel))
     return c
+
+
+def pent_adi_step_batch(hx: Handle, hy: Handle, u: torch.Tensor, nsteps: int, scratch: torch.Tensor | None = None,
+                        stream=None) -> torch.Tensor:
+    """nsteps Peaceman-Rachford ADI steps in place on the field u of shape (Ny, Nx) = (hy.N, hx.N)
+    (PAPER.md:379; include/pent.h)."""
+    _batch(u, "u", (hy.N, hx.N), hx.dtype)
+    if hy.dtype != hx.dtype:
+        raise ValueError("hx and hy must have one dtype")
+    if scratch is not None:
+        _vec(scratch, "scratch", hx.N * hy.N, hx.dtype)
+    _check(lib().pent_adi_step_batch(hx.ptr, hy.ptr, u.data_ptr(), 0 if scratch is None else scratch.data_ptr(),
+                                     nsteps, _stream(stream)))
+    return u
 
 
 def launch_count(reset: bool = False) -> int:

@@ -1,0 +1,120 @@
+// pent_adi.cu -- a 2-D alternating-direction-implicit time step on top of the batched 1-D solver
+// (section IV: "reduced to a series of one-dimensional problems using the ADI technique").
+// Peaceman-Rachford splitting of u_t = D_x u + D_y u with A_x = I - (dt/2) D_x, A_y = I - (dt/2) D_y
+// (reading C-23):
+//     half step 1:   A_x u*      = (2I - A_y) u^n      explicit along y, implicit along x
+//     half step 2:   A_y u^{n+1} = (2I - A_x) u*       explicit along x, implicit along y
+// The field u is Ny x Nx, row-major.  Its ROWS are the x-lines = a system-major batch of Ny systems of length
+// Nx (pent_solve_batch_rows); its COLUMNS are the y-lines = an interleaved batch of Nx systems of length Ny
+// (pent_solve_batch, the library's native layout: element k of system i at k*Nx + i).  Each explicit part is
+// the (2I - A) c stencil of PAPER.md:117 (Eq. 7c) along one axis with the handle's own diagonals.
+#include "pent_internal.h"
+
+namespace pent {
+
+// out = (2I - A) v along the STRIDED axis of an (N x M) array (interleaved batch: the columns of the field);
+// a block covers ROWS rows x blockDim.x systems, every v read once from HBM (+ 4 halo rows per block)
+template <typename T, int ROWS>
+__global__ void adi_rhs_cols_kernel(int N, int64_t M, const T* __restrict__ dg, const T* __restrict__ v,
+                                    T* __restrict__ out)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= M) return;
+    const int k0 = blockIdx.y * ROWS;
+    T w[ROWS + 4];
+#pragma unroll
+    for (int r = 0; r < ROWS + 4; ++r) {
+        const int k = k0 + r - 2;
+        w[r] = (k >= 0 && k < N) ? v[(int64_t)k * M + i] : (T)0;
+    }
+#pragma unroll
+    for (int r = 0; r < ROWS; ++r) {
+        const int k = k0 + r;
+        if (k < N) {
+            const T* dk = dg + 8 * (size_t)k;          // entries outside the matrix are zero in the table
+            T s = __ldg(dk + 2) * w[r + 2];
+            s = fma(__ldg(dk + 1), w[r + 1], s);
+            s = fma(__ldg(dk + 0), w[r], s);
+            s = fma(__ldg(dk + 3), w[r + 3], s);
+            s = fma(__ldg(dk + 4), w[r + 4], s);
+            out[(int64_t)k * M + i] = (T)2 * w[r + 2] - s;
+        }
+    }
+}
+
+// out = (2I - A) v along the CONTIGUOUS axis of an (M x N) array (system-major batch: the rows of the field).
+// Thread = one k for RSYS consecutive systems: its five coefficients are loaded once, consecutive threads =
+// consecutive k (coalesced; the four neighbours of every element come from L1).
+template <typename T, int RSYS>
+__global__ void adi_rhs_rows_kernel(int N, int64_t M, const T* __restrict__ dg, const T* __restrict__ v,
+                                    T* __restrict__ out)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t i0 = ((int64_t)blockIdx.y + (int64_t)blockIdx.z * gridDim.y) * RSYS;
+    if (k >= N || i0 >= M) return;
+    const T* dk = dg + 8 * (size_t)k;                // entries outside the matrix are zero in the table
+    const T ca = __ldg(dk + 0), cb = __ldg(dk + 1), cc = __ldg(dk + 2), cd = __ldg(dk + 3), ce = __ldg(dk + 4);
+    const int km2 = k >= 2 ? k - 2 : k, km1 = k >= 1 ? k - 1 : k, kp1 = k + 1 < N ? k + 1 : k, kp2 = k + 2 < N ? k + 2 : k;
+#pragma unroll 4
+    for (int r = 0; r < RSYS; ++r) {
+        const int64_t i = i0 + r;
+        if (i >= M) break;
+        const T* vi = v + i * (int64_t)N;
+        const T c0 = vi[k];
+        T s = cc * c0;
+        s = fma(cb, vi[km1], s);
+        s = fma(ca, vi[km2], s);
+        s = fma(cd, vi[kp1], s);
+        s = fma(ce, vi[kp2], s);
+        out[i * (int64_t)N + k] = (T)2 * c0 - s;
+    }
+}
+
+template <typename T>
+static int adi_steps_t(const pent_handle* hx, const pent_handle* hy, T* u, T* w, int nsteps, cudaStream_t s)
+{
+    const int Nx = hx->N, Ny = hy->N;
+    constexpr int ROWS = 8;
+    const int tb = 128;
+    const dim3 gcols((unsigned)((Nx + tb - 1) / tb), (unsigned)((Ny + ROWS - 1) / ROWS));
+    constexpr int RSYS = 16;
+    const int64_t nby = ((int64_t)Ny + RSYS - 1) / RSYS;
+    const unsigned gy = nby < 65535 ? (unsigned)nby : 65535u;
+    const dim3 grows((unsigned)((Nx + tb - 1) / tb), gy, (unsigned)((nby + gy - 1) / gy));
+    for (int it = 0; it < nsteps; ++it) {
+        adi_rhs_cols_kernel<T, ROWS><<<gcols, tb, 0, s>>>(Ny, Nx, (const T*)hy->dg, u, w);
+        count_launch();
+        PENT_LAUNCH_CHECK();
+        int rc = pent_solve_batch_rows(hx, Ny, w, w, (void*)s);          // x-lines: rows of the field
+        if (rc != PENT_OK) return rc;
+        adi_rhs_rows_kernel<T, RSYS><<<grows, tb, 0, s>>>(Nx, Ny, (const T*)hx->dg, w, u);
+        count_launch();
+        PENT_LAUNCH_CHECK();
+        rc = pent_solve_batch(hy, Nx, u, u, (void*)s);                   // y-lines: columns of the field
+        if (rc != PENT_OK) return rc;
+    }
+    return PENT_OK;
+}
+}  // namespace pent
+
+extern "C" int pent_adi_step_batch(const pent_handle* hx, const pent_handle* hy, void* u, void* scratch,
+                                   int nsteps, void* stream)
+{
+    if (!hx || !hy || hx->kind != 0 || hy->kind != 0 || hx->periodic || hy->periodic) return PENT_ERR_ARG;
+    if (hx->dtype != hy->dtype || !u || nsteps < 0) return PENT_ERR_ARG;
+    if (nsteps == 0) return PENT_OK;
+    if (!pent::on_handle_device(hx) || !pent::on_handle_device(hy)) return PENT_ERR_ARG;
+    if (!pent::chunked_rows_supported(hx, hy->N)) return PENT_ERR_ARG;       // Nx too long for the on-chip row solve
+    cudaStream_t s = (cudaStream_t)stream;
+    const size_t esz = hx->dtype == PENT_F64 ? 8 : 4;
+    void* w = scratch;
+    if (!w) {
+        cudaError_t er = cudaMallocAsync(&w, (size_t)hx->N * (size_t)hy->N * esz, s);
+        if (er == cudaErrorMemoryAllocation) { cudaGetLastError(); return PENT_ERR_ALLOC; }
+        PENT_CUDA(er);
+    }
+    const int rc = hx->dtype == PENT_F64 ? pent::adi_steps_t<double>(hx, hy, (double*)u, (double*)w, nsteps, s)
+                                         : pent::adi_steps_t<float>(hx, hy, (float*)u, (float*)w, nsteps, s);
+    if (!scratch) cudaFreeAsync(w, s);
+    return rc;
+}

@@ -33,13 +33,25 @@ extern "C" int pent_solve_batch_v(const pent_handle* h, int64_t M, const void* f
 
 // System-major batches ("one system per row", the layout of the paper's serial code; also
 // the access an ADI sweep along the contiguous axis of a 2-D field needs).
-extern "C" int pent_solve_batch_rows(const pent_handle* h, int64_t M, const void* f, void* x, void* stream)
+extern "C" int pent_solve_batch_rows_v(const pent_handle* h, int64_t M, const void* f, void* x, void* stream,
+                                       int kernel)
 {
     if (!h || h->kind != 0 || h->periodic || M < 0) return PENT_ERR_ARG;
     if (M == 0) return PENT_OK;
     if (!f || !x || !pent::on_handle_device(h)) return PENT_ERR_ARG;
-    const int rc = pent::launch_solve_chunked_rows(h, M, f, x, (cudaStream_t)stream);
+    const int loader = (kernel & PENT_ROWS_LDG) ? 1 : (kernel & PENT_ROWS_STG) ? 2 : (kernel & PENT_ROWS_TMA2D) ? 3 : 0;
+    kernel &= ~(PENT_ROWS_LDG | PENT_ROWS_STG | PENT_ROWS_TMA2D);
+    if (kernel < 0 || (kernel >> 24) != 0) return PENT_ERR_ARG;
+    if ((kernel & 0xff) != PENT_KERNEL_AUTO && (kernel & 0xff) != PENT_KERNEL_CHUNKED) return PENT_ERR_ARG;
+    const int Q = (kernel >> 8) & 0xff, S = (kernel >> 16) & 0xff;
+    if ((Q != 0) != (S != 0)) return PENT_ERR_ARG;
+    const int rc = pent::launch_solve_chunked_rows(h, M, f, x, (cudaStream_t)stream, Q, S, loader);
     return rc == pent::PENT_UNSUPPORTED ? PENT_ERR_ARG : rc;           // N too long to keep a tile on chip
+}
+
+extern "C" int pent_solve_batch_rows(const pent_handle* h, int64_t M, const void* f, void* x, void* stream)
+{
+    return pent_solve_batch_rows_v(h, M, f, x, stream, PENT_KERNEL_AUTO);
 }
 
 extern "C" int pent_solve_kernel_choice(const pent_handle* h, int64_t M)

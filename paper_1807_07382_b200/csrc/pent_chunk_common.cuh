@@ -101,6 +101,12 @@ __device__ __forceinline__ void bulk_load_1d(void* dst, const void* src, uint32_
         ::"r"(smem_u32(dst)), "l"((uint64_t)src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
+__device__ __forceinline__ void tma_store_2d(const CUtensorMap* tm, int c0, int c1, const void* src)
+{
+    asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%1, %2}], [%3];"
+                 ::"l"((uint64_t)tm), "r"(c0), "r"(c1), "r"(smem_u32(src)) : "memory");
+}
+
 // per-thread asynchronous copies global -> shared (LDGSTS), 8 or 4 bytes
 __device__ __forceinline__ void cp_async_elem(double* dst, const double* src)
 {
@@ -557,6 +563,8 @@ struct ChunkPlan {
     bool ldg = false;          // LDG loader instead of TMA (pitch not a multiple of 16 bytes, or system-major batch)
     bool rows = false;         // system-major batch: implies ldg
     int band = 2;              // 1: the tridiagonal instantiation and its tables (handle with a == e == 0)
+    int mode = 0;              // ChunkParams::ldg: 0 TMA (interleaved), 1 LDG (interleaved), 2 LDG.256 (system-major),
+                               // 3 swizzled TMA loads + STG.256 stores, 4 swizzled TMA loads AND stores (system-major)
     size_t table_bytes = 0, smem = 0;
 };
 // any_S: accept tile widths the SOLVE kernel is not instantiated for (the step kernel has its own)
@@ -567,5 +575,9 @@ ChunkPlan chunk_auto_plan(const pent_handle* h, int64_t M, const void* f);   // 
 // rank-2 tensor map {M, N} of an interleaved batch with box {S, box_rows}; false on failure
 bool encode_batch_map(CUtensorMap* tm, const void* base, int64_t M, int N, int S, int box_rows, bool f64);
 bool encode_batch_map_cached(CUtensorMap* tm, const void* base, int64_t M, int N, int S, int box_rows, bool f64);
+// launch of a system-major plan (pent_solve_chunked_rows.cu: the LM = 2, 3, 4 instantiations of the kernel)
+int launch_plan_rows(const pent_handle* h, const ChunkPlan& pl, int64_t M, const void* f, void* x, cudaStream_t s);
+// rank-2 tensor map {N, M} of a system-major batch with box {128 bytes, S} and SWIZZLE_128B
+bool encode_rows_map_cached(CUtensorMap* tm, const void* base, int64_t M, int N, int S, bool f64);
 
 }  // namespace pent

@@ -38,26 +38,46 @@ struct ChunkParams {
                       // every thread loads its rows with coalesced LDG instead (no landing buffer, nbox = 0)
                       // 2: SYSTEM-MAJOR batch ("one system per row", the paper's serial layout):
                       // element k of system i at f[i*N + k]; a thread's chunk is one contiguous run of C
-                      // elements, loaded and stored with 16-byte vector accesses
+                      // elements, loaded and stored with 32-byte vector accesses
+                      // 3: system-major batch through TMA: the tensor map is {N, M} with 128-byte x S boxes and
+                      // SWIZZLE_128B, so the global side moves whole 128-byte pieces of every system (prefetched one
+                      // tile ahead like the interleaved loader) and a thread reads its run out of the swizzled
+                      // landing buffer with conflict-free LDS.128; stores as in mode 2
+                      // 5: system-major batch through 1-D bulk copies (cp.async.bulk, UBLKCP): ONE copy per system and tile
+                      // moves that system's whole run of this CTA's rows into a landing buffer whose per-system pitch is
+                      // padded by 16 bytes (conflict-free LDS.128); prefetched one tile ahead.  The tensor-tile TMA of
+                      // mode 3 is bound by its row rate (~8 ns per 128-byte row and SM, profiles/r02_rows_loader.md);
+                      // a 1-D bulk copy has no rows.  Stores as in mode 2.
+                      // 6: mode 5 with the stores through 1-D bulk copies too (x -> padded staging buffer -> one
+                      // copy per system): x leaves as whole lines instead of 32-byte sectors
     T* x;
 };
 
 // PER = true: the periodic (cyclic) solve fused into the kernel, see PeriodicCtx in pent_chunk_common.cuh.
 // BAND = 1: tridiagonal A (a == e == 0, cuThomasBatch's case): one-term recurrences, a 5-word
 // coefficient row instead of 9, scalar chunk states; same data movement.
-template <typename T, int S, bool CLUSTER, bool PER, int BAND>
+// LM = layout / loader mode, compile-time so that every instantiation carries only its own data path (a run-time
+// switch over all of them cost 80-120 bytes of register spills in every instance): 0 = interleaved batch (TMA, or
+// the LDG loader when prm.ldg == 1); 2, 3, 4 = system-major batch, the modes described at ChunkParams::ldg.
+template <typename T, int S, bool CLUSTER, bool PER, int BAND, int LM>
 __global__ void __launch_bounds__(CHUNK_MAX_THREADS, 1)
 solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T> prm,
-                     const __grid_constant__ PeriodicParams<T> pp)
+                     const __grid_constant__ PeriodicParams<T> pp, const __grid_constant__ CUtensorMap tmx)
 {
     static_assert(BAND == 2 || !PER, "the fused periodic tail is built on the pentadiagonal tables");
+    static_assert(LM == 0 || !PER, "periodic handles take interleaved batches only");
     constexpr int C = ChunkCfg<T>::C, BL = chunk_block_len<T, BAND>();
     using T2 = typename Pair<T>::type;
     using ST = typename ChunkState<T, BAND>::type;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int P = prm.P;
-    T* landing = reinterpret_cast<T*>(smem_raw);
-    T* table = landing + (size_t)prm.nbox * prm.box_rows * S;
+    // (mode 3: the 128-byte swizzle pattern repeats every 1024 bytes of the shared-memory ADDRESS)
+    T* landing = reinterpret_cast<T*>(LM == 3 ? smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u) : smem_raw);
+    // modes 5, 6: one padded run per system (pitch in bytes); mode 6: a staging buffer of the same size and layout
+    const uint32_t run_pitch = (uint32_t)(prm.box_rows * sizeof(T)) + 16u;
+    const size_t tile_elems = LM >= 5 ? (size_t)S * run_pitch / sizeof(T) : (size_t)prm.nbox * prm.box_rows * S;
+    T* staging = landing + tile_elems;
+    T* table = staging + (LM == 6 ? tile_elems : 0);
     // chunk states [P][S]: E~ then F_{p-1};  S^ then B_{p+1}
     ST* stE = reinterpret_cast<ST*>(reinterpret_cast<unsigned char*>(table) + prm.table_bytes);
     ST* stS = stE + (size_t)S * P;
@@ -84,6 +104,32 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
     const int64_t stride = CLUSTER ? (int64_t)__clusterGridDimInClusters().x : (int64_t)gridDim.x;
     const int64_t first = CLUSTER ? (int64_t)__clusterIdx().x : (int64_t)blockIdx.x;
 
+    // TMA load(s) of barrier group b (box_rows rows x S systems) of tile t, signalling bars[1 + b]
+    auto issue_box = [&](int b, int64_t t) {
+        if constexpr (LM >= 5) {
+            // one 1-D bulk copy per system of the tile: its run of this CTA's rows (b == 0: a single barrier group)
+            int vr = prm.N - row_base;
+            vr = vr < 0 ? 0 : (vr > prm.box_rows ? prm.box_rows : vr);
+            const uint32_t bytes = (uint32_t)(vr * sizeof(T));
+            int64_t nsys = prm.M - t * S;
+            nsys = nsys > S ? S : nsys;
+            mbar_expect_tx(&bars[1 + b], bytes * (uint32_t)nsys);
+            if (bytes)
+                for (int is = 0; is < (int)nsys; ++is)
+                    bulk_load_1d(reinterpret_cast<unsigned char*>(landing) + (size_t)is * run_pitch,
+                                 prm.f + (t * S + is) * (int64_t)prm.N + row_base, bytes, &bars[1 + b]);
+        } else if constexpr (LM == 3) {
+            mbar_expect_tx(&bars[1 + b], box_bytes);
+            // system-major batch: tensor {N, M}, boxes of 128 bytes (W rows) x S systems, laid out [sub-box][S][128 B]
+            constexpr int W = 128 / (int)sizeof(T);
+            for (int sb = 0; sb < prm.box_rows / W; ++sb)
+                tma_load_2d(landing + ((size_t)b * prm.box_rows + (size_t)sb * W) * S, &tm,
+                            row_base + b * prm.box_rows + sb * W, (int)(t * S), &bars[1 + b]);
+        } else {
+            mbar_expect_tx(&bars[1 + b], box_bytes);
+            tma_load_2d(landing + (size_t)b * prm.box_rows * S, &tm, (int)(t * S), row_base + b * prm.box_rows, &bars[1 + b]);
+        }
+    };
     if (tid == 0) {
         for (int b = 0; b <= MAX_BOXES; ++b) mbar_init(&bars[b], 1);
         for (int b = 0; b < MAX_BOXES; ++b)
@@ -91,6 +137,12 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
         mbar_init(&bars[BAR_F], 1);
         mbar_init(&bars[BAR_B], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    if constexpr (LM >= 5) {
+        // rows >= N of the last rank and systems >= M of the last tile are never copied: give those slots finite
+        // contents once (their coefficients are zero, their results are never stored; 0 * NaN would still poison a run)
+        for (size_t w = tid; w < (LM == 6 ? 2 : 1) * tile_elems; w += blockDim.x) landing[w] = (T)0;
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
     __syncthreads();
@@ -111,11 +163,7 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
 #endif
     if (tid == 0) {
         if (tile < prm.ntiles)
-            for (int b = 0; b < prm.nbox; ++b) {
-                mbar_expect_tx(&bars[1 + b], box_bytes);
-                tma_load_2d(landing + (size_t)b * prm.box_rows * S, &tm, (int)(tile * S),
-                            row_base + b * prm.box_rows, &bars[1 + b]);
-            }
+            for (int b = 0; b < prm.nbox; ++b) issue_box(b, tile);
     }
     // every CTA of the cluster is resident, with its mbarriers initialised, before any DSMEM store
     if constexpr (CLUSTER) cluster_sync_all();
@@ -167,7 +215,36 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
             }
         }
         if (active) {
-            if (!PER && prm.ldg == 2) {
+            if constexpr (LM >= 5) {
+                // ---- system-major batch, padded per-system runs: this thread's chunk is C consecutive elements ----
+                mbar_wait(&bars[1 + mybox], parity);
+                constexpr int V = 16 / (int)sizeof(T);
+                const T* src = reinterpret_cast<const T*>(reinterpret_cast<const unsigned char*>(landing) + (size_t)i * run_pitch) + p * C;
+#pragma unroll
+                for (int c = 0; c < C / V; ++c) {
+                    T w[V];
+                    lds_vec<T, V>(w, src + c * V);
+#pragma unroll
+                    for (int u = 0; u < V; ++u) v[c * V + u] = w[u];
+                }
+            } else if constexpr (LM == 3) {
+                // ---- system-major batch through the swizzled landing buffer: rows [16-byte chunk c of the 128-byte
+                // piece `sb` of system i] sit at chunk c ^ (i & 7) of smem row (sb * S + i) ----
+                mbar_wait(&bars[1 + mybox], parity);
+                constexpr int W = 128 / (int)sizeof(T), V = 16 / (int)sizeof(T);
+                const unsigned char* base = reinterpret_cast<const unsigned char*>(landing) +
+                                            ((size_t)(p * C / W) * S + i) * 128;
+#pragma unroll
+                for (int sb = 0; sb < C / W; ++sb) {
+#pragma unroll
+                    for (int c = 0; c < 8; ++c) {
+                        T w[V];
+                        lds_vec<T, V>(w, reinterpret_cast<const T*>(base + (size_t)sb * S * 128 + ((c ^ (i & 7)) << 4)));
+#pragma unroll
+                        for (int u = 0; u < V; ++u) v[sb * W + c * V + u] = w[u];
+                    }
+                }
+            } else if constexpr (LM == 2) {
                 // ---- system-major batch: this thread's chunk is contiguous in memory ----
                 const int64_t col = tile * S + i;
                 const T* src = prm.f + col * (int64_t)prm.N + row0;
@@ -204,7 +281,7 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
         // warp arrives on the box's "empty" barrier and thread 0 re-arms it with the NEXT tile's
         // TMA load, which then runs under all of this tile's arithmetic and stores.
         __syncwarp();
-        if (lane == 0 && warp * 32 < P * S && !prm.ldg) mbar_arrive(&bars[1 + MAX_BOXES + mybox]);
+        if (lane == 0 && warp * 32 < P * S && (LM >= 3 || (LM == 0 && !prm.ldg))) mbar_arrive(&bars[1 + MAX_BOXES + mybox]);
         if constexpr (CLUSTER) {
             if (tid == 0) {        // arm this tile's aggregate barriers (complete_tx may already have arrived)
                 if (agg_bytes_f) mbar_expect_tx(&bars[BAR_F], agg_bytes_f);
@@ -214,9 +291,7 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
         if (tid == 0 && next_tile < prm.ntiles) {
             for (int b = 0; b < prm.nbox; ++b) {
                 mbar_wait(&bars[1 + MAX_BOXES + b], parity);
-                mbar_expect_tx(&bars[1 + b], box_bytes);
-                tma_load_2d(landing + (size_t)b * prm.box_rows * S, &tm, (int)(next_tile * S),
-                            row_base + b * prm.box_rows, &bars[1 + b]);
+                issue_box(b, next_tile);
             }
         }
         if (active) {
@@ -262,6 +337,9 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
                                                   aggF, aggB, bars, agg_bytes_f, agg_bytes_b, parity);
             }
         }
+        if constexpr (LM == 6) {      // the staging buffer may be overwritten once the previous tile's copies have read it
+            if (tid < S) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+        }
         __syncthreads();
 
         // ---- 4. correction and store ----
@@ -278,7 +356,30 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
             };
             const int64_t col = tile * S + i;
             T* xo = prm.x + (int64_t)row0 * prm.M + col;
-            if (!PER && prm.ldg == 2) {
+            if constexpr (LM == 6) {
+                // system-major batch, stores through bulk copies: x -> padded staging buffer (the previous tile's copies
+                // have read it: the issuing threads waited before the barrier that precedes this stage)
+                constexpr int V = 16 / (int)sizeof(T);
+                T* dst = reinterpret_cast<T*>(reinterpret_cast<unsigned char*>(staging) + (size_t)i * run_pitch) + p * C;
+#pragma unroll
+                for (int jg = 0; jg < C / 4; ++jg) {
+                    T xv[4];
+                    correct4(xv, jg);
+#pragma unroll
+                    for (int u = 0; u < 4 / V; ++u) {
+                        uint4 q;
+                        if constexpr (sizeof(T) == 8) {
+                            q.x = (uint32_t)__double2loint(xv[2 * u]); q.y = (uint32_t)__double2hiint(xv[2 * u]);
+                            q.z = (uint32_t)__double2loint(xv[2 * u + 1]); q.w = (uint32_t)__double2hiint(xv[2 * u + 1]);
+                        } else {
+                            q.x = __float_as_uint(xv[0]); q.y = __float_as_uint(xv[1]);
+                            q.z = __float_as_uint(xv[2]); q.w = __float_as_uint(xv[3]);
+                        }
+                        *reinterpret_cast<uint4*>(dst + 4 * jg + u * V) = q;
+                    }
+                }
+            }
+            if constexpr (LM == 2 || LM == 3 || LM == 5) {
                 // system-major batch: contiguous run of this thread's chunk, 32-byte stores where possible
                 T* xr = prm.x + col * (int64_t)prm.N + row0;
                 const int nrows = col < prm.M ? prm.N - row0 : 0;
@@ -303,7 +404,7 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
             T t0 = 0, t1 = 0;         // periodic: x^ = y - Z t
             if constexpr (PER) { T2 t = stT[i]; t0 = t.x; t1 = t.y; }
             const T2* zr = zs + (size_t)(active ? p : 0) * C;
-            if (!PER && prm.ldg == 2) {
+            if constexpr (LM >= 2) {
                 // stored above
             } else if (rows_full && (tile + 1) * S <= prm.M) {
 #pragma unroll
@@ -335,8 +436,26 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
                 }
             }
         }
+        if constexpr (LM == 6) {
+            // every thread's x is in the staging buffer: generic-proxy writes -> async proxy, block barrier, then thread
+            // `is` < S issues the ONE bulk copy of system `is` (rows >= N and systems >= M are not stored)
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            __syncthreads();
+            if (tid < S && tile * S + tid < prm.M) {
+                int vr = prm.N - row_base;
+                vr = vr < 0 ? 0 : (vr > prm.box_rows ? prm.box_rows : vr);
+                if (vr > 0) {
+                    const unsigned char* src = reinterpret_cast<const unsigned char*>(staging) + (size_t)tid * run_pitch;
+                    T* dst = prm.x + (tile * S + tid) * (int64_t)prm.N + row_base;
+                    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
+                                 ::"l"((uint64_t)dst), "r"(smem_u32(src)), "r"((uint32_t)(vr * sizeof(T))) : "memory");
+                }
+                asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+            }
+        }
         parity ^= 1;
         ++tcount;
     }
+    if constexpr (LM == 6) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
     if constexpr (CLUSTER) cluster_sync_all();   // no CTA leaves while a peer may still address its shared memory
 }

@@ -18,7 +18,7 @@ inline size_t periodic_extra_smem(const ChunkPlan& pl)
     return ((size_t)pl.Pl * ChunkCfg<T>::C + 5 * (size_t)pl.S + (pl.Q > 1 ? (size_t)pl.Q * pl.S : 0)) * 2 * sizeof(T);   // + second aggregate array
 }
 
-template <typename T, int S, bool CLUSTER, bool PER, int BAND = 2>
+template <typename T, int S, bool CLUSTER, bool PER, int BAND = 2, int LM = 0>
 static int launch_inst(const pent_handle* h, const ChunkPlan& pl, int64_t M, const void* f, void* x,
                        cudaStream_t s, const PeriodicParams<T>* per)
 {
@@ -40,10 +40,14 @@ static int launch_inst(const pent_handle* h, const ChunkPlan& pl, int64_t M, con
     prm.table_bytes = (uint32_t)pl.table_bytes;
     prm.x = (T*)x;
     prm.f = (const T*)f;
-    prm.ldg = pl.rows ? 2 : (pl.ldg ? 1 : 0);
+    prm.ldg = pl.mode;
 
     CUtensorMap tm = {};
-    if (!pl.ldg && !encode_batch_map_cached(&tm, f, M, h->N, S, prm.box_rows, sizeof(T) == 8)) {
+    const bool enc_ok = pl.mode == 0 ? encode_batch_map_cached(&tm, f, M, h->N, S, prm.box_rows, sizeof(T) == 8)
+                      : pl.mode == 3 ? encode_rows_map_cached(&tm, f, M, h->N, S, sizeof(T) == 8) : true;
+    CUtensorMap tmx = {};            // (second map: unused since the stores of the system-major modes are bulk copies)
+    const bool encx_ok = true;
+    if (!enc_ok || !encx_ok) {
         g_last_cuda_error = (int)cudaErrorInvalidValue;
         return PENT_ERR_CUDA;
     }
@@ -51,7 +55,8 @@ static int launch_inst(const pent_handle* h, const ChunkPlan& pl, int64_t M, con
     PeriodicParams<T> pp = {};
     if (PER) pp = *per;
     const size_t smem_total = pl.smem + (PER ? periodic_extra_smem<T>(pl) : 0);
-    auto kern = solve_chunked_kernel<T, S, CLUSTER, PER, BAND>;
+    if ((LM == 0) != (pl.mode <= 1) || (LM != 0 && LM != pl.mode)) return PENT_ERR_ARG;
+    auto kern = solve_chunked_kernel<T, S, CLUSTER, PER, BAND, LM>;
     static SmemOnce mark;
     PENT_CUDA(ensure_dynamic_smem(mark, kern, smem_total));
     // the occupancy answer depends only on (device, threads, shared memory, cluster size): keep the last
@@ -82,9 +87,9 @@ static int launch_inst(const pent_handle* h, const ChunkPlan& pl, int64_t M, con
         at[0].val.programmaticStreamSerializationAllowed = 1;
         cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)pl.threads);
         cfg.dynamicSmemBytes = smem_total; cfg.stream = s; cfg.attrs = at; cfg.numAttrs = 1;
-        PENT_CUDA(cudaLaunchKernelEx(&cfg, kern, tm, prm, pp));
+        PENT_CUDA(cudaLaunchKernelEx(&cfg, kern, tm, prm, pp, tmx));
 #else
-        kern<<<(unsigned)grid, pl.threads, smem_total, s>>>(tm, prm, pp);
+        kern<<<(unsigned)grid, pl.threads, smem_total, s>>>(tm, prm, pp, tmx);
 #endif
     } else {
         cudaLaunchConfig_t cfg = {};
@@ -106,7 +111,7 @@ static int launch_inst(const pent_handle* h, const ChunkPlan& pl, int64_t M, con
         int64_t clusters = oc.resident;
         if (clusters > prm.ntiles) clusters = prm.ntiles;
         cfg.gridDim = dim3((unsigned)(clusters * pl.Q));
-        PENT_CUDA(cudaLaunchKernelEx(&cfg, kern, tm, prm, pp));
+        PENT_CUDA(cudaLaunchKernelEx(&cfg, kern, tm, prm, pp, tmx));
     }
     count_launch();
     PENT_LAUNCH_CHECK();

@@ -136,7 +136,8 @@ int launch_solve_chunked_periodic(const pent_handle* h, int64_t M, const void* f
 int solve_periodic(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s, int kernel);
 int step_periodic(const pent_handle* h, int64_t M, void* c, void* scratch, int nsteps, cudaStream_t s);
 bool chunked_rows_supported(const pent_handle* h, int64_t M);
-int launch_solve_chunked_rows(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s);
+int launch_solve_chunked_rows(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s,
+                              int Q = 0, int S = 0, int loader = 0);
 int chunked_choice(const pent_handle* h, int64_t M, int* Q, int* S);   // 1 and the default plan, or 0
 
 }  // namespace pent

@@ -397,6 +397,7 @@ ChunkPlan make_plan(const pent_handle* h, int64_t M, const void* f, int Q, int S
     pl.table_bytes = (pl.table_bytes + 15) & ~(size_t)15;     // cp.async.bulk moves multiples of 16 bytes (the
                                                               // scalar W entries of BAND = 1 need not end on one)
     pl.ldg = ldg;
+    pl.mode = ldg ? 1 : 0;
     if (ldg) pl.nbox = 0;                                    // no landing buffer
     const size_t st = band == 2 ? 2 : 1;                     // words per chunk state
     pl.smem = (size_t)pl.nbox * pl.box_rows * S * esz + pl.table_bytes + (size_t)2 * st * pl.Pl * S * esz +
@@ -520,35 +521,119 @@ int chunked_choice(const pent_handle* h, int64_t M, int* Q, int* S)
     return 1;
 }
 
-// System-major batch (element k of system i at f[i*N + k]): the chunked kernel with its per-thread
-// contiguous loader.  CTAs of <= 256 threads are preferred (no prefetch: two CTAs per SM overlap).
-static ChunkPlan rows_plan(const pent_handle* h, int64_t M)
+// System-major batch (element k of system i at f[i*N + k]).  Default loader: TMA over the tensor {N, M} with
+// 128-byte x S boxes and SWIZZLE_128B (ChunkParams::ldg = 3), prefetched one tile ahead exactly like the
+// interleaved loader, so the shapes follow chunk_auto_plan.  When TMA cannot address the batch (row pitch
+// N*sizeof(T) or base not 16-byte aligned), or on request: the per-thread contiguous LDG.256 loader
+// (ldg = 2; no prefetch, so CTAs of <= 256 threads are preferred: two per SM overlap).
+bool encode_rows_map_cached(CUtensorMap* tm, const void* base, int64_t M, int N, int S, bool f64)
 {
-    if (!h || h->kind != 0 || h->periodic) return ChunkPlan{};
-    const int hb = h->band == 1 ? 1 : 2;
-    const int Sn = h->dtype == PENT_F64 ? 16 : 32, QMAX = 1 << (PENT_NQ - 1);
-    ChunkPlan best;
-    for (int Q = 1; Q <= QMAX && !best.ok; Q *= 2) {
-        ChunkPlan pl = make_plan(h, M, nullptr, Q, Sn, false, true, hb);
-        if (pl.ok && pl.threads <= 256) best = pl;
+    struct Key { const void* base; int64_t M; int N, S, f64; };
+    struct Cache { Key key[8]; CUtensorMap tm[8]; int n = 0, next = 0; };
+    static thread_local Cache c;
+    for (int j = 0; j < c.n; ++j) {
+        const Key& k = c.key[j];
+        if (k.base == base && k.M == M && k.N == N && k.S == S && k.f64 == (int)f64) { *tm = c.tm[j]; return true; }
     }
-    for (int Q = 1; Q <= QMAX && !best.ok; Q *= 2) {
-        ChunkPlan pl = make_plan(h, M, nullptr, Q, Sn, false, true, hb);
-        if (pl.ok) best = pl;
-    }
-    best.rows = best.ok;
-    return best;
+    EncodeTiledFn enc = encode_fn();
+    if (!enc) return false;
+    const size_t esz = f64 ? 8 : 4;
+    cuuint64_t gdim[2] = {(cuuint64_t)N, (cuuint64_t)M};
+    cuuint64_t gstr[1] = {(cuuint64_t)N * esz};
+    cuuint32_t box[2] = {(cuuint32_t)(128 / esz), (cuuint32_t)S};
+    cuuint32_t estr[2] = {1, 1};
+    if (enc(tm, f64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<void*>(base),
+            gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, PENT_L2_PROMOTION,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return false;
+    const int j = c.next;
+    c.key[j] = Key{base, M, N, S, (int)f64};
+    c.tm[j] = *tm;
+    c.next = (c.next + 1) & 7;
+    if (c.n < 8) ++c.n;
+    return true;
 }
 
-bool chunked_rows_supported(const pent_handle* h, int64_t M) { return rows_plan(h, M).ok; }
+// geometry of shape (Q, S) for a system-major batch in loader mode 2, 3, 5 or 6 (ChunkParams::ldg)
+static ChunkPlan rows_shape(const pent_handle* h, int64_t M, const void* f, const void* x, int Q, int S, int mode)
+{
+    const int hb = h->band == 1 ? 1 : 2;
+    ChunkPlan pl = make_plan(h, M, nullptr, Q, S, false, true, hb);          // no landing buffer yet
+    if (!pl.ok) return pl;
+    pl.rows = true;
+    pl.mode = 2;
+    if (mode == 2) return pl;
+    const size_t esz = h->dtype == PENT_F64 ? 8 : 4;
+    const int C = h->dtype == PENT_F64 ? ChunkCfg<double>::C : ChunkCfg<float>::C;
+    pl.ok = false;
+    // TMA and bulk copies address 16-byte aligned runs only
+    if (((size_t)h->N * esz) % 16 != 0 || (f && ((uintptr_t)f % 16) != 0) || M > (int64_t)0x7fffffff) return pl;
+    size_t tile_bytes;
+    if (mode == 3) {                  // swizzled tensor-tile TMA: barrier groups of <= 256 rows, 1 KiB alignment slack
+        if (!encode_fn()) return pl;
+        pl.nbox = (pl.Pl * C + pl.box_rows - 1) / pl.box_rows;
+        tile_bytes = (size_t)pl.nbox * pl.box_rows * S * esz + 1024;
+    } else {                          // 1-D bulk copies: one padded run per system, one barrier group
+        if (mode == 6 && x && ((uintptr_t)x % 16) != 0) return pl;
+        pl.nbox = 1;
+        pl.box_rows = pl.Pl * C;
+        tile_bytes = (size_t)S * ((size_t)pl.box_rows * esz + 16);
+    }
+    pl.smem += tile_bytes * (mode == 6 ? 2 : 1);
+    if (pl.smem > SMEM_LIMIT) return pl;
+    pl.ldg = false;
+    pl.mode = mode;
+    pl.ok = true;
+    return pl;
+}
+
+// loader: 0 = best available (bulk copies both ways, else bulk loads + STG.256 stores, else the LDG.256 loader),
+// 1 = LDG.256 loader, 2 = bulk loads + STG.256 stores, 3 = swizzled tensor-tile TMA loads + STG.256 stores (A/B)
+static ChunkPlan rows_plan(const pent_handle* h, int64_t M, const void* f, const void* x, int Q, int S, int loader)
+{
+    if (!h || h->kind != 0 || h->periodic) return ChunkPlan{};
+    const int Sn = h->dtype == PENT_F64 ? 16 : 32, Sw = 2 * Sn, QMAX = 1 << (PENT_NQ - 1);
+    const int want = loader == 1 ? 2 : loader == 2 ? 5 : loader == 3 ? 3 : 6;
+    if (Q && S) {
+        for (int mode : {want, 5, 2}) {
+            if (mode > want && want != 6) continue;
+            ChunkPlan pl = rows_shape(h, M, f, x, Q, S, mode);
+            if (pl.ok) return pl;
+        }
+        return ChunkPlan{};
+    }
+    if (want != 2) {
+        // Smallest cluster first: a bulk copy then moves the longest contiguous run of a system, which is what the
+        // measured sweep rewards (profiles/r02_rows_loader.md: cfg3 shape Q=1 0.71, Q=2 0.59, Q=4 0.58 of the HBM peak).
+        // Within a cluster size: the wanted mode before its fall-back (bulk loads + STG stores), wide tile first.
+        for (int q = 1; q <= QMAX; q *= 2)
+            for (int pass = 0; pass < 2; ++pass) {
+                if (pass == 1 && want != 6) break;
+                const int mode = pass == 0 ? want : 5;
+                for (int s_ : {Sw, Sn}) { ChunkPlan pl = rows_shape(h, M, f, x, q, s_, mode); if (pl.ok) return pl; }
+            }
+    }
+    for (int q = 1; q <= QMAX; q *= 2) {
+        ChunkPlan pl = rows_shape(h, M, f, x, q, Sn, 2);
+        if (pl.ok && pl.threads <= 256) return pl;
+    }
+    for (int q = 1; q <= QMAX; q *= 2) {
+        ChunkPlan pl = rows_shape(h, M, f, x, q, Sn, 2);
+        if (pl.ok) return pl;
+    }
+    return ChunkPlan{};
+}
+
+bool chunked_rows_supported(const pent_handle* h, int64_t M) { return rows_plan(h, M, nullptr, nullptr, 0, 0, 0).ok; }
 
 static int launch_plan(const pent_handle* h, const ChunkPlan& pl, int64_t M, const void* f, void* x, cudaStream_t s);
 
-int launch_solve_chunked_rows(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s)
+int launch_solve_chunked_rows(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s,
+                              int Q, int S, int loader)
 {
-    const ChunkPlan pl = rows_plan(h, M);
+    const ChunkPlan pl = rows_plan(h, M, f, x, Q, S, loader);
     if (!pl.ok) return PENT_UNSUPPORTED;
-    return launch_plan(h, pl, M, f, x, s);
+    return launch_plan_rows(h, pl, M, f, x, s);
 }
 
 int launch_solve_chunked(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s,

@@ -38,12 +38,6 @@ struct StepChunkParams {
     double dt, t0;
 };
 
-__device__ __forceinline__ void tma_store_2d(const CUtensorMap* tm, int c0, int c1, const void* src)
-{
-    asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%1, %2}], [%3];"
-                 ::"l"((uint64_t)tm), "r"(c0), "r"(c1), "r"(smem_u32(src)) : "memory");
-}
-
 // Barrier of one thread group of a CTA (named barrier 1+g); the whole CTA when there is one group.
 template <int NG>
 __device__ __forceinline__ void group_sync(int g, int nthreads)

@@ -47,6 +47,12 @@ WORKLOADS = {
     "cfg3p": Workload("cfg3p", 1024, 65536, 10.0, "periodic", 8, "uniform", "periodic solve, N=1024, M=65536"),
     "cfg5b": Workload("cfg5b", 1024, 16384, float("nan"), "dirichlet", 6, "uniform",
                       "per-system sigma_i ~ U[0.1,10]"),
+    # cfg3's shape with a TRIDIAGONAL matrix (a = e = 0): A = I - sigma L, the second-order
+    # Crank-Nicolson heat matrix of cuThomasBatch's use case; runs the BAND = 1 instantiation
+    "cfg3t": Workload("cfg3t", 1024, 65536, 10.0, "tridiagonal", 9, "uniform", "tridiagonal, N=1024, M=65536"),
+    # 2-D ADI on a 4096 x 4096 field, heat equation with the Remark-3
+    # fourth-order matrices along both axes, dt/(24 dx^2) = sigma
+    "adi2d": Workload("adi2d", 4096, 4096, 40.0, "heat4", 10, "uniform", "Peaceman-Rachford ADI, 4096 x 4096 field"),
 }
 
 
@@ -73,6 +79,14 @@ def make_matrix(w: Workload, M: int | None = None, col0: int = 0):
     if w.bc == "periodic":
         from . import periodic_hyperdiffusion_diagonals
         return periodic_hyperdiffusion_diagonals(w.N, w.sigma)
+    if w.bc == "tridiagonal":          # I - sigma L (Dirichlet L): diag 1 + 2 sigma, off-diagonals -sigma
+        z = np.zeros(w.N)
+        b = np.full(w.N, -w.sigma); b[0] = 0.0
+        d = np.full(w.N, -w.sigma); d[-1] = 0.0
+        return z, b, np.full(w.N, 1.0 + 2.0 * w.sigma), d, z.copy()
+    if w.bc == "heat4":
+        from . import heat4_cn_diagonals
+        return heat4_cn_diagonals(w.N, w.sigma)
     return diagonals_I_plus_sigma_L2(w.N, w.sigma, w.bc)
 
 

@@ -509,3 +509,82 @@ def test_heat4_crank_nicolson_steps_on_chip():
     mu = 4.0 * np.sin(3 * np.pi / (2 * (N + 1))) ** 2
     lam = 1.0 + s_h * (mu * mu + 12.0 * mu)
     assert normwise(cg.numpy(), ((2.0 - lam) / lam) ** steps * c0) <= 1e-10
+
+
+# ---- system-major batches: both loaders (swizzled TMA = default, per-thread LDG.256) and explicit shapes ----
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("N,M,Q,S,ldg", [(1024, 2048 + 17, 2, 32, 0), (1024, 2048 + 17, 2, 32, 1), (1024, 333, 1, 16, 0),
+                                         (512, 1000, 1, 32, 0), (4096, 96, 4, 16, 0), (4096, 96, 8, 32, 0),
+                                         (1000, 130, 2, 16, 0), (2046, 65, 2, 16, 0), (64, 40, 1, 16, 0),
+                                         (1024, 512, 0, 0, 1), (8192, 40, 8, 16, 0), (1001, 64, 0, 0, 0),
+                                         (1024, 2048 + 17, 2, 16, 0), (1024, 2048 + 17, 4, 32, 0), (1024, 515, 2, 32, 2),
+                                         (1024, 515, 2, 32, 3), (4096, 100, 8, 16, 0), (1000, 130, 4, 16, 2), (1000, 130, 2, 16, 3),
+                                         (6, 5, 1, 16, 0), (2, 40, 1, 16, 0), (200, 1, 1, 16, 0), (1024, 515, 0, 0, 0)])
+def test_system_major_loaders_and_shapes(dtype, N, M, Q, S, ldg):
+    pent = _pent()
+    if dtype == torch.float32:
+        S *= 2
+    diags = pin.random_diag_dominant(610 + N, N)
+    f = pin.uniform_pm1(611 + N, 0, N, M)
+    h = pent.pent_factor(N, *(torch.tensor(v, dtype=dtype) for v in (diags[4], diags[2], diags[3], diags[0], diags[1])))
+    fg, xg = guarded(f.T, dtype), Guarded((M, N), dtype)
+    kern = (pent.KERNEL_CHUNKED_CFG(Q, S) if Q else 0) | {0: 0, 1: pent.ROWS_LDG, 2: pent.ROWS_STG, 3: pent.ROWS_TMA2D}[ldg]
+    pent.pent_solve_batch_rows(h, M, fg.t, xg.t, kernel=kern)
+    fg.check("(f rows)"); xg.check("(x rows)")
+    d64, f64, ref = oracle_for_dtype(diags, f, dtype)
+    tol_x, tol_r = TOL[dtype]
+    x = xg.numpy().T
+    assert normwise(x.astype(np.float64), ref) <= tol_x
+    assert residual(d64, np.ascontiguousarray(x), f64) <= tol_r
+    pent.pent_solve_batch_rows(h, M, fg.t, fg.t, kernel=kern)          # in place, bit-identical
+    fg.check("(in place rows)")
+    assert torch.equal(fg.t, xg.t)
+
+
+# ---- 2-D ADI time step (pent_adi_step_batch) ----
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("Nx,Ny,steps", [(512, 384, 3), (1024, 1024, 2), (200, 130, 4), (64, 48, 1)])
+def test_adi_steps_parity(dtype, Nx, Ny, steps):
+    pent = _pent()
+    hx_, hy_ = 1.0 / (Nx + 1), 1.0 / (Ny + 1)
+    dt = 2e-5
+    dgx = pin.heat4_cn_diagonals(Nx, dt / (24 * hx_ * hx_))
+    dgy = pin.heat4_cn_diagonals(Ny, dt / (24 * hy_ * hy_))
+    if dtype == torch.float32:
+        dgx = tuple(np.asarray(v, dtype=np.float32).astype(np.float64) for v in dgx)
+        dgy = tuple(np.asarray(v, dtype=np.float32).astype(np.float64) for v in dgy)
+    mk = lambda dg: pent.pent_factor(len(dg[2]), *(torch.tensor(v, dtype=dtype) for v in (dg[4], dg[2], dg[3], dg[0], dg[1])))
+    hx, hy = mk(dgx), mk(dgy)
+    u0 = pin.uniform_pm1(820, 0, Ny, Nx)
+    if dtype == torch.float32:
+        u0 = u0.astype(np.float32).astype(np.float64)
+    ug, sg = guarded(u0, dtype), Guarded((Ny, Nx), dtype)
+    pent.pent_adi_step_batch(hx, hy, ug.t, steps, scratch=sg.t)
+    ug.check("(u)"); sg.check("(scratch)")
+    ref = oracle.adi_steps(oracle.factor(*dgx), oracle.factor(*dgy), u0, steps, nthreads=8)
+    got = ug.numpy().astype(np.float64)
+    tol = (1e-11 if dtype == torch.float64 else 2e-5) * 2 * steps
+    assert np.max(np.abs(got - ref)) / np.max(np.abs(ref)) <= tol
+    # without a caller workspace
+    u2 = torch.tensor(u0, dtype=dtype, device="cuda")
+    pent.pent_adi_step_batch(hx, hy, u2, steps)
+    assert torch.equal(u2, ug.t)
+
+
+def test_adi_heat_equation_mode_decay():
+    """u = sin(pi x) sin(pi y) is an eigenmode of both Remark-3 matrices: after n ADI steps it is multiplied by the
+    product of the two Crank-Nicolson amplification factors to the n, which approximates exp(-2 pi^2 t)."""
+    pent = _pent()
+    Nx, Ny, steps, dt = 768, 512, 20, 1e-4
+    hx_, hy_ = 1.0 / (Nx + 1), 1.0 / (Ny + 1)
+    sx, sy = dt / (24 * hx_ * hx_), dt / (24 * hy_ * hy_)
+    dgx, dgy = pin.heat4_cn_diagonals(Nx, sx), pin.heat4_cn_diagonals(Ny, sy)
+    mk = lambda dg: pent.pent_factor(len(dg[2]), *(torch.tensor(v) for v in (dg[4], dg[2], dg[3], dg[0], dg[1])))
+    u0 = np.outer(np.sin(np.pi * np.arange(1, Ny + 1) * hy_), np.sin(np.pi * np.arange(1, Nx + 1) * hx_))
+    u = torch.tensor(u0, device="cuda")
+    pent.pent_adi_step_batch(mk(dgx), mk(dgy), u, steps)
+    mux, muy = 4 * np.sin(np.pi * hx_ / 2) ** 2, 4 * np.sin(np.pi * hy_ / 2) ** 2
+    lx, ly = 1 + sx * (mux * mux + 12 * mux), 1 + sy * (muy * muy + 12 * muy)
+    amp = ((2 - lx) / lx * (2 - ly) / ly) ** steps
+    assert np.max(np.abs(u.cpu().numpy() - amp * u0)) <= 1e-11
+    assert abs(amp - np.exp(-2 * np.pi ** 2 * steps * dt)) <= 1e-6
