@@ -229,6 +229,13 @@ int pent_handle_n(const pent_handle* h);                 /* N, or -1 */
 int pent_handle_dtype(const pent_handle* h);             /* pent_dtype, or -1 */
 int64_t pent_handle_m(const pent_handle* h);             /* M of a per-system handle, 0 for shared A, -1 for NULL */
 int pent_handle_device(const pent_handle* h);            /* CUDA device ordinal of the handle, or -1 */
+/* Stability figures of the chunked evaluation (host, 3 doubles): max |Phi|, |X|, |Psi| = the largest response of the
+ * forward recurrence, of its back substitution and of the backward recurrence to a unit incoming state inside one
+ * chunk of 32 (fp64) / 64 (fp32) rows.  The on-chip kernels restart their local sweeps from a zero state, so their
+ * intermediates (and rounding noise) exceed the serial sweep's by up to this factor; when it exceeds 1e6 (fp64) /
+ * 1e3 (fp32) PENT_KERNEL_AUTO runs the serial thread-per-system kernels instead (pent_solve_kernel_choice says so).
+ * SPD matrices I + sigma L^2: about 5 sqrt(sigma).  Shared-A handles (periodic: of the block E). */
+int pent_handle_growth(const pent_handle* h, double* out3);
 int pent_handle_band(const pent_handle* h);              /* shared A: 1 = tridiagonal (a == e == 0), 2 = pentadiagonal; -1 */
 /* Copies the fp64 factor arrays (N doubles each; any pointer may be NULL) to HOST memory:
  * eps, beta, alpha = bands of L, gamma, delta = bands of R (Eq. 13).  Shared-A only. */

@@ -96,6 +96,7 @@ def lib() -> C.CDLL:
     L.pent_handle_m.restype = i64
     L.pent_handle_device.argtypes = [vp]
     L.pent_handle_band.argtypes = [vp]
+    L.pent_handle_growth.argtypes = [vp, C.POINTER(C.c_double)]
     L.pent_release_thread_cache.argtypes = []
     L.pent_release_thread_cache.restype = None
     L.pent_handle_factors.argtypes = [vp] * 6
@@ -333,6 +334,13 @@ def pent_adi_step_batch(hx: Handle, hy: Handle, u: torch.Tensor, nsteps: int, sc
     _check(lib().pent_adi_step_batch(hx.ptr, hy.ptr, u.data_ptr(), 0 if scratch is None else scratch.data_ptr(),
                                      nsteps, _stream(stream)))
     return u
+
+
+def handle_growth(h: Handle):
+    """(max|Phi|, max|X|, max|Psi|) of pent_handle_growth: the stability figures of the chunked evaluation."""
+    out = (C.c_double * 3)()
+    _check(lib().pent_handle_growth(h.ptr, out))
+    return tuple(out)
 
 
 def launch_count(reset: bool = False) -> int:

@@ -562,6 +562,7 @@ struct ChunkPlan {
     int j = 0, Q = 1, S = 0, Pl = 0, Pw = 1, threads = 0, levels = 0, box_rows = 0, nbox = 0;
     bool ldg = false;          // LDG loader instead of TMA (pitch not a multiple of 16 bytes, or system-major batch)
     bool rows = false;         // system-major batch: implies ldg
+    int pace_ns = 0;           // ChunkParams::pace_ns
     int band = 2;              // 1: the tridiagonal instantiation and its tables (handle with a == e == 0)
     int mode = 0;              // ChunkParams::ldg: 0 TMA (interleaved), 1 LDG (interleaved), 2 LDG.256 (system-major),
                                // 3 swizzled TMA loads + STG.256 stores, 4 swizzled TMA loads AND stores (system-major)

@@ -34,6 +34,7 @@ struct ChunkParams {
     int64_t ntiles;
     const T* table;   // global coefficient tables (layout = shared-memory layout), one per rank
     const T* f;       // right-hand side (used by the LDG loader)
+    unsigned pace_ns; // sleep this long before the store stage (0: none)
     int ldg;          // 1: the pitch M*sizeof(T) is not a multiple of 16 bytes, so TMA cannot address the batch:
                       // every thread loads its rows with coalesced LDG instead (no landing buffer, nbox = 0)
                       // 2: SYSTEM-MAJOR batch ("one system per row", the paper's serial layout):
@@ -342,6 +343,11 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
         }
         __syncthreads();
 
+        // Pacing of the store burst (profiles/r02_pacing.md): the x stores of this tile and the TMA loads of the next
+        // one (in flight since the top of the loop) compete when they overlap in time; holding the stores back for a
+        // fixed time raised the tridiagonal kernel from 0.79 to 0.89 of the HBM peak.  (A run-time value from the
+        // constant bank: the fp64 cluster instantiation has no register to spare.)
+        if (prm.pace_ns) __nanosleep(prm.pace_ns);
         // ---- 4. correction and store ----
         if (active) {
             T F0 = 0, F1 = 0, B0 = 0, B1 = 0;

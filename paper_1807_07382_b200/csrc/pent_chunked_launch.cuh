@@ -2,6 +2,8 @@
 // (PER = false) and pent_solve_chunked_periodic.cu (PER = true) so that the two sets of template
 // instantiations compile in parallel.
 #pragma once
+#include <cstdio>
+#include <cstdlib>
 #include "pent_chunk_common.cuh"
 
 #ifndef PENT_PDL
@@ -41,6 +43,8 @@ static int launch_inst(const pent_handle* h, const ChunkPlan& pl, int64_t M, con
     prm.x = (T*)x;
     prm.f = (const T*)f;
     prm.ldg = pl.mode;
+    prm.pace_ns = (unsigned)pl.pace_ns;
+    if (const char* e = std::getenv("PENT_AB_PACE")) prm.pace_ns = (unsigned)std::atoi(e);      // measurement override (ns)
 
     CUtensorMap tm = {};
     const bool enc_ok = pl.mode == 0 ? encode_batch_map_cached(&tm, f, M, h->N, S, prm.box_rows, sizeof(T) == 8)

@@ -187,7 +187,7 @@ int factor_on_stream(int N, const void* const src[5], pent_dtype dtype, pent_han
     {   // tridiagonal matrix (a == e == 0 inside the matrix)?  cuThomasBatch's case
         bool tri = true;
         for (int k = 0; k < N && tri; ++k) tri = hostdg[k] == 0.0 && hostdg[4 * (size_t)N + k] == 0.0;
-        h->band = tri ? 1 : 2;
+        h->band = (tri && !std::getenv("PENT_AB_NO_TRI")) ? 1 : 2;   // A/B: run a tridiagonal A through the BAND = 2 kernel
     }
     rc = build_chunk_tables(h, s);
     if (rc != PENT_OK) return fail(rc);
@@ -237,6 +237,13 @@ extern "C" int pent_handle_n(const pent_handle* h) { return h ? h->N : -1; }
 extern "C" int pent_handle_dtype(const pent_handle* h) { return h ? (int)h->dtype : -1; }
 extern "C" int64_t pent_handle_m(const pent_handle* h) { return h ? h->M : -1; }
 extern "C" int pent_handle_device(const pent_handle* h) { return h ? h->device : -1; }
+extern "C" int pent_handle_growth(const pent_handle* h, double* out3)
+{
+    if (!h || h->kind != 0 || !out3) return PENT_ERR_ARG;
+    const pent_handle* g = h->periodic ? h->inner : h;
+    for (int j = 0; j < 3; ++j) out3[j] = g->growth[j];
+    return PENT_OK;
+}
 extern "C" int pent_handle_band(const pent_handle* h) { return (h && h->kind == 0) ? (h->periodic ? 2 : h->band) : -1; }
 
 extern "C" int pent_handle_factors(const pent_handle* h, double* eps, double* beta, double* alpha,

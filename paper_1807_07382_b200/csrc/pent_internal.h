@@ -18,6 +18,7 @@ struct pent_handle {
     // second-difference matrix L (what pent_step_batch(kind 0) requires of its handle); -1 otherwise
     int l2_bc;
     double l2_sigma;
+    double growth[3];    // shared A: max |Phi|, |X|, |Psi| inside a chunk (stability guard of the chunk stitching)
     int band;            // shared A: 1 if a == e == 0 inside the matrix (tridiagonal), else 2
     // ---- shared A, all device memory ----
     double* diag;        // 5*N: a,b,c,d,e widened to fp64, out-of-matrix entries zeroed
@@ -127,6 +128,7 @@ int launch_solve_tps(const pent_handle* h, int64_t M, const void* f, void* x, cu
 // Q = CTAs per cluster along k, S = systems per tile; 0 = choose (pent_solve_chunked.cu)
 int launch_solve_chunked(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s,
                          int Q, int S);
+bool chunk_stitching_stable(const pent_handle* h);
 bool chunked_supported(const pent_handle* h, int64_t M, const void* f /* may be null */, int Q, int S);
 bool step_chunked_supported(const pent_handle* h, int64_t M, const void* c /* may be null */);
 int launch_step_chunked(const pent_handle* h, const pent_step_params* p, const pent_forcing* g, int64_t M, void* c,

@@ -31,6 +31,7 @@
 //   aggregates through distributed shared memory (chunk_state_scan in pent_chunk_common.cuh).
 // This file: the tables (built once per handle and cluster size), the launch plans and dispatch.
 #include <cstdio>
+#include <cstring>
 #include "pent_chunked_launch.cuh"
 
 namespace pent {
@@ -43,7 +44,7 @@ namespace pent {
 template <typename T>
 __global__ void build_chunk_tables_kernel(int N, int Pl, int Q, const double* __restrict__ fac,
                                           T* __restrict__ tab, size_t tab_stride,
-                                          double* __restrict__ tmat)
+                                          double* __restrict__ tmat, unsigned long long* __restrict__ growth)
 {
     constexpr int C = ChunkCfg<T>::C;
     constexpr int BL = chunk_block_len<T>();
@@ -54,6 +55,7 @@ __global__ void build_chunk_tables_kernel(int N, int Pl, int Q, const double* __
     T* blk = tab + (size_t)(p / Pl) * tab_stride + (size_t)(p % Pl) * BL;
     const int s = p * C;
     double phi0[C], phi1[C];
+    double gphi = 0.0, gchi = 0.0, gpsi = 0.0;     // growth of the three responses inside this chunk (stability guard)
     // forward: coefficients and Phi
     double h0m2 = 1.0, h0m1 = 0.0, h1m2 = 0.0, h1m1 = 1.0;
     for (int j = 0; j < C; ++j) {
@@ -64,6 +66,7 @@ __global__ void build_chunk_tables_kernel(int N, int Pl, int Q, const double* __
         double h0 = -en * h0m2 - bn * h0m1;
         double h1 = -en * h1m2 - bn * h1m1;
         phi0[j] = h0; phi1[j] = h1;
+        gphi = fmax(gphi, fmax(fabs(h0), fabs(h1)));
         h0m2 = h0m1; h0m1 = h0; h1m2 = h1m1; h1m1 = h1;
     }
     double* cm = tmat + (size_t)p * 12;         // TPhi | TX | TPsi, fp64, for the product kernel
@@ -82,6 +85,8 @@ __global__ void build_chunk_tables_kernel(int N, int Pl, int Q, const double* __
         double q1 = -ga * q1p1 - de * q1p2;
         T* o = blk + 5 * C + 4 * j;
         o[0] = (T)x0; o[1] = (T)x1; o[2] = (T)q0; o[3] = (T)q1;
+        gchi = fmax(gchi, fmax(fabs(x0), fabs(x1)));
+        gpsi = fmax(gpsi, fmax(fabs(q0), fabs(q1)));
         if (j <= 1) {
             cm[4 + 2 * j] = x0; cm[5 + 2 * j] = x1;      // TX rows 0,1
             cm[8 + 2 * j] = q0; cm[9 + 2 * j] = q1;      // TPsi rows 0,1
@@ -90,6 +95,11 @@ __global__ void build_chunk_tables_kernel(int N, int Pl, int Q, const double* __
         q0p2 = q0p1; q0p1 = q0; q1p2 = q1p1; q1p1 = q1;
     }
     for (int j = 9 * C; j < BL; ++j) blk[j] = (T)0;
+    if (growth) {      // non-negative doubles order like their bit patterns; NaN (bits above +inf) wins, as it should
+        atomicMax(&growth[0], (unsigned long long)__double_as_longlong(gphi));
+        atomicMax(&growth[1], (unsigned long long)__double_as_longlong(gchi));
+        atomicMax(&growth[2], (unsigned long long)__double_as_longlong(gpsi));
+    }
 }
 
 __device__ inline void mat2_mul(double* o, const double* A, const double* B)     // o = A B (row-major 2x2)
@@ -291,9 +301,11 @@ static int build_tables_t(pent_handle* h, int j, cudaStream_t s)
     // temporaries are stream-ordered allocations on the factor's private stream (cudaFree would synchronise
     // the whole device)
     auto release = [&]() { if (tmat) cudaFreeAsync(tmat, s); if (lev) cudaFreeAsync(lev, s); };
+    // lev: 2 ints (levels) followed, 8-byte aligned, by 3 x 8 bytes (growth of Phi, X, Psi)
     cudaError_t le = cudaMallocAsync((void**)&tmat, sizeof(double) * 12 * Pl * Q, s);
-    if (le == cudaSuccess) le = cudaMallocAsync((void**)&lev, 2 * sizeof(int), s);
-    if (le == cudaSuccess) le = cudaMemsetAsync(lev, 0, 2 * sizeof(int), s);
+    if (le == cudaSuccess) le = cudaMallocAsync((void**)&lev, 32, s);
+    if (le == cudaSuccess) le = cudaMemsetAsync(lev, 0, 32, s);
+    unsigned long long* growth = (BAND == 2 && j == 0 && lev) ? reinterpret_cast<unsigned long long*>(lev + 2) : nullptr;
     if (le == cudaSuccess) le = cudaMemsetAsync(cfj, 0, tlen * Q * sizeof(T), s);
     if (le != cudaSuccess) {            // temporaries are released on every path; h->cf[j] belongs to the handle
         release();
@@ -302,7 +314,7 @@ static int build_tables_t(pent_handle* h, int j, cudaStream_t s)
     }
     const int tb = 32, nb = (Pl * Q + tb - 1) / tb;
     if constexpr (BAND == 2) {
-        build_chunk_tables_kernel<T><<<nb, tb, 0, s>>>(h->N, Pl, Q, h->fac, (T*)cfj, tlen, tmat);
+        build_chunk_tables_kernel<T><<<nb, tb, 0, s>>>(h->N, Pl, Q, h->fac, (T*)cfj, tlen, tmat, growth);
         build_chunk_products_kernel<T><<<Q, 32, 0, s>>>(Pl, Q, tmat, (T*)cfj, tlen, lev);
     } else {
         build_tri_tables_kernel<T><<<nb, tb, 0, s>>>(h->N, Pl, Q, h->fac, (T*)cfj, tlen, tmat);
@@ -310,11 +322,12 @@ static int build_tables_t(pent_handle* h, int j, cudaStream_t s)
     }
     count_launch(2);
     le = cudaGetLastError();
-    int hl[2] = {0, 0};
-    if (le == cudaSuccess) le = cudaMemcpyAsync(hl, lev, sizeof(hl), cudaMemcpyDeviceToHost, s);
+    int hl[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    if (le == cudaSuccess) le = cudaMemcpyAsync(hl, lev, 32, cudaMemcpyDeviceToHost, s);
     release();
     if (le == cudaSuccess) le = cudaStreamSynchronize(s);
     if (le != cudaSuccess) return cuda_fail(le);
+    if (growth) std::memcpy(h->growth, hl + 2, 3 * sizeof(double));
     if (BAND == 2) { h->cfP[j] = Pl; h->lev_f[j] = hl[0]; h->lev_b[j] = hl[1]; }
     else { h->lev_f1[j] = hl[0]; h->lev_b1[j] = hl[1]; }
     return PENT_OK;
@@ -458,20 +471,44 @@ bool encode_batch_map(CUtensorMap* tm, const void* base, int64_t M, int N, int S
 //     Q=2,S=32 vs 220 at Q=1,S=16; fp32 105.1 at Q=2,S=64 vs 111.5 at Q=1,S=32);
 //   * otherwise the smallest cluster with the narrow tile (cfg5a: 410.6 us at Q=4,S=16 vs 485 at
 //     Q=8,S=32: 8-CTA clusters leave SMs idle on the 16/18/20-SM GPCs).
+// Stability guard of the chunk stitching: the local sweeps restart from a zero state, so their
+// intermediates exceed the serial sweep's by up to G = max |Phi|, |X|, |Psi| (the responses of the two recurrences to
+// a unit incoming state inside one chunk, recorded at factor time), and the rounding noise of the result grows with
+// it.  For the SPD matrices I + sigma L^2 G ~ 5 sqrt(sigma) (cfg3: 4, cfg4: 430); a matrix whose recurrences are
+// unstable inside a chunk gives G ~ rho^C.  Above the bound PENT_KERNEL_AUTO uses the serial thread-per-system kernel.
+bool chunk_stitching_stable(const pent_handle* h)
+{
+    const double g = h->growth[0] > h->growth[1] ? (h->growth[0] > h->growth[2] ? h->growth[0] : h->growth[2])
+                                                 : (h->growth[1] > h->growth[2] ? h->growth[1] : h->growth[2]);
+    return g <= (h->dtype == PENT_F64 ? 1e6 : 1e3);          // NaN compares false
+}
+
 ChunkPlan chunk_auto_plan(const pent_handle* h, int64_t M, const void* f)
 {
     if (!h || h->kind != 0) return ChunkPlan{};
+    if (!chunk_stitching_stable(h)) return ChunkPlan{};
     const int hb = h->band == 1 ? 1 : 2;        // tridiagonal handle: the BAND = 1 instantiation
     const int Sn = h->dtype == PENT_F64 ? 16 : 32, Sw = 2 * Sn, QMAX = 1 << (PENT_NQ - 1);
+    // Store pacing of the BAND = 1 kernel (profiles/r02_pacing.md): with its shorter arithmetic the x stores of a tile
+    // run into the TMA loads of the next one; on the two cluster shapes below, holding the stores back ~1.5 us takes
+    // large batches from 0.79 / 0.72 to 0.89 / 0.83 of the HBM peak (N = 1024 / 4096), while it costs 5-10 % on the
+    // other shapes and on batches of a few tiles per cluster.  Measured heuristic, not a model.
+    auto paced = [&](ChunkPlan pl) {
+        const int64_t tiles_per_cluster = ((M + pl.S - 1) / pl.S) * pl.Q / 148;
+        if (pl.ok && pl.band == 1 && pl.mode == 0 && tiles_per_cluster >= 16 &&
+            ((pl.Q == 2 && pl.S == Sw) || (pl.Q == 4 && pl.S == Sn)))
+            pl.pace_ns = 1500;
+        return pl;
+    };
     ChunkPlan narrow1 = make_plan(h, M, f, 1, Sn, false, false, hb);
     if (narrow1.ok && narrow1.threads <= 256) return narrow1;
     for (int Q = 1; Q <= 4; Q *= 2) {
         ChunkPlan pl = make_plan(h, M, f, Q, Sw, false, false, hb);
-        if (pl.ok) return pl;
+        if (pl.ok) return paced(pl);
     }
     for (int Q = 1; Q <= QMAX; Q *= 2) {
         ChunkPlan pl = make_plan(h, M, f, Q, Sn, false, false, hb);
-        if (pl.ok) return pl;
+        if (pl.ok) return paced(pl);
     }
     for (int Q = 1; Q <= QMAX; Q *= 2) {
         ChunkPlan pl = make_plan(h, M, f, Q, Sw, false, false, hb);
@@ -594,6 +631,7 @@ static ChunkPlan rows_plan(const pent_handle* h, int64_t M, const void* f, const
     if (!h || h->kind != 0 || h->periodic) return ChunkPlan{};
     const int Sn = h->dtype == PENT_F64 ? 16 : 32, Sw = 2 * Sn, QMAX = 1 << (PENT_NQ - 1);
     const int want = loader == 1 ? 2 : loader == 2 ? 5 : loader == 3 ? 3 : 6;
+    if (!(Q && S) && !chunk_stitching_stable(h)) return ChunkPlan{};
     if (Q && S) {
         for (int mode : {want, 5, 2}) {
             if (mode > want && want != 6) continue;

@@ -345,7 +345,7 @@ static StepPlan step_plan(const pent_handle* h, int64_t M, const void* c, int S,
 // systems 20.2 us against 22.2 for one group of 32.
 static StepPlan step_auto_plan(const pent_handle* h, int64_t M, const void* c)
 {
-    if (!h) return StepPlan{};
+    if (!h || !chunk_stitching_stable(h)) return StepPlan{};
     if (h->dtype == PENT_F64) return step_plan(h, M, c, 16, 1);
     StepPlan two = step_plan(h, M, c, 16, 2);
     if (two.ok) return two;

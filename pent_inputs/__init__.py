@@ -212,6 +212,37 @@ def random_diag_dominant(seed: int, N: int, M: int | None = None):
     return a, b, c, d, e
 
 
+def spd_banded_product(seed: int, N: int, rho: float):
+    """Diagonals of A = B B^T, B lower banded with bandwidth 2 whose rows are ~(rho^2, -2 rho, 1) (jittered by
+    +-5 %): symmetric positive definite by construction, NOT diagonally dominant for rho > 0.3, with
+    cond(A) ~ (1 - rho)^-4.  PAPER.md:275-277 names SPD as one of the two classes the algorithm is stable for;
+    the I + sigma L^2 family and the diagonally dominant generator above cover only the other."""
+    j0 = 1.0 + 0.05 * uniform_pm1(seed, 31, N, 1)[:, 0]
+    j1 = 1.0 + 0.05 * uniform_pm1(seed, 32, N, 1)[:, 0]
+    j2 = 1.0 + 0.05 * uniform_pm1(seed, 33, N, 1)[:, 0]
+    b0, b1, b2 = j0, -2.0 * rho * j1, rho * rho * j2          # B[k][k], B[k][k-1], B[k][k-2]
+    b1[0] = 0.0
+    b2[:2] = 0.0
+    a = np.zeros(N); b = np.zeros(N); c = np.zeros(N); d = np.zeros(N); e = np.zeros(N)
+    c[:] = b0 * b0 + b1 * b1 + b2 * b2
+    b[1:] = b1[1:] * b0[:-1] + b2[1:] * b1[:-1]               # A[k][k-1] = B[k][k-1] B[k-1][k-1] + B[k][k-2] B[k-1][k-2]
+    a[2:] = b2[2:] * b0[:-2]                                  # A[k][k-2] = B[k][k-2] B[k-2][k-2]
+    d[:-1] = b[1:]
+    e[:-2] = a[2:]
+    return a, b, c, d, e
+
+
+def transpose_diagonals(a, b, c, d, e):
+    """Row-indexed diagonals of A^T (a column-diagonally-dominant matrix from a row-dominant one)."""
+    N = len(c)
+    at = np.zeros(N); bt = np.zeros(N); dt = np.zeros(N); et = np.zeros(N)
+    at[2:] = np.asarray(e)[:-2]
+    bt[1:] = np.asarray(d)[:-1]
+    dt[:-1] = np.asarray(b)[1:]
+    et[:-2] = np.asarray(a)[2:]
+    return at, bt, np.array(c, dtype=np.float64), dt, et
+
+
 # ----------------------------------------------------------------------------
 # periodic (cyclic) matrices, PAPER.md Eq. 7a-7b
 # ----------------------------------------------------------------------------

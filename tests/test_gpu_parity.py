@@ -588,3 +588,64 @@ def test_adi_heat_equation_mode_decay():
     amp = ((2 - lx) / lx * (2 - ly) / ly) ** steps
     assert np.max(np.abs(u.cpu().numpy() - amp * u0)) <= 1e-11
     assert abs(amp - np.exp(-2 * np.pi ** 2 * steps * dt)) <= 1e-6
+
+
+# ---- the other half of the paper's stability domain ("SPD or diagonally dominant"), and the guard ----
+@pytest.mark.parametrize("rho", [0.5, 0.8, 0.9, 0.93])
+@pytest.mark.parametrize("kernel", [0, 1])
+def test_spd_not_diagonally_dominant(rho, kernel):
+    """A = B B^T (SPD, not diagonally dominant, cond = 90 ... 1e8 at N = 1024).  Error against the long-double
+    truth; bar = 1e-11 or twice what plain fp64 CPU evaluations of the same solve leave (serial sweep; chunked order)."""
+    pent = _pent()
+    N, M = 1024, 256
+    diags = pin.spd_banded_product(40, N, rho)
+    f = pin.uniform_pm1(41, 0, N, M)
+    x, h = gpu_solve(diags, f, kernel=kernel)
+    fac = oracle.factor(*diags)
+    ref = oracle.solve_batch(fac, f, nthreads=8)
+    truth = oracle.ld_solve_batch(diags, f, nthreads=8)
+    evals = [ref] + ([chunked_order_solve_fp64(fac, f)] if kernel == 0 else [])
+    g = pent.handle_growth(h)
+    print(f"SPD rho={rho} kernel={kernel}: growth (Phi, X, Psi) = ({g[0]:.3g}, {g[1]:.3g}, {g[2]:.3g}); vs long double: "
+          f"GPU {normwise(x, truth):.3e}, " + ", ".join(f"fp64 CPU[{j}] {normwise(v, truth):.3e}" for j, v in enumerate(evals)))
+    assert normwise(x, truth) <= envelope_tol(1e-11, truth, *evals)
+
+
+def test_column_dominant_nonsymmetric():
+    N, M = 1000, 130
+    diags = pin.transpose_diagonals(*pin.random_diag_dominant(42, N))
+    A = pin.dense_from_diagonals(*diags)
+    assert not np.all(2 * np.abs(np.diag(A)) > np.abs(A).sum(axis=1))       # not ROW dominant
+    f = pin.uniform_pm1(43, 0, N, M)
+    for kernel in (0, 1):
+        x, _ = gpu_solve(diags, f, kernel=kernel)
+        assert normwise(x, oracle.solve_batch(oracle.factor(*diags), f)) <= 1e-11
+        assert residual(diags, x, f) <= 1e-12
+
+
+def test_stability_guard_routes_unstable_recurrences_to_the_serial_kernel():
+    """A = L R with beta/alpha = 1.6 in L: the forward recurrence grows like 1.6^k, 3.4e6 over one chunk of 32 rows.  The
+    handle reports it, PENT_KERNEL_AUTO then runs the serial sweep, and the result matches the oracle's evaluation."""
+    pent = _pent()
+    N, M = 256, 64
+    z = np.zeros(N)
+    b = np.full(N, 1.6); b[0] = 0.0
+    d = np.full(N, 0.3); d[-1] = 0.0
+    c = np.full(N, 1.0 + 1.6 * 0.3); c[0] = 1.0
+    diags = (z, b, c, d, z.copy())
+    fac = oracle.factor(*diags)
+    assert np.allclose(fac.alpha, 1.0) and np.allclose(fac.beta[1:], 1.6)
+    f = pin.uniform_pm1(44, 0, N, M)
+    x, h = gpu_solve(diags, f)
+    g = pent.handle_growth(h)
+    assert g[0] >= 1e6
+    assert pent.kernel_choice(h, M)["kernel"] == "solve_tps_kernel"
+    assert pent.lib().pent_step_kernel_choice(h.ptr, M) == pent.KERNEL_THREAD_PER_SYSTEM
+    ref = oracle.solve_batch(fac, f)
+    truth = oracle.ld_solve_batch(diags, f)
+    assert normwise(x, truth) <= pinned_tol(1e-11, ref, truth)
+    # the benchmark matrices are far from the bound: ~5 sqrt(sigma)
+    for sigma, bc, lo, hi in ((10.0, "dirichlet", 1.0, 10.0), (1e-2 * 1e-6 * 1024.0 ** 4, "zeroflux", 100.0, 1000.0)):
+        dg = pin.diagonals_I_plus_sigma_L2(1024, sigma, bc)
+        hh = pent.pent_factor(1024, *(torch.tensor(v) for v in (dg[4], dg[2], dg[3], dg[0], dg[1])))
+        assert lo <= max(pent.handle_growth(hh)) <= hi
