@@ -53,7 +53,55 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--suite", default="", metavar="OUT.jsonl",
+                    help="run every workload of SUITE (one bench.py process each, --steps/--warmup as given) and "
+                         "write their JSON lines, each with the command that made it, to OUT.jsonl")
     return ap.parse_args()
+
+
+# the workloads behind DESIGN.md section 10's table: (label, extra arguments)
+SUITE = [
+    ("cfg1", ["--workload", "cfg1"]),
+    ("cfg2", ["--workload", "cfg2"]),
+    ("cfg3 f64", ["--workload", "cfg3"]),
+    ("cfg3 f32", ["--workload", "cfg3", "--dtype", "f32"]),
+    ("cfg3 thread-per-system (the paper's design)", ["--workload", "cfg3", "--kernel", "1"]),
+    ("cfg3 odd M", ["--workload", "cfg3", "--systems", "65535"]),
+    ("cfg3t tridiagonal", ["--workload", "cfg3t"]),
+    ("cfg3p periodic", ["--workload", "cfg3p"]),
+    ("cfg5a", ["--workload", "cfg5a"]),
+    ("N=8192 M=16384", ["--workload", "cfg5a", "--rows-n", "8192", "--systems", "16384"]),
+    ("N=16384 M=8192", ["--workload", "cfg5a", "--rows-n", "16384", "--systems", "8192"]),
+    ("cfg3 rows", ["--workload", "cfg3", "--layout", "rows"]),
+    ("cfg5a rows", ["--workload", "cfg5a", "--layout", "rows"]),
+    ("cfg5b per-system", ["--workload", "cfg5b"]),
+    ("cfg5b per-system f32", ["--workload", "cfg5b", "--dtype", "f32"]),
+    ("cfg4 fused step", ["--workload", "cfg4", "--steps", "1000"]),
+    ("paper_hd", ["--workload", "paper_hd", "--steps", "250"]),
+    ("adi2d", ["--workload", "adi2d"]),
+]
+
+
+def run_suite(args):
+    import subprocess
+    out = []
+    for label, extra in SUITE:
+        cmd = [sys.executable, os.path.join(ROOT, "bench.py"), "--steps", str(args.steps), "--warmup", str(args.warmup),
+               "--no-e2e", "--no-cpu-baseline"] + extra
+        shown = "python bench.py " + " ".join(cmd[2:])
+        try:
+            r = subprocess.run(cmd, capture_output=True, text=True, timeout=900)
+            lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+            rec = json.loads(lines[-1]) if lines else {"error": (r.stderr or r.stdout)[-400:], "rc": r.returncode}
+        except Exception as ex:  # noqa: BLE001
+            rec = {"error": repr(ex)}
+        rec = {"label": label, "cmd": shown, **rec}
+        out.append(rec)
+        print(json.dumps({k: rec.get(k) for k in ("label", "ms_per_step", "value", "error")} |
+                         {"frac": (rec.get("roofline") or {}).get("frac")}), flush=True)
+    with open(args.suite, "w") as fh:
+        for rec in out:
+            fh.write(json.dumps(rec) + "\n")
 
 
 def measured_peak():
@@ -618,6 +666,8 @@ def run_per_system_workload(args, w, rank, world, local):
 
 def main():
     args = parse_args()
+    if args.suite:
+        return run_suite(args)
     if args.impl == "reference":
         run_reference(args)
     else:
