@@ -279,6 +279,97 @@ __device__ __forceinline__ void chunk_correct4(T (&out)[4], const T* v4, const T
         out[r] = fma(w[4 * r + 3], B1, fma(w[4 * r + 2], B0, fma(w[4 * r + 1], F1, fma(w[4 * r], F0, v4[r]))));
 }
 
+// ---- SPT systems per thread (register blocking over systems) ------------------------------------------------
+// A coefficient LDS.128 is a warp broadcast: it costs the shared-memory pipe the same whether the thread then
+// feeds one system's recurrence with it or several.  With one system per thread the coefficient broadcasts are
+// 13 of the ~15 shared-memory wavefronts per warp-row (profiles/r01_ncu_full.md: l1tex 72 %, the busiest unit of
+// the solve kernel, and THE bound of the on-chip step kernel); a thread that carries SPT adjacent systems through
+// the same chunk divides them by SPT (and gives the scheduler SPT independent FMA chains per warp).
+// v[u][j] = row j of the thread's u-th system.  Same arithmetic, same order, per system, as the SPT = 1 functions.
+template <typename T, int SPT>
+__device__ __forceinline__ void lds_sys(T (&o)[SPT], const T* p)
+{
+    if constexpr (SPT == 1) o[0] = *p;
+    else if constexpr (SPT * sizeof(T) == 8) {
+        const float2 q = *reinterpret_cast<const float2*>(p);
+        o[0] = q.x; o[1] = q.y;
+    } else {
+        static_assert((SPT * sizeof(T)) % 16 == 0, "systems per thread");
+        lds_vec<T, SPT>(o, p);
+    }
+}
+template <typename T, int SPT>
+__device__ __forceinline__ void sts_sys(T* p, const T (&o)[SPT])
+{
+    if constexpr (SPT == 1) *p = o[0];
+    else if constexpr (SPT * sizeof(T) == 8) *reinterpret_cast<float2*>(p) = make_float2(o[0], o[1]);
+    else {
+        static_assert(SPT * sizeof(T) == 16, "systems per thread");
+        if constexpr (sizeof(T) == 8) *reinterpret_cast<double2*>(p) = make_double2(o[0], o[1]);
+        else *reinterpret_cast<float4*>(p) = make_float4(o[0], o[1], o[2], o[3]);
+    }
+}
+
+template <typename T, int SPT>
+__device__ __forceinline__ void chunk_local_sweeps_n(T (&v)[SPT][ChunkCfg<T>::C], const T* blk,
+                                                     typename Pair<T>::type (&e)[SPT], typename Pair<T>::type (&s)[SPT])
+{
+    constexpr int C = ChunkCfg<T>::C;
+    T g1[SPT], g2[SPT];
+#pragma unroll
+    for (int u = 0; u < SPT; ++u) { g1[u] = 0; g2[u] = 0; }
+#pragma unroll
+    for (int jg = 0; jg < C / 4; ++jg) {
+        T w[12];
+        lds_vec<T, 12>(w, blk + 12 * jg);
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const int j = 4 * jg + r;
+#pragma unroll
+            for (int u = 0; u < SPT; ++u) {
+                T t = w[3 * r] * v[u][j];
+                t = fma(-w[3 * r + 1], g2[u], t);
+                T g = fma(-w[3 * r + 2], g1[u], t);
+                v[u][j] = g; g2[u] = g1[u]; g1[u] = g;
+            }
+        }
+    }
+    T x1[SPT], x2[SPT];
+#pragma unroll
+    for (int u = 0; u < SPT; ++u) { e[u].x = v[u][C - 2]; e[u].y = v[u][C - 1]; x1[u] = 0; x2[u] = 0; }
+#pragma unroll
+    for (int jg = C / 4 - 1; jg >= 0; --jg) {
+        T w[8];
+        lds_vec<T, 8>(w, blk + 3 * C + 8 * jg);
+#pragma unroll
+        for (int r = 3; r >= 0; --r) {
+            const int j = 4 * jg + r;
+#pragma unroll
+            for (int u = 0; u < SPT; ++u) {
+                T xv = fma(-w[2 * r], x1[u], fma(-w[2 * r + 1], x2[u], v[u][j]));
+                v[u][j] = xv; x2[u] = x1[u]; x1[u] = xv;
+            }
+        }
+    }
+#pragma unroll
+    for (int u = 0; u < SPT; ++u) { s[u].x = v[u][0]; s[u].y = v[u][1]; }
+}
+
+// stage 4, rows 4 jg .. 4 jg + 3 of every system of the thread: out[u][r]
+template <typename T, int SPT>
+__device__ __forceinline__ void chunk_correct4_n(T (&out)[SPT][4], const T (&v)[SPT][ChunkCfg<T>::C], const T* blk, int jg,
+                                                 const T (&F0)[SPT], const T (&F1)[SPT], const T (&B0)[SPT], const T (&B1)[SPT])
+{
+    constexpr int C = ChunkCfg<T>::C;
+    T w[16];
+    lds_vec<T, 16>(w, blk + 5 * C + 16 * jg);
+#pragma unroll
+    for (int r = 0; r < 4; ++r)
+#pragma unroll
+        for (int u = 0; u < SPT; ++u)
+            out[u][r] = fma(w[4 * r + 3], B1[u], fma(w[4 * r + 2], B0[u], fma(w[4 * r + 1], F1[u], fma(w[4 * r], F0[u], v[u][4 * jg + r]))));
+}
+
 // ---- BAND = 1: the same three stages for a tridiagonal A (one-term recurrences) -----------------
 // blk: [ {1/alpha, beta/alpha} x C | gamma x C | {chi, psi} x C ].  v: f -> x^ ; e = last g~ ; s = first x^.
 template <typename T>
@@ -377,6 +468,140 @@ struct PeriodicCtx {
 // PER: also computes t of the periodic reduction (PeriodicCtx) into per.stT[sys] and stores the two
 // tail rows of x; in a cluster every rank then receives every rank's backward aggregate (not only
 // the later ranks') plus (y_{n-2}, y_{n-1}) from rank ra, all under the same mbarrier phase.
+// ---- lean scan for the on-chip step kernel (single CTA, non-periodic) ------------------------------------------
+// In the step kernel the scan runs once per time step with the same lane -> chunk assignment, and it is a pure
+// latency chain (per level: 64-bit shuffles + two dependent FMAs), so everything that does not depend on the data
+// is taken off it (profiles/r02_step_spt.md: the branchy version below spent ~90 cycles per level on shared-memory
+// address arithmetic and reconvergence points; the scan was 37 % of a step):
+//   * the lane's base address and validity bits are computed ONCE per launch (ScanLane, made opaque so that the
+//     compiler does not rematerialise them from the block geometry inside every step); the per-level offsets are
+//     uniform and come from the constant bank (ScanOffsets);
+//   * a lane that takes no part in a level gets a ZERO matrix through a predicated load (inline PTX: the
+//     conditional expression compiled to a branch around the load), so a level is straight-line code;
+//   * R systems per lane (register blocking as in the sweeps): the matrices are loaded once for the R systems and
+//     their R shuffle -> FMA chains overlap.
+// Levels beyond lev_f / lev_b (matrices below 1e-25) are still skipped by a uniform branch.  What remains is bound by
+// the SHFL pipe (8 SHFL.32 per level and warp, all warps of the SM at once: ~150 cycles per level).
+struct ScanOffsets {                  // byte offsets, relative to W, of element e of the level-l matrices of lane q = 0
+    uint32_t f[W_LEVELS][4], b[W_LEVELS][4], tx[4];
+};
+template <typename T>
+inline ScanOffsets make_scan_offsets(int P, const int* woff)
+{
+    ScanOffsets o;
+    for (int l = 0; l < W_LEVELS; ++l) {
+        const int d = 1 << l, n = P - d > 0 ? P - d : 0;
+        for (int e = 0; e < 4; ++e) {
+            o.f[l][e] = (uint32_t)((woff[l] + e * n - d) * (int)sizeof(T));
+            o.b[l][e] = (uint32_t)((woff[l] + 4 * n + e * n) * (int)sizeof(T));
+        }
+    }
+    for (int e = 0; e < 4; ++e) o.tx[e] = (uint32_t)(e * P * (int)sizeof(T));
+    return o;
+}
+struct ScanLane {
+    uint32_t abase;                               // shared-memory byte address of W + q * sizeof(T)
+    uint32_t valid;                               // bit l: forward level l applies; bit 8 + l: backward; bit 16: q < P
+};
+template <typename T>
+__device__ __forceinline__ ScanLane make_scan_lane(const ScanGeom& g, const T* wtab, int q)
+{
+    ScanLane s;
+    const int P = g.P;
+    s.valid = q < P ? 1u << 16 : 0u;
+    s.abase = smem_u32(wtab) + (uint32_t)(q * (int)sizeof(T));
+#pragma unroll
+    for (int l = 0; l < W_LEVELS; ++l) {
+        const int d = 1 << l;
+        const bool vf = l < g.lev_f && q >= d && q < P, vb = l < g.lev_b && q + d <= P - 1;
+        s.valid |= (vf ? 1u : 0u) << l | (vb ? 1u : 0u) << (8 + l);
+    }
+    asm volatile("" : "+r"(s.abase), "+r"(s.valid));
+    return s;
+}
+// value at shared address `addr` if `on`, else 0: one predicated LDS, no branch
+__device__ __forceinline__ double lds_if(uint32_t addr, uint32_t on, double)
+{
+    double v;
+    asm("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\tmov.f64 %0, 0d0000000000000000;\n\t@p ld.shared.f64 %0, [%1];\n\t}"
+        : "=d"(v) : "r"(addr), "r"(on));
+    return v;
+}
+__device__ __forceinline__ float lds_if(uint32_t addr, uint32_t on, float)
+{
+    float v;
+    asm("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\tmov.f32 %0, 0f00000000;\n\t@p ld.shared.f32 %0, [%1];\n\t}"
+        : "=f"(v) : "r"(addr), "r"(on));
+    return v;
+}
+// In: stE[sl[r]] = E~_q, stS[sl[r]] = S^_q of the lane's R systems.  Out: F_{q-1}, B_{q+1} in the same slots.
+// sl[r] < 0: the lane has no r-th system (its states are zero and nothing is stored).
+template <typename T, int R>
+__device__ __forceinline__ void chunk_state_scan_lean(const ScanLane& ln, const ScanOffsets& so, int P, int Pw, int lev_f,
+                                                      int lev_b, int q, typename Pair<T>::type* stE,
+                                                      typename Pair<T>::type* stS, const int (&sl)[R])
+{
+    using T2 = typename Pair<T>::type;
+    T y0[R], y1[R], z0[R], z1[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        y0[r] = 0; y1[r] = 0; z0[r] = 0; z1[r] = 0;
+        if (sl[r] >= 0) { T2 e = stE[sl[r]]; y0[r] = e.x; y1[r] = e.y; T2 s = stS[sl[r]]; z0[r] = s.x; z1[r] = s.y; }
+    }
+#pragma unroll
+    for (int l = 0; l < W_LEVELS; ++l) {
+        if (l < lev_f) {
+            const int d = 1 << l;
+            const uint32_t on = ln.valid & (1u << l);
+            const T m0 = lds_if(ln.abase + so.f[l][0], on, T()), m1 = lds_if(ln.abase + so.f[l][1], on, T()),
+                    m2 = lds_if(ln.abase + so.f[l][2], on, T()), m3 = lds_if(ln.abase + so.f[l][3], on, T());
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const T u0 = shfl_up_t(y0[r], d, Pw), u1 = shfl_up_t(y1[r], d, Pw);
+                y0[r] = fma(m1, u1, fma(m0, u0, y0[r]));
+                y1[r] = fma(m3, u1, fma(m2, u0, y1[r]));
+            }
+        }
+    }
+    T f0[R], f1[R];
+    {
+        const uint32_t on = ln.valid & (1u << 16);
+        const T m0 = lds_if(ln.abase + so.tx[0], on, T()), m1 = lds_if(ln.abase + so.tx[1], on, T()),
+                m2 = lds_if(ln.abase + so.tx[2], on, T()), m3 = lds_if(ln.abase + so.tx[3], on, T());
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            f0[r] = shfl_up_t(y0[r], 1, Pw); f1[r] = shfl_up_t(y1[r], 1, Pw);      // F_{q-1}
+            if (q == 0) { f0[r] = 0; f1[r] = 0; }
+            z0[r] = fma(m1, f1[r], fma(m0, f0[r], z0[r]));                         // TX_q F_{q-1}
+            z1[r] = fma(m3, f1[r], fma(m2, f0[r], z1[r]));
+        }
+    }
+#pragma unroll
+    for (int l = 0; l < W_LEVELS; ++l) {
+        if (l < lev_b) {
+            const int d = 1 << l;
+            const uint32_t on = ln.valid & (1u << (8 + l));
+            const T m0 = lds_if(ln.abase + so.b[l][0], on, T()), m1 = lds_if(ln.abase + so.b[l][1], on, T()),
+                    m2 = lds_if(ln.abase + so.b[l][2], on, T()), m3 = lds_if(ln.abase + so.b[l][3], on, T());
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const T u0 = shfl_down_t(z0[r], d, Pw), u1 = shfl_down_t(z1[r], d, Pw);
+                z0[r] = fma(m1, u1, fma(m0, u0, z0[r]));
+                z1[r] = fma(m3, u1, fma(m2, u0, z1[r]));
+            }
+        }
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        T b0 = shfl_down_t(z0[r], 1, Pw), b1 = shfl_down_t(z1[r], 1, Pw);          // B_{q+1}
+        if (q >= P - 1) { b0 = 0; b1 = 0; }
+        if (sl[r] >= 0) {
+            T2 fo; fo.x = f0[r]; fo.y = f1[r]; stE[sl[r]] = fo;
+            T2 bo; bo.x = b0; bo.y = b1; stS[sl[r]] = bo;
+        }
+    }
+}
+
 template <typename T, int S, bool CLUSTER, bool PER = false>
 __device__ __forceinline__ void chunk_state_scan(const ScanGeom& g, const T* wtab, typename Pair<T>::type* stE,
                                                  typename Pair<T>::type* stS, int sys, int q, bool ok,

@@ -17,6 +17,7 @@
 //  (L v)_k = v_{k-1} + dg_k v_k + v_{k+1}, out-of-range terms dropped; dg_k = -2 except
 //  dg_0 = dg_{N-1} = -1 when bc = 1 (zero-flux).  Same formulas, in the same order, as
 //  step_tps_kernel (pent_step.cu).
+#include <cstdlib>
 #include "pent_chunk_common.cuh"
 
 namespace pent {
@@ -36,6 +37,7 @@ struct StepChunkParams {
     const T* mu1;
     const T* mu2;
     double dt, t0;
+    ScanOffsets so;       // chunk-state scan: uniform byte offsets of the transfer matrices (SPT > 1)
 };
 
 // Barrier of one thread group of a CTA (named barrier 1+g); the whole CTA when there is one group.
@@ -58,11 +60,14 @@ __device__ __forceinline__ void group_sync(int g, int nthreads)
 // keeps the space factors of its FIRST row in registers for the whole launch and steps the sinusoid with the
 // small-angle-stable recurrence  Phi_{j+1} = Phi_j + d_j,  d_{j+1} = d_j - 4 sin^2(pi/N) Phi_{j+1}
 // (error growth ~ j u, not j u / sin(2 pi / N) as for the three-term cosine recurrence): 3 flops per unknown.
-template <typename T, int S, int KIND, int NG, bool FORCED>
-__global__ void __launch_bounds__(CHUNK_MAX_THREADS, 1)
+// SPT: systems per thread (pent_chunk_common.cuh): thread (column i, chunk p) carries systems SPT i .. SPT i + SPT - 1
+// through chunk p, so that every coefficient broadcast feeds SPT recurrences; the CTA has P * S / SPT threads.
+template <typename T, int S, int KIND, int NG, bool FORCED, int SPT>
+__global__ void __launch_bounds__(CHUNK_MAX_THREADS / SPT, 1)
 step_chunked_kernel(const __grid_constant__ CUtensorMap tm, const StepChunkParams<T> prm)
 {
     constexpr int C = ChunkCfg<T>::C, BL = chunk_block_len<T>();
+    constexpr int SL = S / SPT;                  // thread columns of a tile
     using T2 = typename Pair<T>::type;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int P = prm.P, N = prm.N;
@@ -78,7 +83,7 @@ step_chunked_kernel(const __grid_constant__ CUtensorMap tm, const StepChunkParam
     uint64_t* bars = reinterpret_cast<uint64_t*>(amp_all + (FORCED ? (size_t)NG * 2 * S : 0));
     uint64_t* bar_state = &bars[1 + grp_id];                                   // [0] table, [1+g] state of group g
 
-    const int i = tid % S, p = tid / S;
+    const int i = tid % SL, p = tid / SL, sys0 = i * SPT;
     const bool active = p < P;
     const int lane = tid & 31, warp = tid >> 5, nwarps = TG >> 5;
     const uint32_t box_bytes = (uint32_t)(prm.box_rows * S * sizeof(T));
@@ -97,19 +102,40 @@ step_chunked_kernel(const __grid_constant__ CUtensorMap tm, const StepChunkParam
 
     const T* blk = table + (size_t)(active ? p : 0) * BL;
     const T* wtab = table + (size_t)P * BL;
-    const int slot = state_slot<S>(active ? p : 0, i);
+    int slot[SPT];
+#pragma unroll
+    for (int u = 0; u < SPT; ++u) slot[u] = state_slot<S>(active ? p : 0, sys0 + u);
     const int row0 = p * C;
-    T* cs = state + i;                                   // element (k, i) at cs[k*S]
+    T* cs = state + sys0;                                // element (k, sys0 + u) at cs[k*S + u]
     const int Pw = prm.Pw, G = 32 / Pw;
     const int q = lane % Pw, grp = lane / Pw;
     const ScanGeom geom{P, Pw, prm.lev_f, prm.lev_b, prm.woff};
     const int rounds = (S + nwarps * G - 1) / (nwarps * G);
+    // per-lane constants of the chunk-state scan (lane q of warp `warp` scans chunk q of systems (rr nwarps + warp) G + grp).
+    // The one-system-per-thread instantiations, kept for A/B, have no registers for them and use the round-1 scan.
+    ScanLane lane_tab;
+    int scan_slot[SPT];
+    if constexpr (SPT > 1) {
+        lane_tab = make_scan_lane<T>(geom, wtab, q);
+#pragma unroll
+        for (int rr = 0; rr < SPT; ++rr) {
+            const int sys = (rr * nwarps + warp) * G + grp;
+            scan_slot[rr] = (sys < S && q < P) ? state_slot<S>(q, sys) : -1;
+            asm volatile("" : "+r"(scan_slot[rr]));
+        }
+    }
     const T r = prm.r, sigma = prm.sigma;
     constexpr bool incr = (KIND == 2);       // KIND: 0 CH direct form, 2 CH increment form, 1 hyperdiffusion
     const T dg_edge = (prm.bc == 1) ? (T)-1 : (T)-2;
-    auto ldc = [&](int k) -> T { return ((unsigned)k < (unsigned)N) ? cs[(size_t)k * S] : (T)0; };
+    auto ldc = [&](T (&o)[SPT], int k) {
+        if ((unsigned)k < (unsigned)N) lds_sys<T, SPT>(o, cs + (size_t)k * S);
+        else {
+#pragma unroll
+            for (int u = 0; u < SPT; ++u) o[u] = (T)0;
+        }
+    };
     auto Ld = [&](int k) -> T { return (k == 0 || k == N - 1) ? dg_edge : (T)-2; };
-    // Warp-uniform choice: a warp that holds one boundary chunk (S=16: two chunks per warp) takes the
+    // Warp-uniform choice: a warp that holds one boundary chunk (several chunks per warp) takes the
     // general path with ALL its lanes instead of executing both paths one after the other; that warp
     // is the straggler every block barrier waits for.
     const bool first = row0 == 0, last = row0 + C == N;
@@ -125,7 +151,7 @@ step_chunked_kernel(const __grid_constant__ CUtensorMap tm, const StepChunkParam
                 tma_load_2d(state + (size_t)b * prm.box_rows * S, &tm, (int)(tile * S), b * prm.box_rows, bar_state);
         }
         mbar_wait(bar_state, parity);
-        // forcing amplitudes of system tid (threads of chunk 0) at step n -> amp[n & 1][tid]
+        // forcing amplitudes of system tid (threads 0..S-1) at step n -> amp[n & 1][tid]
         double fm1 = 0.0, fm2 = 0.0;
         // space factors of this thread's first row: (cos, sin)(2 pi x_row0) and their first differences along k,
         // (cos, sin)(theta + dl) - (cos, sin)(theta) = -2 sin^2(dl/2) (cos, sin) -+ sin(dl) (sin, cos), dl = 2 pi / N
@@ -143,10 +169,10 @@ step_chunked_kernel(const __grid_constant__ CUtensorMap tm, const StepChunkParam
             }
         }
         auto amp_for_step = [&](int n) {
-            double sn, cs;
-            sincospi(2.0 * fm2 * (prm.t0 + (double)n * prm.dt), &sn, &cs);
+            double sn, cs_;
+            sincospi(2.0 * fm2 * (prm.t0 + (double)n * prm.dt), &sn, &cs_);
             const double am = prm.dt * fm1;
-            T2 ab; ab.x = (T)(am * cs); ab.y = (T)(am * sn);
+            T2 ab; ab.x = (T)(am * cs_); ab.y = (T)(am * sn);
             amp[(n & 1) * S + tid] = ab;
         };
         if constexpr (FORCED) {
@@ -159,7 +185,7 @@ step_chunked_kernel(const __grid_constant__ CUtensorMap tm, const StepChunkParam
         }
 
         for (int step = 0; step < prm.nsteps; ++step) {
-            T v[C];
+            T v[SPT][C];
             if (active) {
                 // ---- explicit right-hand side of rows row0 .. row0+C-1, in registers ----
                 if constexpr (KIND != 1) {
@@ -174,21 +200,41 @@ step_chunked_kernel(const __grid_constant__ CUtensorMap tm, const StepChunkParam
                             if (!incr) return w;
                             return fma(-sigma, cl + fma(dg, cc, cr), r * w);
                         };
-                        const T* cw = cs + (size_t)row0 * S;          // cw[j*S] = c_{row0+j}
-                        T cl = first ? (T)0 : *(cw - 2 * S), cc = first ? (T)0 : *(cw - S), cr = cw[0];
-                        T u_prev = first ? (T)0 : U(cl, cc, cr, (T)-2);                    // u_{row0-1}
-                        cl = cc; cc = cr; cr = cw[S];
-                        T u_cur = U(cl, cc, cr, dfirst);                                   // u_{row0}
+                        const T* cw = cs + (size_t)row0 * S;          // cw[j*S + u] = c_{row0+j} of system u
+                        T cl[SPT], cc[SPT], cr[SPT], u_prev[SPT], u_cur[SPT];
+                        if (first) {
+#pragma unroll
+                            for (int u = 0; u < SPT; ++u) { cl[u] = 0; cc[u] = 0; }
+                        } else {
+                            lds_sys<T, SPT>(cl, cw - 2 * S);
+                            lds_sys<T, SPT>(cc, cw - S);
+                        }
+                        lds_sys<T, SPT>(cr, cw);
+#pragma unroll
+                        for (int u = 0; u < SPT; ++u) {
+                            u_prev[u] = first ? (T)0 : U(cl[u], cc[u], cr[u], (T)-2);        // u_{row0-1}
+                            cl[u] = cc[u]; cc[u] = cr[u];
+                        }
+                        lds_sys<T, SPT>(cr, cw + S);
+#pragma unroll
+                        for (int u = 0; u < SPT; ++u) u_cur[u] = U(cl[u], cc[u], cr[u], dfirst);  // u_{row0}
 #pragma unroll
                         for (int j = 0; j < C; ++j) {
-                            cl = cc; cc = cr;                                              // cl = c_{row0+j}, cc = c_{row0+j+1}
-                            if (j + 2 < C) cr = cw[(j + 2) * S];
-                            else cr = last ? (T)0 : cw[(j + 2) * S];                       // rows N, N+1 do not exist
-                            T u_next = U(cl, cc, cr, (j + 1 == C - 1) ? dlast : (T)-2);    // u_{row0+j+1}
-                            if (j == C - 1 && last) u_next = 0;                            // u_N
-                            T Lu = u_prev + fma(j == 0 ? dfirst : (j == C - 1 ? dlast : (T)-2), u_cur, u_next);
-                            v[j] = incr ? Lu : fma(r, Lu, cl);
-                            u_prev = u_cur; u_cur = u_next;
+#pragma unroll
+                            for (int u = 0; u < SPT; ++u) { cl[u] = cc[u]; cc[u] = cr[u]; }    // cl = c_{row0+j}, cc = c_{row0+j+1}
+                            if (j + 2 < C || !last) lds_sys<T, SPT>(cr, cw + (size_t)(j + 2) * S);
+                            else {
+#pragma unroll
+                                for (int u = 0; u < SPT; ++u) cr[u] = (T)0;                    // rows N, N+1 do not exist
+                            }
+#pragma unroll
+                            for (int u = 0; u < SPT; ++u) {
+                                T u_next = U(cl[u], cc[u], cr[u], (j + 1 == C - 1) ? dlast : (T)-2);   // u_{row0+j+1}
+                                if (j == C - 1 && last) u_next = 0;                                    // u_N
+                                T Lu = u_prev[u] + fma(j == 0 ? dfirst : (j == C - 1 ? dlast : (T)-2), u_cur[u], u_next);
+                                v[u][j] = incr ? Lu : fma(r, Lu, cl[u]);
+                                u_prev[u] = u_cur[u]; u_cur[u] = u_next;
+                            }
                         }
                     } else {
                         auto U = [&](int k, T cl, T cc, T cr) -> T {
@@ -197,104 +243,159 @@ step_chunked_kernel(const __grid_constant__ CUtensorMap tm, const StepChunkParam
                             if (!incr) return w;
                             return fma(-sigma, cl + fma(Ld(k), cc, cr), r * w);
                         };
-                        T cl = ldc(row0 - 2), cc = ldc(row0 - 1), cr = ldc(row0);
-                        T u_prev = U(row0 - 1, cl, cc, cr);
-                        cl = cc; cc = cr; cr = ldc(row0 + 1);
-                        T u_cur = U(row0, cl, cc, cr);
+                        T cl[SPT], cc[SPT], cr[SPT], u_prev[SPT], u_cur[SPT];
+                        ldc(cl, row0 - 2); ldc(cc, row0 - 1); ldc(cr, row0);
+#pragma unroll
+                        for (int u = 0; u < SPT; ++u) {
+                            u_prev[u] = U(row0 - 1, cl[u], cc[u], cr[u]);
+                            cl[u] = cc[u]; cc[u] = cr[u];
+                        }
+                        ldc(cr, row0 + 1);
+#pragma unroll
+                        for (int u = 0; u < SPT; ++u) u_cur[u] = U(row0, cl[u], cc[u], cr[u]);
 #pragma unroll
                         for (int j = 0; j < C; ++j) {
                             const int k = row0 + j;
-                            cl = cc; cc = cr; cr = ldc(k + 2);          // window centred on k+1; cl = c_k
-                            T u_next = U(k + 1, cl, cc, cr);
-                            T Lu = u_prev + fma(Ld(k), u_cur, u_next);
-                            v[j] = incr ? Lu : fma(r, Lu, cl);
-                            u_prev = u_cur; u_cur = u_next;
+#pragma unroll
+                            for (int u = 0; u < SPT; ++u) { cl[u] = cc[u]; cc[u] = cr[u]; }    // window centred on k+1; cl = c_k
+                            ldc(cr, k + 2);
+#pragma unroll
+                            for (int u = 0; u < SPT; ++u) {
+                                T u_next = U(k + 1, cl[u], cc[u], cr[u]);
+                                T Lu = u_prev[u] + fma(Ld(k), u_cur[u], u_next);
+                                v[u][j] = incr ? Lu : fma(r, Lu, cl[u]);
+                                u_prev[u] = u_cur[u]; u_cur[u] = u_next;
+                            }
                         }
                     }
                 } else if (interior) {
                     // (2I - A) c, rows row0 .. row0+C-1 all inside the matrix (see `interior` above); the
                     // entries of the diagonals that fall outside the matrix are zero in prm.dg
                     const T* cw = cs + (size_t)row0 * S;
-                    T cm2 = first ? (T)0 : *(cw - 2 * S), cm1 = first ? (T)0 : *(cw - S), c0 = cw[0], cp1 = cw[S];
+                    T cm2[SPT], cm1[SPT], c0[SPT], cp1[SPT], cp2[SPT];
+                    if (first) {
+#pragma unroll
+                        for (int u = 0; u < SPT; ++u) { cm2[u] = 0; cm1[u] = 0; }
+                    } else {
+                        lds_sys<T, SPT>(cm2, cw - 2 * S);
+                        lds_sys<T, SPT>(cm1, cw - S);
+                    }
+                    lds_sys<T, SPT>(c0, cw);
+                    lds_sys<T, SPT>(cp1, cw + S);
                     const T* dk = prm.dg + 8 * (size_t)row0;
 #pragma unroll
                     for (int j = 0; j < C; ++j) {
-                        T cp2;
-                        if (j + 2 < C) cp2 = cw[(j + 2) * S];
-                        else cp2 = last ? (T)0 : cw[(j + 2) * S];
-                        T s = __ldg(dk + 8 * j + 2) * c0;
-                        s = fma(__ldg(dk + 8 * j + 1), cm1, s);
-                        s = fma(__ldg(dk + 8 * j + 0), cm2, s);
-                        s = fma(__ldg(dk + 8 * j + 3), cp1, s);
-                        s = fma(__ldg(dk + 8 * j + 4), cp2, s);
-                        v[j] = (T)2 * c0 - s;
-                        cm2 = cm1; cm1 = c0; c0 = cp1; cp1 = cp2;
+                        if (j + 2 < C || !last) lds_sys<T, SPT>(cp2, cw + (size_t)(j + 2) * S);
+                        else {
+#pragma unroll
+                            for (int u = 0; u < SPT; ++u) cp2[u] = (T)0;
+                        }
+                        const T da = __ldg(dk + 8 * j + 0), db = __ldg(dk + 8 * j + 1), dc = __ldg(dk + 8 * j + 2),
+                                dd = __ldg(dk + 8 * j + 3), de = __ldg(dk + 8 * j + 4);
+#pragma unroll
+                        for (int u = 0; u < SPT; ++u) {
+                            T s = dc * c0[u];
+                            s = fma(db, cm1[u], s);
+                            s = fma(da, cm2[u], s);
+                            s = fma(dd, cp1[u], s);
+                            s = fma(de, cp2[u], s);
+                            v[u][j] = (T)2 * c0[u] - s;
+                            cm2[u] = cm1[u]; cm1[u] = c0[u]; c0[u] = cp1[u]; cp1[u] = cp2[u];
+                        }
                     }
                 } else {
-                    T cm2 = ldc(row0 - 2), cm1 = ldc(row0 - 1), c0 = ldc(row0), cp1 = ldc(row0 + 1);
+                    T cm2[SPT], cm1[SPT], c0[SPT], cp1[SPT], cp2[SPT];
+                    ldc(cm2, row0 - 2); ldc(cm1, row0 - 1); ldc(c0, row0); ldc(cp1, row0 + 1);
 #pragma unroll
                     for (int j = 0; j < C; ++j) {
                         const int k = row0 + j;
-                        T cp2 = ldc(k + 2);
-                        T rhs = 0;
+                        ldc(cp2, k + 2);
+                        T da = 0, db = 0, dc = 0, dd = 0, de = 0;
                         if (k < N) {
                             const T* dk = prm.dg + 8 * (size_t)k;
-                            T s = __ldg(dk + 2) * c0;
-                            s = fma(__ldg(dk + 1), cm1, s);
-                            s = fma(__ldg(dk + 0), cm2, s);
-                            s = fma(__ldg(dk + 3), cp1, s);
-                            s = fma(__ldg(dk + 4), cp2, s);
-                            rhs = (T)2 * c0 - s;
+                            da = __ldg(dk + 0); db = __ldg(dk + 1); dc = __ldg(dk + 2); dd = __ldg(dk + 3); de = __ldg(dk + 4);
                         }
-                        v[j] = rhs;
-                        cm2 = cm1; cm1 = c0; c0 = cp1; cp1 = cp2;
+#pragma unroll
+                        for (int u = 0; u < SPT; ++u) {
+                            T rhs = 0;
+                            if (k < N) {
+                                T s = dc * c0[u];
+                                s = fma(db, cm1[u], s);
+                                s = fma(da, cm2[u], s);
+                                s = fma(dd, cp1[u], s);
+                                s = fma(de, cp2[u], s);
+                                rhs = (T)2 * c0[u] - s;
+                            }
+                            v[u][j] = rhs;
+                            cm2[u] = cm1[u]; cm1[u] = c0[u]; c0[u] = cp1[u]; cp1[u] = cp2[u];
+                        }
                     }
                 }
                 if constexpr (FORCED) {
-                    const T2 ab = amp[(step & 1) * S + i];
-                    T ph = fma(ab.x, fcx, ab.y * fsx), dph = fma(ab.x, fdcx, ab.y * fdsx);
-                    if (row0 + C <= N) {
 #pragma unroll
-                        for (int j = 0; j < C; ++j) { v[j] += ph; ph += dph; dph = fma(-fkap, ph, dph); }
-                    } else {
+                    for (int u = 0; u < SPT; ++u) {
+                        const T2 ab = amp[(step & 1) * S + sys0 + u];
+                        T ph = fma(ab.x, fcx, ab.y * fsx), dph = fma(ab.x, fdcx, ab.y * fdsx);
+                        if (row0 + C <= N) {
 #pragma unroll
-                        for (int j = 0; j < C; ++j) {
-                            if (row0 + j < N) v[j] += ph;
-                            ph += dph;
-                            dph = fma(-fkap, ph, dph);
+                            for (int j = 0; j < C; ++j) { v[u][j] += ph; ph += dph; dph = fma(-fkap, ph, dph); }
+                        } else {
+#pragma unroll
+                            for (int j = 0; j < C; ++j) {
+                                if (row0 + j < N) v[u][j] += ph;
+                                ph += dph;
+                                dph = fma(-fkap, ph, dph);
+                            }
                         }
                     }
                 }
                 // ---- chunked solve, stages 1+2 ----
-                T2 e, s;
-                chunk_local_sweeps<T>(v, blk, e, s);
-                stE[slot] = e;
-                stS[slot] = s;
+                T2 e[SPT], s[SPT];
+                chunk_local_sweeps_n<T, SPT>(v, blk, e, s);
+#pragma unroll
+                for (int u = 0; u < SPT; ++u) { stE[slot[u]] = e[u]; stS[slot[u]] = s[u]; }
             }
             group_sync<NG>(grp_id, TG);
             if constexpr (FORCED) {
                 if (tid < S && step + 1 < prm.nsteps) amp_for_step(step + 1);   // read after two more barriers
             }
             if (P > 1) {
-                for (int rr = 0; rr < rounds; ++rr) {
-                    const int sys = (rr * nwarps + warp) * G + grp;
-                    chunk_state_scan<T, S, false>(geom, wtab, stE, stS, sys, q, (sys < S) && (q < P), 0, 1,
-                                                  nullptr, nullptr, bars, 0u, 0u, 0u);
+                if (SPT > 1 && rounds == SPT) {   // (P a power of two) every scan lane carries SPT systems at once
+                    chunk_state_scan_lean<T, SPT>(lane_tab, prm.so, P, Pw, prm.lev_f, prm.lev_b, q, stE, stS, scan_slot);
+                } else {
+                    for (int rr = 0; rr < rounds; ++rr) {
+                        const int sys = (rr * nwarps + warp) * G + grp;
+                        chunk_state_scan<T, S, false>(geom, wtab, stE, stS, sys, q, (sys < S) && (q < P), 0, 1,
+                                                      nullptr, nullptr, bars, 0u, 0u, 0u);
+                    }
                 }
             }
             group_sync<NG>(grp_id, TG);
             if (active) {
-                T F0 = 0, F1 = 0, B0 = 0, B1 = 0;
-                if (P > 1) { T2 fo = stE[slot]; F0 = fo.x; F1 = fo.y; T2 bo = stS[slot]; B0 = bo.x; B1 = bo.y; }
+                T F0[SPT], F1[SPT], B0[SPT], B1[SPT];
+#pragma unroll
+                for (int u = 0; u < SPT; ++u) {
+                    F0[u] = 0; F1[u] = 0; B0[u] = 0; B1[u] = 0;
+                    if (P > 1) { T2 fo = stE[slot[u]]; F0[u] = fo.x; F1[u] = fo.y; T2 bo = stS[slot[u]]; B0[u] = bo.x; B1[u] = bo.y; }
+                }
                 T* co = cs + (size_t)row0 * S;
 #pragma unroll
                 for (int jg = 0; jg < C / 4; ++jg) {
-                    T xv[4];
-                    chunk_correct4<T>(xv, &v[4 * jg], blk, jg, F0, F1, B0, B1);
+                    T xv[SPT][4];
+                    chunk_correct4_n<T, SPT>(xv, v, blk, jg, F0, F1, B0, B1);
 #pragma unroll
                     for (int rr = 0; rr < 4; ++rr) {
                         T* o = co + (size_t)(4 * jg + rr) * S;
-                        *o = incr ? *o + xv[rr] : xv[rr];
+                        T nv[SPT];
+                        if (incr) {
+                            lds_sys<T, SPT>(nv, o);
+#pragma unroll
+                            for (int u = 0; u < SPT; ++u) nv[u] += xv[u][rr];
+                        } else {
+#pragma unroll
+                            for (int u = 0; u < SPT; ++u) nv[u] = xv[u][rr];
+                        }
+                        sts_sys<T, SPT>(o, nv);
                     }
                 }
             }
@@ -315,23 +416,24 @@ step_chunked_kernel(const __grid_constant__ CUtensorMap tm, const StepChunkParam
     if (tid == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }
 
-// Shape of a step launch: NG groups of TG threads, each with a tile of S systems.
+// Shape of a step launch: NG groups of TG threads, each with a tile of S systems, SPT systems per thread.
 struct StepPlan {
     bool ok = false;
     ChunkPlan pl;
-    int S = 0, NG = 1, TG = 0;
+    int S = 0, NG = 1, TG = 0, SPT = 1;
     size_t smem = 0;
 };
 
-static StepPlan step_plan(const pent_handle* h, int64_t M, const void* c, int S, int NG)
+static StepPlan step_plan(const pent_handle* h, int64_t M, const void* c, int S, int NG, int SPT)
 {
     StepPlan sp;
     if (!h || h->kind != 0 || h->periodic) return sp;
     const size_t esz = h->dtype == PENT_F64 ? 8 : 4;
     sp.pl = make_plan(h, M, c, 1, S, /*any_S=*/true);
-    if (!sp.pl.ok) return sp;
-    sp.S = S; sp.NG = NG; sp.TG = sp.pl.threads;
-    if (sp.TG * NG > CHUNK_MAX_THREADS) return sp;
+    if (!sp.pl.ok || S % SPT != 0) return sp;
+    sp.S = S; sp.NG = NG; sp.SPT = SPT;
+    sp.TG = (sp.pl.Pl * S / SPT + 31) / 32 * 32;
+    if (sp.TG * NG > CHUNK_MAX_THREADS / SPT) return sp;
     sp.smem = (size_t)NG * ((size_t)sp.pl.nbox * sp.pl.box_rows * S * esz + (size_t)4 * sp.pl.Pl * S * esz) +
               sp.pl.table_bytes + (size_t)(1 + NG) * sizeof(uint64_t) +
               (size_t)NG * 4 * S * esz;                                    // forcing amplitudes (used when FORCED)
@@ -339,20 +441,26 @@ static StepPlan step_plan(const pent_handle* h, int64_t M, const void* c, int S,
     return sp;
 }
 
-// Default, measured on cfg4 (1000 steps, same box, profiles/r01_ab_tuning.md): fp64 one group of 16
-// systems 29.15 us per step against 30.8 for two groups of 8 (narrower tiles double the coefficient
-// broadcasts per system and the shared-memory pipe is the busiest unit); fp32 two groups of 16
-// systems 20.2 us against 22.2 for one group of 32.
+// Default shapes, measured on cfg4 (1000 steps, profiles/r02_step_spt.md).  Two systems per thread halve the
+// coefficient broadcasts per unknown, which is what bounds this kernel (shared-memory wavefronts).
+// PENT_AB_STEP_SPT=1 (environment, measurement only) selects the one-system-per-thread shapes of round 1.
+// Two thread groups of half-width tiles (S = 8 fp64 / 16 fp32, SPT = 2) measured slower: 26.7 against 22.9 us per
+// step (fp32 13.4 against 11.5): a warp then spans 8 chunks and its coefficient loads are no longer broadcasts.
 static StepPlan step_auto_plan(const pent_handle* h, int64_t M, const void* c)
 {
     if (!h || !chunk_stitching_stable(h)) return StepPlan{};
-    if (h->dtype == PENT_F64) return step_plan(h, M, c, 16, 1);
-    StepPlan two = step_plan(h, M, c, 16, 2);
+    static const int spt = []() { const char* e = std::getenv("PENT_AB_STEP_SPT"); return e ? std::atoi(e) : 2; }();
+    if (h->dtype == PENT_F64) {
+        if (spt != 1) { StepPlan two = step_plan(h, M, c, 16, 1, 2); if (two.ok) return two; }
+        return step_plan(h, M, c, 16, 1, 1);
+    }
+    if (spt != 1) { StepPlan w = step_plan(h, M, c, 32, 1, 2); if (w.ok) return w; }
+    StepPlan two = step_plan(h, M, c, 16, 2, 1);
     if (two.ok) return two;
-    return step_plan(h, M, c, 32, 1);
+    return step_plan(h, M, c, 32, 1, 1);
 }
 
-template <typename T, int S, int KIND, int NG, bool FORCED>
+template <typename T, int S, int KIND, int NG, bool FORCED, int SPT>
 static int launch_step_inst(const pent_handle* h, const StepPlan& sp, const pent_step_params* p, const pent_forcing* fg,
                             int64_t M, void* c, int nsteps, cudaStream_t s)
 {
@@ -364,6 +472,7 @@ static int launch_step_inst(const pent_handle* h, const StepPlan& sp, const pent
     prm.lev_f = h->lev_f[0] < lg ? h->lev_f[0] : lg;
     prm.lev_b = h->lev_b[0] < lg ? h->lev_b[0] : lg;
     for (int l = 0; l < W_LEVELS; ++l) prm.woff[l] = w_level_off(pl.Pl, l, 1);
+    prm.so = make_scan_offsets<T>(pl.Pl, prm.woff);
     prm.box_rows = pl.box_rows; prm.nbox = pl.nbox;
     prm.ntiles = (M + S - 1) / S;
     prm.table = (const T*)h->cf[0];
@@ -378,7 +487,7 @@ static int launch_step_inst(const pent_handle* h, const StepPlan& sp, const pent
         g_last_cuda_error = (int)cudaErrorInvalidValue;
         return PENT_ERR_CUDA;
     }
-    auto kern = step_chunked_kernel<T, S, KIND, NG, FORCED>;
+    auto kern = step_chunked_kernel<T, S, KIND, NG, FORCED, SPT>;
     static SmemOnce mark;
     PENT_CUDA(ensure_dynamic_smem(mark, kern, sp.smem));
     const int threads = sp.TG * NG;
@@ -401,17 +510,17 @@ bool step_chunked_supported(const pent_handle* h, int64_t M, const void* c)
     return h && h->kind == 0 && step_auto_plan(h, M, c).ok;
 }
 
-template <typename T, int S, int NG>
+template <typename T, int S, int NG, int SPT>
 static int launch_step_kind(const pent_handle* h, const StepPlan& sp, const pent_step_params* p, const pent_forcing* fg,
                             int64_t M, void* c, int nsteps, cudaStream_t s)
 {
-    if (p->kind == 1) return launch_step_inst<T, S, 1, NG, false>(h, sp, p, nullptr, M, c, nsteps, s);
+    if (p->kind == 1) return launch_step_inst<T, S, 1, NG, false, SPT>(h, sp, p, nullptr, M, c, nsteps, s);
     if (fg) {
-        if (p->form == 1) return launch_step_inst<T, S, 2, NG, true>(h, sp, p, fg, M, c, nsteps, s);
-        return launch_step_inst<T, S, 0, NG, true>(h, sp, p, fg, M, c, nsteps, s);
+        if (p->form == 1) return launch_step_inst<T, S, 2, NG, true, SPT>(h, sp, p, fg, M, c, nsteps, s);
+        return launch_step_inst<T, S, 0, NG, true, SPT>(h, sp, p, fg, M, c, nsteps, s);
     }
-    if (p->form == 1) return launch_step_inst<T, S, 2, NG, false>(h, sp, p, nullptr, M, c, nsteps, s);
-    return launch_step_inst<T, S, 0, NG, false>(h, sp, p, nullptr, M, c, nsteps, s);
+    if (p->form == 1) return launch_step_inst<T, S, 2, NG, false, SPT>(h, sp, p, nullptr, M, c, nsteps, s);
+    return launch_step_inst<T, S, 0, NG, false, SPT>(h, sp, p, nullptr, M, c, nsteps, s);
 }
 
 int launch_step_chunked(const pent_handle* h, const pent_step_params* p, const pent_forcing* fg, int64_t M, void* c,
@@ -419,8 +528,12 @@ int launch_step_chunked(const pent_handle* h, const pent_step_params* p, const p
 {
     const StepPlan sp = step_auto_plan(h, M, c);
     if (!sp.ok) return PENT_ERR_ARG;
-    if (h->dtype == PENT_F64) return launch_step_kind<double, 16, 1>(h, sp, p, fg, M, c, nsteps, s);
-    if (sp.NG == 2) return launch_step_kind<float, 16, 2>(h, sp, p, fg, M, c, nsteps, s);
-    return launch_step_kind<float, 32, 1>(h, sp, p, fg, M, c, nsteps, s);
+    if (h->dtype == PENT_F64) {
+        if (sp.SPT == 2) return launch_step_kind<double, 16, 1, 2>(h, sp, p, fg, M, c, nsteps, s);
+        return launch_step_kind<double, 16, 1, 1>(h, sp, p, fg, M, c, nsteps, s);
+    }
+    if (sp.SPT == 2) return launch_step_kind<float, 32, 1, 2>(h, sp, p, fg, M, c, nsteps, s);
+    if (sp.NG == 2) return launch_step_kind<float, 16, 2, 1>(h, sp, p, fg, M, c, nsteps, s);
+    return launch_step_kind<float, 32, 1, 1>(h, sp, p, fg, M, c, nsteps, s);
 }
 }  // namespace pent
