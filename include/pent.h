@@ -69,7 +69,7 @@ enum {
                                            chunk coupling by the shared correction vectors (2 passes)  */
 };
 /* PENT_KERNEL_CHUNKED with an explicit shape (measurement): Q = CTAs of a thread-block cluster that
- * split k between them (1, 2, 4, 8; 0 = choose), S = systems per tile (16, 32 for fp64; 32, 64 for
+ * split k between them (1, 2, 4, 8, 16 -- 16 is CUDA's non-portable cluster size --; 0 = choose), S = systems per tile (16, 32 for fp64; 32, 64 for
  * fp32; 0 = choose).  PENT_ERR_ARG if that shape does not fit N / M / shared memory. */
 #define PENT_KERNEL_CHUNKED_CFG(Q, S) (2 | ((Q) << 8) | ((S) << 16))
 

@@ -26,19 +26,19 @@ constexpr size_t SMEM_LIMIT = 232448;       // 227 KB dynamic shared memory per 
 //   (the next three only in the tables of a cluster, Q > 1)
 //   PF   : 4 x P     TPhi_q TPhi_{q-1} ... TPhi_{first chunk of the block}   (acts on the F entering the block)
 //   PB   : 4 x P     TPsi_q TPsi_{q+1} ... TPsi_{last chunk of the block}    (acts on the B entering the block)
-//   BLK  : 64        block products of every cluster rank r: TPhiBlock(r) at [4r..4r+3] (contiguous
-//                    2x2), TPsiBlock(r) at [32+4r..]
+//   BLK  : 8 MAXQ    block products of every cluster rank r < MAXQ = 16: TPhiBlock(r) at [4r..4r+3] (contiguous
+//                    2x2), TPsiBlock(r) at [4 MAXQ + 4r..]
 //   then for each Kogge-Stone level l = 0..4, d = 2^l, n = max(0, P-d):
 //   WF_l : 4 x n     TPhi_q TPhi_{q-1} ... TPhi_{q-d+1}  for q >= d,     at [e*n + q-d]
 //   WB_l : 4 x n     TPsi_q TPsi_{q+1} ... TPsi_{q+d-1}  for q+d <= P-1, at [e*n + q]
 // Only the levels a handle needs are staged into shared memory (they come last).
 // BAND = 1 (tridiagonal A, a = e = 0: cuThomasBatch's case): the recurrences have ONE term, the
-// chunk states and every transfer "matrix" are scalars, so every 4 above becomes 1 (BLK: 8 + 8 scalars).
+// chunk states and every transfer "matrix" are scalars, so every 4 above becomes 1 (BLK: MAXQ + MAXQ scalars).
 constexpr int W_LEVELS = 5;
 __host__ __device__ inline int w_level_off(int P, int l, int Q, int BAND = 2)
 {
     const int u = BAND == 2 ? 4 : 1;
-    int off = Q > 1 ? 3 * u * P + 16 * u : u * P;      // PF, PB, BLK exist only in cluster tables
+    int off = Q > 1 ? 3 * u * P + 2 * PENT_MAXQ * u : u * P;      // PF, PB, BLK exist only in cluster tables
     for (int k = 0; k < l; ++k) { int n = P - (1 << k); off += 2 * u * (n > 0 ? n : 0); }
     return off;
 }
@@ -685,7 +685,7 @@ __device__ __forceinline__ void chunk_state_scan(const ScanGeom& g, const T* wta
         for (int rr = Q - 1; rr > rank; --rr) {   // B_in(rr-1) = aggB[rr] + TPsiBlock(rr) B_in(rr)
             T2 a = aggB[rr * S + sy];
             T n0 = a.x, n1 = a.y;
-            mat2_acc(n0, n1, wtab + 12 * P + 32 + 4 * rr, 1, bin0, bin1);
+            mat2_acc(n0, n1, wtab + 12 * P + 4 * PENT_MAXQ + 4 * rr, 1, bin0, bin1);
             bin0 = n0; bin1 = n1;
         }
         if (ok && rank < Q - 1) mat2_acc(z0, z1, wtab + 8 * P + q, P, bin0, bin1);   // PB_q B_in
@@ -693,7 +693,7 @@ __device__ __forceinline__ void chunk_state_scan(const ScanGeom& g, const T* wta
             for (int rr = Q - 1; rr >= 0; --rr) {  // continue the chain down to the first block: B of chunk 0
                 T2 a = aggB[rr * S + sy];
                 T n0 = a.x, n1 = a.y;
-                mat2_acc(n0, n1, wtab + 12 * P + 32 + 4 * rr, 1, B00, B01);
+                mat2_acc(n0, n1, wtab + 12 * P + 4 * PENT_MAXQ + 4 * rr, 1, B00, B01);
                 B00 = n0; B01 = n1;
             }
             T2 yy = per->yab[sy];
@@ -770,7 +770,7 @@ __device__ __forceinline__ void tri_state_scan(const ScanGeom& g, const T* wtab,
         if (ok && q == 0)
             for (int rr = 0; rr < rank; ++rr) st_async_one(&aggB[rank * S + sys], &bars[BAR_B], rr, z);
         if (agg_bytes_b) mbar_wait(&bars[BAR_B], parity);
-        for (int rr = Q - 1; rr > rank; --rr) bin = fma(wtab[3 * P + 8 + rr], bin, aggB[rr * S + sy]);
+        for (int rr = Q - 1; rr > rank; --rr) bin = fma(wtab[3 * P + PENT_MAXQ + rr], bin, aggB[rr * S + sy]);
         if (ok && rank < Q - 1) z = fma(wtab[2 * P + q], bin, z);             // PB_q B_in
     }
     T b = shfl_down_t(z, 1, Pw);

@@ -104,6 +104,16 @@ static int launch_inst(const pent_handle* h, const ChunkPlan& pl, int64_t M, con
         at[0].val.clusterDim.x = (unsigned)pl.Q; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
         cfg.blockDim = dim3((unsigned)pl.threads); cfg.dynamicSmemBytes = smem_total; cfg.stream = s;
         cfg.attrs = at; cfg.numAttrs = 1 + PENT_PDL;
+        if (pl.Q > 8) {           // 16 CTAs per cluster: a non-portable size, allowed once per kernel instance and device
+            static SmemOnce npmark;
+            int d2 = 0;
+            PENT_CUDA(cudaGetDevice(&d2));
+            const uint32_t bit = 1u << (d2 & 31);
+            if (!(npmark.mask.load(std::memory_order_acquire) & bit)) {
+                PENT_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+                npmark.mask.fetch_or(bit, std::memory_order_release);
+            }
+        }
         if (!hit) {
             cfg.gridDim = dim3((unsigned)(pl.Q * oc.nsm));       // upper bound for the occupancy query
             int ncl = 0;

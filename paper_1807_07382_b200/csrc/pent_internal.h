@@ -5,8 +5,10 @@
 #include <atomic>
 #include "pent.h"
 
-// Cluster sizes (CTAs along k) the chunked kernel has tables for: Q = 1 << j, j < PENT_NQ.
-#define PENT_NQ 4
+// Cluster sizes (CTAs along k) the chunked kernel has tables for: Q = 1 << j, j < PENT_NQ.  Q = 16 is a
+// non-portable cluster size (cudaFuncAttributeNonPortableClusterSizeAllowed); PENT_MAXQ sizes the block-product table.
+#define PENT_NQ 5
+#define PENT_MAXQ 16
 
 struct pent_handle {
     int kind;            // 0 = shared A, 1 = per-system factors

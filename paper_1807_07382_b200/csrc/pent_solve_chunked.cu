@@ -123,7 +123,7 @@ __global__ void build_chunk_products_kernel(int Pl, int Q, const double* __restr
                                             int* __restrict__ levels)
 {
     __shared__ double wf[W_LEVELS][MAX_PL][4], wb[W_LEVELS][MAX_PL][4];
-    __shared__ double pf[MAX_PL][4], pb[MAX_PL][4], blkm[64];
+    __shared__ double pf[MAX_PL][4], pb[MAX_PL][4], blkm[8 * PENT_MAXQ];
     __shared__ int need_f, need_b;
     const int q = threadIdx.x, rank = blockIdx.x;
     const double* tm = tmat + (size_t)rank * Pl * 12;
@@ -146,14 +146,14 @@ __global__ void build_chunk_products_kernel(int Pl, int Q, const double* __restr
         for (int j = Pl - 2; j >= 0; --j) mat2_mul(pb[j], tm + j * 12 + 8, pb[j + 1]);
     }
     if (q == 2) {   // block products of every rank (each block computes all of them)
-        for (int r = 0; r < 8; ++r) {
+        for (int r = 0; r < PENT_MAXQ; ++r) {
             double f[4] = {1.0, 0.0, 0.0, 1.0}, b[4] = {1.0, 0.0, 0.0, 1.0};
             if (r < Q) {
                 const double* t = tmat + (size_t)r * Pl * 12;
                 for (int j = 0; j < Pl; ++j) mat2_mul(f, t + j * 12, f);            // TPhi_j ... TPhi_0
                 for (int j = Pl - 1; j >= 0; --j) mat2_mul(b, t + j * 12 + 8, b);   // TPsi_j ... TPsi_last
             }
-            for (int e = 0; e < 4; ++e) { blkm[4 * r + e] = f[e]; blkm[32 + 4 * r + e] = b[e]; }
+            for (int e = 0; e < 4; ++e) { blkm[4 * r + e] = f[e]; blkm[4 * PENT_MAXQ + 4 * r + e] = b[e]; }
         }
     }
     __syncthreads();
@@ -185,7 +185,7 @@ __global__ void build_chunk_products_kernel(int Pl, int Q, const double* __restr
         }
     }
     if (Q > 1)
-        for (int j = q; j < 64; j += blockDim.x) wtab[12 * Pl + j] = (T)blkm[j];
+        for (int j = q; j < 8 * PENT_MAXQ; j += blockDim.x) wtab[12 * Pl + j] = (T)blkm[j];
     __syncthreads();
     if (q == 0) { atomicMax(&levels[0], need_f); atomicMax(&levels[1], need_b); }
 }
@@ -233,7 +233,7 @@ template <typename T>
 __global__ void build_tri_products_kernel(int Pl, int Q, const double* __restrict__ tmat,
                                           T* __restrict__ tab, size_t tab_stride, int* __restrict__ levels)
 {
-    __shared__ double wf[W_LEVELS][MAX_PL], wb[W_LEVELS][MAX_PL], pf[MAX_PL], pb[MAX_PL], blkm[16];
+    __shared__ double wf[W_LEVELS][MAX_PL], wb[W_LEVELS][MAX_PL], pf[MAX_PL], pb[MAX_PL], blkm[2 * PENT_MAXQ];
     __shared__ int need_f, need_b;
     const int q = threadIdx.x, rank = blockIdx.x;
     const double* tm = tmat + (size_t)rank * Pl * 3;
@@ -247,13 +247,13 @@ __global__ void build_tri_products_kernel(int Pl, int Q, const double* __restric
     if (q == 0) { pf[0] = tm[0]; for (int j = 1; j < Pl; ++j) pf[j] = tm[j * 3] * pf[j - 1]; }
     if (q == 1) { pb[Pl - 1] = tm[(Pl - 1) * 3 + 2]; for (int j = Pl - 2; j >= 0; --j) pb[j] = tm[j * 3 + 2] * pb[j + 1]; }
     if (q == 2) {
-        for (int r = 0; r < 8; ++r) {
+        for (int r = 0; r < PENT_MAXQ; ++r) {
             double f = 1.0, b = 1.0;
             if (r < Q) {
                 const double* t = tmat + (size_t)r * Pl * 3;
                 for (int j = 0; j < Pl; ++j) { f *= t[j * 3]; b *= t[j * 3 + 2]; }
             }
-            blkm[r] = f; blkm[8 + r] = b;
+            blkm[r] = f; blkm[PENT_MAXQ + r] = b;
         }
     }
     __syncthreads();
@@ -276,7 +276,7 @@ __global__ void build_tri_products_kernel(int Pl, int Q, const double* __restric
         if (Q > 1) { wtab[Pl + q] = (T)pf[q]; wtab[2 * Pl + q] = (T)pb[q]; }
     }
     if (Q > 1)
-        for (int j = q; j < 16; j += blockDim.x) wtab[3 * Pl + j] = (T)blkm[j];
+        for (int j = q; j < 2 * PENT_MAXQ; j += blockDim.x) wtab[3 * Pl + j] = (T)blkm[j];
     __syncthreads();
     if (q == 0) { atomicMax(&levels[0], need_f); atomicMax(&levels[1], need_b); }
 }

@@ -28,7 +28,7 @@ struct StepChunkParams {
     int woff[W_LEVELS];
     int box_rows, nbox;
     uint32_t table_bytes;
-    int64_t M, ntiles;
+    int64_t M, ntiles, tile0;   // this launch takes tiles [tile0, ntiles) of S systems
     const T* table;
     const T* dg;          // N x {a,b,c,d,e, cos 2 pi x_k, sin 2 pi x_k, 0} (kind 1; forcing)
     int nsteps, bc;
@@ -144,7 +144,7 @@ step_chunked_kernel(const __grid_constant__ CUtensorMap tm, const StepChunkParam
                                                       C >= 4 && N >= 2 * C);
     uint32_t parity = 0;
 
-    for (int64_t tile = (int64_t)blockIdx.x * NG + grp_id; tile < prm.ntiles; tile += (int64_t)gridDim.x * NG) {
+    for (int64_t tile = prm.tile0 + (int64_t)blockIdx.x * NG + grp_id; tile < prm.ntiles; tile += (int64_t)gridDim.x * NG) {
         if (tid == 0) {
             mbar_expect_tx(bar_state, box_bytes * prm.nbox);
             for (int b = 0; b < prm.nbox; ++b)
@@ -460,9 +460,10 @@ static StepPlan step_auto_plan(const pent_handle* h, int64_t M, const void* c)
     return step_plan(h, M, c, 32, 1, 1);
 }
 
+// Systems [sys_lo, sys_hi) of the batch (sys_lo a multiple of S) in tiles of S.
 template <typename T, int S, int KIND, int NG, bool FORCED, int SPT>
 static int launch_step_inst(const pent_handle* h, const StepPlan& sp, const pent_step_params* p, const pent_forcing* fg,
-                            int64_t M, void* c, int nsteps, cudaStream_t s)
+                            int64_t M, void* c, int nsteps, cudaStream_t s, int64_t sys_lo, int64_t sys_hi)
 {
     const ChunkPlan& pl = sp.pl;
     StepChunkParams<T> prm;
@@ -474,7 +475,8 @@ static int launch_step_inst(const pent_handle* h, const StepPlan& sp, const pent
     for (int l = 0; l < W_LEVELS; ++l) prm.woff[l] = w_level_off(pl.Pl, l, 1);
     prm.so = make_scan_offsets<T>(pl.Pl, prm.woff);
     prm.box_rows = pl.box_rows; prm.nbox = pl.nbox;
-    prm.ntiles = (M + S - 1) / S;
+    prm.tile0 = sys_lo / S;
+    prm.ntiles = (sys_hi + S - 1) / S;
     prm.table = (const T*)h->cf[0];
     prm.table_bytes = (uint32_t)pl.table_bytes;
     prm.dg = (const T*)h->dg;
@@ -497,7 +499,7 @@ static int launch_step_inst(const pent_handle* h, const StepPlan& sp, const pent
     PENT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, threads, sp.smem));
     if (occ < 1) return PENT_ERR_ARG;
     int64_t grid = (int64_t)nsm * occ;
-    const int64_t need = (prm.ntiles + NG - 1) / NG;
+    const int64_t need = (prm.ntiles - prm.tile0 + NG - 1) / NG;
     if (grid > need) grid = need;
     kern<<<(unsigned)grid, threads, sp.smem, s>>>(tm, prm);
     count_launch();
@@ -512,28 +514,55 @@ bool step_chunked_supported(const pent_handle* h, int64_t M, const void* c)
 
 template <typename T, int S, int NG, int SPT>
 static int launch_step_kind(const pent_handle* h, const StepPlan& sp, const pent_step_params* p, const pent_forcing* fg,
-                            int64_t M, void* c, int nsteps, cudaStream_t s)
+                            int64_t M, void* c, int nsteps, cudaStream_t s, int64_t lo, int64_t hi)
 {
-    if (p->kind == 1) return launch_step_inst<T, S, 1, NG, false, SPT>(h, sp, p, nullptr, M, c, nsteps, s);
+    if (p->kind == 1) return launch_step_inst<T, S, 1, NG, false, SPT>(h, sp, p, nullptr, M, c, nsteps, s, lo, hi);
     if (fg) {
-        if (p->form == 1) return launch_step_inst<T, S, 2, NG, true, SPT>(h, sp, p, fg, M, c, nsteps, s);
-        return launch_step_inst<T, S, 0, NG, true, SPT>(h, sp, p, fg, M, c, nsteps, s);
+        if (p->form == 1) return launch_step_inst<T, S, 2, NG, true, SPT>(h, sp, p, fg, M, c, nsteps, s, lo, hi);
+        return launch_step_inst<T, S, 0, NG, true, SPT>(h, sp, p, fg, M, c, nsteps, s, lo, hi);
     }
-    if (p->form == 1) return launch_step_inst<T, S, 2, NG, false, SPT>(h, sp, p, nullptr, M, c, nsteps, s);
-    return launch_step_inst<T, S, 0, NG, false, SPT>(h, sp, p, nullptr, M, c, nsteps, s);
+    if (p->form == 1) return launch_step_inst<T, S, 2, NG, false, SPT>(h, sp, p, nullptr, M, c, nsteps, s, lo, hi);
+    return launch_step_inst<T, S, 0, NG, false, SPT>(h, sp, p, nullptr, M, c, nsteps, s, lo, hi);
 }
 
+// The tiles of a launch run in rounds of one tile per SM.  When the last round would fill at most half of the SMs,
+// its systems go to a SECOND launch in tiles of half the width instead (twice the CTAs, each about half the time of a
+// full tile): cfg4's 512 tiles of 16 systems are 3 full rounds on 148 SMs plus 68 tiles, i.e. 4 rounds; as 444 tiles
+// of 16 and 136 tiles of 8 they are 3 rounds plus one short one.  The tile width does not enter the arithmetic of a
+// system, so the result does not depend on the split.
 int launch_step_chunked(const pent_handle* h, const pent_step_params* p, const pent_forcing* fg, int64_t M, void* c,
                         int nsteps, cudaStream_t s)
 {
     const StepPlan sp = step_auto_plan(h, M, c);
     if (!sp.ok) return PENT_ERR_ARG;
-    if (h->dtype == PENT_F64) {
-        if (sp.SPT == 2) return launch_step_kind<double, 16, 1, 2>(h, sp, p, fg, M, c, nsteps, s);
-        return launch_step_kind<double, 16, 1, 1>(h, sp, p, fg, M, c, nsteps, s);
+    int64_t split = M;                       // systems [0, split) in full tiles, [split, M) in half-width tiles
+    StepPlan half;
+    if (sp.SPT == 2 && sp.NG == 1) {
+        static const int no_split = []() { const char* e = std::getenv("PENT_AB_STEP_NOSPLIT"); return e ? std::atoi(e) : 0; }();
+        int dev = 0, nsm = 0;
+        PENT_CUDA(cudaGetDevice(&dev));
+        PENT_CUDA(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+        const int64_t ntiles = (M + sp.S - 1) / sp.S, rem = ntiles % nsm;
+        if (!no_split && ntiles > nsm && rem > 0 && 2 * rem <= nsm) {
+            half = step_plan(h, M, c, sp.S / 2, 1, 2);
+            if (half.ok) split = (ntiles - rem) * sp.S;
+        }
     }
-    if (sp.SPT == 2) return launch_step_kind<float, 32, 1, 2>(h, sp, p, fg, M, c, nsteps, s);
-    if (sp.NG == 2) return launch_step_kind<float, 16, 2, 1>(h, sp, p, fg, M, c, nsteps, s);
-    return launch_step_kind<float, 32, 1, 1>(h, sp, p, fg, M, c, nsteps, s);
+    int rc = PENT_OK;
+    if (h->dtype == PENT_F64) {
+        if (sp.SPT == 2) {
+            rc = launch_step_kind<double, 16, 1, 2>(h, sp, p, fg, M, c, nsteps, s, 0, split);
+            if (rc == PENT_OK && split < M) rc = launch_step_kind<double, 8, 1, 2>(h, half, p, fg, M, c, nsteps, s, split, M);
+            return rc;
+        }
+        return launch_step_kind<double, 16, 1, 1>(h, sp, p, fg, M, c, nsteps, s, 0, M);
+    }
+    if (sp.SPT == 2) {
+        rc = launch_step_kind<float, 32, 1, 2>(h, sp, p, fg, M, c, nsteps, s, 0, split);
+        if (rc == PENT_OK && split < M) rc = launch_step_kind<float, 16, 1, 2>(h, half, p, fg, M, c, nsteps, s, split, M);
+        return rc;
+    }
+    if (sp.NG == 2) return launch_step_kind<float, 16, 2, 1>(h, sp, p, fg, M, c, nsteps, s, 0, M);
+    return launch_step_kind<float, 32, 1, 1>(h, sp, p, fg, M, c, nsteps, s, 0, M);
 }
 }  // namespace pent

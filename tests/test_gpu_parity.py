@@ -226,13 +226,16 @@ def _shape_case(N, M, Q, S, dtype=torch.float64, sigma=None, seed=70):
     (1024, 2048 + 32, 2, 32), (1024, 512, 4, 32), (1024, 512, 2, 16), (512, 1000, 1, 32), (512, 992, 2, 32),
     (2048, 520, 2, 16), (2048, 512, 4, 32), (4096, 304, 4, 16), (4096, 512, 8, 32), (6000, 64, 8, 16), (8192, 48, 8, 16), (64, 32, 2, 16),
     (1000, 200, 2, 32), (3000, 100, 4, 16), (700, 96, 2, 16), (96, 40, 2, 16), (65, 34, 2, 32), (5000, 48, 8, 16),
+    # 16 CTAs per cluster (non-portable size): N up to 16384 fp64 on chip; ragged N, ragged M, a rank with no rows
+    (16384, 40, 16, 16), (12000, 33, 16, 16), (8192, 64, 16, 32), (15000, 16, 16, 16), (9000, 48, 16, 16),
 ])
 def test_chunked_shapes_nonsymmetric_fp64(N, M, Q, S):
     _shape_case(N, M, Q, S)
 
 
 @pytest.mark.parametrize("N,M,Q,S", [(1024, 2048 + 64, 2, 64), (1024, 1024, 1, 32), (512, 640, 1, 64),
-                                     (4096, 512, 4, 32), (4096, 256, 8, 64), (3000, 128, 4, 32)])
+                                     (4096, 512, 4, 32), (4096, 256, 8, 64), (3000, 128, 4, 32), (16384, 64, 16, 32),
+                                     (12000, 96, 16, 32)])
 def test_chunked_shapes_fp32(N, M, Q, S):
     _shape_case(N, M, Q, S, dtype=torch.float32, sigma=10.0)
 
@@ -288,7 +291,7 @@ def test_unaligned_pitch_runs_on_chip_with_the_ldg_loader(dtype, N, M):
 
 def test_auto_choice_is_on_chip_for_every_config_shape():
     pent = _pent()
-    for N, M in ((64, 256), (512, 16384), (1024, 65536), (4096, 32768), (2048, 1024), (8192, 512)):
+    for N, M in ((64, 256), (512, 16384), (1024, 65536), (4096, 32768), (2048, 1024), (8192, 512), (16384, 512), (12288, 64)):
         diags = pin.diagonals_I_plus_sigma_L2(N, 1.0)
         a, b, c, d, e = (torch.tensor(v) for v in diags)
         h = pent.pent_factor(N, e, c, d, a, b)
@@ -439,7 +442,8 @@ def _tri_case(N, M, Q, S, dtype, rows=False):
 
 @pytest.mark.parametrize("N,M,Q,S", [(1024, 2048 + 32, 2, 32), (1024, 512, 1, 16), (512, 1000, 1, 32), (2048, 520, 2, 16),
                                      (4096, 304, 4, 16), (8192, 48, 8, 16), (64, 32, 2, 16), (1000, 200, 2, 32),
-                                     (3000, 100, 4, 16), (33, 18, 1, 16), (5, 4, 1, 16), (1, 6, 1, 16), (1024, 77, 2, 16)])
+                                     (3000, 100, 4, 16), (33, 18, 1, 16), (5, 4, 1, 16), (1, 6, 1, 16), (1024, 77, 2, 16),
+                                     (16384, 40, 16, 16)])
 def test_tridiagonal_instantiation_shapes_fp64(N, M, Q, S):
     _tri_case(N, M, Q, S, torch.float64)
 
