@@ -380,6 +380,8 @@ def run_ours(args):
         fused = args.kernel == 0 and bool(pent.lib().pent_periodic_fused(h.ptr, M))
         ch = {**pent.kernel_choice(h, M), "kernel": "solve_chunked_kernel" if fused else
               "solve_chunked_kernel + periodic_tail_kernel + periodic_update_kernel"}
+    elif args.layout == "rows" and not (args.cluster and args.tile):
+        ch = pent.rows_kernel_choice(h, M)
     elif args.kernel == 0:
         ch = pent.kernel_choice(h, M)
     elif (args.kernel & 0xff) == 2:

@@ -92,7 +92,7 @@ int pent_solve_batch_v(const pent_handle* h, int64_t M, const void* f, void* x, 
 /* Same operation on a SYSTEM-MAJOR batch: f, x: device, M*N elements, element k of system i at i*N + k
  * ("one system per row", the layout of the paper's serial code; it is also what an ADI
  * sweep along the contiguous axis of a 2-D field needs: the sweep along the other axis is
- * pent_solve_batch itself).  x == f allowed.  Shared-A, non-periodic handles with N <= 8192 (fp64);
+ * pent_solve_batch itself).  x == f allowed.  Shared-A, non-periodic handles with N <= 16384;
  * PENT_ERR_ARG otherwise.  Every thread reads and writes one contiguous run of 32 (fp64) / 64 (fp32)
  * elements with 32-byte accesses (16-byte aligned runs fall back to narrower ones): 2 passes over the
  * batch, no transpose. */
@@ -105,6 +105,9 @@ int pent_solve_batch_rows(const pent_handle* h, int64_t M, const void* f, void* 
 #define PENT_ROWS_STG   (1 << 25)   /* bulk loads, 32-byte STG stores */
 #define PENT_ROWS_TMA2D (1 << 26)   /* swizzled tensor-tile TMA loads (128-byte rows), 32-byte STG stores (A/B baseline) */
 int pent_solve_batch_rows_v(const pent_handle* h, int64_t M, const void* f, void* x, void* stream, int kernel);
+/* What pent_solve_batch_rows runs for M systems: PENT_KERNEL_CHUNKED_CFG(Q, S) | (data path << 24), data path 6 = bulk
+ * copies both ways, 5 = bulk loads + STG stores, 3 = swizzled TMA loads, 2 = per-thread LDG / STG; -1 if unsupported. */
+int pent_solve_rows_kernel_choice(const pent_handle* h, int64_t M);
 
 /* Same operation with HOST buffers (pageable or pinned): copies slabs of systems to the device,
  * solves, copies back, pipelined on internal streams; returns when x_host is complete.

@@ -31,6 +31,16 @@ def kernel_choice(h: "Handle", M: int) -> dict:
     if (v & 0xff) == KERNEL_CHUNKED:
         return {"kernel": "solve_chunked_kernel", "Q": (v >> 8) & 0xff, "S": (v >> 16) & 0xff}
     return {"kernel": "solve_tps_kernel", "Q": 0, "S": 0}
+def rows_kernel_choice(h: "Handle", M: int) -> dict:
+    """What pent_solve_batch_rows runs for M systems: cluster size, tile width and data path."""
+    v = lib().pent_solve_rows_kernel_choice(h.ptr, M)
+    if v < 0:
+        return {"kernel": None, "Q": 0, "S": 0, "path": None}
+    path = {6: "1-D bulk copies both ways", 5: "bulk loads + STG.256 stores", 3: "swizzled TMA loads + STG.256 stores",
+            2: "LDG.256 / STG.256"}.get(v >> 24, str(v >> 24))
+    return {"kernel": "solve_chunked_kernel", "Q": (v >> 8) & 0xff, "S": (v >> 16) & 0xff, "path": path}
+
+
 _ERR = {1: "invalid argument", 2: "zero or non-finite pivot", 3: "CUDA error", 4: "allocation failure"}
 
 _lib = None
@@ -101,6 +111,7 @@ def lib() -> C.CDLL:
     L.pent_release_thread_cache.restype = None
     L.pent_handle_factors.argtypes = [vp] * 6
     L.pent_solve_kernel_choice.argtypes = [vp, i64]
+    L.pent_solve_rows_kernel_choice.argtypes = [vp, i64]
     L.pent_launch_count.argtypes = [ci]
     L.pent_launch_count.restype = i64
     L.pent_version.restype = C.c_char_p

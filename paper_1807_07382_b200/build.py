@@ -65,5 +65,19 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def build_ubench() -> str:
+    """The standalone microbenchmark of csrc/pent_ubench.cu (FP64 FMA, shared-memory load and shuffle rates)."""
+    out = os.path.join(PKG, "pent_ubench")
+    r = subprocess.run([nvcc_path(), "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a",
+                        "-o", out, os.path.join(CSRC, "pent_ubench.cu")], capture_output=True, text=True)
+    if r.returncode != 0:
+        sys.stderr.write(r.stdout + r.stderr)
+        raise RuntimeError("nvcc failed building pent_ubench")
+    return out
+
+
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    if "--ubench" in sys.argv:
+        print(build_ubench())
+    else:
+        print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

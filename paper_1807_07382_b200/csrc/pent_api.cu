@@ -63,6 +63,14 @@ extern "C" int pent_solve_kernel_choice(const pent_handle* h, int64_t M)
     return PENT_KERNEL_CHUNKED_CFG(Q, S);
 }
 
+extern "C" int pent_solve_rows_kernel_choice(const pent_handle* h, int64_t M)
+{
+    if (!h || h->kind != 0 || h->periodic) return -1;
+    int Q = 0, S = 0, mode = 0;
+    if (!pent::chunked_rows_choice(h, M, &Q, &S, &mode)) return -1;
+    return PENT_KERNEL_CHUNKED_CFG(Q, S) | (mode << 24);
+}
+
 extern "C" int pent_solve_batch(const pent_handle* h, int64_t M, const void* f, void* x,
                                 void* stream)
 {

@@ -143,5 +143,6 @@ bool chunked_rows_supported(const pent_handle* h, int64_t M);
 int launch_solve_chunked_rows(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s,
                               int Q = 0, int S = 0, int loader = 0);
 int chunked_choice(const pent_handle* h, int64_t M, int* Q, int* S);   // 1 and the default plan, or 0
+int chunked_rows_choice(const pent_handle* h, int64_t M, int* Q, int* S, int* mode);   // the same for a system-major batch
 
 }  // namespace pent

@@ -664,6 +664,14 @@ static ChunkPlan rows_plan(const pent_handle* h, int64_t M, const void* f, const
 
 bool chunked_rows_supported(const pent_handle* h, int64_t M) { return rows_plan(h, M, nullptr, nullptr, 0, 0, 0).ok; }
 
+int chunked_rows_choice(const pent_handle* h, int64_t M, int* Q, int* S, int* mode)
+{
+    const ChunkPlan pl = rows_plan(h, M, nullptr, nullptr, 0, 0, 0);
+    if (!pl.ok) return 0;
+    *Q = pl.Q; *S = pl.S; *mode = pl.mode;
+    return 1;
+}
+
 static int launch_plan(const pent_handle* h, const ChunkPlan& pl, int64_t M, const void* f, void* x, cudaStream_t s);
 
 int launch_solve_chunked_rows(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s,
