@@ -46,6 +46,11 @@ struct pent_handle {
     void* pz[PENT_NQ];   // Z rows per cluster rank for the fused kernel: [Q][Pl*C] x {z0, z1} in T (0: not built)
     void* dgp;
     double pc[10];
+    // on-chip periodic time step (pent_step_chunked.cu): per chunk of C rows (Q = 1 chunking) the chunk states of the
+    // Z solve, [P][8] in T = {g^Z of rows s-2, s-1 | Z of rows e+1, e+2} x 2 columns (zero for the first and last
+    // chunk), and the explicit rows of Z of the first and the last chunk, [2][C] x {z0, z1} in T
+    void* pfold;
+    void* pzedge;
     // ---- per-system factors, device, interleaved, in T ----
     void* ms;            // 5*N*M: ia, en, bn, gamma, delta
 };
@@ -139,6 +144,8 @@ bool periodic_fused_supported(const pent_handle* h, int64_t M, const void* f /* 
 int launch_solve_chunked_periodic(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s);
 int solve_periodic(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s, int kernel);
 int step_periodic(const pent_handle* h, int64_t M, void* c, void* scratch, int nsteps, cudaStream_t s);
+bool step_chunked_periodic_supported(const pent_handle* h, int64_t M, const void* c /* may be null */);
+int launch_step_chunked_periodic(const pent_handle* h, int64_t M, void* c, int nsteps, cudaStream_t s);
 bool chunked_rows_supported(const pent_handle* h, int64_t M);
 int launch_solve_chunked_rows(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s,
                               int Q = 0, int S = 0, int loader = 0);

@@ -11,6 +11,7 @@
 // which is Eq. 11-12 with E^{-1} applied to f^ first: h^T E^{-1} f^ = h^T y, E^{-1} k = Z.
 // In the interleaved layout the first N-2 rows of a batch ARE an interleaved (N-2) x M batch,
 // so the inner solve needs no copy.
+#include <cstdlib>
 #include <new>
 #include "pent_chunk_common.cuh"
 
@@ -18,8 +19,11 @@ namespace pent {
 
 // thread j < 2: z_j = E^{-1} k_j by the paper's sweeps (true divisions, fp64); then thread 0:
 // S2 = C2 - h^T Z, out[0..5] = h entries, out[6..9] = S2^{-1} row-major, status = 0 / 1 (singular)
+// G (2 x n): the forward-sweep intermediates g = L^{-1} k of the two solves (the chunk states of the Z solve, needed by
+// the on-chip periodic time step)
 __global__ void periodic_setup_kernel(int N, const double* __restrict__ fac, const double* __restrict__ dg,
-                                      double* __restrict__ Z, double* __restrict__ out, int* __restrict__ status)
+                                      double* __restrict__ Z, double* __restrict__ G, double* __restrict__ out,
+                                      int* __restrict__ status)
 {
     const int n = N - 2, j = threadIdx.x;
     const double *a = dg, *b = dg + N, *c = dg + 2 * N, *d = dg + 3 * N, *e = dg + 4 * N;
@@ -33,7 +37,7 @@ __global__ void periodic_setup_kernel(int N, const double* __restrict__ fac, con
         double g1 = 0.0, g2 = 0.0;
         for (int i = 0; i < n; ++i) {
             double g = __ddiv_rn(z[i] - eps[i] * g2 - beta[i] * g1, alpha[i]);
-            z[i] = g; g2 = g1; g1 = g;
+            z[i] = g; G[(size_t)j * n + i] = g; g2 = g1; g1 = g;
         }
         double x1 = 0.0, x2 = 0.0;
         for (int i = n - 1; i >= 0; --i) {
@@ -85,6 +89,34 @@ __global__ void periodic_zslices_kernel(int n, int rows_total, const double* __r
     z.x = k < n ? (T)Z[k] : (T)0;
     z.y = k < n ? (T)Z[n + k] : (T)0;
     out[k] = z;
+}
+
+// On-chip periodic time step: x^ = y - Z t without the rows of Z in shared memory.  Inside an interior chunk Z is a
+// homogeneous solution of the two recurrences, Z_rows = chi F^Z_{p-1} + psi B^Z_{p+1}, so  y - Z t  is the usual
+// correction with the chunk states F - F^Z t, B - B^Z t.  fold[p] = {g^Z_0, g^Z_1 of row s-2 | of row s-1 | Z_0, Z_1 of
+// row e+1 | of row e+2} (s = pC, e = s+C-1; zero outside 0..n-1, and all zero for the first and the last chunk, which
+// hold the non-zero rows of k and subtract their explicit rows of Z instead: zedge[0][j], zedge[1][j]).
+template <typename T>
+__global__ void periodic_fold_kernel(int n, int P, const double* __restrict__ Z, const double* __restrict__ G,
+                                     T* __restrict__ fold, typename Vec<T>::T2* __restrict__ zedge)
+{
+    constexpr int C = ChunkCfg<T>::C;
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p < P) {
+        const int s = p * C, e = s + C - 1;
+        const bool edge = p == 0 || p == P - 1;
+        auto at = [&](const double* v, int col, int k) -> T { return (!edge && k >= 0 && k < n) ? (T)v[(size_t)col * n + k] : (T)0; };
+        T* o = fold + 8 * (size_t)p;
+        o[0] = at(G, 0, s - 2); o[1] = at(G, 1, s - 2); o[2] = at(G, 0, s - 1); o[3] = at(G, 1, s - 1);
+        o[4] = at(Z, 0, e + 1); o[5] = at(Z, 1, e + 1); o[6] = at(Z, 0, e + 2); o[7] = at(Z, 1, e + 2);
+    }
+    if (p < 2 * C) {
+        const int which = p / C, j = p % C, k = (which == 0 ? 0 : (P - 1) * C) + j;
+        typename Vec<T>::T2 z;
+        z.x = k < n ? (T)Z[k] : (T)0;
+        z.y = k < n ? (T)Z[(size_t)n + k] : (T)0;
+        zedge[p] = z;
+    }
 }
 
 template <typename T>
@@ -213,6 +245,10 @@ static int step_periodic_t(const pent_handle* h, int64_t M, void* c, void* scrat
 
 int step_periodic(const pent_handle* h, int64_t M, void* c, void* scratch, int nsteps, cudaStream_t s)
 {
+    // default: the whole loop in ONE launch with the state on chip (pent_step_chunked.cu); otherwise one right-hand-side
+    // kernel and one fused periodic solve per step
+    static const int two_kernels = []() { const char* e = std::getenv("PENT_AB_PERIODIC_STEP_UNFUSED"); return e ? std::atoi(e) : 0; }();
+    if (!two_kernels && step_chunked_periodic_supported(h, M, c)) return launch_step_chunked_periodic(h, M, c, nsteps, s);
     if (h->dtype == PENT_F64) return step_periodic_t<double>(h, M, c, scratch, nsteps, s);
     return step_periodic_t<float>(h, M, c, scratch, nsteps, s);
 }
@@ -231,7 +267,7 @@ static int factor_periodic_t(int N, const void* const src[5], pent_dtype dtype, 
     // Everything runs on the private non-blocking stream `s`; temporaries are stream-ordered allocations.
     const int n = N - 2;
     T* stage = nullptr;
-    double *dg64 = nullptr, *Z = nullptr, *coef = nullptr;
+    double *dg64 = nullptr, *Z = nullptr, *G = nullptr, *coef = nullptr;
     int* status = nullptr;
     pent_handle* h = new (std::nothrow) pent_handle();
     if (!h) return PENT_ERR_ALLOC;
@@ -243,6 +279,7 @@ static int factor_periodic_t(int N, const void* const src[5], pent_dtype dtype, 
         if (stage) cudaFreeAsync(stage, s);
         if (dg64) cudaFreeAsync(dg64, s);
         if (Z) cudaFreeAsync(Z, s);
+        if (G) cudaFreeAsync(G, s);
         if (coef) cudaFreeAsync(coef, s);
         if (status) cudaFreeAsync(status, s);
         cudaStreamSynchronize(s);
@@ -262,7 +299,7 @@ static int factor_periodic_t(int N, const void* const src[5], pent_dtype dtype, 
         return true;
     };
     if (!alloc_tmp((void**)&stage, sizeof(T) * 5 * (size_t)N) || !alloc_tmp((void**)&dg64, sizeof(double) * 5 * (size_t)N) ||
-        !alloc_tmp((void**)&Z, sizeof(double) * 2 * (size_t)n) || !alloc_tmp((void**)&coef, sizeof(double) * 10) ||
+        !alloc_tmp((void**)&Z, sizeof(double) * 2 * (size_t)n) || !alloc_tmp((void**)&G, sizeof(double) * 2 * (size_t)n) || !alloc_tmp((void**)&coef, sizeof(double) * 10) ||
         !alloc_tmp((void**)&status, sizeof(int)) || !alloc(&h->Zt, sizeof(T) * 2 * (size_t)n) ||
         !alloc(&h->dgp, sizeof(T) * 8 * (size_t)N))
         return done(rc);
@@ -279,7 +316,7 @@ static int factor_periodic_t(int N, const void* const src[5], pent_dtype dtype, 
     h->inner->band = 2;               // the fused periodic kernel reads the pentadiagonal tables
     const int tb = 128, nb = (N + tb - 1) / tb;
     periodic_tables_kernel<T><<<nb, tb, 0, s>>>(N, stage, nullptr, nullptr, (T*)h->dgp, dg64);
-    periodic_setup_kernel<<<1, 32, 0, s>>>(N, h->inner->fac, dg64, Z, coef, status);
+    periodic_setup_kernel<<<1, 32, 0, s>>>(N, h->inner->fac, dg64, Z, G, coef, status);
     periodic_tables_kernel<T><<<nb, tb, 0, s>>>(N, stage, Z, (typename Vec<T>::T2*)h->Zt, (T*)h->dgp, nullptr);
     count_launch(3);
     for (int j = 0; j < PENT_NQ; ++j) {
@@ -288,6 +325,12 @@ static int factor_periodic_t(int N, const void* const src[5], pent_dtype dtype, 
         const int rows_total = (1 << j) * Pl * ChunkCfg<T>::C;
         if (!alloc(&h->pz[j], sizeof(T) * 2 * (size_t)rows_total)) return done(rc);
         periodic_zslices_kernel<T><<<(rows_total + tb - 1) / tb, tb, 0, s>>>(n, rows_total, Z, (typename Vec<T>::T2*)h->pz[j]);
+        count_launch();
+    }
+    if (N % ChunkCfg<T>::C == 0 && h->inner->cfP[0] == N / ChunkCfg<T>::C) {      // tables of the on-chip time step
+        const int P = N / ChunkCfg<T>::C, C2 = 2 * ChunkCfg<T>::C, nt = P > C2 ? P : C2;
+        if (!alloc(&h->pfold, sizeof(T) * 8 * (size_t)P) || !alloc(&h->pzedge, sizeof(T) * 2 * (size_t)C2)) return done(rc);
+        periodic_fold_kernel<T><<<(nt + tb - 1) / tb, tb, 0, s>>>(n, P, Z, G, (T*)h->pfold, (typename Vec<T>::T2*)h->pzedge);
         count_launch();
     }
     cudaError_t le = cudaGetLastError();

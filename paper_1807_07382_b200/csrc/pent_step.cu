@@ -193,6 +193,6 @@ extern "C" int pent_step_batch(const pent_handle* h, const pent_step_params* p, 
 extern "C" int pent_step_kernel_choice(const pent_handle* h, int64_t M)
 {
     if (!h || h->kind != 0) return -1;
-    if (h->periodic) return PENT_KERNEL_THREAD_PER_SYSTEM;
+    if (h->periodic) return pent::step_chunked_periodic_supported(h, M, nullptr) ? PENT_KERNEL_CHUNKED : PENT_KERNEL_THREAD_PER_SYSTEM;
     return pent::step_chunked_supported(h, M, nullptr) ? PENT_KERNEL_CHUNKED : PENT_KERNEL_THREAD_PER_SYSTEM;
 }

@@ -13,7 +13,10 @@
 //
 //  kind 0  Cahn-Hilliard:  form 0  A c+ = c + r L (c^3 - c)
 //                          form 1  q = r (c^3 - c) - sigma L c ;  A delta = L q ;  c+ = c + delta
-//  kind 1  hyperdiffusion Crank-Nicolson:  A c+ = (2I - A) c   (diagonals read from the handle)
+//  kind 1  hyperdiffusion Crank-Nicolson:  A c+ = (2I - A) c, evaluated as c+ = 2 A^{-1} c - c (no stencil at all)
+//          KIND 3 = the same on a PERIODIC handle (the paper's own loop): wrap-around halo rows, the
+//          chunked solve of the (N-2) x (N-2) block E, then the Navon tail t and x^ = y - Z t with Z folded into the
+//          chunk states (periodic_fold_kernel in pent_periodic.cu); N a multiple of the chunk length
 //  (L v)_k = v_{k-1} + dg_k v_k + v_{k+1}, out-of-range terms dropped; dg_k = -2 except
 //  dg_0 = dg_{N-1} = -1 when bc = 1 (zero-flux).  Same formulas, in the same order, as
 //  step_tps_kernel (pent_step.cu).
@@ -38,6 +41,11 @@ struct StepChunkParams {
     const T* mu2;
     double dt, t0;
     ScanOffsets so;       // chunk-state scan: uniform byte offsets of the transfer matrices (SPT > 1)
+    // periodic handle (KIND 3; Eqs. 8-12): chunk states of the Z solve, explicit Z rows of the first and last
+    // chunk, the six entries of h and the inverted 2 x 2 Schur complement
+    const T* pfold;
+    const typename Vec<T>::T2* pzedge;
+    T ph[6], pi[4];
 };
 
 // Barrier of one thread group of a CTA (named barrier 1+g); the whole CTA when there is one group.
@@ -125,7 +133,9 @@ step_chunked_kernel(const __grid_constant__ CUtensorMap tm, const StepChunkParam
         }
     }
     const T r = prm.r, sigma = prm.sigma;
-    constexpr bool incr = (KIND == 2);       // KIND: 0 CH direct form, 2 CH increment form, 1 hyperdiffusion
+    constexpr bool incr = (KIND == 2);       // KIND: 0 CH direct form, 2 CH increment form, 1 hyperdiffusion, 3 periodic
+    constexpr bool PER = (KIND == 3);
+    static_assert(!PER || SPT == 2, "the periodic step is built on the two-systems-per-thread shape");
     const T dg_edge = (prm.bc == 1) ? (T)-1 : (T)-2;
     auto ldc = [&](T (&o)[SPT], int k) {
         if ((unsigned)k < (unsigned)N) lds_sys<T, SPT>(o, cs + (size_t)k * S);
@@ -140,8 +150,9 @@ step_chunked_kernel(const __grid_constant__ CUtensorMap tm, const StepChunkParam
     // is the straggler every block barrier waits for.
     const bool first = row0 == 0, last = row0 + C == N;
     const T dfirst = first ? dg_edge : (T)-2, dlast = last ? dg_edge : (T)-2;
-    const bool interior = __all_sync(0xffffffffu, active && (first || row0 >= 2) && (last || row0 + C + 2 <= N - 1) &&
-                                                      C >= 4 && N >= 2 * C);
+    // (lanes beyond the last chunk execute neither path: they do not vote it down)
+    const bool interior = __all_sync(0xffffffffu, !active || ((first || row0 >= 2) && (last || row0 + C + 2 <= N - 1) &&
+                                                              C >= 4 && N >= 2 * C));
     uint32_t parity = 0;
 
     for (int64_t tile = prm.tile0 + (int64_t)blockIdx.x * NG + grp_id; tile < prm.ntiles; tile += (int64_t)gridDim.x * NG) {
@@ -188,7 +199,7 @@ step_chunked_kernel(const __grid_constant__ CUtensorMap tm, const StepChunkParam
             T v[SPT][C];
             if (active) {
                 // ---- explicit right-hand side of rows row0 .. row0+C-1, in registers ----
-                if constexpr (KIND != 1) {
+                if constexpr (KIND == 0 || KIND == 2) {
                     // u_k = w_k = c_k^3 - c_k (form 0) or q_k = r w_k - sigma (L c)_k (form 1), 0 outside 0..N-1
                     if (interior) {
                         // Interior chunk, or the first / last chunk of a system whose length is a multiple
@@ -268,66 +279,27 @@ step_chunked_kernel(const __grid_constant__ CUtensorMap tm, const StepChunkParam
                             }
                         }
                     }
-                } else if (interior) {
-                    // (2I - A) c, rows row0 .. row0+C-1 all inside the matrix (see `interior` above); the
-                    // entries of the diagonals that fall outside the matrix are zero in prm.dg
-                    const T* cw = cs + (size_t)row0 * S;
-                    T cm2[SPT], cm1[SPT], c0[SPT], cp1[SPT], cp2[SPT];
-                    if (first) {
-#pragma unroll
-                        for (int u = 0; u < SPT; ++u) { cm2[u] = 0; cm1[u] = 0; }
-                    } else {
-                        lds_sys<T, SPT>(cm2, cw - 2 * S);
-                        lds_sys<T, SPT>(cm1, cw - S);
-                    }
-                    lds_sys<T, SPT>(c0, cw);
-                    lds_sys<T, SPT>(cp1, cw + S);
-                    const T* dk = prm.dg + 8 * (size_t)row0;
-#pragma unroll
-                    for (int j = 0; j < C; ++j) {
-                        if (j + 2 < C || !last) lds_sys<T, SPT>(cp2, cw + (size_t)(j + 2) * S);
-                        else {
-#pragma unroll
-                            for (int u = 0; u < SPT; ++u) cp2[u] = (T)0;
-                        }
-                        const T da = __ldg(dk + 8 * j + 0), db = __ldg(dk + 8 * j + 1), dc = __ldg(dk + 8 * j + 2),
-                                dd = __ldg(dk + 8 * j + 3), de = __ldg(dk + 8 * j + 4);
-#pragma unroll
-                        for (int u = 0; u < SPT; ++u) {
-                            T s = dc * c0[u];
-                            s = fma(db, cm1[u], s);
-                            s = fma(da, cm2[u], s);
-                            s = fma(dd, cp1[u], s);
-                            s = fma(de, cp2[u], s);
-                            v[u][j] = (T)2 * c0[u] - s;
-                            cm2[u] = cm1[u]; cm1[u] = c0[u]; c0[u] = cp1[u]; cp1[u] = cp2[u];
-                        }
-                    }
                 } else {
-                    T cm2[SPT], cm1[SPT], c0[SPT], cp1[SPT], cp2[SPT];
-                    ldc(cm2, row0 - 2); ldc(cm1, row0 - 1); ldc(c0, row0); ldc(cp1, row0 + 1);
+                    // Crank-Nicolson hyperdiffusion, A c+ = (2I - A) c (Eq. 6 / 7c), evaluated as  c+ = 2 A^{-1} c - c
+                    // (A^{-1} (2I - A) = 2 A^{-1} - I): the right-hand side of the solve is the state itself -- no stencil,
+                    // no halo rows, none of the matrix's diagonals (which would have to come from L2: shared memory is
+                    // full) -- and the write-back below forms 2 y - c.  Same scheme, another order of evaluation.
+                    const T* cw = cs + (size_t)row0 * S;
+                    if (row0 + C <= N) {
 #pragma unroll
-                    for (int j = 0; j < C; ++j) {
-                        const int k = row0 + j;
-                        ldc(cp2, k + 2);
-                        T da = 0, db = 0, dc = 0, dd = 0, de = 0;
-                        if (k < N) {
-                            const T* dk = prm.dg + 8 * (size_t)k;
-                            da = __ldg(dk + 0); db = __ldg(dk + 1); dc = __ldg(dk + 2); dd = __ldg(dk + 3); de = __ldg(dk + 4);
+                        for (int j = 0; j < C; ++j) {
+                            T cj[SPT];
+                            lds_sys<T, SPT>(cj, cw + (size_t)j * S);
+#pragma unroll
+                            for (int u = 0; u < SPT; ++u) v[u][j] = cj[u];
                         }
+                    } else {
 #pragma unroll
-                        for (int u = 0; u < SPT; ++u) {
-                            T rhs = 0;
-                            if (k < N) {
-                                T s = dc * c0[u];
-                                s = fma(db, cm1[u], s);
-                                s = fma(da, cm2[u], s);
-                                s = fma(dd, cp1[u], s);
-                                s = fma(de, cp2[u], s);
-                                rhs = (T)2 * c0[u] - s;
-                            }
-                            v[u][j] = rhs;
-                            cm2[u] = cm1[u]; cm1[u] = c0[u]; c0[u] = cp1[u]; cp1[u] = cp2[u];
+                        for (int j = 0; j < C; ++j) {
+                            T cj[SPT];
+                            ldc(cj, row0 + j);
+#pragma unroll
+                            for (int u = 0; u < SPT; ++u) v[u][j] = cj[u];
                         }
                     }
                 }
@@ -349,7 +321,7 @@ step_chunked_kernel(const __grid_constant__ CUtensorMap tm, const StepChunkParam
                         }
                     }
                 }
-                // ---- chunked solve, stages 1+2 ----
+                // ---- chunked solve, stages 1+2 ----  (periodic: of the block E; its rows N-2, N-1 have zero coefficients)
                 T2 e[SPT], s[SPT];
                 chunk_local_sweeps_n<T, SPT>(v, blk, e, s);
 #pragma unroll
@@ -371,26 +343,94 @@ step_chunked_kernel(const __grid_constant__ CUtensorMap tm, const StepChunkParam
                 }
             }
             group_sync<NG>(grp_id, TG);
+            T F0[SPT], F1[SPT], B0[SPT], B1[SPT];
             if (active) {
-                T F0[SPT], F1[SPT], B0[SPT], B1[SPT];
 #pragma unroll
                 for (int u = 0; u < SPT; ++u) {
                     F0[u] = 0; F1[u] = 0; B0[u] = 0; B1[u] = 0;
                     if (P > 1) { T2 fo = stE[slot[u]]; F0[u] = fo.x; F1[u] = fo.y; T2 bo = stS[slot[u]]; B0[u] = bo.x; B1[u] = bo.y; }
                 }
+                if constexpr (PER) {
+                    // the first chunk publishes (y_0, y_1), the last one (y_{n-2}, y_{n-1}) (its rows C-4, C-3), each into
+                    // its OWN stE slot (already read above; nobody else reads it before the barrier below)
+                    if (first || last) {
+                        const T* cr = blk + 5 * C + 4 * (first ? 0 : C - 4);
+#pragma unroll
+                        for (int u = 0; u < SPT; ++u) {
+                            const T xa = first ? v[u][0] : v[u][C - 4], xb = first ? v[u][1] : v[u][C - 3];
+                            T2 y;
+                            y.x = fma(cr[3], B1[u], fma(cr[2], B0[u], fma(cr[1], F1[u], fma(cr[0], F0[u], xa))));
+                            y.y = fma(cr[7], B1[u], fma(cr[6], B0[u], fma(cr[5], F1[u], fma(cr[4], F0[u], xb))));
+                            stE[slot[u]] = y;
+                        }
+                        if (last) {   // ... and the right-hand side of the two tail rows, (c_{N-2}, c_{N-1}), into its stS slot
+                            T fa[SPT], fb[SPT];
+                            lds_sys<T, SPT>(fa, cs + (size_t)(N - 2) * S);
+                            lds_sys<T, SPT>(fb, cs + (size_t)(N - 1) * S);
+#pragma unroll
+                            for (int u = 0; u < SPT; ++u) { T2 ft; ft.x = fa[u]; ft.y = fb[u]; stS[slot[u]] = ft; }
+                        }
+                    }
+                }
+            }
+            T t0[SPT], t1[SPT];
+            if constexpr (PER) {
+                group_sync<NG>(grp_id, TG);
+                if (active) {
+                    // t = S2^{-1} [ (f_{N-2}, f_{N-1}) - h^T y ]  (Eq. 12), redundantly by every thread of the system, then
+                    // Z folded into the chunk states: F - F^Z t, B - B^Z t
+                    T fz[8];
+#pragma unroll
+                    for (int w = 0; w < 8; ++w) fz[w] = __ldg(prm.pfold + 8 * (size_t)p + w);
+#pragma unroll
+                    for (int u = 0; u < SPT; ++u) {
+                        const T2 y0 = stE[state_slot<S>(0, sys0 + u)], yl = stE[state_slot<S>(P - 1, sys0 + u)];
+                        const T2 ft = stS[state_slot<S>(P - 1, sys0 + u)];
+                        const T r0 = ft.x - fma(prm.ph[2], yl.y, fma(prm.ph[1], yl.x, prm.ph[0] * y0.x));
+                        const T r1 = ft.y - fma(prm.ph[5], yl.y, fma(prm.ph[4], y0.y, prm.ph[3] * y0.x));
+                        t0[u] = fma(prm.pi[1], r1, prm.pi[0] * r0);
+                        t1[u] = fma(prm.pi[3], r1, prm.pi[2] * r0);
+                        F0[u] = fma(-fz[1], t1[u], fma(-fz[0], t0[u], F0[u]));
+                        F1[u] = fma(-fz[3], t1[u], fma(-fz[2], t0[u], F1[u]));
+                        B0[u] = fma(-fz[5], t1[u], fma(-fz[4], t0[u], B0[u]));
+                        B1[u] = fma(-fz[7], t1[u], fma(-fz[6], t0[u], B1[u]));
+                    }
+                }
+            }
+            if (active) {
                 T* co = cs + (size_t)row0 * S;
 #pragma unroll
                 for (int jg = 0; jg < C / 4; ++jg) {
                     T xv[SPT][4];
                     chunk_correct4_n<T, SPT>(xv, v, blk, jg, F0, F1, B0, B1);
+                    if constexpr (PER) {
+                        if (first || last) {        // the chunks that hold the non-zero rows of k: explicit rows of Z
+#pragma unroll
+                            for (int rr = 0; rr < 4; ++rr) {
+                                const typename Vec<T>::T2 z = __ldg(prm.pzedge + (first ? 0 : C) + 4 * jg + rr);
+#pragma unroll
+                                for (int u = 0; u < SPT; ++u) xv[u][rr] = fma(-z.y, t1[u], fma(-z.x, t0[u], xv[u][rr]));
+                            }
+                        }
+                    }
 #pragma unroll
                     for (int rr = 0; rr < 4; ++rr) {
                         T* o = co + (size_t)(4 * jg + rr) * S;
                         T nv[SPT];
+                        if constexpr (PER) {
+                            if (last && 4 * jg + rr >= C - 2) {      // rows N-2, N-1 of the solution are t (Eq. 12)
+#pragma unroll
+                                for (int u = 0; u < SPT; ++u) xv[u][rr] = (4 * jg + rr == C - 2) ? t0[u] : t1[u];
+                            }
+                        }
                         if (incr) {
                             lds_sys<T, SPT>(nv, o);
 #pragma unroll
                             for (int u = 0; u < SPT; ++u) nv[u] += xv[u][rr];
+                        } else if (KIND == 1 || KIND == 3) {
+                            lds_sys<T, SPT>(nv, o);
+#pragma unroll
+                            for (int u = 0; u < SPT; ++u) nv[u] = fma((T)2, xv[u][rr], -nv[u]);
                         } else {
 #pragma unroll
                             for (int u = 0; u < SPT; ++u) nv[u] = xv[u][rr];
@@ -460,14 +500,17 @@ static StepPlan step_auto_plan(const pent_handle* h, int64_t M, const void* c)
     return step_plan(h, M, c, 32, 1, 1);
 }
 
-// Systems [sys_lo, sys_hi) of the batch (sys_lo a multiple of S) in tiles of S.
+// Systems [sys_lo, sys_hi) of the batch (sys_lo a multiple of S) in tiles of S.  KIND 3: hp = the periodic handle, h = its
+// inner handle (the block E, whose tables the solve stages read); otherwise hp == h.
 template <typename T, int S, int KIND, int NG, bool FORCED, int SPT>
 static int launch_step_inst(const pent_handle* h, const StepPlan& sp, const pent_step_params* p, const pent_forcing* fg,
-                            int64_t M, void* c, int nsteps, cudaStream_t s, int64_t sys_lo, int64_t sys_hi)
+                            int64_t M, void* c, int nsteps, cudaStream_t s, int64_t sys_lo, int64_t sys_hi,
+                            const pent_handle* hp = nullptr)
 {
+    if (!hp) hp = h;
     const ChunkPlan& pl = sp.pl;
     StepChunkParams<T> prm;
-    prm.N = h->N; prm.P = pl.Pl; prm.Pw = pl.Pw; prm.M = M;
+    prm.N = hp->N; prm.P = pl.Pl; prm.Pw = pl.Pw; prm.M = M;
     int lg = 0;
     while ((1 << lg) < pl.Pw) ++lg;
     prm.lev_f = h->lev_f[0] < lg ? h->lev_f[0] : lg;
@@ -479,13 +522,21 @@ static int launch_step_inst(const pent_handle* h, const StepPlan& sp, const pent
     prm.ntiles = (sys_hi + S - 1) / S;
     prm.table = (const T*)h->cf[0];
     prm.table_bytes = (uint32_t)pl.table_bytes;
-    prm.dg = (const T*)h->dg;
+    prm.dg = (const T*)(KIND == 3 ? hp->dgp : h->dg);
     prm.nsteps = nsteps; prm.bc = p->bc;
     prm.r = (T)p->r; prm.sigma = (T)p->sigma;
+    prm.pfold = nullptr; prm.pzedge = nullptr;
+    for (int w = 0; w < 6; ++w) prm.ph[w] = (T)0;
+    for (int w = 0; w < 4; ++w) prm.pi[w] = (T)0;
+    if (KIND == 3) {
+        prm.pfold = (const T*)hp->pfold; prm.pzedge = (const typename Vec<T>::T2*)hp->pzedge;
+        for (int w = 0; w < 6; ++w) prm.ph[w] = (T)hp->pc[w];
+        for (int w = 0; w < 4; ++w) prm.pi[w] = (T)hp->pc[6 + w];
+    }
     prm.mu1 = prm.mu2 = nullptr; prm.dt = prm.t0 = 0.0;
     if (FORCED) { prm.mu1 = (const T*)fg->mu1; prm.mu2 = (const T*)fg->mu2; prm.dt = fg->dt; prm.t0 = fg->t0; }
     CUtensorMap tm;
-    if (!encode_batch_map_cached(&tm, c, M, h->N, S, prm.box_rows, sizeof(T) == 8)) {
+    if (!encode_batch_map_cached(&tm, c, M, hp->N, S, prm.box_rows, sizeof(T) == 8)) {
         g_last_cuda_error = (int)cudaErrorInvalidValue;
         return PENT_ERR_CUDA;
     }
@@ -564,5 +615,52 @@ int launch_step_chunked(const pent_handle* h, const pent_step_params* p, const p
     }
     if (sp.NG == 2) return launch_step_kind<float, 16, 2, 1>(h, sp, p, fg, M, c, nsteps, s, 0, M);
     return launch_step_kind<float, 32, 1, 1>(h, sp, p, fg, M, c, nsteps, s, 0, M);
+}
+
+// ---- periodic handles: the paper's own loop with the state on chip, KIND 3 ----------------------------
+// The tile holds all N rows of the state; the solve stages run on the tables of the inner handle (the (N-2) x (N-2)
+// block E), whose last chunk ends with the two tail rows (zero coefficients).
+static StepPlan step_periodic_plan(const pent_handle* h, int64_t M, const void* c, int S)
+{
+    StepPlan sp;
+    if (!h || !h->periodic || !h->inner || !h->pfold || !h->pzedge) return sp;
+    const pent_handle* hi = h->inner;
+    const int C = h->dtype == PENT_F64 ? ChunkCfg<double>::C : ChunkCfg<float>::C;
+    if (h->N % C != 0 || h->N < 2 * C || hi->cfP[0] != h->N / C || !chunk_stitching_stable(hi)) return sp;
+    sp = step_plan(hi, M, c, S, 1, 2);     // rows per tile = Pl * C = N: the two tail rows are part of the boxes
+    return sp;
+}
+
+bool step_chunked_periodic_supported(const pent_handle* h, int64_t M, const void* c)
+{
+    return step_periodic_plan(h, M, c, h && h->dtype == PENT_F64 ? 16 : 32).ok;
+}
+
+int launch_step_chunked_periodic(const pent_handle* h, int64_t M, void* c, int nsteps, cudaStream_t s)
+{
+    const int Sf = h->dtype == PENT_F64 ? 16 : 32;
+    const StepPlan sp = step_periodic_plan(h, M, c, Sf);
+    if (!sp.ok) return PENT_ERR_ARG;
+    pent_step_params p = {};
+    p.kind = 1;
+    int64_t split = M;                       // leftover round in half-width tiles, as in launch_step_chunked
+    StepPlan half;
+    int dev = 0, nsm = 0;
+    PENT_CUDA(cudaGetDevice(&dev));
+    PENT_CUDA(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+    const int64_t ntiles = (M + sp.S - 1) / sp.S, rem = ntiles % nsm;
+    if (ntiles > nsm && rem > 0 && 2 * rem <= nsm) {
+        half = step_periodic_plan(h, M, c, Sf / 2);
+        if (half.ok) split = (ntiles - rem) * sp.S;
+    }
+    int rc;
+    if (h->dtype == PENT_F64) {
+        rc = launch_step_inst<double, 16, 3, 1, false, 2>(h->inner, sp, &p, nullptr, M, c, nsteps, s, 0, split, h);
+        if (rc == PENT_OK && split < M) rc = launch_step_inst<double, 8, 3, 1, false, 2>(h->inner, half, &p, nullptr, M, c, nsteps, s, split, M, h);
+        return rc;
+    }
+    rc = launch_step_inst<float, 32, 3, 1, false, 2>(h->inner, sp, &p, nullptr, M, c, nsteps, s, 0, split, h);
+    if (rc == PENT_OK && split < M) rc = launch_step_inst<float, 16, 3, 1, false, 2>(h->inner, half, &p, nullptr, M, c, nsteps, s, split, M, h);
+    return rc;
 }
 }  // namespace pent
