@@ -448,7 +448,8 @@ struct PeriodicParams {                   // kernel parameter (constant bank)
     int ra, pa, ja, pb, jb;               // location of rows n-2 and n-1: cluster rank, local chunk, row in chunk
     T h00, h0a, h0b, h10, h11, h1a;       // h (Eq. 9): row N-2 of A at cols 0, N-4, N-3; row N-1 at cols 0, 1, N-3
     T i00, i01, i10, i11;                 // inverse of the 2 x 2 Schur complement (Eq. 12)
-    const T* zt;                          // Z = E^{-1} k as [Q][P*C] x {z0, z1}: rank r's rows at zt + r * 2*P*C
+    const T* fold;                        // chunk states of the Z solve, 8 values per GLOBAL chunk (periodic_fold_kernel)
+    const typename Pair<T>::type* zedge;  // explicit rows of Z of chunk 0 and of the chunks of rows n-2, n-1: [3][C]
     const T* f;                           // the caller's right-hand side (rows n, n+1 are read directly)
 };
 template <typename T>

@@ -1,9 +1,6 @@
 // pent_chunked_kernel.cuh -- device code of the chunked on-chip solve (included by
 // pent_solve_chunked.cu inside namespace pent; see the algorithm notes at the top of that file).
 #pragma once
-#ifndef PENT_AB_NO_Z
-#define PENT_AB_NO_Z 0
-#endif
 
 // Measured A/B switches (cfg3 fp64 on B200, profiles/r01_ab_tuning.md).  Default = fastest:
 //   store policy of the x stream: plain write-back st.global (201 us) beat .cs (212), .cg (210), .wt (211)
@@ -88,9 +85,11 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
     // rank's backward aggregate and keeps two.
     ST* aggF = stS + (size_t)S * P;
     ST* aggB = aggF + ((CLUSTER && PER) ? (size_t)prm.Q * S : 0);
-    // periodic: this CTA's rows of Z, then x^ of rows n-2/n-1, (y_{n-2}, y_{n-1}), (f_n, f_{n+1}), t  ([S] each)
-    T2* zs = reinterpret_cast<T2*>(aggB + (CLUSTER ? (size_t)prm.Q * S : 0));
-    T2* ypub = zs + (PER ? (size_t)P * C : 0);
+    // periodic: the Z-solve chunk states of this CTA's chunks (8 values each), the explicit rows of Z of the three edge
+    // chunks, then x^ of rows n-2/n-1, (y_{n-2}, y_{n-1}), (f_n, f_{n+1}), t  ([S] each)
+    T2* zfold = reinterpret_cast<T2*>(aggB + (CLUSTER ? (size_t)prm.Q * S : 0));
+    T2* zedge = zfold + (PER ? (size_t)4 * P : 0);
+    T2* ypub = zedge + (PER ? (size_t)3 * C : 0);
     T2* yab = ypub + (PER ? S : 0);
     T2* ftail2 = yab + (PER ? S : 0);             // [2][S]
     T2* stT = ftail2 + (PER ? 2 * S : 0);
@@ -152,10 +151,13 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
 #endif
     int64_t tile = first;
     if (tid == 0) {
-        const uint32_t z_bytes = PER ? (uint32_t)(P * C * sizeof(T2)) : 0u;
-        mbar_expect_tx(&bars[0], prm.table_bytes + z_bytes);
+        const uint32_t fold_bytes = PER ? (uint32_t)(4 * P * sizeof(T2)) : 0u, edge_bytes = PER ? (uint32_t)(3 * C * sizeof(T2)) : 0u;
+        mbar_expect_tx(&bars[0], prm.table_bytes + fold_bytes + edge_bytes);
         bulk_load_1d(table, prm.table + (size_t)rank * prm.table_stride, prm.table_bytes, &bars[0]);
-        if constexpr (PER) bulk_load_1d(zs, pp.zt + (size_t)rank * 2 * P * C, z_bytes, &bars[0]);
+        if constexpr (PER) {
+            bulk_load_1d(zfold, pp.fold + (size_t)rank * 8 * P, fold_bytes, &bars[0]);
+            bulk_load_1d(zedge, pp.zedge, edge_bytes, &bars[0]);
+        }
     }
 #if PENT_PDL
     // the previous kernel on the stream may have written f or may still read x: wait for it before the
@@ -407,20 +409,51 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
                     }
                 }
             }
-            T t0 = 0, t1 = 0;         // periodic: x^ = y - Z t
-            if constexpr (PER) { T2 t = stT[i]; t0 = t.x; t1 = t.y; }
-            const T2* zr = zs + (size_t)(active ? p : 0) * C;
+            // periodic: x^ = y - Z t.  Z is folded into the chunk states (F - F^Z t, B - B^Z t); the chunks that hold the
+            // non-zero rows of k (chunk 0, the chunks of rows n-2 and n-1) subtract their explicit rows of Z from x^ here,
+            // inside the store loops (edge4 below)
+            if constexpr (PER) {
+                const T2 t = stT[i];
+                const T2* fz = zfold + 4 * (size_t)p;
+                const T2 a = fz[0], b = fz[1], c = fz[2], d = fz[3];
+                F0 = fma(-a.y, t.y, fma(-a.x, t.x, F0)); F1 = fma(-b.y, t.y, fma(-b.x, t.x, F1));
+                B0 = fma(-c.y, t.y, fma(-c.x, t.x, B0)); B1 = fma(-d.y, t.y, fma(-d.x, t.x, B1));
+            }
+            // The chunks that hold the non-zero rows of k take a store loop of their own (the round-1 loop: explicit rows
+            // of Z, t in registers); every other chunk runs the loop of the non-periodic kernel.  Two loops rather than
+            // a test inside one: the fp64 cluster instantiation is at its 128-register limit, and the test cost 164
+            // bytes of spills and 20 % of the kernel's time.
+            bool edge_done = false;
+            if constexpr (PER) {
+                const bool e0 = rank == 0 && p == 0, ea = rank == pp.ra && p == pp.pa, eb = rank == pp.ra && p == pp.pb;
+                if (e0 || ea || eb) {
+                    edge_done = true;
+                    const T2 t = stT[i];
+                    const T2* zr = zedge + (e0 ? 0 : ea ? C : 2 * C);
+                    const int nrows = (col < prm.M) ? prm.N - row0 : 0;
+#pragma unroll
+                    for (int jg = 0; jg < C / 4; ++jg) {
+                        T xv[4];
+                        correct4(xv, jg);
+#pragma unroll
+                        for (int r = 0; r < 4; ++r) {
+                            const T2 z = zr[4 * jg + r];
+                            xv[r] = fma(-z.y, t.y, fma(-z.x, t.x, xv[r]));
+                            if (4 * jg + r < nrows) PENT_STORE(xo, xv[r]);
+                            xo += prm.M;
+                        }
+                    }
+                }
+            }
             if constexpr (LM >= 2) {
+                // stored above
+            } else if (edge_done) {
                 // stored above
             } else if (rows_full && (tile + 1) * S <= prm.M) {
 #pragma unroll
                 for (int jg = 0; jg < C / 4; ++jg) {
                     T xv[4];
                     correct4(xv, jg);
-                    if constexpr (PER && !PENT_AB_NO_Z) {
-#pragma unroll
-                        for (int r = 0; r < 4; ++r) { T2 z = zr[4 * jg + r]; xv[r] = fma(-z.y, t1, fma(-z.x, t0, xv[r])); }
-                    }
 #pragma unroll
                     for (int r = 0; r < 4; ++r) { PENT_STORE(xo, xv[r]); xo += prm.M; }
                 }
@@ -430,10 +463,6 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
                 for (int jg = 0; jg < C / 4; ++jg) {
                     T xv[4];
                     correct4(xv, jg);
-                    if constexpr (PER && !PENT_AB_NO_Z) {
-#pragma unroll
-                        for (int r = 0; r < 4; ++r) { T2 z = zr[4 * jg + r]; xv[r] = fma(-z.y, t1, fma(-z.x, t0, xv[r])); }
-                    }
 #pragma unroll
                     for (int r = 0; r < 4; ++r) {
                         if (4 * jg + r < nrows) PENT_STORE(xo, xv[r]);

@@ -13,11 +13,12 @@
 namespace pent {
 #include "pent_chunked_kernel.cuh"
 
-// extra dynamic shared memory of the periodic kernel: this CTA's rows of Z and four [S] pair arrays
+// extra dynamic shared memory of the periodic kernel: the Z-solve chunk states of this CTA's chunks (4 pairs each), the
+// explicit rows of Z of the three edge chunks, five [S] pair arrays and the second aggregate array of a cluster
 template <typename T>
 inline size_t periodic_extra_smem(const ChunkPlan& pl)
 {
-    return ((size_t)pl.Pl * ChunkCfg<T>::C + 5 * (size_t)pl.S + (pl.Q > 1 ? (size_t)pl.Q * pl.S : 0)) * 2 * sizeof(T);   // + second aggregate array
+    return ((size_t)4 * pl.Pl + 3 * (size_t)ChunkCfg<T>::C + 5 * (size_t)pl.S + (pl.Q > 1 ? (size_t)pl.Q * pl.S : 0)) * 2 * sizeof(T);
 }
 
 template <typename T, int S, bool CLUSTER, bool PER, int BAND = 2, int LM = 0>

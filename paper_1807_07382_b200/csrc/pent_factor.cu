@@ -228,7 +228,6 @@ extern "C" void pent_destroy(pent_handle* h)
     cudaFree(h->diag); cudaFree(h->fac); cudaFree(h->fw); cudaFree(h->bw);
     for (int j = 0; j < PENT_NQ; ++j) { cudaFree(h->cf[j]); cudaFree(h->cf1[j]); }
     cudaFree(h->dg); cudaFree(h->ms); cudaFree(h->Zt); cudaFree(h->dgp); cudaFree(h->pfold); cudaFree(h->pzedge);
-    for (int j = 0; j < PENT_NQ; ++j) cudaFree(h->pz[j]);
     pent_destroy(h->inner);
     delete h;
 }

@@ -43,12 +43,12 @@ struct pent_handle {
     int periodic;
     pent_handle* inner;
     void* Zt;
-    void* pz[PENT_NQ];   // Z rows per cluster rank for the fused kernel: [Q][Pl*C] x {z0, z1} in T (0: not built)
     void* dgp;
     double pc[10];
-    // on-chip periodic time step (pent_step_chunked.cu): per chunk of C rows (Q = 1 chunking) the chunk states of the
-    // Z solve, [P][8] in T = {g^Z of rows s-2, s-1 | Z of rows e+1, e+2} x 2 columns (zero for the first and last
-    // chunk), and the explicit rows of Z of the first and the last chunk, [2][C] x {z0, z1} in T
+    // x^ = y - Z t without the rows of Z on chip (fused periodic solve, on-chip periodic time step): per chunk of C rows
+    // the chunk states of the Z solve, [chunks + PENT_MAXQ][8] in T = {g^Z of rows s-2, s-1 | Z of rows e+1, e+2} x 2
+    // columns (zero for the chunks that hold the non-zero rows of k), and the explicit rows of Z of those chunks,
+    // [3][C] x {z0, z1} in T: chunk 0, the chunk of row n-2, the chunk of row n-1 (periodic_fold_kernel)
     void* pfold;
     void* pzedge;
     // ---- per-system factors, device, interleaved, in T ----

@@ -78,40 +78,30 @@ __global__ void periodic_tables_kernel(int N, const T* __restrict__ stage, const
     if (Z && k < n) { typename Vec<T>::T2 z; z.x = (T)Z[k]; z.y = (T)Z[n + k]; Zt[k] = z; }
 }
 
-// Z rows regrouped per cluster rank for the fused kernel: out[(r*PlC + j)] = {Z0, Z1}[r*PlC + j], 0 beyond n
+// x^ = y - Z t without the rows of Z in shared memory (the fused periodic solve and the on-chip periodic time step).
+// Inside a chunk that holds no non-zero row of k, Z is a homogeneous solution of the two recurrences,
+// Z_rows = chi F^Z_{p-1} + psi B^Z_{p+1}, so  y - Z t  is the usual correction with the chunk states F - F^Z t, B - B^Z t.
+// fold[p] = {g^Z_0, g^Z_1 of row s-2 | of row s-1 | Z_0, Z_1 of row e+1 | of row e+2} (s = pC, e = s+C-1; zero outside
+// 0..n-1).  The chunks that hold the non-zero rows of k (rows 0, 1 and n-2, n-1: chunk 0 and the chunks of rows n-2 and
+// n-1) get fold = 0 and subtract their explicit rows of Z instead: zedge[0] = chunk 0, zedge[1] = the chunk of row n-2,
+// zedge[2] = the chunk of row n-1 (C rows x {z0, z1} each).  Pt >= the number of chunks: entries beyond it are zero.
 template <typename T>
-__global__ void periodic_zslices_kernel(int n, int rows_total, const double* __restrict__ Z,
-                                        typename Vec<T>::T2* __restrict__ out)
-{
-    int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= rows_total) return;
-    typename Vec<T>::T2 z;
-    z.x = k < n ? (T)Z[k] : (T)0;
-    z.y = k < n ? (T)Z[n + k] : (T)0;
-    out[k] = z;
-}
-
-// On-chip periodic time step: x^ = y - Z t without the rows of Z in shared memory.  Inside an interior chunk Z is a
-// homogeneous solution of the two recurrences, Z_rows = chi F^Z_{p-1} + psi B^Z_{p+1}, so  y - Z t  is the usual
-// correction with the chunk states F - F^Z t, B - B^Z t.  fold[p] = {g^Z_0, g^Z_1 of row s-2 | of row s-1 | Z_0, Z_1 of
-// row e+1 | of row e+2} (s = pC, e = s+C-1; zero outside 0..n-1, and all zero for the first and the last chunk, which
-// hold the non-zero rows of k and subtract their explicit rows of Z instead: zedge[0][j], zedge[1][j]).
-template <typename T>
-__global__ void periodic_fold_kernel(int n, int P, const double* __restrict__ Z, const double* __restrict__ G,
+__global__ void periodic_fold_kernel(int n, int Pt, const double* __restrict__ Z, const double* __restrict__ G,
                                      T* __restrict__ fold, typename Vec<T>::T2* __restrict__ zedge)
 {
     constexpr int C = ChunkCfg<T>::C;
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
-    if (p < P) {
+    const int ga = (n - 2) / C, gb = (n - 1) / C;
+    if (p < Pt) {
         const int s = p * C, e = s + C - 1;
-        const bool edge = p == 0 || p == P - 1;
+        const bool edge = p == 0 || p == ga || p == gb || s >= n;
         auto at = [&](const double* v, int col, int k) -> T { return (!edge && k >= 0 && k < n) ? (T)v[(size_t)col * n + k] : (T)0; };
         T* o = fold + 8 * (size_t)p;
         o[0] = at(G, 0, s - 2); o[1] = at(G, 1, s - 2); o[2] = at(G, 0, s - 1); o[3] = at(G, 1, s - 1);
         o[4] = at(Z, 0, e + 1); o[5] = at(Z, 1, e + 1); o[6] = at(Z, 0, e + 2); o[7] = at(Z, 1, e + 2);
     }
-    if (p < 2 * C) {
-        const int which = p / C, j = p % C, k = (which == 0 ? 0 : (P - 1) * C) + j;
+    if (p < 3 * C) {
+        const int which = p / C, j = p % C, k = (which == 0 ? 0 : which == 1 ? ga : gb) * C + j;
         typename Vec<T>::T2 z;
         z.x = k < n ? (T)Z[k] : (T)0;
         z.y = k < n ? (T)Z[(size_t)n + k] : (T)0;
@@ -319,18 +309,11 @@ static int factor_periodic_t(int N, const void* const src[5], pent_dtype dtype, 
     periodic_setup_kernel<<<1, 32, 0, s>>>(N, h->inner->fac, dg64, Z, G, coef, status);
     periodic_tables_kernel<T><<<nb, tb, 0, s>>>(N, stage, Z, (typename Vec<T>::T2*)h->Zt, (T*)h->dgp, nullptr);
     count_launch(3);
-    for (int j = 0; j < PENT_NQ; ++j) {
-        const int Pl = h->inner->cfP[j];
-        if (Pl < 1) continue;
-        const int rows_total = (1 << j) * Pl * ChunkCfg<T>::C;
-        if (!alloc(&h->pz[j], sizeof(T) * 2 * (size_t)rows_total)) return done(rc);
-        periodic_zslices_kernel<T><<<(rows_total + tb - 1) / tb, tb, 0, s>>>(n, rows_total, Z, (typename Vec<T>::T2*)h->pz[j]);
-        count_launch();
-    }
-    if (N % ChunkCfg<T>::C == 0 && h->inner->cfP[0] == N / ChunkCfg<T>::C) {      // tables of the on-chip time step
-        const int P = N / ChunkCfg<T>::C, C2 = 2 * ChunkCfg<T>::C, nt = P > C2 ? P : C2;
-        if (!alloc(&h->pfold, sizeof(T) * 8 * (size_t)P) || !alloc(&h->pzedge, sizeof(T) * 2 * (size_t)C2)) return done(rc);
-        periodic_fold_kernel<T><<<(nt + tb - 1) / tb, tb, 0, s>>>(n, P, Z, G, (T*)h->pfold, (typename Vec<T>::T2*)h->pzedge);
+    {       // chunk states of the Z solve + explicit edge rows (fused periodic solve, on-chip time step)
+        constexpr int C = ChunkCfg<T>::C;
+        const int Pt = (n + C - 1) / C + PENT_MAXQ, C3 = 3 * C, nt = Pt > C3 ? Pt : C3;   // any rank's slice stays inside
+        if (!alloc(&h->pfold, sizeof(T) * 8 * (size_t)Pt) || !alloc(&h->pzedge, sizeof(T) * 2 * (size_t)C3)) return done(rc);
+        periodic_fold_kernel<T><<<(nt + tb - 1) / tb, tb, 0, s>>>(n, Pt, Z, G, (T*)h->pfold, (typename Vec<T>::T2*)h->pzedge);
         count_launch();
     }
     cudaError_t le = cudaGetLastError();

@@ -2,7 +2,8 @@
 // (Eqs. 8-12; PER = true instantiations of solve_chunked_kernel, see PeriodicCtx in
 // pent_chunk_common.cuh): y = E^{-1} f^, the 2 x 2 tail solve and x^ = y - Z t in ONE kernel,
 // 2 passes over the batch.  The unfused 3-kernel path of pent_periodic.cu stays as the fallback
-// (shared memory too small for the Z rows, or rows n-2 / n-1 in different cluster ranks).
+// (rows n-2 / n-1 in different cluster ranks, or no on-chip plan for E).  Z itself is not on chip: it is folded into
+// the chunk states (periodic_fold_kernel in pent_periodic.cu).
 #include "pent_chunked_launch.cuh"
 
 namespace pent {
@@ -19,7 +20,7 @@ static PeriodicPlan periodic_plan(const pent_handle* h, int64_t M, const void* f
     if (!h || !h->periodic || !h->inner) return pp;
     const pent_handle* in = h->inner;
     pp.pl = chunk_auto_plan(in, M, f);            // (not ok when the stitching of E is flagged unstable)
-    if (!pp.pl.ok || !h->pz[pp.pl.j]) return pp;
+    if (!pp.pl.ok || !h->pfold || !h->pzedge) return pp;
     const bool f64 = h->dtype == PENT_F64;
     const int C = f64 ? ChunkCfg<double>::C : ChunkCfg<float>::C;
     const int n = in->N;
@@ -48,7 +49,8 @@ static int launch_periodic_t(const pent_handle* h, const PeriodicPlan& pl, int64
     pp.h00 = (T)h->pc[0]; pp.h0a = (T)h->pc[1]; pp.h0b = (T)h->pc[2];
     pp.h10 = (T)h->pc[3]; pp.h11 = (T)h->pc[4]; pp.h1a = (T)h->pc[5];
     pp.i00 = (T)h->pc[6]; pp.i01 = (T)h->pc[7]; pp.i10 = (T)h->pc[8]; pp.i11 = (T)h->pc[9];
-    pp.zt = (const T*)h->pz[pl.pl.j];
+    pp.fold = (const T*)h->pfold;
+    pp.zedge = (const typename Pair<T>::type*)h->pzedge;
     pp.f = (const T*)f;
     const pent_handle* in = h->inner;
     const bool cl = pl.pl.Q > 1;
