@@ -76,8 +76,11 @@ SUITE = [
     ("cfg5a rows", ["--workload", "cfg5a", "--layout", "rows"]),
     ("cfg5b per-system", ["--workload", "cfg5b"]),
     ("cfg5b per-system f32", ["--workload", "cfg5b", "--dtype", "f32"]),
+    ("N=12288 M=8192", ["--workload", "cfg5a", "--rows-n", "12288", "--systems", "8192"]),
     ("cfg4 fused step", ["--workload", "cfg4", "--steps", "1000"]),
+    ("cfg4 fused step f32", ["--workload", "cfg4", "--steps", "1000", "--dtype", "f32"]),
     ("paper_hd", ["--workload", "paper_hd", "--steps", "250"]),
+    ("paper_hd f32", ["--workload", "paper_hd", "--steps", "250", "--dtype", "f32"]),
     ("adi2d", ["--workload", "adi2d"]),
 ]
 
@@ -541,6 +544,24 @@ def run_paper_workload(args, w, rank, world, local):
     alg = 2.0 * esz * N * M * args.steps
     achieved = alg / (ms * 1e-3) / 1e9
     on_chip = pent.lib().pent_step_kernel_choice(h.ptr, M) == 2 and not os.environ.get("PENT_AB_PERIODIC_STEP_UNFUSED")
+    if on_chip:
+        # ALU bound as for cfg4: the stencil-free Crank-Nicolson step c+ = 2 A^-1 c - c costs 9 fused
+        # multiply-adds for the solve and 1 for the update per unknown and step (tail and fold: per chunk, not per unknown)
+        fma_per_unknown = 10.0
+        sm_mhz = clocks.get("sm_max_mhz") or 1965.0
+        alu_peak = 2.0 * (64.0 if args.dtype == "f64" else 128.0) * 148 * sm_mhz * 1e6 / 1e12
+        flops = 2.0 * fma_per_unknown * N * M * args.steps / (ms * 1e-3) / 1e12
+        roof = {"bound": "alu", "achieved": flops, "peak": alu_peak, "unit": "TFLOP/s", "frac": flops / alu_peak, "traffic": None,
+                "peak_source": "derived: FMA/clk/SM x 148 SMs x SM clock (DESIGN.md section 6.4)",
+                "flops_per_unknown_step": 2.0 * fma_per_unknown, "kernel": "step_chunked_kernel",
+                "hbm_equivalent_gbs": achieved, "hbm_equivalent_frac": achieved / peak,
+                "note": "state stays in shared memory across the steps of a launch: HBM is touched twice per LAUNCH; "
+                        "hbm_equivalent = rate of streaming the state once in, once out per step"}
+    else:
+        roof = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                "peak_source": peak_src, "algorithmic_bytes_per_launch": alg, "kernel": "solve_chunked_kernel",
+                "note": "algorithmic = read the state once, write it once per step; the two-kernel path makes 4 passes per "
+                        "step, mostly served by L2 at this size"}
     line = {
         "metric": METRIC, "value": whole_job_rate(N * M * args.steps, world, ms * 1e-3), "unit": UNIT,
         "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps,
@@ -551,11 +572,7 @@ def run_paper_workload(args, w, rank, world, local):
                    "kernel": "step_chunked_kernel (periodic)" if on_chip else "periodic_rhs_kernel + solve_chunked_kernel",
                    "state_on_chip_across_steps": bool(on_chip),
                    "l2": "state 64 MiB fits the 126 MB L2"},
-        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": None, "peak_source": peak_src, "algorithmic_bytes_per_launch": alg,
-                     "kernel": "step_chunked_kernel" if on_chip else "solve_chunked_kernel",
-                     "note": "HBM-equivalent: algorithmic = read the state once, write it once per step; the on-chip kernel "
-                             "touches HBM twice per LAUNCH, the two-kernel path makes 4 passes per step, mostly served by L2"},
+        "roofline": roof,
         "clocks": clocks, "gpu_launches": int(launches),
     }
     _finish_line(line, world)

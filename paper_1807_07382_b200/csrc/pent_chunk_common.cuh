@@ -790,7 +790,7 @@ struct ChunkPlan {
     bool rows = false;         // system-major batch: implies ldg
     int pace_ns = 0;           // ChunkParams::pace_ns
     int band = 2;              // 1: the tridiagonal instantiation and its tables (handle with a == e == 0)
-    int mode = 0;              // ChunkParams::ldg: 0 TMA (interleaved), 1 LDG (interleaved), 2 LDG.256 (system-major),
+    int mode = 0;              // ChunkParams::ldg: 0 TMA (interleaved), 1 LDG (interleaved), 4 cp.async ring (interleaved), 2 LDG.256 (system-major),
                                // 3 swizzled TMA loads + STG.256 stores, 4 swizzled TMA loads AND stores (system-major)
     size_t table_bytes = 0, smem = 0;
 };
@@ -798,7 +798,7 @@ struct ChunkPlan {
 // ldg: plan for the LDG loader (no TMA alignment requirements, no landing buffer)
 ChunkPlan make_plan(const pent_handle* h, int64_t M, const void* f, int Q, int S, bool any_S = false,
                     bool ldg = false, int band = 2);
-ChunkPlan chunk_auto_plan(const pent_handle* h, int64_t M, const void* f);   // what PENT_KERNEL_AUTO runs
+ChunkPlan chunk_auto_plan(const pent_handle* h, int64_t M, const void* f, bool ring_ok = true);   // what PENT_KERNEL_AUTO runs
 // rank-2 tensor map {M, N} of an interleaved batch with box {S, box_rows}; false on failure
 bool encode_batch_map(CUtensorMap* tm, const void* base, int64_t M, int N, int S, int box_rows, bool f64);
 bool encode_batch_map_cached(CUtensorMap* tm, const void* base, int64_t M, int N, int S, int box_rows, bool f64);

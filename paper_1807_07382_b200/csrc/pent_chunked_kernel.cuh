@@ -24,6 +24,7 @@ struct ChunkParams {
     int woff[W_LEVELS]; // w_level_off(P, l)
     int box_rows;     // rows per TMA box
     int nbox;         // boxes per tile
+    int land_rows;    // rows of the landing buffer (nbox * box_rows for TMA; P * C for the cp.async loader; 0: none)
     int wcount[MAX_BOXES]; // warps that read each box (arrival count of its "empty" barrier)
     uint32_t table_bytes;  // bytes of the per-CTA table staged into shared memory
     int64_t table_stride;  // elements between the tables of consecutive cluster ranks
@@ -34,6 +35,9 @@ struct ChunkParams {
     unsigned pace_ns; // sleep this long before the store stage (0: none)
     int ldg;          // 1: the pitch M*sizeof(T) is not a multiple of 16 bytes, so TMA cannot address the batch:
                       // every thread loads its rows with coalesced LDG instead (no landing buffer, nbox = 0)
+                      // 4: the same batch through per-thread cp.async copies (LDGSTS) into a landing buffer, one tile ahead:
+                      // every thread copies the C rows IT will read, so it waits only for its own copies (no barrier)
+                      // and re-issues them for the next tile as soon as its values are in registers
                       // 2: SYSTEM-MAJOR batch ("one system per row", the paper's serial layout):
                       // element k of system i at f[i*N + k]; a thread's chunk is one contiguous run of C
                       // elements, loaded and stored with 32-byte vector accesses
@@ -73,7 +77,7 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
     T* landing = reinterpret_cast<T*>(LM == 3 ? smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u) : smem_raw);
     // modes 5, 6: one padded run per system (pitch in bytes); mode 6: a staging buffer of the same size and layout
     const uint32_t run_pitch = (uint32_t)(prm.box_rows * sizeof(T)) + 16u;
-    const size_t tile_elems = LM >= 5 ? (size_t)S * run_pitch / sizeof(T) : (size_t)prm.nbox * prm.box_rows * S;
+    const size_t tile_elems = LM >= 5 ? (size_t)S * run_pitch / sizeof(T) : (size_t)prm.land_rows * S;
     T* staging = landing + tile_elems;
     T* table = staging + (LM == 6 ? tile_elems : 0);
     // chunk states [P][S]: E~ then F_{p-1};  S^ then B_{p+1}
@@ -190,6 +194,22 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
     const ScanGeom geom{P, Pw, prm.lev_f, prm.lev_b, prm.woff};
     const int rounds = (S + nwarps * G - 1) / (nwarps * G);     // host guarantees 1 when CLUSTER
 
+    // cp.async loader (prm.ldg == 4): this thread's C rows of tile t -> its own slots of the landing buffer
+    auto ring_issue = [&](int64_t t) {
+        if (active) {
+            const int64_t col = t * S + i;
+            const int nrows = (t < prm.ntiles && col < prm.M) ? prm.N - row0 : 0;
+            const T* src = prm.f + (int64_t)row0 * prm.M + col;
+            T* dst = landing + (size_t)p * C * S + i;
+#pragma unroll
+            for (int j = 0; j < C; ++j)
+                if (j < nrows) cp_async_elem(dst + j * S, src + (int64_t)j * prm.M);
+        }
+        cp_async_commit();
+    };
+    if constexpr (LM == 0 && !PER) {
+        if (prm.ldg == 4) ring_issue(tile);
+    }
     int tcount = 0;
     if constexpr (PER) {
         if (tid < S) {
@@ -265,6 +285,15 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
 #pragma unroll
                     for (int j = 0; j < C; ++j) v[j] = (j < nrows) ? __ldcs(src + j) : (T)0;
                 }
+            } else if (!PER && prm.ldg == 4) {
+                // ---- tile data: this thread's own cp.async copies -> registers; rows / systems beyond the batch were
+                // not copied and read as zero (their slots hold stale values) ----
+                cp_async_wait<0>();
+                const int64_t col = tile * S + i;
+                const int nrows = col < prm.M ? prm.N - row0 : 0;
+                const T* src = landing + (size_t)p * C * S + i;
+#pragma unroll
+                for (int j = 0; j < C; ++j) v[j] = (j < nrows) ? src[j * S] : (T)0;
             } else if (prm.ldg) {
                 // ---- tile data: global -> registers (C independent loads in flight per thread) ----
                 const int64_t col = tile * S + i;
@@ -283,6 +312,9 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
         // The box is free once every warp that reads it has its values in registers: each such
         // warp arrives on the box's "empty" barrier and thread 0 re-arms it with the NEXT tile's
         // TMA load, which then runs under all of this tile's arithmetic and stores.
+        if constexpr (LM == 0 && !PER) {
+            if (prm.ldg == 4) ring_issue(next_tile);      // the slots are free: their values are in registers
+        }
         __syncwarp();
         if (lane == 0 && warp * 32 < P * S && (LM >= 3 || (LM == 0 && !prm.ldg))) mbar_arrive(&bars[1 + MAX_BOXES + mybox]);
         if constexpr (CLUSTER) {

@@ -35,6 +35,7 @@ static int launch_inst(const pent_handle* h, const ChunkPlan& pl, int64_t M, con
     prm.lev_b = hlb < lg ? hlb : lg;
     for (int l = 0; l < W_LEVELS; ++l) prm.woff[l] = w_level_off(pl.Pl, l, pl.Q, BAND);
     prm.box_rows = pl.box_rows; prm.nbox = pl.nbox;
+    prm.land_rows = pl.mode == 4 ? pl.Pl * C : pl.nbox * pl.box_rows;
     prm.ntiles = (M + S - 1) / S;
     for (int b = 0; b < MAX_BOXES; ++b) prm.wcount[b] = 0;
     for (int w = 0; w * 32 < pl.Pl * S; ++w) prm.wcount[((w * 32 / S) * C) / prm.box_rows] += 1;
@@ -60,7 +61,7 @@ static int launch_inst(const pent_handle* h, const ChunkPlan& pl, int64_t M, con
     PeriodicParams<T> pp = {};
     if (PER) pp = *per;
     const size_t smem_total = pl.smem + (PER ? periodic_extra_smem<T>(pl) : 0);
-    if ((LM == 0) != (pl.mode <= 1) || (LM != 0 && LM != pl.mode)) return PENT_ERR_ARG;
+    if ((LM == 0) != (pl.mode <= 1 || pl.mode == 4) || (LM != 0 && LM != pl.mode) || (PER && pl.mode == 4)) return PENT_ERR_ARG;
     auto kern = solve_chunked_kernel<T, S, CLUSTER, PER, BAND, LM>;
     static SmemOnce mark;
     PENT_CUDA(ensure_dynamic_smem(mark, kern, smem_total));

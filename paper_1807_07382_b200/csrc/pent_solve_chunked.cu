@@ -31,6 +31,7 @@
 //   aggregates through distributed shared memory (chunk_state_scan in pent_chunk_common.cuh).
 // This file: the tables (built once per handle and cluster size), the launch plans and dispatch.
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include "pent_chunked_launch.cuh"
 
@@ -483,7 +484,7 @@ bool chunk_stitching_stable(const pent_handle* h)
     return g <= (h->dtype == PENT_F64 ? 1e6 : 1e3);          // NaN compares false
 }
 
-ChunkPlan chunk_auto_plan(const pent_handle* h, int64_t M, const void* f)
+ChunkPlan chunk_auto_plan(const pent_handle* h, int64_t M, const void* f, bool ring_ok)
 {
     if (!h || h->kind != 0) return ChunkPlan{};
     if (!chunk_stitching_stable(h)) return ChunkPlan{};
@@ -514,9 +515,30 @@ ChunkPlan chunk_auto_plan(const pent_handle* h, int64_t M, const void* f)
         ChunkPlan pl = make_plan(h, M, f, Q, Sw, false, false, hb);
         if (pl.ok) return pl;
     }
-    // TMA cannot address this batch (pitch or base not 16-byte aligned): LDG loader.  It has no
-    // prefetch of the next tile, so prefer CTAs of <= 256 threads: two of them share an SM and one
-    // loads while the other computes.
+    // TMA cannot address this batch (pitch or base not 16-byte aligned).  First choice: the same shapes with the
+    // cp.async loader (mode 4: per-thread LDGSTS into a landing buffer, one tile ahead).  The fused periodic kernel
+    // (which keeps a cp.async group of its own for the tail rows: ring_ok = false) and shapes whose landing buffer does
+    // not fit: the LDG loader.  It has no prefetch of the next tile, so prefer CTAs of <= 256 threads: two of them share an SM and
+    // one loads while the other computes.
+    static const int no_ring = []() { const char* e = std::getenv("PENT_AB_NO_RING"); return e ? std::atoi(e) : 0; }();   // A/B
+    if (ring_ok && !no_ring) {
+        const size_t esz = h->dtype == PENT_F64 ? 8 : 4;
+        const int C = h->dtype == PENT_F64 ? ChunkCfg<double>::C : ChunkCfg<float>::C;
+        auto ring = [&](int Q, int S) {
+            ChunkPlan pl = make_plan(h, M, f, Q, S, false, true, hb);
+            if (!pl.ok) return pl;
+            pl.smem += (size_t)pl.Pl * C * S * esz;          // the landing buffer the LDG plan does without
+            pl.mode = 4;
+            pl.ok = pl.smem <= SMEM_LIMIT;
+            return pl;
+        };
+        // (a system that fits a single CTA of <= 256 threads keeps the LDG loader: two such CTAs per SM overlap their
+        // loads better than one CTA with a landing buffer, cfg2's shape with M = 16383: 34.1 against 49.1 us)
+        ChunkPlan n1 = make_plan(h, M, f, 1, Sn, false, true, hb);
+        if (n1.ok && n1.threads <= 256) return n1;
+        for (int Q = 1; Q <= 4; Q *= 2) { ChunkPlan pl = ring(Q, Sw); if (pl.ok) return pl; }
+        for (int Q = 1; Q <= QMAX; Q *= 2) { ChunkPlan pl = ring(Q, Sn); if (pl.ok) return pl; }
+    }
     for (int Q = 1; Q <= QMAX; Q *= 2) {
         ChunkPlan pl = make_plan(h, M, f, Q, Sn, false, true, hb);
         if (pl.ok && pl.threads <= 256) return pl;

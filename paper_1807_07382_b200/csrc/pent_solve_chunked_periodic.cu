@@ -19,7 +19,7 @@ static PeriodicPlan periodic_plan(const pent_handle* h, int64_t M, const void* f
     PeriodicPlan pp;
     if (!h || !h->periodic || !h->inner) return pp;
     const pent_handle* in = h->inner;
-    pp.pl = chunk_auto_plan(in, M, f);            // (not ok when the stitching of E is flagged unstable)
+    pp.pl = chunk_auto_plan(in, M, f, /*ring_ok=*/false);   // (not ok when the stitching of E is flagged unstable)
     if (!pp.pl.ok || !h->pfold || !h->pzedge) return pp;
     const bool f64 = h->dtype == PENT_F64;
     const int C = f64 ? ChunkCfg<double>::C : ChunkCfg<float>::C;

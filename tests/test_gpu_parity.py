@@ -269,10 +269,12 @@ def test_chunked_cluster_slowly_decaying_coupling(Q, S):
 
 
 @pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
-@pytest.mark.parametrize("N,M", [(1024, 1001), (512, 333), (4096, 77), (2000, 129), (100, 7)])
+@pytest.mark.parametrize("N,M", [(1024, 1001), (512, 333), (4096, 77), (2000, 129), (100, 7), (1000, 2051), (3000, 515),
+                                 (8192, 35), (16384, 19), (1024, 5001)])
 def test_unaligned_pitch_runs_on_chip_with_the_ldg_loader(dtype, N, M):
-    """M*sizeof(T) not a multiple of 16 bytes: TMA cannot address the batch; the chunked kernel then
-    loads with LDG (still 2 passes) instead of falling back to the 4-pass kernel."""
+    """M*sizeof(T) not a multiple of 16 bytes: TMA cannot address the batch; the chunked kernel then loads with
+    per-thread cp.async copies one tile ahead (or plain LDG when the system fits one small CTA): still 2 passes
+    instead of falling back to the 4-pass kernel."""
     pent = _pent()
     diags = pin.diagonals_I_plus_sigma_L2(N, 2.0)
     f = pin.uniform_pm1(90 + N, 0, N, M)
@@ -451,6 +453,20 @@ def test_tridiagonal_instantiation_shapes_fp64(N, M, Q, S):
 @pytest.mark.parametrize("N,M,Q,S", [(1024, 2048 + 64, 2, 64), (1024, 1024, 1, 32), (4096, 512, 4, 32), (700, 333, 1, 32)])
 def test_tridiagonal_instantiation_shapes_fp32(N, M, Q, S):
     _tri_case(N, M, Q, S, torch.float32)
+
+
+@pytest.mark.parametrize("N,M", [(1024, 2049), (4096, 131), (300, 77)])
+def test_tridiagonal_unaligned_pitch_default_plan(N, M):
+    """Odd M with a tridiagonal handle: the BAND = 1 instantiation behind the cp.async / LDG loaders (AUTO plan)."""
+    pent = _pent()
+    a, b, c, d, e = pin.random_diag_dominant(720 + N, N)
+    a[:] = 0.0
+    e[:] = 0.0
+    f = pin.uniform_pm1(721 + N, 0, N, M)
+    x, h = gpu_solve((a, b, c, d, e), f)
+    assert pent.lib().pent_handle_band(h.ptr) == 1
+    assert normwise(x, oracle.solve_batch(oracle.factor(a, b, c, d, e), f)) <= 1e-11
+    assert residual((a, b, c, d, e), x, f) <= 1e-12
 
 
 @pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
