@@ -295,6 +295,195 @@ factor_solve_ring_kernel(int N, int64_t M, const T* __restrict__ a, const T* __r
     cp_async_wait<0>();
 }
 
+// ---------------------------------------------------------------------------------------------
+// Two threads per system ("burn at both ends"): M is the only parallelism of the per-system problem (cfg5b: 16384
+// systems = 3.5 warps per SM with one thread per system), and each thread is one long dependent chain (a division per
+// row), so the ring kernel above is bound by the latency of single warps (issue 20 %, no unit above 55 %).  Here the
+// system is cut in the middle, m = ceil(N/2):
+//     thread T: rows 0 .. m-1 top-down  = LU of the leading block A_TT, forward sweep of f_T;
+//     thread B: rows N-1 .. m bottom-up = the same recurrence on the REVERSED trailing block (reversing rows and
+//               columns of a pentadiagonal matrix swaps a <-> e, b <-> d), forward sweep of the reversed f_B.
+// The halves are coupled only through (x_{m-2}, x_{m-1}) and (x_m, x_{m+1}): A_TT x_T = f_T - C_T (x_m, x_{m+1}) with C_T
+// non-zero in its last two rows only, so L_T^{-1} C_T is non-zero in its last two rows only and the last two unknowns of
+// each half are  p - P (the other half's two)  with p (2 values) and P (2 x 2) known at the end of its forward loop.  The two
+// threads swap (p, P) through shared memory, each solves the 4 x 4 interface system (as two 2 x 2), and then runs its
+// ordinary back substitution outward from the two interface values; the rows above the interface use the spilled
+// gamma, delta, g unchanged.  Same traffic as the ring kernel (13 words per unknown), twice the warps, chains of half
+// the length.  Exactly A_i^{-1} f_i (a twisted factorisation, no pivoting: the leading and the reversed trailing block of
+// an SPD / diagonally dominant matrix are SPD / diagonally dominant); it differs from the oracle's LU by rounding only.
+// info[i]: the first zero / non-finite pivot met by thread T, else by thread B, as row + 1 (a pivot of the twisted
+// factorisation; for the top half it is the pivot of the paper's LU).
+// Block = TW_SYS threads T followed by TW_SYS threads B of the same TW_SYS systems.  Measured on cfg5b (profiles/
+// r02_bench_all.jsonl; A/B PENT_AB_PER_SYSTEM_ONE_THREAD=1): 381.5 -> 361 us fp64, 240 -> 207 us fp32: the kernel was NOT
+// bound by the latency of its few warps after all (twice the warps bought 5 %); 32 or 64 systems per block measure the same.
+// ---------------------------------------------------------------------------------------------
+constexpr int TW_STAGES = 4, TW_SYS = 64;
+
+template <typename T>
+__global__ void __launch_bounds__(2 * TW_SYS)
+factor_solve_twist_kernel(int N, int64_t M, const T* __restrict__ a, const T* __restrict__ b,
+                          const T* __restrict__ c, const T* __restrict__ d, const T* __restrict__ e,
+                          const T* f, T* x, T* __restrict__ scratch, int* __restrict__ info)
+{
+    constexpr int R = RING_ROWS, NST = TW_STAGES, TB = 2 * TW_SYS;
+    extern __shared__ __align__(16) unsigned char ring_raw[];
+    T* ring = reinterpret_cast<T*>(ring_raw);           // [NST][RING_SLOTS][TB]
+    T* xch = ring + (size_t)NST * RING_SLOTS * TB;       // [2][7][TW_SYS]: p (2), P (4), bad pivot
+    const int lane = threadIdx.x & (TW_SYS - 1), half = threadIdx.x / TW_SYS;
+    int64_t i = (int64_t)blockIdx.x * TW_SYS + lane;
+    const bool writer = i < M;
+    if (i >= M) i = M - 1;                                // tail lanes redo the last system (no divergent exits)
+    const int m = (N + 1) / 2, len = half ? N - m : m;   // rows of this thread's half
+    // local step s = 0 .. len-1  <->  row k(s); the roles of the diagonals in the (reversed) local system
+    auto krow = [&](int s) -> int { return half ? N - 1 - s : s; };
+    const T* sub2 = half ? e : a;
+    const T* sub1 = half ? d : b;
+    const T* sup1 = half ? b : d;
+    const T* sup2 = half ? a : e;
+    T* mine = ring + threadIdx.x;
+    T* sc = scratch + (size_t)blockIdx.x * N * 3 * TW_SYS + lane;       // [k][3][TW_SYS], private to the block
+    auto slot = [&](int stage, int v) -> T* { return mine + (size_t)(stage * RING_SLOTS + v) * TB; };
+
+    // ---------------- forward: factor the rows of this half and sweep in the same loop ----------------
+    const int nblk = (len + R - 1) / R;
+    auto issue_fwd = [&](int blk) {
+        if (blk < nblk) {
+            const int st = blk % NST;
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const int s = blk * R + r;
+                if (s < len) {
+                    const int64_t o = (int64_t)krow(s) * M + i;
+                    cp_async_elem(slot(st, 0 * R + r), sub2 + o);
+                    cp_async_elem(slot(st, 1 * R + r), sub1 + o);
+                    cp_async_elem(slot(st, 2 * R + r), c + o);
+                    cp_async_elem(slot(st, 3 * R + r), sup1 + o);
+                    cp_async_elem(slot(st, 4 * R + r), sup2 + o);
+                    cp_async_elem(slot(st, 5 * R + r), f + o);
+                }
+            }
+        }
+        cp_async_commit();
+    };
+    for (int blk = 0; blk < NST - 1; ++blk) issue_fwd(blk);
+    T ga1 = 0, ga2 = 0, de1 = 0, de2 = 0, g1 = 0, g2 = 0;
+    T inv1 = 0, inv2 = 0, be1 = 0;             // 1/alpha of the last two rows, beta of the last row
+    T c20 = 0, c10 = 0, c11 = 0;               // couplings to the other half: sup2 of row len-2; sup1, sup2 of row len-1
+    int bad = 0;
+    for (int blk = 0; blk < nblk; ++blk) {
+        issue_fwd(blk + NST - 1);
+        cp_async_wait<NST - 1>();
+        const int st = blk % NST;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int s = blk * R + r;
+            if (s < len) {
+                const int k = krow(s);
+                const T ak = (s >= 2) ? *slot(st, 0 * R + r) : (T)0;
+                const T bk = (s >= 1) ? *slot(st, 1 * R + r) : (T)0;
+                const T ck = *slot(st, 2 * R + r);
+                const T dr = *slot(st, 3 * R + r), er = *slot(st, 4 * R + r);
+                const T dk = (s + 1 < len) ? dr : (T)0;          // entries that leave the half are not part of its LU
+                const T ek = (s + 2 < len) ? er : (T)0;
+                if (s == len - 2) c20 = er;
+                if (s == len - 1) { c10 = dr; c11 = er; }
+                const T fk = *slot(st, 5 * R + r);
+                T be = fma(-ak, ga2, bk);
+                T al = fma(-be, ga1, fma(-ak, de2, ck));
+                if (bad == 0 && (al == (T)0 || !isfinite(al))) bad = k + 1;
+                T inv = (T)1 / al;
+                T ga = fma(-be, de1, dk) * inv;
+                T de = ek * inv;
+                T g = fma(-be, g1, fma(-ak, g2, fk)) * inv;
+                { T* w = sc + (size_t)k * 3 * TW_SYS; w[0] = ga; w[TW_SYS] = de; w[2 * TW_SYS] = g; }
+                g2 = g1; g1 = g;
+                ga2 = ga1; ga1 = ga; de2 = de1; de1 = de;
+                inv2 = inv1; inv1 = inv; be1 = be;
+            }
+        }
+    }
+    cp_async_wait<0>();
+    __threadfence();              // this thread's gamma, delta, g are in L2 before it copies them back
+
+    // ---------------- interface: (y_{len-2}, y_{len-1}) = p - P u,  u = the other half's (y_{len-1}, y_{len-2}) -----------
+    // rows len-2, len-1 of L^{-1} C (C = the couplings above, columns u0, u1), then two steps of back substitution
+    // (ga2 = gamma of row len-2 after the loop's last shift)
+    // (columns outside the matrix -- row N of the top half when N is odd and tiny -- do not occur: N >= 8)
+    const T G20 = c20 * inv2;                                   // row len-2: [c20, 0]
+    const T G10 = fma(-be1, G20, c10) * inv1, G11 = c11 * inv1; // row len-1: [c10, c11] - beta [G20, 0]
+    T pv[2], Pm[4];
+    pv[1] = g1;                      Pm[2] = G10;                   Pm[3] = G11;
+    pv[0] = fma(-ga2, g1, g2);       Pm[0] = fma(-ga2, G10, G20);   Pm[1] = -ga2 * G11;
+    {
+        T* o = xch + (size_t)half * 7 * TW_SYS + lane;
+        o[0] = pv[0]; o[TW_SYS] = pv[1]; o[2 * TW_SYS] = Pm[0]; o[3 * TW_SYS] = Pm[1]; o[4 * TW_SYS] = Pm[2]; o[5 * TW_SYS] = Pm[3];
+        o[6 * TW_SYS] = (T)bad;
+    }
+    __syncthreads();
+    T qv[2], Qm[4];
+    {
+        const T* o = xch + (size_t)(1 - half) * 7 * TW_SYS + lane;
+        qv[0] = o[0]; qv[1] = o[TW_SYS]; Qm[0] = o[2 * TW_SYS]; Qm[1] = o[3 * TW_SYS]; Qm[2] = o[4 * TW_SYS]; Qm[3] = o[5 * TW_SYS];
+        const int obad = (int)o[6 * TW_SYS];
+        if (info && writer && half == 0) info[i] = bad ? bad : obad;
+    }
+    // mine = pv - Pm S other,  other = qv - Qm S mine  (S swaps the two entries)  =>  (I - Pm S Qm S) mine = pv - Pm S qv
+    // Pm S = columns swapped: (Pm S)[r] = {Pm[2r+1], Pm[2r]}
+    T y2, y1;                                  // this half's (y_{len-2}, y_{len-1})
+    {
+        const T A0 = Pm[1], A1 = Pm[0], A2 = Pm[3], A3 = Pm[2];          // Pm S
+        const T B0 = Qm[1], B1 = Qm[0], B2 = Qm[3], B3 = Qm[2];          // Qm S
+        const T K0 = (T)1 - fma(A0, B0, A1 * B2), K1 = -fma(A0, B1, A1 * B3);
+        const T K2 = -fma(A2, B0, A3 * B2), K3 = (T)1 - fma(A2, B1, A3 * B3);
+        const T r0 = pv[0] - fma(A0, qv[0], A1 * qv[1]), r1 = pv[1] - fma(A2, qv[0], A3 * qv[1]);
+        const T det = fma(K0, K3, -K1 * K2);
+        y2 = fma(K3, r0, -K1 * r1) / det;
+        y1 = fma(K0, r1, -K2 * r0) / det;
+    }
+
+    // ---------------- backward: outward from the interface, x_s = g_s - gamma_s x_{s+1} - delta_s x_{s+2} ----------------
+    if (writer) {
+        __stcs(x + (int64_t)krow(len - 1) * M + i, y1);
+        __stcs(x + (int64_t)krow(len - 2) * M + i, y2);
+    }
+    constexpr int RB = 2 * R;
+    const int rest = len - 2;                   // local steps len-3 .. 0
+    const int nblk_b = (rest + RB - 1) / RB;
+    auto issue_bwd = [&](int blk) {
+        if (blk < nblk_b) {
+            const int st = blk % NST;
+#pragma unroll
+            for (int r = 0; r < RB; ++r) {
+                const int s = rest - 1 - (blk * RB + r);
+                if (s >= 0) {
+                    const T* w = sc + (size_t)krow(s) * 3 * TW_SYS;
+                    cp_async_elem(slot(st, 0 * RB + r), w);
+                    cp_async_elem(slot(st, 1 * RB + r), w + TW_SYS);
+                    cp_async_elem(slot(st, 2 * RB + r), w + 2 * TW_SYS);
+                }
+            }
+        }
+        cp_async_commit();
+    };
+    for (int blk = 0; blk < NST - 1; ++blk) issue_bwd(blk);
+    T x1 = y2, x2 = y1;
+    for (int blk = 0; blk < nblk_b; ++blk) {
+        issue_bwd(blk + NST - 1);
+        cp_async_wait<NST - 1>();
+        const int st = blk % NST;
+#pragma unroll
+        for (int r = 0; r < RB; ++r) {
+            const int s = rest - 1 - (blk * RB + r);
+            if (s >= 0) {
+                T xv = fma(-*slot(st, 1 * RB + r), x2, fma(-*slot(st, 0 * RB + r), x1, *slot(st, 2 * RB + r)));
+                if (writer) __stcs(x + (int64_t)krow(s) * M + i, xv);
+                x2 = x1; x1 = xv;
+            }
+        }
+    }
+    cp_async_wait<0>();
+}
+
 // Solve with stored per-system factors (layout ms: ia, en, bn, gamma, delta, each N*M).
 template <typename T>
 __global__ void __launch_bounds__(PS_THREADS)
@@ -369,11 +558,21 @@ static int factor_solve_impl(int N, int64_t M, const void* e, const void* c, con
                                               (const T*)d, (const T*)e, (const T*)f, (T*)x,
                                               scratch, scratch + NM, nullptr, nullptr, nullptr, info);
 #else
-    const size_t smem = (size_t)RING_STAGES * RING_SLOTS * PS_THREADS * sizeof(T);
-    static SmemOnce mark;
-    PENT_CUDA(ensure_dynamic_smem(mark, factor_solve_ring_kernel<T>, smem));
-    factor_solve_ring_kernel<T><<<nb, tb, smem, s>>>(N, M, (const T*)a, (const T*)b, (const T*)c, (const T*)d,
-                                                     (const T*)e, (const T*)f, (T*)x, scratch, info);
+    static const int one_thread = []() { const char* ev = std::getenv("PENT_AB_PER_SYSTEM_ONE_THREAD"); return ev ? std::atoi(ev) : 0; }();
+    if (N >= 8 && !one_thread) {        // two threads per system (workspace: 3 N ceil64(M), the contract's size)
+        const size_t smem = ((size_t)TW_STAGES * RING_SLOTS * 2 * TW_SYS + 2 * 7 * TW_SYS) * sizeof(T);
+        static SmemOnce mark2;
+        PENT_CUDA(ensure_dynamic_smem(mark2, factor_solve_twist_kernel<T>, smem));
+        nb = (unsigned)((M + TW_SYS - 1) / TW_SYS);
+        factor_solve_twist_kernel<T><<<nb, 2 * TW_SYS, smem, s>>>(N, M, (const T*)a, (const T*)b, (const T*)c, (const T*)d,
+                                                                   (const T*)e, (const T*)f, (T*)x, scratch, info);
+    } else {
+        const size_t smem = (size_t)RING_STAGES * RING_SLOTS * PS_THREADS * sizeof(T);
+        static SmemOnce mark;
+        PENT_CUDA(ensure_dynamic_smem(mark, factor_solve_ring_kernel<T>, smem));
+        factor_solve_ring_kernel<T><<<nb, tb, smem, s>>>(N, M, (const T*)a, (const T*)b, (const T*)c, (const T*)d,
+                                                         (const T*)e, (const T*)f, (T*)x, scratch, info);
+    }
 #endif
     count_launch();
     cudaError_t le = cudaGetLastError();

@@ -29,7 +29,7 @@ def _dev(v, dtype=torch.float64):
 
 
 # ---- per-system matrices ------------------------------------------------------------------
-@pytest.mark.parametrize("N,M", [(64, 100), (1024, 2048 + 37), (5, 3), (3, 70)])
+@pytest.mark.parametrize("N,M", [(64, 100), (1024, 2048 + 37), (5, 3), (3, 70), (8, 33), (9, 40), (1023, 130), (2001, 64)])
 def test_factor_solve_batch_parity(N, M):
     pent = _pent()
     if N >= 4:
@@ -56,6 +56,31 @@ def test_factor_solve_batch_parity(N, M):
     check_all(fg, xg2, ig2, *gs)
     assert not info2.cpu().numpy().any()
     assert normwise(x2.cpu().numpy(), ref) <= 1e-11
+
+
+@pytest.mark.parametrize("N,M", [(257, 96), (64, 31), (12, 200)])
+def test_factor_solve_batch_nonsymmetric_two_threads_per_system(N, M):
+    """Non-symmetric per-system matrices (nothing of the twisted factorisation may rely on symmetry: the bottom half is
+    factored bottom-up with a <-> e, b <-> d), plus a singular pivot in the BOTTOM half of one system."""
+    pent = _pent()
+    diags = pin.random_diag_dominant(66 + N, N, M)
+    f = pin.uniform_pm1(67, 0, N, M)
+    gs = [guarded(v) for v in diags]
+    a, b, c, d, e = (g.t for g in gs)
+    fg, xg, ig = guarded(f), Guarded((N, M)), Guarded((M,), torch.int32)
+    x, info = pent.pent_factor_solve_batch(N, M, e, c, d, a, b, fg.t, xg.t, ig.t)
+    check_all(fg, xg, ig, *gs)
+    ref, rinfo = oracle.factor_solve_batch(*diags, f)
+    assert not info.cpu().numpy().any() and not rinfo.any()
+    assert normwise(x.cpu().numpy(), ref) <= 1e-11
+    assert residual(diags, x.cpu().numpy(), f) <= 1e-12
+    # the last row is the FIRST pivot of the bottom-up thread: c[N-1] = 0 makes it exactly zero
+    c2 = c.clone(); c2[N - 1, 5] = 0.0
+    x2, info2 = pent.pent_factor_solve_batch(N, M, e, c2, d, a, b, fg.t)
+    info2 = info2.cpu().numpy()
+    assert info2[5] == N and np.count_nonzero(info2) == 1
+    keep = np.arange(M) != 5
+    assert np.array_equal(x2.cpu().numpy()[:, keep], x.cpu().numpy()[:, keep])
 
 
 def test_cfg5b_full_size():
