@@ -669,6 +669,8 @@ def run_per_system_workload(args, w, rank, world, local):
         return
     per = np.array([evs[i].elapsed_time(evs[i + 1]) for i in range(args.steps)])
     peak, peak_src = measured_peak()
+    kname = ("factor_solve_twist_kernel" if N >= 8 and not os.environ.get("PENT_AB_PER_SYSTEM_ONE_THREAD")
+             else "factor_solve_ring_kernel")
     alg = 7.0 * esz * N * M                        # 5 diagonals + f in, x out
     achieved = alg / (float(per.mean()) * 1e-3) / 1e9
     line = {
@@ -676,10 +678,11 @@ def run_per_system_workload(args, w, rank, world, local):
         "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
         "config": {"workload": w.name, "N": N, "M_per_gpu": M, "matrix": "per-system I+sigma_i*L^2, sigma_i~U[0.1,10]",
-                   "kernel": "factor_solve_ring_kernel", "l2": f"inputs+outputs {int(alg) >> 20} MiB per step exceed the 126 MB L2"},
+                   "kernel": kname, "threads_per_system": 2 if kname == "factor_solve_twist_kernel" else 1,
+                   "l2": f"inputs+outputs {int(alg) >> 20} MiB per step exceed the 126 MB L2"},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": ncu_traffic(w.name, args.dtype, "factor_solve_ring_kernel"), "peak_source": peak_src,
-                     "algorithmic_bytes_per_launch": alg, "kernel": "factor_solve_ring_kernel",
+                     "traffic": ncu_traffic(w.name, args.dtype, kname), "peak_source": peak_src,
+                     "algorithmic_bytes_per_launch": alg, "kernel": kname,
                      "avg_launch_ms": float(per.mean()), "min_launch_ms": float(per.min())},
         "clocks": clocks, "gpu_launches": int(launches),
     }

@@ -125,8 +125,10 @@ void pent_destroy(pent_handle* h);          /* NULL is allowed */
  * entries).  N >= 6.  Set-up = the reduction of Eqs. 8-12: factor the (N-2) x (N-2) block E,
  * E^{-1} k and the inverted 2 x 2 Schur complement are computed once and kept in the handle.
  * The handle is used with pent_solve_batch / _v / _host (f, x: N*M elements, interleaved) and with
- * pent_step_batch (kind 1 only: A c+ = (2I - A) c with the cyclic A, Eq. 6 / 7c; `scratch` = N*M
- * elements or NULL).  PENT_ERR_PIVOT: *bad_row = failing row of E, or N-2 if the 2 x 2 Schur
+ * pent_step_batch (kind 1 only: A c+ = (2I - A) c with the cyclic A, Eq. 6 / 7c = the paper's own time loop,
+ * PAPER.md:281; ONE launch for all nsteps with the state on chip when N is a multiple of 32 (fp64) / 64 (fp32) and the
+ * tile fits, evaluated as c+ = 2 A^{-1} c - c; otherwise a right-hand-side kernel and a fused periodic solve per step with
+ * `scratch` = N*M elements or NULL).  PENT_ERR_PIVOT: *bad_row = failing row of E, or N-2 if the 2 x 2 Schur
  * complement is singular. */
 int pent_factor_periodic(int N, const void* e, const void* c, const void* d, const void* a, const void* b,
                          pent_dtype dtype, pent_handle** out, int* bad_row);
@@ -142,7 +144,10 @@ int pent_handle_periodic(const pent_handle* h);          /* 1 for a periodic han
  * e,c,d,a,b,f,x: device, N*M elements each, interleaved like f (diagonal entry k of system i at
  * k*M+i).  x == f (in place) is allowed; any other overlap is undefined.  info: device int[M] or NULL; info[i] = 0, or (first bad row + 1) if system i met a
  * zero / non-finite pivot (its x is then unspecified; other systems are unaffected).
- * pent_factor_solve_batch factors and solves in ONE kernel and keeps nothing.
+ * pent_factor_solve_batch factors and solves in ONE kernel and keeps nothing.  For N >= 8 it cuts every system in the
+ * middle and gives each half a thread (top-down LU of the leading block, the same recurrence bottom-up on the reversed
+ * trailing block, a 4 x 4 interface system): x_i = A_i^{-1} f_i by a twisted factorisation without pivoting, which differs
+ * from the paper's LU by rounding only; info[i] is then the first bad pivot of the top-down half, else of the bottom-up half.
  * pent_factor_batch keeps the M factorisations in the handle (5*N*M elements of device memory)
  * for repeated pent_solve_batch_multi calls (M is fixed by the handle). */
 int pent_factor_solve_batch(int N, int64_t M, const void* e, const void* c, const void* d,

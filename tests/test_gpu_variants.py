@@ -74,6 +74,10 @@ def test_factor_solve_batch_nonsymmetric_two_threads_per_system(N, M):
     assert not info.cpu().numpy().any() and not rinfo.any()
     assert normwise(x.cpu().numpy(), ref) <= 1e-11
     assert residual(diags, x.cpu().numpy(), f) <= 1e-12
+    # in place (x == f, which include/pent.h allows): every read of f precedes the first write of x within a system
+    fi = fg.t.clone()
+    xi, _ = pent.pent_factor_solve_batch(N, M, e, c, d, a, b, fi, fi)
+    assert np.array_equal(xi.cpu().numpy(), x.cpu().numpy())
     # the last row is the FIRST pivot of the bottom-up thread: c[N-1] = 0 makes it exactly zero
     c2 = c.clone(); c2[N - 1, 5] = 0.0
     x2, info2 = pent.pent_factor_solve_batch(N, M, e, c2, d, a, b, fg.t)
