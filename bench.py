@@ -53,6 +53,9 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--graph", action="store_true",
+                    help="shared-A solve workloads: capture the K launches of the timed region in ONE CUDA graph and time its "
+                         "replay (removes the host side of a launch through the Python binding: cfg1, cfg2)")
     ap.add_argument("--suite", default="", metavar="OUT.jsonl",
                     help="run every workload of SUITE (one bench.py process each, --steps/--warmup as given) and "
                          "write their JSON lines, each with the command that made it, to OUT.jsonl")
@@ -62,7 +65,9 @@ def parse_args():
 # the workloads behind DESIGN.md section 10's table: (label, extra arguments)
 SUITE = [
     ("cfg1", ["--workload", "cfg1"]),
+    ("cfg1 (CUDA graph of the K launches)", ["--workload", "cfg1", "--graph"]),
     ("cfg2", ["--workload", "cfg2"]),
+    ("cfg2 (CUDA graph of the K launches)", ["--workload", "cfg2", "--graph"]),
     ("cfg3 f64", ["--workload", "cfg3"]),
     ("cfg3 f32", ["--workload", "cfg3", "--dtype", "f32"]),
     ("cfg3 thread-per-system (the paper's design)", ["--workload", "cfg3", "--kernel", "1"]),
@@ -340,13 +345,33 @@ def run_ours(args):
     sampler.start()
     # the timed region: K launches back to back on the launching stream, one event on each side
     # (an event between launches costs 2-3 us of stream latency: 10 % of a 28 us cfg2 kernel)
-    ev0.record(stream)
-    for i in range(args.steps):
-        solve()
-    ev1.record(stream)
+    if args.graph:
+        # the same K launches, captured once and replayed: what a launch-bound caller (a time loop of small solves) would do
+        cs = torch.cuda.Stream()
+        cs.wait_stream(stream)
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.stream(cs):
+            solve()                                  # every lazy attribute / cache is set before the capture
+            cs.synchronize()
+            with torch.cuda.graph(graph, stream=cs):
+                for i in range(args.steps):
+                    solve()
+        stream.wait_stream(cs)
+        graph.replay()                               # warm replay
+        torch.cuda.synchronize()
+        pent.launch_count(reset=True)
+        ev0.record(stream)
+        graph.replay()
+        ev1.record(stream)
+        graph_launches = args.steps
+    else:
+        ev0.record(stream)
+        for i in range(args.steps):
+            solve()
+        ev1.record(stream)
     barrier()
     clocks = sampler.stop()
-    launches = pent.launch_count()
+    launches = graph_launches if args.graph else pent.launch_count()
     total_ms = ev0.elapsed_time(ev1)
     # per-launch spread (min / median), outside the timed region, with an event after every launch
     nper = min(args.steps, 30)
@@ -410,6 +435,7 @@ def run_ours(args):
                              ("system-major f[i*N+k], " + ("LDG.256 loader" if args.rows_ldg else "bulk loads + STG.256 stores" if args.rows_stg
                                                          else "swizzled TMA loads + STG.256 stores" if args.rows_tma2d else "1-D bulk copies both ways")),
                    "kernel": kname, "band": int(pent.lib().pent_handle_band(h.ptr)),
+                   "launch": "K launches captured in one CUDA graph, replay timed" if args.graph else "K library calls back to back",
                    "cluster_ctas_along_k": ch["Q"], "systems_per_tile": ch["S"],
                    "l2": f"inputs+outputs {2 * esz * N * M >> 20} MiB per step exceed the 126 MB L2"},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",

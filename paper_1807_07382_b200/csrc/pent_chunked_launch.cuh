@@ -123,7 +123,9 @@ static int launch_inst(const pent_handle* h, const ChunkPlan& pl, int64_t M, con
             oc.resident = ncl;                                   // clusters resident at once
             oc.dev = dev; oc.threads = pl.threads; oc.smem = smem_total; oc.Q = pl.Q;
         }
-        if (oc.resident < 1) return PENT_ERR_ARG;
+        // no cluster of this size is schedulable here (a partitioned GPU, a 16-CTA cluster on a device whose GPCs are
+        // smaller): not an error of the caller; PENT_KERNEL_AUTO then runs the thread-per-system kernel
+        if (oc.resident < 1) return PENT_UNSUPPORTED;
         int64_t clusters = oc.resident;
         if (clusters > prm.ntiles) clusters = prm.ntiles;
         cfg.gridDim = dim3((unsigned)(clusters * pl.Q));

@@ -184,8 +184,10 @@ static PeriodicCoef<T> coef_of(const pent_handle* h)
 template <typename T>
 static int solve_periodic_t(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s, int kernel)
 {
-    if (kernel == PENT_KERNEL_AUTO && periodic_fused_supported(h, M, f))
-        return launch_solve_chunked_periodic(h, M, f, x, s);          // one kernel, 2 passes
+    if (kernel == PENT_KERNEL_AUTO && periodic_fused_supported(h, M, f)) {
+        const int rc = launch_solve_chunked_periodic(h, M, f, x, s);  // one kernel, 2 passes
+        if (rc != PENT_UNSUPPORTED) return rc;                         // (cluster size not schedulable on this device: unfused)
+    }
     if ((kernel & 0xff) == PENT_KERNEL_CHUNKED && kernel != PENT_KERNEL_CHUNKED) return PENT_ERR_ARG;
     // unfused: inner solve (chunked when kernel == PENT_KERNEL_CHUNKED or AUTO) + tail + rank-2 update
     int rc = pent_solve_batch_v(h->inner, M, f, x, (void*)s, kernel == PENT_KERNEL_CHUNKED ? PENT_KERNEL_AUTO : kernel);
