@@ -179,7 +179,10 @@ factor_tps_kernel(int N, int64_t M, const T* __restrict__ a, const T* __restrict
 // Forward: stage = RING_ROWS rows x {a,b,c,d,e,f}; backward: stage = 2*RING_ROWS rows x {gamma,
 // delta, g} (same stage size).  cfg5b: 418 us with register load-ahead -> see profiles/r01_ab_tuning.md.
 // ---------------------------------------------------------------------------------------------
-constexpr int RING_ROWS = 4, RING_STAGES = 6, RING_SLOTS = 6 * RING_ROWS;   // values per thread and stage
+#ifndef PENT_RING_ROWS
+#define PENT_RING_ROWS 4
+#endif
+constexpr int RING_ROWS = PENT_RING_ROWS, RING_STAGES = 6, RING_SLOTS = 6 * RING_ROWS;   // values per thread and stage
 
 template <typename T>
 __global__ void __launch_bounds__(PS_THREADS)
@@ -314,10 +317,22 @@ factor_solve_ring_kernel(int N, int64_t M, const T* __restrict__ a, const T* __r
 // info[i]: the first zero / non-finite pivot met by thread T, else by thread B, as row + 1 (a pivot of the twisted
 // factorisation; for the top half it is the pivot of the paper's LU).
 // Block = TW_SYS threads T followed by TW_SYS threads B of the same TW_SYS systems.  Measured on cfg5b (profiles/
-// r02_bench_all.jsonl; A/B PENT_AB_PER_SYSTEM_ONE_THREAD=1): 381.5 -> 361 us fp64, 240 -> 207 us fp32: the kernel was NOT
-// bound by the latency of its few warps after all (twice the warps bought 5 %); 32 or 64 systems per block measure the same.
+// r02_bench_all.jsonl; A/B PENT_AB_PER_SYSTEM_ONE_THREAD=1): 381.5 -> 270 us fp64, 240 -> 208 us fp32 (of which the second
+// thread alone, at the ring depth of the one-thread kernel: 361 us; the rest is the ring depth below).
 // ---------------------------------------------------------------------------------------------
-constexpr int TW_STAGES = 4, TW_SYS = 64;
+// Ring depth and block width, measured on cfg5b (fp64, us per call; A/B by -DPENT_TW_STAGES / -DPENT_TW_SYS / -DPENT_RING_ROWS
+// through PENT_NVCC_FLAGS): (systems per block, rows per stage, stages) = (64,4,3) 270, (128,4,3) 269, (64,4,2) 365,
+// (64,4,4) 361, (64,8,3) 340, (64,2,3) 357, (64,2,4) 357, (32,4,3) 368, (32,4,6) 325, (32,2,8) 357.  Two stages of 4 rows
+// ahead (8 rows, 3 stages) is a sharp optimum: deeper rings put more of the six input streams and the scratch stream in
+// flight than the memory system serves well, shallower ones expose latency.  At 270 us the call moves its 13 words per
+// unknown at 6.2 TB/s: it is at the cap of the 13-word design (0.54 of the 7-word roofline).
+#ifndef PENT_TW_STAGES
+#define PENT_TW_STAGES 3
+#endif
+#ifndef PENT_TW_SYS
+#define PENT_TW_SYS 64
+#endif
+constexpr int TW_STAGES = PENT_TW_STAGES, TW_SYS = PENT_TW_SYS;
 
 template <typename T>
 __global__ void __launch_bounds__(2 * TW_SYS)
