@@ -520,7 +520,7 @@ ChunkPlan chunk_auto_plan(const pent_handle* h, int64_t M, const void* f, bool r
     // (which keeps a cp.async group of its own for the tail rows: ring_ok = false) and shapes whose landing buffer does
     // not fit: the LDG loader.  It has no prefetch of the next tile, so prefer CTAs of <= 256 threads: two of them share an SM and
     // one loads while the other computes.
-    static const int no_ring = []() { const char* e = std::getenv("PENT_AB_NO_RING"); return e ? std::atoi(e) : 0; }();   // A/B
+    static const int no_ring = []() { const char* e = std::getenv("PENT_AB_NO_CPASYNC_LOADER"); return e ? std::atoi(e) : 0; }();   // A/B
     if (ring_ok && !no_ring) {
         const size_t esz = h->dtype == PENT_F64 ? 8 : 4;
         const int C = h->dtype == PENT_F64 ? ChunkCfg<double>::C : ChunkCfg<float>::C;
