@@ -144,3 +144,38 @@ def test_paper_time_loop_decay_and_convergence_order():
         errs.append(np.sqrt(np.mean((c[:, 0] - exact) ** 2)))
     slope = np.polyfit(np.log(Ns), np.log(errs), 1)[0]
     assert abs(slope + 2.0) <= 0.05
+
+
+# ---- the paper's time loop with the state on chip (KIND 3 of the step kernel) -------------------
+@pytest.mark.parametrize("N,M,steps,dtype,on_chip", [
+    (64, 40, 5, torch.float64, True), (96, 34, 4, torch.float64, True), (1024, 2406, 3, torch.float64, True),
+    (512, 300, 7, torch.float64, True), (256, 76, 6, torch.float32, True), (128, 4808, 2, torch.float32, True),
+    (1000, 50, 3, torch.float64, False), (40, 10, 3, torch.float64, False), (96, 20, 3, torch.float32, False),
+    (64, 41, 3, torch.float64, False),           # pitch not a multiple of 16 bytes: TMA cannot address the state
+])
+def test_periodic_time_loop_on_chip_parity(N, M, steps, dtype, on_chip):
+    """Crank-Nicolson steps A c+ = (2I - A) c with a NON-symmetric cyclic A and random states, every system against the
+    oracle (which forms (2I - A) c and solves, Eq. 7c; the kernel evaluates 2 A^{-1} c - c): wrap-around, the Navon
+    tail, Z folded into the chunk states, the explicit edge rows, ragged M, the leftover round in half-width tiles
+    (M = 2406: 151 tiles of 16 -> 148 + 6 half tiles; fp32 M = 4808: 151 tiles of 32).  N not a multiple of the chunk length runs the two-kernel path."""
+    pent = _pent()
+    f32 = dtype == torch.float32
+    diags = pin.random_periodic_diag_dominant(500 + N, N)
+    c0 = pin.uniform_pm1(501 + N, 0, N, M)
+    if f32:
+        diags = [np.asarray(v, dtype=np.float32).astype(np.float64) for v in diags]
+        c0 = c0.astype(np.float32).astype(np.float64)
+    h = _handle(diags, dtype)
+    assert (pent.lib().pent_step_kernel_choice(h.ptr, M) == pent.KERNEL_CHUNKED) == on_chip
+    cg = guarded(c0, dtype)
+    pent.pent_step_batch(h, M, cg.t, steps, kind=1)
+    cg.check()
+    got = cg.numpy().astype(np.float64)
+    ref = oracle.step_periodic_batch(oracle.factor_periodic(*diags), c0, steps, nthreads=8)
+    assert normwise(got, ref) <= (2e-5 if f32 else 1e-11)
+    # n steps in one launch = n launches of one step, bit for bit
+    c1 = guarded(c0, dtype)
+    for _ in range(steps):
+        pent.pent_step_batch(h, M, c1.t, 1, kind=1)
+    c1.check()
+    assert np.array_equal(c1.numpy(), cg.numpy())
