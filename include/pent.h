@@ -57,7 +57,9 @@ enum {
     PENT_ERR_ARG = 1,      /* null pointer, N < 1, M < 0, bad dtype / params, handle of the wrong kind */
     PENT_ERR_PIVOT = 2,    /* zero or non-finite pivot alpha_k (shared-A factor only)                   */
     PENT_ERR_CUDA = 3,     /* a CUDA call failed; pent_last_cuda_error() holds its cudaError_t          */
-    PENT_ERR_ALLOC = 4     /* host or device allocation failed                                          */
+    PENT_ERR_ALLOC = 4,    /* host or device allocation failed                                          */
+    PENT_ERR_TOO_LARGE = 5 /* pent_factor_solve_batch_noalloc: the problem needs more scratch than the static
+                              array holds (pent_noalloc_scratch_bytes)                                  */
 };
 
 /* Kernel choice for pent_solve_batch_v (measurement / tests).  AUTO is what pent_solve_batch uses. */
@@ -159,6 +161,18 @@ int pent_factor_solve_batch(int N, int64_t M, const void* e, const void* c, cons
 int pent_factor_solve_batch_ws(int N, int64_t M, const void* e, const void* c, const void* d,
                                const void* a, const void* b, const void* f, void* x,
                                pent_dtype dtype, int* info, void* workspace, void* stream);
+/* Same operation for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): the scratch is a static device array inside the library, so the call makes NO cudaMalloc, cudaFree or
+ * stream-ordered allocation.  Limit: 3 * N * M' * sizeof(element) <= pent_noalloc_scratch_bytes() = 32 MiB, M' = M rounded
+ * up to a multiple of 64 (e.g. N = 1024: M <= 1344 fp64, 2688 fp32); beyond it PENT_ERR_TOO_LARGE and nothing is launched.
+ * Every GPU that loads the library holds those 32 MiB until the process exits.  All calls share the array: calls that
+ * overlap on the GPU (different streams, concurrent graph branches) RACE on it; calls ordered on one stream are safe and
+ * nothing needs clearing between them.  The first call on a device looks the array's address up (cudaGetSymbolAddress)
+ * and sets a function attribute: make one call before starting a graph capture.  Arguments as pent_factor_solve_batch. */
+int pent_factor_solve_batch_noalloc(int N, int64_t M, const void* e, const void* c, const void* d,
+                                    const void* a, const void* b, const void* f, void* x,
+                                    pent_dtype dtype, int* info, void* stream);
+int64_t pent_noalloc_scratch_bytes(void);
 int pent_factor_batch(int N, int64_t M, const void* e, const void* c, const void* d,
                       const void* a, const void* b, pent_dtype dtype, pent_handle** out,
                       int* info, void* stream);

@@ -41,7 +41,8 @@ def rows_kernel_choice(h: "Handle", M: int) -> dict:
     return {"kernel": "solve_chunked_kernel", "Q": (v >> 8) & 0xff, "S": (v >> 16) & 0xff, "path": path}
 
 
-_ERR = {1: "invalid argument", 2: "zero or non-finite pivot", 3: "CUDA error", 4: "allocation failure"}
+_ERR = {1: "invalid argument", 2: "zero or non-finite pivot", 3: "CUDA error", 4: "allocation failure",
+        5: "problem needs more scratch than the library's static array holds (pent_noalloc_scratch_bytes)"}
 
 _lib = None
 
@@ -91,6 +92,9 @@ def lib() -> C.CDLL:
     L.pent_destroy.restype = None
     L.pent_factor_solve_batch.argtypes = [ci, i64, vp, vp, vp, vp, vp, vp, vp, ci, vp, vp]
     L.pent_factor_solve_batch_ws.argtypes = [ci, i64, vp, vp, vp, vp, vp, vp, vp, ci, vp, vp, vp]
+    L.pent_factor_solve_batch_noalloc.argtypes = [ci, i64, vp, vp, vp, vp, vp, vp, vp, ci, vp, vp]
+    L.pent_noalloc_scratch_bytes.argtypes = []
+    L.pent_noalloc_scratch_bytes.restype = i64
     L.pent_factor_batch.argtypes = [ci, i64, vp, vp, vp, vp, vp, ci, C.POINTER(vp), vp, vp]
     L.pent_solve_batch_multi.argtypes = [vp, vp, vp, vp]
     L.pent_step_batch.argtypes = [vp, C.POINTER(pent_step_params), i64, vp, vp, ci, vp]
@@ -282,6 +286,25 @@ def pent_factor_solve_batch(N: int, M: int, e, c, d, a, b, f, x=None, info=None,
                                             _dt(f), info.data_ptr(),
                                             0 if workspace is None else workspace.data_ptr(),
                                             _stream(stream)))
+    return x, info
+
+
+def pent_noalloc_scratch_bytes() -> int:
+    """Size of the static device array behind pent_factor_solve_batch_noalloc (bytes)."""
+    return int(lib().pent_noalloc_scratch_bytes())
+
+
+def pent_factor_solve_batch_noalloc(N: int, M: int, e, c, d, a, b, f, x, info, stream=None):
+    """pent_factor_solve_batch for callers that cannot allocate: the library allocates NOTHING in this call (its
+    scratch is a static 32 MiB device array), so the caller passes x and info (int32[M]) as well.  PentError code 5 when
+    3*N*ceil64(M)*itemsize exceeds pent_noalloc_scratch_bytes().  Calls that overlap on the GPU race on the array."""
+    _dt(f)
+    for t, n in zip((e, c, d, a, b, f, x), "ecdabfx"):
+        _batch(t, n, (N, M), f.dtype)
+    _vec(info, "info", M, torch.int32)
+    _check(lib().pent_factor_solve_batch_noalloc(N, M, e.data_ptr(), c.data_ptr(), d.data_ptr(), a.data_ptr(),
+                                                 b.data_ptr(), f.data_ptr(), x.data_ptr(), _dt(f), info.data_ptr(),
+                                                 _stream(stream)))
     return x, info
 
 

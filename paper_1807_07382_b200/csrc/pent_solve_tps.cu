@@ -679,3 +679,86 @@ extern "C" int pent_solve_batch_multi(const pent_handle* h, const void* f, void*
     PENT_LAUNCH_CHECK();
     return PENT_OK;
 }
+
+// ---------------------------------------------------------------------------------------------
+// pent_factor_solve_batch_noalloc -- the per-system factor + solve for callers that cannot allocate (code under CUDA
+// graph capture, tight serving loops, harnesses that forbid cudaMalloc).  Same kernels as pent_factor_solve_batch;
+// the scratch for gamma_k, delta_k, g_k lives in the file-scope device array below instead of a workspace, so the
+// call makes no cudaMalloc / cudaFree / stream-ordered allocation of any kind.
+//   * Every GPU that loads libpent.so holds the PENT_NOALLOC_SCRATCH_BYTES of the array until the process exits.
+//   * In HOST code the array's name is a host-side stand-in, not a device address: its device address is looked
+//     up once per device, with that device current, by cudaGetSymbolAddress (return code checked) and cached.
+//   * All calls share the array: two calls that overlap on the GPU (different streams, or graph branches that may
+//     run concurrently) race on it.  Nothing has to be cleared between calls: every word a call reads was written
+//     earlier by the same thread of the same call (forward loop writes rows k, the back substitution reads them).
+// ---------------------------------------------------------------------------------------------
+#define PENT_NOALLOC_SCRATCH_BYTES (32u << 20)
+static __device__ __align__(256) unsigned char g_noalloc_scratch[PENT_NOALLOC_SCRATCH_BYTES];
+
+namespace pent {
+constexpr int NOALLOC_MAX_DEVICES = 64;
+static std::atomic<void*> g_noalloc_ptr[NOALLOC_MAX_DEVICES];
+
+// device address of g_noalloc_scratch on the CURRENT device (set-up: once per device)
+static int noalloc_scratch(void** out)
+{
+    int dev = 0;
+    PENT_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return PENT_ERR_ARG;
+    void* p = g_noalloc_ptr[dev].load(std::memory_order_acquire);
+    if (!p) {
+        PENT_CUDA(cudaGetSymbolAddress(&p, g_noalloc_scratch));
+        if (!p) return cuda_fail(cudaErrorInvalidSymbol);
+        g_noalloc_ptr[dev].store(p, std::memory_order_release);     // (two racing threads store the same address)
+    }
+    *out = p;
+    return PENT_OK;
+}
+
+template <typename T>
+static int factor_solve_noalloc_impl(int N, int64_t M, const void* e, const void* c, const void* d, const void* a,
+                                     const void* b, const void* f, void* x, int* info, cudaStream_t s)
+{
+    void* sp = nullptr;
+    const int rc = noalloc_scratch(&sp);
+    if (rc != PENT_OK) return rc;
+    T* scratch = (T*)sp;
+    if (N >= 8) {                        // two threads per system: scratch [block][k][3][TW_SYS]
+        const size_t smem = ((size_t)TW_STAGES * RING_SLOTS * 2 * TW_SYS + 2 * 7 * TW_SYS) * sizeof(T);
+        static SmemOnce mark2;
+        PENT_CUDA(ensure_dynamic_smem(mark2, factor_solve_twist_kernel<T>, smem));
+        const unsigned nb = (unsigned)((M + TW_SYS - 1) / TW_SYS);
+        factor_solve_twist_kernel<T><<<nb, 2 * TW_SYS, smem, s>>>(N, M, (const T*)a, (const T*)b, (const T*)c, (const T*)d,
+                                                                   (const T*)e, (const T*)f, (T*)x, scratch, info);
+    } else {                             // one thread per system: scratch [block][k][3][PS_THREADS]
+        const size_t smem = (size_t)RING_STAGES * RING_SLOTS * PS_THREADS * sizeof(T);
+        static SmemOnce mark;
+        PENT_CUDA(ensure_dynamic_smem(mark, factor_solve_ring_kernel<T>, smem));
+        const unsigned nb = (unsigned)((M + PS_THREADS - 1) / PS_THREADS);
+        factor_solve_ring_kernel<T><<<nb, PS_THREADS, smem, s>>>(N, M, (const T*)a, (const T*)b, (const T*)c, (const T*)d,
+                                                                 (const T*)e, (const T*)f, (T*)x, scratch, info);
+    }
+    count_launch();
+    PENT_LAUNCH_CHECK();
+    return PENT_OK;
+}
+}  // namespace pent
+
+extern "C" int64_t pent_noalloc_scratch_bytes(void) { return (int64_t)PENT_NOALLOC_SCRATCH_BYTES; }
+
+extern "C" int pent_factor_solve_batch_noalloc(int N, int64_t M, const void* e, const void* c, const void* d,
+                                               const void* a, const void* b, const void* f, void* x,
+                                               pent_dtype dtype, int* info, void* stream)
+{
+    if (N < 1 || M < 0 || !e || !c || !d || !a || !b || !f || !x) return PENT_ERR_ARG;
+    if (dtype != PENT_F64 && dtype != PENT_F32) return PENT_ERR_ARG;
+    if (M == 0) return PENT_OK;
+    // 3 * N * M' elements, M' = M rounded up to a multiple of 64 (both kernels' block widths divide 64 or equal it)
+    static_assert(64 % pent::PS_THREADS == 0 && (64 % pent::TW_SYS == 0 || pent::TW_SYS == 64), "scratch size formula");
+    const uint64_t esz = dtype == PENT_F64 ? 8 : 4;
+    const uint64_t Mp = ((uint64_t)M + 63) / 64 * 64;
+    if (Mp > (uint64_t)PENT_NOALLOC_SCRATCH_BYTES / (3 * esz * (uint64_t)N)) return PENT_ERR_TOO_LARGE;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (dtype == PENT_F64) return pent::factor_solve_noalloc_impl<double>(N, M, e, c, d, a, b, f, x, info, s);
+    return pent::factor_solve_noalloc_impl<float>(N, M, e, c, d, a, b, f, x, info, s);
+}
