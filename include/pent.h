@@ -259,6 +259,11 @@ int pent_handle_device(const pent_handle* h);            /* CUDA device ordinal 
  * SPD matrices I + sigma L^2: about 5 sqrt(sigma).  Shared-A handles (periodic: of the block E). */
 int pent_handle_growth(const pent_handle* h, double* out3);
 int pent_handle_band(const pent_handle* h);              /* shared A: 1 = tridiagonal (a == e == 0), 2 = pentadiagonal; -1 */
+/* Cluster kernels (Q = 2, 4, 8, 16 CTAs split k): with how many neighbouring ranks on each side a CTA NEEDS to exchange its
+ * block aggregates (the kernels use it for Q >= 8, where it pays).  1 when every block transfer product of the handle is below 1e-25 (a state entering a block of >= 32 chunks
+ * has decayed to nothing by its end: the usual case for diagonally dominant matrices), else Q - 1 (every rank).  -1: no
+ * tables for that cluster size. */
+int pent_handle_exchange_depth(const pent_handle* h, int Q);
 /* Copies the fp64 factor arrays (N doubles each; any pointer may be NULL) to HOST memory:
  * eps, beta, alpha = bands of L, gamma, delta = bands of R (Eq. 13).  Shared-A only. */
 int pent_handle_factors(const pent_handle* h, double* eps, double* beta, double* alpha,

@@ -110,6 +110,7 @@ def lib() -> C.CDLL:
     L.pent_handle_m.restype = i64
     L.pent_handle_device.argtypes = [vp]
     L.pent_handle_band.argtypes = [vp]
+    L.pent_handle_exchange_depth.argtypes = [vp, ci]
     L.pent_handle_growth.argtypes = [vp, C.POINTER(C.c_double)]
     L.pent_release_thread_cache.argtypes = []
     L.pent_release_thread_cache.restype = None

@@ -603,7 +603,11 @@ __device__ __forceinline__ void chunk_state_scan_lean(const ScanLane& ln, const 
     }
 }
 
-template <typename T, int S, bool CLUSTER, bool PER = false>
+// NBR (CLUSTER, not PER): neighbour-only exchange.  When every block transfer product of the handle is below 1e-25
+// (pent_handle::xdepth == 1: a state entering a block of >= 32 chunks has decayed to nothing by its end) the state
+// entering this CTA's block is the adjacent rank's aggregate alone: one send and one receive per direction, no chain
+// over the ranks.  A compile-time variant so that the full-exchange code (and its SASS) stays what it was.
+template <typename T, int S, bool CLUSTER, bool PER = false, bool NBR = false>
 __device__ __forceinline__ void chunk_state_scan(const ScanGeom& g, const T* wtab, typename Pair<T>::type* stE,
                                                  typename Pair<T>::type* stS, int sys, int q, bool ok,
                                                  int rank, int Q, typename Pair<T>::type* aggF,
@@ -630,10 +634,16 @@ __device__ __forceinline__ void chunk_state_scan(const ScanGeom& g, const T* wta
     if constexpr (CLUSTER) {
         // y = F of chunk q for a ZERO state entering the block.  The last chunk's value is the
         // block aggregate: send it to every later rank, then chain the earlier ranks' aggregates.
+        if constexpr (NBR) {
+            if (ok && q == P - 1 && rank + 1 < Q) st_async_pair(&aggF[rank * S + sys], &bars[BAR_F], rank + 1, y0, y1);
+            if (agg_bytes_f) mbar_wait(&bars[BAR_F], parity);
+            if (rank > 0) { T2 a = aggF[(rank - 1) * S + sy]; fin0 = a.x; fin1 = a.y; }
+        } else {
         if (ok && q == P - 1)
             for (int rr = rank + 1; rr < Q; ++rr) st_async_pair(&aggF[rank * S + sys], &bars[BAR_F], rr, y0, y1);
         if (agg_bytes_f) mbar_wait(&bars[BAR_F], parity);
-        for (int rr = 0; rr < rank; ++rr) {        // F_in(rr+1) = aggF[rr] + TPhiBlock(rr) F_in(rr)
+        }
+        for (int rr = 0; rr < (NBR ? 0 : rank); ++rr) {        // F_in(rr+1) = aggF[rr] + TPhiBlock(rr) F_in(rr)
             T2 a = aggF[rr * S + sy];
             T n0 = a.x, n1 = a.y;
             mat2_acc(n0, n1, wtab + 12 * P + 4 * rr, 1, fin0, fin1);
@@ -678,12 +688,17 @@ __device__ __forceinline__ void chunk_state_scan(const ScanGeom& g, const T* wta
                 for (int rr = 0; rr < Q; ++rr) st_async_pair(&aggB[rank * S + sys], &bars[BAR_B], rr, z0, z1);
                 if (rank == per->pp->ra)
                     for (int rr = 0; rr < Q; ++rr) st_async_pair(&per->yab[sys], &bars[BAR_B], rr, ya, yb);
+            } else if constexpr (NBR) {
+                if (rank > 0) st_async_pair(&aggB[rank * S + sys], &bars[BAR_B], rank - 1, z0, z1);
             } else {
                 for (int rr = 0; rr < rank; ++rr) st_async_pair(&aggB[rank * S + sys], &bars[BAR_B], rr, z0, z1);
             }
         }
         if (agg_bytes_b) mbar_wait(&bars[BAR_B], parity);
-        for (int rr = Q - 1; rr > rank; --rr) {   // B_in(rr-1) = aggB[rr] + TPsiBlock(rr) B_in(rr)
+        if constexpr (NBR) {
+            if (rank < Q - 1) { T2 a = aggB[(rank + 1) * S + sy]; bin0 = a.x; bin1 = a.y; }
+        }
+        for (int rr = Q - 1; rr > (NBR ? Q - 1 : rank); --rr) {   // B_in(rr-1) = aggB[rr] + TPsiBlock(rr) B_in(rr)
             T2 a = aggB[rr * S + sy];
             T n0 = a.x, n1 = a.y;
             mat2_acc(n0, n1, wtab + 12 * P + 4 * PENT_MAXQ + 4 * rr, 1, bin0, bin1);
@@ -729,7 +744,7 @@ __device__ __forceinline__ void chunk_state_scan(const ScanGeom& g, const T* wta
 
 // stage 3 for BAND = 1: scalar states, scalar transfer coefficients (layout: see w_level_off with BAND = 1).
 //   F_q = E~_q + TPhi_q F_{q-1};  B_q = (S^_q + TX_q F_{q-1}) + TPsi_q B_{q+1}
-template <typename T, int S, bool CLUSTER>
+template <typename T, int S, bool CLUSTER, bool NBR = false>
 __device__ __forceinline__ void tri_state_scan(const ScanGeom& g, const T* wtab, T* stE, T* stS, int sys, int q, bool ok,
                                                int rank, int Q, T* aggF, T* aggB, uint64_t* bars,
                                                uint32_t agg_bytes_f, uint32_t agg_bytes_b, uint32_t parity)
@@ -749,10 +764,16 @@ __device__ __forceinline__ void tri_state_scan(const ScanGeom& g, const T* wtab,
     }
     T fin = 0;
     if constexpr (CLUSTER) {
+        if constexpr (NBR) {
+            if (ok && q == P - 1 && rank + 1 < Q) st_async_one(&aggF[rank * S + sys], &bars[BAR_F], rank + 1, y);
+            if (agg_bytes_f) mbar_wait(&bars[BAR_F], parity);
+            if (rank > 0) fin = aggF[(rank - 1) * S + sy];
+        } else {
         if (ok && q == P - 1)
             for (int rr = rank + 1; rr < Q; ++rr) st_async_one(&aggF[rank * S + sys], &bars[BAR_F], rr, y);
         if (agg_bytes_f) mbar_wait(&bars[BAR_F], parity);
         for (int rr = 0; rr < rank; ++rr) fin = fma(wtab[3 * P + rr], fin, aggF[rr * S + sy]);
+        }
         if (ok && rank > 0) y = fma(wtab[P + q], fin, y);                     // PF_q F_in
     }
     T f = shfl_up_t(y, 1, Pw);
@@ -768,10 +789,16 @@ __device__ __forceinline__ void tri_state_scan(const ScanGeom& g, const T* wtab,
     }
     T bin = 0;
     if constexpr (CLUSTER) {
+        if constexpr (NBR) {
+            if (ok && q == 0 && rank > 0) st_async_one(&aggB[rank * S + sys], &bars[BAR_B], rank - 1, z);
+            if (agg_bytes_b) mbar_wait(&bars[BAR_B], parity);
+            if (rank < Q - 1) bin = aggB[(rank + 1) * S + sy];
+        } else {
         if (ok && q == 0)
             for (int rr = 0; rr < rank; ++rr) st_async_one(&aggB[rank * S + sys], &bars[BAR_B], rr, z);
         if (agg_bytes_b) mbar_wait(&bars[BAR_B], parity);
         for (int rr = Q - 1; rr > rank; --rr) bin = fma(wtab[3 * P + PENT_MAXQ + rr], bin, aggB[rr * S + sy]);
+        }
         if (ok && rank < Q - 1) z = fma(wtab[2 * P + q], bin, z);             // PB_q B_in
     }
     T b = shfl_down_t(z, 1, Pw);

@@ -61,7 +61,8 @@ struct ChunkParams {
 // LM = layout / loader mode, compile-time so that every instantiation carries only its own data path (a run-time
 // switch over all of them cost 80-120 bytes of register spills in every instance): 0 = interleaved batch (TMA, or
 // the LDG loader when prm.ldg == 1); 2, 3, 4 = system-major batch, the modes described at ChunkParams::ldg.
-template <typename T, int S, bool CLUSTER, bool PER, int BAND, int LM>
+// NBR: neighbour-only cluster exchange (see chunk_state_scan); chosen by the launcher for Q >= 4 when the handle allows it.
+template <typename T, int S, bool CLUSTER, bool PER, int BAND, int LM, bool NBR = false>
 __global__ void __launch_bounds__(CHUNK_MAX_THREADS, 1)
 solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T> prm,
                      const __grid_constant__ PeriodicParams<T> pp, const __grid_constant__ CUtensorMap tmx)
@@ -174,9 +175,12 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
     }
     // every CTA of the cluster is resident, with its mbarriers initialised, before any DSMEM store
     if constexpr (CLUSTER) cluster_sync_all();
-    const uint32_t agg_bytes_f = (uint32_t)(rank * S * sizeof(ST));                 // from the earlier ranks
+    static_assert(!NBR || (CLUSTER && !PER), "neighbour-only exchange: cluster kernels, non-periodic");
+    const uint32_t agg_bytes_f = NBR ? (uint32_t)((rank > 0 ? 1 : 0) * S * sizeof(ST))   // from the rank before
+                                     : (uint32_t)(rank * S * sizeof(ST));                 // from the earlier ranks
     // from the later ranks; periodic: from EVERY rank (itself included) plus (y_{n-2}, y_{n-1}) from rank ra
-    const uint32_t agg_bytes_b = PER ? (uint32_t)((prm.Q + 1) * S * sizeof(ST))
+    const uint32_t agg_bytes_b = NBR ? (uint32_t)((rank < prm.Q - 1 ? 1 : 0) * S * sizeof(ST))
+                               : PER ? (uint32_t)((prm.Q + 1) * S * sizeof(ST))
                                      : (uint32_t)((prm.Q - 1 - rank) * S * sizeof(ST));
     mbar_wait(&bars[0], 0);
 
@@ -365,10 +369,10 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
             for (int r = 0; r < rounds; ++r) {
                 const int sys = (r * nwarps + warp) * G + grp;
                 if constexpr (BAND == 2)
-                    chunk_state_scan<T, S, CLUSTER, PER>(geom, wtab, stE, stS, sys, q, (sys < S) && (q < P), rank,
+                    chunk_state_scan<T, S, CLUSTER, PER, NBR>(geom, wtab, stE, stS, sys, q, (sys < S) && (q < P), rank,
                                                          prm.Q, aggF, aggB, bars, agg_bytes_f, agg_bytes_b, parity, &per);
                 else
-                    tri_state_scan<T, S, CLUSTER>(geom, wtab, stE, stS, sys, q, (sys < S) && (q < P), rank, prm.Q,
+                    tri_state_scan<T, S, CLUSTER, NBR>(geom, wtab, stE, stS, sys, q, (sys < S) && (q < P), rank, prm.Q,
                                                   aggF, aggB, bars, agg_bytes_f, agg_bytes_b, parity);
             }
         }

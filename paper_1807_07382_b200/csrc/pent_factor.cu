@@ -244,6 +244,15 @@ extern "C" int pent_handle_growth(const pent_handle* h, double* out3)
     return PENT_OK;
 }
 extern "C" int pent_handle_band(const pent_handle* h) { return (h && h->kind == 0) ? (h->periodic ? 2 : h->band) : -1; }
+extern "C" int pent_handle_exchange_depth(const pent_handle* h, int Q)
+{
+    if (!h || h->kind != 0) return -1;
+    if (h->periodic) return pent_handle_exchange_depth(h->inner, Q) < 0 ? -1 : (Q > 1 ? Q - 1 : 1);   // the fused periodic kernel exchanges with every rank
+    int j = 0;
+    while ((1 << j) < Q) ++j;
+    if ((1 << j) != Q || j >= PENT_NQ || !h->cf[j]) return -1;
+    return h->band == 1 ? h->xdepth1[j] : h->xdepth[j];
+}
 
 extern "C" int pent_handle_factors(const pent_handle* h, double* eps, double* beta, double* alpha,
                                    double* gamma, double* delta)

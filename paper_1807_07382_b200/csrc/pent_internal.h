@@ -33,6 +33,10 @@ struct pent_handle {
     void* cf[PENT_NQ];
     int cfP[PENT_NQ];
     int lev_f[PENT_NQ], lev_b[PENT_NQ];   // Kogge-Stone levels the chunk-state scans need
+    // cluster exchange depth: how many neighbouring ranks on each side a CTA exchanges block aggregates with: 1 when
+    // every block transfer product is below 1e-25 (diagonally dominant matrices: the state entering a block of >= 32
+    // chunks has decayed to nothing by its end), else Q - 1 (every rank); xdepth1: the tridiagonal tables
+    int xdepth[PENT_NQ], xdepth1[PENT_NQ];
     // the same for the tridiagonal instantiation (band == 1 only): 5-word coefficient rows, scalar transfers
     void* cf1[PENT_NQ];
     int lev_f1[PENT_NQ], lev_b1[PENT_NQ];

@@ -155,6 +155,10 @@ __global__ void build_chunk_products_kernel(int Pl, int Q, const double* __restr
                 for (int j = Pl - 1; j >= 0; --j) mat2_mul(b, t + j * 12 + 8, b);   // TPsi_j ... TPsi_last
             }
             for (int e = 0; e < 4; ++e) { blkm[4 * r + e] = f[e]; blkm[4 * PENT_MAXQ + 4 * r + e] = b[e]; }
+            // levels[8]: some block transfer product is not negligible -> the cluster must exchange with every rank
+            if (r < Q)
+                for (int e = 0; e < 4; ++e)
+                    if (!(fabs(f[e]) < 1e-25) || !(fabs(b[e]) < 1e-25)) atomicMax(&levels[8], 1);
         }
     }
     __syncthreads();
@@ -255,6 +259,7 @@ __global__ void build_tri_products_kernel(int Pl, int Q, const double* __restric
                 for (int j = 0; j < Pl; ++j) { f *= t[j * 3]; b *= t[j * 3 + 2]; }
             }
             blkm[r] = f; blkm[PENT_MAXQ + r] = b;
+            if (r < Q && (!(fabs(f) < 1e-25) || !(fabs(b) < 1e-25))) atomicMax(&levels[8], 1);
         }
     }
     __syncthreads();
@@ -302,10 +307,10 @@ static int build_tables_t(pent_handle* h, int j, cudaStream_t s)
     // temporaries are stream-ordered allocations on the factor's private stream (cudaFree would synchronise
     // the whole device)
     auto release = [&]() { if (tmat) cudaFreeAsync(tmat, s); if (lev) cudaFreeAsync(lev, s); };
-    // lev: 2 ints (levels) followed, 8-byte aligned, by 3 x 8 bytes (growth of Phi, X, Psi)
+    // lev: 2 ints (levels) followed, 8-byte aligned, by 3 x 8 bytes (growth of Phi, X, Psi), then int [8] = full-exchange flag
     cudaError_t le = cudaMallocAsync((void**)&tmat, sizeof(double) * 12 * Pl * Q, s);
-    if (le == cudaSuccess) le = cudaMallocAsync((void**)&lev, 32, s);
-    if (le == cudaSuccess) le = cudaMemsetAsync(lev, 0, 32, s);
+    if (le == cudaSuccess) le = cudaMallocAsync((void**)&lev, 48, s);
+    if (le == cudaSuccess) le = cudaMemsetAsync(lev, 0, 48, s);
     unsigned long long* growth = (BAND == 2 && j == 0 && lev) ? reinterpret_cast<unsigned long long*>(lev + 2) : nullptr;
     if (le == cudaSuccess) le = cudaMemsetAsync(cfj, 0, tlen * Q * sizeof(T), s);
     if (le != cudaSuccess) {            // temporaries are released on every path; h->cf[j] belongs to the handle
@@ -323,14 +328,15 @@ static int build_tables_t(pent_handle* h, int j, cudaStream_t s)
     }
     count_launch(2);
     le = cudaGetLastError();
-    int hl[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-    if (le == cudaSuccess) le = cudaMemcpyAsync(hl, lev, 32, cudaMemcpyDeviceToHost, s);
+    int hl[12] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+    if (le == cudaSuccess) le = cudaMemcpyAsync(hl, lev, 48, cudaMemcpyDeviceToHost, s);
     release();
     if (le == cudaSuccess) le = cudaStreamSynchronize(s);
     if (le != cudaSuccess) return cuda_fail(le);
     if (growth) std::memcpy(h->growth, hl + 2, 3 * sizeof(double));
-    if (BAND == 2) { h->cfP[j] = Pl; h->lev_f[j] = hl[0]; h->lev_b[j] = hl[1]; }
-    else { h->lev_f1[j] = hl[0]; h->lev_b1[j] = hl[1]; }
+    const int xd = (hl[8] || Q < 2) ? (Q > 1 ? Q - 1 : 1) : 1;
+    if (BAND == 2) { h->cfP[j] = Pl; h->lev_f[j] = hl[0]; h->lev_b[j] = hl[1]; h->xdepth[j] = xd; }
+    else { h->lev_f1[j] = hl[0]; h->lev_b1[j] = hl[1]; h->xdepth1[j] = xd; }
     return PENT_OK;
 }
 
@@ -715,7 +721,15 @@ int launch_solve_chunked(const pent_handle* h, int64_t M, const void* f, void* x
 static int launch_plan(const pent_handle* h, const ChunkPlan& pl, int64_t M, const void* f, void* x, cudaStream_t s)
 {
     const bool cl = pl.Q > 1;
-#define PENT_INST(T_, S_, B_) (cl ? launch_inst<T_, S_, true, false, B_>(h, pl, M, f, x, s, nullptr) \
+    // Neighbour-only exchange (chunk_state_scan, NBR): clusters of >= 8 CTAs whose handle says that a state does not survive
+    // a whole block (pent_handle::xdepth == 1).  Measured against the all-ranks exchange (A/B: PENT_AB_FULL_EXCHANGE=1 in the
+    // environment; M as in bench.py's suite): N=8192 (Q=8) 485 -> 409 us, N=12288 (Q=16) 528 -> 354, N=16384 (Q=16) 834 -> 654.
+    // With 4 CTAs it is SLOWER (cfg5a 417 -> 437 us, fp32 200 -> 215: the all-ranks wait keeps the four CTAs of a tile in
+    // lock-step, which their shared HBM rows reward), with 2 CTAs the neighbour is every rank: both run the full exchange.
+    static const int full = []() { const char* e = std::getenv("PENT_AB_FULL_EXCHANGE"); return e ? std::atoi(e) : 0; }();
+    const bool nbr = pl.Q >= 8 && !full && (pl.band == 2 ? h->xdepth[pl.j] : h->xdepth1[pl.j]) == 1;
+#define PENT_INST(T_, S_, B_) (cl ? (nbr ? launch_inst<T_, S_, true, false, B_, 0, true>(h, pl, M, f, x, s, nullptr)  \
+                                         : launch_inst<T_, S_, true, false, B_>(h, pl, M, f, x, s, nullptr))          \
                                   : launch_inst<T_, S_, false, false, B_>(h, pl, M, f, x, s, nullptr))
     if (h->dtype == PENT_F64) {
         if (pl.S == 16) return pl.band == 1 ? PENT_INST(double, 16, 1) : PENT_INST(double, 16, 2);

@@ -268,6 +268,29 @@ def test_chunked_cluster_slowly_decaying_coupling(Q, S):
     assert res_gpu <= max(1e-12, 2.0 * max(res_cpu))
 
 
+def test_cluster_exchange_depth_and_full_exchange_on_a_large_cluster():
+    """The cluster kernels exchange block aggregates with ONE neighbour on each side when every block transfer product is
+    below 1e-25 (diagonally dominant matrices; covered by the shape tests above at Q = 4, 8, 16) and with every rank
+    otherwise.  Here: the handle reports the depth, and a matrix whose coupling survives a whole block (sigma = 1e5 at
+    N = 4096 on 8 CTAs: 0.944^512 = 1e-13 per block) is solved with the full exchange, every system against the truth."""
+    pent = _pent()
+    L = pent.lib()
+    for N, sigma, Q, want in ((4096, 0.5, 4, 1), (8192, 10.0, 8, 1), (16384, 1.0, 16, 1), (1024, 1.1e4, 4, 3),
+                              (4096, 1e5, 8, 7), (1024, 10.0, 2, 1)):
+        a, b, c, d, e = (torch.tensor(v) for v in pin.diagonals_I_plus_sigma_L2(N, sigma))
+        h = pent.pent_factor(N, e, c, d, a, b)
+        assert L.pent_handle_exchange_depth(h.ptr, Q) == want, (N, sigma, Q)
+    N, M, sigma = 4096, 48, 1e5
+    diags = pin.diagonals_I_plus_sigma_L2(N, sigma)
+    f = pin.uniform_pm1(83, 0, N, M)
+    x, _ = gpu_solve(diags, f, kernel=pent.KERNEL_CHUNKED_CFG(8, 16))
+    fac = oracle.factor(*diags)
+    ref, truth, order = oracle.solve_batch(fac, f), oracle.ld_solve_batch(diags, f), chunked_order_solve_fp64(fac, f)
+    print(f"sigma=1e5 N=4096 Q=8: vs long double: GPU {normwise(x, truth):.3e}, fp64 oracle {normwise(ref, truth):.3e}, "
+          f"fp64 CPU in chunked order {normwise(order, truth):.3e}")
+    assert normwise(x, truth) <= envelope_tol(1e-11, truth, ref, order)
+
+
 @pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
 @pytest.mark.parametrize("N,M", [(1024, 1001), (512, 333), (4096, 77), (2000, 129), (100, 7), (1000, 2051), (3000, 515),
                                  (8192, 35), (16384, 19), (1024, 5001)])
