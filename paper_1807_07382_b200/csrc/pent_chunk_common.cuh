@@ -635,9 +635,10 @@ __device__ __forceinline__ void chunk_state_scan(const ScanGeom& g, const T* wta
         // y = F of chunk q for a ZERO state entering the block.  The last chunk's value is the
         // block aggregate: send it to every later rank, then chain the earlier ranks' aggregates.
         if constexpr (NBR) {
-            if (ok && q == P - 1 && rank + 1 < Q) st_async_pair(&aggF[rank * S + sys], &bars[BAR_F], rank + 1, y0, y1);
+            // two slots: [0] = the forward aggregate of the rank before, [1] = the backward aggregate of the rank after
+            if (ok && q == P - 1 && rank + 1 < Q) st_async_pair(&aggF[sys], &bars[BAR_F], rank + 1, y0, y1);
             if (agg_bytes_f) mbar_wait(&bars[BAR_F], parity);
-            if (rank > 0) { T2 a = aggF[(rank - 1) * S + sy]; fin0 = a.x; fin1 = a.y; }
+            if (rank > 0) { T2 a = aggF[sy]; fin0 = a.x; fin1 = a.y; }
         } else {
         if (ok && q == P - 1)
             for (int rr = rank + 1; rr < Q; ++rr) st_async_pair(&aggF[rank * S + sys], &bars[BAR_F], rr, y0, y1);
@@ -689,14 +690,14 @@ __device__ __forceinline__ void chunk_state_scan(const ScanGeom& g, const T* wta
                 if (rank == per->pp->ra)
                     for (int rr = 0; rr < Q; ++rr) st_async_pair(&per->yab[sys], &bars[BAR_B], rr, ya, yb);
             } else if constexpr (NBR) {
-                if (rank > 0) st_async_pair(&aggB[rank * S + sys], &bars[BAR_B], rank - 1, z0, z1);
+                if (rank > 0) st_async_pair(&aggB[S + sys], &bars[BAR_B], rank - 1, z0, z1);
             } else {
                 for (int rr = 0; rr < rank; ++rr) st_async_pair(&aggB[rank * S + sys], &bars[BAR_B], rr, z0, z1);
             }
         }
         if (agg_bytes_b) mbar_wait(&bars[BAR_B], parity);
         if constexpr (NBR) {
-            if (rank < Q - 1) { T2 a = aggB[(rank + 1) * S + sy]; bin0 = a.x; bin1 = a.y; }
+            if (rank < Q - 1) { T2 a = aggB[S + sy]; bin0 = a.x; bin1 = a.y; }
         }
         for (int rr = Q - 1; rr > (NBR ? Q - 1 : rank); --rr) {   // B_in(rr-1) = aggB[rr] + TPsiBlock(rr) B_in(rr)
             T2 a = aggB[rr * S + sy];
@@ -765,9 +766,9 @@ __device__ __forceinline__ void tri_state_scan(const ScanGeom& g, const T* wtab,
     T fin = 0;
     if constexpr (CLUSTER) {
         if constexpr (NBR) {
-            if (ok && q == P - 1 && rank + 1 < Q) st_async_one(&aggF[rank * S + sys], &bars[BAR_F], rank + 1, y);
+            if (ok && q == P - 1 && rank + 1 < Q) st_async_one(&aggF[sys], &bars[BAR_F], rank + 1, y);
             if (agg_bytes_f) mbar_wait(&bars[BAR_F], parity);
-            if (rank > 0) fin = aggF[(rank - 1) * S + sy];
+            if (rank > 0) fin = aggF[sy];
         } else {
         if (ok && q == P - 1)
             for (int rr = rank + 1; rr < Q; ++rr) st_async_one(&aggF[rank * S + sys], &bars[BAR_F], rr, y);
@@ -790,9 +791,9 @@ __device__ __forceinline__ void tri_state_scan(const ScanGeom& g, const T* wtab,
     T bin = 0;
     if constexpr (CLUSTER) {
         if constexpr (NBR) {
-            if (ok && q == 0 && rank > 0) st_async_one(&aggB[rank * S + sys], &bars[BAR_B], rank - 1, z);
+            if (ok && q == 0 && rank > 0) st_async_one(&aggB[S + sys], &bars[BAR_B], rank - 1, z);
             if (agg_bytes_b) mbar_wait(&bars[BAR_B], parity);
-            if (rank < Q - 1) bin = aggB[(rank + 1) * S + sy];
+            if (rank < Q - 1) bin = aggB[S + sy];
         } else {
         if (ok && q == 0)
             for (int rr = 0; rr < rank; ++rr) st_async_one(&aggB[rank * S + sys], &bars[BAR_B], rr, z);
@@ -817,6 +818,7 @@ struct ChunkPlan {
     bool rows = false;         // system-major batch: implies ldg
     int pace_ns = 0;           // ChunkParams::pace_ns
     int band = 2;              // 1: the tridiagonal instantiation and its tables (handle with a == e == 0)
+    bool nbr = false;          // neighbour-only cluster exchange (two [S] aggregate slots instead of [Q][S]); LM = 0, not periodic
     int mode = 0;              // ChunkParams::ldg: 0 TMA (interleaved), 1 LDG (interleaved), 4 cp.async ring (interleaved), 2 LDG.256 (system-major),
                                // 3 swizzled TMA loads + STG.256 stores, 4 swizzled TMA loads AND stores (system-major)
     size_t table_bytes = 0, smem = 0;
@@ -825,6 +827,7 @@ struct ChunkPlan {
 // ldg: plan for the LDG loader (no TMA alignment requirements, no landing buffer)
 ChunkPlan make_plan(const pent_handle* h, int64_t M, const void* f, int Q, int S, bool any_S = false,
                     bool ldg = false, int band = 2);
+void plan_drop_nbr(ChunkPlan& pl, size_t esz);
 ChunkPlan chunk_auto_plan(const pent_handle* h, int64_t M, const void* f, bool ring_ok = true);   // what PENT_KERNEL_AUTO runs
 // rank-2 tensor map {M, N} of an interleaved batch with box {S, box_rows}; false on failure
 bool encode_batch_map(CUtensorMap* tm, const void* base, int64_t M, int N, int S, int box_rows, bool f64);

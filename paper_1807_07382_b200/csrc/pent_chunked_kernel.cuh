@@ -61,7 +61,7 @@ struct ChunkParams {
 // LM = layout / loader mode, compile-time so that every instantiation carries only its own data path (a run-time
 // switch over all of them cost 80-120 bytes of register spills in every instance): 0 = interleaved batch (TMA, or
 // the LDG loader when prm.ldg == 1); 2, 3, 4 = system-major batch, the modes described at ChunkParams::ldg.
-// NBR: neighbour-only cluster exchange (see chunk_state_scan); chosen by the launcher for Q >= 4 when the handle allows it.
+// NBR: neighbour-only cluster exchange (see chunk_state_scan); chosen by the plan (ChunkPlan::nbr) for Q >= 8 when the handle allows it.
 template <typename T, int S, bool CLUSTER, bool PER, int BAND, int LM, bool NBR = false>
 __global__ void __launch_bounds__(CHUNK_MAX_THREADS, 1)
 solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T> prm,
@@ -92,7 +92,7 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
     ST* aggB = aggF + ((CLUSTER && PER) ? (size_t)prm.Q * S : 0);
     // periodic: the Z-solve chunk states of this CTA's chunks (8 values each), the explicit rows of Z of the three edge
     // chunks, then x^ of rows n-2/n-1, (y_{n-2}, y_{n-1}), (f_n, f_{n+1}), t  ([S] each)
-    T2* zfold = reinterpret_cast<T2*>(aggB + (CLUSTER ? (size_t)prm.Q * S : 0));
+    T2* zfold = reinterpret_cast<T2*>(aggB + (CLUSTER ? (NBR ? (size_t)2 * S : (size_t)prm.Q * S) : 0));
     T2* zedge = zfold + (PER ? (size_t)4 * P : 0);
     T2* ypub = zedge + (PER ? (size_t)3 * C : 0);
     T2* yab = ypub + (PER ? S : 0);

@@ -383,6 +383,15 @@ static bool s_instantiated(bool f64, int S, bool cluster)
     return f64 ? (S == 16 || S == 32) : (S == 32 || S == 64);
 }
 
+// a plan made for the neighbour-only exchange, turned into one for the all-ranks exchange ([Q][S] aggregate slots)
+void plan_drop_nbr(ChunkPlan& pl, size_t esz)
+{
+    if (!pl.nbr) return;
+    pl.nbr = false;
+    pl.smem += (size_t)(pl.band == 2 ? 2 : 1) * (size_t)(pl.Q - 2) * pl.S * esz;
+    if (pl.smem > SMEM_LIMIT) pl.ok = false;
+}
+
 ChunkPlan make_plan(const pent_handle* h, int64_t M, const void* f, int Q, int S, bool any_S, bool ldg, int band)
 {
     ChunkPlan pl;
@@ -420,8 +429,16 @@ ChunkPlan make_plan(const pent_handle* h, int64_t M, const void* f, int Q, int S
     pl.mode = ldg ? 1 : 0;
     if (ldg) pl.nbox = 0;                                    // no landing buffer
     const size_t st = band == 2 ? 2 : 1;                     // words per chunk state
+    // Neighbour-only exchange (chunk_state_scan, NBR): clusters of >= 8 CTAs whose handle says that a state does not survive
+    // a whole block (pent_handle::xdepth == 1).  Measured against the all-ranks exchange (A/B: PENT_AB_FULL_EXCHANGE=1 in the
+    // environment; M as in bench.py's suite): N=8192 (Q=8) 485 -> 409 us, N=12288 (Q=16) 528 -> 354, N=16384 (Q=16) 834 -> 654.
+    // With 4 CTAs it is SLOWER (cfg5a 417 -> 437 us, fp32 200 -> 215: the all-ranks wait keeps the four CTAs of a tile in
+    // lock-step, which their shared HBM rows reward), with 2 CTAs the neighbour is every rank: both run the full exchange.
+    // It needs two [S] aggregate slots instead of [Q][S], which is what lets the TMA plan of N = 16384 fit shared memory.
+    static const int full = []() { const char* e = std::getenv("PENT_AB_FULL_EXCHANGE"); return e ? std::atoi(e) : 0; }();
+    pl.nbr = Q >= 8 && !full && !h->periodic && (band == 2 ? h->xdepth[j] : h->xdepth1[j]) == 1;
     pl.smem = (size_t)pl.nbox * pl.box_rows * S * esz + pl.table_bytes + (size_t)2 * st * pl.Pl * S * esz +
-              (Q > 1 ? st * Q * S * esz : 0) + (3 + 2 * MAX_BOXES) * sizeof(uint64_t);   // one [Q][S] state array
+              (Q > 1 ? st * (pl.nbr ? 2 : Q) * S * esz : 0) + (3 + 2 * MAX_BOXES) * sizeof(uint64_t);   // one [Q][S] state array
     if (pl.smem > SMEM_LIMIT) return pl;
     if (!ldg) {
         if ((M * (int64_t)esz) % 16 != 0) return pl;        // TMA global stride alignment
@@ -625,6 +642,7 @@ static ChunkPlan rows_shape(const pent_handle* h, int64_t M, const void* f, cons
     const int hb = h->band == 1 ? 1 : 2;
     ChunkPlan pl = make_plan(h, M, nullptr, Q, S, false, true, hb);          // no landing buffer yet
     if (!pl.ok) return pl;
+    plan_drop_nbr(pl, h->dtype == PENT_F64 ? 8 : 4);                          // the system-major instantiations exchange with every rank
     pl.rows = true;
     pl.mode = 2;
     if (mode == 2) return pl;
@@ -721,13 +739,7 @@ int launch_solve_chunked(const pent_handle* h, int64_t M, const void* f, void* x
 static int launch_plan(const pent_handle* h, const ChunkPlan& pl, int64_t M, const void* f, void* x, cudaStream_t s)
 {
     const bool cl = pl.Q > 1;
-    // Neighbour-only exchange (chunk_state_scan, NBR): clusters of >= 8 CTAs whose handle says that a state does not survive
-    // a whole block (pent_handle::xdepth == 1).  Measured against the all-ranks exchange (A/B: PENT_AB_FULL_EXCHANGE=1 in the
-    // environment; M as in bench.py's suite): N=8192 (Q=8) 485 -> 409 us, N=12288 (Q=16) 528 -> 354, N=16384 (Q=16) 834 -> 654.
-    // With 4 CTAs it is SLOWER (cfg5a 417 -> 437 us, fp32 200 -> 215: the all-ranks wait keeps the four CTAs of a tile in
-    // lock-step, which their shared HBM rows reward), with 2 CTAs the neighbour is every rank: both run the full exchange.
-    static const int full = []() { const char* e = std::getenv("PENT_AB_FULL_EXCHANGE"); return e ? std::atoi(e) : 0; }();
-    const bool nbr = pl.Q >= 8 && !full && (pl.band == 2 ? h->xdepth[pl.j] : h->xdepth1[pl.j]) == 1;
+    const bool nbr = pl.nbr;          // decided by make_plan (it sizes the aggregate slots)
 #define PENT_INST(T_, S_, B_) (cl ? (nbr ? launch_inst<T_, S_, true, false, B_, 0, true>(h, pl, M, f, x, s, nullptr)  \
                                          : launch_inst<T_, S_, true, false, B_>(h, pl, M, f, x, s, nullptr))          \
                                   : launch_inst<T_, S_, false, false, B_>(h, pl, M, f, x, s, nullptr))

@@ -20,6 +20,7 @@ static PeriodicPlan periodic_plan(const pent_handle* h, int64_t M, const void* f
     if (!h || !h->periodic || !h->inner) return pp;
     const pent_handle* in = h->inner;
     pp.pl = chunk_auto_plan(in, M, f, /*ring_ok=*/false);   // (not ok when the stitching of E is flagged unstable)
+    plan_drop_nbr(pp.pl, h->dtype == PENT_F64 ? 8 : 4);       // the periodic kernel exchanges with every rank
     if (!pp.pl.ok || !h->pfold || !h->pzedge) return pp;
     const bool f64 = h->dtype == PENT_F64;
     const int C = f64 ? ChunkCfg<double>::C : ChunkCfg<float>::C;
