@@ -524,15 +524,25 @@ ChunkPlan chunk_auto_plan(const pent_handle* h, int64_t M, const void* f, bool r
             pl.pace_ns = 1500;
         return pl;
     };
+    // Where the rules below arrive at a 4-CTA cluster, an 8-CTA cluster with the WIDE tile is faster when it can use the
+    // neighbour-only exchange (fp64, pentadiagonal; measured, M as large as fits: N=1536 336 -> 302 us, N=2048 400 -> 370,
+    // N=3072 336 -> 332, N=4096 (cfg5a) 416 -> 406; N=2048 with M=4096: 34.2 -> 31.5; fp32: no difference, left alone)
+    auto prefer8 = [&](ChunkPlan pl) {
+        if (pl.ok && pl.Q == 4 && hb == 2 && h->dtype == PENT_F64) {
+            ChunkPlan p8 = make_plan(h, M, f, 8, Sw, false, false, hb);
+            if (p8.ok && p8.nbr) return p8;
+        }
+        return paced(pl);
+    };
     ChunkPlan narrow1 = make_plan(h, M, f, 1, Sn, false, false, hb);
     if (narrow1.ok && narrow1.threads <= 256) return narrow1;
     for (int Q = 1; Q <= 4; Q *= 2) {
         ChunkPlan pl = make_plan(h, M, f, Q, Sw, false, false, hb);
-        if (pl.ok) return paced(pl);
+        if (pl.ok) return prefer8(pl);
     }
     for (int Q = 1; Q <= QMAX; Q *= 2) {
         ChunkPlan pl = make_plan(h, M, f, Q, Sn, false, false, hb);
-        if (pl.ok) return paced(pl);
+        if (pl.ok) return prefer8(pl);
     }
     for (int Q = 1; Q <= QMAX; Q *= 2) {
         ChunkPlan pl = make_plan(h, M, f, Q, Sw, false, false, hb);

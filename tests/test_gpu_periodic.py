@@ -49,7 +49,7 @@ def test_periodic_nonsymmetric_parity(kernel, N, M):
 
 def test_fused_kernel_is_the_default_where_it_fits():
     pent = _pent()
-    for N, M, want in ((1024, 65536, 1), (512, 4096, 1), (64, 256, 1), (2048, 1024, 1), (1024, 65535, 1), (4096, 1024, 0)):
+    for N, M, want in ((1024, 65536, 1), (512, 4096, 1), (64, 256, 1), (2048, 1024, 1), (1024, 65535, 1), (4096, 1024, 1), (16384, 256, 0)):
         h = _handle(pin.periodic_hyperdiffusion_diagonals(N, 1.0))
         assert pent.lib().pent_periodic_fused(h.ptr, M) == want, (N, M)
 
