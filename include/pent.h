@@ -95,9 +95,10 @@ int pent_solve_batch_v(const pent_handle* h, int64_t M, const void* f, void* x, 
  * ("one system per row", the layout of the paper's serial code; it is also what an ADI
  * sweep along the contiguous axis of a 2-D field needs: the sweep along the other axis is
  * pent_solve_batch itself).  x == f allowed.  Shared-A, non-periodic handles with N <= 16384;
- * PENT_ERR_ARG otherwise.  Every thread reads and writes one contiguous run of 32 (fp64) / 64 (fp32)
- * elements with 32-byte accesses (16-byte aligned runs fall back to narrower ones): 2 passes over the
- * batch, no transpose. */
+ * PENT_ERR_ARG otherwise.  2 passes over the batch, no transpose: a system's run of rows moves global <-> shared memory
+ * by 1-D bulk copies when N * sizeof(element) and the base addresses are 16-byte aligned; otherwise every thread reads and
+ * writes its contiguous run of 32 (fp64) / 64 (fp32) elements itself, with 32-byte accesses when the run is 32-byte aligned
+ * and element-wise accesses when it is not. */
 int pent_solve_batch_rows(const pent_handle* h, int64_t M, const void* f, void* x, void* stream);
 /* Same with an explicit shape / data path (measurement): kernel = PENT_KERNEL_AUTO or PENT_KERNEL_CHUNKED_CFG(Q, S),
  * optionally OR-ed with one of the flags below.  Default: one 1-D bulk copy (cp.async.bulk) per system and tile in
