@@ -242,7 +242,9 @@ int pent_step_batch_forced_v(const pent_handle* h, const pent_step_params* p, co
  *     A_x u* = (2I - A_y) u^n  (explicit along y, implicit along x),   A_y u^{n+1} = (2I - A_x) u*.
  * u: device, Ny x Nx elements, row-major (u[y*Nx + x]), updated in place: its rows are solved as a system-major
  * batch (pent_solve_batch_rows), its columns as an interleaved batch (pent_solve_batch).  scratch: device,
- * Ny*Nx elements, or NULL (stream-ordered temporary).  hx, hy: shared-A, non-periodic, same dtype;
+ * Ny*Nx elements, or NULL (stream-ordered temporary).  After the first explicit half of a call every later one is formed
+ * as 2 x - f in the store stage of the solve before it ((2I - A) A^{-1} f = 2 A^{-1} f - f): two launches and 4 passes over
+ * the field per step, the same scheme in another order of evaluation.  hx, hy: shared-A, non-periodic, same dtype;
  * PENT_ERR_ARG otherwise, or when Nx is too long for the on-chip row solve.  Asynchronous on `stream`. */
 int pent_adi_step_batch(const pent_handle* hx, const pent_handle* hy, void* u, void* scratch, int nsteps,
                         void* stream);

@@ -11,7 +11,7 @@ ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
 LIB = os.path.join(PKG, "libpent.so")
 SOURCES = ["pent_factor.cu", "pent_solve_tps.cu", "pent_solve_chunked.cu", "pent_step.cu", "pent_step_chunked.cu", "pent_periodic.cu", "pent_solve_chunked_periodic.cu",
-           "pent_api.cu", "pent_adi.cu", "pent_solve_chunked_rows.cu"]
+           "pent_api.cu", "pent_adi.cu", "pent_solve_chunked_rows.cu", "pent_solve_chunked_epi.cu"]
 
 
 def nvcc_path() -> str:

@@ -8,6 +8,7 @@
 // Nx (pent_solve_batch_rows); its COLUMNS are the y-lines = an interleaved batch of Nx systems of length Ny
 // (pent_solve_batch, the library's native layout: element k of system i at k*Nx + i).  Each explicit part is
 // the (2I - A) c stencil of PAPER.md:117 (Eq. 7c) along one axis with the handle's own diagonals.
+#include <cstdlib>
 #include "pent_internal.h"
 
 namespace pent {
@@ -81,6 +82,28 @@ static int adi_steps_t(const pent_handle* hx, const pent_handle* hy, T* u, T* w,
     const int64_t nby = ((int64_t)Ny + RSYS - 1) / RSYS;
     const unsigned gy = nby < 65535 ? (unsigned)nby : 65535u;
     const dim3 grows((unsigned)((Nx + tb - 1) / tb), gy, (unsigned)((nby + gy - 1) / gy));
+    // Stencil-free loop (default; pentadiagonal handles).  With r1 = (2I - A_y) u the step is
+    //     u* = A_x^{-1} r1,   r2 = (2I - A_x) u* = 2 u* - r1,   u+ = A_y^{-1} r2,   next r1 = (2I - A_y) u+ = 2 u+ - r2:
+    // after the first stencil every explicit half is "2 x - f" of the solve before it, which the solve kernels form in
+    // their store stage (EPI, pent_solve_chunked_epi.cu).  A step is then TWO launches and 4 passes over the field instead
+    // of four launches and 8 passes; the last column solve of the call stores u+ itself.  Same scheme, another order of
+    // evaluation (the oracle keeps the stencil form; parity is a tolerance).  PENT_AB_ADI_STENCILS=1: the four-kernel loop.
+    static const int stencils = []() { const char* e = std::getenv("PENT_AB_ADI_STENCILS"); return e ? std::atoi(e) : 0; }();
+    if (!stencils && hx->band == 2 && hy->band == 2) {
+        adi_rhs_cols_kernel<T, ROWS><<<gcols, tb, 0, s>>>(Ny, Nx, (const T*)hy->dg, u, w);          // r1 of the first step
+        count_launch();
+        PENT_LAUNCH_CHECK();
+        int rc = PENT_OK;
+        for (int it = 0; it < nsteps && rc == PENT_OK; ++it) {
+            rc = launch_solve_chunked_rows_epi(hx, Ny, w, w, s);                                     // w = r2
+            if (rc != PENT_OK) break;
+            if (it + 1 < nsteps) rc = launch_solve_chunked_epi(hy, Nx, w, w, s);                     // w = next r1
+            else rc = pent_solve_batch(hy, Nx, w, u, (void*)s);                                      // u = u+
+        }
+        if (rc != PENT_UNSUPPORTED) return rc;
+        // (no plan with the epilogue for this shape: nothing has been written to u yet -- w holds intermediate data only
+        //  when a LATER launch failed, which returns above -- fall through to the four-kernel loop)
+    }
     for (int it = 0; it < nsteps; ++it) {
         adi_rhs_cols_kernel<T, ROWS><<<gcols, tb, 0, s>>>(Ny, Nx, (const T*)hy->dg, u, w);
         count_launch();

@@ -834,6 +834,8 @@ bool encode_batch_map(CUtensorMap* tm, const void* base, int64_t M, int N, int S
 bool encode_batch_map_cached(CUtensorMap* tm, const void* base, int64_t M, int N, int S, int box_rows, bool f64);
 // launch of a system-major plan (pent_solve_chunked_rows.cu: the LM = 2, 3, 4 instantiations of the kernel)
 int launch_plan_rows(const pent_handle* h, const ChunkPlan& pl, int64_t M, const void* f, void* x, cudaStream_t s);
+// the same plans launched with the 2 x - f epilogue (pent_solve_chunked_epi.cu: BAND = 2, all-ranks exchange, LM 0, 2, 5, 6)
+int launch_plan_epi(const pent_handle* h, const ChunkPlan& pl, int64_t M, const void* f, void* x, cudaStream_t s);
 // rank-2 tensor map {N, M} of a system-major batch with box {128 bytes, S} and SWIZZLE_128B
 bool encode_rows_map_cached(CUtensorMap* tm, const void* base, int64_t M, int N, int S, bool f64);
 

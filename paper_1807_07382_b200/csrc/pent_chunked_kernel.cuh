@@ -62,7 +62,10 @@ struct ChunkParams {
 // switch over all of them cost 80-120 bytes of register spills in every instance): 0 = interleaved batch (TMA, or
 // the LDG loader when prm.ldg == 1); 2, 3, 4 = system-major batch, the modes described at ChunkParams::ldg.
 // NBR: neighbour-only cluster exchange (see chunk_state_scan); chosen by the plan (ChunkPlan::nbr) for Q >= 8 when the handle allows it.
-template <typename T, int S, bool CLUSTER, bool PER, int BAND, int LM, bool NBR = false>
+// EPI: the kernel stores 2 x - f instead of x (f = its own right-hand side, re-read from global memory / L2 just before the
+// store; x == f allowed).  With A = I - (dt/2) D this is (2I - A) A^{-1} f, the explicit half of the NEXT half step of a
+// Peaceman-Rachford ADI sweep (pent_adi.cu): the stencil kernels between the solves disappear.
+template <typename T, int S, bool CLUSTER, bool PER, int BAND, int LM, bool NBR = false, bool EPI = false>
 __global__ void __launch_bounds__(CHUNK_MAX_THREADS, 1)
 solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T> prm,
                      const __grid_constant__ PeriodicParams<T> pp, const __grid_constant__ CUtensorMap tmx)
@@ -176,6 +179,7 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
     // every CTA of the cluster is resident, with its mbarriers initialised, before any DSMEM store
     if constexpr (CLUSTER) cluster_sync_all();
     static_assert(!NBR || (CLUSTER && !PER), "neighbour-only exchange: cluster kernels, non-periodic");
+    static_assert(!EPI || (!PER && BAND == 2 && LM != 3), "2x - f epilogue: pentadiagonal, non-periodic");
     const uint32_t agg_bytes_f = NBR ? (uint32_t)((rank > 0 ? 1 : 0) * S * sizeof(ST))   // from the rank before
                                      : (uint32_t)(rank * S * sizeof(ST));                 // from the earlier ranks
     // from the later ranks; periodic: from EVERY rank (itself included) plus (y_{n-2}, y_{n-1}) from rank ra
@@ -397,6 +401,39 @@ solve_chunked_kernel(const __grid_constant__ CUtensorMap tm, const ChunkParams<T
             auto correct4 = [&](T (&out)[4], int jg) {
                 if constexpr (BAND == 2) chunk_correct4<T>(out, &v[4 * jg], blk, jg, F0, F1, B0, B1);
                 else tri_correct4<T>(out, &v[4 * jg], blk, jg, F0, B0);
+                if constexpr (EPI) {
+                    const int64_t ecol = tile * S + i;
+                    const int k0 = row0 + 4 * jg;
+                    if (ecol < prm.M) {
+                        if constexpr (LM >= 5) {          // system-major, 16-byte aligned runs: vector loads of the 4 rows
+                            if (k0 + 4 <= prm.N) {
+                                T fv[4];
+                                const uint4* src = reinterpret_cast<const uint4*>(prm.f + ecol * (int64_t)prm.N + k0);
+                                if constexpr (sizeof(T) == 8) {
+                                    const uint4 q0 = src[0], q1 = src[1];
+                                    fv[0] = __hiloint2double((int)q0.y, (int)q0.x); fv[1] = __hiloint2double((int)q0.w, (int)q0.z);
+                                    fv[2] = __hiloint2double((int)q1.y, (int)q1.x); fv[3] = __hiloint2double((int)q1.w, (int)q1.z);
+                                } else {
+                                    const uint4 q0 = src[0];
+                                    fv[0] = __uint_as_float(q0.x); fv[1] = __uint_as_float(q0.y);
+                                    fv[2] = __uint_as_float(q0.z); fv[3] = __uint_as_float(q0.w);
+                                }
+#pragma unroll
+                                for (int r = 0; r < 4; ++r) out[r] = fma((T)2, out[r], -fv[r]);
+                            } else {
+#pragma unroll
+                                for (int r = 0; r < 4; ++r)
+                                    if (k0 + r < prm.N) out[r] = fma((T)2, out[r], -prm.f[ecol * (int64_t)prm.N + k0 + r]);
+                            }
+                        } else {
+#pragma unroll
+                            for (int r = 0; r < 4; ++r)
+                                if (k0 + r < prm.N)
+                                    out[r] = fma((T)2, out[r], -(LM == 0 ? prm.f[(int64_t)(k0 + r) * prm.M + ecol]
+                                                                          : prm.f[ecol * (int64_t)prm.N + k0 + r]));
+                        }
+                    }
+                }
             };
             const int64_t col = tile * S + i;
             T* xo = prm.x + (int64_t)row0 * prm.M + col;

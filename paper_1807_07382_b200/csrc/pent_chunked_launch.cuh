@@ -21,7 +21,7 @@ inline size_t periodic_extra_smem(const ChunkPlan& pl)
     return ((size_t)4 * pl.Pl + 3 * (size_t)ChunkCfg<T>::C + 5 * (size_t)pl.S + (pl.Q > 1 ? (size_t)pl.Q * pl.S : 0)) * 2 * sizeof(T);
 }
 
-template <typename T, int S, bool CLUSTER, bool PER, int BAND = 2, int LM = 0, bool NBR = false>
+template <typename T, int S, bool CLUSTER, bool PER, int BAND = 2, int LM = 0, bool NBR = false, bool EPI = false>
 static int launch_inst(const pent_handle* h, const ChunkPlan& pl, int64_t M, const void* f, void* x,
                        cudaStream_t s, const PeriodicParams<T>* per)
 {
@@ -62,7 +62,7 @@ static int launch_inst(const pent_handle* h, const ChunkPlan& pl, int64_t M, con
     if (PER) pp = *per;
     const size_t smem_total = pl.smem + (PER ? periodic_extra_smem<T>(pl) : 0);
     if ((LM == 0) != (pl.mode <= 1 || pl.mode == 4) || (LM != 0 && LM != pl.mode) || (PER && pl.mode == 4)) return PENT_ERR_ARG;
-    auto kern = solve_chunked_kernel<T, S, CLUSTER, PER, BAND, LM, NBR>;
+    auto kern = solve_chunked_kernel<T, S, CLUSTER, PER, BAND, LM, NBR, EPI>;
     static SmemOnce mark;
     PENT_CUDA(ensure_dynamic_smem(mark, kern, smem_total));
     // the occupancy answer depends only on (device, threads, shared memory, cluster size): keep the last

@@ -153,6 +153,9 @@ int launch_step_chunked_periodic(const pent_handle* h, int64_t M, void* c, int n
 bool chunked_rows_supported(const pent_handle* h, int64_t M);
 int launch_solve_chunked_rows(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s,
                               int Q = 0, int S = 0, int loader = 0);
+// x = 2 A^{-1} f - f on an interleaved / a system-major batch (default plans, pentadiagonal tables); PENT_UNSUPPORTED: no plan
+int launch_solve_chunked_epi(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s);
+int launch_solve_chunked_rows_epi(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s);
 int chunked_choice(const pent_handle* h, int64_t M, int* Q, int* S);   // 1 and the default plan, or 0
 int chunked_rows_choice(const pent_handle* h, int64_t M, int* Q, int* S, int* mode);   // the same for a system-major batch
 

@@ -738,6 +738,26 @@ int launch_solve_chunked_rows(const pent_handle* h, int64_t M, const void* f, vo
     return launch_plan_rows(h, pl, M, f, x, s);
 }
 
+// The 2 x - f epilogue (ADI): the default plans with the pentadiagonal tables and the all-ranks exchange (the instantiations
+// of pent_solve_chunked_epi.cu); tridiagonal handles are refused (the caller keeps its stencil path)
+int launch_solve_chunked_epi(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s)
+{
+    if (!h || h->kind != 0 || h->periodic || h->band != 2) return PENT_UNSUPPORTED;
+    ChunkPlan pl = chunk_auto_plan(h, M, f);
+    if (!pl.ok) return PENT_UNSUPPORTED;
+    plan_drop_nbr(pl, h->dtype == PENT_F64 ? 8 : 4);
+    if (!pl.ok) return PENT_UNSUPPORTED;
+    return launch_plan_epi(h, pl, M, f, x, s);
+}
+
+int launch_solve_chunked_rows_epi(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s)
+{
+    if (!h || h->kind != 0 || h->periodic || h->band != 2) return PENT_UNSUPPORTED;
+    const ChunkPlan pl = rows_plan(h, M, f, x, 0, 0, 0);
+    if (!pl.ok || pl.mode == 3) return PENT_UNSUPPORTED;
+    return launch_plan_epi(h, pl, M, f, x, s);
+}
+
 int launch_solve_chunked(const pent_handle* h, int64_t M, const void* f, void* x, cudaStream_t s,
                          int Q, int S)
 {
