@@ -649,13 +649,17 @@ def run_adi_workload(args, w, rank, world, local):
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
         "config": {"workload": w.name, "N": N, "M_per_gpu": N, "field": f"{N} x {N}, row-major",
                    "matrix": f"Remark-3 fourth-order Crank-Nicolson heat matrix, sigma={w.sigma}, both axes",
-                   "step": "Peaceman-Rachford ADI: rhs along y, solve rows (system-major), rhs along x, solve columns (interleaved)",
-                   "kernel": "adi_rhs_cols_kernel + solve_chunked_kernel(rows) + adi_rhs_rows_kernel + solve_chunked_kernel",
+                   "step": ("Peaceman-Rachford ADI, four kernels per step: rhs along y, solve rows, rhs along x, solve columns"
+                            if os.environ.get("PENT_AB_ADI_STENCILS") else
+                            "Peaceman-Rachford ADI, two kernels per step: solve rows (system-major) and solve columns (interleaved), "
+                            "each storing 2x - f = the explicit half of the next half step"),
+                   "kernel": ("adi_rhs_cols_kernel + solve_chunked_kernel(rows) + adi_rhs_rows_kernel + solve_chunked_kernel"
+                              if os.environ.get("PENT_AB_ADI_STENCILS") else "solve_chunked_kernel(rows, EPI) + solve_chunked_kernel(EPI)"),
                    "l2": f"field {esz * N * N >> 20} MiB + scratch of the same size"},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": None, "peak_source": peak_src, "algorithmic_bytes_per_launch": alg,
                      "kernel": "solve_chunked_kernel",
-                     "note": "algorithmic = 2 passes over the field per half step (4 per step); the unfused path makes 8"},
+                     "note": "algorithmic = 2 passes over the field per half step (4 per step); the four-kernel loop makes 8"},
         "clocks": clocks, "gpu_launches": int(launches),
     }
     _finish_line(line, world)

@@ -168,6 +168,17 @@ extern "C" int pent_step_batch_forced_v(const pent_handle* h, const pent_step_pa
     if (kernel == PENT_KERNEL_CHUNKED && !on_chip) return PENT_ERR_ARG;
     if (kernel != PENT_KERNEL_THREAD_PER_SYSTEM && on_chip)
         return pent::launch_step_chunked(h, p, g, M, c_inout, nsteps, s);
+    // Crank-Nicolson hyperdiffusion whose state does not fit on chip (N > 1024): A c+ = (2I - A) c  <=>  c+ = 2 A^{-1} c - c,
+    // i.e. ONE chunked solve with the "2x - f" epilogue per step, in place: 2 passes over the state per step instead of the
+    // 4 passes of the thread-per-system step kernel (pent_solve_chunked_epi.cu; pentadiagonal tables)
+    if (kernel == PENT_KERNEL_AUTO && p->kind == 1) {
+        int rc = PENT_OK;
+        for (int it = 0; it < nsteps && rc == PENT_OK; ++it) {
+            rc = pent::launch_solve_chunked_epi(h, M, c_inout, c_inout, s);
+            if (rc == pent::PENT_UNSUPPORTED && it > 0) rc = PENT_ERR_ARG;      // (cannot happen: the plan does not depend on the step)
+        }
+        if (rc != pent::PENT_UNSUPPORTED) return rc;
+    }
     if (h->dtype == PENT_F64) return pent::step_impl<double>(h, p, g, M, c_inout, scratch, nsteps, s);
     return pent::step_impl<float>(h, p, g, M, c_inout, scratch, nsteps, s);
 }

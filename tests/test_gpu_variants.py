@@ -185,6 +185,34 @@ def test_hyperdiffusion_step_parity_general_matrix(kernel, N, M):
     assert normwise(cg.numpy(), ref) <= 1e-11
 
 
+@pytest.mark.parametrize("N,M,dtype", [(2048, 200, torch.float64), (4096, 96, torch.float64), (3000, 64, torch.float64),
+                                       (4096, 130, torch.float32), (1500, 37, torch.float64)])
+def test_hyperdiffusion_step_beyond_the_on_chip_size(N, M, dtype):
+    """N > 1024: the state does not fit on chip; a Crank-Nicolson step is then one chunked solve with the 2x - f epilogue
+    (c+ = 2 A^-1 c - c), in place, against the oracle's (2I - A) c followed by a solve.  M = 37: the LDG loader."""
+    pent = _pent()
+    f32 = dtype == torch.float32
+    diags = pin.random_diag_dominant(23, N)
+    c0 = pin.uniform_pm1(24, 0, N, M)
+    if f32:
+        diags = tuple(np.asarray(v, dtype=np.float32).astype(np.float64) for v in diags)
+        c0 = c0.astype(np.float32).astype(np.float64)
+    a, b, c, d, e = (torch.tensor(v, dtype=dtype) for v in diags)
+    h = pent.pent_factor(N, e, c, d, a, b)
+    assert pent.lib().pent_step_kernel_choice(h.ptr, M) == pent.KERNEL_THREAD_PER_SYSTEM      # = "not the on-chip step kernel"
+    cg = guarded(c0, dtype)
+    n0 = pent.launch_count(reset=True)
+    pent.pent_step_batch(h, M, cg.t, 3, kind=1)
+    assert pent.launch_count() == 3                      # one solve launch per step, no scratch
+    cg.check()
+    ref = oracle.step_batch(oracle.factor(*diags), 1, 0, 0, 0.0, 0.0, c0, 3, nthreads=4)
+    assert normwise(cg.numpy().astype(np.float64), ref) <= (2e-5 if f32 else 1e-11)
+    # the thread-per-system kernel (4 passes) still answers the same question
+    c2 = guarded(c0, dtype)
+    pent.pent_step_batch(h, M, c2.t, 3, kind=1, kernel=1)
+    assert normwise(c2.numpy().astype(np.float64), ref) <= (2e-5 if f32 else 1e-11)
+
+
 def test_multi_step_on_chip_equals_repeated_single_steps():
     """The on-chip kernel keeps the state in shared memory across steps: n steps in one launch must
     give bit-identical results to n launches of one step (same arithmetic, same order)."""
