@@ -191,6 +191,8 @@ int pent_solve_batch_multi(const pent_handle* h, const void* f, void* x, void* s
  *     (algebraically identical; form 1 conserves mean(c) to rounding when bc = 1).
  *  kind 1, hyperdiffusion Crank-Nicolson (PAPER.md:87-89 Eq. 6, :117 Eq. 7c):
  *     A c+ = (2I - A) c, with the handle's own diagonals (bc, form, r, sigma ignored).
+ *     Evaluated as c+ = 2 A^{-1} c - c (the same scheme, no stencil): on chip for N <= 1024, else one chunked solve with a
+ *     2x - f store stage per step (2 passes over the state, no scratch).
  *  bc 0: Dirichlet L (diag -2, off 1).  bc 1: zero-flux L (corner diagonal entries -1).
  *  kind 0, form 1 is the scheme of Eq. 2 only if the handle's A IS I + sigma L^2 with this sigma and bc:
  *  pent_factor records whether its matrix has that form (and which sigma, bc), and the call returns
